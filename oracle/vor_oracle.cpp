@@ -1,0 +1,370 @@
+// CPU ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, obviously-correct restatement of what the hot path of
+// arXiv:1607.00908 ("GPU Based Detection of Topological Changes in Voronoi
+// Diagrams") computes, in the reading fixed by BASELINE.json / SURVEY.md §8(c)
+// and listed in DESIGN.md §3.  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference legs may call it.  It shares no
+// code with the CUDA path (paper_1607_00908_b200/csrc) and neither includes,
+// links nor imports the other.
+//
+// Conventions:  L = lattice side, P = 256*L = period in
+// fixed-point units; cell (x,y), 0<=x,y<L, has centre (256x+128, 256y+128);
+// linear index = y*L + x.  Sites: int32 fixed point in [0,P).  Labels int32.
+// Edge key = (uint64)i<<32 | j with i<j.
+//
+// Parity pins (tests/test_oracle_*.py): every function below is pinned — see
+// DESIGN.md §4 for the table.  None is "parity unpinned".
+//
+// Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
+// OpenMP is used only as "for each lattice row, independently"; threads<=0
+// means "all cores the process may use".
+
+#include <algorithm>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <queue>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef int64_t i64;
+typedef uint64_t u64;
+
+// Minimum-image squared distance between cell centre (cx,cy) and site (sx,sy),
+// all in fixed point, period P.  PAPER.md:131 (§III.B.1: "calculating just the
+// squared distance"), periodic metric per BASELINE.json config 1.
+inline i64 min_image_d2(i64 cx, i64 cy, i64 sx, i64 sy, i64 P) {
+    i64 ax = cx > sx ? cx - sx : sx - cx;
+    i64 dx = ax < P - ax ? ax : P - ax;
+    i64 ay = cy > sy ? cy - sy : sy - cy;
+    i64 dy = ay < P - ay ? ay : P - ay;
+    return dx * dx + dy * dy;
+}
+
+inline int resolve_threads(int threads) {
+#ifdef _OPENMP
+    return threads > 0 ? threads : omp_get_max_threads();
+#else
+    (void)threads;
+    return 1;
+#endif
+}
+
+// O1a for one cell: argmin over ALL sites of (d2, index), PAPER.md:35 (region
+// definition) + PAPER.md:131 (each lattice site computes its distance from all
+// the centres); ties to the smallest index (reading R1).
+inline int32_t brute_one(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy, i64 x, i64 y) {
+    const i64 P = 256 * (i64)L;
+    const i64 cx = 256 * x + 128, cy = 256 * y + 128;
+    i64 best = INT64_MAX;
+    int32_t besti = -1;
+    for (int32_t i = 0; i < n; ++i) {
+        i64 d2 = min_image_d2(cx, cy, sx[i], sy[i], P);
+        if (d2 < best) { best = d2; besti = i; }   // strict '<' + ascending i  => smallest index wins ties
+    }
+    return besti;
+}
+
+// Cell list for O1b: buckets of `bs` x `bs` cells (w = 256*bs fixed-point units).
+struct CellList {
+    int32_t nb;                    // buckets per side
+    i64 w;                         // bucket width in fixed point
+    std::vector<int32_t> start;    // nb*nb+1
+    std::vector<int32_t> items;    // site indices, bucket by bucket, ascending inside a bucket
+};
+
+CellList make_cell_list(int32_t L, int32_t bs, int32_t n, const int32_t* sx, const int32_t* sy) {
+    CellList cl;
+    cl.nb = L / bs;
+    cl.w = 256 * (i64)bs;
+    cl.start.assign((size_t)cl.nb * cl.nb + 1, 0);
+    for (int32_t i = 0; i < n; ++i) {
+        i64 b = (sy[i] / cl.w) * cl.nb + (sx[i] / cl.w);
+        cl.start[b + 1]++;
+    }
+    for (size_t b = 0; b < (size_t)cl.nb * cl.nb; ++b) cl.start[b + 1] += cl.start[b];
+    cl.items.resize(n);
+    std::vector<int32_t> fill(cl.start.begin(), cl.start.end() - 1);
+    for (int32_t i = 0; i < n; ++i) {
+        i64 b = (sy[i] / cl.w) * cl.nb + (sx[i] / cl.w);
+        cl.items[fill[b]++] = i;
+    }
+    return cl;
+}
+
+// O1b for one cell: ring search over cell-list buckets with the exactness stop
+// rule of reading R3.  After all buckets at Chebyshev bucket
+// distance <= r from the cell's own bucket have been scanned, every unscanned
+// site has |dx| or |dy| strictly greater than r*w, hence d2 > (r*w)^2; stop when
+// best_d2 <= (r*w)^2.  If the next ring would wrap onto itself (2r+1 >= nb) the
+// cell is finished by the O1a loop over all sites.
+inline int32_t ring_one(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy,
+                        const CellList& cl, i64 x, i64 y) {
+    const i64 P = 256 * (i64)L;
+    const i64 cx = 256 * x + 128, cy = 256 * y + 128;
+    const int32_t nb = cl.nb;
+    const int32_t bx = (int32_t)(cx / cl.w), by = (int32_t)(cy / cl.w);
+    i64 best = INT64_MAX;
+    int32_t besti = -1;
+    for (int32_t r = 0;; ++r) {
+        if (2 * r + 1 >= nb) return brute_one(L, n, sx, sy, x, y);
+        for (int32_t oy = -r; oy <= r; ++oy) {
+            for (int32_t ox = -r; ox <= r; ++ox) {
+                if (std::max(std::abs(ox), std::abs(oy)) != r) continue;   // ring r only
+                int32_t qx = ((bx + ox) % nb + nb) % nb, qy = ((by + oy) % nb + nb) % nb;
+                size_t b = (size_t)qy * nb + qx;
+                for (int32_t k = cl.start[b]; k < cl.start[b + 1]; ++k) {
+                    int32_t i = cl.items[k];
+                    i64 d2 = min_image_d2(cx, cy, sx[i], sy[i], P);
+                    if (d2 < best || (d2 == best && i < besti)) { best = d2; besti = i; }
+                }
+            }
+        }
+        i64 rw = (i64)r * cl.w;
+        if (besti >= 0 && r >= 1 && best <= rw * rw) return besti;
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+// O1a — brute-force labels for the whole lattice.  labels[y*L+x].
+void orc_label_brute(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy,
+                     int32_t* labels, int threads) {
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int32_t y = 0; y < L; ++y)
+        for (int32_t x = 0; x < L; ++x)
+            labels[(size_t)y * L + x] = brute_one(L, n, sx, sy, x, y);
+}
+
+// O1a on m sampled cells (linear indices) — used at sizes where the full lattice
+// is unaffordable (config 5).
+void orc_label_brute_at(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy,
+                        int64_t m, const int64_t* cells, int32_t* out, int threads) {
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int64_t k = 0; k < m; ++k)
+        out[k] = brute_one(L, n, sx, sy, cells[k] % L, cells[k] / L);
+}
+
+// O1b — cell-list ring search for the whole lattice.  bucket_cells must divide L.
+// Returns 0, or -1 on a bad bucket size.
+int orc_label_cells(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy,
+                    int32_t bucket_cells, int32_t* labels, int threads) {
+    if (bucket_cells < 1 || L % bucket_cells != 0) return -1;
+    CellList cl = make_cell_list(L, bucket_cells, n, sx, sy);
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int32_t y = 0; y < L; ++y)
+        for (int32_t x = 0; x < L; ++x)
+            labels[(size_t)y * L + x] = ring_one(L, n, sx, sy, cl, x, y);
+    return 0;
+}
+
+// O1b on m sampled cells.
+int orc_label_cells_at(int32_t L, int32_t n, const int32_t* sx, const int32_t* sy,
+                       int32_t bucket_cells, int64_t m, const int64_t* cells, int32_t* out,
+                       int threads) {
+    if (bucket_cells < 1 || L % bucket_cells != 0) return -1;
+    CellList cl = make_cell_list(L, bucket_cells, n, sx, sy);
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int64_t k = 0; k < m; ++k)
+        out[k] = ring_one(L, n, sx, sy, cl, cells[k] % L, cells[k] / L);
+    return 0;
+}
+
+// O2 — site-adjacency (digital Delaunay) edge set from 4-connected label
+// discontinuities including the periodic wrap (reading R6; the paper's analogue
+// is the adjacency matrix of PAPER.md:121, 139-191, compressed by sort+unique,
+// PAPER.md:207).  Output ascending packed keys (i<<32|j, i<j).  Returns the
+// number of unique edges; writes at most `cap` of them.
+int64_t orc_edges(int32_t L, const int32_t* labels, uint64_t* out, int64_t cap) {
+    std::vector<u64> keys;
+    for (int32_t y = 0; y < L; ++y) {
+        for (int32_t x = 0; x < L; ++x) {
+            int32_t a = labels[(size_t)y * L + x];
+            int32_t b = labels[(size_t)y * L + (x + 1) % L];
+            int32_t c = labels[(size_t)((y + 1) % L) * L + x];
+            if (a != b) keys.push_back(((u64)(uint32_t)std::min(a, b) << 32) | (uint32_t)std::max(a, b));
+            if (a != c) keys.push_back(((u64)(uint32_t)std::min(a, c) << 32) | (uint32_t)std::max(a, c));
+        }
+    }
+    std::sort(keys.begin(), keys.end());
+    keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+    int64_t m = (int64_t)keys.size();
+    for (int64_t k = 0; k < m && k < cap; ++k) out[k] = keys[k];
+    return m;
+}
+
+// Number of raw (not de-duplicated) discontinuities — workload statistic only.
+int64_t orc_count_discontinuities(int32_t L, const int32_t* labels) {
+    int64_t m = 0;
+    for (int32_t y = 0; y < L; ++y)
+        for (int32_t x = 0; x < L; ++x) {
+            int32_t a = labels[(size_t)y * L + x];
+            m += a != labels[(size_t)y * L + (x + 1) % L];
+            m += a != labels[(size_t)((y + 1) % L) * L + x];
+        }
+    return m;
+}
+
+// O3 — frame-to-frame diff (PAPER.md:213-221 translation + comparison; PAPER.md:223
+// appearing/disappearing bubbles excluded; PAPER.md:266 breaking = in D_P only,
+// arising = in D_N only).  p2n / n2p may be NULL (persistent identity).
+// With maps: each prev edge (i,j) -> (p2n[i], p2n[j]), dropped if either is -1,
+// re-packed (min,max), sorted, uniqued; each now edge with an endpoint whose
+// n2p is -1 is dropped.  created = now \ prev, destroyed = prev \ now, both
+// ascending, in NOW index space.  Counts returned through n_created/n_destroyed;
+// at most cap entries written to each list.
+void orc_diff(const uint64_t* prev, int64_t n_prev, const uint64_t* now, int64_t n_now,
+              const int32_t* p2n, const int32_t* n2p,
+              uint64_t* created, uint64_t* destroyed, int64_t cap,
+              int64_t* n_created, int64_t* n_destroyed) {
+    std::vector<u64> P, N;
+    for (int64_t k = 0; k < n_prev; ++k) {
+        int64_t i = (int64_t)(prev[k] >> 32), j = (int64_t)(prev[k] & 0xffffffffu);
+        if (p2n) {
+            i = p2n[i]; j = p2n[j];
+            if (i < 0 || j < 0 || i == j) continue;
+        }
+        P.push_back(((u64)std::min(i, j) << 32) | (u64)std::max(i, j));
+    }
+    std::sort(P.begin(), P.end());
+    P.erase(std::unique(P.begin(), P.end()), P.end());
+    for (int64_t k = 0; k < n_now; ++k) {
+        int64_t i = (int64_t)(now[k] >> 32), j = (int64_t)(now[k] & 0xffffffffu);
+        if (n2p && (n2p[i] < 0 || n2p[j] < 0)) continue;
+        N.push_back(now[k]);
+    }
+    std::sort(N.begin(), N.end());
+    std::vector<u64> C, D;
+    std::set_difference(N.begin(), N.end(), P.begin(), P.end(), std::back_inserter(C));
+    std::set_difference(P.begin(), P.end(), N.begin(), N.end(), std::back_inserter(D));
+    *n_created = (int64_t)C.size();
+    *n_destroyed = (int64_t)D.size();
+    for (int64_t k = 0; k < (int64_t)C.size() && k < cap; ++k) created[k] = C[k];
+    for (int64_t k = 0; k < (int64_t)D.size() && k < cap; ++k) destroyed[k] = D[k];
+}
+
+// O4 — threshold + connected components (Ising-like variable from
+// the threshold, then cluster labelling).  mask = above ? field>thr : field<thr
+// (NaN -> false).  4-connected, periodic (readings R8, R9).  Scan linear indices
+// ascending; an unvisited mask cell seeds a breadth-first search that writes the
+// seed's linear index to every member — the seed is the component's minimum
+// index by construction.  Background -1.
+void orc_threshold_ccl(int32_t L, const float* field, float thr, int above, int32_t* ccl) {
+    const size_t n = (size_t)L * L;
+    std::vector<uint8_t> mask(n);
+    for (size_t i = 0; i < n; ++i) mask[i] = above ? (field[i] > thr) : (field[i] < thr);
+    for (size_t i = 0; i < n; ++i) ccl[i] = -1;
+    std::vector<int32_t> queue;
+    for (size_t seed = 0; seed < n; ++seed) {
+        if (!mask[seed] || ccl[seed] != -1) continue;
+        queue.clear();
+        queue.push_back((int32_t)seed);
+        ccl[seed] = (int32_t)seed;
+        for (size_t head = 0; head < queue.size(); ++head) {
+            int32_t c = queue[head];
+            int32_t x = c % L, y = c / L;
+            const int32_t nbr[4] = {
+                y * L + (x + 1) % L, y * L + (x + L - 1) % L,
+                ((y + 1) % L) * L + x, ((y + L - 1) % L) * L + x};
+            for (int k = 0; k < 4; ++k)
+                if (mask[nbr[k]] && ccl[nbr[k]] == -1) {
+                    ccl[nbr[k]] = (int32_t)seed;
+                    queue.push_back(nbr[k]);
+                }
+        }
+    }
+}
+
+// O5 — per-component size and centre of mass (count the lattice
+// points of each bubble, "sum, separately, the coordinates of the lattice points
+// that form the bubble and divide by the size"; unweighted reading R10, periodic
+// unwrap relative to the root cell R11, integer sums, floor to fixed point R12).
+// Components with size < min_size are dropped; survivors are numbered 0..K-1 by
+// ascending root index.  Returns K (writes at most cap entries).
+int32_t orc_centroids(int32_t L, const int32_t* ccl, int32_t min_size,
+                      double* cx, double* cy, int32_t* sx, int32_t* sy,
+                      int32_t* size, int32_t* root, int32_t cap) {
+    const size_t n = (size_t)L * L;
+    const i64 P = 256 * (i64)L;
+    std::vector<i64> cnt(n, 0), Sx(n, 0), Sy(n, 0);     // indexed by root cell
+    for (size_t i = 0; i < n; ++i) {
+        int32_t r = ccl[i];
+        if (r < 0) continue;
+        i64 x = (i64)(i % L), y = (i64)(i / L), xr = r % L, yr = r / L;
+        i64 dx = x - xr;
+        if (2 * dx >= L) dx -= L; else if (2 * dx < -(i64)L) dx += L;
+        i64 dy = y - yr;
+        if (2 * dy >= L) dy -= L; else if (2 * dy < -(i64)L) dy += L;
+        cnt[r] += 1; Sx[r] += dx; Sy[r] += dy;
+    }
+    int32_t K = 0;
+    for (size_t r = 0; r < n; ++r) {
+        if (cnt[r] == 0 || cnt[r] < min_size) continue;
+        if (K < cap) {
+            i64 xr = (i64)(r % L), yr = (i64)(r / L), m = cnt[r];
+            // floor division toward -inf, then non-negative mod P
+            i64 qx = 256 * Sx[r], qy = 256 * Sy[r];
+            i64 fx = qx >= 0 ? qx / m : -((-qx + m - 1) / m);
+            i64 fy = qy >= 0 ? qy / m : -((-qy + m - 1) / m);
+            sx[K] = (int32_t)((((256 * xr + 128 + fx) % P) + P) % P);
+            sy[K] = (int32_t)((((256 * yr + 128 + fy) % P) + P) % P);
+            double ux = (double)xr + 0.5 + (double)Sx[r] / (double)m;
+            double uy = (double)yr + 0.5 + (double)Sy[r] / (double)m;
+            if (ux < 0) ux += L; else if (ux >= L) ux -= L;
+            if (uy < 0) uy += L; else if (uy >= L) uy -= L;
+            cx[K] = ux; cy[K] = uy;
+            size[K] = (int32_t)m;
+            root[K] = (int32_t)r;
+        }
+        ++K;
+    }
+    return K;
+}
+
+// O6 — isomorphism Phi P->N by comparing the two sets of centres,
+// unmatched = appeared / disappeared.  Rule (reading R13): mutual
+// nearest neighbour under the minimum-image metric on fixed-point coordinates,
+// within the inclusive radius, ties to the smallest index.  -1 = dead / born.
+void orc_match(int32_t L, const int32_t* px, const int32_t* py, int32_t n_prev,
+               const int32_t* nx, const int32_t* ny, int32_t n_now, int32_t radius_fp,
+               int32_t* p2n, int32_t* n2p) {
+    const i64 P = 256 * (i64)L, r2 = (i64)radius_fp * radius_fp;
+    std::vector<int32_t> bp(n_now, -1), bn(n_prev, -1);
+    for (int32_t j = 0; j < n_now; ++j) {
+        i64 best = INT64_MAX;
+        for (int32_t i = 0; i < n_prev; ++i) {
+            i64 d2 = min_image_d2(nx[j], ny[j], px[i], py[i], P);
+            if (d2 < best) { best = d2; bp[j] = i; }
+        }
+        if (best > r2) bp[j] = -1;
+    }
+    for (int32_t i = 0; i < n_prev; ++i) {
+        i64 best = INT64_MAX;
+        for (int32_t j = 0; j < n_now; ++j) {
+            i64 d2 = min_image_d2(px[i], py[i], nx[j], ny[j], P);
+            if (d2 < best) { best = d2; bn[i] = j; }
+        }
+        if (best > r2) bn[i] = -1;
+    }
+    for (int32_t i = 0; i < n_prev; ++i) p2n[i] = (bn[i] >= 0 && bp[bn[i]] == i) ? bn[i] : -1;
+    for (int32_t j = 0; j < n_now; ++j) n2p[j] = (bp[j] >= 0 && bn[bp[j]] == j) ? bp[j] : -1;
+}
+
+int orc_num_threads(int threads) { return resolve_threads(threads); }
+
+}  // extern "C"
