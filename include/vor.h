@@ -1,0 +1,152 @@
+/* vor.h — C ABI of libvor: the data-parallel hot path of arXiv:1607.00908
+ * ("GPU Based Detection of Topological Changes in Voronoi Diagrams"), re-designed for one
+ * NVIDIA B200 (sm_100a).  "PAPER.md:n" cites a line of the paper text plus its section.
+ *
+ * Conventions
+ *   L            lattice side; the lattice is an L x L torus.  P = 256*L is the period in
+ *                fixed-point units (1 cell = 256 units).
+ *   cell (x,y)   0 <= x,y < L, centre (256x+128, 256y+128), linear index y*L + x.
+ *   sites        SoA int32 arrays sx[n], sy[n], each coordinate in [0, P).  Coordinates outside
+ *                that range are undefined behaviour.
+ *   labels       int32[L*L], row-major.
+ *   edge key     (uint64)i << 32 | j with i < j (site indices); lists are ascending and unique.
+ *   -1           background cell / unmatched component.
+ *
+ * Pointers named d_* are DEVICE memory owned by the caller (e.g. torch tensors); h_* are HOST
+ * memory owned by the caller.  The library neither frees nor keeps them beyond the stream work it
+ * enqueues, except where stated.  `stream` is a cudaStream_t passed as void* (NULL = default
+ * stream).  All d_* entry points are asynchronous: they enqueue work and return; counts are
+ * written to device scalars so that no call forces a host synchronisation.
+ *
+ * Every function returns a vor_status.  Nothing throws or aborts across this boundary.
+ * Capacity overflows never write out of bounds: the kernels store the REQUIRED count in the
+ * device scalar, write nothing beyond `cap`, and latch a sticky device-side flag that the next
+ * vor_sync_status() reports as VOR_ECAPACITY.
+ */
+#ifndef VOR_H_
+#define VOR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vor_ctx vor_ctx; /* opaque; owns all scratch memory (cell list, key buffers, sort and
+                                   union-find temporaries, the e2e pipeline's device buffers) */
+
+typedef enum {
+    VOR_OK = 0,
+    VOR_EINVAL = -1,    /* bad argument (null pointer, size out of range) */
+    VOR_ECAPACITY = -2, /* an output or scratch buffer was too small (sticky, see above) */
+    VOR_ECUDA = -3,     /* a CUDA runtime call failed; vor_last_error() has the text */
+    VOR_ESTATE = -4     /* call order violation (e.g. vor_label before vor_build_cells) */
+} vor_status;
+
+/* Create a context for an L x L lattice (2 <= L <= 2^22) and at most max_sites sites
+ * (1 <= max_sites < 2^31).  max_raw_keys sizes the scratch that receives the (partly
+ * de-duplicated) edge keys before sorting; 0 selects a default (max(2^20, 16*max_sites), never
+ * more than the hard worst case 2*L*L).  Allocates device memory on the CURRENT device. */
+int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys);
+int vor_destroy(vor_ctx* ctx);
+
+/* Text of the last failure on this context (ctx-owned storage; never free it). */
+const char* vor_last_error(const vor_ctx* ctx);
+
+/* Synchronise `stream`, then return and clear the sticky device-side status. */
+int vor_sync_status(vor_ctx* ctx, void* stream);
+
+/* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t vor_launch_count(const vor_ctx* ctx);
+
+/* Tuning knobs (integers).  Unknown names -> VOR_EINVAL.
+ *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 100) */
+int vor_set_option(vor_ctx* ctx, const char* name, int64_t value);
+
+/* ---- a1: counting-sort cell list of the sites (not in the paper, which loops over all centres,
+ * PAPER.md:131 §III.B.1; named by BASELINE.json north_star).  Reads d_sx/d_sy[n_sites]; the
+ * context keeps its own bucket-ordered copy, so the caller may overwrite the inputs once the
+ * stream work has run. */
+int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
+                    void* stream);
+
+/* ---- a2: digital Voronoi colouring (§II region definition; PAPER.md:129-131
+ * §III.B.1 "coloring itself with the label of the nearest center of mass", squared distance).
+ * labels[y*L+x] = argmin_i (minimum-image squared distance from the cell centre to site i, i),
+ * exact integer arithmetic, ties to the smallest index.  Uses the cell list of the last
+ * vor_build_cells on this context (none -> VOR_ESTATE).  Writes d_labels[L*L]. */
+int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream);
+
+/* ---- a3+a4: site adjacency (digital Delaunay edge set; PAPER.md:121 adjacency matrix,
+ * PAPER.md:207 compress by sort+unique).  Rule (R6): every 4-connected label
+ * discontinuity, including across the periodic wrap, contributes the pair (min,max).
+ * Reads d_labels[L*L] (values in [0, n_sites) of the last vor_build_cells, or any int32 >= 0
+ * if label_bits is given through vor_edges_ex); writes the ascending unique keys to
+ * d_edges[0..min(E,cap)) and E to *d_n_edges. */
+int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
+              int64_t* d_n_edges, void* stream);
+
+/* ---- a5: frame-to-frame comparison (§III.B.3 translation + comparison;
+ * PAPER.md:223 appearing/disappearing bubbles excluded; §III.B.4 "breaking" = in
+ * D_P only, "arising" = in D_N only).  d_prev/d_now are ascending unique key lists with device
+ * counts.  d_p2n[i] (prev label -> now label or -1) and d_n2p (now -> prev or -1) may both be
+ * NULL: persistent identity.  With maps: prev edges are translated, dropped if an endpoint is -1
+ * or both endpoints collapse, re-sorted and uniqued; now edges with an unmatched endpoint are
+ * dropped.  created = now \ prev, destroyed = prev \ now, ascending, in NOW index space.
+ * n_prev_labels / n_now_labels bound the label values (needed only with maps; pass 0 otherwise). */
+int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+             const uint64_t* d_now, const int64_t* d_n_now,
+             const int32_t* d_p2n, const int32_t* d_n2p, int32_t n_prev_labels, int32_t n_now_labels,
+             uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
+             int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
+
+/* ---- a6: bubble identification (§III.A: threshold -> two-valued variable ->
+ * cluster labelling).  mask = above ? field > thr : field < thr (strict; NaN -> background).
+ * 4-connected periodic components; d_ccl[c] = smallest linear index in c's component, or -1. */
+int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr, int above,
+                        int32_t* d_ccl, void* stream);
+
+/* ---- a7: bubble sizes and centres of mass (§III.A: count the lattice points
+ * of each bubble; sum the coordinates and divide by the size).  Unweighted, periodic unwrap
+ * relative to the root cell, integer sums; components smaller than min_size are dropped; the K
+ * survivors are ordered by ascending root.  Outputs (each capacity `cap`): centroid in lattice
+ * units (float64, in [0,L)), fixed-point site coordinates (floor), size, root; K to *d_n_comp. */
+int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_size,
+                    double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
+                    int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp, void* stream);
+
+/* ---- a8: isomorphism Phi P->N "by simply comparing the two sets of centers of mass"
+ * (§III.B.3); unmatched = appeared / disappeared.  Mutual nearest
+ * neighbour under the minimum-image metric on fixed-point coordinates, squared distance
+ * <= radius_fp^2, ties to the smallest index.  Counts are device scalars (int32) so the call
+ * chains after field_centroids without a host sync; cap_* bound the array lengths. */
+int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_py, const int32_t* d_n_prev,
+                const int32_t* d_nx, const int32_t* d_ny, const int32_t* d_n_now,
+                int32_t cap_prev, int32_t cap_now, int32_t radius_fp,
+                int32_t* d_p2n, int32_t* d_n2p, void* stream);
+
+/* ---- end-to-end, HOST buffers (bench.py's e2e leg): one site-driven frame.
+ * Copies h_sx/h_sy[n_sites] to the device, runs a1..a5 against the edge list kept from the
+ * previous call on this context (the first call diffs against an empty list), copies the
+ * created/destroyed lists (at most cap each) and h_counts[3] = {n_edges, n_created, n_destroyed}
+ * back, and synchronises.  The label image stays on the device (not copying it is
+ * the point of the method); vor_frame_labels() exposes it. */
+int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
+                   uint64_t* h_created, uint64_t* h_destroyed, int64_t cap, int64_t* h_counts,
+                   void* stream);
+/* Same pipeline with DEVICE site arrays and no host copies or synchronisation: results stay in
+ * context-owned device buffers (vor_frame_results).  bench.py's device-resident leg. */
+int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
+                     void* stream);
+/* Forget the previous frame's edge list (start a new sequence). */
+int vor_frame_reset(vor_ctx* ctx);
+/* Device pointers to the context-owned results of the last vor_frame_* call:
+ * labels int32[L*L]; edges / created / destroyed uint64 lists; counts int64[3] (device). */
+int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const uint64_t** d_edges,
+                      const uint64_t** d_created, const uint64_t** d_destroyed,
+                      const int64_t** d_counts);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOR_H_ */

@@ -1,0 +1,193 @@
+"""ctypes binding of libvor.so — argument marshalling only.
+
+Every step of the hot path runs inside the CUDA kernels of libvor.so (include/vor.h); this module
+turns torch CUDA tensors into raw device pointers and the current torch stream into a cudaStream_t.
+There is no CPU fallback: a missing library or a failing call raises.  This package never imports
+`oracle/`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvor.so")
+
+VOR_OK, VOR_EINVAL, VOR_ECAPACITY, VOR_ECUDA, VOR_ESTATE = 0, -1, -2, -3, -4
+_STATUS = {0: "VOR_OK", -1: "VOR_EINVAL", -2: "VOR_ECAPACITY", -3: "VOR_ECUDA", -4: "VOR_ESTATE"}
+
+# name -> (restype, argtypes); mirrors include/vor.h one to one
+_P = C.c_void_p
+SIGNATURES = {
+    "vor_create": (C.c_int, [C.POINTER(_P), C.c_int32, C.c_int32, C.c_int64]),
+    "vor_destroy": (C.c_int, [_P]),
+    "vor_last_error": (C.c_char_p, [_P]),
+    "vor_sync_status": (C.c_int, [_P, _P]),
+    "vor_launch_count": (C.c_int64, [_P]),
+    "vor_set_option": (C.c_int, [_P, C.c_char_p, C.c_int64]),
+    "vor_build_cells": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
+    "vor_label": (C.c_int, [_P, _P, _P]),
+    "vor_edges": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P]),
+    "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
+    "field_threshold_ccl": (C.c_int, [_P, _P, C.c_float, C.c_int, _P, _P]),
+    "field_centroids": (C.c_int, [_P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
+    "match_sites": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P, _P]),
+    "vor_frame_host": (C.c_int, [_P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P]),
+    "vor_frame_device": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
+    "vor_frame_reset": (C.c_int, [_P]),
+    "vor_frame_results": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P)]),
+}
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libvor.so (no GPU needed for this step) and declare every prototype."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1607_00908_b200.build` "
+                "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)          # AttributeError if the symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+class VorError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("expected a CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Vor:
+    """One libvor context on the current CUDA device.  Methods carry the C names."""
+
+    def __init__(self, L: int, max_sites: int, max_raw_keys: int = 0):
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("libvor needs a CUDA device; there is no CPU fallback")
+        torch.cuda.init()
+        torch.zeros(1, device="cuda")        # make sure the primary context exists
+        h = C.c_void_p()
+        rc = self.lib.vor_create(C.byref(h), L, max_sites, max_raw_keys)
+        if rc != VOR_OK:
+            raise VorError(rc, "vor_create failed")
+        self.h = h
+        self.L = L
+        self.max_sites = max_sites
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.vor_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != VOR_OK:
+            raise VorError(rc, self.lib.vor_last_error(self.h).decode())
+
+    # ---- plumbing
+    def vor_sync_status(self):
+        self._check(self.lib.vor_sync_status(self.h, _stream()))
+
+    def vor_launch_count(self) -> int:
+        return int(self.lib.vor_launch_count(self.h))
+
+    def vor_set_option(self, name: str, value: int):
+        self._check(self.lib.vor_set_option(self.h, name.encode(), int(value)))
+
+    # ---- site path
+    def vor_build_cells(self, sx, sy):
+        assert sx.shape == sy.shape and sx.dim() == 1
+        self._check(self.lib.vor_build_cells(self.h, _ptr(sx, torch.int32), _ptr(sy, torch.int32),
+                                             sx.numel(), _stream()))
+
+    def vor_label(self, labels):
+        assert labels.numel() == self.L * self.L
+        self._check(self.lib.vor_label(self.h, _ptr(labels, torch.int32), _stream()))
+
+    def vor_edges(self, labels, edges, n_edges):
+        """edges: int64/uint64 tensor viewed as packed keys; n_edges: int64[1] device scalar."""
+        assert labels.numel() == self.L * self.L and n_edges.numel() >= 1
+        self._check(self.lib.vor_edges(self.h, _ptr(labels, torch.int32), _ptr(edges, torch.int64),
+                                       edges.numel(), _ptr(n_edges, torch.int64), _stream()))
+
+    def vor_diff(self, prev, n_prev, now, n_now, created, destroyed, n_created, n_destroyed,
+                 p2n=None, n2p=None, n_prev_labels=0, n_now_labels=0):
+        cap = min(created.numel(), destroyed.numel())
+        self._check(self.lib.vor_diff(
+            self.h, _ptr(prev, torch.int64), _ptr(n_prev, torch.int64), _ptr(now, torch.int64),
+            _ptr(n_now, torch.int64), _ptr(p2n, torch.int32), _ptr(n2p, torch.int32),
+            n_prev_labels, n_now_labels, _ptr(created, torch.int64), _ptr(destroyed, torch.int64), cap,
+            _ptr(n_created, torch.int64), _ptr(n_destroyed, torch.int64), _stream()))
+
+    # ---- field path
+    def field_threshold_ccl(self, field, thr: float, above: bool, ccl):
+        assert field.numel() == self.L * self.L == ccl.numel()
+        self._check(self.lib.field_threshold_ccl(self.h, _ptr(field, torch.float32), C.c_float(thr),
+                                                 1 if above else 0, _ptr(ccl, torch.int32), _stream()))
+
+    def field_centroids(self, ccl, min_size: int, cx, cy, sx, sy, size, root, n_comp):
+        cap = min(t.numel() for t in (cx, cy, sx, sy, size, root))
+        self._check(self.lib.field_centroids(
+            self.h, _ptr(ccl, torch.int32), min_size, _ptr(cx, torch.float64), _ptr(cy, torch.float64),
+            _ptr(sx, torch.int32), _ptr(sy, torch.int32), _ptr(size, torch.int32), _ptr(root, torch.int32),
+            cap, _ptr(n_comp, torch.int32), _stream()))
+
+    def match_sites(self, px, py, n_prev, nx, ny, n_now, radius_fp: int, p2n, n2p):
+        cap_prev = min(px.numel(), py.numel(), p2n.numel())
+        cap_now = min(nx.numel(), ny.numel(), n2p.numel())
+        self._check(self.lib.match_sites(
+            self.h, _ptr(px, torch.int32), _ptr(py, torch.int32), _ptr(n_prev, torch.int32),
+            _ptr(nx, torch.int32), _ptr(ny, torch.int32), _ptr(n_now, torch.int32),
+            cap_prev, cap_now, radius_fp, _ptr(p2n, torch.int32), _ptr(n2p, torch.int32), _stream()))
+
+    # ---- frame pipeline
+    def vor_frame_reset(self):
+        self._check(self.lib.vor_frame_reset(self.h))
+
+    def vor_frame_device(self, sx, sy):
+        self._check(self.lib.vor_frame_device(self.h, _ptr(sx, torch.int32), _ptr(sy, torch.int32),
+                                              sx.numel(), _stream()))
+
+    def vor_frame_host(self, h_sx, h_sy, h_created, h_destroyed, h_counts):
+        """All arguments are HOST numpy arrays (int32 sites, uint64 lists, int64[3] counts)."""
+        cap = min(len(h_created), len(h_destroyed))
+        self._check(self.lib.vor_frame_host(
+            self.h, h_sx.ctypes.data_as(_P), h_sy.ctypes.data_as(_P), len(h_sx),
+            h_created.ctypes.data_as(_P), h_destroyed.ctypes.data_as(_P), cap,
+            h_counts.ctypes.data_as(_P), _stream()))
+
+    def vor_frame_results(self):
+        """Raw device pointers (ints) of the context-owned results: labels, edges, created,
+        destroyed, counts."""
+        ps = [C.c_void_p() for _ in range(5)]
+        self._check(self.lib.vor_frame_results(self.h, *[C.byref(p) for p in ps]))
+        return tuple(p.value for p in ps)

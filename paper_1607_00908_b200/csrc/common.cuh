@@ -1,0 +1,122 @@
+// Shared declarations of libvor's translation units (context layout, launch helpers).
+// Product code: never includes or links anything from oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/vor.h"
+
+#define FP_ONE 256
+#define FP_HALF 128
+
+constexpr int kNumSMs = 148;               // B200: 2 dies x 74 SMs
+constexpr int kSortBlocks = kNumSMs;       // persistent one-CTA-per-SM kernels (sort, unique, diff)
+constexpr int kSortThreads = 1024;
+
+// error flag bits latched on the device (ctx->d_flags[0])
+enum : int {
+    FLAG_RAWKEY_OVERFLOW = 1,
+    FLAG_EDGE_CAP = 2,
+    FLAG_DIFF_CAP = 4,
+    FLAG_COMP_CAP = 8,
+    FLAG_MATCH_CAP = 16,
+};
+
+struct vor_ctx {
+    int32_t L;
+    int64_t P;                 // 256 * L
+    int32_t max_sites;
+    int64_t max_raw_keys;
+    int device;
+
+    // options
+    int64_t bucket_occ_x100;
+    int64_t label_bits_override;   // 0 = derive from n_sites
+    int64_t label_path;            // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8
+
+    // ---- cell list (a1)
+    int32_t nb_max;            // allocation bound for buckets per side
+    int32_t nb;                // buckets per side of the last build (0 = none)
+    int32_t w;                 // bucket width in fixed-point units, w * nb == P
+    int32_t n_sites;           // of the last build
+    int32_t* d_bucket_start;   // [nb_max^2 + 1]
+    int32_t* d_bucket_fill;    // [nb_max^2]  (scatter cursors)
+    int4* d_sorted;            // [max_sites]  (x, y, original index, bucket)
+    int32_t* d_scan_part;      // scratch for device scans
+
+    // ---- edges (a3/a4)
+    uint64_t* d_keys_a;        // [max_raw_keys]  raw keys / sort ping
+    uint64_t* d_keys_b;        // [max_raw_keys]  sort pong
+    int64_t* d_n_raw;          // device scalar: number of raw keys
+    uint32_t* d_hist;          // [kSortBlocks * 256] per-block digit histograms
+    int64_t* d_blk_count;      // [2 * kSortBlocks] per-block counts for compactions
+    uint8_t* d_mark;           // [max_raw_keys] flags for compactions
+
+    // ---- diff with maps: translated / filtered lists
+    uint64_t* d_tr_prev;       // lazily sized to max_raw_keys
+    uint64_t* d_tr_now;
+    int64_t* d_tr_counts;      // [4]
+
+    // ---- field path (a6..a8)
+    int32_t* d_rank;           // [L*L] root -> component rank
+    int64_t* d_acc;            // [3 * max_comp] n, Sx, Sy
+    int32_t* d_comp_root;      // [max_comp]
+    int32_t max_comp;
+    int32_t* d_comp_count;     // device scalars [4]
+    int32_t* d_best;           // [best_cap] best partner per prev / now (lazily sized)
+    int64_t best_cap;
+
+    // ---- frame pipeline (e2e)
+    int32_t* d_fr_sx;
+    int32_t* d_fr_sy;
+    int32_t* d_fr_labels;      // [L*L]
+    uint64_t* d_fr_edges[2];   // ping-pong prev / now
+    int64_t* d_fr_nedges[2];
+    uint64_t* d_fr_created;
+    uint64_t* d_fr_destroyed;
+    int64_t* d_fr_counts;      // [3]
+    int64_t* h_fr_counts;      // pinned [3]
+    int32_t* h_fr_sites;       // pinned [2 * max_sites]
+    uint64_t* h_fr_lists;      // pinned [2 * fr_cap]
+    int64_t fr_cap;
+    int fr_cur;                // index of the "now" buffer of the last frame; -1 = none
+    int fr_have_prev;
+
+    int32_t* d_flags;          // [1] sticky error bits
+    int64_t launches;
+    char err[512];
+};
+
+inline int vor_fail(vor_ctx* ctx, int code, const char* what) {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", what);
+    return code;
+}
+
+inline int vor_cuda_fail(vor_ctx* ctx, cudaError_t e, const char* where) {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s: %s", where, cudaGetErrorString(e));
+    return VOR_ECUDA;
+}
+
+#define VOR_CUDA(call)                                                          \
+    do {                                                                        \
+        cudaError_t e_ = (call);                                                \
+        if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #call);            \
+    } while (0)
+
+// launch + count + check
+#define VOR_LAUNCH(kernel, grid, block, smem, stream, ...)                      \
+    do {                                                                        \
+        kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);             \
+        ctx->launches++;                                                        \
+        cudaError_t e_ = cudaGetLastError();                                    \
+        if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #kernel);          \
+    } while (0)
+
+// internal entry points shared between translation units
+int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n_in, int key_bits,
+                         uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
+                         cudaStream_t stream);
+int vor_label_bits(const vor_ctx* ctx);

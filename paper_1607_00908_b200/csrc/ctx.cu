@@ -1,0 +1,133 @@
+// Context life cycle, options, sticky status.  See include/vor.h.
+#include <stdlib.h>
+
+#include "common.cuh"
+
+namespace {
+
+template <typename T>
+cudaError_t dmalloc(T** p, size_t n) {
+    return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+}
+
+}  // namespace
+
+extern "C" {
+
+int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys) {
+    if (!out) return VOR_EINVAL;
+    *out = nullptr;
+    if (L < 2 || L > (1 << 22) || max_sites < 1) return VOR_EINVAL;
+    vor_ctx* ctx = (vor_ctx*)calloc(1, sizeof(vor_ctx));
+    if (!ctx) return VOR_ECUDA;
+    ctx->L = L;
+    ctx->P = (int64_t)FP_ONE * L;
+    ctx->max_sites = max_sites;
+    const int64_t worst = 2 * (int64_t)L * L;
+    if (max_raw_keys <= 0) {
+        max_raw_keys = 16 * (int64_t)max_sites;
+        if (max_raw_keys < (1 << 20)) max_raw_keys = 1 << 20;
+    }
+    if (max_raw_keys > worst) max_raw_keys = worst;
+    ctx->max_raw_keys = max_raw_keys;
+    ctx->bucket_occ_x100 = 100;
+    if (const char* e = getenv("VOR_BUCKET_OCC_X100")) ctx->bucket_occ_x100 = atoll(e);
+    ctx->fr_cur = -1;
+    cudaError_t e = cudaGetDevice(&ctx->device);
+    if (e != cudaSuccess) { free(ctx); return VOR_ECUDA; }
+
+    ctx->nb_max = L / 2 < 1 ? 1 : (L / 2 > 4096 ? 4096 : L / 2);
+    const size_t nbuckets = (size_t)ctx->nb_max * ctx->nb_max;
+    bool ok = true;
+    ok = ok && dmalloc(&ctx->d_bucket_start, nbuckets + 1) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_bucket_fill, nbuckets) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_sorted, (size_t)max_sites) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_scan_part, 8192) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_keys_a, (size_t)max_raw_keys) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_keys_b, (size_t)max_raw_keys) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_mark, (size_t)max_raw_keys) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_n_raw, 4) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_hist, (size_t)kSortBlocks * 256) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_blk_count, (size_t)4 * kSortBlocks) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_tr_counts, 4) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_comp_count, 4) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_flags, 4) == cudaSuccess;
+    if (ok) ok = cudaMemset(ctx->d_flags, 0, 4 * sizeof(int32_t)) == cudaSuccess;
+    if (!ok) {
+        vor_destroy(ctx);
+        return VOR_ECUDA;
+    }
+    *out = ctx;
+    return VOR_OK;
+}
+
+int vor_destroy(vor_ctx* ctx) {
+    if (!ctx) return VOR_EINVAL;
+    cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
+    cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
+    cudaFree(ctx->d_mark); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
+    cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts);
+    cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
+    cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best);
+    cudaFree(ctx->d_fr_sx); cudaFree(ctx->d_fr_sy); cudaFree(ctx->d_fr_labels);
+    cudaFree(ctx->d_fr_edges[0]); cudaFree(ctx->d_fr_edges[1]);
+    cudaFree(ctx->d_fr_nedges[0]); cudaFree(ctx->d_fr_nedges[1]);
+    cudaFree(ctx->d_fr_created); cudaFree(ctx->d_fr_destroyed); cudaFree(ctx->d_fr_counts);
+    cudaFreeHost(ctx->h_fr_counts); cudaFreeHost(ctx->h_fr_sites); cudaFreeHost(ctx->h_fr_lists);
+    cudaFree(ctx->d_flags);
+    free(ctx);
+    return VOR_OK;
+}
+
+const char* vor_last_error(const vor_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int64_t vor_launch_count(const vor_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
+    if (!ctx || !name) return VOR_EINVAL;
+    if (!strcmp(name, "bucket_occupancy_x100")) {
+        if (value < 1) return vor_fail(ctx, VOR_EINVAL, "bucket_occupancy_x100 must be >= 1");
+        ctx->bucket_occ_x100 = value;
+        return VOR_OK;
+    }
+    if (!strcmp(name, "label_bits")) {
+        if (value < 0 || value > 31) return vor_fail(ctx, VOR_EINVAL, "label_bits must be in [0,31]");
+        ctx->label_bits_override = value;
+        return VOR_OK;
+    }
+    if (!strcmp(name, "label_path")) {
+        if (value < 0 || value > 3) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,3]");
+        ctx->label_path = value;
+        return VOR_OK;
+    }
+    return vor_fail(ctx, VOR_EINVAL, "unknown option");
+}
+
+int vor_sync_status(vor_ctx* ctx, void* stream) {
+    if (!ctx) return VOR_EINVAL;
+    VOR_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    int32_t flags = 0;
+    VOR_CUDA(cudaMemcpy(&flags, ctx->d_flags, sizeof(flags), cudaMemcpyDeviceToHost));
+    if (flags) {
+        VOR_CUDA(cudaMemset(ctx->d_flags, 0, sizeof(int32_t)));
+        snprintf(ctx->err, sizeof(ctx->err), "capacity exceeded:%s%s%s%s%s",
+                 (flags & FLAG_RAWKEY_OVERFLOW) ? " raw-key scratch (max_raw_keys)" : "",
+                 (flags & FLAG_EDGE_CAP) ? " edge list" : "",
+                 (flags & FLAG_DIFF_CAP) ? " created/destroyed list" : "",
+                 (flags & FLAG_COMP_CAP) ? " component arrays" : "",
+                 (flags & FLAG_MATCH_CAP) ? " match arrays" : "");
+        return VOR_ECAPACITY;
+    }
+    return VOR_OK;
+}
+
+}  // extern "C"
+
+// Number of significant bits of a label value (site index) for the radix sort.
+int vor_label_bits(const vor_ctx* ctx) {
+    if (ctx->label_bits_override > 0) return (int)ctx->label_bits_override;
+    if (ctx->n_sites <= 0) return 31;
+    int bits = 1;
+    while (bits < 31 && ((int64_t)1 << bits) < (int64_t)ctx->n_sites) ++bits;
+    return bits;
+}

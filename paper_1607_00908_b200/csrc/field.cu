@@ -1,0 +1,355 @@
+// a6..a8 — the field-derived front end: bubbles from a thresholded scalar field.
+//  a6 field_threshold_ccl  PAPER.md:95 (§III.A): threshold -> two-valued variable -> cluster labelling
+//                          (the paper adapts the label-equivalence method of its ref. [6]); here a
+//                          lock-free union-find whose roots are the minimum linear index.
+//  a7 field_centroids      PAPER.md:95-101: bubble size by atomic counting, centre of mass = sum of
+//                          the lattice coordinates / size.  Integer sums (order independent), periodic
+//                          unwrap relative to the root cell, one float64 divide.
+//  a8 match_sites          PAPER.md:213, 223: isomorphism P->N from the two sets of centres; mutual
+//                          nearest neighbour within a radius; unmatched = appeared / disappeared.
+#include "common.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------------------------ a6: CCL
+__global__ void ccl_init_kernel(const float* __restrict__ field, float thr, int above, int64_t n,
+                                int32_t* __restrict__ parent) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float v = field[i];
+        const bool m = above ? (v > thr) : (v < thr);      // NaN compares false both ways
+        parent[i] = m ? (int32_t)i : -1;
+    }
+}
+
+__device__ __forceinline__ int32_t uf_find(const int32_t* parent, int32_t a) {
+    int32_t p = parent[a];
+    while (p != a) { a = p; p = parent[a]; }
+    return a;
+}
+
+// roots are always the smallest index of their tree: link the larger root under the smaller one
+__device__ __forceinline__ void uf_union(int32_t* parent, int32_t a, int32_t b) {
+    for (;;) {
+        a = uf_find(parent, a);
+        b = uf_find(parent, b);
+        if (a == b) return;
+        if (a < b) { const int32_t t = a; a = b; b = t; }      // a > b
+        const int32_t old = atomicMin(&parent[a], b);
+        if (old == a) return;
+        a = old;                                                // someone re-rooted a meanwhile
+    }
+}
+
+__global__ void ccl_merge_kernel(int32_t L, int32_t* __restrict__ parent) {
+    const int64_t n = (int64_t)L * L;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        if (parent[i] < 0) continue;
+        const int32_t x = (int32_t)(i % L), y = (int32_t)(i / L);
+        const int64_t r = (int64_t)y * L + (x + 1 == L ? 0 : x + 1);
+        const int64_t d = (int64_t)(y + 1 == L ? 0 : y + 1) * L + x;
+        if (r != i && parent[r] >= 0) uf_union(parent, (int32_t)i, (int32_t)r);
+        if (d != i && parent[d] >= 0) uf_union(parent, (int32_t)i, (int32_t)d);
+    }
+}
+
+__global__ void ccl_flatten_kernel(int64_t n, int32_t* __restrict__ parent) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        if (parent[i] < 0) continue;
+        parent[i] = uf_find(parent, (int32_t)i);
+    }
+}
+
+// ------------------------------------------------------------------------------------ compaction
+// Order-preserving compaction of the items i in [0, n) that satisfy pred(i); persistent chunks.
+constexpr int kCompThreads = 1024;
+
+__device__ __forceinline__ void comp_chunk(int64_t n, int64_t* beg, int64_t* end) {
+    int64_t C = (n + gridDim.x - 1) / gridDim.x;
+    C = (C + kCompThreads - 1) / kCompThreads * kCompThreads;
+    int64_t s = (int64_t)blockIdx.x * C;
+    *beg = s < n ? s : n;
+    *end = s + C < n ? s + C : n;
+}
+
+__device__ __forceinline__ int64_t comp_block_sum(int64_t v, int64_t* sh) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    int64_t t = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    __syncthreads();
+    return t;
+}
+
+template <typename Pred>
+__global__ void __launch_bounds__(kCompThreads) comp_count_kernel(Pred pred, int64_t* __restrict__ blk_count) {
+    __shared__ int64_t sh[32];
+    const int64_t n = pred.size();
+    int64_t beg, end;
+    comp_chunk(n, &beg, &end);
+    int64_t c = 0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kCompThreads) c += pred(i);
+    c = comp_block_sum(c, sh);
+    if (threadIdx.x == 0) blk_count[blockIdx.x] = c;
+}
+
+template <typename Pred, typename Sink>
+__global__ void __launch_bounds__(kCompThreads) comp_write_kernel(Pred pred, Sink sink,
+                                                                  const int64_t* __restrict__ blk_count) {
+    __shared__ int64_t sh[32];
+    __shared__ int32_t wtot[kCompThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t n = pred.size();
+    int64_t beg, end;
+    comp_chunk(n, &beg, &end);
+    int64_t before = 0, all = 0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += kCompThreads) {
+        const int64_t v = blk_count[b];
+        all += v;
+        if (b < (int)blockIdx.x) before += v;
+    }
+    before = comp_block_sum(before, sh);
+    all = comp_block_sum(all, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) sink.total(all);
+    int64_t run = before;
+    for (int64_t sub = beg; sub < end; sub += kCompThreads) {
+        const int64_t i = sub + threadIdx.x;
+        const bool keep = i < end && pred(i);
+        const unsigned ball = __ballot_sync(0xffffffffu, keep);
+        if (lane == 0) wtot[wid] = __popc(ball);
+        __syncthreads();
+        int32_t wbase = 0, total = 0;
+        for (int w = 0; w < kCompThreads / 32; ++w) {
+            const int32_t t = wtot[w];
+            if (w < wid) wbase += t;
+            total += t;
+        }
+        if (keep) sink.put(run + wbase + __popc(ball & ((1u << lane) - 1u)), i);
+        run += total;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------ a7: centroids
+struct RootPred {
+    const int32_t* ccl;
+    int64_t n;
+    __device__ int64_t size() const { return n; }
+    __device__ bool operator()(int64_t i) const { return ccl[i] == (int32_t)i; }
+};
+struct RootSink {
+    int32_t* comp_root;
+    int32_t* rank;
+    int32_t max_comp;
+    int32_t* n_raw;
+    int32_t* flags;
+    __device__ void total(int64_t t) const {
+        *n_raw = (int32_t)(t < max_comp ? t : max_comp);
+        if (t > max_comp) atomicOr(flags, FLAG_COMP_CAP);
+    }
+    __device__ void put(int64_t pos, int64_t i) const {
+        rank[i] = pos < max_comp ? (int32_t)pos : -1;
+        if (pos < max_comp) comp_root[pos] = (int32_t)i;
+    }
+};
+
+__global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const int32_t* __restrict__ rank,
+                                  int32_t L, unsigned long long* __restrict__ acc, int32_t max_comp) {
+    const int64_t n = (int64_t)L * L;
+    const int64_t nround = (n + 31) / 32 * 32;     // keep warps converged for the warp collectives
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t r = i < n ? ccl[i] : -1;
+        const unsigned peers = __match_any_sync(0xffffffffu, r);
+        if (r < 0) continue;                        // whole peer group leaves together
+        const int32_t x = (int32_t)(i % L), y = (int32_t)(i / L), xr = r % L, yr = r / L;
+        int32_t dx = x - xr;
+        if (2 * dx >= L) dx -= L; else if (2 * dx < -L) dx += L;
+        int32_t dy = y - yr;
+        if (2 * dy >= L) dy -= L; else if (2 * dy < -L) dy += L;
+        const int32_t sx = __reduce_add_sync(peers, dx);
+        const int32_t sy = __reduce_add_sync(peers, dy);
+        if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
+            const int32_t k = rank[r];
+            if (k >= 0) {
+                atomicAdd(&acc[k], (unsigned long long)__popc(peers));
+                atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)(long long)sx);
+                atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)(long long)sy);
+            }
+        }
+    }
+}
+
+struct SizePred {
+    const long long* acc;
+    const int32_t* n_raw;
+    int32_t min_size;
+    __device__ int64_t size() const { return *n_raw; }
+    __device__ bool operator()(int64_t k) const { return acc[k] >= (long long)min_size && acc[k] > 0; }
+};
+struct CentroidSink {
+    const long long* acc;
+    const int32_t* comp_root;
+    int32_t max_comp, L, cap;
+    double* cx; double* cy; int32_t* sx; int32_t* sy; int32_t* size; int32_t* root;
+    int32_t* n_comp; int32_t* flags;
+    __device__ void total(int64_t t) const {
+        *n_comp = (int32_t)t;
+        if (t > cap) atomicOr(flags, FLAG_COMP_CAP);
+    }
+    __device__ static long long floor_div(long long a, long long b) {      // b > 0
+        return a >= 0 ? a / b : -((-a + b - 1) / b);
+    }
+    __device__ void put(int64_t pos, int64_t k) const {
+        if (pos >= cap) return;
+        const long long m = acc[k], Sx = acc[(size_t)max_comp + k], Sy = acc[2 * (size_t)max_comp + k];
+        const int32_t r = comp_root[k];
+        const long long xr = r % L, yr = r / L, P = (long long)FP_ONE * L;
+        const long long fx = floor_div(FP_ONE * Sx, m), fy = floor_div(FP_ONE * Sy, m);
+        sx[pos] = (int32_t)((((FP_ONE * xr + FP_HALF + fx) % P) + P) % P);
+        sy[pos] = (int32_t)((((FP_ONE * yr + FP_HALF + fy) % P) + P) % P);
+        double ux = __dadd_rn(__dadd_rn((double)xr, 0.5), __ddiv_rn((double)Sx, (double)m));
+        double uy = __dadd_rn(__dadd_rn((double)yr, 0.5), __ddiv_rn((double)Sy, (double)m));
+        if (ux < 0) ux += L; else if (ux >= L) ux -= L;
+        if (uy < 0) uy += L; else if (uy >= L) uy -= L;
+        cx[pos] = ux; cy[pos] = uy;
+        size[pos] = (int32_t)m;
+        root[pos] = r;
+    }
+};
+
+// ------------------------------------------------------------------------------------ a8: match
+constexpr int kMatchThreads = 256;
+
+// blocks [0, gq) : queries = now, targets = prev -> best[cap_prev + j];  blocks [gq, ..): the reverse
+__global__ void __launch_bounds__(kMatchThreads) match_best_kernel(
+        const int32_t* __restrict__ px, const int32_t* __restrict__ py, const int32_t* __restrict__ n_prev_p,
+        const int32_t* __restrict__ nx, const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
+        int32_t cap_prev, int32_t cap_now, int32_t blocks_now, long long P, long long r2,
+        int32_t* __restrict__ best, int32_t* __restrict__ flags) {
+    __shared__ int32_t tx[kMatchThreads], ty[kMatchThreads];
+    const bool q_is_now = (int)blockIdx.x < blocks_now;
+    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
+    if (blockIdx.x == 0 && threadIdx.x == 0 && (*n_prev_p > cap_prev || *n_now_p > cap_now))
+        atomicOr(flags, FLAG_MATCH_CAP);
+    const int32_t* qx = q_is_now ? nx : px; const int32_t* qy = q_is_now ? ny : py;
+    const int32_t* sx = q_is_now ? px : nx; const int32_t* sy = q_is_now ? py : ny;
+    const int32_t nq = q_is_now ? n_now : n_prev, nt = q_is_now ? n_prev : n_now;
+    const int32_t q = (q_is_now ? blockIdx.x : blockIdx.x - blocks_now) * kMatchThreads + threadIdx.x;
+    if ((q_is_now ? blockIdx.x : blockIdx.x - blocks_now) * kMatchThreads >= nq) return;
+    const long long ax = q < nq ? qx[q] : 0, ay = q < nq ? qy[q] : 0;
+    long long bd = INT64_MAX;
+    int32_t bi = -1;
+    for (int32_t base = 0; base < nt; base += kMatchThreads) {
+        const int32_t t = base + threadIdx.x;
+        __syncthreads();
+        tx[threadIdx.x] = t < nt ? sx[t] : 0;
+        ty[threadIdx.x] = t < nt ? sy[t] : 0;
+        __syncthreads();
+        const int32_t lim = min(kMatchThreads, nt - base);
+        for (int32_t k = 0; k < lim; ++k) {
+            long long dx = ax > tx[k] ? ax - tx[k] : tx[k] - ax; dx = dx < P - dx ? dx : P - dx;
+            long long dy = ay > ty[k] ? ay - ty[k] : ty[k] - ay; dy = dy < P - dy ? dy : P - dy;
+            const long long d2 = dx * dx + dy * dy;
+            if (d2 < bd) { bd = d2; bi = base + k; }
+        }
+    }
+    if (q < nq) best[(q_is_now ? cap_prev : 0) + q] = (bi >= 0 && bd <= r2) ? bi : -1;
+}
+
+__global__ void match_combine_kernel(const int32_t* __restrict__ n_prev_p, const int32_t* __restrict__ n_now_p,
+                                     int32_t cap_prev, int32_t cap_now, const int32_t* __restrict__ best,
+                                     int32_t* __restrict__ p2n, int32_t* __restrict__ n2p) {
+    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
+    const int32_t* bn = best;                 // best now for each prev
+    const int32_t* bp = best + cap_prev;      // best prev for each now
+    for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < cap_prev + cap_now; i += gridDim.x * blockDim.x) {
+        if (i < cap_prev) {
+            int32_t v = -1;
+            if (i < n_prev) { const int32_t j = bn[i]; if (j >= 0 && bp[j] == i) v = j; }
+            p2n[i] = v;
+        } else {
+            const int32_t j = i - cap_prev;
+            int32_t v = -1;
+            if (j < n_now) { const int32_t k = bp[j]; if (k >= 0 && bn[k] == j) v = k; }
+            n2p[j] = v;
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr, int above,
+                                   int32_t* d_ccl, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_field || !d_ccl) return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: null pointer");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int64_t n = (int64_t)ctx->L * ctx->L;
+    const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
+    VOR_LAUNCH(ccl_init_kernel, grid, 256, 0, stream, d_field, thr, above ? 1 : 0, n, d_ccl);
+    VOR_LAUNCH(ccl_merge_kernel, grid, 256, 0, stream, ctx->L, d_ccl);
+    VOR_LAUNCH(ccl_flatten_kernel, grid, 256, 0, stream, n, d_ccl);
+    return VOR_OK;
+}
+
+extern "C" int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_size,
+                               double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
+                               int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp,
+                               void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_ccl || !d_cx || !d_cy || !d_sx || !d_sy || !d_size || !d_root || !d_n_comp || cap < 0)
+        return vor_fail(ctx, VOR_EINVAL, "field_centroids: null pointer or negative capacity");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int64_t n = (int64_t)ctx->L * ctx->L;
+    if (!ctx->d_rank) {
+        int64_t mc = (n + 1) / 2;
+        if (mc > (1 << 22)) mc = 1 << 22;
+        ctx->max_comp = (int32_t)mc;
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_rank, n * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_acc, 3 * (size_t)mc * sizeof(int64_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_comp_root, (size_t)mc * sizeof(int32_t)));
+    }
+    VOR_CUDA(cudaMemsetAsync(ctx->d_acc, 0, 3 * (size_t)ctx->max_comp * sizeof(int64_t), stream));
+    RootPred rp{d_ccl, n};
+    RootSink rs{ctx->d_comp_root, ctx->d_rank, ctx->max_comp, &ctx->d_comp_count[0], ctx->d_flags};
+    VOR_LAUNCH(comp_count_kernel<RootPred>, kNumSMs, kCompThreads, 0, stream, rp, ctx->d_blk_count);
+    VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kNumSMs, kCompThreads, 0, stream, rp, rs,
+               ctx->d_blk_count);
+    const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
+    VOR_LAUNCH(accumulate_kernel, grid, 256, 0, stream, d_ccl, ctx->d_rank, ctx->L,
+               (unsigned long long*)ctx->d_acc, ctx->max_comp);
+    SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
+    CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->L, cap,
+                    d_cx, d_cy, d_sx, d_sy, d_size, d_root, d_n_comp, ctx->d_flags};
+    VOR_LAUNCH(comp_count_kernel<SizePred>, kNumSMs, kCompThreads, 0, stream, sp, ctx->d_blk_count);
+    VOR_LAUNCH((comp_write_kernel<SizePred, CentroidSink>), kNumSMs, kCompThreads, 0, stream, sp, cs,
+               ctx->d_blk_count);
+    return VOR_OK;
+}
+
+extern "C" int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_py,
+                           const int32_t* d_n_prev, const int32_t* d_nx, const int32_t* d_ny,
+                           const int32_t* d_n_now, int32_t cap_prev, int32_t cap_now,
+                           int32_t radius_fp, int32_t* d_p2n, int32_t* d_n2p, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_px || !d_py || !d_n_prev || !d_nx || !d_ny || !d_n_now || !d_p2n || !d_n2p)
+        return vor_fail(ctx, VOR_EINVAL, "match_sites: null pointer");
+    if (cap_prev < 1 || cap_now < 1 || radius_fp < 0)
+        return vor_fail(ctx, VOR_EINVAL, "match_sites: capacities must be >= 1, radius >= 0");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int64_t need = (int64_t)cap_prev + cap_now;
+    if (!ctx->d_best || ctx->best_cap < need) {
+        if (ctx->d_best) { VOR_CUDA(cudaStreamSynchronize(stream)); VOR_CUDA(cudaFree(ctx->d_best)); ctx->d_best = nullptr; }
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_best, need * sizeof(int32_t)));
+        ctx->best_cap = need;
+    }
+    const int bn = (cap_now + kMatchThreads - 1) / kMatchThreads, bp = (cap_prev + kMatchThreads - 1) / kMatchThreads;
+    VOR_LAUNCH(match_best_kernel, bn + bp, kMatchThreads, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny,
+               d_n_now, cap_prev, cap_now, bn, (long long)ctx->P, (long long)radius_fp * radius_fp,
+               ctx->d_best, ctx->d_flags);
+    VOR_LAUNCH(match_combine_kernel, 2 * kNumSMs, 256, 0, stream, d_n_prev, d_n_now, cap_prev, cap_now,
+               ctx->d_best, d_p2n, d_n2p);
+    return VOR_OK;
+}

@@ -1,0 +1,119 @@
+// One site-driven frame of the hot path (a1..a5) on context-owned buffers: the call a user makes
+// once per simulation snapshot (the paper's "trigger").  The previous frame's
+// edge list is the only state carried between calls.
+#include "common.cuh"
+
+namespace {
+
+__global__ void gather_counts_kernel(const int64_t* __restrict__ n_edges, const int64_t* __restrict__ n_created,
+                                     const int64_t* __restrict__ n_destroyed, int64_t* __restrict__ out) {
+    out[0] = *n_edges; out[1] = *n_created; out[2] = *n_destroyed;
+}
+
+int ensure_frame_buffers(vor_ctx* ctx) {
+    if (ctx->d_fr_labels) return VOR_OK;
+    const size_t cells = (size_t)ctx->L * ctx->L;
+    int64_t cap = 4 * (int64_t)ctx->max_sites + 1024;
+    if (cap > ctx->max_raw_keys) cap = ctx->max_raw_keys;
+    ctx->fr_cap = cap;
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_sx, (size_t)ctx->max_sites * sizeof(int32_t)));
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_sy, (size_t)ctx->max_sites * sizeof(int32_t)));
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_labels, cells * sizeof(int32_t)));
+    for (int k = 0; k < 2; ++k) {
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_edges[k], (size_t)cap * sizeof(uint64_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_nedges[k], sizeof(int64_t)));
+        VOR_CUDA(cudaMemset(ctx->d_fr_nedges[k], 0, sizeof(int64_t)));
+    }
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_created, (size_t)cap * sizeof(uint64_t)));
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_destroyed, (size_t)cap * sizeof(uint64_t)));
+    VOR_CUDA(cudaMalloc((void**)&ctx->d_fr_counts, 4 * sizeof(int64_t)));
+    VOR_CUDA(cudaMallocHost((void**)&ctx->h_fr_counts, 4 * sizeof(int64_t)));
+    VOR_CUDA(cudaMallocHost((void**)&ctx->h_fr_sites, 2 * (size_t)ctx->max_sites * sizeof(int32_t)));
+    VOR_CUDA(cudaMallocHost((void**)&ctx->h_fr_lists, 2 * (size_t)cap * sizeof(uint64_t)));
+    ctx->fr_cur = -1;
+    return VOR_OK;
+}
+
+}  // namespace
+
+extern "C" int vor_frame_reset(vor_ctx* ctx) {
+    if (!ctx) return VOR_EINVAL;
+    ctx->fr_cur = -1;
+    return VOR_OK;
+}
+
+extern "C" int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
+                                int32_t n_sites, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    int rc = ensure_frame_buffers(ctx);
+    if (rc != VOR_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int now = ctx->fr_cur < 0 ? 0 : 1 - ctx->fr_cur, prev = 1 - now;
+    if (ctx->fr_cur < 0) VOR_CUDA(cudaMemsetAsync(ctx->d_fr_nedges[prev], 0, sizeof(int64_t), stream));
+    if ((rc = vor_build_cells(ctx, d_sx, d_sy, n_sites, stream)) != VOR_OK) return rc;
+    if ((rc = vor_label(ctx, ctx->d_fr_labels, stream)) != VOR_OK) return rc;
+    if ((rc = vor_edges(ctx, ctx->d_fr_labels, ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now],
+                        stream)) != VOR_OK) return rc;
+    if ((rc = vor_diff(ctx, ctx->d_fr_edges[prev], ctx->d_fr_nedges[prev], ctx->d_fr_edges[now],
+                       ctx->d_fr_nedges[now], nullptr, nullptr, 0, 0, ctx->d_fr_created,
+                       ctx->d_fr_destroyed, ctx->fr_cap, &ctx->d_fr_counts[1], &ctx->d_fr_counts[2],
+                       stream)) != VOR_OK) return rc;
+    VOR_LAUNCH(gather_counts_kernel, 1, 1, 0, stream, ctx->d_fr_nedges[now], &ctx->d_fr_counts[1],
+               &ctx->d_fr_counts[2], ctx->d_fr_counts);
+    ctx->fr_cur = now;
+    return VOR_OK;
+}
+
+extern "C" int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
+                              uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
+                              int64_t* h_counts, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!h_sx || !h_sy || !h_counts || cap < 0 || (cap > 0 && (!h_created || !h_destroyed)))
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_host: null pointer or negative capacity");
+    if (n_sites < 1 || n_sites > ctx->max_sites)
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_host: n_sites out of range");
+    int rc = ensure_frame_buffers(ctx);
+    if (rc != VOR_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    // stage through pinned memory so the copies are true async DMA whatever the caller's buffers are
+    memcpy(ctx->h_fr_sites, h_sx, (size_t)n_sites * sizeof(int32_t));
+    memcpy(ctx->h_fr_sites + ctx->max_sites, h_sy, (size_t)n_sites * sizeof(int32_t));
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sx, ctx->h_fr_sites, (size_t)n_sites * sizeof(int32_t),
+                             cudaMemcpyHostToDevice, stream));
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sy, ctx->h_fr_sites + ctx->max_sites,
+                             (size_t)n_sites * sizeof(int32_t), cudaMemcpyHostToDevice, stream));
+    if ((rc = vor_frame_device(ctx, ctx->d_fr_sx, ctx->d_fr_sy, n_sites, stream)) != VOR_OK) return rc;
+    VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_counts, ctx->d_fr_counts, 3 * sizeof(int64_t),
+                             cudaMemcpyDeviceToHost, stream));
+    VOR_CUDA(cudaStreamSynchronize(stream));
+    h_counts[0] = ctx->h_fr_counts[0]; h_counts[1] = ctx->h_fr_counts[1]; h_counts[2] = ctx->h_fr_counts[2];
+    int64_t nc = h_counts[1] < ctx->fr_cap ? h_counts[1] : ctx->fr_cap;
+    int64_t nd = h_counts[2] < ctx->fr_cap ? h_counts[2] : ctx->fr_cap;
+    if (nc > cap) nc = cap;
+    if (nd > cap) nd = cap;
+    if (nc > 0)
+        VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_lists, ctx->d_fr_created, (size_t)nc * sizeof(uint64_t),
+                                 cudaMemcpyDeviceToHost, stream));
+    if (nd > 0)
+        VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_lists + ctx->fr_cap, ctx->d_fr_destroyed,
+                                 (size_t)nd * sizeof(uint64_t), cudaMemcpyDeviceToHost, stream));
+    rc = vor_sync_status(ctx, stream);
+    if (nc > 0) memcpy(h_created, ctx->h_fr_lists, (size_t)nc * sizeof(uint64_t));
+    if (nd > 0) memcpy(h_destroyed, ctx->h_fr_lists + ctx->fr_cap, (size_t)nd * sizeof(uint64_t));
+    if (rc == VOR_OK && (h_counts[1] > cap || h_counts[2] > cap))
+        return vor_fail(ctx, VOR_ECAPACITY, "vor_frame_host: created/destroyed list larger than cap");
+    return rc;
+}
+
+extern "C" int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const uint64_t** d_edges,
+                                 const uint64_t** d_created, const uint64_t** d_destroyed,
+                                 const int64_t** d_counts) {
+    if (!ctx) return VOR_EINVAL;
+    if (ctx->fr_cur < 0 || !ctx->d_fr_labels) return vor_fail(ctx, VOR_ESTATE, "no frame processed yet");
+    if (d_labels) *d_labels = ctx->d_fr_labels;
+    if (d_edges) *d_edges = ctx->d_fr_edges[ctx->fr_cur];
+    if (d_created) *d_created = ctx->d_fr_created;
+    if (d_destroyed) *d_destroyed = ctx->d_fr_destroyed;
+    if (d_counts) *d_counts = ctx->d_fr_counts;
+    return VOR_OK;
+}

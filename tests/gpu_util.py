@@ -1,0 +1,103 @@
+"""Helpers for the -m gpu parity tests: thin wrappers that run one libvor call on numpy inputs."""
+import ctypes as C
+
+import numpy as np
+import torch
+
+from paper_1607_00908_b200.binding import Vor
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def u64(t, n=None):
+    a = t.cpu().numpy().view(np.uint64)
+    return a if n is None else a[:n]
+
+
+def gpu_labels(v: Vor, sx, sy):
+    dsx, dsy = dev(sx), dev(sy)
+    lab = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")
+    v.vor_build_cells(dsx, dsy)
+    v.vor_label(lab)
+    v.vor_sync_status()
+    return lab.cpu().numpy().reshape(v.L, v.L)
+
+
+def gpu_edges(v: Vor, labels, cap=None):
+    L = v.L
+    cap = cap or max(1024, 8 * v.max_sites)
+    d = dev(labels.astype(np.int32).ravel())
+    out = torch.empty(cap, dtype=torch.int64, device="cuda")
+    n = torch.zeros(1, dtype=torch.int64, device="cuda")
+    v.vor_edges(d, out, n)
+    v.vor_sync_status()
+    return u64(out, int(n.item())).copy()
+
+
+def gpu_diff(v: Vor, prev, now, p2n=None, n2p=None):
+    cap = max(1, len(prev) + len(now))
+    dp = dev(np.asarray(prev, np.uint64).view(np.int64)) if len(prev) else torch.empty(1, dtype=torch.int64, device="cuda")
+    dn = dev(np.asarray(now, np.uint64).view(np.int64)) if len(now) else torch.empty(1, dtype=torch.int64, device="cuda")
+    npv = torch.tensor([len(prev)], dtype=torch.int64, device="cuda")
+    nnv = torch.tensor([len(now)], dtype=torch.int64, device="cuda")
+    c = torch.empty(cap, dtype=torch.int64, device="cuda")
+    d = torch.empty(cap, dtype=torch.int64, device="cuda")
+    nc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nd = torch.zeros(1, dtype=torch.int64, device="cuda")
+    kw = {}
+    if p2n is not None:
+        kw = dict(p2n=dev(np.asarray(p2n, np.int32)), n2p=dev(np.asarray(n2p, np.int32)),
+                  n_prev_labels=len(p2n), n_now_labels=len(n2p))
+    v.vor_diff(dp, npv, dn, nnv, c, d, nc, nd, **kw)
+    v.vor_sync_status()
+    return u64(c, int(nc.item())).copy(), u64(d, int(nd.item())).copy()
+
+
+def gpu_ccl(v: Vor, field, thr, above=True):
+    f = dev(field.astype(np.float32).ravel())
+    ccl = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")
+    v.field_threshold_ccl(f, thr, above, ccl)
+    v.vor_sync_status()
+    return ccl
+
+
+def gpu_centroids(v: Vor, ccl_dev, min_size, cap=None):
+    cap = cap or max(16, v.L * v.L // 2)
+    cx = torch.empty(cap, dtype=torch.float64, device="cuda"); cy = torch.empty_like(cx)
+    sx = torch.empty(cap, dtype=torch.int32, device="cuda"); sy = torch.empty_like(sx)
+    size = torch.empty_like(sx); root = torch.empty_like(sx)
+    n = torch.zeros(1, dtype=torch.int32, device="cuda")
+    v.field_centroids(ccl_dev, min_size, cx, cy, sx, sy, size, root, n)
+    v.vor_sync_status()
+    K = int(n.item())
+    g = lambda t: t[:K].cpu().numpy()
+    return dict(cx=g(cx), cy=g(cy), sx=g(sx), sy=g(sy), size=g(size), root=g(root))
+
+
+def gpu_match(v: Vor, px, py, nx, ny, radius_fp, pad=7):
+    """pad > 0 exercises capacity > count."""
+    P, N = len(px), len(nx)
+    mk = lambda a, n: dev(np.concatenate([np.asarray(a, np.int32), np.zeros(pad, np.int32)]))
+    dpx, dpy, dnx, dny = mk(px, P), mk(py, P), mk(nx, N), mk(ny, N)
+    p2n = torch.full((P + pad,), -7, dtype=torch.int32, device="cuda")
+    n2p = torch.full((N + pad,), -7, dtype=torch.int32, device="cuda")
+    v.match_sites(dpx, dpy, torch.tensor([P], dtype=torch.int32, device="cuda"),
+                  dnx, dny, torch.tensor([N], dtype=torch.int32, device="cuda"), radius_fp, p2n, n2p)
+    v.vor_sync_status()
+    return p2n[:P].cpu().numpy(), n2p[:N].cpu().numpy()
+
+
+def from_device_ptr(ptr, count, dtype):
+    """Copy `count` elements of torch dtype from a raw device pointer into a new tensor."""
+    t = torch.empty(count, dtype=dtype, device="cuda")
+    if count:
+        cudart = C.CDLL("libcudart.so.12")
+        rc = cudart.cudaMemcpy(C.c_void_p(t.data_ptr()), C.c_void_p(ptr),
+                               C.c_size_t(count * t.element_size()), C.c_int(3))
+        assert rc == 0, rc
+    return t

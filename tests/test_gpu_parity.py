@@ -1,0 +1,335 @@
+"""-m gpu: element-by-element parity of the CUDA path (through the C ABI) with the CPU oracle.
+
+Integer / index work: bit-exact.  Centroids (float64): |diff| <= 1e-9 lattice units (north_star).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from helpers import FP, hex_sites, pack, pairs, read_golden, rhombus_sites
+from paper_1607_00908_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import gpu_util
+    return gpu_util
+
+
+def make(L, max_sites, **kw):
+    from paper_1607_00908_b200.binding import Vor
+    return Vor(L, max_sites, **kw)
+
+
+def rnd(seed, L, n):
+    rng = np.random.default_rng(seed)
+    return rng.integers(0, FP * L, n).astype(np.int32), rng.integers(0, FP * L, n).astype(np.int32)
+
+
+# ------------------------------------------------------------------ labels (a1 + a2)
+def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3), ref=None, occ=None):
+    ref = oracle.label_brute(L, sx, sy) if ref is None else ref
+    v = make(L, max(len(sx), 1))
+    if occ:
+        v.vor_set_option("bucket_occupancy_x100", occ)
+    for path in paths:
+        v.vor_set_option("label_path", path)
+        got = G.gpu_labels(v, sx, sy)
+        bad = np.argwhere(got != ref)
+        assert len(bad) == 0, f"path {path}: {len(bad)} cells differ, first {bad[:5].tolist()}"
+    v.close()
+
+
+def test_labels_config1_both_frames(G):
+    w = W.config(1)
+    for sx, sy in w.frames():
+        check_labels(G, w.L, sx, sy)
+
+
+def test_labels_config2_two_frames(G):
+    w = W.config(2)
+    for sx, sy in w.frames(2):
+        check_labels(G, w.L, sx, sy)
+
+
+@pytest.mark.parametrize("L", [512, 1024])
+def test_labels_scaled_config5(G, L):
+    w = W.scaled(5, L)
+    fr = list(w.frames(6))
+    for sx, sy in (fr[0], fr[5]):
+        check_labels(G, L, sx, sy, ref=oracle.label_cells(L, sx, sy, 16))
+
+
+ADVERSARIAL = [
+    ("single", 64, lambda rng, P: (np.array([5], np.int32), np.array([P - 1], np.int32))),
+    ("one_bucket", 64, lambda rng, P: (rng.integers(0, 8 * FP, 30).astype(np.int32),
+                                       rng.integers(0, 8 * FP, 30).astype(np.int32))),
+    ("empty_quadrants", 256, lambda rng, P: (rng.integers(0, P // 4, 200).astype(np.int32),
+                                             rng.integers(P // 2, 3 * P // 4, 200).astype(np.int32))),
+    ("corners", 64, lambda rng, P: (np.array([0, P - 1, 0, P - 1], np.int32),
+                                    np.array([0, 0, P - 1, P - 1], np.int32))),
+    ("lattice_aligned_ties", 256, lambda rng, P: ((rng.integers(0, 16, 150) * 16 * FP + 128).astype(np.int32),
+                                                  (rng.integers(0, 16, 150) * 16 * FP + 128).astype(np.int32))),
+    ("regular_grid_all_ties", 256, lambda rng, P: (np.tile(np.arange(16) * 16 * FP, 16).astype(np.int32),
+                                                   np.repeat(np.arange(16) * 16 * FP, 16).astype(np.int32))),
+    ("dense", 48, lambda rng, P: (rng.integers(0, P, 3000).astype(np.int32),
+                                  rng.integers(0, P, 3000).astype(np.int32))),
+    ("duplicates", 128, lambda rng, P: (np.repeat(rng.integers(0, P, 40), 3).astype(np.int32),
+                                        np.repeat(rng.integers(0, P, 40), 3).astype(np.int32))),
+    ("cluster_plus_void", 512, lambda rng, P: (np.concatenate([rng.integers(0, P // 16, 300), rng.integers(0, P, 30)]).astype(np.int32),
+                                               np.concatenate([rng.integers(0, P // 16, 300), rng.integers(0, P, 30)]).astype(np.int32))),
+]
+
+
+@pytest.mark.parametrize("name,L,gen", ADVERSARIAL, ids=[a[0] for a in ADVERSARIAL])
+def test_labels_adversarial(G, name, L, gen):
+    rng = np.random.default_rng(abs(hash(name)) % 2**32)
+    sx, sy = gen(rng, FP * L)
+    check_labels(G, L, sx, sy)
+
+
+@pytest.mark.parametrize("L,n", [(100, 40), (250, 434), (17, 5), (2, 1), (2, 3), (333, 3000), (1000, 3000)])
+def test_labels_ragged_lattices(G, L, n):
+    sx, sy = rnd(L * 7 + n, L, n)
+    check_labels(G, L, sx, sy)
+
+
+@pytest.mark.parametrize("occ", [25, 400])
+def test_labels_bucket_size_independent(G, occ):
+    w = W.scaled(5, 512)
+    sx, sy = next(iter(w.frames(1)))
+    check_labels(G, 512, sx, sy, occ=occ)
+
+
+def test_labels_hex_and_rhombus_constructions(G):
+    g = read_golden("hex_lattice.txt")
+    sx, sy = hex_sites(g["L"][0], g["cols"][0], g["rows"][0], g["jitter"][0], seed=3)
+    check_labels(G, g["L"][0], sx, sy)
+    sx, sy = rhombus_sites(256, 24)        # exactly cocircular rhombus: ties along Voronoi edges
+    check_labels(G, 256, sx, sy)
+
+
+# ------------------------------------------------------------------ edges (a3 + a4)
+def check_edges(G, labels, max_sites):
+    L = labels.shape[0]
+    v = make(L, max_sites)
+    got = G.gpu_edges(v, labels, cap=max(1024, 2 * L * L))
+    ref = oracle.edges(labels)
+    v.close()
+    assert got.dtype == np.uint64 and np.array_equal(got, ref), (len(got), len(ref))
+
+
+def test_edges_hand_images(G):
+    lab = np.array([[3, 3, 7, 7], [3, 3, 7, 7], [3, 5, 7, 7], [3, 3, 7, 7]], dtype=np.int32)
+    check_edges(G, lab, 8)
+    check_edges(G, np.full((6, 6), 9, np.int32), 16)           # no edges at all
+    lab = np.zeros((6, 6), np.int32); lab[:, 5] = 2; lab[5, :] = 4   # wrap-only adjacency
+    check_edges(G, lab, 8)
+    rng = np.random.default_rng(0)
+    check_edges(G, rng.integers(0, 1000, (37, 37)).astype(np.int32), 1000)      # ragged, noise labels
+    check_edges(G, rng.integers(0, 2 ** 31 - 1, (64, 64)).astype(np.int32), 1)  # 31-bit labels
+    check_edges(G, rng.integers(0, 50000, (256, 256)).astype(np.int32), 50000)  # hash-set overflow path
+
+
+@pytest.mark.parametrize("cfg,L", [(1, None), (2, None), (5, 512), (5, 1000), (5, 2048)])
+def test_edges_on_oracle_labels(G, cfg, L):
+    w = W.config(cfg) if L is None else W.scaled(cfg, L)
+    sx, sy = next(iter(w.frames(1)))
+    lab = oracle.label_cells(w.L, sx, sy, 8)
+    check_edges(G, lab, w.n_sites)
+
+
+def test_edges_capacity_overflow_is_reported(G):
+    from paper_1607_00908_b200.binding import VorError, VOR_ECAPACITY
+    w = W.scaled(5, 512)
+    sx, sy = next(iter(w.frames(1)))
+    lab = oracle.label_cells(w.L, sx, sy, 16)
+    ref = oracle.edges(lab)
+    v = make(w.L, w.n_sites)
+    d = G.dev(lab.ravel())
+    out = torch.full((100,), -1, dtype=torch.int64, device="cuda")
+    guard = out[90:]                                   # cap = 90: entries beyond must stay untouched
+    n = torch.zeros(1, dtype=torch.int64, device="cuda")
+    v.lib.vor_edges(v.h, d.data_ptr(), out.data_ptr(), 90, n.data_ptr(), None)
+    with pytest.raises(VorError) as e:
+        v.vor_sync_status()
+    assert e.value.status == VOR_ECAPACITY
+    assert int(n.item()) == len(ref)                   # required count is reported
+    assert np.array_equal(G.u64(out, 90), ref[:90]) and bool((guard == -1).all())
+    v.vor_sync_status()                                # sticky flag was cleared
+    v.close()
+
+
+# ------------------------------------------------------------------ diff (a5)
+def test_diff_hand_and_random(G):
+    v = make(64, 64)
+    prev = pack([(0, 1), (0, 2), (1, 2), (2, 5), (7, 9)])
+    now = pack([(0, 1), (1, 2), (1, 5), (2, 5), (3, 4), (7, 9)])
+    for a, b in ((prev, now), (now, prev), (prev, prev), (np.empty(0, np.uint64), now), (now, np.empty(0, np.uint64))):
+        c, d = G.gpu_diff(v, a, b)
+        rc, rd = oracle.diff(a, b)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd)
+    rng = np.random.default_rng(5)
+    for n in (10, 5000, 200000):
+        mk = lambda: np.unique((rng.integers(0, 3000, n).astype(np.uint64) << np.uint64(32))
+                               | rng.integers(3000, 6000, n).astype(np.uint64))
+        a, b = mk(), mk()
+        c, d = G.gpu_diff(v, a, b)
+        rc, rd = oracle.diff(a, b)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd)
+    v.close()
+
+
+def test_diff_with_maps(G):
+    v = make(64, 64)
+    p2n = np.array([2, 0, -1, 1], np.int32); n2p = np.array([1, 3, 0, -1], np.int32)
+    prev = pack([(0, 1), (0, 2), (1, 3), (2, 3)]); now = pack([(0, 1), (1, 2), (0, 3), (2, 3)])
+    c, d = G.gpu_diff(v, prev, now, p2n, n2p)
+    rc, rd = oracle.diff(prev, now, p2n, n2p)
+    assert np.array_equal(c, rc) and np.array_equal(d, rd) and pairs(c) == {(1, 2)} and pairs(d) == {(0, 2)}
+    rng = np.random.default_rng(8)
+    for _ in range(3):
+        K = 500
+        perm = rng.permutation(K).astype(np.int32)
+        p2n = perm.copy(); p2n[rng.random(K) < 0.1] = -1
+        n2p = np.full(K, -1, np.int32); ok = p2n >= 0; n2p[p2n[ok]] = np.nonzero(ok)[0]
+        mk = lambda: np.unique((rng.integers(0, K // 2, 3000).astype(np.uint64) << np.uint64(32))
+                               | rng.integers(K // 2, K, 3000).astype(np.uint64))
+        a, b = mk(), mk()
+        c, d = G.gpu_diff(v, a, b, p2n, n2p)
+        rc, rd = oracle.diff(a, b, p2n, n2p)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd)
+    v.close()
+
+
+def test_rhombus_flip_end_to_end_golden(G):
+    g = read_golden("rhombus_flip.txt")
+    L = g["L"][0]
+    v = make(L, 14)
+    e = []
+    for h in (g["h_prev"][0], g["h_now"][0]):
+        sx, sy = rhombus_sites(L, h)
+        e.append(G.gpu_edges(v, G.gpu_labels(v, sx, sy)))
+    c, d = G.gpu_diff(v, e[0], e[1])
+    assert pairs(c) == {tuple(g["created"])} and pairs(d) == {tuple(g["destroyed"])}
+    assert len(e[0]) == len(e[1]) == g["n_edges_each"][0]
+    v.close()
+
+
+# ------------------------------------------------------------------ frame pipeline (a1..a5 chained)
+@pytest.mark.parametrize("cfg,L,nfr", [(1, None, 2), (2, None, 4), (5, 1024, 4)])
+def test_frame_host_sequence_matches_oracle(G, cfg, L, nfr):
+    w = W.config(cfg) if L is None else W.scaled(cfg, L)
+    v = make(w.L, w.n_sites)
+    cap = 8 * w.n_sites + 64
+    hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+    prev = np.empty(0, np.uint64)
+    for sx, sy in w.frames(nfr):
+        v.vor_frame_host(sx, sy, hc, hd, cnt)
+        lab = oracle.label_cells(w.L, sx, sy, w.bucket_cells)
+        e = oracle.edges(lab)
+        rc, rd = oracle.diff(prev, e)
+        assert cnt.tolist() == [len(e), len(rc), len(rd)]
+        assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd)
+        pl, pe, _, _, _ = v.vor_frame_results()
+        assert np.array_equal(G.from_device_ptr(pl, w.L * w.L, torch.int32).cpu().numpy().reshape(w.L, w.L), lab)
+        assert np.array_equal(G.u64(G.from_device_ptr(pe, len(e), torch.int64)), e)
+        prev = e
+    v.close()
+
+
+# ------------------------------------------------------------------ field path (a6..a8)
+def check_field_frame(G, v, field, thr, min_size, above=True):
+    ref_ccl = oracle.threshold_ccl(field, thr, above)
+    ccl = G.gpu_ccl(v, field, thr, above)
+    got = ccl.cpu().numpy().reshape(v.L, v.L)
+    assert np.array_equal(got, ref_ccl), f"{(got != ref_ccl).sum()} ccl cells differ"
+    rc = oracle.centroids(ref_ccl, min_size)
+    gc = G.gpu_centroids(v, ccl, min_size)
+    for k in ("sx", "sy", "size", "root"):
+        assert np.array_equal(gc[k], rc[k]), k
+    assert len(gc["cx"]) == len(rc["cx"])
+    if len(rc["cx"]):
+        assert np.abs(gc["cx"] - rc["cx"]).max() <= 1e-9 and np.abs(gc["cy"] - rc["cy"]).max() <= 1e-9
+    return rc
+
+
+def test_ccl_and_centroids_hand_cases(G):
+    L = 8
+    v = make(L, 64)
+    f = np.zeros((L, L), np.float32)
+    f[0, 0] = f[0, 7] = f[7, 0] = 2; f[4, :] = 2; f[2, 3] = 2
+    check_field_frame(G, v, f, 1.0, 1)
+    check_field_frame(G, v, np.full((L, L), 5, np.float32), 1.0, 1)
+    check_field_frame(G, v, np.zeros((L, L), np.float32), 1.0, 1)
+    check_field_frame(G, v, np.zeros((L, L), np.float32), 1.0, 1, above=False)
+    check_field_frame(G, v, np.full((L, L), np.nan, np.float32), 1.0, 1)
+    check_field_frame(G, v, np.full((L, L), 1.0, np.float32), 1.0, 1)
+    check_field_frame(G, v, np.full((L, L), 1e-40, np.float32), 0.0, 1)      # denormal > 0
+    v.close()
+
+
+@pytest.mark.parametrize("L,p,seed", [(64, 0.4, 0), (100, 0.59, 1), (257, 0.62, 2), (512, 0.5, 3)])
+def test_ccl_and_centroids_random_masks(G, L, p, seed):
+    rng = np.random.default_rng(seed)
+    v = make(L, 1024)
+    check_field_frame(G, v, rng.random((L, L)).astype(np.float32), 1.0 - p, 1)
+    check_field_frame(G, v, rng.random((L, L)).astype(np.float32), 1.0 - p, 20)
+    v.close()
+
+
+def test_ccl_serpentine_long_chains(G):
+    L = 256
+    f = np.zeros((L, L), np.float32)
+    f[::2, :] = 1                                  # rows, joined alternately at the ends: one snake
+    f[1::4, L - 1] = 1
+    f[3::4, 0] = 1
+    v = make(L, 16)
+    check_field_frame(G, v, f, 0.5, 1)
+    v.close()
+
+
+@pytest.mark.parametrize("cfg,L,nfr", [(3, 256, 3), (3, 1024, 2), (4, 512, 3)])
+def test_field_pipeline_scaled_configs(G, cfg, L, nfr):
+    """threshold -> CCL -> centroids -> match -> label -> edges -> diff(maps), frame by frame."""
+    w = W.scaled(cfg, L)
+    v = make(L, 65536)
+    R = int(w.match_radius_cells * FP)
+    prev_c, prev_e = None, None
+    for field in w.frames(nfr):
+        rc = check_field_frame(G, v, field, w.threshold, w.min_size)
+        K = len(rc["sx"])
+        assert K > 3
+        lab = oracle.label_cells(L, rc["sx"], rc["sy"], 16 if L % 16 == 0 else 1)
+        assert np.array_equal(G.gpu_labels(v, rc["sx"], rc["sy"]), lab)
+        e = oracle.edges(lab)
+        assert np.array_equal(G.gpu_edges(v, lab), e)
+        if prev_c is not None:
+            p2n, n2p = oracle.match(L, prev_c["sx"], prev_c["sy"], rc["sx"], rc["sy"], R)
+            gp, gn = G.gpu_match(v, prev_c["sx"], prev_c["sy"], rc["sx"], rc["sy"], R)
+            assert np.array_equal(gp, p2n) and np.array_equal(gn, n2p)
+            assert (p2n >= 0).mean() > 0.5
+            c, d = G.gpu_diff(v, prev_e, e, p2n, n2p)
+            oc, od = oracle.diff(prev_e, e, p2n, n2p)
+            assert np.array_equal(c, oc) and np.array_equal(d, od)
+        prev_c, prev_e = rc, e
+    v.close()
+
+
+def test_match_invariants_and_random(G):
+    v = make(64, 256)
+    rng = np.random.default_rng(13)
+    P = FP * 64
+    for _ in range(4):
+        px, py = rng.integers(0, P, 80).astype(np.int32), rng.integers(0, P, 80).astype(np.int32)
+        nx, ny = rng.integers(0, P, 70).astype(np.int32), rng.integers(0, P, 70).astype(np.int32)
+        for R in (0, 3 * FP, 6 * FP, 40 * FP):
+            a, b = G.gpu_match(v, px, py, nx, ny, R)
+            ra, rb = oracle.match(64, px, py, nx, ny, R)
+            assert np.array_equal(a, ra) and np.array_equal(b, rb)
+    a, b = G.gpu_match(v, np.array([1000, 1000]), np.array([1000, 1000]), np.array([1100]), np.array([1000]), 4 * FP)
+    assert a.tolist() == [0, -1] and b.tolist() == [0]
+    v.close()
