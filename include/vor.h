@@ -60,7 +60,7 @@ int vor_sync_status(vor_ctx* ctx, void* stream);
 int64_t vor_launch_count(const vor_ctx* ctx);
 
 /* Tuning knobs (integers).  Unknown names -> VOR_EINVAL.
- *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 100) */
+ *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 25) */
 int vor_set_option(vor_ctx* ctx, const char* name, int64_t value);
 
 /* ---- a1: counting-sort cell list of the sites (not in the paper, which loops over all centres,

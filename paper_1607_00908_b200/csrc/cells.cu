@@ -5,6 +5,8 @@
 // Layout: d_bucket_start[nb*nb + 1] (exclusive prefix), d_sorted[n] = int4(x, y, original index,
 // bucket) in bucket order.  Order inside a bucket is arbitrary (atomic cursors); the label kernel
 // never depends on it because ties are resolved by the original index explicitly.
+#include <math.h>
+
 #include "common.cuh"
 
 namespace {
@@ -123,12 +125,15 @@ extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t*
         return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: n_sites out of range [1, max_sites]");
     cudaStream_t stream = (cudaStream_t)stream_;
 
-    // buckets per side: ~ sqrt(n / occupancy), bucket >= 2 cells, nb divides P
-    double target = (double)n_sites * 100.0 / (double)ctx->bucket_occ_x100;
-    int64_t nb = 1;
-    while ((nb + 1) * (nb + 1) <= target) ++nb;
-    if (nb > ctx->nb_max) nb = ctx->nb_max;
-    while (nb > 1 && ctx->P % nb != 0) --nb;
+    // buckets per side: the divisor of P nearest (in ratio) to sqrt(n / occupancy), bucket >= 2 cells
+    const double target = sqrt((double)n_sites * 100.0 / (double)ctx->bucket_occ_x100);
+    int64_t lo = (int64_t)target, hi = (int64_t)target + 1;
+    if (lo < 1) lo = 1;
+    if (lo > ctx->nb_max) lo = ctx->nb_max;
+    while (lo > 1 && ctx->P % lo != 0) --lo;
+    while (hi <= ctx->nb_max && ctx->P % hi != 0) ++hi;
+    int64_t nb = lo;
+    if (hi <= ctx->nb_max && (double)hi / target < target / (double)lo) nb = hi;
     ctx->nb = (int32_t)nb;
     ctx->w = (int32_t)(ctx->P / nb);
     ctx->n_sites = n_sites;

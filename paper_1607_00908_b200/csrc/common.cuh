@@ -36,6 +36,8 @@ struct vor_ctx {
     int64_t bucket_occ_x100;
     int64_t label_bits_override;   // 0 = derive from n_sites
     int64_t label_path;            // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8
+    int64_t label_halo_x100;       // fast-path halo = r_quad + this/100 * mean site spacing
+    int64_t label_fast_off;        // 1 = skip the quadrant fast path (testing)
 
     // ---- cell list (a1)
     int32_t nb_max;            // allocation bound for buckets per side

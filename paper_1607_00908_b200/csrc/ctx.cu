@@ -30,7 +30,8 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     }
     if (max_raw_keys > worst) max_raw_keys = worst;
     ctx->max_raw_keys = max_raw_keys;
-    ctx->bucket_occ_x100 = 100;
+    ctx->bucket_occ_x100 = 25;
+    ctx->label_halo_x100 = 90;
     if (const char* e = getenv("VOR_BUCKET_OCC_X100")) ctx->bucket_occ_x100 = atoll(e);
     ctx->fr_cur = -1;
     cudaError_t e = cudaGetDevice(&ctx->device);
@@ -95,8 +96,17 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         ctx->label_bits_override = value;
         return VOR_OK;
     }
+    if (!strcmp(name, "label_halo_x100")) {
+        if (value < 0 || value > 1000) return vor_fail(ctx, VOR_EINVAL, "label_halo_x100 must be in [0,1000]");
+        ctx->label_halo_x100 = value;
+        return VOR_OK;
+    }
+    if (!strcmp(name, "label_fast_off")) {
+        ctx->label_fast_off = value != 0;
+        return VOR_OK;
+    }
     if (!strcmp(name, "label_path")) {
-        if (value < 0 || value > 3) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,3]");
+        if (value < 0 || value > 4) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,4]");
         ctx->label_path = value;
         return VOR_OK;
     }

@@ -18,6 +18,12 @@
 //      5. every lane scans the survivors for its TW*TH/32 cells using
 //         d2 = |c|^2 + (|s|^2 - 2 c.s): only t = |s|^2 - 2 cx sx - 2 cy sy is compared, in int32,
 //         coordinates relative to the tile centre (|s| <= 23170 guarantees no overflow).
+//    The common case runs a leaner variant of the same argument (tile_fast): at most 32 gathered
+//    sites (one per lane, kept in registers, sorted by index once), and the bound applied per
+//    QUADRANT of the tile (probe = quadrant centre, r = quadrant radius), which halves the halo and
+//    the candidates per cell; each lane's cells lie in one quadrant, so it scans that quadrant's list.
+//    Anything the lean variant cannot prove (too many sites, halo too small) falls back to the
+//    generic tile code above, and from there to the general path.
 //  * general path: one thread per cell, ring search over cell-list buckets in int64 with the
 //    minimum-image metric.  After scanning all buckets within Chebyshev bucket distance r of the
 //    cell's own bucket every other site has |dx| or |dy| > r*w, so the search stops once
@@ -37,9 +43,17 @@ struct LabelParams {
     const int4* __restrict__ sorted;
     int32_t tiles_x;
     int32_t tiles_y;
-    int32_t halo0;             // initial halo, fixed point
+    int32_t halo0;             // initial halo of the generic tile path, fixed point
     int32_t r_tile;            // ceil(sqrt(hx^2 + hy^2)), fixed point
+    int32_t halo_fast;         // halo of the quadrant fast path, fixed point
+    int32_t r_quad;            // ceil(radius of a quadrant's cell-centre box), fixed point
+    uint32_t div_m, div_s1, div_s2;   // floor(x / w) for 0 <= x < 2^32 (Granlund-Montgomery)
 };
+
+__device__ __forceinline__ int32_t div_w(const LabelParams& p, int32_t x /* >= 0 */) {
+    const uint32_t t = __umulhi(p.div_m, (uint32_t)x);
+    return (int32_t)((t + (((uint32_t)x - t) >> p.div_s1)) >> p.div_s2);
+}
 
 constexpr int kWarpsPerCta = 8;
 constexpr int kCapGather = 160;    // gathered sites per tile
@@ -183,100 +197,431 @@ __device__ __forceinline__ int32_t gather_region(const LabelParams& p, WarpScrat
     return total;
 }
 
-template <int TW, int TH>
-__global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelParams p,
-                                                                       int32_t* __restrict__ labels) {
-    constexpr int HX = FP_HALF * (TW - 1), HY = FP_HALF * (TH - 1);
-    constexpr int GROUPS = 32 / TW;            // lane groups stacked in y
-    constexpr int ROWS = TH / GROUPS;          // rows per lane
-    static_assert(TW * GROUPS == 32 && ROWS * GROUPS == TH, "tile shape");
-    __shared__ WarpScratch scratch[kWarpsPerCta];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    WarpScratch& ws = scratch[wid];
-    const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + wid;
-    if (tile >= (int64_t)p.tiles_x * p.tiles_y) return;
-    const int32_t tx0 = (int32_t)(tile % p.tiles_x) * TW, ty0 = (int32_t)(tile / p.tiles_x) * TH;
-    const int32_t cxm = FP_ONE * tx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HY;
-    const int32_t lx = lane % TW, ly0 = (lane / TW) * ROWS;
+constexpr int kListCap = 16;       // candidates per quadrant list of the fast path
 
-    // ---- 1,2: gather with a halo that provably covers U
+struct FastScratch {
+    int32_t sx[32], sy[32], si[32];          // gathered sites in ascending original index
+    int4 list[4][kListCap];                  // per quadrant: (2*rx, 2*ry, rx^2+ry^2, original index)
+};
+struct WideScratch {
+    int4 list[8][kListCap];                  // per 8x8 quadrant: packed-key candidate entries
+};
+union TileScratch {
+    WarpScratch generic;
+    FastScratch fast;
+    WideScratch wide;
+};
+
+// ceil(sqrt(f)) or slightly more, f >= 0: one MUFU.RSQ; relative error of the product < 2^-21
+__device__ __forceinline__ int32_t isqrt_up(int32_t f) {
+    const float x = fmaxf((float)f, 1.0f);
+    return (int32_t)(x * __frsqrt_rn(x)) + 2;
+}
+
+// Quadrant fast path.  Returns false (nothing written) when it cannot prove exactness cheaply.
+template <int TW, int TH>
+__device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs, int lane,
+                                          int32_t tx0, int32_t ty0, int32_t cxm, int32_t cym,
+                                          int32_t* __restrict__ labels) {
+    constexpr int HX = FP_HALF * (TW - 1), HY = FP_HALF * (TH - 1);
+    constexpr int QW = TW / 2, QH = TH / 2;
+    constexpr int QCX = FP_HALF * QW, QCY = FP_HALF * QH;            // quadrant centre offsets
+    constexpr int QHX = FP_HALF * (QW - 1), QHY = FP_HALF * (QH - 1); // quadrant box half extents
+    constexpr int GROUPS = 32 / TW, ROWS = TH / GROUPS;
+    static_assert(QH % ROWS == 0, "a lane's rows must lie in one quadrant");
+    const unsigned full = 0xffffffffu;
+    const int32_t H = p.halo_fast, P = p.P, half = p.P >> 1;
+
+    // ---- bucket range of the region, relative bounds
+    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
+    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
+    const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
+    if (ncols * p.w > half || nrows * p.w > half) return false;
+    const int32_t RX0 = q0 * p.w - cxm, RX1 = (q1 + 1) * p.w - cxm;     // region [RX0, RX1) rel. to centre
+    const int32_t RY0 = r0 * p.w - cym, RY1 = (r1 + 1) * p.w - cym;
+    if (-RX0 > kMaxRel || RX1 > kMaxRel || -RY0 > kMaxRel || RY1 > kMaxRel) return false;
+    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
+    const bool split = a0 + ncols > p.nb;
+    const int32_t nseg = split ? 2 * nrows : nrows;
+    if (nseg > 32) return false;
+
+    // ---- one lane per segment (contiguous run of buckets in one bucket row)
+    int32_t beg = 0, cnt = 0;
+    if (lane < nseg) {
+        const int32_t row = split ? lane >> 1 : lane;
+        int32_t ay = r0 + row;
+        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
+        int32_t c0, c1;
+        if (!split) { c0 = a0; c1 = a0 + ncols; }
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
+        else { c0 = 0; c1 = a0 + ncols - p.nb; }
+        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
+        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
+    }
+    int32_t inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int32_t t = __shfl_up_sync(full, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const int32_t total = __shfl_sync(full, inc, 31);
+    if (total == 0 || total > 32) return false;
+    const int32_t exc = inc - cnt;
+
+    // ---- one lane per site
+    int32_t seg = 0;
+    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= lane);
+    const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
+    const bool valid = lane < total;
+    int32_t rx = 0, ry = 0, idx = INT32_MAX;
+    if (valid) {
+        const int4 s = __ldg(&p.sorted[sbeg + (lane - sexc)]);
+        rx = s.x - cxm; ry = s.y - cym; idx = s.z;
+        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
+        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+    }
+    // ---- sort by original index: rank = number of sites with a smaller index (indices distinct)
+    int32_t rank = 0;
+    for (int32_t b = 0; b < total; ++b) rank += (__shfl_sync(full, idx, b) < idx);
+    if (valid) { fs.sx[rank] = rx; fs.sy[rank] = ry; fs.si[rank] = idx; }
+    __syncwarp();
+    if (valid) { rx = fs.sx[lane]; ry = fs.sy[lane]; idx = fs.si[lane]; }
+
+    // ---- per-quadrant bound U_q = dist(quadrant centre, nearest site) + quadrant radius
+    const int32_t ax = rx - QCX, bx = rx + QCX, ay_ = ry - QCY, by = ry + QCY;
+    const int32_t ax2 = ax * ax, bx2 = bx * bx, ay2 = ay_ * ay_, by2 = by * by;
+    int32_t d[4] = {bx2 + by2, ax2 + by2, bx2 + ay2, ax2 + ay2};   // q = 2*row + col, centre (-/+QCX, -/+QCY)
+    int32_t U[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int32_t f = __reduce_min_sync(full, valid ? d[q] : INT32_MAX);
+        U[q] = __float2int_ru(sqrtf((float)f)) + 1 + p.r_quad;
+    }
+    // every site within U_q of quadrant q's box must lie inside the gathered region
+    const int32_t mx0 = min(-QCX - QHX - RX0 + 1, RX1 - (-QCX + QHX));
+    const int32_t mx1 = min(QCX - QHX - RX0 + 1, RX1 - (QCX + QHX));
+    const int32_t my0 = min(-QCY - QHY - RY0 + 1, RY1 - (-QCY + QHY));
+    const int32_t my1 = min(QCY - QHY - RY0 + 1, RY1 - (QCY + QHY));
+    if (U[0] >= min(mx0, my0) || U[1] >= min(mx1, my0) || U[2] >= min(mx0, my1) || U[3] >= min(mx1, my1))
+        return false;
+
+    // ---- candidate list of quadrant q: sites within U_q of its box, in ascending index order
+    const int32_t ex0 = max(abs(bx) - QHX, 0), ex1 = max(abs(ax) - QHX, 0);
+    const int32_t ey0 = max(abs(by) - QHY, 0), ey1 = max(abs(ay_) - QHY, 0);
+    const int32_t ex0s = ex0 * ex0, ex1s = ex1 * ex1, ey0s = ey0 * ey0, ey1s = ey1 * ey1;
+    const bool k0 = valid && ex0s + ey0s <= U[0] * U[0], k1 = valid && ex1s + ey0s <= U[1] * U[1];
+    const bool k2 = valid && ex0s + ey1s <= U[2] * U[2], k3 = valid && ex1s + ey1s <= U[3] * U[3];
+    const unsigned K0 = __ballot_sync(full, k0), K1 = __ballot_sync(full, k1);
+    const unsigned K2 = __ballot_sync(full, k2), K3 = __ballot_sync(full, k3);
+    if (__popc(K0) > kListCap || __popc(K1) > kListCap || __popc(K2) > kListCap || __popc(K3) > kListCap)
+        return false;
+    const unsigned lt = (1u << lane) - 1u;
+    const int4 entry = make_int4(2 * rx, 2 * ry, rx * rx + ry * ry, idx);
+    if (k0) fs.list[0][__popc(K0 & lt)] = entry;
+    if (k1) fs.list[1][__popc(K1 & lt)] = entry;
+    if (k2) fs.list[2][__popc(K2 & lt)] = entry;
+    if (k3) fs.list[3][__popc(K3 & lt)] = entry;
+    __syncwarp();
+
+    // ---- each lane scans its quadrant's list for its ROWS cells (column lx)
+    const int32_t lx = lane % TW, ly0 = (lane / TW) * ROWS;
+    const int myq = (ly0 / QH) * 2 + (lx / QW);
+    const unsigned Kq = myq == 0 ? K0 : (myq == 1 ? K1 : (myq == 2 ? K2 : K3));
+    const int32_t n = __popc(Kq);
+    const int4* __restrict__ list = fs.list[myq];
+    const int32_t cxr = FP_ONE * lx - HX, cyr0 = FP_ONE * ly0 - HY;
+    int32_t best[ROWS], bi[ROWS];
+#pragma unroll
+    for (int j = 0; j < ROWS; ++j) { best[j] = INT32_MAX; bi[j] = 0; }
+    for (int32_t k = 0; k < n; ++k) {
+        const int4 c = list[k];
+        const int32_t a = c.z - cxr * c.x;
+#pragma unroll
+        for (int j = 0; j < ROWS; ++j) {
+            const int32_t t = a - (cyr0 + FP_ONE * j) * c.y;
+            if (t < best[j]) { best[j] = t; bi[j] = k; }
+        }
+    }
+    const int32_t x = tx0 + lx;
+    if (x < p.L) {
+        int32_t* __restrict__ out = labels + (int64_t)(ty0 + ly0) * p.L + x;
+#pragma unroll
+        for (int j = 0; j < ROWS; ++j)
+            if (ty0 + ly0 + j < p.L) out[(int64_t)j * p.L] = list[bi[j]].w;
+    }
+    return true;
+}
+
+// Generic tile path (any number of gathered sites up to kCapGather, adaptive halo).
+template <int TW, int TH>
+__device__ __noinline__ bool tile_generic(const LabelParams& p, WarpScratch& ws, int lane,
+                                          int32_t tx0, int32_t ty0, int32_t cxm, int32_t cym,
+                                          int32_t* __restrict__ labels) {
+    constexpr int HX = FP_HALF * (TW - 1), HY = FP_HALF * (TH - 1);
+    constexpr int GROUPS = 32 / TW, ROWS = TH / GROUPS;
+    const int32_t lx = lane % TW, ly0 = (lane / TW) * ROWS;
     int32_t total = -1, margin = 0, dc2 = 0, U = 0;
     int32_t H = p.halo0;
-    bool fast = false;
+    bool ok = false;
     for (int attempt = 0; attempt < 4; ++attempt) {
         total = gather_region<HX, HY>(p, ws, lane, cxm, cym, H, &margin, &dc2);
         if (total < 0) break;
         if (total == 0) { H = 2 * H + p.w; continue; }
         U = __float2int_ru(sqrtf((float)dc2)) + 1 + p.r_tile;
-        if (U < margin) { fast = true; break; }
+        if (U < margin) { ok = true; break; }
         H = U;
     }
-
-    if (fast) {
-        // ---- 3: keep sites within U of the tile's cell-centre box (compaction in place)
-        int32_t m = 0;
-        const int32_t U2 = U * U;
-        for (int32_t base = 0; base < total; base += 32) {
-            const int32_t i = base + lane;
-            int32_t rx = 0, ry = 0, idx = 0;
-            bool keep = false;
-            if (i < total) {
-                rx = ws.g_rx[i]; ry = ws.g_ry[i]; idx = ws.g_idx[i];
-                const int32_t ddx = max(abs(rx) - HX, 0), ddy = max(abs(ry) - HY, 0);
-                keep = ddx * ddx + ddy * ddy <= U2;
-            }
-            const unsigned ball = __ballot_sync(0xffffffffu, keep);
-            __syncwarp();
-            if (keep) {
-                const int32_t pos = m + __popc(ball & ((1u << lane) - 1u));
-                ws.g_rx[pos] = rx; ws.g_ry[pos] = ry; ws.g_idx[pos] = idx;
-            }
-            m += __popc(ball);
-            __syncwarp();
+    if (!ok) return false;
+    // keep sites within U of the tile's cell-centre box (compaction in place)
+    int32_t m = 0;
+    const int32_t U2 = U * U;
+    for (int32_t base = 0; base < total; base += 32) {
+        const int32_t i = base + lane;
+        int32_t rx = 0, ry = 0, idx = 0;
+        bool keep = false;
+        if (i < total) {
+            rx = ws.g_rx[i]; ry = ws.g_ry[i]; idx = ws.g_idx[i];
+            const int32_t ddx = max(abs(rx) - HX, 0), ddy = max(abs(ry) - HY, 0);
+            keep = ddx * ddx + ddy * ddy <= U2;
         }
-        if (m > kCapCand) fast = false;
-        else {
-            // ---- 4: rank by original index (indices are distinct)
-            for (int32_t j = lane; j < m; j += 32) {
-                const int32_t idx = ws.g_idx[j];
-                int32_t rank = 0;
-                for (int32_t k = 0; k < m; ++k) rank += (ws.g_idx[k] < idx);
-                const int32_t rx = ws.g_rx[j], ry = ws.g_ry[j];
-                ws.cand[rank] = make_int4(2 * rx, 2 * ry, rx * rx + ry * ry, idx);
-            }
-            __syncwarp();
-            // ---- 5: every lane scans the candidates for its ROWS cells (column lx)
-            const int32_t cxr = FP_ONE * lx - HX;               // cell centre relative to tile centre
-            int32_t best[ROWS], bi[ROWS];
+        const unsigned ball = __ballot_sync(0xffffffffu, keep);
+        __syncwarp();
+        if (keep) {
+            const int32_t pos = m + __popc(ball & ((1u << lane) - 1u));
+            ws.g_rx[pos] = rx; ws.g_ry[pos] = ry; ws.g_idx[pos] = idx;
+        }
+        m += __popc(ball);
+        __syncwarp();
+    }
+    if (m > kCapCand) return false;
+    // rank by original index (indices are distinct)
+    for (int32_t j = lane; j < m; j += 32) {
+        const int32_t idx = ws.g_idx[j];
+        int32_t rank = 0;
+        for (int32_t k = 0; k < m; ++k) rank += (ws.g_idx[k] < idx);
+        const int32_t rx = ws.g_rx[j], ry = ws.g_ry[j];
+        ws.cand[rank] = make_int4(2 * rx, 2 * ry, rx * rx + ry * ry, idx);
+    }
+    __syncwarp();
+    const int32_t cxr = FP_ONE * lx - HX, cyr0 = FP_ONE * ly0 - HY;
+    int32_t best[ROWS], bi[ROWS];
 #pragma unroll
-            for (int j = 0; j < ROWS; ++j) { best[j] = INT32_MAX; bi[j] = 0; }
-            const int32_t cyr0 = FP_ONE * ly0 - HY;
-            for (int32_t k = 0; k < m; ++k) {
-                const int4 c = ws.cand[k];
-                const int32_t a = c.z - cxr * c.x;
+    for (int j = 0; j < ROWS; ++j) { best[j] = INT32_MAX; bi[j] = 0; }
+    for (int32_t k = 0; k < m; ++k) {
+        const int4 c = ws.cand[k];
+        const int32_t a = c.z - cxr * c.x;
 #pragma unroll
-                for (int j = 0; j < ROWS; ++j) {
-                    const int32_t t = a - (cyr0 + FP_ONE * j) * c.y;
-                    if (t < best[j]) { best[j] = t; bi[j] = k; }
-                }
-            }
-            const int32_t x = tx0 + lx;
-            if (x < p.L) {
-#pragma unroll
-                for (int j = 0; j < ROWS; ++j) {
-                    const int32_t y = ty0 + ly0 + j;
-                    if (y < p.L) labels[(int64_t)y * p.L + x] = ws.cand[bi[j]].w;
-                }
-            }
+        for (int j = 0; j < ROWS; ++j) {
+            const int32_t t = a - (cyr0 + FP_ONE * j) * c.y;
+            if (t < best[j]) { best[j] = t; bi[j] = k; }
         }
     }
-    if (!fast) {
-        const int32_t x = tx0 + lx;
-#pragma unroll 1
+    const int32_t x = tx0 + lx;
+    if (x < p.L) {
+#pragma unroll
         for (int j = 0; j < ROWS; ++j) {
             const int32_t y = ty0 + ly0 + j;
-            if (x < p.L && y < p.L) labels[(int64_t)y * p.L + x] = label_cell_general(p, x, y);
+            if (y < p.L) labels[(int64_t)y * p.L + x] = ws.cand[bi[j]].w;
         }
+    }
+    return true;
+}
+
+// Wide fast path: one warp per 32 x 16 tile = 4 x 2 quadrants of 8 x 8 cells; lane = column.
+// Same exactness argument as tile_fast, per quadrant.  Candidate keys are packed as
+// 16 * (|s|^2 - 2 c.s) + k  (coordinates relative to the quadrant centre, k = position in the
+// index-ordered list), so that one integer min per (cell, candidate) yields both the nearest site
+// and the smallest-index tie-break.  |key| < 2^31 is guaranteed by U_q <= kMaxUWide.
+constexpr int kMaxUWide = 6400;
+
+__device__ __forceinline__ bool tile_wide(const LabelParams& p, WideScratch& wsx, int lane,
+                                          int32_t tx0, int32_t ty0, int32_t* __restrict__ labels) {
+    constexpr int HX = FP_HALF * 31, HY = FP_HALF * 15;
+    constexpr int QC = 4 * FP_ONE;                 // quadrant centres at -3QC/4.. : (2*qx-3)*QC/... see qcx()
+    constexpr int QHW = FP_HALF * 7;               // quadrant box half extent (cell centres)
+    const unsigned full = 0xffffffffu;
+    const int32_t cxm = FP_ONE * tx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HY;
+    const int32_t H = p.halo_fast, P = p.P, half = p.P >> 1;
+
+    // ---- bucket range of the region
+    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
+    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
+    const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
+    if (ncols * p.w > half || nrows * p.w > half) return false;
+    const int32_t RX0 = q0 * p.w - cxm, RX1 = (q1 + 1) * p.w - cxm;
+    const int32_t RY0 = r0 * p.w - cym, RY1 = (r1 + 1) * p.w - cym;
+    if (-RX0 > kMaxRel || RX1 > kMaxRel || -RY0 > kMaxRel || RY1 > kMaxRel) return false;
+    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
+    const bool split = a0 + ncols > p.nb;
+    const int32_t nseg = split ? 2 * nrows : nrows;
+    if (nseg > 32) return false;
+
+    int32_t beg = 0, cnt = 0;
+    if (lane < nseg) {
+        const int32_t row = split ? lane >> 1 : lane;
+        int32_t ay = r0 + row;
+        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
+        int32_t c0, c1;
+        if (!split) { c0 = a0; c1 = a0 + ncols; }
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
+        else { c0 = 0; c1 = a0 + ncols - p.nb; }
+        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
+        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
+    }
+    int32_t inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int32_t t = __shfl_up_sync(full, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const int32_t total = __shfl_sync(full, inc, 31);
+    if (total == 0 || total > 32) return false;
+    const int32_t exc = inc - cnt;
+    int32_t seg = 0;
+    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= lane);
+    const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
+    const bool valid = lane < total;
+    int32_t rx = 0, ry = 0, idx = INT32_MAX;
+    if (valid) {
+        const int4 s = __ldg(&p.sorted[sbeg + (lane - sexc)]);
+        rx = s.x - cxm; ry = s.y - cym; idx = s.z;
+        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
+        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+    }
+    // ---- rank by original index (indices distinct; invalid lanes rank last)
+    int32_t rank = 0;
+    for (int32_t b = 0; b < total; ++b) rank += (__shfl_sync(full, idx, b) < idx);
+    const unsigned rbit = valid ? (1u << rank) : 0u, rlt = (1u << rank) - 1u;
+
+    // ---- per quadrant: offsets from the quadrant centre, bound U_q, exactness check
+    int32_t ox[4], oy[2], ox2[4], oy2[2];
+#pragma unroll
+    for (int qx = 0; qx < 4; ++qx) { ox[qx] = rx - (2 * qx - 3) * QC; ox2[qx] = ox[qx] * ox[qx]; }
+#pragma unroll
+    for (int qy = 0; qy < 2; ++qy) { oy[qy] = ry - (2 * qy - 1) * QC; oy2[qy] = oy[qy] * oy[qy]; }
+    int32_t U[8];
+    bool ok = true;
+#pragma unroll
+    for (int qy = 0; qy < 2; ++qy) {
+        const int32_t my = min((2 * qy - 1) * QC - QHW - RY0 + 1, RY1 - ((2 * qy - 1) * QC + QHW));
+#pragma unroll
+        for (int qx = 0; qx < 4; ++qx) {
+            const int32_t mx = min((2 * qx - 3) * QC - QHW - RX0 + 1, RX1 - ((2 * qx - 3) * QC + QHW));
+            const int32_t f = __reduce_min_sync(full, valid ? ox2[qx] + oy2[qy] : INT32_MAX);
+            const int32_t u = isqrt_up(f) + p.r_quad;
+            U[qy * 4 + qx] = u;
+            ok = ok && u < min(mx, my) && u <= kMaxUWide;
+        }
+    }
+    if (!ok) return false;
+
+    // ---- candidate lists: sites within U_q of the quadrant box, ascending index, packed keys
+    int32_t ex2[4], ey2[2];
+#pragma unroll
+    for (int qx = 0; qx < 4; ++qx) { const int32_t e = max(abs(ox[qx]) - QHW, 0); ex2[qx] = e * e; }
+#pragma unroll
+    for (int qy = 0; qy < 2; ++qy) { const int32_t e = max(abs(oy[qy]) - QHW, 0); ey2[qy] = e * e; }
+    unsigned M[8];
+    bool fits = true;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const int qx = q & 3, qy = q >> 2;
+        const bool keep = valid && ex2[qx] + ey2[qy] <= U[q] * U[q];
+        M[q] = __reduce_or_sync(full, keep ? rbit : 0u);
+        fits = fits && __popc(M[q]) <= kListCap;
+        if (keep) {
+            const int32_t pos = __popc(M[q] & rlt);
+            if (pos < kListCap)
+                wsx.list[q][pos] = make_int4(-32 * ox[qx], -32 * oy[qy], 16 * (ox2[qx] + oy2[qy]) + pos, idx);
+        }
+    }
+    if (!fits) return false;
+    __syncwarp();
+
+    // ---- scan: lane = column; rows 0-7 use quadrant (qx, 0), rows 8-15 quadrant (qx, 1)
+    const int qx = lane >> 3;
+    const int32_t cxr = FP_ONE * (lane & 7) - QHW;
+    const int32_t x = tx0 + lane;
+#pragma unroll
+    for (int qy = 0; qy < 2; ++qy) {
+        const unsigned Mq = qx == 0 ? M[qy * 4] : (qx == 1 ? M[qy * 4 + 1] : (qx == 2 ? M[qy * 4 + 2] : M[qy * 4 + 3]));
+        const int32_t n = __popc(Mq);
+        const int4* __restrict__ list = wsx.list[qy * 4 + qx];
+        int32_t best[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) best[j] = INT32_MAX;
+        for (int32_t k = 0; k < n; ++k) {
+            const int4 c = list[k];
+            const int32_t a = c.z + cxr * c.x;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) best[j] = min(best[j], a + (FP_ONE * j - QHW) * c.y);
+        }
+        if (x < p.L) {
+            int32_t* __restrict__ out = labels + (int64_t)(ty0 + 8 * qy) * p.L + x;
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+                if (ty0 + 8 * qy + j < p.L) out[(int64_t)j * p.L] = list[best[j] & (kListCap - 1)].w;
+        }
+    }
+    return true;
+}
+
+// fallback of the wide kernel: the two 16 x 16 halves through the narrower paths
+__device__ __noinline__ void tile_wide_fallback(const LabelParams& p, TileScratch& ts, int lane,
+                                                int32_t tx0, int32_t ty0, int32_t* __restrict__ labels) {
+    constexpr int HX = FP_HALF * 15;
+    for (int h = 0; h < 2; ++h) {
+        const int32_t hx0 = tx0 + 16 * h;
+        if (hx0 >= p.L) break;
+        const int32_t cxm = FP_ONE * hx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HX;
+        __syncwarp();
+        if (tile_fast<16, 16>(p, ts.fast, lane, hx0, ty0, cxm, cym, labels)) continue;
+        __syncwarp();
+        if (tile_generic<16, 16>(p, ts.generic, lane, hx0, ty0, cxm, cym, labels)) continue;
+        const int32_t x = hx0 + (lane & 15), yb = ty0 + (lane >> 4) * 8;
+        for (int j = 0; j < 8; ++j)
+            if (x < p.L && yb + j < p.L) labels[(int64_t)(yb + j) * p.L + x] = label_cell_general(p, x, yb + j);
+    }
+}
+
+__global__ void __launch_bounds__(kWarpsPerCta * 32) label_wide_kernel(const __grid_constant__ LabelParams p,
+                                                                       int32_t* __restrict__ labels) {
+    __shared__ TileScratch scratch[kWarpsPerCta];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + wid;
+    if (tile >= (int64_t)p.tiles_x * p.tiles_y) return;
+    const int32_t tiy = (int32_t)(tile / p.tiles_x);
+    const int32_t tx0 = (int32_t)(tile - (int64_t)tiy * p.tiles_x) * 32, ty0 = tiy * 16;
+    if (tile_wide(p, scratch[wid].wide, lane, tx0, ty0, labels)) return;
+    tile_wide_fallback(p, scratch[wid], lane, tx0, ty0, labels);
+}
+
+
+template <int TW, int TH>
+__global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelParams p,
+                                                                       int32_t* __restrict__ labels,
+                                                                       int use_fast) {
+    constexpr int HX = FP_HALF * (TW - 1), HY = FP_HALF * (TH - 1);
+    constexpr int GROUPS = 32 / TW;            // lane groups stacked in y
+    constexpr int ROWS = TH / GROUPS;          // rows per lane
+    static_assert(TW * GROUPS == 32 && ROWS * GROUPS == TH, "tile shape");
+    __shared__ TileScratch scratch[kWarpsPerCta];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + wid;
+    if (tile >= (int64_t)p.tiles_x * p.tiles_y) return;
+    const int32_t tiy = (int32_t)(tile / p.tiles_x);
+    const int32_t tx0 = (int32_t)(tile - (int64_t)tiy * p.tiles_x) * TW, ty0 = tiy * TH;
+    const int32_t cxm = FP_ONE * tx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HY;
+
+    if (use_fast && tile_fast<TW, TH>(p, scratch[wid].fast, lane, tx0, ty0, cxm, cym, labels)) return;
+    __syncwarp();
+    if (tile_generic<TW, TH>(p, scratch[wid].generic, lane, tx0, ty0, cxm, cym, labels)) return;
+    const int32_t lx = lane % TW, ly0 = (lane / TW) * ROWS;
+    const int32_t x = tx0 + lx;
+#pragma unroll 1
+    for (int j = 0; j < ROWS; ++j) {
+        const int32_t y = ty0 + ly0 + j;
+        if (x < p.L && y < p.L) labels[(int64_t)y * p.L + x] = label_cell_general(p, x, y);
     }
 }
 
@@ -291,10 +636,10 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     p.L = ctx->L; p.P = (int32_t)ctx->P; p.nb = ctx->nb; p.w = ctx->w; p.n = ctx->n_sites;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
     const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_sites);   // cells
-    int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8
-    if (path == 0) path = spacing >= 10.0 ? 2 : (spacing >= 4.0 ? 3 : 1);
+    int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8, 4 wide 32x16
+    if (path == 0) path = spacing >= 10.0 ? 4 : (spacing >= 4.0 ? 3 : 1);
     if (ctx->L < 16) path = 1;
-    const int tw = path == 2 ? 16 : 8;
+    const int tw = (path == 2 || path == 4) ? 16 : 8;
     if (path == 1) {
         const int64_t bw = (ctx->L + 15) / 16;
         const int64_t blocks = bw * bw;
@@ -306,11 +651,31 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     const double hx = 128.0 * (tw - 1);
     p.r_tile = (int32_t)ceil(sqrt(2.0 * hx * hx));
     p.halo0 = p.r_tile + (int32_t)(0.75 * spacing * FP_ONE);
+    const double qh = 128.0 * (tw / 2 - 1);
+    p.r_quad = (int32_t)ceil(sqrt(2.0 * qh * qh));
+    p.halo_fast = p.r_quad + (int32_t)(0.01 * (double)ctx->label_halo_x100 * spacing * FP_ONE);
+    {   // magic numbers for floor(x / w), x < 2^32
+        const uint32_t d = (uint32_t)ctx->w;
+        uint32_t l = 0;
+        while (((uint64_t)1 << l) < d) ++l;
+        p.div_m = (uint32_t)((((uint64_t)1 << 32) * (((uint64_t)1 << l) - d)) / d + 1);
+        p.div_s1 = l < 1 ? l : 1;
+        p.div_s2 = l > 0 ? l - 1 : 0;
+    }
+    const int use_fast = ctx->label_fast_off ? 0 : 1;
+    if (path == 4) {
+        p.tiles_x = (ctx->L + 31) / 32;
+        p.tiles_y = (ctx->L + 15) / 16;
+        const int64_t wtiles = (int64_t)p.tiles_x * p.tiles_y;
+        VOR_LAUNCH(label_wide_kernel, (unsigned)((wtiles + kWarpsPerCta - 1) / kWarpsPerCta),
+                   kWarpsPerCta * 32, 0, stream, p, d_labels);
+        return VOR_OK;
+    }
     const int64_t tiles = (int64_t)p.tiles_x * p.tiles_y;
     const unsigned grid = (unsigned)((tiles + kWarpsPerCta - 1) / kWarpsPerCta);
     if (path == 2)
-        VOR_LAUNCH((label_tile_kernel<16, 16>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels);
+        VOR_LAUNCH((label_tile_kernel<16, 16>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels, use_fast);
     else
-        VOR_LAUNCH((label_tile_kernel<8, 8>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels);
+        VOR_LAUNCH((label_tile_kernel<8, 8>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels, use_fast);
     return VOR_OK;
 }

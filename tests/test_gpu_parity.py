@@ -30,16 +30,18 @@ def rnd(seed, L, n):
 
 
 # ------------------------------------------------------------------ labels (a1 + a2)
-def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3), ref=None, occ=None):
+def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3, 4), ref=None, occ=None):
     ref = oracle.label_brute(L, sx, sy) if ref is None else ref
     v = make(L, max(len(sx), 1))
     if occ:
         v.vor_set_option("bucket_occupancy_x100", occ)
     for path in paths:
-        v.vor_set_option("label_path", path)
-        got = G.gpu_labels(v, sx, sy)
-        bad = np.argwhere(got != ref)
-        assert len(bad) == 0, f"path {path}: {len(bad)} cells differ, first {bad[:5].tolist()}"
+        for fast_off in ((0, 1) if path in (0, 2, 3) else (0,)):
+            v.vor_set_option("label_path", path)
+            v.vor_set_option("label_fast_off", fast_off)
+            got = G.gpu_labels(v, sx, sy)
+            bad = np.argwhere(got != ref)
+            assert len(bad) == 0, f"path {path} fast_off {fast_off}: {len(bad)} cells differ, first {bad[:5].tolist()}"
     v.close()
 
 
@@ -102,6 +104,20 @@ def test_labels_bucket_size_independent(G, occ):
     w = W.scaled(5, 512)
     sx, sy = next(iter(w.frames(1)))
     check_labels(G, 512, sx, sy, occ=occ)
+
+
+@pytest.mark.parametrize("halo", [0, 30, 60, 150, 400])
+def test_labels_halo_independent(G, halo):
+    """The fast path's halo is a performance knob: too small a halo must fall back, never mislabel."""
+    w = W.scaled(5, 512)
+    sx, sy = list(w.frames(4))[3]
+    ref = oracle.label_cells(512, sx, sy, 16)
+    v = make(512, len(sx))
+    v.vor_set_option("label_halo_x100", halo)
+    for path in (2, 3, 4):
+        v.vor_set_option("label_path", path)
+        assert np.array_equal(G.gpu_labels(v, sx, sy), ref)
+    v.close()
 
 
 def test_labels_hex_and_rhombus_constructions(G):
