@@ -106,7 +106,7 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         return VOR_OK;
     }
     if (!strcmp(name, "label_path")) {
-        if (value < 0 || value > 4) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,4]");
+        if (value < 0 || value > 5) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,5]");
         ctx->label_path = value;
         return VOR_OK;
     }

@@ -215,7 +215,9 @@ union TileScratch {
 // ceil(sqrt(f)) or slightly more, f >= 0: one MUFU.RSQ; relative error of the product < 2^-21
 __device__ __forceinline__ int32_t isqrt_up(int32_t f) {
     const float x = fmaxf((float)f, 1.0f);
-    return (int32_t)(x * __frsqrt_rn(x)) + 2;
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return (int32_t)(x * r) + 2;
 }
 
 // Quadrant fast path.  Returns false (nothing written) when it cannot prove exactness cheaply.
@@ -597,6 +599,227 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_wide_kernel(const __g
 }
 
 
+// ---------------------------------------------------------------- CTA three-phase path (default)
+// The per-quadrant candidate lists are inherently small, scalar work (a few dozen distance tests per
+// 8 x 8 quadrant), so they are built by a few threads per quadrant instead of one warp per tile.
+// A CTA of 128 threads covers 64 x 32 cells = 8 x 4 quadrants:
+//   phase G  the sites of the cell-list buckets covering the CTA's cells plus the halo are gathered
+//            into shared memory (coalesced row segments, coordinates relative to the CTA centre);
+//            every warp computes the segment prefix, warp w loads items [32w, 32w+32);
+//   phase A  4 lanes per quadrant build its candidate list from the shared site list:
+//            U_q = dist(quadrant centre, nearest gathered site) + quadrant radius; the gathered region
+//            must reach U_q beyond the quadrant box on every side; candidates = gathered sites within
+//            U_q of the box, ordered by original index;
+//   phase B  every warp scans its 32 x 16 cells (lane = column) against its quadrants' lists with
+//            packed keys 16 * (|o|^2 - 2 c.o) + position: one integer min per (cell, candidate)
+//            gives the nearest site and the smallest-index tie-break; full 128-byte row stores.
+// A quadrant whose bound cannot be proven this way is marked and its cells take the general search.
+constexpr int kCtaQX = 8, kCtaQY = 4;                 // quadrants per CTA
+constexpr int kCtaQ = kCtaQX * kCtaQY;
+constexpr int kCtaThreads = 128;
+constexpr int kCtaCapSites = 128;                     // = kCtaThreads: one gathered site per thread
+constexpr int kCtaMaxExtent = 23000;                  // |relative site coordinate| bound
+constexpr int kCtaMaxU = 20000;                       // |o| <= 896 + U <= 20896: t = |o|^2 - 2 c.o fits int32
+constexpr int kUnpackedFlag = 1 << 16;
+
+struct CtaShared {
+    int32_t sx[kCtaCapSites], sy[kCtaCapSites], si[kCtaCapSites];
+    int4 list[kListCap][kCtaQ];                       // [k][quadrant]: conflict-free across quadrants
+    int4 tmp[kListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
+    int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
+};
+
+// Returns the number of gathered sites (0 = region unusable).  Region bounds relative to the CTA
+// centre are returned through R[4] = {RX0, RX1, RY0, RY1}.
+__device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& sh, int lane, int wid,
+                                              int32_t cxm, int32_t cym, int32_t H, int32_t* R) {
+    constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
+    const unsigned full = 0xffffffffu;
+    const int32_t P = p.P, half = p.P >> 1;
+    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
+    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
+    const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
+    if (ncols * p.w > half || nrows * p.w > half) return 0;
+    R[0] = q0 * p.w - cxm; R[1] = (q1 + 1) * p.w - cxm;
+    R[2] = r0 * p.w - cym; R[3] = (r1 + 1) * p.w - cym;
+    if (-R[0] > kCtaMaxExtent || R[1] > kCtaMaxExtent || -R[2] > kCtaMaxExtent || R[3] > kCtaMaxExtent) return 0;
+    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
+    const bool split = a0 + ncols > p.nb;
+    const int32_t nseg = split ? 2 * nrows : nrows;
+    if (nseg > 32) return 0;
+    int32_t beg = 0, cnt = 0;
+    if (lane < nseg) {
+        const int32_t row = split ? lane >> 1 : lane;
+        int32_t ay = r0 + row;
+        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
+        int32_t c0, c1;
+        if (!split) { c0 = a0; c1 = a0 + ncols; }
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
+        else { c0 = 0; c1 = a0 + ncols - p.nb; }
+        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
+        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
+    }
+    int32_t inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int32_t t = __shfl_up_sync(full, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const int32_t total = __shfl_sync(full, inc, 31);
+    if (total > kCtaCapSites) return 0;
+    const int32_t exc = inc - cnt;
+    const int32_t i = 32 * wid + lane;                 // this thread's item
+    int32_t seg = 0;
+    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= i);
+    const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
+    if (i < total) {
+        const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
+        int32_t rx = s.x - cxm, ry = s.y - cym;
+        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
+        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+        sh.sx[i] = rx; sh.sy[i] = ry; sh.si[i] = s.z;
+    }
+    return total;
+}
+
+// 4 consecutive lanes (sub = 0..3) build the list of quadrant q; qcx, qcy: its centre relative to the
+// CTA centre.  Lane sub == 0 publishes sh.count[q] = length | flags, or -1.
+__device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& sh, int q, int sub,
+                                               int32_t ns, const int32_t* R, int32_t qcx, int32_t qcy,
+                                               bool active) {
+    constexpr int QHW = FP_HALF * 7;
+    const unsigned full = 0xffffffffu;
+    if (!active) ns = 0;
+    int32_t f = INT32_MAX;
+    for (int32_t i = sub; i < ns; i += 4) {
+        const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
+        f = min(f, ox * ox + oy * oy);
+    }
+    f = min(f, __shfl_xor_sync(full, f, 1));
+    f = min(f, __shfl_xor_sync(full, f, 2));
+    const int32_t U = isqrt_up(f) + p.r_quad;
+    int32_t margin = min(qcx - QHW - R[0] + 1, R[1] - (qcx + QHW));
+    margin = min(margin, min(qcy - QHW - R[2] + 1, R[3] - (qcy + QHW)));
+    const bool ok = ns > 0 && U < margin && U <= kCtaMaxU;
+    const int32_t U2 = U * U;
+    if (ok) {
+        for (int32_t i = sub; i < ns; i += 4) {
+            const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
+            const int32_t ex = min(max(abs(ox) - QHW, 0), U + 1), ey = min(max(abs(oy) - QHW, 0), U + 1);
+            if (ex * ex + ey * ey <= U2) {
+                const int32_t slot = atomicAdd(&sh.count[q], 1);
+                if (slot < kListCap) sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, ox * ox + oy * oy, sh.si[i]);
+            }
+        }
+    }
+    __syncwarp();
+    const int32_t n = sh.count[q];
+    __syncwarp();
+    if (ok && n <= kListCap) {
+        // order by original index: rank = number of survivors with a smaller index (indices distinct)
+        for (int32_t k = sub; k < n; k += 4) {
+            const int4 e = sh.tmp[k][q];
+            int32_t r = 0;
+            for (int32_t j = 0; j < n; ++j) r += (sh.tmp[j][q].w < e.w);
+            sh.list[r][q] = e;
+        }
+    }
+    if (sub == 0 && active)
+        sh.count[q] = (ok && n <= kListCap) ? (U <= kMaxUWide ? n : n | kUnpackedFlag) : -1;
+}
+
+__global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_constant__ LabelParams p,
+                                                                int32_t* __restrict__ labels) {
+    constexpr int QHW = FP_HALF * 7;
+    constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
+    __shared__ CtaShared sh;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t X0 = blockIdx.x * (8 * kCtaQX), Y0 = blockIdx.y * (8 * kCtaQY);
+    // ---- phases G + A; quadrants whose bound could not be proven get one retry with a wider halo
+    if (threadIdx.x < kCtaQ) sh.count[threadIdx.x] = 0;
+    {
+        const int q = threadIdx.x >> 2, sub = threadIdx.x & 3;
+        const int qx = q % kCtaQX, qy = q / kCtaQX;
+        bool active = true;
+        for (int attempt = 0; attempt < 2; ++attempt) {
+            int32_t R[4] = {0, 0, 0, 0};
+            const int32_t H = attempt == 0 ? p.halo_fast : 2 * p.halo_fast + p.w;
+            const int32_t ns = cta_gather(p, sh, lane, wid, FP_ONE * X0 + FP_HALF + HX,
+                                          FP_ONE * Y0 + FP_HALF + HY, H, R);
+            __syncthreads();
+            cta_build_list(p, sh, q, sub, ns, R, 8 * FP_ONE * qx + QHW - HX, 8 * FP_ONE * qy + QHW - HY, active);
+            __syncthreads();
+            active = sh.count[q] < 0;
+            if (!__syncthreads_or(active)) break;
+            if (attempt == 0 && active && sub == 0) sh.count[q] = 0;     // reset the survivor counter
+            __syncthreads();
+        }
+    }
+    // ---- phase B: warp = 32 x 16 cells, lane = column
+    const int wx = wid & 1, wy = wid >> 1;
+    const int32_t x = X0 + 32 * wx + lane;
+    const int qx = 4 * wx + (lane >> 3);
+    const int32_t cxr = FP_ONE * (lane & 7) - QHW;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int q = (2 * wy + h) * kCtaQX + qx;
+        const int32_t y0 = Y0 + 16 * wy + 8 * h;
+        if (x >= p.L || y0 >= p.L) continue;
+        const int32_t cnt = sh.count[q];
+        int32_t* __restrict__ out = labels + (int64_t)y0 * p.L + x;
+        if (cnt < 0) {
+            for (int j = 0; j < 8; ++j)
+                if (y0 + j < p.L) out[(int64_t)j * p.L] = label_cell_general(p, x, y0 + j);
+            continue;
+        }
+        const int32_t n = cnt & (kUnpackedFlag - 1);
+        int32_t sel[8];                                  // position of the winning candidate
+        if (!(cnt & kUnpackedFlag)) {
+            int32_t best[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) best[j] = INT32_MAX;
+            int32_t k = 0;
+            for (; k + 2 <= n; k += 2) {                 // two candidates per step: 3-input min
+                const int4 c0 = sh.list[k][q], c1 = sh.list[k + 1][q];
+                const int32_t a0 = 16 * (c0.z + cxr * c0.x) + k, y0s = 16 * c0.y;
+                const int32_t a1 = 16 * (c1.z + cxr * c1.x) + k + 1, y1s = 16 * c1.y;
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    best[j] = min(best[j], min(a0 + (FP_ONE * j - QHW) * y0s, a1 + (FP_ONE * j - QHW) * y1s));
+            }
+            if (k < n) {
+                const int4 c0 = sh.list[k][q];
+                const int32_t a0 = 16 * (c0.z + cxr * c0.x) + k, y0s = 16 * c0.y;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) best[j] = min(best[j], a0 + (FP_ONE * j - QHW) * y0s);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sel[j] = best[j] & (kListCap - 1);
+        } else {
+            // far sites (large U): same scan with an explicit (value, position) pair
+            int32_t best[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { best[j] = INT32_MAX; sel[j] = 0; }
+            for (int32_t k = 0; k < n; ++k) {
+                const int4 c = sh.list[k][q];
+                const int32_t a = c.z + cxr * c.x;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int32_t t = a + (FP_ONE * j - QHW) * c.y;
+                    if (t < best[j]) { best[j] = t; sel[j] = k; }
+                }
+            }
+        }
+        if (y0 + 8 <= p.L) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { *out = sh.list[sel[j]][q].w; out += p.L; }
+        } else {
+            for (int j = 0; j < 8; ++j)
+                if (y0 + j < p.L) out[(int64_t)j * p.L] = sh.list[sel[j]][q].w;
+        }
+    }
+}
+
 template <int TW, int TH>
 __global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelParams p,
                                                                        int32_t* __restrict__ labels,
@@ -636,10 +859,10 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     p.L = ctx->L; p.P = (int32_t)ctx->P; p.nb = ctx->nb; p.w = ctx->w; p.n = ctx->n_sites;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
     const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_sites);   // cells
-    int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8, 4 wide 32x16
-    if (path == 0) path = spacing >= 10.0 ? 4 : (spacing >= 4.0 ? 3 : 1);
+    int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8, 4 wide 32x16, 5 CTA
+    if (path == 0) path = spacing >= 7.0 ? 5 : (spacing >= 4.0 ? 3 : 1);
     if (ctx->L < 16) path = 1;
-    const int tw = (path == 2 || path == 4) ? 16 : 8;
+    const int tw = (path == 2 || path >= 4) ? 16 : 8;
     if (path == 1) {
         const int64_t bw = (ctx->L + 15) / 16;
         const int64_t blocks = bw * bw;
@@ -663,6 +886,11 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
         p.div_s2 = l > 0 ? l - 1 : 0;
     }
     const int use_fast = ctx->label_fast_off ? 0 : 1;
+    if (path == 5) {
+        dim3 grid((ctx->L + 8 * kCtaQX - 1) / (8 * kCtaQX), (ctx->L + 8 * kCtaQY - 1) / (8 * kCtaQY));
+        VOR_LAUNCH(label_cta_kernel, grid, kCtaThreads, 0, stream, p, d_labels);
+        return VOR_OK;
+    }
     if (path == 4) {
         p.tiles_x = (ctx->L + 31) / 32;
         p.tiles_y = (ctx->L + 15) / 16;

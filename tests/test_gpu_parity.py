@@ -30,7 +30,7 @@ def rnd(seed, L, n):
 
 
 # ------------------------------------------------------------------ labels (a1 + a2)
-def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3, 4), ref=None, occ=None):
+def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3, 4, 5), ref=None, occ=None):
     ref = oracle.label_brute(L, sx, sy) if ref is None else ref
     v = make(L, max(len(sx), 1))
     if occ:
@@ -114,7 +114,7 @@ def test_labels_halo_independent(G, halo):
     ref = oracle.label_cells(512, sx, sy, 16)
     v = make(512, len(sx))
     v.vor_set_option("label_halo_x100", halo)
-    for path in (2, 3, 4):
+    for path in (2, 3, 4, 5):
         v.vor_set_option("label_path", path)
         assert np.array_equal(G.gpu_labels(v, sx, sy), ref)
     v.close()
