@@ -60,7 +60,11 @@ int vor_sync_status(vor_ctx* ctx, void* stream);
 int64_t vor_launch_count(const vor_ctx* ctx);
 
 /* Tuning knobs (integers).  Unknown names -> VOR_EINVAL.
- *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 25) */
+ *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 25)
+ *   "row_slots"              adjacency-matrix slots used per site in vor_edges: 4, 8, 12 or 16
+ *                            (default 16); pairs that do not fit take the sorted overflow path,
+ *                            so the result never depends on it
+ *   "label_path", "label_halo_x100", "label_fast_off", "label_bits"   kernel selection for tests */
 int vor_set_option(vor_ctx* ctx, const char* name, int64_t value);
 
 /* ---- a1: counting-sort cell list of the sites (not in the paper, which loops over all centres,

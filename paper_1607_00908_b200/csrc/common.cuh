@@ -12,9 +12,11 @@
 #define FP_ONE 256
 #define FP_HALF 128
 
-constexpr int kNumSMs = 148;               // B200: 2 dies x 74 SMs
-constexpr int kSortBlocks = kNumSMs;       // persistent one-CTA-per-SM kernels (sort, unique, diff)
-constexpr int kSortThreads = 1024;
+constexpr int kNumSMs = 148;               // B200: 2 dies x 74 SMs (grid sizing of the streaming kernels)
+constexpr int kSortThreads = 1024;         // block size of the persistent cooperative kernels
+constexpr int kMaxCoopBlocks = 1024;       // allocation bound for per-block scratch of those kernels
+constexpr int kRowStride = 16;             // adjacency-row slots per site (64-byte rows)
+constexpr uint32_t kEmptySlot = 0xffffffffu;
 
 // error flag bits latched on the device (ctx->d_flags[0])
 enum : int {
@@ -50,12 +52,15 @@ struct vor_ctx {
     int32_t* d_scan_part;      // scratch for device scans
 
     // ---- edges (a3/a4)
-    uint64_t* d_keys_a;        // [max_raw_keys]  raw keys / sort ping
+    uint32_t* d_rows;          // [max_sites * kRowStride] per-site sets of larger-index neighbours;
+                               //   all kEmptySlot between calls (the finish kernel restores that)
+    int64_t row_slots;         // slots used per row (option; 4..kRowStride, multiple of 4)
+    uint64_t* d_keys_a;        // [max_raw_keys]  overflow keys / sort ping
     uint64_t* d_keys_b;        // [max_raw_keys]  sort pong
-    int64_t* d_n_raw;          // device scalar: number of raw keys
-    uint32_t* d_hist;          // [kSortBlocks * 256] per-block digit histograms
-    int64_t* d_blk_count;      // [2 * kSortBlocks] per-block counts for compactions
-    uint8_t* d_mark;           // [max_raw_keys] flags for compactions
+    int64_t* d_n_raw;          // device control block [8]: 0 = raw/overflow key count, 1 = filtered
+                               //   overflow count, 2 = OR of the overflow keys
+    uint32_t* d_hist;          // [kMaxCoopBlocks * 256] per-block digit histograms
+    int64_t* d_blk_count;      // [2 * kMaxCoopBlocks] per-block counts for compactions
 
     // ---- diff with maps: translated / filtered lists
     uint64_t* d_tr_prev;       // lazily sized to max_raw_keys
@@ -88,6 +93,8 @@ struct vor_ctx {
     int fr_have_prev;
 
     int32_t* d_flags;          // [1] sticky error bits
+    int num_sms;               // of the device the context lives on
+    int coop_blocks[4];        // cached grid sizes of the cooperative kernels (0 = not yet queried)
     int64_t launches;
     char err[512];
 };
@@ -108,6 +115,29 @@ inline int vor_cuda_fail(vor_ctx* ctx, cudaError_t e, const char* where) {
         if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #call);            \
     } while (0)
 
+// Grid size for a cooperative (grid-synchronising) kernel: every block must be co-resident.
+inline int vor_coop_grid(vor_ctx* ctx, int slot, const void* func, int threads, int max_per_sm) {
+    if (ctx->coop_blocks[slot] == 0) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, func, threads, 0) != cudaSuccess || per_sm < 1)
+            per_sm = 1;
+        if (per_sm > max_per_sm) per_sm = max_per_sm;
+        int g = per_sm * ctx->num_sms;
+        if (g > kMaxCoopBlocks) g = kMaxCoopBlocks;
+        ctx->coop_blocks[slot] = g;
+    }
+    return ctx->coop_blocks[slot];
+}
+
+#define VOR_LAUNCH_COOP(kernel, grid, block, stream, ...)                                         \
+    do {                                                                                           \
+        void* args_[] = {__VA_ARGS__};                                                             \
+        cudaError_t e_ = cudaLaunchCooperativeKernel((const void*)kernel, dim3(grid), dim3(block), \
+                                                     args_, 0, (stream));                          \
+        ctx->launches++;                                                                           \
+        if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #kernel);                             \
+    } while (0)
+
 // launch + count + check
 #define VOR_LAUNCH(kernel, grid, block, smem, stream, ...)                      \
     do {                                                                        \
@@ -121,4 +151,5 @@ inline int vor_cuda_fail(vor_ctx* ctx, cudaError_t e, const char* where) {
 int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n_in, int key_bits,
                          uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
                          cudaStream_t stream);
+int vor_reset_rows(vor_ctx* ctx);
 int vor_label_bits(const vor_ctx* ctx);

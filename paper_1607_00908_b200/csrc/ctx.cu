@@ -32,10 +32,18 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     ctx->max_raw_keys = max_raw_keys;
     ctx->bucket_occ_x100 = 25;
     ctx->label_halo_x100 = 90;
+    ctx->row_slots = kRowStride;
     if (const char* e = getenv("VOR_BUCKET_OCC_X100")) ctx->bucket_occ_x100 = atoll(e);
     ctx->fr_cur = -1;
     cudaError_t e = cudaGetDevice(&ctx->device);
     if (e != cudaSuccess) { free(ctx); return VOR_ECUDA; }
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess ||
+        ctx->num_sms < 1 || !coop) {
+        free(ctx);
+        return VOR_ECUDA;
+    }
 
     ctx->nb_max = L / 2 < 1 ? 1 : (L / 2 > 4096 ? 4096 : L / 2);
     const size_t nbuckets = (size_t)ctx->nb_max * ctx->nb_max;
@@ -46,14 +54,15 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     ok = ok && dmalloc(&ctx->d_scan_part, 8192) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_keys_a, (size_t)max_raw_keys) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_keys_b, (size_t)max_raw_keys) == cudaSuccess;
-    ok = ok && dmalloc(&ctx->d_mark, (size_t)max_raw_keys) == cudaSuccess;
-    ok = ok && dmalloc(&ctx->d_n_raw, 4) == cudaSuccess;
-    ok = ok && dmalloc(&ctx->d_hist, (size_t)kSortBlocks * 256) == cudaSuccess;
-    ok = ok && dmalloc(&ctx->d_blk_count, (size_t)4 * kSortBlocks) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_rows, (size_t)max_sites * kRowStride) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_n_raw, 8) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_hist, (size_t)kMaxCoopBlocks * 256) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_blk_count, (size_t)2 * kMaxCoopBlocks) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_tr_counts, 4) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_comp_count, 4) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_flags, 4) == cudaSuccess;
     if (ok) ok = cudaMemset(ctx->d_flags, 0, 4 * sizeof(int32_t)) == cudaSuccess;
+    if (ok) ok = vor_reset_rows(ctx) == VOR_OK;
     if (!ok) {
         vor_destroy(ctx);
         return VOR_ECUDA;
@@ -66,7 +75,7 @@ int vor_destroy(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
     cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
     cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
-    cudaFree(ctx->d_mark); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
+    cudaFree(ctx->d_rows); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
     cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts);
     cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
     cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best);
@@ -101,6 +110,12 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         ctx->label_halo_x100 = value;
         return VOR_OK;
     }
+    if (!strcmp(name, "row_slots")) {
+        if (value < 4 || value > kRowStride || value % 4)
+            return vor_fail(ctx, VOR_EINVAL, "row_slots must be 4, 8, 12 or 16");
+        ctx->row_slots = value;
+        return VOR_OK;
+    }
     if (!strcmp(name, "label_fast_off")) {
         ctx->label_fast_off = value != 0;
         return VOR_OK;
@@ -132,6 +147,12 @@ int vor_sync_status(vor_ctx* ctx, void* stream) {
 }
 
 }  // extern "C"
+
+// All adjacency rows empty (the invariant vor_edges relies on between calls).
+int vor_reset_rows(vor_ctx* ctx) {
+    VOR_CUDA(cudaMemset(ctx->d_rows, 0xff, (size_t)ctx->max_sites * kRowStride * sizeof(uint32_t)));
+    return VOR_OK;
+}
 
 // Number of significant bits of a label value (site index) for the radix sort.
 int vor_label_bits(const vor_ctx* ctx) {

@@ -4,29 +4,38 @@
 // and classify the couples connected in only one triangulation as "breaking" (in
 // D_P only) or "arising" (in D_N only).  Here both sets are ascending unique key
 // lists, so breaking = prev \ now (destroyed) and arising = now \ prev (created) are sorted set
-// differences: each key is binary-searched in the other list (both lists are L2-resident), then an
-// order-preserving compaction writes the survivors.
+// differences.  ONE cooperative kernel: half of the blocks take each direction; a block owns a
+// contiguous chunk of its list A, finds for every 1024-key batch the matching window of the other
+// list B (batch boundaries are binary-searched once, in parallel), stages the window in shared
+// memory and searches there; membership bits stay in shared memory across the grid sync that
+// separates counting from the order-preserving write.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
 constexpr int kDiffThreads = kSortThreads;
+constexpr int kDiffWindow = 3072;          // keys of B staged per batch
+constexpr int kDiffMaxBatches = 128;       // batches per block whose membership bits are cached
 
-__device__ __forceinline__ bool contains(const uint64_t* __restrict__ a, int64_t n, uint64_t key) {
-    int64_t lo = 0, hi = n;
+struct DiffShared {
+    uint64_t win[kDiffWindow];
+    uint32_t bits[kDiffMaxBatches][kDiffThreads / 32];
+    int64_t bstart[kDiffMaxBatches + 1];
+    int64_t red[32];
+    int32_t wtot[kDiffThreads / 32];
+};
+
+__device__ __forceinline__ int64_t lower_bound(const uint64_t* __restrict__ a, int64_t lo, int64_t hi,
+                                               uint64_t key) {
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
         if (a[mid] < key) lo = mid + 1; else hi = mid;
     }
-    return lo < n && a[lo] == key;
-}
-
-__device__ __forceinline__ void chunk_of(int64_t n, int nblocks, int b, int64_t* beg, int64_t* end) {
-    int64_t C = (n + nblocks - 1) / nblocks;
-    C = (C + kDiffThreads - 1) / kDiffThreads * kDiffThreads;
-    int64_t s = (int64_t)b * C;
-    *beg = s < n ? s : n;
-    *end = s + C < n ? s + C : n;
+    return lo;
 }
 
 __device__ __forceinline__ int64_t block_sum(int64_t v, int64_t* sh) {
@@ -42,79 +51,139 @@ __device__ __forceinline__ int64_t block_sum(int64_t v, int64_t* sh) {
     return t;
 }
 
-// grid = 2 * nb blocks: blocks [0, nb) handle created = now \ prev, [nb, 2nb) destroyed = prev \ now
-__global__ void __launch_bounds__(kDiffThreads) diff_count_kernel(
-        const uint64_t* __restrict__ prev, const int64_t* __restrict__ n_prev_p,
-        const uint64_t* __restrict__ now, const int64_t* __restrict__ n_now_p,
-        int64_t* __restrict__ blk_count) {
-    __shared__ int64_t sh[32];
-    const int nb = gridDim.x >> 1;
-    const bool second = (int)blockIdx.x >= nb;
-    const uint64_t* A = second ? prev : now;        // elements of A not in B
-    const uint64_t* B = second ? now : prev;
-    const int64_t nA = second ? *n_prev_p : *n_now_p, nB = second ? *n_now_p : *n_prev_p;
-    int64_t beg, end;
-    chunk_of(nA, nb, second ? blockIdx.x - nb : blockIdx.x, &beg, &end);
-    int64_t c = 0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kDiffThreads) c += !contains(B, nB, A[i]);
-    c = block_sum(c, sh);
-    if (threadIdx.x == 0) blk_count[blockIdx.x] = c;
+// bstart[k] = lower_bound(B, first key of batch k) for the batches [g0, g0 + nb) of this block's
+// chunk; bstart[nb] closes the last window.
+__device__ __forceinline__ void batch_windows(const uint64_t* __restrict__ A, int64_t beg, int64_t nA,
+                                              const uint64_t* __restrict__ B, int64_t nB, int64_t g0,
+                                              int nb, DiffShared& sh) {
+    for (int k = threadIdx.x; k <= nb; k += kDiffThreads) {
+        const int64_t i = beg + (g0 + k) * kDiffThreads;
+        // the window of batch k must hold every B key <= the batch's last key: close it with the
+        // first key of the next batch (keys are unique, so B keys equal to batch keys lie before it)
+        sh.bstart[k] = i < nA ? lower_bound(B, 0, nB, A[i]) : nB;
+    }
+    __syncthreads();
 }
 
-__global__ void __launch_bounds__(kDiffThreads) diff_write_kernel(
-        const uint64_t* __restrict__ prev, const int64_t* __restrict__ n_prev_p,
-        const uint64_t* __restrict__ now, const int64_t* __restrict__ n_now_p,
-        const int64_t* __restrict__ blk_count, uint64_t* __restrict__ created,
-        uint64_t* __restrict__ destroyed, int64_t cap, int64_t* __restrict__ n_created,
-        int64_t* __restrict__ n_destroyed, int32_t* __restrict__ flags) {
-    __shared__ int64_t sh[32];
-    __shared__ int32_t wtot[kDiffThreads / 32];
+// Is A[i] absent from B?  One batch of kDiffThreads keys; B window [w0, w1).
+__device__ __forceinline__ bool batch_absent(const uint64_t* __restrict__ A, int64_t i, int64_t end,
+                                             const uint64_t* __restrict__ B, int64_t w0, int64_t w1,
+                                             DiffShared& sh, uint64_t* key_out) {
+    const int64_t wn = w1 - w0;
+    const bool staged = wn <= kDiffWindow;
+    if (staged)
+        for (int64_t k = threadIdx.x; k < wn; k += kDiffThreads) sh.win[k] = B[w0 + k];
+    __syncthreads();
+    bool absent = false;
+    if (i < end) {
+        const uint64_t key = A[i];
+        *key_out = key;
+        if (staged) {
+            int lo = 0, hi = (int)wn;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (sh.win[mid] < key) lo = mid + 1; else hi = mid;
+            }
+            absent = !(lo < (int)wn && sh.win[lo] == key);
+        } else {
+            const int64_t lo = lower_bound(B, w0, w1, key);
+            absent = !(lo < w1 && B[lo] == key);
+        }
+    }
+    __syncthreads();
+    return absent;
+}
+
+struct DiffParams {
+    const uint64_t* prev; const int64_t* n_prev;
+    const uint64_t* now;  const int64_t* n_now;
+    uint64_t* created; uint64_t* destroyed; int64_t cap;
+    int64_t* n_created; int64_t* n_destroyed;
+    int64_t* partial;          // [gridDim]
+    int32_t* flags;
+};
+
+// grid = 2 * nb blocks: blocks [0, nb) handle created = now \ prev, [nb, 2nb) destroyed = prev \ now
+__global__ void __launch_bounds__(kDiffThreads) diff_kernel(const DiffParams p) {
+    __shared__ DiffShared sh;
+    cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int nb = gridDim.x >> 1;
     const bool second = (int)blockIdx.x >= nb;
     const int me = second ? blockIdx.x - nb : blockIdx.x;
-    const uint64_t* A = second ? prev : now;
-    const uint64_t* B = second ? now : prev;
-    const int64_t nA = second ? *n_prev_p : *n_now_p, nB = second ? *n_now_p : *n_prev_p;
-    uint64_t* out = second ? destroyed : created;
-    int64_t beg, end;
-    chunk_of(nA, nb, me, &beg, &end);
+    const uint64_t* __restrict__ A = second ? p.prev : p.now;        // elements of A not in B
+    const uint64_t* __restrict__ B = second ? p.now : p.prev;
+    const int64_t nA = second ? *p.n_prev : *p.n_now, nB = second ? *p.n_now : *p.n_prev;
+    uint64_t* __restrict__ out = second ? p.destroyed : p.created;
+    int64_t C = (nA + nb - 1) / nb;
+    C = (C + kDiffThreads - 1) / kDiffThreads * kDiffThreads;
+    const int64_t beg = (int64_t)me * C < nA ? (int64_t)me * C : nA;
+    const int64_t end = beg + C < nA ? beg + C : nA;
+    const int64_t nbatch = (end - beg + kDiffThreads - 1) / kDiffThreads;
+    const bool cached = nbatch <= kDiffMaxBatches;
+
+    // ---- pass 1: membership + count
+    int64_t c = 0;
+    for (int64_t g0 = 0; g0 < nbatch; g0 += kDiffMaxBatches) {
+        const int gb = (int)(nbatch - g0 < kDiffMaxBatches ? nbatch - g0 : kDiffMaxBatches);
+        batch_windows(A, beg, nA, B, nB, g0, gb, sh);
+        for (int k = 0; k < gb; ++k) {
+            uint64_t key;
+            const bool absent = batch_absent(A, beg + (g0 + k) * kDiffThreads + threadIdx.x, end, B,
+                                             sh.bstart[k], sh.bstart[k + 1], sh, &key);
+            const unsigned ball = __ballot_sync(0xffffffffu, absent);
+            if (cached && lane == 0) sh.bits[k][wid] = ball;
+            c += absent;
+        }
+        __syncthreads();
+    }
+    c = block_sum(c, sh.red);
+    if (threadIdx.x == 0) p.partial[blockIdx.x] = c;
+    grid.sync();
+
+    // ---- pass 2: order-preserving write
     int64_t before = 0, all = 0;
     for (int b = threadIdx.x; b < nb; b += kDiffThreads) {
-        const int64_t v = blk_count[(second ? nb : 0) + b];
+        const int64_t v = __ldcg(p.partial + (second ? nb : 0) + b);
         all += v;
         if (b < me) before += v;
     }
-    before = block_sum(before, sh);
-    all = block_sum(all, sh);
+    before = block_sum(before, sh.red);
+    all = block_sum(all, sh.red);
     if (me == 0 && threadIdx.x == 0) {
-        *(second ? n_destroyed : n_created) = all;
-        if (all > cap) atomicOr(flags, FLAG_DIFF_CAP);
+        *(second ? p.n_destroyed : p.n_created) = all;
+        if (all > p.cap) atomicOr(p.flags, FLAG_DIFF_CAP);
     }
     int64_t run = before;
-    for (int64_t sub = beg; sub < end; sub += kDiffThreads) {
-        const int64_t i = sub + threadIdx.x;
-        uint64_t k = 0;
-        bool keep = false;
-        if (i < end) {
-            k = A[i];
-            keep = !contains(B, nB, k);
+    for (int64_t g0 = 0; g0 < nbatch; g0 += kDiffMaxBatches) {
+        const int gb = (int)(nbatch - g0 < kDiffMaxBatches ? nbatch - g0 : kDiffMaxBatches);
+        if (!cached) batch_windows(A, beg, nA, B, nB, g0, gb, sh);
+        for (int k = 0; k < gb; ++k) {
+            const int64_t i = beg + (g0 + k) * kDiffThreads + threadIdx.x;
+            uint64_t key = 0;
+            unsigned ball;
+            if (cached) {
+                ball = sh.bits[k][wid];
+                if (ball >> lane & 1) key = A[i];
+            } else {
+                const bool absent = batch_absent(A, i, end, B, sh.bstart[k], sh.bstart[k + 1], sh, &key);
+                ball = __ballot_sync(0xffffffffu, absent);
+            }
+            if (lane == 0) sh.wtot[wid] = __popc(ball);
+            __syncthreads();
+            int32_t wbase = 0, total = 0;
+            for (int w = 0; w < kDiffThreads / 32; ++w) {
+                const int32_t t = sh.wtot[w];
+                if (w < wid) wbase += t;
+                total += t;
+            }
+            if (ball >> lane & 1) {
+                const int64_t pos = run + wbase + __popc(ball & ((1u << lane) - 1u));
+                if (pos < p.cap) out[pos] = key;
+            }
+            run += total;
+            __syncthreads();
         }
-        const unsigned ball = __ballot_sync(0xffffffffu, keep);
-        if (lane == 0) wtot[wid] = __popc(ball);
-        __syncthreads();
-        int32_t wbase = 0, total = 0;
-        for (int w = 0; w < kDiffThreads / 32; ++w) {
-            const int32_t t = wtot[w];
-            if (w < wid) wbase += t;
-            total += t;
-        }
-        if (keep) {
-            const int64_t pos = run + wbase + __popc(ball & ((1u << lane) - 1u));
-            if (pos < cap) out[pos] = k;
-        }
-        run += total;
-        __syncthreads();
     }
 }
 
@@ -205,9 +274,11 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
         P = ctx->d_tr_prev; nP = &ctx->d_tr_counts[0];
         N = ctx->d_tr_now;  nN = &ctx->d_tr_counts[1];
     }
-    VOR_LAUNCH(diff_count_kernel, 2 * kSortBlocks, kDiffThreads, 0, stream, P, nP, N, nN,
-               ctx->d_blk_count);
-    VOR_LAUNCH(diff_write_kernel, 2 * kSortBlocks, kDiffThreads, 0, stream, P, nP, N, nN,
-               ctx->d_blk_count, d_created, d_destroyed, cap, d_n_created, d_n_destroyed, ctx->d_flags);
+    DiffParams dp{P, nP, N, nN, d_created, d_destroyed, cap, d_n_created, d_n_destroyed,
+                  ctx->d_blk_count, ctx->d_flags};
+    int grid = vor_coop_grid(ctx, 2, (const void*)diff_kernel, kDiffThreads, 1);
+    grid &= ~1;                                         // one half per direction
+    if (grid < 2) return vor_fail(ctx, VOR_ECUDA, "vor_diff: device too small for the cooperative grid");
+    VOR_LAUNCH_COOP(diff_kernel, grid, kDiffThreads, stream, (void*)&dp);
     return VOR_OK;
 }

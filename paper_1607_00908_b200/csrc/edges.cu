@@ -1,237 +1,319 @@
 // a3 + a4 — site-adjacency (digital Delaunay) edge set.
-// Paper: the Delaunay graph as an adjacency matrix (§III.B) filled from the coloured
-// lattice and "compressed" by sort + unique.  This build's rule
-// (R6, BASELINE.json): every 4-connected label discontinuity (right, down, periodic wrap)
-// contributes the pair (min,max), packed as (min << 32 | max); the result is the ascending unique list.
+// Paper: the Delaunay graph as an adjacency matrix with one row per label, pre-filled with a
+// sentinel (§III.B), filled from the coloured lattice and
+// "compressed" by sort + unique per row.  This build's rule (R6,
+// BASELINE.json): every 4-connected label discontinuity (right, down, periodic wrap) contributes the
+// pair (min,max), packed as (min << 32 | max); the result is the ascending unique list.
 //
-//   emit:   stream the label image once (128-bit loads), compare right/down, de-duplicate keys in a
-//           per-CTA shared-memory hash set, append the CTA's distinct keys to a global buffer with
-//           one atomic per CTA.  ~40 raw discontinuities per site collapse to ~4 keys per site.
-//   sort:   LSD radix sort, 8 bits per pass, only the 2*ceil(log2 N) significant bits; persistent
-//           one-CTA-per-SM kernels, each CTA owns a contiguous chunk (stable by construction).
-//   unique: head flags + order-preserving compaction (count kernel, write kernel).
+//   emit    stream the label image once (128-bit loads); every warp compacts the discontinuities of
+//           a row into a shared-memory queue and inserts them 32 at a time into a per-CTA hash set;
+//           at the end the CTA's distinct pairs (a < b) are inserted into row a of a global
+//           adjacency matrix (kRowStride slots per site, exact set insertion with atomicCAS).
+//           Pairs that do not fit (row full, or label >= number of rows) go to an overflow list.
+//   finish  ONE cooperative kernel: [only if the overflow list is not empty: radix-sort it, drop
+//           duplicates and keys already present in their row] -> per-row counts -> grid sync ->
+//           every row is sorted in registers and written at its final position (merged with its
+//           overflow keys, if any); rows are reset to empty on the way.
+// The matrix rows are in ascending site order and each row is sorted, so the concatenation IS the
+// globally sorted list: no global sort on the common path.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr uint64_t kEmpty = ~0ull;
+constexpr uint64_t kEmptyKey = ~0ull;
+
+struct RowSet {
+    uint32_t* rows;            // [n_rows * kRowStride]
+    int32_t n_rows;
+    int32_t S;                 // slots used per row
+    uint64_t* ovf;             // overflow keys (unordered, may repeat)
+    int64_t ovf_cap;
+    unsigned long long* n_ovf;
+    int32_t* flags;
+};
+
+__device__ __forceinline__ void ovf_push(const RowSet& rs, uint32_t a, uint32_t b) {
+    const unsigned long long pos = atomicAdd(rs.n_ovf, 1ull);
+    if ((int64_t)pos < rs.ovf_cap) rs.ovf[pos] = ((uint64_t)a << 32) | b;
+    else atomicOr(rs.flags, FLAG_RAWKEY_OVERFLOW);
+}
+
+// Insert b into the set stored in row a (a < b).  Slots fill front to back and never change once
+// set, so a value can never end up in two slots.
+__device__ __noinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b) {
+    if (a < (uint32_t)rs.n_rows) {
+        uint32_t* row = rs.rows + (size_t)a * kRowStride;
+        for (int q = 0; q < rs.S; q += 4) {
+            const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
+            const uint32_t e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                uint32_t cur = e[k];
+                if (cur == b) return;
+                if (cur == kEmptySlot) {
+                    cur = atomicCAS(row + q + k, kEmptySlot, b);
+                    if (cur == kEmptySlot || cur == b) return;
+                }
+            }
+        }
+    }
+    ovf_push(rs, a, b);
+}
 
 // ------------------------------------------------------------------------------------ emit
 constexpr int kEmitThreads = 256;
+constexpr int kEmitWarps = kEmitThreads / 32;
 constexpr int kEmitCols = 128;          // per CTA tile: 32 lanes x 4 labels
-constexpr int kEmitRowsPerWarp = 8;
-constexpr int kEmitRows = (kEmitThreads / 32) * kEmitRowsPerWarp;   // 64
-constexpr int kHashSlots = 1024;
-constexpr int kMaxProbe = 48;
+constexpr int kEmitRowsPerWarp = 16;
+constexpr int kEmitRows = kEmitWarps * kEmitRowsPerWarp;   // 128
+constexpr int kHashSlots = 2048;
+constexpr int kMaxProbe = 32;
+constexpr int kQueueCap = 32 + 256;     // < 32 pending + at most 8 pairs per lane per row
 
 __device__ __forceinline__ uint32_t hash_key(uint32_t a, uint32_t b) {
     uint32_t h = a * 0x9E3779B1u ^ (b * 0x85EBCA77u);
-    h ^= h >> 15;
-    return h;
+    return h ^ (h >> 15);
 }
 
-struct EmitShared {
-    unsigned long long table[kHashSlots];
-    int32_t scan[kEmitThreads / 32];
-    long long base;
-};
-
-__device__ __forceinline__ void emit_pair(int32_t a, int32_t b, EmitShared& sh,
-                                          uint64_t* __restrict__ keys, int64_t cap,
-                                          unsigned long long* __restrict__ n_raw, int32_t* flags) {
-    const uint32_t lo = (uint32_t)min(a, b), hi = (uint32_t)max(a, b);
+__device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned long long* table,
+                                            const RowSet& rs) {
+    const uint32_t lo = min(a, b), hi = max(a, b);
     const unsigned long long key = ((unsigned long long)lo << 32) | hi;
     uint32_t h = hash_key(lo, hi) & (kHashSlots - 1);
     for (int probe = 0; probe < kMaxProbe; ++probe) {
-        const unsigned long long cur = sh.table[h];
+        const unsigned long long cur = table[h];
         if (cur == key) return;
-        if (cur == kEmpty) {
-            const unsigned long long old = atomicCAS(&sh.table[h], kEmpty, key);
-            if (old == kEmpty || old == key) return;
+        if (cur == kEmptyKey) {
+            const unsigned long long old = atomicCAS(&table[h], kEmptyKey, key);
+            if (old == kEmptyKey || old == key) return;
         }
         h = (h + 1) & (kHashSlots - 1);
     }
-    // table crowded (very dense sites): emit straight to global, duplicates are removed later
-    const unsigned long long pos = atomicAdd(n_raw, 1ull);
-    if ((int64_t)pos < cap) keys[pos] = key;
-    else atomicOr(flags, FLAG_RAWKEY_OVERFLOW);
+    row_insert(rs, lo, hi);    // table crowded (very dense sites): straight to the matrix
 }
 
 template <bool VEC>
-__global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(
-        const int32_t* __restrict__ labels, int32_t L, uint64_t* __restrict__ keys, int64_t cap,
-        unsigned long long* __restrict__ n_raw, int32_t* __restrict__ flags) {
-    __shared__ EmitShared sh;
-    for (int i = threadIdx.x; i < kHashSlots; i += kEmitThreads) sh.table[i] = kEmpty;
+__global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t* __restrict__ labels,
+                                                                  int32_t L, const RowSet rs) {
+    __shared__ unsigned long long table[kHashSlots];
+    __shared__ uint2 queue[kEmitWarps][kQueueCap];
+    for (int i = threadIdx.x; i < kHashSlots; i += kEmitThreads) table[i] = kEmptyKey;
     __syncthreads();
+    const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int32_t x0 = blockIdx.x * kEmitCols + lane * 4;
     const int32_t ybeg = blockIdx.y * kEmitRows + wid * kEmitRowsPerWarp;
-    const bool active = x0 < L;                    // VEC: L % 4 == 0, so 4 columns are all in or out
+    uint2* __restrict__ q = queue[wid];
+    int qn = 0;                                    // warp-uniform queue fill
     if (ybeg < L) {
-        int32_t c[4], nx[4];
-        auto load_row = [&](int32_t y, int32_t* v) {
-            if (!active) { v[0] = v[1] = v[2] = v[3] = 0; return; }
-            const int32_t* row = labels + (int64_t)y * L;
+        auto load_row = [&](const int32_t* __restrict__ row, int32_t* v) {
             if (VEC) {
-                const int4 t = __ldg(reinterpret_cast<const int4*>(row + x0));
-                v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+                if (x0 < L) {
+                    const int4 t = __ldcs(reinterpret_cast<const int4*>(row + x0));
+                    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+                } else {
+                    v[0] = v[1] = v[2] = v[3] = 0;
+                }
             } else {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) v[k] = x0 + k < L ? __ldg(row + x0 + k) : -1;
+                for (int k = 0; k < 4; ++k) v[k] = x0 + k < L ? __ldg(row + x0 + k) : 0;
             }
         };
-        load_row(ybeg, c);
+        int32_t c[4], nx[4];
+        load_row(labels + (int64_t)ybeg * L, c);
         const int32_t yend = min(ybeg + kEmitRowsPerWarp, L);
         for (int32_t y = ybeg; y < yend; ++y) {
-            const int32_t yn = y + 1 == L ? 0 : y + 1;
-            load_row(yn, nx);
-            // right neighbour of my 4th column: next lane's first column, or a wrapped load
-            int32_t r = __shfl_down_sync(0xffffffffu, c[0], 1);
-            if (active) {
-                const int32_t xr = x0 + 4;
-                if (lane == 31 || xr >= L) r = __ldg(labels + (int64_t)y * L + (xr >= L ? xr - L : xr));
-                if (VEC) {
-                    if (c[0] != c[1]) emit_pair(c[0], c[1], sh, keys, cap, n_raw, flags);
-                    if (c[1] != c[2]) emit_pair(c[1], c[2], sh, keys, cap, n_raw, flags);
-                    if (c[2] != c[3]) emit_pair(c[2], c[3], sh, keys, cap, n_raw, flags);
-                    if (c[3] != r) emit_pair(c[3], r, sh, keys, cap, n_raw, flags);
+            const int32_t* __restrict__ row = labels + (int64_t)y * L;
+            load_row(labels + (int64_t)(y + 1 == L ? 0 : y + 1) * L, nx);
+            // right neighbours: next column, next lane's first column, or column 0 through the wrap
+            int32_t rr[4] = {c[1], c[2], c[3], __shfl_down_sync(full, c[0], 1)};
+            if (lane == 31 && x0 + 4 < L) rr[3] = __ldg(row + x0 + 4);
+            if (x0 + 4 >= L && x0 < L) {
+                const int32_t first = __ldg(row);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (c[k] != nx[k]) emit_pair(c[k], nx[k], sh, keys, cap, n_raw, flags);
-                } else {
-                    // ragged row end: column k's right neighbour is k+1, or column 0 through the wrap
+                for (int k = 0; k < 4; ++k)
+                    if (x0 + k + 1 >= L) rr[k] = first;
+            }
+            unsigned bits = 0;
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        if (x0 + k >= L) break;
-                        int32_t rk;
-                        if (x0 + k + 1 >= L) rk = __ldg(labels + (int64_t)y * L);
-                        else rk = k < 3 ? c[k + 1] : r;
-                        if (c[k] != rk) emit_pair(c[k], rk, sh, keys, cap, n_raw, flags);
-                        if (c[k] != nx[k]) emit_pair(c[k], nx[k], sh, keys, cap, n_raw, flags);
-                    }
+            for (int k = 0; k < 4; ++k) {
+                const bool valid = VEC ? (x0 < L) : (x0 + k < L);
+                bits |= (unsigned)(valid && c[k] != rr[k]) << k;
+                bits |= (unsigned)(valid && c[k] != nx[k]) << (4 + k);
+            }
+            const int cnt = __popc(bits);
+            int inc = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(full, inc, o);
+                if (lane >= o) inc += t;
+            }
+            const int total = __shfl_sync(full, inc, 31);
+            if (total) {
+                int pos = qn + inc - cnt;
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (bits & (1u << k)) q[pos++] = make_uint2((uint32_t)c[k], (uint32_t)rr[k]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (bits & (16u << k)) q[pos++] = make_uint2((uint32_t)c[k], (uint32_t)nx[k]);
+                qn += total;
+                __syncwarp();
+                while (qn >= 32) {
+                    qn -= 32;
+                    const uint2 it = q[qn + lane];
+                    hash_insert(it.x, it.y, table, rs);
                 }
+                __syncwarp();
             }
 #pragma unroll
             for (int k = 0; k < 4; ++k) c[k] = nx[k];
         }
+        if (lane < qn) {
+            const uint2 it = q[lane];
+            hash_insert(it.x, it.y, table, rs);
+        }
     }
     __syncthreads();
-    // compact the hash set: 4 slots per thread
-    unsigned long long mine[kHashSlots / kEmitThreads];
-    int32_t cnt = 0;
+    // the CTA's distinct pairs go to the adjacency matrix
 #pragma unroll
     for (int k = 0; k < kHashSlots / kEmitThreads; ++k) {
-        mine[k] = sh.table[threadIdx.x * (kHashSlots / kEmitThreads) + k];
-        cnt += mine[k] != kEmpty;
+        const unsigned long long key = table[k * kEmitThreads + threadIdx.x];
+        if (key != kEmptyKey) row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
     }
-    int32_t inc = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) sh.scan[wid] = inc;
-    __syncthreads();
-    int32_t wbase = 0, total = 0;
-#pragma unroll
-    for (int k = 0; k < kEmitThreads / 32; ++k) {
-        if (k < wid) wbase += sh.scan[k];
-        total += sh.scan[k];
-    }
-    if (threadIdx.x == 0) sh.base = total ? (long long)atomicAdd(n_raw, (unsigned long long)total) : 0;
-    __syncthreads();
-    if (total == 0) return;
-    const int64_t base = sh.base;
-    if (base + total > cap) {
-        if (threadIdx.x == 0) atomicOr(flags, FLAG_RAWKEY_OVERFLOW);
-        return;
-    }
-    int64_t pos = base + wbase + inc - cnt;
-#pragma unroll
-    for (int k = 0; k < kHashSlots / kEmitThreads; ++k)
-        if (mine[k] != kEmpty) keys[pos++] = mine[k];
 }
 
-// ------------------------------------------------------------------------------------ radix sort
+// ------------------------------------------------------------------------------------ block helpers
+constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kKeysPerThread = 4;
 constexpr int kSubTile = kSortThreads * kKeysPerThread;       // 4096 keys
-constexpr int kSortWarps = kSortThreads / 32;
 
-struct DigitSpec {
-    int label_bits;    // significant bits of each 32-bit half
-    int shift;         // 8 * pass
+struct CoopShared {
+    uint32_t cnt[kSortWarps][256];     // radix: per-warp digit counts, then per-warp bases
+    uint32_t running[256];
+    uint32_t wsum[8];
+    int64_t red[32];
+    int32_t wtot[kSortWarps];
 };
 
-__device__ __forceinline__ uint32_t digit_of(uint64_t key, DigitSpec ds) {
-    const uint64_t compact = ((key >> 32) << ds.label_bits) | (key & 0xffffffffull);
-    return (uint32_t)(compact >> ds.shift) & 255u;
-}
-
-// chunk of block b: [b*C, min((b+1)*C, n)), C = ceil(n / gridDim) rounded up to the sub-tile size
-__device__ __forceinline__ void block_chunk(int64_t n, int64_t* beg, int64_t* end) {
+// chunk of block b: [b*C, min((b+1)*C, n)), C = ceil(n / gridDim) rounded up to a multiple of `unit`
+__device__ __forceinline__ void block_chunk(int64_t n, int64_t unit, int64_t* beg, int64_t* end) {
     int64_t C = (n + gridDim.x - 1) / gridDim.x;
-    C = (C + kSubTile - 1) / kSubTile * kSubTile;
-    int64_t b = (int64_t)blockIdx.x * C;
+    C = (C + unit - 1) / unit * unit;
+    const int64_t b = (int64_t)blockIdx.x * C;
     *beg = b < n ? b : n;
     *end = b + C < n ? b + C : n;
 }
 
-__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(
-        const uint64_t* __restrict__ in, const int64_t* __restrict__ n_ptr, int64_t n_cap,
-        DigitSpec ds, uint32_t* __restrict__ hist) {
-    __shared__ uint32_t h[256];
-    if (threadIdx.x < 256) h[threadIdx.x] = 0;
+// sum over the block, returned to every thread (two barriers)
+__device__ __forceinline__ int64_t block_sum_i64(int64_t v, int64_t* sh /* [32] */) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) sh[wid] = v;
     __syncthreads();
-    const int64_t n = min(*n_ptr, n_cap);
-    int64_t beg, end;
-    block_chunk(n, &beg, &end);
-    for (int64_t i = beg + threadIdx.x; i < end; i += kSortThreads) atomicAdd(&h[digit_of(in[i], ds)], 1u);
+    int64_t t = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
     __syncthreads();
-    if (threadIdx.x < 256) hist[blockIdx.x * 256 + threadIdx.x] = h[threadIdx.x];
+    return t;
 }
 
-__global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(
-        const uint64_t* __restrict__ in, uint64_t* __restrict__ out, const int64_t* __restrict__ n_ptr,
-        int64_t n_cap, DigitSpec ds, const uint32_t* __restrict__ hist) {
-    __shared__ uint32_t cnt[kSortWarps][256];      // per-warp digit counts, then per-warp bases
-    __shared__ uint32_t running[256];
-    __shared__ uint32_t wsum[8];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t n = min(*n_ptr, n_cap);
-    int64_t beg, end;
-    block_chunk(n, &beg, &end);
-    if (beg >= end) return;
+// (sum of partial[b] for b < me, sum of all) over `count` per-block values
+__device__ __forceinline__ void partial_prefix(const int64_t* __restrict__ partial, int count, int me,
+                                               int64_t* sh, int64_t* before, int64_t* all) {
+    int64_t bf = 0, al = 0;
+    for (int b = threadIdx.x; b < count; b += blockDim.x) {
+        const int64_t v = __ldcg(partial + b);
+        al += v;
+        if (b < me) bf += v;
+    }
+    *before = block_sum_i64(bf, sh);
+    *all = block_sum_i64(al, sh);
+}
 
+// Order-preserving compaction step for one batch of blockDim.x items: returns this thread's output
+// position (valid if keep) and advances *run by the batch total.
+__device__ __forceinline__ int64_t compact_pos(bool keep, int64_t* run, int32_t* wtot) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned ball = __ballot_sync(0xffffffffu, keep);
+    if (lane == 0) wtot[wid] = __popc(ball);
+    __syncthreads();
+    int32_t wbase = 0, total = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+        const int32_t t = wtot[w];
+        if (w < wid) wbase += t;
+        total += t;
+    }
+    const int64_t pos = *run + wbase + __popc(ball & ((1u << lane) - 1u));
+    *run += total;
+    __syncthreads();
+    return pos;
+}
+
+// ------------------------------------------------------------------------------------ radix sort
+struct DigitSpec {
+    int label_bits;    // significant bits of each 32-bit half (32 = sort the key as it is)
+    int shift;         // 8 * pass
+};
+
+__device__ __forceinline__ uint64_t compact_key(uint64_t key, int label_bits) {
+    return ((key >> 32) << label_bits) | (key & 0xffffffffull);
+}
+__device__ __forceinline__ uint32_t digit_of(uint64_t key, DigitSpec ds) {
+    return (uint32_t)(compact_key(key, ds.label_bits) >> ds.shift) & 255u;
+}
+
+__device__ void radix_hist(const uint64_t* __restrict__ in, int64_t n, DigitSpec ds,
+                           uint32_t* __restrict__ hist, CoopShared& sh) {
+    if (threadIdx.x < 256) sh.running[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t beg, end;
+    block_chunk(n, kSubTile, &beg, &end);
+    for (int64_t i = beg + threadIdx.x; i < end; i += kSortThreads)
+        atomicAdd(&sh.running[digit_of(in[i], ds)], 1u);
+    __syncthreads();
+    if (threadIdx.x < 256) hist[blockIdx.x * 256 + threadIdx.x] = sh.running[threadIdx.x];
+    __syncthreads();
+}
+
+// stable: every block owns a contiguous chunk, processed front to back
+__device__ void radix_scatter(const uint64_t* __restrict__ in, uint64_t* __restrict__ out, int64_t n,
+                              DigitSpec ds, const uint32_t* __restrict__ hist, CoopShared& sh) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int64_t beg, end;
+    block_chunk(n, kSubTile, &beg, &end);
     // global base of (digit d, this block) = sum over digits < d of all blocks + blocks < me of d
     if (threadIdx.x < 256) {
         const int d = threadIdx.x;
         uint32_t total = 0, before = 0;
         for (int b = 0; b < (int)gridDim.x; ++b) {
-            const uint32_t v = hist[b * 256 + d];
+            const uint32_t v = __ldcg(hist + b * 256 + d);
             total += v;
             if (b < (int)blockIdx.x) before += v;
         }
-        // exclusive scan of `total` over the 256 digits (8 warps)
         uint32_t inc = total;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
             if (lane >= o) inc += t;
         }
-        if (lane == 31) wsum[wid] = inc;
-        running[d] = inc - total + before;          // completed below with the warp offsets
+        if (lane == 31) sh.wsum[wid] = inc;
+        sh.running[d] = inc - total + before;          // completed below with the warp offsets
     }
     __syncthreads();
     if (threadIdx.x < 256) {
         uint32_t off = 0;
-        for (int k = 0; k < wid; ++k) off += wsum[k];
-        running[threadIdx.x] += off;
+        for (int k = 0; k < wid; ++k) off += sh.wsum[k];
+        sh.running[threadIdx.x] += off;
     }
     __syncthreads();
-
     for (int64_t sub = beg; sub < end; sub += kSubTile) {
-        for (int i = threadIdx.x; i < kSortWarps * 256; i += kSortThreads) (&cnt[0][0])[i] = 0;
+        for (int i = threadIdx.x; i < kSortWarps * 256; i += kSortThreads) (&sh.cnt[0][0])[i] = 0;
         __syncthreads();
         uint64_t key[kKeysPerThread];
         uint32_t dg[kKeysPerThread], rk[kKeysPerThread];
@@ -246,8 +328,8 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(
             const int leader = __ffs(peers) - 1;
             uint32_t old = 0;
             if (valid && lane == leader) {
-                old = cnt[wid][dg[it]];
-                cnt[wid][dg[it]] = old + __popc(peers);
+                old = sh.cnt[wid][dg[it]];
+                sh.cnt[wid][dg[it]] = old + __popc(peers);
             }
             old = __shfl_sync(0xffffffffu, old, leader);
             rk[it] = old + __popc(peers & ((1u << lane) - 1u));
@@ -256,73 +338,59 @@ __global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(
         __syncthreads();
         if (threadIdx.x < 256) {
             const int d = threadIdx.x;
-            uint32_t run = running[d];
+            uint32_t run = sh.running[d];
 #pragma unroll 4
             for (int w = 0; w < kSortWarps; ++w) {
-                const uint32_t t = cnt[w][d];
-                cnt[w][d] = run;
+                const uint32_t t = sh.cnt[w][d];
+                sh.cnt[w][d] = run;
                 run += t;
             }
-            running[d] = run;
+            sh.running[d] = run;
         }
         __syncthreads();
 #pragma unroll
         for (int it = 0; it < kKeysPerThread; ++it)
-            if (dg[it] < 256u) out[cnt[wid][dg[it]] + rk[it]] = key[it];
+            if (dg[it] < 256u) out[sh.cnt[wid][dg[it]] + rk[it]] = key[it];
         __syncthreads();
     }
 }
 
-// ------------------------------------------------------------------------------------ unique
-__device__ __forceinline__ int64_t block_sum_i64(int64_t v, int64_t* sh /* [32] */) {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) sh[wid] = v;
-    __syncthreads();
-    int64_t t = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    __syncthreads();
-    return t;
+// LSD radix sort of a[0..n) with b as the pong buffer; passes whose digit is 0 in every key
+// (per `mask`, an OR of the compacted keys or any superset) are skipped.  Returns the sorted buffer.
+__device__ uint64_t* coop_sort(cg::grid_group& grid, uint64_t* a, uint64_t* b, int64_t n,
+                               int label_bits, uint64_t mask, uint32_t* hist, CoopShared& sh) {
+    uint64_t* src = a;
+    uint64_t* dst = b;
+    for (int pass = 0; pass < 8; ++pass) {
+        if (((mask >> (8 * pass)) & 255ull) == 0) continue;
+        const DigitSpec ds{label_bits, 8 * pass};
+        radix_hist(src, n, ds, hist, sh);
+        grid.sync();
+        radix_scatter(src, dst, n, ds, hist, sh);
+        grid.sync();
+        uint64_t* t = src; src = dst; dst = t;
+    }
+    return src;
 }
 
-__global__ void __launch_bounds__(kSortThreads) unique_count_kernel(
-        const uint64_t* __restrict__ keys, const int64_t* __restrict__ n_ptr, int64_t n_cap,
-        int64_t* __restrict__ blk_count) {
-    __shared__ int64_t sh[32];
-    const int64_t n = min(*n_ptr, n_cap);
+// Ascending unique keys of the sorted list `keys` that satisfy `keep`, written to out[0..cap).
+// Returns the number of survivors (to every thread).  Two grid syncs.
+template <typename Keep>
+__device__ int64_t coop_unique(cg::grid_group& grid, const uint64_t* __restrict__ keys, int64_t n,
+                               uint64_t* __restrict__ out, int64_t cap, Keep keep,
+                               int64_t* __restrict__ partial, CoopShared& sh) {
     int64_t beg, end;
-    block_chunk(n, &beg, &end);
+    block_chunk(n, kSortThreads, &beg, &end);
     int64_t c = 0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kSortThreads)
-        c += (i == 0 || keys[i] != keys[i - 1]);
-    c = block_sum_i64(c, sh);
-    if (threadIdx.x == 0) blk_count[blockIdx.x] = c;
-}
-
-__global__ void __launch_bounds__(kSortThreads) unique_write_kernel(
-        const uint64_t* __restrict__ keys, const int64_t* __restrict__ n_ptr, int64_t n_cap,
-        const int64_t* __restrict__ blk_count, uint64_t* __restrict__ out, int64_t cap,
-        int64_t* __restrict__ n_out, int32_t* __restrict__ flags, int flag_bit) {
-    __shared__ int64_t sh[32];
-    __shared__ int32_t wtot[kSortWarps];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t n = min(*n_ptr, n_cap);
-    int64_t beg, end;
-    block_chunk(n, &beg, &end);
-    int64_t before = 0, all = 0;
-    for (int b = threadIdx.x; b < (int)gridDim.x; b += kSortThreads) {
-        const int64_t v = blk_count[b];
-        all += v;
-        if (b < (int)blockIdx.x) before += v;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kSortThreads) {
+        const uint64_t k = keys[i];
+        c += (i == 0 || k != keys[i - 1]) && keep(k);
     }
-    before = block_sum_i64(before, sh);
-    all = block_sum_i64(all, sh);
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        *n_out = all;
-        if (all > cap) atomicOr(flags, flag_bit);
-    }
+    c = block_sum_i64(c, sh.red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = c;
+    grid.sync();
+    int64_t before, all;
+    partial_prefix(partial, gridDim.x, blockIdx.x, sh.red, &before, &all);
     int64_t run = before;
     for (int64_t sub = beg; sub < end; sub += kSortThreads) {
         const int64_t i = sub + threadIdx.x;
@@ -330,23 +398,239 @@ __global__ void __launch_bounds__(kSortThreads) unique_write_kernel(
         bool head = false;
         if (i < end) {
             k = keys[i];
-            head = (i == 0 || k != keys[i - 1]);
+            head = (i == 0 || k != keys[i - 1]) && keep(k);
         }
-        const unsigned ball = __ballot_sync(0xffffffffu, head);
-        if (lane == 0) wtot[wid] = __popc(ball);
+        const int64_t pos = compact_pos(head, &run, sh.wtot);
+        if (head && pos < cap) out[pos] = k;
+    }
+    grid.sync();
+    return all;
+}
+
+struct KeepAll {
+    __device__ bool operator()(uint64_t) const { return true; }
+};
+// overflow key (a, b) is redundant if row a already holds b
+struct KeepNotInRow {
+    const uint32_t* rows;
+    int32_t n_rows, S;
+    __device__ bool operator()(uint64_t key) const {
+        const uint32_t a = (uint32_t)(key >> 32), b = (uint32_t)key;
+        if (a >= (uint32_t)n_rows) return true;
+        const uint32_t* row = rows + (size_t)a * kRowStride;
+        for (int k = 0; k < S; ++k) {
+            const uint32_t v = __ldcg(row + k);
+            if (v == b) return false;
+            if (v == kEmptySlot) break;
+        }
+        return true;
+    }
+};
+
+__device__ __forceinline__ int64_t lower_bound_u64(const uint64_t* __restrict__ a, int64_t n, uint64_t key) {
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (a[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// ------------------------------------------------------------------------------------ finish
+template <int N>
+__device__ __forceinline__ void bitonic_sort(uint32_t* e) {
+#pragma unroll
+    for (int k = 2; k <= N; k <<= 1) {
+#pragma unroll
+        for (int j = k >> 1; j > 0; j >>= 1) {
+#pragma unroll
+            for (int i = 0; i < N; ++i) {
+                const int l = i ^ j;
+                if (l > i) {
+                    const uint32_t lo = min(e[i], e[l]), hi = max(e[i], e[l]);
+                    const bool up = (i & k) == 0;
+                    e[i] = up ? lo : hi;
+                    e[l] = up ? hi : lo;
+                }
+            }
+        }
+    }
+}
+
+struct FinishParams {
+    uint32_t* rows;
+    int32_t n_rows;
+    int32_t S;
+    uint64_t* keys_a;          // overflow keys (raw)
+    uint64_t* keys_b;
+    int64_t keys_cap;
+    int64_t* ctl;              // [0] raw overflow count, [1] filtered overflow count, [2] OR of the keys
+    uint32_t* hist;
+    int64_t* partial;          // [2 * gridDim]
+    uint64_t* out;
+    int64_t cap;
+    int64_t* n_out;
+    int32_t* flags;
+};
+
+__global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const FinishParams p) {
+    __shared__ CoopShared sh;
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+    // ---- overflow keys (normally none): sorted, unique, not already in their row
+    const uint64_t* ovf = nullptr;
+    int64_t n_ovf = __ldcg(p.ctl) < p.keys_cap ? __ldcg(p.ctl) : p.keys_cap;
+    if (n_ovf > 0) {                                   // grid-uniform
+        int64_t beg, end;
+        block_chunk(n_ovf, kSortThreads, &beg, &end);
+        unsigned long long m = 0;
+        for (int64_t i = beg + threadIdx.x; i < end; i += kSortThreads) m |= p.keys_a[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m |= __shfl_xor_sync(0xffffffffu, m, o);
+        if (lane == 0 && m) atomicOr((unsigned long long*)&p.ctl[2], m);
+        grid.sync();
+        const uint64_t mask = (uint64_t)__ldcg(&p.ctl[2]);
+        uint64_t* sorted = coop_sort(grid, p.keys_a, p.keys_b, n_ovf, 32, mask, p.hist, sh);
+        uint64_t* dst = sorted == p.keys_a ? p.keys_b : p.keys_a;
+        n_ovf = coop_unique(grid, sorted, n_ovf, dst, p.keys_cap, KeepNotInRow{p.rows, p.n_rows, p.S},
+                            p.partial, sh);
+        ovf = dst;
+    }
+
+    // ---- rows, pass 1: entries per block chunk
+    int64_t rbeg, rend;
+    block_chunk(p.n_rows, kSortThreads, &rbeg, &rend);
+    {
+        int64_t c = 0;
+        for (int64_t a = rbeg + threadIdx.x; a < rend; a += kSortThreads) {
+            const uint32_t* row = p.rows + (size_t)a * kRowStride;
+            for (int q = 0; q < p.S; q += 4) {
+                const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
+                const int m = (v.x != kEmptySlot) + (v.y != kEmptySlot) + (v.z != kEmptySlot) + (v.w != kEmptySlot);
+                c += m;
+                if (m < 4) break;
+            }
+        }
+        c = block_sum_i64(c, sh.red);
+        if (threadIdx.x == 0) p.partial[gridDim.x + blockIdx.x] = c;
+    }
+    grid.sync();
+
+    // ---- rows, pass 2: sort every row in registers and write it at its final position
+    int64_t before, all;
+    partial_prefix(p.partial + gridDim.x, gridDim.x, blockIdx.x, sh.red, &before, &all);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        *p.n_out = all + n_ovf;
+        if (all + n_ovf > p.cap) atomicOr(p.flags, FLAG_EDGE_CAP);
+    }
+    int64_t run = before;
+    for (int64_t base = rbeg; base < rend; base += kSortThreads) {
+        const int64_t a = base + threadIdx.x;
+        uint32_t e[kRowStride];
+#pragma unroll
+        for (int k = 0; k < kRowStride; ++k) e[k] = kEmptySlot;
+        int n = 0;
+        if (a < rend) {
+            uint32_t* row = p.rows + (size_t)a * kRowStride;
+#pragma unroll
+            for (int q = 0; q < kRowStride; q += 4) {
+                if (q < p.S && (q == 0 || e[q - 1] != kEmptySlot)) {
+                    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
+                    e[q] = v.x; e[q + 1] = v.y; e[q + 2] = v.z; e[q + 3] = v.w;
+                    if (v.x != kEmptySlot)            // leave the row empty for the next call
+                        *reinterpret_cast<uint4*>(row + q) = make_uint4(kEmptySlot, kEmptySlot, kEmptySlot, kEmptySlot);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < kRowStride; ++k) n += e[k] != kEmptySlot;
+            if (n > 8) bitonic_sort<16>(e);
+            else if (n > 4) bitonic_sort<8>(e);
+            else if (n > 1) bitonic_sort<4>(e);
+        }
+        // exclusive scan of n over the block
+        int inc = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) sh.wtot[wid] = inc;
         __syncthreads();
-        int32_t wbase = 0, total = 0;
+        int wbase = 0, total = 0;
         for (int w = 0; w < kSortWarps; ++w) {
-            const int32_t t = wtot[w];
+            const int t = sh.wtot[w];
             if (w < wid) wbase += t;
             total += t;
         }
-        if (head) {
-            const int64_t pos = run + wbase + __popc(ball & ((1u << lane) - 1u));
-            if (pos < cap) out[pos] = k;
-        }
+        int64_t pos = run + wbase + inc - n;
         run += total;
         __syncthreads();
+        if (a < rend) {
+            const uint64_t hi = (uint64_t)a << 32;
+            int64_t o0 = 0, o1 = 0;
+            if (n_ovf > 0) {
+                o0 = lower_bound_u64(ovf, n_ovf, hi);
+                o1 = lower_bound_u64(ovf, n_ovf, hi + (1ull << 32));
+                pos += o0;
+            }
+            if (o1 == o0) {
+#pragma unroll
+                for (int k = 0; k < kRowStride; ++k)
+                    if (k < n && pos + k < p.cap) p.out[pos + k] = hi | e[k];
+            } else {
+                // rare: merge the row with its overflow keys (disjoint by construction)
+                uint32_t r[kRowStride];
+#pragma unroll
+                for (int k = 0; k < kRowStride; ++k) r[k] = e[k];
+                int i = 0;
+                int64_t j = o0;
+                while (i < n || j < o1) {
+                    uint64_t key;
+                    if (j >= o1 || (i < n && (hi | r[i]) < ovf[j])) key = hi | r[i++];
+                    else key = ovf[j++];
+                    if (pos < p.cap) p.out[pos] = key;
+                    ++pos;
+                }
+            }
+        }
+    }
+    // ---- overflow keys whose smaller label has no row come last
+    if (n_ovf > 0) {
+        const int64_t t0 = lower_bound_u64(ovf, n_ovf, (uint64_t)p.n_rows << 32);
+        for (int64_t j = t0 + (int64_t)blockIdx.x * kSortThreads + threadIdx.x; j < n_ovf;
+             j += (int64_t)gridDim.x * kSortThreads)
+            if (all + j < p.cap) p.out[all + j] = ovf[j];
+    }
+}
+
+// ------------------------------------------------------------------------------------ plain sort + unique
+struct SortUniqueParams {
+    uint64_t* keys_a;
+    uint64_t* keys_b;
+    const int64_t* n_in;
+    int64_t keys_cap;
+    int label_bits;
+    uint32_t* hist;
+    int64_t* partial;
+    uint64_t* out;
+    int64_t cap;
+    int64_t* n_out;
+    int32_t* flags;
+    int flag_bit;
+};
+
+__global__ void __launch_bounds__(kSortThreads) sort_unique_kernel(const SortUniqueParams p) {
+    __shared__ CoopShared sh;
+    cg::grid_group grid = cg::this_grid();
+    const int64_t n = __ldcg(p.n_in) < p.keys_cap ? __ldcg(p.n_in) : p.keys_cap;
+    const int bits = 2 * p.label_bits;
+    const uint64_t mask = bits >= 64 ? ~0ull : ((1ull << bits) - 1ull);
+    uint64_t* sorted = coop_sort(grid, p.keys_a, p.keys_b, n, p.label_bits, mask, p.hist, sh);
+    const int64_t all = coop_unique(grid, sorted, n, p.out, p.cap, KeepAll{}, p.partial, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        *p.n_out = all;
+        if (all > p.cap) atomicOr(p.flags, p.flag_bit);
     }
 }
 
@@ -354,25 +638,14 @@ __global__ void __launch_bounds__(kSortThreads) unique_write_kernel(
 
 // Sort the *d_n_in keys held in ctx->d_keys_a (d_keys_in_a must be that buffer) and write the
 // ascending unique list to d_out[0..cap), its length to *d_n_out.  key_bits = significant bits of
-// each 32-bit half.  Uses ctx->d_keys_b as the pong buffer.
+// each 32-bit half.  Uses ctx->d_keys_b as the pong buffer.  One cooperative launch.
 int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n_in, int key_bits,
                          uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
                          cudaStream_t stream) {
-    const int passes = (2 * key_bits + 7) / 8;
-    uint64_t* src = d_keys_in_a;
-    uint64_t* dst = ctx->d_keys_b;
-    for (int pass = 0; pass < passes; ++pass) {
-        DigitSpec ds{key_bits, 8 * pass};
-        VOR_LAUNCH(radix_hist_kernel, kSortBlocks, kSortThreads, 0, stream, src, d_n_in,
-                   ctx->max_raw_keys, ds, ctx->d_hist);
-        VOR_LAUNCH(radix_scatter_kernel, kSortBlocks, kSortThreads, 0, stream, src, dst, d_n_in,
-                   ctx->max_raw_keys, ds, ctx->d_hist);
-        uint64_t* t = src; src = dst; dst = t;
-    }
-    VOR_LAUNCH(unique_count_kernel, kSortBlocks, kSortThreads, 0, stream, src, d_n_in,
-               ctx->max_raw_keys, ctx->d_blk_count);
-    VOR_LAUNCH(unique_write_kernel, kSortBlocks, kSortThreads, 0, stream, src, d_n_in,
-               ctx->max_raw_keys, ctx->d_blk_count, d_out, cap, d_n_out, ctx->d_flags, flag_bit);
+    SortUniqueParams p{d_keys_in_a, ctx->d_keys_b, d_n_in, ctx->max_raw_keys, key_bits, ctx->d_hist,
+                       ctx->d_blk_count, d_out, cap, d_n_out, ctx->d_flags, flag_bit};
+    const int grid = vor_coop_grid(ctx, 1, (const void*)sort_unique_kernel, kSortThreads, 1);
+    VOR_LAUNCH_COOP(sort_unique_kernel, grid, kSortThreads, stream, (void*)&p);
     return VOR_OK;
 }
 
@@ -382,16 +655,23 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     if (!d_labels || !d_edges || !d_n_edges || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_edges: null pointer or negative capacity");
     cudaStream_t stream = (cudaStream_t)stream_;
-    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, sizeof(int64_t), stream));
+    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 4 * sizeof(int64_t), stream));
     const int32_t L = ctx->L;
+    RowSet rs;
+    rs.rows = ctx->d_rows;
+    rs.n_rows = ctx->n_sites > 0 ? ctx->n_sites : ctx->max_sites;
+    rs.S = (int32_t)ctx->row_slots;
+    rs.ovf = ctx->d_keys_a;
+    rs.ovf_cap = ctx->max_raw_keys;
+    rs.n_ovf = (unsigned long long*)ctx->d_n_raw;
+    rs.flags = ctx->d_flags;
     dim3 grid((L + kEmitCols - 1) / kEmitCols, (L + kEmitRows - 1) / kEmitRows);
     const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0);
-    if (vec)
-        VOR_LAUNCH(edges_emit_kernel<true>, grid, kEmitThreads, 0, stream, d_labels, L, ctx->d_keys_a,
-                   ctx->max_raw_keys, (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
-    else
-        VOR_LAUNCH(edges_emit_kernel<false>, grid, kEmitThreads, 0, stream, d_labels, L, ctx->d_keys_a,
-                   ctx->max_raw_keys, (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
-    return vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, vor_label_bits(ctx), d_edges, cap,
-                                d_n_edges, FLAG_EDGE_CAP, stream);
+    if (vec) VOR_LAUNCH(edges_emit_kernel<true>, grid, kEmitThreads, 0, stream, d_labels, L, rs);
+    else VOR_LAUNCH(edges_emit_kernel<false>, grid, kEmitThreads, 0, stream, d_labels, L, rs);
+    FinishParams fp{ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
+                    ctx->d_n_raw, ctx->d_hist, ctx->d_blk_count, d_edges, cap, d_n_edges, ctx->d_flags};
+    const int fgrid = vor_coop_grid(ctx, 0, (const void*)edges_finish_kernel, kSortThreads, 1);
+    VOR_LAUNCH_COOP(edges_finish_kernel, fgrid, kSortThreads, stream, (void*)&fp);
+    return VOR_OK;
 }

@@ -129,13 +129,16 @@ def test_labels_hex_and_rhombus_constructions(G):
 
 
 # ------------------------------------------------------------------ edges (a3 + a4)
-def check_edges(G, labels, max_sites):
+def check_edges(G, labels, max_sites, row_slots=(16,)):
     L = labels.shape[0]
     v = make(L, max_sites)
-    got = G.gpu_edges(v, labels, cap=max(1024, 2 * L * L))
     ref = oracle.edges(labels)
+    for s in row_slots:
+        v.vor_set_option("row_slots", s)
+        for _ in range(2):                             # twice: the rows must be left empty
+            got = G.gpu_edges(v, labels, cap=max(1024, 2 * L * L))
+            assert got.dtype == np.uint64 and np.array_equal(got, ref), (s, len(got), len(ref))
     v.close()
-    assert got.dtype == np.uint64 and np.array_equal(got, ref), (len(got), len(ref))
 
 
 def test_edges_hand_images(G):
@@ -155,7 +158,22 @@ def test_edges_on_oracle_labels(G, cfg, L):
     w = W.config(cfg) if L is None else W.scaled(cfg, L)
     sx, sy = next(iter(w.frames(1)))
     lab = oracle.label_cells(w.L, sx, sy, 8)
-    check_edges(G, lab, w.n_sites)
+    check_edges(G, lab, w.n_sites, row_slots=(16, 4))   # 4 slots: many rows spill to the overflow path
+
+
+def test_edges_overflow_paths(G):
+    """Rows that overflow, labels beyond the row range, and both at once."""
+    rng = np.random.default_rng(11)
+    # a hub: label 0 touches 300 other labels (row 0 overflows for any slot count)
+    lab = np.zeros((64, 64), np.int32)
+    ys, xs = np.nonzero((np.arange(64)[:, None] % 3 == 1) & (np.arange(64)[None, :] % 3 == 1))
+    lab[ys[:300], xs[:300]] = 1 + np.arange(300)
+    check_edges(G, lab, 400, row_slots=(16, 8, 4))
+    # max_sites smaller than the largest label: pairs whose smaller label has no row
+    check_edges(G, rng.integers(0, 500, (96, 96)).astype(np.int32), 100, row_slots=(16, 4))
+    check_edges(G, rng.integers(0, 40, (200, 200)).astype(np.int32), 40, row_slots=(16, 12, 4))
+    # stripes: every label has exactly two neighbours, one of them through the wrap
+    check_edges(G, np.repeat(np.arange(50, dtype=np.int32), 4)[None, :].repeat(200, 0), 50)
 
 
 def test_edges_capacity_overflow_is_reported(G):
@@ -189,10 +207,17 @@ def test_diff_hand_and_random(G):
         rc, rd = oracle.diff(a, b)
         assert np.array_equal(c, rc) and np.array_equal(d, rd)
     rng = np.random.default_rng(5)
-    for n in (10, 5000, 200000):
+    for n in (10, 5000, 200000, 3000000):
         mk = lambda: np.unique((rng.integers(0, 3000, n).astype(np.uint64) << np.uint64(32))
                                | rng.integers(3000, 6000, n).astype(np.uint64))
         a, b = mk(), mk()
+        c, d = G.gpu_diff(v, a, b)
+        rc, rd = oracle.diff(a, b)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd)
+    # very different densities: the window of the dense list does not fit in shared memory
+    dense = np.unique(rng.integers(0, 1 << 40, 2000000).astype(np.uint64))
+    sparse = np.unique(np.concatenate([dense[::1000], rng.integers(0, 1 << 40, 1500).astype(np.uint64)]))
+    for a, b in ((dense, sparse), (sparse, dense)):
         c, d = G.gpu_diff(v, a, b)
         rc, rd = oracle.diff(a, b)
         assert np.array_equal(c, rc) and np.array_equal(d, rd)
