@@ -116,6 +116,10 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         ctx->row_slots = value;
         return VOR_OK;
     }
+    if (!strcmp(name, "edges_generic")) {
+        ctx->edges_generic = value != 0;
+        return VOR_OK;
+    }
     if (!strcmp(name, "label_fast_off")) {
         ctx->label_fast_off = value != 0;
         return VOR_OK;

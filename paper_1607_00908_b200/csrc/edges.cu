@@ -33,6 +33,9 @@ struct RowSet {
     uint64_t* ovf;             // overflow keys (unordered, may repeat)
     int64_t ovf_cap;
     unsigned long long* n_ovf;
+    uint64_t* raw;             // per-CTA distinct keys, appended by the emit kernels
+    int64_t raw_cap;
+    unsigned long long* n_raw;
     int32_t* flags;
 };
 
@@ -65,11 +68,6 @@ __device__ __noinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b
 }
 
 // ------------------------------------------------------------------------------------ emit
-constexpr int kEmitThreads = 256;
-constexpr int kEmitWarps = kEmitThreads / 32;
-constexpr int kEmitCols = 128;          // per CTA tile: 32 lanes x 4 labels
-constexpr int kEmitRowsPerWarp = 16;
-constexpr int kEmitRows = kEmitWarps * kEmitRowsPerWarp;   // 128
 constexpr int kHashSlots = 2048;
 constexpr int kMaxProbe = 32;
 constexpr int kQueueCap = 32 + 256;     // < 32 pending + at most 8 pairs per lane per row
@@ -96,11 +94,218 @@ __device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned lon
     row_insert(rs, lo, hi);    // table crowded (very dense sites): straight to the matrix
 }
 
-template <bool VEC>
+// ---- streaming kernel (L % 4 == 0, 16-byte aligned image).
+// A warp owns a strip of 128 columns x kStripRows rows and walks down it, 4 columns per lane, rows
+// prefetched two ahead in registers.  Work is done in three stages of decreasing volume, each one
+// dense over the 32 lanes:
+//   A  per row and lane: is any of the lane's 8 compared pairs (cell | right neighbour, row above |
+//      cell) a discontinuity?  One OR of XORs.  Rows that repeat the row above exactly (a vertical
+//      boundary running down the strip) are skipped: their pairs were seen there.  "Dirty" lane-rows
+//      are compacted (ballot) into a queue of 9-label records {row, row above, right neighbour}.
+//   B  32 records at a time: if the 9 labels take only two values {a, b} - the usual case, one
+//      boundary crossing the window - the record contributes exactly the key (a, b): one hash
+//      insertion.  Otherwise (a Voronoi vertex nearby) its discontinuities are expanded into a
+//      second queue of (label, label) pairs.
+//   C  32 pairs at a time: hash insertion.
+// The CTA's hash set ends up holding every distinct key of its tile; it is appended to a global
+// raw-key list (one atomic per CTA) that the finish kernel inserts into the adjacency matrix.
+constexpr int kStrWarpsX = 2, kStrWarpsY = 4;
+constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
+constexpr int kStrThreads = 32 * kStrWarps;                     // 256
+constexpr int kStripCols = 128;
+constexpr int kStripRows = 32;                                  // rows per warp
+constexpr int kRecCap = 64;                                     // < 32 pending + 32 per row
+constexpr int kPairCap = 32 + 256;                              // < 32 pending + 8 per record
+
+struct __align__(16) Rec {
+    int4 c;        // the lane-row's 4 labels
+    int4 pc;       // the 4 labels above them
+    int32_t rr3;   // right neighbour of c.w
+    int32_t pad[3];
+};
+
+struct StreamShared {
+    unsigned long long table[kHashSlots];
+    Rec rec[kStrWarps][kRecCap];
+    uint2 pairs[kStrWarps][kPairCap];
+    int32_t scan[kStrWarps + 1];
+};
+
+// Append the CTA's distinct keys to the global raw list (falls back to direct insertion if full).
+__device__ __forceinline__ void hash_flush(const unsigned long long* table, const RowSet& rs,
+                                           int32_t* scan /* [warps + 1] */) {
+    constexpr int kPer = kHashSlots / kStrThreads;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    unsigned long long mine[kPer];
+    int cnt = 0;
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) {
+        mine[k] = table[k * kStrThreads + threadIdx.x];
+        cnt += mine[k] != kEmptyKey;
+    }
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) scan[wid] = inc;
+    __syncthreads();
+    int wbase = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kStrWarps; ++w) {
+        if (w < wid) wbase += scan[w];
+        total += scan[w];
+    }
+    __shared__ long long base_sh;
+    if (threadIdx.x == 0) base_sh = total ? (long long)atomicAdd(rs.n_raw, (unsigned long long)total) : 0;
+    __syncthreads();
+    const int64_t base = base_sh;
+    if (base + total <= rs.raw_cap) {
+        int64_t pos = base + wbase + inc - cnt;
+#pragma unroll
+        for (int k = 0; k < kPer; ++k)
+            if (mine[k] != kEmptyKey) rs.raw[pos++] = mine[k];
+    } else {
+#pragma unroll 1
+        for (int k = 0; k < kPer; ++k)
+            if (mine[k] != kEmptyKey) row_insert(rs, (uint32_t)(mine[k] >> 32), (uint32_t)mine[k]);
+    }
+}
+
+__global__ void __launch_bounds__(kStrThreads, 3) edges_stream_kernel(const int32_t* __restrict__ labels,
+                                                                      int32_t L, const RowSet rs) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    StreamShared& sh = *reinterpret_cast<StreamShared*>(smem_raw);
+    for (int i = threadIdx.x; i < kHashSlots; i += kStrThreads) sh.table[i] = kEmptyKey;
+    __syncthreads();
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    const int32_t xbase = (blockIdx.x * kStrWarpsX + (wid % kStrWarpsX)) * kStripCols;
+    const int32_t x0 = xbase + 4 * lane;
+    const int32_t ybeg = (blockIdx.y * kStrWarpsY + (wid / kStrWarpsX)) * kStripRows;
+    const int32_t yend = min(ybeg + kStripRows, L);
+    Rec* __restrict__ rq = sh.rec[wid];
+    uint2* __restrict__ pq = sh.pairs[wid];
+    int rn = 0, pn = 0;                            // warp-uniform queue fills
+
+    // stage C: one dense pass over 32 queued pairs
+    auto drain_pairs = [&](bool all) {
+        while (pn >= 32 || (all && pn > 0)) {
+            const int take = min(pn, 32);
+            pn -= take;
+            if (lane < take) {
+                const uint2 it = pq[pn + lane];
+                hash_insert(it.x, it.y, sh.table, rs);
+            }
+            __syncwarp();
+        }
+    };
+    // stage B: one dense pass over `take` queued records
+    auto process_recs = [&](int take) {
+        rn -= take;
+        int4 c = make_int4(0, 0, 0, 0), pc = c;
+        int32_t rr3 = 0;
+        if (lane < take) {
+            const Rec& r = rq[rn + lane];
+            c = r.c; pc = r.pc; rr3 = r.rr3;
+        }
+        __syncwarp();
+        const uint32_t a = (uint32_t)c.x;
+        const uint32_t t1 = c.y ^ a, t2 = c.z ^ a, t3 = c.w ^ a, t4 = rr3 ^ a;
+        const uint32_t t5 = pc.x ^ a, t6 = pc.y ^ a, t7 = pc.z ^ a, t8 = pc.w ^ a;
+        const uint32_t X = t1 | t2 | t3 | t4 | t5 | t6 | t7 | t8;
+        // a label other than a and a ^ X shows as a t that is neither 0 nor X
+        const uint32_t bad = min(t1, t1 ^ X) | min(t2, t2 ^ X) | min(t3, t3 ^ X) | min(t4, t4 ^ X) |
+                             min(t5, t5 ^ X) | min(t6, t6 ^ X) | min(t7, t7 ^ X) | min(t8, t8 ^ X);
+        if (X != 0 && bad == 0) hash_insert(a, a ^ X, sh.table, rs);
+        const unsigned badm = __ballot_sync(full, bad != 0);
+        if (badm) {                                // expand the discontinuities of >2-label records
+            unsigned bits = 0;
+            if (bad != 0)
+                bits = (unsigned)(c.x != c.y) | (unsigned)(c.y != c.z) << 1 | (unsigned)(c.z != c.w) << 2 |
+                       (unsigned)(c.w != rr3) << 3 | (unsigned)(pc.x != c.x) << 4 | (unsigned)(pc.y != c.y) << 5 |
+                       (unsigned)(pc.z != c.z) << 6 | (unsigned)(pc.w != c.w) << 7;
+            const int cnt = __popc(bits);
+            int inc = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(full, inc, o);
+                if (lane >= o) inc += t;
+            }
+            int pos = pn + inc - cnt;
+            if (bits & 1u) pq[pos++] = make_uint2(c.x, c.y);
+            if (bits & 2u) pq[pos++] = make_uint2(c.y, c.z);
+            if (bits & 4u) pq[pos++] = make_uint2(c.z, c.w);
+            if (bits & 8u) pq[pos++] = make_uint2(c.w, rr3);
+            if (bits & 16u) pq[pos++] = make_uint2(pc.x, c.x);
+            if (bits & 32u) pq[pos++] = make_uint2(pc.y, c.y);
+            if (bits & 64u) pq[pos++] = make_uint2(pc.z, c.z);
+            if (bits & 128u) pq[pos++] = make_uint2(pc.w, c.w);
+            pn += __shfl_sync(full, inc, 31);
+            __syncwarp();
+            drain_pairs(false);
+        }
+    };
+
+    if (xbase < L && ybeg < L) {                   // warp-uniform
+        const bool active = x0 < L;                // L % 4 == 0: a lane's 4 columns are all in or all out
+        const bool halo = active && (lane == 31 || x0 + 4 >= L);   // right neighbour not in the next lane
+        const int32_t xh = x0 + 4 >= L ? 0 : x0 + 4;
+        auto load4 = [&](int32_t y) {
+            return active ? __ldcs(reinterpret_cast<const int4*>(labels + (int64_t)y * L + x0)) : make_int4(0, 0, 0, 0);
+        };
+        auto loadh = [&](int32_t y) { return halo ? __ldg(labels + (int64_t)y * L + xh) : 0; };
+        int4 pc = load4(ybeg == 0 ? L - 1 : ybeg - 1);          // the row above the strip (wrapped)
+        int32_t prr3 = 0;
+        uint32_t force = 1;                                     // first row: nothing may be skipped
+        int4 n0 = load4(ybeg), n1 = ybeg + 1 < yend ? load4(ybeg + 1) : n0;
+        int32_t h0 = loadh(ybeg), h1 = ybeg + 1 < yend ? loadh(ybeg + 1) : 0;
+#pragma unroll 4
+        for (int32_t y = ybeg; y < yend; ++y) {
+            const int4 c = n0;
+            const int32_t hc = h0;
+            n0 = n1; h0 = h1;
+            if (y + 2 < yend) { n1 = load4(y + 2); h1 = loadh(y + 2); }
+            const int32_t nb = __shfl_down_sync(full, c.x, 1);
+            const int32_t rr3 = halo ? hc : nb;
+            const uint32_t dh = (c.x ^ c.y) | (c.y ^ c.z) | (c.z ^ c.w) | (c.w ^ rr3);
+            const uint32_t dv = (pc.x ^ c.x) | (pc.y ^ c.y) | (pc.z ^ c.z) | (pc.w ^ c.w);
+            const uint32_t e = (uint32_t)(rr3 ^ prr3) | force;
+            // identical to the row above (dv == 0, e == 0): same horizontal pairs, no vertical ones
+            const bool dirty = active && (dv != 0 || (dh != 0 && e != 0));
+            const unsigned m = __ballot_sync(full, dirty);
+            if (m) {
+                if (dirty) {
+                    Rec& r = rq[rn + __popc(m & lt)];
+                    r.c = c; r.pc = pc; r.rr3 = rr3;
+                }
+                rn += __popc(m);
+                __syncwarp();
+                if (rn >= 32) process_recs(32);
+            }
+            pc = c; prr3 = rr3; force = 0;
+        }
+        if (rn > 0) process_recs(rn);
+        drain_pairs(true);
+    }
+    __syncthreads();
+    hash_flush(sh.table, rs, sh.scan);
+}
+
+// ---- generic kernel (any L, any alignment): scalar loads, every discontinuity goes to the hash set.
+constexpr int kEmitThreads = 256;
+constexpr int kEmitCols = 128;          // per CTA tile: 32 lanes x 4 labels
+constexpr int kEmitRowsPerWarp = 16;
+constexpr int kEmitRows = (kEmitThreads / 32) * kEmitRowsPerWarp;   // 128
+
 __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t* __restrict__ labels,
                                                                   int32_t L, const RowSet rs) {
     __shared__ unsigned long long table[kHashSlots];
-    __shared__ uint2 queue[kEmitWarps][kQueueCap];
+    __shared__ uint2 queue[kEmitThreads / 32][kQueueCap];
+    __shared__ int32_t scan[kEmitThreads / 32 + 1];
+    static_assert(kEmitThreads == kStrThreads, "hash_flush is written for one block size");
     for (int i = threadIdx.x; i < kHashSlots; i += kEmitThreads) table[i] = kEmptyKey;
     __syncthreads();
     const unsigned full = 0xffffffffu;
@@ -111,17 +316,8 @@ __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t*
     int qn = 0;                                    // warp-uniform queue fill
     if (ybeg < L) {
         auto load_row = [&](const int32_t* __restrict__ row, int32_t* v) {
-            if (VEC) {
-                if (x0 < L) {
-                    const int4 t = __ldcs(reinterpret_cast<const int4*>(row + x0));
-                    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
-                } else {
-                    v[0] = v[1] = v[2] = v[3] = 0;
-                }
-            } else {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) v[k] = x0 + k < L ? __ldg(row + x0 + k) : 0;
-            }
+            for (int k = 0; k < 4; ++k) v[k] = x0 + k < L ? __ldg(row + x0 + k) : 0;
         };
         int32_t c[4], nx[4];
         load_row(labels + (int64_t)ybeg * L, c);
@@ -141,7 +337,7 @@ __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t*
             unsigned bits = 0;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const bool valid = VEC ? (x0 < L) : (x0 + k < L);
+                const bool valid = x0 + k < L;
                 bits |= (unsigned)(valid && c[k] != rr[k]) << k;
                 bits |= (unsigned)(valid && c[k] != nx[k]) << (4 + k);
             }
@@ -179,12 +375,7 @@ __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t*
         }
     }
     __syncthreads();
-    // the CTA's distinct pairs go to the adjacency matrix
-#pragma unroll
-    for (int k = 0; k < kHashSlots / kEmitThreads; ++k) {
-        const unsigned long long key = table[k * kEmitThreads + threadIdx.x];
-        if (key != kEmptyKey) row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
-    }
+    hash_flush(table, rs, scan);
 }
 
 // ------------------------------------------------------------------------------------ block helpers
@@ -458,13 +649,14 @@ __device__ __forceinline__ void bitonic_sort(uint32_t* e) {
 }
 
 struct FinishParams {
+    RowSet rs;                 // matrix, raw list (keys_b) and overflow list (keys_a)
     uint32_t* rows;
     int32_t n_rows;
     int32_t S;
-    uint64_t* keys_a;          // overflow keys (raw)
-    uint64_t* keys_b;
+    uint64_t* keys_a;          // overflow keys (unordered)
+    uint64_t* keys_b;          // raw keys of the emit kernel; later the sort's pong buffer
     int64_t keys_cap;
-    int64_t* ctl;              // [0] raw overflow count, [1] filtered overflow count, [2] OR of the keys
+    int64_t* ctl;              // [0] overflow count, [2] OR of the overflow keys, [3] raw key count
     uint32_t* hist;
     int64_t* partial;          // [2 * gridDim]
     uint64_t* out;
@@ -477,6 +669,17 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
     __shared__ CoopShared sh;
     cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+    // ---- the CTAs' distinct keys -> adjacency matrix (exact set insertion; full rows overflow)
+    {
+        const int64_t n_raw = __ldcg(&p.ctl[3]) < p.keys_cap ? __ldcg(&p.ctl[3]) : p.keys_cap;
+        for (int64_t i = (int64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n_raw;
+             i += (int64_t)gridDim.x * kSortThreads) {
+            const uint64_t key = __ldcs(p.keys_b + i);
+            row_insert(p.rs, (uint32_t)(key >> 32), (uint32_t)key);
+        }
+    }
+    grid.sync();
 
     // ---- overflow keys (normally none): sorted, unique, not already in their row
     const uint64_t* ovf = nullptr;
@@ -664,12 +867,23 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     rs.ovf = ctx->d_keys_a;
     rs.ovf_cap = ctx->max_raw_keys;
     rs.n_ovf = (unsigned long long*)ctx->d_n_raw;
+    rs.raw = ctx->d_keys_b;
+    rs.raw_cap = ctx->max_raw_keys;
+    rs.n_raw = (unsigned long long*)&ctx->d_n_raw[3];
     rs.flags = ctx->d_flags;
-    dim3 grid((L + kEmitCols - 1) / kEmitCols, (L + kEmitRows - 1) / kEmitRows);
-    const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0);
-    if (vec) VOR_LAUNCH(edges_emit_kernel<true>, grid, kEmitThreads, 0, stream, d_labels, L, rs);
-    else VOR_LAUNCH(edges_emit_kernel<false>, grid, kEmitThreads, 0, stream, d_labels, L, rs);
-    FinishParams fp{ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
+    const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
+    if (vec) {
+        static_assert(sizeof(StreamShared) <= 74 * 1024, "three CTAs per SM");
+        VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sizeof(StreamShared)));
+        dim3 grid((L + kStrWarpsX * kStripCols - 1) / (kStrWarpsX * kStripCols),
+                  (L + kStrWarpsY * kStripRows - 1) / (kStrWarpsY * kStripRows));
+        VOR_LAUNCH(edges_stream_kernel, grid, kStrThreads, sizeof(StreamShared), stream, d_labels, L, rs);
+    } else {
+        dim3 grid((L + kEmitCols - 1) / kEmitCols, (L + kEmitRows - 1) / kEmitRows);
+        VOR_LAUNCH(edges_emit_kernel, grid, kEmitThreads, 0, stream, d_labels, L, rs);
+    }
+    FinishParams fp{rs, ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
                     ctx->d_n_raw, ctx->d_hist, ctx->d_blk_count, d_edges, cap, d_n_edges, ctx->d_flags};
     const int fgrid = vor_coop_grid(ctx, 0, (const void*)edges_finish_kernel, kSortThreads, 1);
     VOR_LAUNCH_COOP(edges_finish_kernel, fgrid, kSortThreads, stream, (void*)&fp);

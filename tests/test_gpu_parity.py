@@ -135,9 +135,10 @@ def check_edges(G, labels, max_sites, row_slots=(16,)):
     ref = oracle.edges(labels)
     for s in row_slots:
         v.vor_set_option("row_slots", s)
-        for _ in range(2):                             # twice: the rows must be left empty
+        for generic in (0, 1, 0):                      # repeated: the rows must be left empty
+            v.vor_set_option("edges_generic", generic)
             got = G.gpu_edges(v, labels, cap=max(1024, 2 * L * L))
-            assert got.dtype == np.uint64 and np.array_equal(got, ref), (s, len(got), len(ref))
+            assert got.dtype == np.uint64 and np.array_equal(got, ref), (s, generic, len(got), len(ref))
     v.close()
 
 
@@ -151,6 +152,11 @@ def test_edges_hand_images(G):
     check_edges(G, rng.integers(0, 1000, (37, 37)).astype(np.int32), 1000)      # ragged, noise labels
     check_edges(G, rng.integers(0, 2 ** 31 - 1, (64, 64)).astype(np.int32), 1)  # 31-bit labels
     check_edges(G, rng.integers(0, 50000, (256, 256)).astype(np.int32), 50000)  # hash-set overflow path
+    check_edges(G, rng.integers(0, 3, (4, 4)).astype(np.int32), 3)              # one lane, halo = column 0
+    check_edges(G, rng.integers(0, 9, (132, 132)).astype(np.int32), 9)          # ragged strips, noisy rows
+    lab = np.zeros((520, 520), np.int32); lab[:, 130:391] = 1; lab[259:262, :] = 2   # long straight boundaries
+    lab[300:, 128] = 3; lab[77, 3:9] = 4
+    check_edges(G, lab, 5)
 
 
 @pytest.mark.parametrize("cfg,L", [(1, None), (2, None), (5, 512), (5, 1000), (5, 2048)])
