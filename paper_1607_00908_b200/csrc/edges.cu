@@ -95,18 +95,20 @@ __device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned lon
 }
 
 // ---- streaming kernel (L % 4 == 0, 16-byte aligned image).
-// A warp owns a strip of 128 columns x kStripRows rows and walks down it, 4 columns per lane, rows
-// prefetched two ahead in registers.  Work is done in three stages of decreasing volume, each one
-// dense over the 32 lanes:
+// A warp owns a strip of 128 columns x kStripRows rows and walks down it, 4 columns per lane, kPf
+// rows in flight per lane (register prefetch; pointers advance by L, no per-row address arithmetic).
+// Work is done in three stages of decreasing volume, each one dense over the 32 lanes:
 //   A  per row and lane: is any of the lane's 8 compared pairs (cell | right neighbour, row above |
-//      cell) a discontinuity?  One OR of XORs.  Rows that repeat the row above exactly (a vertical
-//      boundary running down the strip) are skipped: their pairs were seen there.  "Dirty" lane-rows
-//      are compacted (ballot) into a queue of 9-label records {row, row above, right neighbour}.
+//      cell) a discontinuity?  A few ORs of XORs.  A lane-row that repeats the row above exactly over
+//      its 5 columns is skipped: it has no vertical pair and its horizontal pairs are those of the row
+//      above, which its owner (this warp, or the warp / CTA above) reports.  The chain ends at
+//      row 0 at the latest, which is never skipped, so every distinct pair is reported at least once;
+//      the set insertion downstream makes "at least once" enough.  "Dirty" lane-rows are compacted
+//      (ballot) into a queue of 9-label records {row, row above, right neighbour}.
 //   B  32 records at a time: if the 9 labels take only two values {a, b} - the usual case, one
 //      boundary crossing the window - the record contributes exactly the key (a, b): one hash
-//      insertion.  Otherwise (a Voronoi vertex nearby) its discontinuities are expanded into a
-//      second queue of (label, label) pairs.
-//   C  32 pairs at a time: hash insertion.
+//      insertion.  Otherwise (a Voronoi vertex nearby) the record moves on to a second queue.
+//   C  32 such records at a time: each of the 8 compared pairs that differ is inserted.
 // The CTA's hash set ends up holding every distinct key of its tile; it is appended to a global
 // raw-key list (one atomic per CTA) that the finish kernel inserts into the adjacency matrix.
 constexpr int kStrWarpsX = 2, kStrWarpsY = 4;
@@ -114,20 +116,20 @@ constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
 constexpr int kStrThreads = 32 * kStrWarps;                     // 256
 constexpr int kStripCols = 128;
 constexpr int kStripRows = 32;                                  // rows per warp
-constexpr int kRecCap = 64;                                     // < 32 pending + 32 per row
-constexpr int kPairCap = 32 + 256;                              // < 32 pending + 8 per record
+constexpr int kPf = 4;                                          // rows in flight per lane
+constexpr int kRecCap = 96;                                     // < 32 pending + 2 rows x 32
+constexpr int kMultiCap = 64;                                   // < 32 pending + 32 per batch
 
-struct __align__(16) Rec {
-    int4 c;        // the lane-row's 4 labels
-    int4 pc;       // the 4 labels above them
-    int32_t rr3;   // right neighbour of c.w
-    int32_t pad[3];
+struct RecQueue {                                               // SoA: conflict-free 128-bit accesses
+    int4 c[kRecCap];       // the lane-row's 4 labels
+    int4 pc[kRecCap];      // the 4 labels above them
+    int32_t rr3[kRecCap];  // right neighbour of c.w
 };
 
 struct StreamShared {
     unsigned long long table[kHashSlots];
-    Rec rec[kStrWarps][kRecCap];
-    uint2 pairs[kStrWarps][kPairCap];
+    RecQueue rec[kStrWarps];
+    int32_t multi[kStrWarps][kMultiCap * 9];   // 9 labels per record (c0..c3, rr3, pc0..pc3); odd stride
     int32_t scan[kStrWarps + 1];
 };
 
@@ -186,109 +188,123 @@ __global__ void __launch_bounds__(kStrThreads, 3) edges_stream_kernel(const int3
     const int32_t x0 = xbase + 4 * lane;
     const int32_t ybeg = (blockIdx.y * kStrWarpsY + (wid / kStrWarpsX)) * kStripRows;
     const int32_t yend = min(ybeg + kStripRows, L);
-    Rec* __restrict__ rq = sh.rec[wid];
-    uint2* __restrict__ pq = sh.pairs[wid];
-    int rn = 0, pn = 0;                            // warp-uniform queue fills
+    RecQueue& rq = sh.rec[wid];
+    int32_t* __restrict__ mq = sh.multi[wid];
+    int rn = 0, mn = 0;                            // warp-uniform queue fills
 
-    // stage C: one dense pass over 32 queued pairs
-    auto drain_pairs = [&](bool all) {
-        while (pn >= 32 || (all && pn > 0)) {
-            const int take = min(pn, 32);
-            pn -= take;
+    // stage C: every differing pair of `take` queued multi-label records.  Pair k < 4 is
+    // (label k, label k + 1) of {c0..c3, rr3}; pair k >= 4 is (pc[k-4], c[k-4]) = (label k + 1, label k - 4).
+    auto process_multi = [&](int take) {
+        mn -= take;
+        const int32_t* __restrict__ r = mq + (mn + lane) * 9;
+#pragma unroll 1
+        for (int k = 0; k < 8; ++k) {
             if (lane < take) {
-                const uint2 it = pq[pn + lane];
-                hash_insert(it.x, it.y, sh.table, rs);
+                const int32_t u = r[k < 4 ? k : k + 1], v = r[k < 4 ? k + 1 : k - 4];
+                if (u != v) hash_insert(u, v, sh.table, rs);
             }
-            __syncwarp();
         }
+        __syncwarp();
     };
     // stage B: one dense pass over `take` queued records
     auto process_recs = [&](int take) {
         rn -= take;
         int4 c = make_int4(0, 0, 0, 0), pc = c;
         int32_t rr3 = 0;
-        if (lane < take) {
-            const Rec& r = rq[rn + lane];
-            c = r.c; pc = r.pc; rr3 = r.rr3;
-        }
+        if (lane < take) { c = rq.c[rn + lane]; pc = rq.pc[rn + lane]; rr3 = rq.rr3[rn + lane]; }
         __syncwarp();
         const uint32_t a = (uint32_t)c.x;
         const uint32_t t1 = c.y ^ a, t2 = c.z ^ a, t3 = c.w ^ a, t4 = rr3 ^ a;
         const uint32_t t5 = pc.x ^ a, t6 = pc.y ^ a, t7 = pc.z ^ a, t8 = pc.w ^ a;
-        const uint32_t X = t1 | t2 | t3 | t4 | t5 | t6 | t7 | t8;
-        // a label other than a and a ^ X shows as a t that is neither 0 nor X
-        const uint32_t bad = min(t1, t1 ^ X) | min(t2, t2 ^ X) | min(t3, t3 ^ X) | min(t4, t4 ^ X) |
-                             min(t5, t5 ^ X) | min(t6, t6 ^ X) | min(t7, t7 ^ X) | min(t8, t8 ^ X);
-        if (X != 0 && bad == 0) hash_insert(a, a ^ X, sh.table, rs);
-        const unsigned badm = __ballot_sync(full, bad != 0);
-        if (badm) {                                // expand the discontinuities of >2-label records
-            unsigned bits = 0;
-            if (bad != 0)
-                bits = (unsigned)(c.x != c.y) | (unsigned)(c.y != c.z) << 1 | (unsigned)(c.z != c.w) << 2 |
-                       (unsigned)(c.w != rr3) << 3 | (unsigned)(pc.x != c.x) << 4 | (unsigned)(pc.y != c.y) << 5 |
-                       (unsigned)(pc.z != c.z) << 6 | (unsigned)(pc.w != c.w) << 7;
-            const int cnt = __popc(bits);
-            int inc = cnt;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(full, inc, o);
-                if (lane >= o) inc += t;
+        // two labels {a, b}  <=>  every non-zero t equals the largest one (b = a ^ max t)
+        const uint32_t mx = max(max(max(t1, t2), max(t3, t4)), max(max(t5, t6), max(t7, t8)));
+        const uint32_t lo = min(min(min(t1 - 1u, t2 - 1u), min(t3 - 1u, t4 - 1u)),
+                                min(min(t5 - 1u, t6 - 1u), min(t7 - 1u, t8 - 1u)));   // 0 -> 2^32 - 1
+        const bool any = mx != 0, two = lo == mx - 1u;
+        if (any && two) hash_insert(a, a ^ mx, sh.table, rs);
+        const bool multi = any && !two;
+        const unsigned mm = __ballot_sync(full, multi);
+        if (mm) {
+            if (multi) {
+                int32_t* __restrict__ r = mq + (mn + __popc(mm & lt)) * 9;
+                r[0] = c.x; r[1] = c.y; r[2] = c.z; r[3] = c.w; r[4] = rr3;
+                r[5] = pc.x; r[6] = pc.y; r[7] = pc.z; r[8] = pc.w;
             }
-            int pos = pn + inc - cnt;
-            if (bits & 1u) pq[pos++] = make_uint2(c.x, c.y);
-            if (bits & 2u) pq[pos++] = make_uint2(c.y, c.z);
-            if (bits & 4u) pq[pos++] = make_uint2(c.z, c.w);
-            if (bits & 8u) pq[pos++] = make_uint2(c.w, rr3);
-            if (bits & 16u) pq[pos++] = make_uint2(pc.x, c.x);
-            if (bits & 32u) pq[pos++] = make_uint2(pc.y, c.y);
-            if (bits & 64u) pq[pos++] = make_uint2(pc.z, c.z);
-            if (bits & 128u) pq[pos++] = make_uint2(pc.w, c.w);
-            pn += __shfl_sync(full, inc, 31);
+            mn += __popc(mm);
             __syncwarp();
-            drain_pairs(false);
+            if (mn >= 32) process_multi(32);
         }
     };
 
     if (xbase < L && ybeg < L) {                   // warp-uniform
         const bool active = x0 < L;                // L % 4 == 0: a lane's 4 columns are all in or all out
         const bool halo = active && (lane == 31 || x0 + 4 >= L);   // right neighbour not in the next lane
-        const int32_t xh = x0 + 4 >= L ? 0 : x0 + 4;
-        auto load4 = [&](int32_t y) {
-            return active ? __ldcs(reinterpret_cast<const int4*>(labels + (int64_t)y * L + x0)) : make_int4(0, 0, 0, 0);
-        };
-        auto loadh = [&](int32_t y) { return halo ? __ldg(labels + (int64_t)y * L + xh) : 0; };
-        int4 pc = load4(ybeg == 0 ? L - 1 : ybeg - 1);          // the row above the strip (wrapped)
-        int32_t prr3 = 0;
-        uint32_t force = 1;                                     // first row: nothing may be skipped
-        int4 n0 = load4(ybeg), n1 = ybeg + 1 < yend ? load4(ybeg + 1) : n0;
-        int32_t h0 = loadh(ybeg), h1 = ybeg + 1 < yend ? loadh(ybeg + 1) : 0;
-#pragma unroll 4
-        for (int32_t y = ybeg; y < yend; ++y) {
-            const int4 c = n0;
-            const int32_t hc = h0;
-            n0 = n1; h0 = h1;
-            if (y + 2 < yend) { n1 = load4(y + 2); h1 = loadh(y + 2); }
-            const int32_t nb = __shfl_down_sync(full, c.x, 1);
-            const int32_t rr3 = halo ? hc : nb;
-            const uint32_t dh = (c.x ^ c.y) | (c.y ^ c.z) | (c.z ^ c.w) | (c.w ^ rr3);
-            const uint32_t dv = (pc.x ^ c.x) | (pc.y ^ c.y) | (pc.z ^ c.z) | (pc.w ^ c.w);
-            const uint32_t e = (uint32_t)(rr3 ^ prr3) | force;
-            // identical to the row above (dv == 0, e == 0): same horizontal pairs, no vertical ones
-            const bool dirty = active && (dv != 0 || (dh != 0 && e != 0));
-            const unsigned m = __ballot_sync(full, dirty);
-            if (m) {
-                if (dirty) {
-                    Rec& r = rq[rn + __popc(m & lt)];
-                    r.c = c; r.pc = pc; r.rr3 = rr3;
+        const uint32_t amask = active ? 0xffffffffu : 0u;
+        // inactive lanes (ragged last strip) read a valid address and never report anything
+        const uint32_t col = active ? x0 : xbase;
+        const uint32_t colh = halo ? (x0 + 4 >= L ? 0 : x0 + 4) : xbase;
+        const int32_t* __restrict__ p = labels + (int64_t)ybeg * L + col;      // load cursors: main, halo
+        const int32_t* __restrict__ ph = labels + (int64_t)ybeg * L + colh;
+        int4 pc;
+        int32_t prr3;
+        {
+            const int32_t* __restrict__ up = labels + (int64_t)(ybeg == 0 ? L - 1 : ybeg - 1) * L;   // wrapped
+            pc = __ldg(reinterpret_cast<const int4*>(up + col));
+            const int32_t hup = __ldg(up + colh);
+            const int32_t nb = __shfl_down_sync(full, pc.x, 1);
+            prr3 = halo ? hup : nb;
+        }
+        uint32_t force = ybeg == 0 ? 1u : 0u;      // row 0 ends every chain: nothing is skipped there
+        // The load cursor stops on the strip's last row: a ragged strip re-reads it, and a repeated
+        // row equals the row above it, so it is never dirty.  Every strip runs kStripRows rows.
+        int32_t ahead = yend - ybeg - 1;           // rows below the cursor
+        int4 buf[kPf];
+        int32_t hb[kPf];
+#pragma unroll
+        for (int j = 0; j < kPf; ++j) {
+            buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
+            hb[j] = __ldg(ph);
+            const int32_t step = ahead > 0 ? L : 0;
+            p += step; ph += step;
+            --ahead;
+        }
+#pragma unroll 1
+        for (int it = 0; it < kStripRows / kPf; ++it) {
+#pragma unroll
+            for (int j = 0; j < kPf; ++j) {
+                const int4 c = buf[j];
+                const int32_t hc = hb[j];
+                buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
+                hb[j] = __ldg(ph);
+                const int32_t step = ahead > 0 ? L : 0;
+                p += step; ph += step;
+                --ahead;
+                const int32_t nb = __shfl_down_sync(full, c.x, 1);
+                const int32_t rr3 = halo ? hc : nb;
+                const uint32_t dh = (c.x ^ c.y) | (c.y ^ c.z) | (c.z ^ c.w) | (c.w ^ rr3);
+                const uint32_t dv = (pc.x ^ c.x) | (pc.y ^ c.y) | (pc.z ^ c.z) | (pc.w ^ c.w);
+                uint32_t any = (dv | dh) & amask;
+                // dv5 == 0: identical to the row above over the 5 columns -> skipped (see above)
+                uint32_t dv5 = dv | (uint32_t)(rr3 ^ prr3) | force;
+                asm volatile("" : "+r"(any), "+r"(dv5));     // keep the OR-of-XOR form (LOP3)
+                const bool dirty = (any != 0) & (dv5 != 0);
+                const unsigned m = __ballot_sync(full, dirty);
+                if (m) {
+                    if (dirty) {
+                        const int pos = rn + __popc(m & lt);
+                        rq.c[pos] = c; rq.pc[pos] = pc; rq.rr3[pos] = rr3;
+                    }
+                    rn += __popc(m);
                 }
-                rn += __popc(m);
-                __syncwarp();
-                if (rn >= 32) process_recs(32);
+                pc = c; prr3 = rr3; force = 0;
+                if (j & 1) {                       // every second row: at most 31 + 64 records queued
+                    __syncwarp();
+                    while (rn >= 32) process_recs(32);
+                }
             }
-            pc = c; prr3 = rr3; force = 0;
         }
         if (rn > 0) process_recs(rn);
-        drain_pairs(true);
+        if (mn > 0) process_multi(mn);
     }
     __syncthreads();
     hash_flush(sh.table, rs, sh.scan);
