@@ -115,7 +115,7 @@ constexpr int kStrWarpsX = 2, kStrWarpsY = 4;
 constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
 constexpr int kStrThreads = 32 * kStrWarps;                     // 256
 constexpr int kStripCols = 128;
-constexpr int kStripRows = 32;                                  // rows per warp
+constexpr int kStripRows = 64;                                  // rows per warp
 constexpr int kPf = 4;                                          // rows in flight per lane
 constexpr int kRecCap = 96;                                     // < 32 pending + 2 rows x 32
 constexpr int kMultiCap = 64;                                   // < 32 pending + 32 per batch
