@@ -668,16 +668,18 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
     const int32_t total = __shfl_sync(full, inc, 31);
     if (total > kCtaCapSites) return 0;
     const int32_t exc = inc - cnt;
-    const int32_t i = 32 * wid + lane;                 // this thread's item
-    int32_t seg = 0;
-    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= i);
-    const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
-    if (i < total) {
-        const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
-        int32_t rx = s.x - cxm, ry = s.y - cym;
-        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
-        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
-        sh.sx[i] = rx; sh.sy[i] = ry; sh.si[i] = s.z;
+    if (32 * wid < total) {                            // warp-uniform: this warp owns items [32 wid, 32 wid + 32)
+        const int32_t i = 32 * wid + lane;             // this thread's item
+        int32_t seg = 0;
+        for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= i);
+        const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
+        if (i < total) {
+            const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
+            int32_t rx = s.x - cxm, ry = s.y - cym;
+            rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
+            ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+            sh.sx[i] = rx; sh.sy[i] = ry; sh.si[i] = s.z;
+        }
     }
     return total;
 }
