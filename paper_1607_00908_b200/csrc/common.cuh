@@ -52,8 +52,9 @@ struct vor_ctx {
     int32_t* d_scan_part;      // scratch for device scans
 
     // ---- edges (a3/a4)
-    uint32_t* d_rows;          // [max_sites * kRowStride] per-site sets of larger-index neighbours;
-                               //   all kEmptySlot between calls (the finish kernel restores that)
+    uint32_t* d_rows;          // [max_sites * kRowStride] per-site lists of larger-index neighbours
+    uint32_t* d_row_cnt;       // [max_sites] entries appended to each row; all 0 between calls (the
+                               //   finish kernel restores that), so stale row contents are never read
     int64_t row_slots;         // slots used per row (option; 4..kRowStride, multiple of 4)
     int64_t edges_generic;     // 1 = force the generic emit kernel (testing)
     uint64_t* d_keys_a;        // [max_raw_keys]  overflow keys / sort ping

@@ -55,6 +55,7 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     ok = ok && dmalloc(&ctx->d_keys_a, (size_t)max_raw_keys) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_keys_b, (size_t)max_raw_keys) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_rows, (size_t)max_sites * kRowStride) == cudaSuccess;
+    ok = ok && dmalloc(&ctx->d_row_cnt, (size_t)max_sites) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_n_raw, 8) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_hist, (size_t)kMaxCoopBlocks * 256) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_blk_count, (size_t)2 * kMaxCoopBlocks) == cudaSuccess;
@@ -75,7 +76,7 @@ int vor_destroy(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
     cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
     cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
-    cudaFree(ctx->d_rows); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
+    cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
     cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts);
     cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
     cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best);
@@ -154,7 +155,7 @@ int vor_sync_status(vor_ctx* ctx, void* stream) {
 
 // All adjacency rows empty (the invariant vor_edges relies on between calls).
 int vor_reset_rows(vor_ctx* ctx) {
-    VOR_CUDA(cudaMemset(ctx->d_rows, 0xff, (size_t)ctx->max_sites * kRowStride * sizeof(uint32_t)));
+    VOR_CUDA(cudaMemset(ctx->d_row_cnt, 0, (size_t)ctx->max_sites * sizeof(uint32_t)));
     return VOR_OK;
 }
 

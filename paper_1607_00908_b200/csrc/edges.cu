@@ -5,15 +5,18 @@
 // BASELINE.json): every 4-connected label discontinuity (right, down, periodic wrap) contributes the
 // pair (min,max), packed as (min << 32 | max); the result is the ascending unique list.
 //
-//   emit    stream the label image once (128-bit loads); every warp compacts the discontinuities of
-//           a row into a shared-memory queue and inserts them 32 at a time into a per-CTA hash set;
-//           at the end the CTA's distinct pairs (a < b) are inserted into row a of a global
-//           adjacency matrix (kRowStride slots per site, exact set insertion with atomicCAS).
-//           Pairs that do not fit (row full, or label >= number of rows) go to an overflow list.
+//   emit    stream the label image once (128-bit loads); every warp compacts the lane-rows that hold a
+//           discontinuity into a shared-memory queue and inserts their pairs, 32 records at a time,
+//           into a per-CTA hash set; the CTA's distinct pairs go to a global raw-key list.
+//   insert  every raw key (a < b) is appended to row a of a global adjacency matrix (kRowStride
+//           slots per site): slot = atomicAdd(row counter), plain store.  A pair seen by several
+//           CTAs is appended several times; pairs that do not fit (row full, or label >= number of
+//           rows) go to an overflow list.
 //   finish  ONE cooperative kernel: [only if the overflow list is not empty: radix-sort it, drop
-//           duplicates and keys already present in their row] -> per-row counts -> grid sync ->
-//           every row is sorted in registers and written at its final position (merged with its
-//           overflow keys, if any); rows are reset to empty on the way.
+//           duplicates and keys already present in their row] -> every row is sorted in registers,
+//           its duplicates dropped, written back and counted -> grid sync -> every row is copied to
+//           its final position (merged with its overflow keys, if any); the row counters are reset
+//           to 0 on the way.
 // The matrix rows are in ascending site order and each row is sorted, so the concatenation IS the
 // globally sorted list: no global sort on the common path.
 #include <cooperative_groups.h>
@@ -28,6 +31,7 @@ constexpr uint64_t kEmptyKey = ~0ull;
 
 struct RowSet {
     uint32_t* rows;            // [n_rows * kRowStride]
+    uint32_t* cnt;             // [n_rows] entries appended to each row (may exceed S: the excess overflowed)
     int32_t n_rows;
     int32_t S;                 // slots used per row
     uint64_t* ovf;             // overflow keys (unordered, may repeat)
@@ -45,23 +49,14 @@ __device__ __forceinline__ void ovf_push(const RowSet& rs, uint32_t a, uint32_t 
     else atomicOr(rs.flags, FLAG_RAWKEY_OVERFLOW);
 }
 
-// Insert b into the set stored in row a (a < b).  Slots fill front to back and never change once
-// set, so a value can never end up in two slots.
-__device__ __noinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b) {
+// Append b to row a (a < b).  The row may receive the same b more than once (from different CTAs):
+// the finish kernel drops the repeats when it sorts the row.
+__device__ __forceinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b) {
     if (a < (uint32_t)rs.n_rows) {
-        uint32_t* row = rs.rows + (size_t)a * kRowStride;
-        for (int q = 0; q < rs.S; q += 4) {
-            const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
-            const uint32_t e[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                uint32_t cur = e[k];
-                if (cur == b) return;
-                if (cur == kEmptySlot) {
-                    cur = atomicCAS(row + q + k, kEmptySlot, b);
-                    if (cur == kEmptySlot || cur == b) return;
-                }
-            }
+        const uint32_t slot = atomicAdd(rs.cnt + a, 1u);
+        if (slot < (uint32_t)rs.S) {
+            rs.rows[(size_t)a * kRowStride + slot] = b;
+            return;
         }
     }
     ovf_push(rs, a, b);
@@ -620,16 +615,15 @@ struct KeepAll {
 // overflow key (a, b) is redundant if row a already holds b
 struct KeepNotInRow {
     const uint32_t* rows;
+    const uint32_t* cnt;
     int32_t n_rows, S;
     __device__ bool operator()(uint64_t key) const {
         const uint32_t a = (uint32_t)(key >> 32), b = (uint32_t)key;
         if (a >= (uint32_t)n_rows) return true;
         const uint32_t* row = rows + (size_t)a * kRowStride;
-        for (int k = 0; k < S; ++k) {
-            const uint32_t v = __ldcg(row + k);
-            if (v == b) return false;
-            if (v == kEmptySlot) break;
-        }
+        const int n = (int)min(__ldcg(cnt + a), (uint32_t)S);
+        for (int k = 0; k < n; ++k)
+            if (__ldcg(row + k) == b) return false;
         return true;
     }
 };
@@ -641,6 +635,21 @@ __device__ __forceinline__ int64_t lower_bound_u64(const uint64_t* __restrict__ 
         if (a[mid] < key) lo = mid + 1; else hi = mid;
     }
     return lo;
+}
+
+// ------------------------------------------------------------------------------------ insert
+// The CTAs' distinct keys (raw list) -> adjacency matrix: exact set insertion, full rows overflow.
+// One atomic on a 4-byte counter (the counters stay in L2) and one fire-and-forget store per key.
+constexpr int kInsertThreads = 256;
+
+__global__ void __launch_bounds__(kInsertThreads) rows_insert_kernel(const RowSet rs) {
+    const unsigned long long have = *rs.n_raw;
+    const int64_t n_raw = (int64_t)have < rs.raw_cap ? (int64_t)have : rs.raw_cap;
+    for (int64_t i = (int64_t)blockIdx.x * kInsertThreads + threadIdx.x; i < n_raw;
+         i += (int64_t)gridDim.x * kInsertThreads) {
+        const uint64_t key = __ldcs(rs.raw + i);
+        row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
+    }
 }
 
 // ------------------------------------------------------------------------------------ finish
@@ -686,17 +695,7 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
     cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 
-    // ---- the CTAs' distinct keys -> adjacency matrix (exact set insertion; full rows overflow)
-    {
-        const int64_t n_raw = __ldcg(&p.ctl[3]) < p.keys_cap ? __ldcg(&p.ctl[3]) : p.keys_cap;
-        for (int64_t i = (int64_t)blockIdx.x * kSortThreads + threadIdx.x; i < n_raw;
-             i += (int64_t)gridDim.x * kSortThreads) {
-            const uint64_t key = __ldcs(p.keys_b + i);
-            row_insert(p.rs, (uint32_t)(key >> 32), (uint32_t)key);
-        }
-    }
-    grid.sync();
-
+    // (the CTAs' distinct keys were inserted into the adjacency matrix by rows_insert_kernel)
     // ---- overflow keys (normally none): sorted, unique, not already in their row
     const uint64_t* ovf = nullptr;
     int64_t n_ovf = __ldcg(p.ctl) < p.keys_cap ? __ldcg(p.ctl) : p.keys_cap;
@@ -712,31 +711,46 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
         const uint64_t mask = (uint64_t)__ldcg(&p.ctl[2]);
         uint64_t* sorted = coop_sort(grid, p.keys_a, p.keys_b, n_ovf, 32, mask, p.hist, sh);
         uint64_t* dst = sorted == p.keys_a ? p.keys_b : p.keys_a;
-        n_ovf = coop_unique(grid, sorted, n_ovf, dst, p.keys_cap, KeepNotInRow{p.rows, p.n_rows, p.S},
+        n_ovf = coop_unique(grid, sorted, n_ovf, dst, p.keys_cap, KeepNotInRow{p.rows, p.rs.cnt, p.n_rows, p.S},
                             p.partial, sh);
         ovf = dst;
     }
 
-    // ---- rows, pass 1: entries per block chunk
+    // ---- rows, pass 1: sort every row in registers, drop repeats, write it back, count
     int64_t rbeg, rend;
     block_chunk(p.n_rows, kSortThreads, &rbeg, &rend);
     {
         int64_t c = 0;
         for (int64_t a = rbeg + threadIdx.x; a < rend; a += kSortThreads) {
-            const uint32_t* row = p.rows + (size_t)a * kRowStride;
-            for (int q = 0; q < p.S; q += 4) {
-                const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
-                const int m = (v.x != kEmptySlot) + (v.y != kEmptySlot) + (v.z != kEmptySlot) + (v.w != kEmptySlot);
-                c += m;
-                if (m < 4) break;
+            const int n = (int)min(__ldcg(p.rs.cnt + a), (uint32_t)p.S);
+            if (n == 0) continue;
+            uint32_t* row = p.rows + (size_t)a * kRowStride;
+            if (n == 1) { c += 1; continue; }              // nothing to sort; the counter is already right
+            uint32_t e[kRowStride];
+#pragma unroll
+            for (int q = 0; q < kRowStride; q += 4) {
+                uint4 v = make_uint4(kEmptySlot, kEmptySlot, kEmptySlot, kEmptySlot);
+                if (q < n) v = __ldcg(reinterpret_cast<const uint4*>(row + q));
+                e[q] = q < n ? v.x : kEmptySlot; e[q + 1] = q + 1 < n ? v.y : kEmptySlot;
+                e[q + 2] = q + 2 < n ? v.z : kEmptySlot; e[q + 3] = q + 3 < n ? v.w : kEmptySlot;
             }
+            if (n > 8) bitonic_sort<16>(e);
+            else if (n > 4) bitonic_sort<8>(e);
+            else bitonic_sort<4>(e);
+            int m = 0;                                      // ascending, repeats adjacent, padding last
+#pragma unroll
+            for (int k = 0; k < kRowStride; ++k) {
+                if (k < n && (k == 0 || e[k] != e[k - 1])) { row[m] = e[k]; ++m; }
+            }
+            p.rs.cnt[a] = (uint32_t)m;
+            c += m;
         }
         c = block_sum_i64(c, sh.red);
         if (threadIdx.x == 0) p.partial[gridDim.x + blockIdx.x] = c;
     }
     grid.sync();
 
-    // ---- rows, pass 2: sort every row in registers and write it at its final position
+    // ---- rows, pass 2: copy every row to its final position; reset the counters
     int64_t before, all;
     partial_prefix(p.partial + gridDim.x, gridDim.x, blockIdx.x, sh.red, &before, &all);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -746,26 +760,10 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
     int64_t run = before;
     for (int64_t base = rbeg; base < rend; base += kSortThreads) {
         const int64_t a = base + threadIdx.x;
-        uint32_t e[kRowStride];
-#pragma unroll
-        for (int k = 0; k < kRowStride; ++k) e[k] = kEmptySlot;
         int n = 0;
         if (a < rend) {
-            uint32_t* row = p.rows + (size_t)a * kRowStride;
-#pragma unroll
-            for (int q = 0; q < kRowStride; q += 4) {
-                if (q < p.S && (q == 0 || e[q - 1] != kEmptySlot)) {
-                    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
-                    e[q] = v.x; e[q + 1] = v.y; e[q + 2] = v.z; e[q + 3] = v.w;
-                    if (v.x != kEmptySlot)            // leave the row empty for the next call
-                        *reinterpret_cast<uint4*>(row + q) = make_uint4(kEmptySlot, kEmptySlot, kEmptySlot, kEmptySlot);
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < kRowStride; ++k) n += e[k] != kEmptySlot;
-            if (n > 8) bitonic_sort<16>(e);
-            else if (n > 4) bitonic_sort<8>(e);
-            else if (n > 1) bitonic_sort<4>(e);
+            n = (int)min(__ldcg(p.rs.cnt + a), (uint32_t)p.S);
+            if (n) p.rs.cnt[a] = 0;                        // leave the row empty for the next call
         }
         // exclusive scan of n over the block
         int inc = n;
@@ -785,7 +783,8 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
         int64_t pos = run + wbase + inc - n;
         run += total;
         __syncthreads();
-        if (a < rend) {
+        if (a < rend && n > 0) {
+            const uint32_t* row = p.rows + (size_t)a * kRowStride;
             const uint64_t hi = (uint64_t)a << 32;
             int64_t o0 = 0, o1 = 0;
             if (n_ovf > 0) {
@@ -795,23 +794,29 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
             }
             if (o1 == o0) {
 #pragma unroll
-                for (int k = 0; k < kRowStride; ++k)
-                    if (k < n && pos + k < p.cap) p.out[pos + k] = hi | e[k];
+                for (int q = 0; q < kRowStride; q += 4) {
+                    if (q < n) {
+                        const uint4 v = __ldcg(reinterpret_cast<const uint4*>(row + q));
+                        const uint32_t e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            if (q + k < n && pos + q + k < p.cap) p.out[pos + q + k] = hi | e[k];
+                    }
+                }
             } else {
                 // rare: merge the row with its overflow keys (disjoint by construction)
-                uint32_t r[kRowStride];
-#pragma unroll
-                for (int k = 0; k < kRowStride; ++k) r[k] = e[k];
                 int i = 0;
                 int64_t j = o0;
                 while (i < n || j < o1) {
                     uint64_t key;
-                    if (j >= o1 || (i < n && (hi | r[i]) < ovf[j])) key = hi | r[i++];
+                    if (j >= o1 || (i < n && (hi | __ldcg(row + i)) < ovf[j])) key = hi | __ldcg(row + i++);
                     else key = ovf[j++];
                     if (pos < p.cap) p.out[pos] = key;
                     ++pos;
                 }
             }
+        } else if (a < rend && n_ovf > 0) {
+            // an empty row can still own overflow keys only if S == 0, which set_option forbids
         }
     }
     // ---- overflow keys whose smaller label has no row come last
@@ -878,6 +883,7 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     const int32_t L = ctx->L;
     RowSet rs;
     rs.rows = ctx->d_rows;
+    rs.cnt = ctx->d_row_cnt;
     rs.n_rows = ctx->n_sites > 0 ? ctx->n_sites : ctx->max_sites;
     rs.S = (int32_t)ctx->row_slots;
     rs.ovf = ctx->d_keys_a;
@@ -901,6 +907,7 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     }
     FinishParams fp{rs, ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
                     ctx->d_n_raw, ctx->d_hist, ctx->d_blk_count, d_edges, cap, d_n_edges, ctx->d_flags};
+    VOR_LAUNCH(rows_insert_kernel, 8 * ctx->num_sms, kInsertThreads, 0, stream, rs);
     const int fgrid = vor_coop_grid(ctx, 0, (const void*)edges_finish_kernel, kSortThreads, 1);
     VOR_LAUNCH_COOP(edges_finish_kernel, fgrid, kSortThreads, stream, (void*)&fp);
     return VOR_OK;
