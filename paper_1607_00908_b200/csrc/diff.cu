@@ -5,10 +5,10 @@
 // D_P only) or "arising" (in D_N only).  Here both sets are ascending unique key
 // lists, so breaking = prev \ now (destroyed) and arising = now \ prev (created) are sorted set
 // differences.  ONE cooperative kernel: half of the blocks take each direction; a block owns a
-// contiguous chunk of its list A, finds for every 1024-key batch the matching window of the other
-// list B (batch boundaries are binary-searched once, in parallel), stages the window in shared
-// memory and searches there; membership bits stay in shared memory across the grid sync that
-// separates counting from the order-preserving write.
+// contiguous chunk of its list A; every thread takes kDiffKeys consecutive keys of A, finds the
+// position of the first one in the other list B with one binary search (the top levels of the search
+// tree stay in L1) and walks B from there.  The per-thread membership masks stay in shared memory
+// across the grid sync that separates counting from the order-preserving write.
 #include <cooperative_groups.h>
 
 #include "common.cuh"
@@ -17,14 +17,13 @@ namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int kDiffThreads = kSortThreads;
-constexpr int kDiffWindow = 3072;          // keys of B staged per batch
-constexpr int kDiffMaxBatches = 128;       // batches per block whose membership bits are cached
+constexpr int kDiffThreads = 512;
+constexpr int kDiffKeys = 8;                       // consecutive keys of A per thread per batch
+constexpr int kDiffBatch = kDiffThreads * kDiffKeys;
+constexpr int kDiffMaxBatches = 48;                // batches per block whose masks are cached
 
 struct DiffShared {
-    uint64_t win[kDiffWindow];
-    uint32_t bits[kDiffMaxBatches][kDiffThreads / 32];
-    int64_t bstart[kDiffMaxBatches + 1];
+    uint8_t mask[kDiffMaxBatches][kDiffThreads];
     int64_t red[32];
     int32_t wtot[kDiffThreads / 32];
 };
@@ -33,7 +32,7 @@ __device__ __forceinline__ int64_t lower_bound(const uint64_t* __restrict__ a, i
                                                uint64_t key) {
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
-        if (a[mid] < key) lo = mid + 1; else hi = mid;
+        if (__ldg(a + mid) < key) lo = mid + 1; else hi = mid;
     }
     return lo;
 }
@@ -51,47 +50,22 @@ __device__ __forceinline__ int64_t block_sum(int64_t v, int64_t* sh) {
     return t;
 }
 
-// bstart[k] = lower_bound(B, first key of batch k) for the batches [g0, g0 + nb) of this block's
-// chunk; bstart[nb] closes the last window.
-__device__ __forceinline__ void batch_windows(const uint64_t* __restrict__ A, int64_t beg, int64_t nA,
-                                              const uint64_t* __restrict__ B, int64_t nB, int64_t g0,
-                                              int nb, DiffShared& sh) {
-    for (int k = threadIdx.x; k <= nb; k += kDiffThreads) {
-        const int64_t i = beg + (g0 + k) * kDiffThreads;
-        // the window of batch k must hold every B key <= the batch's last key: close it with the
-        // first key of the next batch (keys are unique, so B keys equal to batch keys lie before it)
-        sh.bstart[k] = i < nA ? lower_bound(B, 0, nB, A[i]) : nB;
-    }
-    __syncthreads();
-}
-
-// Is A[i] absent from B?  One batch of kDiffThreads keys; B window [w0, w1).
-__device__ __forceinline__ bool batch_absent(const uint64_t* __restrict__ A, int64_t i, int64_t end,
-                                             const uint64_t* __restrict__ B, int64_t w0, int64_t w1,
-                                             DiffShared& sh, uint64_t* key_out) {
-    const int64_t wn = w1 - w0;
-    const bool staged = wn <= kDiffWindow;
-    if (staged)
-        for (int64_t k = threadIdx.x; k < wn; k += kDiffThreads) sh.win[k] = B[w0 + k];
-    __syncthreads();
-    bool absent = false;
-    if (i < end) {
-        const uint64_t key = A[i];
-        *key_out = key;
-        if (staged) {
-            int lo = 0, hi = (int)wn;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (sh.win[mid] < key) lo = mid + 1; else hi = mid;
-            }
-            absent = !(lo < (int)wn && sh.win[lo] == key);
-        } else {
-            const int64_t lo = lower_bound(B, w0, w1, key);
-            absent = !(lo < w1 && B[lo] == key);
+// Bit k of the result: A[i0 + k] (i0 + k < end) is absent from B.
+__device__ __forceinline__ uint32_t absent_mask(const uint64_t* __restrict__ A, int64_t i0, int64_t end,
+                                                const uint64_t* __restrict__ B, int64_t nB) {
+    if (i0 >= end) return 0u;
+    uint32_t m = 0;
+    int64_t j = lower_bound(B, 0, nB, __ldg(A + i0));
+    uint64_t bj = j < nB ? __ldg(B + j) : ~0ull;       // ~0 is never a key (i < j < 2^32)
+#pragma unroll
+    for (int k = 0; k < kDiffKeys; ++k) {
+        if (i0 + k < end) {
+            const uint64_t key = __ldg(A + i0 + k);
+            while (bj < key) { ++j; bj = j < nB ? __ldg(B + j) : ~0ull; }
+            m |= (uint32_t)(bj != key) << k;
         }
     }
-    __syncthreads();
-    return absent;
+    return m;
 }
 
 struct DiffParams {
@@ -104,7 +78,7 @@ struct DiffParams {
 };
 
 // grid = 2 * nb blocks: blocks [0, nb) handle created = now \ prev, [nb, 2nb) destroyed = prev \ now
-__global__ void __launch_bounds__(kDiffThreads) diff_kernel(const DiffParams p) {
+__global__ void __launch_bounds__(kDiffThreads, 3) diff_kernel(const DiffParams p) {
     __shared__ DiffShared sh;
     cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -116,26 +90,17 @@ __global__ void __launch_bounds__(kDiffThreads) diff_kernel(const DiffParams p) 
     const int64_t nA = second ? *p.n_prev : *p.n_now, nB = second ? *p.n_now : *p.n_prev;
     uint64_t* __restrict__ out = second ? p.destroyed : p.created;
     int64_t C = (nA + nb - 1) / nb;
-    C = (C + kDiffThreads - 1) / kDiffThreads * kDiffThreads;
+    C = (C + 32 * kDiffKeys - 1) / (32 * kDiffKeys) * (32 * kDiffKeys);    // whole warps of full threads
     const int64_t beg = (int64_t)me * C < nA ? (int64_t)me * C : nA;
     const int64_t end = beg + C < nA ? beg + C : nA;
-    const int64_t nbatch = (end - beg + kDiffThreads - 1) / kDiffThreads;
-    const bool cached = nbatch <= kDiffMaxBatches;
+    const int64_t nbatch = (end - beg + kDiffBatch - 1) / kDiffBatch;
 
     // ---- pass 1: membership + count
     int64_t c = 0;
-    for (int64_t g0 = 0; g0 < nbatch; g0 += kDiffMaxBatches) {
-        const int gb = (int)(nbatch - g0 < kDiffMaxBatches ? nbatch - g0 : kDiffMaxBatches);
-        batch_windows(A, beg, nA, B, nB, g0, gb, sh);
-        for (int k = 0; k < gb; ++k) {
-            uint64_t key;
-            const bool absent = batch_absent(A, beg + (g0 + k) * kDiffThreads + threadIdx.x, end, B,
-                                             sh.bstart[k], sh.bstart[k + 1], sh, &key);
-            const unsigned ball = __ballot_sync(0xffffffffu, absent);
-            if (cached && lane == 0) sh.bits[k][wid] = ball;
-            c += absent;
-        }
-        __syncthreads();
+    for (int64_t k = 0; k < nbatch; ++k) {
+        const uint32_t m = absent_mask(A, beg + k * kDiffBatch + (int64_t)threadIdx.x * kDiffKeys, end, B, nB);
+        if (k < kDiffMaxBatches) sh.mask[k][threadIdx.x] = (uint8_t)m;
+        c += __popc(m);
     }
     c = block_sum(c, sh.red);
     if (threadIdx.x == 0) p.partial[blockIdx.x] = c;
@@ -155,35 +120,35 @@ __global__ void __launch_bounds__(kDiffThreads) diff_kernel(const DiffParams p) 
         if (all > p.cap) atomicOr(p.flags, FLAG_DIFF_CAP);
     }
     int64_t run = before;
-    for (int64_t g0 = 0; g0 < nbatch; g0 += kDiffMaxBatches) {
-        const int gb = (int)(nbatch - g0 < kDiffMaxBatches ? nbatch - g0 : kDiffMaxBatches);
-        if (!cached) batch_windows(A, beg, nA, B, nB, g0, gb, sh);
-        for (int k = 0; k < gb; ++k) {
-            const int64_t i = beg + (g0 + k) * kDiffThreads + threadIdx.x;
-            uint64_t key = 0;
-            unsigned ball;
-            if (cached) {
-                ball = sh.bits[k][wid];
-                if (ball >> lane & 1) key = A[i];
-            } else {
-                const bool absent = batch_absent(A, i, end, B, sh.bstart[k], sh.bstart[k + 1], sh, &key);
-                ball = __ballot_sync(0xffffffffu, absent);
-            }
-            if (lane == 0) sh.wtot[wid] = __popc(ball);
-            __syncthreads();
-            int32_t wbase = 0, total = 0;
-            for (int w = 0; w < kDiffThreads / 32; ++w) {
-                const int32_t t = sh.wtot[w];
-                if (w < wid) wbase += t;
-                total += t;
-            }
-            if (ball >> lane & 1) {
-                const int64_t pos = run + wbase + __popc(ball & ((1u << lane) - 1u));
-                if (pos < p.cap) out[pos] = key;
-            }
-            run += total;
-            __syncthreads();
+    for (int64_t k = 0; k < nbatch; ++k) {
+        const int64_t i0 = beg + k * kDiffBatch + (int64_t)threadIdx.x * kDiffKeys;
+        const uint32_t m = k < kDiffMaxBatches ? (uint32_t)sh.mask[k][threadIdx.x] : absent_mask(A, i0, end, B, nB);
+        const int n = __popc(m);
+        int inc = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
         }
+        if (lane == 31) sh.wtot[wid] = inc;
+        __syncthreads();
+        int32_t wbase = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kDiffThreads / 32; ++w) {
+            const int32_t t = sh.wtot[w];
+            if (w < wid) wbase += t;
+            total += t;
+        }
+        int64_t pos = run + wbase + inc - n;
+#pragma unroll
+        for (int q = 0; q < kDiffKeys; ++q) {
+            if (m >> q & 1u) {
+                if (pos < p.cap) out[pos] = __ldg(A + i0 + q);
+                ++pos;
+            }
+        }
+        run += total;
+        __syncthreads();
     }
 }
 
@@ -276,7 +241,7 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
     }
     DiffParams dp{P, nP, N, nN, d_created, d_destroyed, cap, d_n_created, d_n_destroyed,
                   ctx->d_blk_count, ctx->d_flags};
-    int grid = vor_coop_grid(ctx, 2, (const void*)diff_kernel, kDiffThreads, 1);
+    int grid = vor_coop_grid(ctx, 2, (const void*)diff_kernel, kDiffThreads, 3);
     grid &= ~1;                                         // one half per direction
     if (grid < 2) return vor_fail(ctx, VOR_ECUDA, "vor_diff: device too small for the cooperative grid");
     VOR_LAUNCH_COOP(diff_kernel, grid, kDiffThreads, stream, (void*)&dp);
