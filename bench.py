@@ -25,6 +25,19 @@ sys.path.insert(0, ROOT)
 
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
+# Algorithmic integer work of exact labelling per lattice cell: 7 candidate sites (a
+# Voronoi region has 6 neighbours on average, plus the owner) x 3 ops (two multiply-adds of the
+# distance expansion, one min) + 1 store.
+LABEL_OPS_PER_CELL = 22
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r1c_full_summary.md); config 5 only.
+NCU_TRAFFIC_BYTES = {}
+
+
+def edges_bytes(cells, n_edges):
+    return 4.0 * cells + 8.0 * n_edges
+
+
 METRIC = "lattice cells/s labelled+edge-extracted+diffed (frames/s = value / L^2)"
 UNIT = "cells/s"
 
@@ -48,6 +61,30 @@ def get_workload(name: str):
         base, L = name.split("@")
         return W.scaled(int(base[3:]), int(L))
     return W.config(int(name[3:]))
+
+
+# ---- multi-rank host logic (exercised on CPU with gloo by tests/test_bench_ranks.py)
+def rank_workload(w, rank: int):
+    """Weak scaling: every rank processes its own independent, seeded frame sequence of the same
+    configuration (no data-path collective)."""
+    import dataclasses
+    return dataclasses.replace(w, seed=w.seed + 1000 * rank)
+
+
+def reduce_max(x: float, world: int, device) -> float:
+    """Max over ranks of a per-rank duration (the job is as slow as its slowest rank)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, cells_per_step: int, ms_total: float) -> float:
+    """Cells all ranks processed / the slowest rank's time."""
+    return world * steps * cells_per_step / (ms_total * 1e-3)
 
 
 def peaks():
@@ -169,15 +206,9 @@ def run_ours(args, w):
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_max(x, world, "cuda")
 
-    # weak scaling: every rank processes its own independent frame sequence (no data-path collective)
-    import dataclasses
-    wr = dataclasses.replace(w, seed=w.seed + 1000 * rank)
+    wr = rank_workload(w, rank)
     W_, K = args.warmup, args.steps
     frames = list(wr.frames(W_ + K))
     L, n = wr.L, wr.n_sites
@@ -232,26 +263,47 @@ def run_ours(args, w):
     counts = {"n_edges": int(n_edges[(W_ + K - 1) & 1].item()), "n_created": int(n_c.item()),
               "n_destroyed": int(n_d.item())}
     cells_per_step = L * L
-    value = world * K * cells_per_step / (ms_total * 1e-3)
+    value = whole_job_value(world, K, cells_per_step, ms_total)
+
+    # ---- per-kernel durations: the same K frames again with the library's per-launch CUDA events
+    # (recorded on the launching stream); outside the timed region so they cannot perturb `value`
+    v.vor_profile_begin()
+    for k in range(K):
+        step(W_ + k)
+    prof = v.vor_profile_end()
+    per_kernel = {}
+    for nm, ms in prof:
+        per_kernel.setdefault(nm, []).append(ms)
+    kernel_launch_ms = {nm: float(np.mean(x)) for nm, x in per_kernel.items()}
+    kernel_launches_per_step = {nm: len(x) / K for nm, x in per_kernel.items()}
 
     # ---- e2e: the same frames through vor_frame_host (host buffers, H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
-        hc = np.empty(cap_e, np.uint64); hd = np.empty(cap_e, np.uint64); cnt = np.zeros(3, np.int64)
+        # page-locked host buffers (the user's side of the API): inputs are DMA'd straight from them
+        def pinned(shape, dtype):
+            return torch.empty(shape, dtype=dtype, pin_memory=True).numpy()
+        hc = pinned(cap_e, torch.int64).view(np.uint64); hd = pinned(cap_e, torch.int64).view(np.uint64)
+        cnt = np.zeros(3, np.int64)
+        hframes = []
+        for sx, sy in frames:
+            px, py = pinned(n, torch.int32), pinned(n, torch.int32)
+            px[:] = sx; py[:] = sy
+            hframes.append((px, py))
         v.vor_frame_reset()
         for i in range(W_):
-            v.vor_frame_host(frames[i][0], frames[i][1], hc, hd, cnt)
+            v.vor_frame_host(hframes[i][0], hframes[i][1], hc, hd, cnt)
         barrier()
         d2h = 0
         t0 = time.perf_counter()
         for k in range(K):
-            v.vor_frame_host(frames[W_ + k][0], frames[W_ + k][1], hc, hd, cnt)
+            v.vor_frame_host(hframes[W_ + k][0], hframes[W_ + k][1], hc, hd, cnt)
             d2h += 8 * (int(cnt[1]) + int(cnt[2])) + 24
         torch.cuda.synchronize()
         secs = max_over_ranks(time.perf_counter() - t0)
         e2e = {"value": world * K * cells_per_step / secs, "unit": UNIT, "ms_per_step": 1e3 * secs / K,
                "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": d2h // K,
-               "api": "vor_frame_host (C ABI, host buffers; label image stays on the device)"}
+               "api": "vor_frame_host (C ABI, pinned host buffers; label image stays on the device)"}
 
     if rank != 0:
         if world > 1:
@@ -259,15 +311,42 @@ def run_ours(args, w):
         return
 
     hbm_peak, peak_src, sm_max_mhz = peaks()
-    # dominant kernel = vor_label (one launch per step).  Algorithmic HBM bytes: 4 B/cell written
-    # (SURVEY.md §8d); sites are L2-served.  It is ALU/issue-bound, so the HBM fraction is a floor view.
-    label_s = kernel_ms["label"] * 1e-3
-    label_bytes = 4.0 * cells_per_step
-    roofline = {"kernel": "label_tile_kernel", "bound": "hbm", "achieved": label_bytes / label_s / 1e9,
-                "peak": hbm_peak, "unit": "GB/s", "frac": label_bytes / label_s / 1e9 / hbm_peak,
-                "traffic": None, "peak_source": peak_src,
-                "note": "ALU/issue-bound kernel; algorithmic bytes = 4 B/cell label write"}
-    edges_bytes = 4.0 * cells_per_step
+    # Dominant kernel = label_cta_kernel (one launch per step).  It is bound by plain
+    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.6
+    # derives (SMs x 128 lanes x max SM clock); algorithmic work = 22 integer ops per cell.
+    lab_name = max((nm for nm in kernel_launch_ms if "label" in nm), key=lambda nm: kernel_launch_ms[nm])
+    label_s = kernel_launch_ms[lab_name] * 1e-3
+    alu_peak = 148 * 128 * sm_max_mhz * 1e6 / 1e12            # Tera int32 lane-ops / s
+    alu_ops = LABEL_OPS_PER_CELL * cells_per_step
+    roofline = {"kernel": lab_name, "bound": "alu", "achieved": alu_ops / label_s / 1e12, "peak": alu_peak,
+                "unit": "Tera int32 op/s", "frac": alu_ops / label_s / 1e12 / alu_peak,
+                "traffic": NCU_TRAFFIC_BYTES.get(lab_name),
+                "launch_ms": kernel_launch_ms[lab_name],
+                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.6)",
+                "algorithmic": f"{LABEL_OPS_PER_CELL} int32 ops/cell x {cells_per_step} cells",
+                "hbm_view": {"achieved": 4.0 * cells_per_step / label_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": 4.0 * cells_per_step / label_s / 1e9 / hbm_peak,
+                             "algorithmic": "4 B/cell label write", "peak_source": peak_src}}
+
+    def hbm_roof(name, nbytes, what):
+        if name not in kernel_launch_ms:
+            return None
+        sec = kernel_launch_ms[name] * 1e-3
+        return {"bound": "hbm", "achieved": nbytes / sec / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": nbytes / sec / 1e9 / hbm_peak, "launch_ms": kernel_launch_ms[name],
+                "traffic": NCU_TRAFFIC_BYTES.get(name), "algorithmic": what, "peak_source": peak_src}
+
+    ne = counts["n_edges"]
+    others = {
+        "edges_stream_kernel": hbm_roof("edges_stream_kernel", 4.0 * cells_per_step, "4 B/cell label read"),
+        "diff_kernel": hbm_roof("diff_kernel", 16.0 * ne + 8.0 * (counts["n_created"] + counts["n_destroyed"]),
+                                "8 B x (E_prev + E_now) read + 8 B x (created + destroyed) written; L2-resident"),
+        "vor_edges (stream + insert + finish)": {
+            "bound": "hbm", "achieved": edges_bytes(cells_per_step, ne) / (kernel_ms["edges"] * 1e-3) / 1e9,
+            "peak": hbm_peak, "unit": "GB/s",
+            "frac": edges_bytes(cells_per_step, ne) / (kernel_ms["edges"] * 1e-3) / 1e9 / hbm_peak,
+            "algorithmic": "4 B/cell label read + 8 B/edge written"},
+    }
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -277,14 +356,9 @@ def run_ours(args, w):
                    "l2_policy": "working set per step (1 GiB label image written then read) exceeds the 126 MB L2"},
         "frames_per_s": world * K / (ms_total * 1e-3),
         "kernel_ms": kernel_ms, "counts": counts,
+        "kernel_launch_ms": kernel_launch_ms, "kernel_launches_per_step": kernel_launches_per_step,
         "roofline": roofline,
-        "rooflines_other": {
-            "edges(emit+sort+unique)": {"bound": "hbm", "achieved": edges_bytes / (kernel_ms["edges"] * 1e-3) / 1e9,
-                                        "peak": hbm_peak, "unit": "GB/s",
-                                        "frac": edges_bytes / (kernel_ms["edges"] * 1e-3) / 1e9 / hbm_peak},
-            "diff": {"bound": "hbm", "achieved": 16.0 * counts["n_edges"] / (kernel_ms["diff"] * 1e-3) / 1e9,
-                     "peak": hbm_peak, "unit": "GB/s",
-                     "frac": 16.0 * counts["n_edges"] / (kernel_ms["diff"] * 1e-3) / 1e9 / hbm_peak}},
+        "rooflines_other": {k: r for k, r in others.items() if r},
         "clocks": clocks, "gpu_launches": int(launches),
     }
     if e2e:

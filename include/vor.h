@@ -59,6 +59,14 @@ int vor_sync_status(vor_ctx* ctx, void* stream);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t vor_launch_count(const vor_ctx* ctx);
 
+/* Per-kernel timing for bench.py's roofline figures.  vor_profile_begin() arms the context: every
+ * kernel the library launches afterwards (at most 256) is bracketed by CUDA events on its own stream.
+ * vor_profile_end() disarms it, synchronises `stream`, and returns the number n of launches timed
+ * (or a negative vor_status): ms[i] = duration of launch i, names = their kernel names separated by
+ * '\n' (truncated to names_len bytes; n is reduced accordingly).  Launch order is preserved. */
+int vor_profile_begin(vor_ctx* ctx);
+int vor_profile_end(vor_ctx* ctx, void* stream, char* names, int32_t names_len, float* ms, int32_t cap);
+
 /* Tuning knobs (integers).  Unknown names -> VOR_EINVAL.
  *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 25)
  *   "row_slots"              adjacency-matrix slots used per site in vor_edges: 4, 8, 12 or 16

@@ -27,6 +27,8 @@ SIGNATURES = {
     "vor_sync_status": (C.c_int, [_P, _P]),
     "vor_launch_count": (C.c_int64, [_P]),
     "vor_set_option": (C.c_int, [_P, C.c_char_p, C.c_int64]),
+    "vor_profile_begin": (C.c_int, [_P]),
+    "vor_profile_end": (C.c_int, [_P, _P, C.c_char_p, C.c_int32, C.POINTER(C.c_float), C.c_int32]),
     "vor_build_cells": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
     "vor_label": (C.c_int, [_P, _P, _P]),
     "vor_edges": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P]),
@@ -119,6 +121,19 @@ class Vor:
 
     def vor_launch_count(self) -> int:
         return int(self.lib.vor_launch_count(self.h))
+
+    def vor_profile_begin(self):
+        self._check(self.lib.vor_profile_begin(self.h))
+
+    def vor_profile_end(self):
+        """-> list of (kernel name, milliseconds) for every launch since vor_profile_begin()."""
+        cap = 256
+        names = C.create_string_buffer(64 * cap)
+        ms = (C.c_float * cap)()
+        n = self.lib.vor_profile_end(self.h, _stream(), names, len(names), ms, cap)
+        if n < 0:
+            self._check(n)
+        return list(zip(names.value.decode().split("\n")[:n], [float(ms[i]) for i in range(n)]))
 
     def vor_set_option(self, name: str, value: int):
         self._check(self.lib.vor_set_option(self.h, name.encode(), int(value)))

@@ -17,6 +17,7 @@ constexpr int kSortThreads = 1024;         // block size of the persistent coope
 constexpr int kMaxCoopBlocks = 1024;       // allocation bound for per-block scratch of those kernels
 constexpr int kRowStride = 16;             // adjacency-row slots per site (64-byte rows)
 constexpr uint32_t kEmptySlot = 0xffffffffu;
+constexpr int kMaxProfLaunches = 256;      // launches timed per vor_profile_begin/end bracket
 
 // error flag bits latched on the device (ctx->d_flags[0])
 enum : int {
@@ -98,8 +99,19 @@ struct vor_ctx {
     int num_sms;               // of the device the context lives on
     int coop_blocks[4];        // cached grid sizes of the cooperative kernels (0 = not yet queried)
     int64_t launches;
+    // per-launch timing (vor_profile_begin / vor_profile_end): events around every kernel launch
+    int prof_on;
+    int prof_n;
+    cudaEvent_t prof_ev[kMaxProfLaunches][2];
+    const char* prof_name[kMaxProfLaunches];
     char err[512];
 };
+
+inline void vor_prof_mark(vor_ctx* ctx, int which, const char* name, cudaStream_t stream) {
+    if (!ctx->prof_on || ctx->prof_n >= kMaxProfLaunches) return;
+    cudaEventRecord(ctx->prof_ev[ctx->prof_n][which], stream);
+    if (which == 1) ctx->prof_name[ctx->prof_n++] = name;
+}
 
 inline int vor_fail(vor_ctx* ctx, int code, const char* what) {
     if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s", what);
@@ -134,8 +146,10 @@ inline int vor_coop_grid(vor_ctx* ctx, int slot, const void* func, int threads, 
 #define VOR_LAUNCH_COOP(kernel, grid, block, stream, ...)                                         \
     do {                                                                                           \
         void* args_[] = {__VA_ARGS__};                                                             \
+        vor_prof_mark(ctx, 0, #kernel, (stream));                                                  \
         cudaError_t e_ = cudaLaunchCooperativeKernel((const void*)kernel, dim3(grid), dim3(block), \
                                                      args_, 0, (stream));                          \
+        vor_prof_mark(ctx, 1, #kernel, (stream));                                                  \
         ctx->launches++;                                                                           \
         if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #kernel);                             \
     } while (0)
@@ -143,7 +157,9 @@ inline int vor_coop_grid(vor_ctx* ctx, int slot, const void* func, int threads, 
 // launch + count + check
 #define VOR_LAUNCH(kernel, grid, block, smem, stream, ...)                      \
     do {                                                                        \
+        vor_prof_mark(ctx, 0, #kernel, (stream));                               \
         kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);             \
+        vor_prof_mark(ctx, 1, #kernel, (stream));                               \
         ctx->launches++;                                                        \
         cudaError_t e_ = cudaGetLastError();                                    \
         if (e_ != cudaSuccess) return vor_cuda_fail(ctx, e_, #kernel);          \

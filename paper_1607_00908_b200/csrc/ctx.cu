@@ -86,6 +86,9 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_fr_created); cudaFree(ctx->d_fr_destroyed); cudaFree(ctx->d_fr_counts);
     cudaFreeHost(ctx->h_fr_counts); cudaFreeHost(ctx->h_fr_sites); cudaFreeHost(ctx->h_fr_lists);
     cudaFree(ctx->d_flags);
+    if (ctx->prof_ev[0][0])
+        for (int i = 0; i < kMaxProfLaunches; ++i)
+            for (int k = 0; k < 2; ++k) cudaEventDestroy(ctx->prof_ev[i][k]);
     free(ctx);
     return VOR_OK;
 }
@@ -93,6 +96,35 @@ int vor_destroy(vor_ctx* ctx) {
 const char* vor_last_error(const vor_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
 int64_t vor_launch_count(const vor_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int vor_profile_begin(vor_ctx* ctx) {
+    if (!ctx) return VOR_EINVAL;
+    if (!ctx->prof_ev[0][0])
+        for (int i = 0; i < kMaxProfLaunches; ++i)
+            for (int k = 0; k < 2; ++k) VOR_CUDA(cudaEventCreate(&ctx->prof_ev[i][k]));
+    ctx->prof_n = 0;
+    ctx->prof_on = 1;
+    return VOR_OK;
+}
+
+int vor_profile_end(vor_ctx* ctx, void* stream, char* names, int32_t names_len, float* ms, int32_t cap) {
+    if (!ctx || !names || !ms || names_len < 1 || cap < 0) return VOR_EINVAL;
+    ctx->prof_on = 0;
+    VOR_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    int n = ctx->prof_n < cap ? ctx->prof_n : cap;
+    int used = 0;
+    names[0] = 0;
+    for (int i = 0; i < n; ++i) {
+        VOR_CUDA(cudaEventElapsedTime(&ms[i], ctx->prof_ev[i][0], ctx->prof_ev[i][1]));
+        const int len = (int)strlen(ctx->prof_name[i]);
+        if (used + len + 2 > names_len) { n = i; break; }
+        memcpy(names + used, ctx->prof_name[i], len);
+        names[used + len] = '\n';
+        used += len + 1;
+        names[used] = 0;
+    }
+    return n;
+}
 
 int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
     if (!ctx || !name) return VOR_EINVAL;

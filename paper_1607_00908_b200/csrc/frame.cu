@@ -10,6 +10,14 @@ __global__ void gather_counts_kernel(const int64_t* __restrict__ n_edges, const 
     out[0] = *n_edges; out[1] = *n_created; out[2] = *n_destroyed;
 }
 
+// Page-locked host memory (cudaMallocHost / cudaHostRegister / torch pin_memory) can be the source or
+// target of a true asynchronous DMA; anything else is staged through the context's pinned buffers.
+bool is_pinned(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost;
+}
+
 int ensure_frame_buffers(vor_ctx* ctx) {
     if (ctx->d_fr_labels) return VOR_OK;
     const size_t cells = (size_t)ctx->L * ctx->L;
@@ -75,13 +83,18 @@ extern "C" int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* 
     int rc = ensure_frame_buffers(ctx);
     if (rc != VOR_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
-    // stage through pinned memory so the copies are true async DMA whatever the caller's buffers are
-    memcpy(ctx->h_fr_sites, h_sx, (size_t)n_sites * sizeof(int32_t));
-    memcpy(ctx->h_fr_sites + ctx->max_sites, h_sy, (size_t)n_sites * sizeof(int32_t));
-    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sx, ctx->h_fr_sites, (size_t)n_sites * sizeof(int32_t),
+    // pageable caller buffers are staged through pinned memory so that the copies are true async DMA
+    const int32_t* src_x = h_sx;
+    const int32_t* src_y = h_sy;
+    if (!is_pinned(h_sx) || !is_pinned(h_sy)) {
+        memcpy(ctx->h_fr_sites, h_sx, (size_t)n_sites * sizeof(int32_t));
+        memcpy(ctx->h_fr_sites + ctx->max_sites, h_sy, (size_t)n_sites * sizeof(int32_t));
+        src_x = ctx->h_fr_sites; src_y = ctx->h_fr_sites + ctx->max_sites;
+    }
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sx, src_x, (size_t)n_sites * sizeof(int32_t),
                              cudaMemcpyHostToDevice, stream));
-    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sy, ctx->h_fr_sites + ctx->max_sites,
-                             (size_t)n_sites * sizeof(int32_t), cudaMemcpyHostToDevice, stream));
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_fr_sy, src_y, (size_t)n_sites * sizeof(int32_t),
+                             cudaMemcpyHostToDevice, stream));
     if ((rc = vor_frame_device(ctx, ctx->d_fr_sx, ctx->d_fr_sy, n_sites, stream)) != VOR_OK) return rc;
     VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_counts, ctx->d_fr_counts, 3 * sizeof(int64_t),
                              cudaMemcpyDeviceToHost, stream));
@@ -91,15 +104,20 @@ extern "C" int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* 
     int64_t nd = h_counts[2] < ctx->fr_cap ? h_counts[2] : ctx->fr_cap;
     if (nc > cap) nc = cap;
     if (nd > cap) nd = cap;
+    const bool direct = (nc == 0 || is_pinned(h_created)) && (nd == 0 || is_pinned(h_destroyed));
+    uint64_t* dst_c = direct ? h_created : ctx->h_fr_lists;
+    uint64_t* dst_d = direct ? h_destroyed : ctx->h_fr_lists + ctx->fr_cap;
     if (nc > 0)
-        VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_lists, ctx->d_fr_created, (size_t)nc * sizeof(uint64_t),
+        VOR_CUDA(cudaMemcpyAsync(dst_c, ctx->d_fr_created, (size_t)nc * sizeof(uint64_t),
                                  cudaMemcpyDeviceToHost, stream));
     if (nd > 0)
-        VOR_CUDA(cudaMemcpyAsync(ctx->h_fr_lists + ctx->fr_cap, ctx->d_fr_destroyed,
-                                 (size_t)nd * sizeof(uint64_t), cudaMemcpyDeviceToHost, stream));
+        VOR_CUDA(cudaMemcpyAsync(dst_d, ctx->d_fr_destroyed, (size_t)nd * sizeof(uint64_t),
+                                 cudaMemcpyDeviceToHost, stream));
     rc = vor_sync_status(ctx, stream);
-    if (nc > 0) memcpy(h_created, ctx->h_fr_lists, (size_t)nc * sizeof(uint64_t));
-    if (nd > 0) memcpy(h_destroyed, ctx->h_fr_lists + ctx->fr_cap, (size_t)nd * sizeof(uint64_t));
+    if (!direct) {
+        if (nc > 0) memcpy(h_created, dst_c, (size_t)nc * sizeof(uint64_t));
+        if (nd > 0) memcpy(h_destroyed, dst_d, (size_t)nd * sizeof(uint64_t));
+    }
     if (rc == VOR_OK && (h_counts[1] > cap || h_counts[2] > cap))
         return vor_fail(ctx, VOR_ECAPACITY, "vor_frame_host: created/destroyed list larger than cap");
     return rc;

@@ -380,3 +380,45 @@ def test_match_invariants_and_random(G):
     a, b = G.gpu_match(v, np.array([1000, 1000]), np.array([1000, 1000]), np.array([1100]), np.array([1000]), 4 * FP)
     assert a.tolist() == [0, -1] and b.tolist() == [0]
     v.close()
+
+
+# ------------------------------------------------------------------ full size, bench.py's launch configuration
+def test_config5_full_size_two_frames(G):
+    """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites) through the same calls, buffers
+    and capacities bench.py times.  Every label, edge key and flip is compared with the oracle
+    (O1b finishes a full frame in seconds), and O1b itself is cross-checked here against brute force
+    over all 10^6 sites on sampled cells."""
+    w = W.config(5)
+    L, n = w.L, w.n_sites
+    v = make(L, n, max_raw_keys=max(1 << 20, 16 * n))
+    cap_e = 4 * n + 1024
+    labels = torch.empty(L * L, dtype=torch.int32, device="cuda")
+    edges = [torch.empty(cap_e, dtype=torch.int64, device="cuda") for _ in range(2)]
+    n_edges = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(2)]
+    created = torch.empty(cap_e, dtype=torch.int64, device="cuda")
+    destroyed = torch.empty(cap_e, dtype=torch.int64, device="cuda")
+    n_c = torch.zeros(1, dtype=torch.int64, device="cuda")
+    n_d = torch.zeros(1, dtype=torch.int64, device="cuda")
+    rng = np.random.default_rng(5)
+    prev = np.empty(0, np.uint64)
+    for i, (sx, sy) in enumerate(w.frames(2)):
+        now, prv = i & 1, 1 - (i & 1)
+        v.vor_build_cells(G.dev(sx), G.dev(sy))
+        v.vor_label(labels)
+        v.vor_edges(labels, edges[now], n_edges[now])
+        v.vor_diff(edges[prv], n_edges[prv], edges[now], n_edges[now], created, destroyed, n_c, n_d)
+        v.vor_sync_status()
+        ref = oracle.label_cells(L, sx, sy, w.bucket_cells)
+        got = labels.cpu().numpy().reshape(L, L)
+        assert np.array_equal(got, ref), f"frame {i}: {int((got != ref).sum())} labels differ"
+        cells = rng.integers(0, L * L, 1500)
+        assert np.array_equal(ref.ravel()[cells], oracle.label_brute_at(L, sx, sy, cells))
+        e = oracle.edges(ref)
+        assert np.array_equal(G.u64(edges[now], int(n_edges[now].item())), e)
+        rc, rd = oracle.diff(prev, e)
+        assert np.array_equal(G.u64(created, int(n_c.item())), rc)
+        assert np.array_equal(G.u64(destroyed, int(n_d.item())), rd)
+        prev = e
+        del ref, got
+    assert 2.9 * n < len(prev) < 3.0 * n            # E slightly below 3N (R6), as the survey's probe found
+    v.close()
