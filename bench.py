@@ -321,7 +321,7 @@ def run_ours(args, w):
     alu_ops = LABEL_OPS_PER_CELL * cells_per_step
     roofline = {"kernel": lab_name, "bound": "alu", "achieved": alu_ops / label_s / 1e12, "peak": alu_peak,
                 "unit": "Tera int32 op/s", "frac": alu_ops / label_s / 1e12 / alu_peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(lab_name) if wr.name.startswith("cfg5_") else None,
+                "traffic": NCU_TRAFFIC_BYTES.get(lab_name) if wr.name == "cfg5_throughput_stress" else None,
                 "launch_ms": kernel_launch_ms[lab_name],
                 "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.6)",
                 "algorithmic": f"{LABEL_OPS_PER_CELL} int32 ops/cell x {cells_per_step} cells",
@@ -335,7 +335,7 @@ def run_ours(args, w):
         sec = kernel_launch_ms[name] * 1e-3
         return {"bound": "hbm", "achieved": nbytes / sec / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": nbytes / sec / 1e9 / hbm_peak, "launch_ms": kernel_launch_ms[name],
-                "traffic": NCU_TRAFFIC_BYTES.get(name) if wr.name.startswith("cfg5_") else None, "algorithmic": what, "peak_source": peak_src}
+                "traffic": NCU_TRAFFIC_BYTES.get(name) if wr.name == "cfg5_throughput_stress" else None, "algorithmic": what, "peak_source": peak_src}
 
     ne = counts["n_edges"]
     others = {
