@@ -339,10 +339,12 @@ def test_ccl_serpentine_long_chains(G):
     v.close()
 
 
-@pytest.mark.parametrize("cfg,L,nfr", [(3, 256, 3), (3, 1024, 2), (4, 512, 3)])
+@pytest.mark.parametrize("cfg,L,nfr", [(3, 256, 3), (3, 1024, 2), (4, 512, 3), (3, None, 2), (4, None, 2)])
 def test_field_pipeline_scaled_configs(G, cfg, L, nfr):
-    """threshold -> CCL -> centroids -> match -> label -> edges -> diff(maps), frame by frame."""
-    w = W.scaled(cfg, L)
+    """threshold -> CCL -> centroids -> match -> label -> edges -> diff(maps), frame by frame.
+    L = None: the configuration at its full BASELINE.json size (2048^2 / 4096^2)."""
+    w = W.config(cfg) if L is None else W.scaled(cfg, L)
+    L = w.L
     v = make(L, 65536)
     R = int(w.match_radius_cells * FP)
     prev_c, prev_e = None, None
