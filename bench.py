@@ -49,7 +49,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg5", help="cfg5 (default) | cfg2 | cfg5@L e.g. cfg5@4096")
+    ap.add_argument("--workload", default="cfg5", help="cfg5 (default) | cfg1 | cfg2 | cfg5@L e.g. cfg5@4096 | cfg3 | cfg4 (field path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-L", type=int, default=0,
@@ -378,10 +378,100 @@ def run_ours(args, w):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------ field path
+def run_field(args, w):
+    """--workload cfg3 | cfg4: one step = one frame of the field-derived path, rows a6..a8 then a1..a5
+    (threshold+CCL -> centroids -> match -> cell list -> label -> edges -> diff with maps).  Single GPU;
+    not the default bench line (the metric is quoted on config 5) - reported for the §8(a) field rows."""
+    import torch
+    from paper_1607_00908_b200.binding import Vor
+    torch.cuda.set_device(0)
+    W_, K = args.warmup, args.steps
+    L = w.L
+    frames = [torch.from_numpy(f).cuda().reshape(-1) for f in w.frames(W_ + K)]
+    cap = 1 << 16
+    v = Vor(L, cap)
+    i32 = dict(dtype=torch.int32, device="cuda")
+    ccl = torch.empty(L * L, **i32)
+    labels = torch.empty(L * L, **i32)
+    comp = [dict(cx=torch.empty(cap, dtype=torch.float64, device="cuda"), cy=torch.empty(cap, dtype=torch.float64, device="cuda"),
+                 sx=torch.empty(cap, **i32), sy=torch.empty(cap, **i32), size=torch.empty(cap, **i32),
+                 root=torch.empty(cap, **i32), n=torch.zeros(1, **i32)) for _ in range(2)]
+    p2n, n2p = torch.empty(cap, **i32), torch.empty(cap, **i32)
+    cap_e = 8 * cap
+    edges = [torch.empty(cap_e, dtype=torch.int64, device="cuda") for _ in range(2)]
+    n_edges = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(2)]
+    created, destroyed = torch.empty(cap_e, dtype=torch.int64, device="cuda"), torch.empty(cap_e, dtype=torch.int64, device="cuda")
+    n_c, n_d = torch.zeros(1, dtype=torch.int64, device="cuda"), torch.zeros(1, dtype=torch.int64, device="cuda")
+    stream = torch.cuda.current_stream()
+    names = ["threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"]
+    R = int(w.match_radius_cells * W.FP_ONE)
+    kn = [0, 0]
+
+    def step(i, ev=None):
+        now, prv = i & 1, 1 - (i & 1)
+        c, pc = comp[now], comp[prv]
+        rec = (lambda j: ev[j].record(stream)) if ev else (lambda j: None)
+        rec(0); v.field_threshold_ccl(frames[i], w.threshold, True, ccl)
+        rec(1); v.field_centroids(ccl, w.min_size, c["cx"], c["cy"], c["sx"], c["sy"], c["size"], c["root"], c["n"])
+        rec(2)
+        if i > 0:
+            v.match_sites(pc["sx"], pc["sy"], pc["n"], c["sx"], c["sy"], c["n"], R, p2n, n2p)
+        kn[now] = int(c["n"].item())               # vor_build_cells takes n_sites on the host: one sync per frame
+        rec(3); v.vor_build_cells(c["sx"][:kn[now]], c["sy"][:kn[now]])
+        rec(4); v.vor_label(labels)
+        rec(5); v.vor_edges(labels, edges[now], n_edges[now])
+        rec(6)
+        if i > 0:
+            v.vor_diff(edges[prv], n_edges[prv], edges[now], n_edges[now], created, destroyed, n_c, n_d,
+                       p2n=p2n, n2p=n2p, n_prev_labels=max(kn[prv], 1), n_now_labels=max(kn[now], 1))
+        rec(7)
+
+    for i in range(W_):
+        step(i)
+    v.vor_sync_status()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in range(K)]
+    sampler = ClockSampler(0)
+    torch.cuda.synchronize()
+    sampler.start()
+    l0 = v.vor_launch_count()
+    t0 = time.perf_counter()
+    for k in range(K):
+        step(W_ + k, evs[k])
+    torch.cuda.synchronize()
+    secs = time.perf_counter() - t0
+    clocks = sampler.stop()
+    launches = v.vor_launch_count() - l0
+    v.vor_sync_status()
+    kernel_ms = {nm: float(np.mean([evs[k][j].elapsed_time(evs[k][j + 1]) for k in range(K)])) for j, nm in enumerate(names)}
+    hbm_peak, peak_src, _ = peaks()
+    cells = L * L
+    def roof(ms, nbytes, what):
+        return {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "algorithmic": what, "peak_source": peak_src}
+    out = {"metric": METRIC, "value": K * cells / secs, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W_,
+           "ms_per_step": 1e3 * secs / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "int32", "data": "synthetic",
+           "config": {"workload": w.name, "L": L, "components": kn[(W_ + K - 1) & 1], "frames": K,
+                      "timing": "wall clock around K frames (one host sync per frame for the component count)"},
+           "frames_per_s": K / secs, "kernel_ms": kernel_ms,
+           "counts": {"n_edges": int(n_edges[(W_ + K - 1) & 1].item()), "n_created": int(n_c.item()), "n_destroyed": int(n_d.item())},
+           "roofline": dict(roof(kernel_ms["threshold_ccl"], 8.0 * cells, "4 B/cell field read + 4 B/cell label written"),
+                            kernel="field_threshold_ccl (3 kernels)"),
+           "rooflines_other": {"field_centroids": roof(kernel_ms["centroids"], 4.0 * cells, "4 B/cell read")},
+           "clocks": clocks, "gpu_launches": int(launches)}
+    print(json.dumps(out), flush=True)
+    v.close()
+
+
 def main():
     args = parse()
     w = get_workload(args.workload)
-    if args.impl == "reference":
+    if isinstance(w, W.FieldWorkload):
+        if args.impl == "reference" or args.gpus != 1:
+            raise SystemExit("field workloads: --impl ours --gpus 1 only")
+        run_field(args, w)
+    elif args.impl == "reference":
         run_reference(args, w)
     else:
         run_ours(args, w)

@@ -17,6 +17,8 @@ constexpr int kSortThreads = 1024;         // block size of the persistent coope
 constexpr int kMaxCoopBlocks = 1024;       // allocation bound for per-block scratch of those kernels
 constexpr int kRowStride = 16;             // adjacency-row slots per site (64-byte rows)
 constexpr uint32_t kEmptySlot = 0xffffffffu;
+constexpr int kMatchGrid = 512;            // match_sites: buckets per side (at most), kMatchSlots sites per bucket
+constexpr int kMatchSlots = 4;
 constexpr int kMaxProfLaunches = 256;      // launches timed per vor_profile_begin/end bracket
 
 // error flag bits latched on the device (ctx->d_flags[0])
@@ -78,6 +80,7 @@ struct vor_ctx {
     int32_t* d_comp_count;     // device scalars [4]
     int32_t* d_best;           // [best_cap] best partner per prev / now (lazily sized)
     int64_t best_cap;
+    int32_t* d_mgrid;          // match grid: [2][kMatchGrid^2] counts, then [2][kMatchGrid^2 * kMatchSlots] site ids
 
     // ---- frame pipeline (e2e)
     int32_t* d_fr_sx;

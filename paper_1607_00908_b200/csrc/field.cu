@@ -221,19 +221,90 @@ struct CentroidSink {
 };
 
 // ------------------------------------------------------------------------------------ a8: match
+// Fast path: both point sets are hashed into a uniform grid of nbm x nbm buckets whose width is at
+// least the matching radius, so that every partner within the radius lies in the 3 x 3 buckets around
+// the query (with wrap).  A bucket holds kMatchSlots ids; if any bucket overflows a device flag makes
+// the brute-force kernel below redo the search (same result by definition), so the outcome never
+// depends on the grid.
 constexpr int kMatchThreads = 256;
+
+struct MatchGrid {
+    int32_t* cnt[2];           // [nbm * nbm] per set (0 = prev, 1 = now)
+    int32_t* ids[2];           // [nbm * nbm * kMatchSlots]
+    int32_t nbm;
+    int32_t* overflow;         // device flag
+};
+
+__device__ __forceinline__ int32_t mbucket(int32_t v, long long P, int32_t nbm) {
+    return (int32_t)(((long long)v * nbm) / P);
+}
+
+__global__ void match_fill_kernel(const int32_t* __restrict__ px, const int32_t* __restrict__ py,
+                                  const int32_t* __restrict__ n_prev_p, const int32_t* __restrict__ nx,
+                                  const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
+                                  int32_t cap_prev, int32_t cap_now, long long P, MatchGrid g) {
+    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
+    for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_prev + n_now; i += gridDim.x * blockDim.x) {
+        const int set = i >= n_prev;
+        const int32_t k = set ? i - n_prev : i;
+        const int32_t x = set ? nx[k] : px[k], y = set ? ny[k] : py[k];
+        const int32_t b = mbucket(y, P, g.nbm) * g.nbm + mbucket(x, P, g.nbm);
+        const int32_t slot = atomicAdd(&g.cnt[set][b], 1);
+        if (slot < kMatchSlots) g.ids[set][(size_t)b * kMatchSlots + slot] = k;
+        else *g.overflow = 1;
+    }
+}
+
+// best[q] for every query of both directions: nearest target within the radius (ties: smallest index)
+__global__ void match_grid_kernel(const int32_t* __restrict__ px, const int32_t* __restrict__ py,
+                                  const int32_t* __restrict__ n_prev_p, const int32_t* __restrict__ nx,
+                                  const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
+                                  int32_t cap_prev, int32_t cap_now, long long P, long long r2, MatchGrid g,
+                                  int32_t* __restrict__ best) {
+    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
+    for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_prev + n_now; i += gridDim.x * blockDim.x) {
+        const bool q_is_now = i >= n_prev;                  // now queries search the prev set
+        const int32_t q = q_is_now ? i - n_prev : i;
+        const int tset = q_is_now ? 0 : 1;
+        const int32_t* __restrict__ tx = q_is_now ? px : nx;
+        const int32_t* __restrict__ ty = q_is_now ? py : ny;
+        const long long ax = q_is_now ? nx[q] : px[q], ay = q_is_now ? ny[q] : py[q];
+        const int32_t bx = mbucket((int32_t)ax, P, g.nbm), by = mbucket((int32_t)ay, P, g.nbm);
+        long long bd = INT64_MAX;
+        int32_t bi = -1;
+        const int span = g.nbm >= 3 ? 3 : g.nbm;             // tiny grids: every bucket once
+        for (int oy = 0; oy < span; ++oy) {
+            const int32_t cy = g.nbm >= 3 ? (by + oy - 1 + g.nbm) % g.nbm : oy;
+            for (int ox = 0; ox < span; ++ox) {
+                const int32_t cx = g.nbm >= 3 ? (bx + ox - 1 + g.nbm) % g.nbm : ox;
+                const int32_t b = cy * g.nbm + cx;
+                const int32_t c = min(g.cnt[tset][b], kMatchSlots);
+                for (int32_t s = 0; s < c; ++s) {
+                    const int32_t t = g.ids[tset][(size_t)b * kMatchSlots + s];
+                    const long long vx = tx[t], vy = ty[t];
+                    long long dx = ax > vx ? ax - vx : vx - ax; dx = dx < P - dx ? dx : P - dx;
+                    long long dy = ay > vy ? ay - vy : vy - ay; dy = dy < P - dy ? dy : P - dy;
+                    const long long d2 = dx * dx + dy * dy;
+                    if (d2 < bd || (d2 == bd && t < bi)) { bd = d2; bi = t; }
+                }
+            }
+        }
+        best[(q_is_now ? cap_prev : 0) + q] = (bi >= 0 && bd <= r2) ? bi : -1;
+    }
+}
 
 // blocks [0, gq) : queries = now, targets = prev -> best[cap_prev + j];  blocks [gq, ..): the reverse
 __global__ void __launch_bounds__(kMatchThreads) match_best_kernel(
         const int32_t* __restrict__ px, const int32_t* __restrict__ py, const int32_t* __restrict__ n_prev_p,
         const int32_t* __restrict__ nx, const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
         int32_t cap_prev, int32_t cap_now, int32_t blocks_now, long long P, long long r2,
-        int32_t* __restrict__ best, int32_t* __restrict__ flags) {
+        int32_t* __restrict__ best, int32_t* __restrict__ flags, const int32_t* __restrict__ needed) {
     __shared__ int32_t tx[kMatchThreads], ty[kMatchThreads];
-    const bool q_is_now = (int)blockIdx.x < blocks_now;
-    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
     if (blockIdx.x == 0 && threadIdx.x == 0 && (*n_prev_p > cap_prev || *n_now_p > cap_now))
         atomicOr(flags, FLAG_MATCH_CAP);
+    if (needed && *needed == 0) return;                   // the grid path answered every query
+    const bool q_is_now = (int)blockIdx.x < blocks_now;
+    const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
     const int32_t* qx = q_is_now ? nx : px; const int32_t* qy = q_is_now ? ny : py;
     const int32_t* sx = q_is_now ? px : nx; const int32_t* sy = q_is_now ? py : ny;
     const int32_t nq = q_is_now ? n_now : n_prev, nt = q_is_now ? n_prev : n_now;
@@ -346,9 +417,28 @@ extern "C" int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_p
         ctx->best_cap = need;
     }
     const int bn = (cap_now + kMatchThreads - 1) / kMatchThreads, bp = (cap_prev + kMatchThreads - 1) / kMatchThreads;
+    const long long r2 = (long long)radius_fp * radius_fp;
+    // grid path: bucket width P / nbm >= radius
+    int64_t nbm = radius_fp > 0 ? ctx->P / radius_fp : kMatchGrid;
+    if (nbm > kMatchGrid) nbm = kMatchGrid;
+    if (nbm < 1) nbm = 1;
+    const size_t cells = (size_t)kMatchGrid * kMatchGrid;
+    if (!ctx->d_mgrid)
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_mgrid, (2 * cells + 2 * cells * kMatchSlots + 1) * sizeof(int32_t)));
+    MatchGrid g;
+    g.cnt[0] = ctx->d_mgrid; g.cnt[1] = ctx->d_mgrid + cells;
+    g.ids[0] = ctx->d_mgrid + 2 * cells; g.ids[1] = g.ids[0] + cells * kMatchSlots;
+    g.overflow = g.ids[1] + cells * kMatchSlots;
+    g.nbm = (int32_t)nbm;
+    VOR_CUDA(cudaMemsetAsync(ctx->d_mgrid, 0, 2 * cells * sizeof(int32_t), stream));
+    VOR_CUDA(cudaMemsetAsync(g.overflow, 0, sizeof(int32_t), stream));
+    VOR_LAUNCH(match_fill_kernel, 2 * kNumSMs, 256, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny, d_n_now,
+               cap_prev, cap_now, (long long)ctx->P, g);
+    VOR_LAUNCH(match_grid_kernel, 4 * kNumSMs, 128, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny, d_n_now,
+               cap_prev, cap_now, (long long)ctx->P, r2, g, ctx->d_best);
     VOR_LAUNCH(match_best_kernel, bn + bp, kMatchThreads, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny,
-               d_n_now, cap_prev, cap_now, bn, (long long)ctx->P, (long long)radius_fp * radius_fp,
-               ctx->d_best, ctx->d_flags);
+               d_n_now, cap_prev, cap_now, bn, (long long)ctx->P, r2,
+               ctx->d_best, ctx->d_flags, (const int32_t*)g.overflow);
     VOR_LAUNCH(match_combine_kernel, 2 * kNumSMs, 256, 0, stream, d_n_prev, d_n_now, cap_prev, cap_now,
                ctx->d_best, d_p2n, d_n2p);
     return VOR_OK;

@@ -381,6 +381,28 @@ def test_match_invariants_and_random(G):
             assert np.array_equal(a, ra) and np.array_equal(b, rb)
     a, b = G.gpu_match(v, np.array([1000, 1000]), np.array([1000, 1000]), np.array([1100]), np.array([1000]), 4 * FP)
     assert a.tolist() == [0, -1] and b.tolist() == [0]
+    # a crowded bucket (grid path overflows -> brute-force redo) next to the seam, plus scattered points
+    cx = np.concatenate([rng.integers(P - 300, P + 300, 150) % P, rng.integers(0, P, 60)]).astype(np.int32)
+    cy = np.concatenate([rng.integers(-200, 400, 150) % P, rng.integers(0, P, 60)]).astype(np.int32)
+    mx = ((cx.astype(np.int64) + rng.integers(-150, 150, len(cx))) % P).astype(np.int32)
+    my = ((cy.astype(np.int64) + rng.integers(-150, 150, len(cy))) % P).astype(np.int32)
+    for R in (1 * FP, 3 * FP):
+        a, b = G.gpu_match(v, cx, cy, mx[::-1].copy(), my[::-1].copy(), R)
+        ra, rb = oracle.match(64, cx, cy, mx[::-1].copy(), my[::-1].copy(), R)
+        assert np.array_equal(a, ra) and np.array_equal(b, rb)
+    v.close()
+    # grid path proper: many well-separated points on a large lattice, seam included
+    L = 2048
+    v = make(L, 8192)
+    P = FP * L
+    g = np.arange(64) * (P // 64)
+    px, py = (np.repeat(g, 64) + rng.integers(0, 2000, 4096)) % P, (np.tile(g, 64) + rng.integers(0, 2000, 4096)) % P
+    keep = rng.random(4096) > 0.05
+    nx = ((px + rng.integers(-700, 700, 4096)) % P)[keep][::-1].copy()
+    ny = ((py + rng.integers(-700, 700, 4096)) % P)[keep][::-1].copy()
+    a, b = G.gpu_match(v, px.astype(np.int32), py.astype(np.int32), nx.astype(np.int32), ny.astype(np.int32), 4 * FP)
+    ra, rb = oracle.match(L, px.astype(np.int32), py.astype(np.int32), nx.astype(np.int32), ny.astype(np.int32), 4 * FP)
+    assert np.array_equal(a, ra) and np.array_equal(b, rb) and (ra >= 0).sum() > 3000
     v.close()
 
 
