@@ -1,7 +1,8 @@
 // a6..a8 — the field-derived front end: bubbles from a thresholded scalar field.
 //  a6 field_threshold_ccl  PAPER.md:95 (§III.A): threshold -> two-valued variable -> cluster labelling
 //                          (the paper adapts the label-equivalence method of its ref. [6]); here a
-//                          lock-free union-find whose roots are the minimum linear index.
+//                          lock-free union-find whose roots are the minimum linear index, run first
+//                          per 64 x 32 tile in shared memory, then over the tile seams in HBM.
 //  a7 field_centroids      PAPER.md:95-101: bubble size by atomic counting, centre of mass = sum of
 //                          the lattice coordinates / size.  Integer sums (order independent), periodic
 //                          unwrap relative to the root cell, one float64 divide.
@@ -12,15 +13,6 @@
 namespace {
 
 // ------------------------------------------------------------------------------------ a6: CCL
-__global__ void ccl_init_kernel(const float* __restrict__ field, float thr, int above, int64_t n,
-                                int32_t* __restrict__ parent) {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const float v = field[i];
-        const bool m = above ? (v > thr) : (v < thr);      // NaN compares false both ways
-        parent[i] = m ? (int32_t)i : -1;
-    }
-}
-
 __device__ __forceinline__ int32_t uf_find(const int32_t* parent, int32_t a) {
     int32_t p = parent[a];
     while (p != a) { a = p; p = parent[a]; }
@@ -40,15 +32,100 @@ __device__ __forceinline__ void uf_union(int32_t* parent, int32_t a, int32_t b) 
     }
 }
 
-__global__ void ccl_merge_kernel(int32_t L, int32_t* __restrict__ parent) {
-    const int64_t n = (int64_t)L * L;
+// Tile stage: one CTA thresholds a kTileW x kTileH tile into shared memory, runs the same union-find
+// on the tile's own right / down pairs there (roots = smallest local index = smallest global index of
+// the tile-component, because local row-major order follows the global one), flattens, and writes
+// parent[cell] = global index of its tile root.  HBM: 4 B/cell read, 4 B/cell written.
+constexpr int kTileW = 64, kTileH = 32, kTileThreads = 256;
+constexpr int kTileRows = kTileW * kTileH / kTileThreads;     // rows per thread (8)
+
+__device__ __forceinline__ int32_t suf_find(const int32_t* parent, int32_t a) {
+    int32_t p = parent[a];
+    while (p != a) { a = p; p = parent[a]; }
+    return a;
+}
+__device__ __forceinline__ void suf_union(int32_t* parent, int32_t a, int32_t b) {
+    for (;;) {
+        a = suf_find(parent, a);
+        b = suf_find(parent, b);
+        if (a == b) return;
+        if (a < b) { const int32_t t = a; a = b; b = t; }
+        const int32_t old = atomicMin(&parent[a], b);
+        if (old == a) return;
+        a = old;
+    }
+}
+
+__global__ void __launch_bounds__(kTileThreads) ccl_tile_kernel(const float* __restrict__ field, float thr,
+                                                                int above, int32_t L,
+                                                                int32_t* __restrict__ parent) {
+    __shared__ int32_t lab[kTileH * kTileW];
+    const int32_t X0 = blockIdx.x * kTileW, Y0 = blockIdx.y * kTileH;
+    const int lane = threadIdx.x & 31;
+    const int lx = threadIdx.x & (kTileW - 1), ly0 = (threadIdx.x / kTileW) * kTileRows;
+    const int32_t x = X0 + lx;
+    // a warp holds 32 consecutive columns of one row: every cell starts out pointing at the first
+    // cell of its horizontal run inside those 32 columns, so no union is needed along rows
+#pragma unroll
+    for (int j = 0; j < kTileRows; ++j) {
+        const int32_t y = Y0 + ly0 + j;
+        bool m = false;
+        if (x < L && y < L) {
+            const float v = __ldcs(field + (int64_t)y * L + x);
+            m = above ? (v > thr) : (v < thr);             // NaN compares false both ways
+        }
+        const unsigned bits = __ballot_sync(0xffffffffu, m);
+        const int run = __clz((int)~(bits << (31 - lane)));   // set cells ending at this lane (>= 1 if m)
+        const int li = (ly0 + j) * kTileW + lx;
+        lab[li] = m ? li - run + 1 : -1;
+    }
+    __syncthreads();
+    // unions: the two 32-column halves of a row, and vertically adjacent runs (once per overlap: at
+    // the overlap's leftmost column the cell to the left is unset in one of the two rows)
+#pragma unroll
+    for (int j = 0; j < kTileRows; ++j) {
+        const int li = (ly0 + j) * kTileW + lx;
+        if (lab[li] < 0) continue;
+        if (lx == 32 && lab[li - 1] >= 0) suf_union(lab, li, li - 1);
+        if (ly0 + j + 1 < kTileH && lab[li + kTileW] >= 0 &&
+            (lx == 0 || lab[li - 1] < 0 || lab[li + kTileW - 1] < 0))
+            suf_union(lab, li, li + kTileW);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kTileRows; ++j) {
+        const int32_t y = Y0 + ly0 + j;
+        if (x >= L || y >= L) continue;
+        const int li = (ly0 + j) * kTileW + lx;
+        int32_t out = -1;
+        if (lab[li] >= 0) {
+            const int32_t r = suf_find(lab, li);
+            out = (int32_t)((int64_t)(Y0 + r / kTileW) * L + X0 + (r & (kTileW - 1)));
+        }
+        parent[(int64_t)y * L + x] = out;
+    }
+}
+
+// Seam stage: the pairs that straddle tile borders (including the periodic wrap and the ragged last
+// tiles) are united in the global array.  Items [0, ntx * L): vertical seam lines (cell | right
+// neighbour); items [ntx * L, (ntx + nty) * L): horizontal seam lines (cell | down neighbour).
+__global__ void ccl_seam_kernel(int32_t L, int32_t ntx, int32_t nty, int32_t* __restrict__ parent) {
+    const int64_t n = (int64_t)(ntx + nty) * L;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        if (parent[i] < 0) continue;
-        const int32_t x = (int32_t)(i % L), y = (int32_t)(i / L);
-        const int64_t r = (int64_t)y * L + (x + 1 == L ? 0 : x + 1);
-        const int64_t d = (int64_t)(y + 1 == L ? 0 : y + 1) * L + x;
-        if (r != i && parent[r] >= 0) uf_union(parent, (int32_t)i, (int32_t)r);
-        if (d != i && parent[d] >= 0) uf_union(parent, (int32_t)i, (int32_t)d);
+        int64_t a, b;
+        if (i < (int64_t)ntx * L) {
+            const int32_t k = (int32_t)(i / L), y = (int32_t)(i % L);
+            const int32_t x = min((k + 1) * kTileW - 1, L - 1);
+            a = (int64_t)y * L + x;
+            b = (int64_t)y * L + (x + 1 == L ? 0 : x + 1);
+        } else {
+            const int64_t r = i - (int64_t)ntx * L;
+            const int32_t k = (int32_t)(r / L), x = (int32_t)(r % L);
+            const int32_t y = min((k + 1) * kTileH - 1, L - 1);
+            a = (int64_t)y * L + x;
+            b = (int64_t)(y + 1 == L ? 0 : y + 1) * L + x;
+        }
+        if (a != b && parent[a] >= 0 && parent[b] >= 0) uf_union(parent, (int32_t)a, (int32_t)b);
     }
 }
 
@@ -359,8 +436,11 @@ extern "C" int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr
     cudaStream_t stream = (cudaStream_t)stream_;
     const int64_t n = (int64_t)ctx->L * ctx->L;
     const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
-    VOR_LAUNCH(ccl_init_kernel, grid, 256, 0, stream, d_field, thr, above ? 1 : 0, n, d_ccl);
-    VOR_LAUNCH(ccl_merge_kernel, grid, 256, 0, stream, ctx->L, d_ccl);
+    const int32_t ntx = (ctx->L + kTileW - 1) / kTileW, nty = (ctx->L + kTileH - 1) / kTileH;
+    VOR_LAUNCH(ccl_tile_kernel, dim3(ntx, nty), kTileThreads, 0, stream, d_field, thr, above ? 1 : 0, ctx->L, d_ccl);
+    const int64_t seams = (int64_t)(ntx + nty) * ctx->L;
+    const int sgrid = (int)((seams + 255) / 256 < 8 * kNumSMs ? (seams + 255) / 256 : 8 * kNumSMs);
+    VOR_LAUNCH(ccl_seam_kernel, sgrid, 256, 0, stream, ctx->L, ntx, nty, d_ccl);
     VOR_LAUNCH(ccl_flatten_kernel, grid, 256, 0, stream, n, d_ccl);
     return VOR_OK;
 }
