@@ -138,11 +138,14 @@ __global__ void ccl_flatten_kernel(int64_t n, int32_t* __restrict__ parent) {
 
 // ------------------------------------------------------------------------------------ compaction
 // Order-preserving compaction of the items i in [0, n) that satisfy pred(i); persistent chunks.
-constexpr int kCompThreads = 1024;
+constexpr int kCompThreads = 512;
+constexpr int kCompItems = 8;                      // items per thread per batch (warp-strided: coalesced)
+constexpr int kCompBatch = kCompThreads * kCompItems;
+constexpr int kCompGrid = 4 * kNumSMs;             // <= 2 * kMaxCoopBlocks entries of d_blk_count
 
 __device__ __forceinline__ void comp_chunk(int64_t n, int64_t* beg, int64_t* end) {
     int64_t C = (n + gridDim.x - 1) / gridDim.x;
-    C = (C + kCompThreads - 1) / kCompThreads * kCompThreads;
+    C = (C + kCompBatch - 1) / kCompBatch * kCompBatch;
     int64_t s = (int64_t)blockIdx.x * C;
     *beg = s < n ? s : n;
     *end = s + C < n ? s + C : n;
@@ -192,11 +195,18 @@ __global__ void __launch_bounds__(kCompThreads) comp_write_kernel(Pred pred, Sin
     all = comp_block_sum(all, sh);
     if (blockIdx.x == 0 && threadIdx.x == 0) sink.total(all);
     int64_t run = before;
-    for (int64_t sub = beg; sub < end; sub += kCompThreads) {
-        const int64_t i = sub + threadIdx.x;
-        const bool keep = i < end && pred(i);
-        const unsigned ball = __ballot_sync(0xffffffffu, keep);
-        if (lane == 0) wtot[wid] = __popc(ball);
+    for (int64_t sub = beg; sub < end; sub += kCompBatch) {
+        // warp w owns items [sub + 256 w, sub + 256 w + 256): item = base + 32 k + lane, k = 0..7
+        const int64_t wb = sub + (int64_t)wid * (32 * kCompItems) + lane;
+        unsigned ball[kCompItems];
+        int32_t mine = 0;
+#pragma unroll
+        for (int k = 0; k < kCompItems; ++k) {
+            const int64_t i = wb + 32 * k;
+            ball[k] = __ballot_sync(0xffffffffu, i < end && pred(i));
+            mine += __popc(ball[k]);
+        }
+        if (lane == 0) wtot[wid] = mine;
         __syncthreads();
         int32_t wbase = 0, total = 0;
         for (int w = 0; w < kCompThreads / 32; ++w) {
@@ -204,7 +214,12 @@ __global__ void __launch_bounds__(kCompThreads) comp_write_kernel(Pred pred, Sin
             if (w < wid) wbase += t;
             total += t;
         }
-        if (keep) sink.put(run + wbase + __popc(ball & ((1u << lane) - 1u)), i);
+        int64_t pos = run + wbase;
+#pragma unroll
+        for (int k = 0; k < kCompItems; ++k) {
+            if (ball[k] >> lane & 1u) sink.put(pos + __popc(ball[k] & ((1u << lane) - 1u)), wb + 32 * k);
+            pos += __popc(ball[k]);
+        }
         run += total;
         __syncthreads();
     }
@@ -465,8 +480,8 @@ extern "C" int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_s
     VOR_CUDA(cudaMemsetAsync(ctx->d_acc, 0, 3 * (size_t)ctx->max_comp * sizeof(int64_t), stream));
     RootPred rp{d_ccl, n};
     RootSink rs{ctx->d_comp_root, ctx->d_rank, ctx->max_comp, &ctx->d_comp_count[0], ctx->d_flags};
-    VOR_LAUNCH(comp_count_kernel<RootPred>, kNumSMs, kCompThreads, 0, stream, rp, ctx->d_blk_count);
-    VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kNumSMs, kCompThreads, 0, stream, rp, rs,
+    VOR_LAUNCH(comp_count_kernel<RootPred>, kCompGrid, kCompThreads, 0, stream, rp, ctx->d_blk_count);
+    VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kCompGrid, kCompThreads, 0, stream, rp, rs,
                ctx->d_blk_count);
     const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
     VOR_LAUNCH(accumulate_kernel, grid, 256, 0, stream, d_ccl, ctx->d_rank, ctx->L,
@@ -474,8 +489,8 @@ extern "C" int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_s
     SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
     CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->L, cap,
                     d_cx, d_cy, d_sx, d_sy, d_size, d_root, d_n_comp, ctx->d_flags};
-    VOR_LAUNCH(comp_count_kernel<SizePred>, kNumSMs, kCompThreads, 0, stream, sp, ctx->d_blk_count);
-    VOR_LAUNCH((comp_write_kernel<SizePred, CentroidSink>), kNumSMs, kCompThreads, 0, stream, sp, cs,
+    VOR_LAUNCH(comp_count_kernel<SizePred>, kCompGrid, kCompThreads, 0, stream, sp, ctx->d_blk_count);
+    VOR_LAUNCH((comp_write_kernel<SizePred, CentroidSink>), kCompGrid, kCompThreads, 0, stream, sp, cs,
                ctx->d_blk_count);
     return VOR_OK;
 }
