@@ -25,7 +25,7 @@ sys.path.insert(0, ROOT)
 
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
-# Algorithmic integer work of exact labelling per lattice cell (DESIGN.md §5.6): 7 candidate sites (a
+# Algorithmic integer work of exact labelling per lattice cell (DESIGN.md §5.8): 7 candidate sites (a
 # Voronoi region has 6 neighbours on average, plus the owner) x 3 ops (two multiply-adds of the
 # distance expansion, one min) + 1 store.
 LABEL_OPS_PER_CELL = 22
@@ -313,7 +313,7 @@ def run_ours(args, w):
 
     hbm_peak, peak_src, sm_max_mhz = peaks()
     # Dominant kernel = label_cta_kernel (one launch per step).  It is bound by plain
-    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.6
+    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.8
     # derives (SMs x 128 lanes x max SM clock); algorithmic work = 22 integer ops per cell.
     lab_name = max((nm for nm in kernel_launch_ms if "label" in nm), key=lambda nm: kernel_launch_ms[nm])
     label_s = kernel_launch_ms[lab_name] * 1e-3
@@ -323,7 +323,7 @@ def run_ours(args, w):
                 "unit": "Tera int32 op/s", "frac": alu_ops / label_s / 1e12 / alu_peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(lab_name) if wr.name == "cfg5_throughput_stress" else None,
                 "launch_ms": kernel_launch_ms[lab_name],
-                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.6)",
+                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.8)",
                 "algorithmic": f"{LABEL_OPS_PER_CELL} int32 ops/cell x {cells_per_step} cells",
                 "hbm_view": {"achieved": 4.0 * cells_per_step / label_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
                              "frac": 4.0 * cells_per_step / label_s / 1e9 / hbm_peak,
