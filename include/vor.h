@@ -68,7 +68,7 @@ int vor_profile_begin(vor_ctx* ctx);
 int vor_profile_end(vor_ctx* ctx, void* stream, char* names, int32_t names_len, float* ms, int32_t cap);
 
 /* Tuning knobs (integers).  Unknown names -> VOR_EINVAL.
- *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 25)
+ *   "bucket_occupancy_x100"  target sites per cell-list bucket * 100 (default 100)
  *   "row_slots"              adjacency-matrix slots used per site in vor_edges: 4, 8, 12 or 16
  *                            (default 16); pairs that do not fit take the sorted overflow path,
  *                            so the result never depends on it
