@@ -153,6 +153,21 @@ def match(L, px, py, nx, ny, radius_fp):
     return p2n, n2p
 
 
+def events(prev, now, n):
+    """O7: trigger[n], events_indices, count_prev[n], count_now[n], global_trigger (PAPER.md:215-236)."""
+    prev = np.ascontiguousarray(prev, dtype=np.uint64)
+    now = np.ascontiguousarray(now, dtype=np.uint64)
+    trig = np.zeros(n, np.int32); idx = np.zeros(max(n, 1), np.int32)
+    cp = np.zeros(n, np.int32); cn = np.zeros(n, np.int32)
+    m = C.c_int32(0)
+    lib().orc_events.restype = C.c_int32
+    g = lib().orc_events(_p(prev, C.c_uint64), C.c_int64(len(prev)), _p(now, C.c_uint64), C.c_int64(len(now)),
+                         C.c_int32(n), _p(trig, C.c_int32), _p(idx, C.c_int32), C.byref(m),
+                         _p(cp, C.c_int32), _p(cn, C.c_int32))
+    return dict(trigger=trig, events_indices=idx[:m.value].copy(), count_prev=cp, count_now=cn,
+                global_trigger=int(g))
+
+
 def unpack(keys):
     """uint64 packed keys -> (i, j) int64 arrays."""
     keys = np.asarray(keys, dtype=np.uint64)

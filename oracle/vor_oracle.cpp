@@ -365,6 +365,45 @@ void orc_match(int32_t L, const int32_t* px, const int32_t* py, int32_t n_prev,
     for (int32_t j = 0; j < n_now; ++j) n2p[j] = (bp[j] >= 0 && bn[bp[j]] == j) ? bp[j] : -1;
 }
 
+// O7 — trigger and event counts (§III.B.3: every row of (E_P)_PN is compared with
+// its isomorphic row of (E_N)_NN; a vertex whose rows differ gets local_trigger = 1, and
+// global_trigger says whether any did; §III.B.4: the triggering indices are written to
+// eventsIndices, their number to eventsNumber; for every active index, eventsCount =
+// how many active sites are connected to it, "repeated for the active indices of the two
+// triangulations").  Inputs: the two ascending unique edge lists in ONE index space (past list
+// already translated) over n vertices.  Written out as the definition:
+// row(i) = sorted neighbour list of i; trigger[i] = rows differ.
+// Outputs: trigger[n] (0/1), events_indices (ascending, first *events_number entries),
+// count_prev[n], count_now[n] (0 for inactive vertices).  Returns global_trigger.
+int32_t orc_events(const u64* prev, i64 n_prev, const u64* now, i64 n_now, int32_t n,
+                   int32_t* trigger, int32_t* events_indices, int32_t* events_number,
+                   int32_t* count_prev, int32_t* count_now) {
+    std::vector<std::vector<int32_t>> rp(n), rn(n);
+    for (i64 k = 0; k < n_prev; ++k) {
+        const int32_t i = (int32_t)(prev[k] >> 32), j = (int32_t)(prev[k] & 0xffffffffu);
+        if (i < n && j < n) { rp[i].push_back(j); rp[j].push_back(i); }
+    }
+    for (i64 k = 0; k < n_now; ++k) {
+        const int32_t i = (int32_t)(now[k] >> 32), j = (int32_t)(now[k] & 0xffffffffu);
+        if (i < n && j < n) { rn[i].push_back(j); rn[j].push_back(i); }
+    }
+    int32_t m = 0, any = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        std::sort(rp[i].begin(), rp[i].end());
+        std::sort(rn[i].begin(), rn[i].end());
+        trigger[i] = rp[i] != rn[i];
+        if (trigger[i]) { events_indices[m++] = i; any = 1; }
+    }
+    *events_number = m;
+    for (int32_t i = 0; i < n; ++i) {
+        count_prev[i] = count_now[i] = 0;
+        if (!trigger[i]) continue;
+        for (int32_t j : rp[i]) count_prev[i] += trigger[j];
+        for (int32_t j : rn[i]) count_now[i] += trigger[j];
+    }
+    return any;
+}
+
 int orc_num_threads(int threads) { return resolve_threads(threads); }
 
 }  // extern "C"
