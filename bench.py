@@ -25,7 +25,7 @@ sys.path.insert(0, ROOT)
 
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
-# Algorithmic integer work of exact labelling per lattice cell (DESIGN.md §5.8): 7 candidate sites (a
+# Algorithmic integer work of exact labelling per lattice cell (DESIGN.md §5.9): 7 candidate sites (a
 # Voronoi region has 6 neighbours on average, plus the owner) x 3 ops (two multiply-adds of the
 # distance expansion, one min) + 1 store.
 LABEL_OPS_PER_CELL = 22
@@ -278,6 +278,25 @@ def run_ours(args, w):
     kernel_launch_ms = {nm: float(np.mean(x)) for nm, x in per_kernel.items()}
     kernel_launches_per_step = {nm: len(x) / K for nm, x in per_kernel.items()}
 
+    # ---- event layer (not part of the step): vor_events on the last frame's lists
+    i32 = dict(dtype=torch.int32, device="cuda")
+    ev_bufs = [torch.empty(n, **i32) for _ in range(4)]
+    ev_m, ev_g = torch.zeros(1, **i32), torch.zeros(1, **i32)
+    last = (W_ + K - 1) & 1
+    def events():
+        v.vor_events(edges[1 - last], n_edges[1 - last], edges[last], n_edges[last], created, n_c, destroyed, n_d,
+                     ev_bufs[0], ev_bufs[1], ev_m, ev_g, ev_bufs[2], ev_bufs[3])
+    for _ in range(3):
+        events()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(10):
+        events()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    events_info = {"ms": e0.elapsed_time(e1) / 10, "events_number": int(ev_m.item()), "global_trigger": int(ev_g.item()),
+                   "api": "vor_events: local_trigger, eventsIndices, eventsCount past/now (PAPER.md:215-236)"}
+
     # ---- e2e: the same frames through vor_frame_host (host buffers, H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -313,7 +332,7 @@ def run_ours(args, w):
 
     hbm_peak, peak_src, sm_max_mhz = peaks()
     # Dominant kernel = label_cta_kernel (one launch per step).  It is bound by plain
-    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.8
+    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.9
     # derives (SMs x 128 lanes x max SM clock); algorithmic work = 22 integer ops per cell.
     lab_name = max((nm for nm in kernel_launch_ms if "label" in nm), key=lambda nm: kernel_launch_ms[nm])
     label_s = kernel_launch_ms[lab_name] * 1e-3
@@ -323,7 +342,7 @@ def run_ours(args, w):
                 "unit": "Tera int32 op/s", "frac": alu_ops / label_s / 1e12 / alu_peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(lab_name) if wr.name == "cfg5_throughput_stress" else None,
                 "launch_ms": kernel_launch_ms[lab_name],
-                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.8)",
+                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.9)",
                 "algorithmic": f"{LABEL_OPS_PER_CELL} int32 ops/cell x {cells_per_step} cells",
                 "hbm_view": {"achieved": 4.0 * cells_per_step / label_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
                              "frac": 4.0 * cells_per_step / label_s / 1e9 / hbm_peak,
@@ -360,6 +379,7 @@ def run_ours(args, w):
         "kernel_launch_ms": kernel_launch_ms, "kernel_launches_per_step": kernel_launches_per_step,
         "roofline": roofline,
         "rooflines_other": {k: r for k, r in others.items() if r},
+        "events": events_info,
         "clocks": clocks, "gpu_launches": int(launches),
     }
     if e2e:

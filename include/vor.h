@@ -112,6 +112,25 @@ int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
              uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
              int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
 
+/* ---- trigger and event counts: the paper's own outputs on top of the diff (PAPER.md:215-221
+ * §III.B.3 local_trigger / global_trigger; §III.B.4 eventsIndices / eventsNumber;
+ * PAPER.md:236 eventsCount for both triangulations).  All four lists are ascending unique key lists
+ * in ONE index space with labels < n_labels (site path: as given to / returned by vor_diff; keys
+ * with a label >= n_labels are ignored).  d_created / d_destroyed must be the diff of d_prev / d_now.
+ * Outputs, device memory owned by the caller:
+ *   d_trigger[n_labels]         1 if the vertex's adjacency row changed (endpoint of a created or
+ *                               destroyed edge), else 0
+ *   d_events_indices[n_labels]  the active vertices in ascending order (first *d_events_number entries)
+ *   d_events_number, d_global_trigger   device scalars (global_trigger = events_number > 0)
+ *   d_count_prev / d_count_now[n_labels]  for an active vertex: number of active vertices adjacent to
+ *                               it in the past / present edge list; 0 for inactive vertices. */
+int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+               const uint64_t* d_now, const int64_t* d_n_now,
+               const uint64_t* d_created, const int64_t* d_n_created,
+               const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int32_t n_labels,
+               int32_t* d_trigger, int32_t* d_events_indices, int32_t* d_events_number,
+               int32_t* d_global_trigger, int32_t* d_count_prev, int32_t* d_count_now, void* stream);
+
 /* ---- a6: bubble identification (§III.A: threshold -> two-valued variable ->
  * cluster labelling).  mask = above ? field > thr : field < thr (strict; NaN -> background).
  * 4-connected periodic components; d_ccl[c] = smallest linear index in c's component, or -1. */

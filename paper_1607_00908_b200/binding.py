@@ -33,6 +33,7 @@ SIGNATURES = {
     "vor_label": (C.c_int, [_P, _P, _P]),
     "vor_edges": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P]),
     "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
+    "vor_events": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, _P]),
     "field_threshold_ccl": (C.c_int, [_P, _P, C.c_float, C.c_int, _P, _P]),
     "field_centroids": (C.c_int, [_P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
     "match_sites": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P, _P]),
@@ -162,6 +163,16 @@ class Vor:
             _ptr(n_now, torch.int64), _ptr(p2n, torch.int32), _ptr(n2p, torch.int32),
             n_prev_labels, n_now_labels, _ptr(created, torch.int64), _ptr(destroyed, torch.int64), cap,
             _ptr(n_created, torch.int64), _ptr(n_destroyed, torch.int64), _stream()))
+
+    def vor_events(self, prev, n_prev, now, n_now, created, n_created, destroyed, n_destroyed,
+                   trigger, events_indices, events_number, global_trigger, count_prev, count_now):
+        n_labels = min(t.numel() for t in (trigger, events_indices, count_prev, count_now))
+        i64, i32 = torch.int64, torch.int32
+        self._check(self.lib.vor_events(
+            self.h, _ptr(prev, i64), _ptr(n_prev, i64), _ptr(now, i64), _ptr(n_now, i64),
+            _ptr(created, i64), _ptr(n_created, i64), _ptr(destroyed, i64), _ptr(n_destroyed, i64), n_labels,
+            _ptr(trigger, i32), _ptr(events_indices, i32), _ptr(events_number, i32), _ptr(global_trigger, i32),
+            _ptr(count_prev, i32), _ptr(count_now, i32), _stream()))
 
     # ---- field path
     def field_threshold_ccl(self, field, thr: float, above: bool, ccl):

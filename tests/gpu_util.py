@@ -58,6 +58,25 @@ def gpu_diff(v: Vor, prev, now, p2n=None, n2p=None):
     return u64(c, int(nc.item())).copy(), u64(d, int(nd.item())).copy()
 
 
+def gpu_events(v: Vor, prev, now, n):
+    """vor_diff then vor_events on host lists; returns the same dict as oracle.events()."""
+    mk = lambda a: dev(np.asarray(a, np.uint64).view(np.int64)) if len(a) else torch.empty(1, dtype=torch.int64, device="cuda")
+    dp, dn = mk(prev), mk(now)
+    i64 = dict(dtype=torch.int64, device="cuda"); i32 = dict(dtype=torch.int32, device="cuda")
+    npv, nnv = torch.tensor([len(prev)], **i64), torch.tensor([len(now)], **i64)
+    cap = max(1, len(prev) + len(now))
+    c, d = torch.empty(cap, **i64), torch.empty(cap, **i64)
+    nc, nd = torch.zeros(1, **i64), torch.zeros(1, **i64)
+    v.vor_diff(dp, npv, dn, nnv, c, d, nc, nd)
+    trig = torch.full((n,), -5, **i32); idx = torch.full((n,), -5, **i32)
+    cp = torch.full((n,), -5, **i32); cn = torch.full((n,), -5, **i32)
+    m, g = torch.full((1,), -5, **i32), torch.full((1,), -5, **i32)
+    v.vor_events(dp, npv, dn, nnv, c, nc, d, nd, trig, idx, m, g, cp, cn)
+    v.vor_sync_status()
+    return dict(trigger=trig.cpu().numpy(), events_indices=idx[:int(m.item())].cpu().numpy(),
+                count_prev=cp.cpu().numpy(), count_now=cn.cpu().numpy(), global_trigger=int(g.item()))
+
+
 def gpu_ccl(v: Vor, field, thr, above=True):
     f = dev(field.astype(np.float32).ravel())
     ccl = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")

@@ -406,6 +406,47 @@ def test_match_invariants_and_random(G):
     v.close()
 
 
+# ------------------------------------------------------------------ event layer (trigger, eventsIndices, eventsCount)
+def check_events(G, v, prev, now, n):
+    got, ref = G.gpu_events(v, prev, now, n), oracle.events(prev, now, n)
+    for k in ("trigger", "events_indices", "count_prev", "count_now"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert got["global_trigger"] == ref["global_trigger"]
+    return got
+
+
+def test_events_hand_random_and_golden(G):
+    v = make(64, 64)
+    common = [(0, 1), (1, 2), (2, 3), (0, 3), (0, 4), (1, 4), (2, 5), (3, 5), (4, 5)]
+    ev = check_events(G, v, pack(common + [(1, 3)]), pack(common + [(0, 2)]), 6)
+    assert ev["count_prev"].tolist() == [2, 3, 2, 3, 0, 0] and ev["count_now"].tolist() == [3, 2, 3, 2, 0, 0]
+    check_events(G, v, pack(common), pack(common), 6)                  # nothing happened
+    check_events(G, v, np.empty(0, np.uint64), pack([(0, 2)]), 3)      # empty past list
+    check_events(G, v, pack([(0, 1), (1, 2), (0, 2)]), pack([(0, 1), (1, 2)]), 3)
+    check_events(G, v, pack([(0, 1)]), pack([(0, 1)]), 1)              # n_labels below the labels: keys ignored
+    rng = np.random.default_rng(17)
+    for n in (2, 33, 1000, 5000):                                      # several batches and a ragged tail
+        i = rng.integers(0, n, 6 * n); j = rng.integers(0, n, 6 * n)
+        keep = i != j
+        a = np.unique((np.minimum(i, j)[keep].astype(np.uint64) << np.uint64(32)) | np.maximum(i, j)[keep].astype(np.uint64))
+        b = np.unique(np.concatenate([a[rng.random(len(a)) < 0.97], a[:5] + np.uint64(1) if len(a) > 5 else a]))
+        b = b[(b & np.uint64(0xffffffff)) < np.uint64(n)]
+        b = b[(b >> np.uint64(32)) < (b & np.uint64(0xffffffff))]
+        check_events(G, v, a, b, n)
+    v.close()
+    g = read_golden("rhombus_flip.txt")
+    L = g["L"][0]
+    v = make(L, 16)
+    lists = []
+    for h in (g["h_prev"][0], g["h_now"][0]):
+        sx, sy = rhombus_sites(L, h)
+        lists.append(G.gpu_edges(v, G.gpu_labels(v, sx, sy)))
+    ev = check_events(G, v, lists[0], lists[1], g["n_sites"][0])
+    assert ev["events_indices"].tolist() == g["events_indices"]
+    assert ev["count_prev"][:4].tolist() == g["count_prev"] and ev["count_now"][:4].tolist() == g["count_now"]
+    v.close()
+
+
 # ------------------------------------------------------------------ full size, bench.py's launch configuration
 def test_config5_full_size_two_frames(G):
     """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites) through the same calls, buffers
@@ -442,6 +483,17 @@ def test_config5_full_size_two_frames(G):
         rc, rd = oracle.diff(prev, e)
         assert np.array_equal(G.u64(created, int(n_c.item())), rc)
         assert np.array_equal(G.u64(destroyed, int(n_d.item())), rd)
+        if i == 1:                                  # event layer at full size, on the device-resident lists
+            i32 = dict(dtype=torch.int32, device="cuda")
+            trig, idx, cp, cn = (torch.empty(n, **i32) for _ in range(4))
+            m, g = torch.zeros(1, **i32), torch.zeros(1, **i32)
+            v.vor_events(edges[prv], n_edges[prv], edges[now], n_edges[now], created, n_c, destroyed, n_d,
+                         trig, idx, m, g, cp, cn)
+            v.vor_sync_status()
+            ev = oracle.events(prev, e, n)
+            assert np.array_equal(trig.cpu().numpy(), ev["trigger"]) and int(g.item()) == 1
+            assert np.array_equal(idx[:int(m.item())].cpu().numpy(), ev["events_indices"])
+            assert np.array_equal(cp.cpu().numpy(), ev["count_prev"]) and np.array_equal(cn.cpu().numpy(), ev["count_now"])
         prev = e
         del ref, got
     assert 2.9 * n < len(prev) < 3.0 * n            # E slightly below 3N (R6), as the survey's probe found
