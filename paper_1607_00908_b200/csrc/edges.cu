@@ -63,7 +63,7 @@ __device__ __forceinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_
 }
 
 // ------------------------------------------------------------------------------------ emit
-constexpr int kHashSlots = 2048;
+constexpr int kHashSlots = 1024;
 constexpr int kMaxProbe = 32;
 constexpr int kQueueCap = 32 + 256;     // < 32 pending + at most 8 pairs per lane per row
 
@@ -110,7 +110,7 @@ constexpr int kStrWarpsX = 2, kStrWarpsY = 4;
 constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
 constexpr int kStrThreads = 32 * kStrWarps;                     // 256
 constexpr int kStripCols = 128;
-constexpr int kStripRows = 64;                                  // rows per warp
+constexpr int kStripRows = 32;                                  // rows per warp
 constexpr int kPf = 4;                                          // rows in flight per lane
 constexpr int kRecCap = 96;                                     // < 32 pending + 2 rows x 32
 constexpr int kMultiCap = 64;                                   // < 32 pending + 32 per batch
@@ -170,7 +170,7 @@ __device__ __forceinline__ void hash_flush(const unsigned long long* table, cons
     }
 }
 
-__global__ void __launch_bounds__(kStrThreads, 3) edges_stream_kernel(const int32_t* __restrict__ labels,
+__global__ void __launch_bounds__(kStrThreads, 4) edges_stream_kernel(const int32_t* __restrict__ labels,
                                                                       int32_t L, const RowSet rs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     StreamShared& sh = *reinterpret_cast<StreamShared*>(smem_raw);
@@ -895,7 +895,7 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     rs.flags = ctx->d_flags;
     const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
     if (vec) {
-        static_assert(sizeof(StreamShared) <= 74 * 1024, "three CTAs per SM");
+        static_assert(sizeof(StreamShared) <= 55 * 1024, "four CTAs per SM");
         VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(StreamShared)));
         dim3 grid((L + kStrWarpsX * kStripCols - 1) / (kStrWarpsX * kStripCols),
