@@ -192,11 +192,16 @@ __global__ void __launch_bounds__(kStrThreads, 4) edges_stream_kernel(const int3
     auto process_multi = [&](int take) {
         mn -= take;
         const int32_t* __restrict__ r = mq + (mn + lane) * 9;
-#pragma unroll 1
-        for (int k = 0; k < 8; ++k) {
-            if (lane < take) {
-                const int32_t u = r[k < 4 ? k : k + 1], v = r[k < 4 ? k + 1 : k - 4];
-                if (u != v) hash_insert(u, v, sh.table, rs);
+        unsigned bits = 0;                             // bit k: pair k differs
+        if (lane < take) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) bits |= (unsigned)(r[k < 4 ? k : k + 1] != r[k < 4 ? k + 1 : k - 4]) << k;
+        }
+        while (__any_sync(full, bits != 0)) {          // every trip is dense over the lanes that still have pairs
+            if (bits) {
+                const int k = __ffs(bits) - 1;
+                bits &= bits - 1;
+                hash_insert(r[k < 4 ? k : k + 1], r[k < 4 ? k + 1 : k - 4], sh.table, rs);
             }
         }
         __syncwarp();
