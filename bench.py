@@ -315,16 +315,35 @@ def run_ours(args, w):
         for i in range(W_):
             v.vor_frame_host(hframes[i][0], hframes[i][1], hc, hd, cnt)
         barrier()
-        d2h = 0
         t0 = time.perf_counter()
         for k in range(K):
             v.vor_frame_host(hframes[W_ + k][0], hframes[W_ + k][1], hc, hd, cnt)
-            d2h += 8 * (int(cnt[1]) + int(cnt[2])) + 24
+        torch.cuda.synchronize()
+        secs_sync = max_over_ranks(time.perf_counter() - t0)
+        # pipelined: frame k+1 is submitted before frame k is collected, so the uploads and downloads
+        # (own copy streams) overlap the kernels; every copy is still inside the timed region
+        v.vor_frame_reset()
+        for i in range(W_):
+            v.vor_frame_submit(hframes[i][0], hframes[i][1])
+            v.vor_frame_collect(hc, hd, cnt)
+        barrier()
+        d2h = 0
+        t0 = time.perf_counter()
+        v.vor_frame_submit(hframes[W_][0], hframes[W_][1])
+        for k in range(1, K):
+            v.vor_frame_submit(hframes[W_ + k][0], hframes[W_ + k][1])
+            v.vor_frame_collect(hc, hd, cnt)
+            d2h += 8 * (int(cnt[1]) + int(cnt[2])) + 32
+        v.vor_frame_collect(hc, hd, cnt)
+        d2h += 8 * (int(cnt[1]) + int(cnt[2])) + 32
         torch.cuda.synchronize()
         secs = max_over_ranks(time.perf_counter() - t0)
         e2e = {"value": world * K * cells_per_step / secs, "unit": UNIT, "ms_per_step": 1e3 * secs / K,
                "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": d2h // K,
-               "api": "vor_frame_host (C ABI, pinned host buffers; label image stays on the device)"}
+               "api": "vor_frame_submit / vor_frame_collect (C ABI, pinned host buffers, two frames in flight; "
+                      "label image stays on the device)",
+               "sync_api_ms_per_step": 1e3 * secs_sync / K,
+               "sync_api": "vor_frame_host, one frame at a time (copies not overlapped)"}
 
     clocks = sampler.stop()
     if rank != 0:

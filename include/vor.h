@@ -165,6 +165,17 @@ int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_py, const in
 int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
                    uint64_t* h_created, uint64_t* h_destroyed, int64_t cap, int64_t* h_counts,
                    void* stream);
+/* Pipelined form of vor_frame_host for a stream of frames: vor_frame_submit() enqueues the upload
+ * (on a copy stream of the context), a1..a5 (on `stream`) and the download of the counts, and
+ * returns without waiting; vor_frame_collect() waits for the OLDEST frame in flight, downloads its
+ * created / destroyed lists (on a second copy stream) and returns them like vor_frame_host.  At most
+ * two frames may be in flight (a third submit -> VOR_ESTATE), so submit(k+1) before collect(k)
+ * overlaps frame k's downloads and frame k+1's upload with the kernels.  Page-locked caller buffers
+ * are used directly; the input arrays of a submitted frame must stay unchanged until it is
+ * collected.  Frames are diffed in submission order; vor_frame_reset() drops frames in flight. */
+int vor_frame_submit(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites, void* stream);
+int vor_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
+                      int64_t* h_counts);
 /* Same pipeline with DEVICE site arrays and no host copies or synchronisation: results stay in
  * context-owned device buffers (vor_frame_results).  bench.py's device-resident leg. */
 int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,

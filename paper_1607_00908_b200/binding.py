@@ -39,6 +39,8 @@ SIGNATURES = {
     "match_sites": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P, _P]),
     "vor_frame_host": (C.c_int, [_P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P]),
     "vor_frame_device": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
+    "vor_frame_submit": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
+    "vor_frame_collect": (C.c_int, [_P, _P, _P, C.c_int64, _P]),
     "vor_frame_reset": (C.c_int, [_P]),
     "vor_frame_results": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P)]),
 }
@@ -210,6 +212,16 @@ class Vor:
             self.h, h_sx.ctypes.data_as(_P), h_sy.ctypes.data_as(_P), len(h_sx),
             h_created.ctypes.data_as(_P), h_destroyed.ctypes.data_as(_P), cap,
             h_counts.ctypes.data_as(_P), _stream()))
+
+    def vor_frame_submit(self, h_sx, h_sy):
+        """Enqueue one frame (HOST numpy int32 arrays; keep them alive and unchanged until collected)."""
+        self._check(self.lib.vor_frame_submit(self.h, h_sx.ctypes.data_as(_P), h_sy.ctypes.data_as(_P),
+                                              len(h_sx), _stream()))
+
+    def vor_frame_collect(self, h_created, h_destroyed, h_counts):
+        cap = min(len(h_created), len(h_destroyed))
+        self._check(self.lib.vor_frame_collect(self.h, h_created.ctypes.data_as(_P),
+                                               h_destroyed.ctypes.data_as(_P), cap, h_counts.ctypes.data_as(_P)))
 
     def vor_frame_results(self):
         """Raw device pointers (ints) of the context-owned results: labels, edges, created,

@@ -97,6 +97,17 @@ struct vor_ctx {
     int64_t fr_cap;
     int fr_cur;                // index of the "now" buffer of the last frame; -1 = none
     int fr_have_prev;
+    // pipelined variant (vor_frame_submit / vor_frame_collect): two frames in flight, copies on own streams
+    int32_t* d_pp_sx[2];
+    int32_t* d_pp_sy[2];
+    uint64_t* d_pp_created[2];
+    uint64_t* d_pp_destroyed[2];
+    int64_t* d_pp_counts[2];   // [4]: n_edges, n_created, n_destroyed, sticky flags
+    int64_t* h_pp_counts[2];   // pinned [4]
+    int32_t* h_pp_sites[2];    // pinned staging [2 * max_sites] for pageable inputs
+    cudaStream_t pp_h2d, pp_d2h, pp_lst;   // uploads; counts (waits for the kernels); list downloads
+    cudaEvent_t pp_ev_in[2], pp_ev_done[2], pp_ev_cnt[2];
+    int64_t pp_head, pp_tail;  // frames submitted / collected
 
     int32_t* d_flags;          // [1] sticky error bits
     int num_sms;               // of the device the context lives on

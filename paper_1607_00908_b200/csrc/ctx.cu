@@ -85,6 +85,13 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_fr_nedges[0]); cudaFree(ctx->d_fr_nedges[1]);
     cudaFree(ctx->d_fr_created); cudaFree(ctx->d_fr_destroyed); cudaFree(ctx->d_fr_counts);
     cudaFreeHost(ctx->h_fr_counts); cudaFreeHost(ctx->h_fr_sites); cudaFreeHost(ctx->h_fr_lists);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(ctx->d_pp_sx[k]); cudaFree(ctx->d_pp_sy[k]); cudaFree(ctx->d_pp_created[k]);
+        cudaFree(ctx->d_pp_destroyed[k]); cudaFree(ctx->d_pp_counts[k]);
+        cudaFreeHost(ctx->h_pp_counts[k]); cudaFreeHost(ctx->h_pp_sites[k]);
+        if (ctx->pp_ev_in[k]) { cudaEventDestroy(ctx->pp_ev_in[k]); cudaEventDestroy(ctx->pp_ev_done[k]); cudaEventDestroy(ctx->pp_ev_cnt[k]); }
+    }
+    if (ctx->pp_h2d) { cudaStreamDestroy(ctx->pp_h2d); cudaStreamDestroy(ctx->pp_d2h); cudaStreamDestroy(ctx->pp_lst); }
     cudaFree(ctx->d_flags);
     if (ctx->prof_ev[0][0])
         for (int i = 0; i < kMaxProfLaunches; ++i)

@@ -6,8 +6,49 @@
 namespace {
 
 __global__ void gather_counts_kernel(const int64_t* __restrict__ n_edges, const int64_t* __restrict__ n_created,
-                                     const int64_t* __restrict__ n_destroyed, int64_t* __restrict__ out) {
-    out[0] = *n_edges; out[1] = *n_created; out[2] = *n_destroyed;
+                                     const int64_t* __restrict__ n_destroyed, const int32_t* __restrict__ flags,
+                                     int64_t* __restrict__ out) {
+    out[0] = *n_edges; out[1] = *n_created; out[2] = *n_destroyed; out[3] = *flags;
+}
+
+// a1..a5 for one frame on the context's label image and ping-pong edge lists; the flip lists and
+// the 4 counts go to the given buffers.
+int frame_compute(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
+                  uint64_t* d_created, uint64_t* d_destroyed, int64_t* d_counts, cudaStream_t stream) {
+    int rc;
+    const int now = ctx->fr_cur < 0 ? 0 : 1 - ctx->fr_cur, prev = 1 - now;
+    if (ctx->fr_cur < 0) VOR_CUDA(cudaMemsetAsync(ctx->d_fr_nedges[prev], 0, sizeof(int64_t), stream));
+    if ((rc = vor_build_cells(ctx, d_sx, d_sy, n_sites, stream)) != VOR_OK) return rc;
+    if ((rc = vor_label(ctx, ctx->d_fr_labels, stream)) != VOR_OK) return rc;
+    if ((rc = vor_edges(ctx, ctx->d_fr_labels, ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now],
+                        stream)) != VOR_OK) return rc;
+    if ((rc = vor_diff(ctx, ctx->d_fr_edges[prev], ctx->d_fr_nedges[prev], ctx->d_fr_edges[now],
+                       ctx->d_fr_nedges[now], nullptr, nullptr, 0, 0, d_created, d_destroyed, ctx->fr_cap,
+                       &d_counts[1], &d_counts[2], stream)) != VOR_OK) return rc;
+    VOR_LAUNCH(gather_counts_kernel, 1, 1, 0, stream, ctx->d_fr_nedges[now], &d_counts[1], &d_counts[2],
+               ctx->d_flags, d_counts);
+    ctx->fr_cur = now;
+    return VOR_OK;
+}
+
+int ensure_pipe_buffers(vor_ctx* ctx) {
+    if (ctx->pp_h2d) return VOR_OK;
+    for (int k = 0; k < 2; ++k) {
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_pp_sx[k], (size_t)ctx->max_sites * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_pp_sy[k], (size_t)ctx->max_sites * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_pp_created[k], (size_t)ctx->fr_cap * sizeof(uint64_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_pp_destroyed[k], (size_t)ctx->fr_cap * sizeof(uint64_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_pp_counts[k], 4 * sizeof(int64_t)));
+        VOR_CUDA(cudaMallocHost((void**)&ctx->h_pp_counts[k], 4 * sizeof(int64_t)));
+        VOR_CUDA(cudaMallocHost((void**)&ctx->h_pp_sites[k], 2 * (size_t)ctx->max_sites * sizeof(int32_t)));
+        VOR_CUDA(cudaEventCreateWithFlags(&ctx->pp_ev_in[k], cudaEventDisableTiming));
+        VOR_CUDA(cudaEventCreateWithFlags(&ctx->pp_ev_done[k], cudaEventDisableTiming));
+        VOR_CUDA(cudaEventCreateWithFlags(&ctx->pp_ev_cnt[k], cudaEventDisableTiming));
+    }
+    VOR_CUDA(cudaStreamCreateWithFlags(&ctx->pp_d2h, cudaStreamNonBlocking));
+    VOR_CUDA(cudaStreamCreateWithFlags(&ctx->pp_lst, cudaStreamNonBlocking));
+    VOR_CUDA(cudaStreamCreateWithFlags(&ctx->pp_h2d, cudaStreamNonBlocking));
+    return VOR_OK;
 }
 
 // Page-locked host memory (cudaMallocHost / cudaHostRegister / torch pin_memory) can be the source or
@@ -47,6 +88,12 @@ int ensure_frame_buffers(vor_ctx* ctx) {
 extern "C" int vor_frame_reset(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
     ctx->fr_cur = -1;
+    if (ctx->pp_h2d) {                                   // drop frames still in flight
+        cudaStreamSynchronize(ctx->pp_h2d);
+        cudaStreamSynchronize(ctx->pp_d2h);
+        cudaStreamSynchronize(ctx->pp_lst);
+    }
+    ctx->pp_tail = ctx->pp_head;
     return VOR_OK;
 }
 
@@ -55,21 +102,8 @@ extern "C" int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t
     if (!ctx) return VOR_EINVAL;
     int rc = ensure_frame_buffers(ctx);
     if (rc != VOR_OK) return rc;
-    cudaStream_t stream = (cudaStream_t)stream_;
-    const int now = ctx->fr_cur < 0 ? 0 : 1 - ctx->fr_cur, prev = 1 - now;
-    if (ctx->fr_cur < 0) VOR_CUDA(cudaMemsetAsync(ctx->d_fr_nedges[prev], 0, sizeof(int64_t), stream));
-    if ((rc = vor_build_cells(ctx, d_sx, d_sy, n_sites, stream)) != VOR_OK) return rc;
-    if ((rc = vor_label(ctx, ctx->d_fr_labels, stream)) != VOR_OK) return rc;
-    if ((rc = vor_edges(ctx, ctx->d_fr_labels, ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now],
-                        stream)) != VOR_OK) return rc;
-    if ((rc = vor_diff(ctx, ctx->d_fr_edges[prev], ctx->d_fr_nedges[prev], ctx->d_fr_edges[now],
-                       ctx->d_fr_nedges[now], nullptr, nullptr, 0, 0, ctx->d_fr_created,
-                       ctx->d_fr_destroyed, ctx->fr_cap, &ctx->d_fr_counts[1], &ctx->d_fr_counts[2],
-                       stream)) != VOR_OK) return rc;
-    VOR_LAUNCH(gather_counts_kernel, 1, 1, 0, stream, ctx->d_fr_nedges[now], &ctx->d_fr_counts[1],
-               &ctx->d_fr_counts[2], ctx->d_fr_counts);
-    ctx->fr_cur = now;
-    return VOR_OK;
+    return frame_compute(ctx, d_sx, d_sy, n_sites, ctx->d_fr_created, ctx->d_fr_destroyed, ctx->d_fr_counts,
+                         (cudaStream_t)stream_);
 }
 
 extern "C" int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
@@ -133,5 +167,76 @@ extern "C" int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const u
     if (d_created) *d_created = ctx->d_fr_created;
     if (d_destroyed) *d_destroyed = ctx->d_fr_destroyed;
     if (d_counts) *d_counts = ctx->d_fr_counts;
+    return VOR_OK;
+}
+
+extern "C" int vor_frame_submit(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
+                                void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!h_sx || !h_sy) return vor_fail(ctx, VOR_EINVAL, "vor_frame_submit: null pointer");
+    if (n_sites < 1 || n_sites > ctx->max_sites)
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_submit: n_sites out of range");
+    int rc = ensure_frame_buffers(ctx);
+    if (rc != VOR_OK) return rc;
+    if ((rc = ensure_pipe_buffers(ctx)) != VOR_OK) return rc;
+    if (ctx->pp_head - ctx->pp_tail >= 2)
+        return vor_fail(ctx, VOR_ESTATE, "vor_frame_submit: two frames in flight, collect one first");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int s = (int)(ctx->pp_head & 1);
+    // inputs: own stream, so that the upload overlaps the previous frame's kernels; the slot's device
+    // buffers were last read by frame head-2, which has been collected, hence finished
+    const int32_t* src_x = h_sx;
+    const int32_t* src_y = h_sy;
+    if (!is_pinned(h_sx) || !is_pinned(h_sy)) {
+        memcpy(ctx->h_pp_sites[s], h_sx, (size_t)n_sites * sizeof(int32_t));
+        memcpy(ctx->h_pp_sites[s] + ctx->max_sites, h_sy, (size_t)n_sites * sizeof(int32_t));
+        src_x = ctx->h_pp_sites[s]; src_y = ctx->h_pp_sites[s] + ctx->max_sites;
+    }
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_pp_sx[s], src_x, (size_t)n_sites * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->pp_h2d));
+    VOR_CUDA(cudaMemcpyAsync(ctx->d_pp_sy[s], src_y, (size_t)n_sites * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->pp_h2d));
+    VOR_CUDA(cudaEventRecord(ctx->pp_ev_in[s], ctx->pp_h2d));
+    VOR_CUDA(cudaStreamWaitEvent(stream, ctx->pp_ev_in[s], 0));
+    if ((rc = frame_compute(ctx, ctx->d_pp_sx[s], ctx->d_pp_sy[s], n_sites, ctx->d_pp_created[s],
+                            ctx->d_pp_destroyed[s], ctx->d_pp_counts[s], stream)) != VOR_OK) return rc;
+    VOR_CUDA(cudaEventRecord(ctx->pp_ev_done[s], stream));
+    VOR_CUDA(cudaStreamWaitEvent(ctx->pp_d2h, ctx->pp_ev_done[s], 0));
+    VOR_CUDA(cudaMemcpyAsync(ctx->h_pp_counts[s], ctx->d_pp_counts[s], 4 * sizeof(int64_t), cudaMemcpyDeviceToHost, ctx->pp_d2h));
+    VOR_CUDA(cudaEventRecord(ctx->pp_ev_cnt[s], ctx->pp_d2h));
+    ctx->pp_head++;
+    return VOR_OK;
+}
+
+extern "C" int vor_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
+                                 int64_t* h_counts) {
+    if (!ctx) return VOR_EINVAL;
+    if (!h_counts || cap < 0 || (cap > 0 && (!h_created || !h_destroyed)))
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_collect: null pointer or negative capacity");
+    if (!ctx->pp_h2d || ctx->pp_tail == ctx->pp_head)
+        return vor_fail(ctx, VOR_ESTATE, "vor_frame_collect: no frame in flight");
+    const int s = (int)(ctx->pp_tail & 1);
+    VOR_CUDA(cudaEventSynchronize(ctx->pp_ev_cnt[s]));
+    const int64_t* c = ctx->h_pp_counts[s];
+    h_counts[0] = c[0]; h_counts[1] = c[1]; h_counts[2] = c[2];
+    int64_t nc = c[1] < ctx->fr_cap ? c[1] : ctx->fr_cap, nd = c[2] < ctx->fr_cap ? c[2] : ctx->fr_cap;
+    if (nc > cap) nc = cap;
+    if (nd > cap) nd = cap;
+    const bool direct = (nc == 0 || is_pinned(h_created)) && (nd == 0 || is_pinned(h_destroyed));
+    uint64_t* dst_c = direct ? h_created : ctx->h_fr_lists;
+    uint64_t* dst_d = direct ? h_destroyed : ctx->h_fr_lists + ctx->fr_cap;
+    // own stream: pp_d2h already holds the wait for the NEXT frame's kernels
+    if (nc > 0) VOR_CUDA(cudaMemcpyAsync(dst_c, ctx->d_pp_created[s], (size_t)nc * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->pp_lst));
+    if (nd > 0) VOR_CUDA(cudaMemcpyAsync(dst_d, ctx->d_pp_destroyed[s], (size_t)nd * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->pp_lst));
+    VOR_CUDA(cudaStreamSynchronize(ctx->pp_lst));
+    if (!direct) {
+        if (nc > 0) memcpy(h_created, dst_c, (size_t)nc * sizeof(uint64_t));
+        if (nd > 0) memcpy(h_destroyed, dst_d, (size_t)nd * sizeof(uint64_t));
+    }
+    ctx->pp_tail++;
+    if (c[3] != 0) {                                     // a kernel of this (or an earlier) frame latched an overflow
+        VOR_CUDA(cudaDeviceSynchronize());
+        return vor_sync_status(ctx, nullptr);
+    }
+    if (c[1] > cap || c[2] > cap)
+        return vor_fail(ctx, VOR_ECAPACITY, "vor_frame_collect: created/destroyed list larger than cap");
     return VOR_OK;
 }

@@ -288,6 +288,52 @@ def test_frame_host_sequence_matches_oracle(G, cfg, L, nfr):
     v.close()
 
 
+@pytest.mark.parametrize("pin", [False, True])
+def test_frame_pipeline_submit_collect(G, pin):
+    """Two frames in flight (submit k+1 before collect k): same results, in order, as the oracle;
+    a third submit and a collect with nothing in flight are refused."""
+    from paper_1607_00908_b200.binding import VorError, VOR_ESTATE
+    w = W.scaled(5, 1024)
+    v = make(w.L, w.n_sites)
+    cap = 8 * w.n_sites + 64
+    def buf(n, dt):
+        return torch.empty(n, dtype=dt, pin_memory=True).numpy() if pin else np.empty(n, torch.empty(0, dtype=dt).numpy().dtype)
+    hc, hd = buf(cap, torch.int64).view(np.uint64), buf(cap, torch.int64).view(np.uint64)
+    cnt = np.zeros(3, np.int64)
+    frames = []
+    for sx, sy in w.frames(5):
+        px, py = buf(w.n_sites, torch.int32), buf(w.n_sites, torch.int32)
+        px[:] = sx; py[:] = sy
+        frames.append((px, py))
+    refs, prev = [], np.empty(0, np.uint64)
+    for sx, sy in frames:
+        e = oracle.edges(oracle.label_cells(w.L, sx, sy, w.bucket_cells))
+        refs.append((e,) + oracle.diff(prev, e))
+        prev = e
+    with pytest.raises(VorError) as ex:
+        v.vor_frame_collect(hc, hd, cnt)
+    assert ex.value.status == VOR_ESTATE
+    def collect(k):
+        v.vor_frame_collect(hc, hd, cnt)
+        e, rc, rd = refs[k]
+        assert cnt.tolist() == [len(e), len(rc), len(rd)], k
+        assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd), k
+    v.vor_frame_submit(*frames[0])
+    for k in range(1, len(frames)):
+        v.vor_frame_submit(*frames[k])
+        if k == 1:
+            with pytest.raises(VorError) as ex:
+                v.vor_frame_submit(*frames[2])
+            assert ex.value.status == VOR_ESTATE
+        collect(k - 1)
+    collect(len(frames) - 1)
+    # the synchronous call continues the same sequence (same previous edge list)
+    sx, sy = frames[-1]
+    v.vor_frame_host(sx, sy, hc, hd, cnt)
+    assert cnt.tolist() == [len(refs[-1][0]), 0, 0]
+    v.close()
+
+
 # ------------------------------------------------------------------ field path (a6..a8)
 def check_field_frame(G, v, field, thr, min_size, above=True):
     ref_ccl = oracle.threshold_ccl(field, thr, above)
