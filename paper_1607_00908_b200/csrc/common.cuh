@@ -182,6 +182,6 @@ inline int vor_coop_grid(vor_ctx* ctx, int slot, const void* func, int threads, 
 // internal entry points shared between translation units
 int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n_in, int key_bits,
                          uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
-                         cudaStream_t stream);
+                         int64_t n_hint /* expected number of keys, 0 = unknown */, cudaStream_t stream);
 int vor_reset_rows(vor_ctx* ctx);
 int vor_label_bits(const vor_ctx* ctx);

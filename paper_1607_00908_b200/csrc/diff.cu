@@ -227,14 +227,16 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
                    n_prev_labels, ctx->d_keys_a, ctx->max_raw_keys,
                    (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
         int rc = vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits, ctx->d_tr_prev,
-                                      ctx->max_raw_keys, &ctx->d_tr_counts[0], FLAG_RAWKEY_OVERFLOW, stream);
+                                      ctx->max_raw_keys, &ctx->d_tr_counts[0], FLAG_RAWKEY_OVERFLOW,
+                                      4 * (int64_t)n_prev_labels, stream);
         if (rc != VOR_OK) return rc;
         // filtered now -> d_keys_a -> sort/unique -> d_tr_now
         VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, sizeof(int64_t), stream));
         VOR_LAUNCH(filter_now_kernel, 4 * kNumSMs, 256, 0, stream, d_now, d_n_now, d_n2p, n_now_labels,
                    ctx->d_keys_a, ctx->max_raw_keys, (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
         rc = vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits, ctx->d_tr_now,
-                                  ctx->max_raw_keys, &ctx->d_tr_counts[1], FLAG_RAWKEY_OVERFLOW, stream);
+                                  ctx->max_raw_keys, &ctx->d_tr_counts[1], FLAG_RAWKEY_OVERFLOW,
+                                  4 * (int64_t)n_now_labels, stream);
         if (rc != VOR_OK) return rc;
         P = ctx->d_tr_prev; nP = &ctx->d_tr_counts[0];
         N = ctx->d_tr_now;  nN = &ctx->d_tr_counts[1];

@@ -870,10 +870,15 @@ __global__ void __launch_bounds__(kSortThreads) sort_unique_kernel(const SortUni
 // each 32-bit half.  Uses ctx->d_keys_b as the pong buffer.  One cooperative launch.
 int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n_in, int key_bits,
                          uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
-                         cudaStream_t stream) {
+                         int64_t n_hint, cudaStream_t stream) {
     SortUniqueParams p{d_keys_in_a, ctx->d_keys_b, d_n_in, ctx->max_raw_keys, key_bits, ctx->d_hist,
                        ctx->d_blk_count, d_out, cap, d_n_out, ctx->d_flags, flag_bit};
-    const int grid = vor_coop_grid(ctx, 1, (const void*)sort_unique_kernel, kSortThreads, 1);
+    int grid = vor_coop_grid(ctx, 1, (const void*)sort_unique_kernel, kSortThreads, 1);
+    // short lists: fewer blocks make the grid synchronisations cheaper (any grid size is correct)
+    if (n_hint > 0) {
+        const int64_t want = (n_hint + kSubTile - 1) / kSubTile;
+        if (want < grid) grid = want < 1 ? 1 : (int)want;
+    }
     VOR_LAUNCH_COOP(sort_unique_kernel, grid, kSortThreads, stream, (void*)&p);
     return VOR_OK;
 }
