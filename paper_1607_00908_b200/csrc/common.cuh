@@ -54,6 +54,12 @@ struct vor_ctx {
     int4* d_sorted;            // [max_sites]  (x, y, original index, bucket)
     int32_t* d_scan_part;      // scratch for device scans
 
+    int2* d_lab_fail;          // CTA label path: quadrants whose bound was not proven (x0, y0), lazily sized
+    int32_t* d_lab_fail_n;     // their number: two device scalars used alternately (the fix-up kernel of one
+                               //   call zeroes the other call's counter, so no memset is needed)
+    int32_t lab_fail_cap;
+    int lab_fail_turn;
+
     // ---- edges (a3/a4)
     uint32_t* d_rows;          // [max_sites * kRowStride] per-site lists of larger-index neighbours
     uint32_t* d_row_cnt;       // [max_sites] entries appended to each row; all 0 between calls (the

@@ -76,6 +76,7 @@ int vor_destroy(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
     cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
     cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
+    cudaFree(ctx->d_lab_fail); cudaFree(ctx->d_lab_fail_n);
     cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
     cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts);
     cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);

@@ -48,6 +48,10 @@ struct LabelParams {
     int32_t halo_fast;         // halo of the quadrant fast path, fixed point
     int32_t r_quad;            // ceil(radius of a quadrant's cell-centre box), fixed point
     uint32_t div_m, div_s1, div_s2;   // floor(x / w) for 0 <= x < 2^32 (Granlund-Montgomery)
+    int2* fail_items;          // CTA path: quadrants left to label_fixup_kernel
+    int32_t* fail_count;
+    int32_t* fail_count_next;  // counter of the next call: zeroed by label_fixup_kernel
+    int32_t fail_cap;
 };
 
 __device__ __forceinline__ int32_t div_w(const LabelParams& p, int32_t x /* >= 0 */) {
@@ -770,8 +774,15 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
         const int32_t cnt = sh.count[q];
         int32_t* __restrict__ out = labels + (int64_t)y0 * p.L + x;
         if (cnt < 0) {
-            for (int j = 0; j < 8; ++j)
-                if (y0 + j < p.L) out[(int64_t)j * p.L] = label_cell_general(p, x, y0 + j);
+            // not proven: the quadrant goes to label_fixup_kernel (one warp per quadrant, adaptive
+            // halo).  The list holds every quadrant of the lattice, or is disabled (fail_cap == 0) and
+            // the cells take the general search here; the quadrant's first lane is always in range.
+            if (p.fail_cap > 0) {
+                if ((lane & 7) == 0) p.fail_items[atomicAdd(p.fail_count, 1)] = make_int2(x, y0);
+            } else {
+                for (int j = 0; j < 8; ++j)
+                    if (y0 + j < p.L) out[(int64_t)j * p.L] = label_cell_general(p, x, y0 + j);
+            }
             continue;
         }
         const int32_t n = cnt & (kUnpackedFlag - 1);
@@ -850,6 +861,28 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelPara
     }
 }
 
+// Second pass of the CTA path: the quadrants whose bound label_cta_kernel could not prove (sparse or
+// clustered sites, voids wider than its halo).  One warp per 8 x 8 quadrant: the generic tile code
+// with its adaptive halo, then the general search.
+__global__ void __launch_bounds__(kWarpsPerCta * 32) label_fixup_kernel(LabelParams p, int32_t* __restrict__ labels) {
+    constexpr int HX = FP_HALF * 7;
+    __shared__ WarpScratch scratch[kWarpsPerCta];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t n = min(*p.fail_count, p.fail_cap);
+    if (blockIdx.x == 0 && threadIdx.x == 0) *p.fail_count_next = 0;
+    for (int32_t i = blockIdx.x * kWarpsPerCta + wid; i < n; i += gridDim.x * kWarpsPerCta) {
+        const int2 it = p.fail_items[i];
+        const int32_t tx0 = it.x, ty0 = it.y;
+        __syncwarp();
+        if (tile_generic<8, 8>(p, scratch[wid], lane, tx0, ty0, FP_ONE * tx0 + FP_HALF + HX,
+                               FP_ONE * ty0 + FP_HALF + HX, labels)) continue;
+        const int32_t x = tx0 + (lane & 7), yb = ty0 + (lane >> 3) * 2;
+#pragma unroll 1
+        for (int j = 0; j < 2; ++j)
+            if (x < p.L && yb + j < p.L) labels[(int64_t)(yb + j) * p.L + x] = label_cell_general(p, x, yb + j);
+    }
+}
+
 }  // namespace
 
 extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
@@ -860,6 +893,7 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     LabelParams p;
     p.L = ctx->L; p.P = (int32_t)ctx->P; p.nb = ctx->nb; p.w = ctx->w; p.n = ctx->n_sites;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
+    p.fail_items = nullptr; p.fail_count = nullptr; p.fail_count_next = nullptr; p.fail_cap = 0;
     const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_sites);   // cells
     int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8, 4 wide 32x16, 5 CTA
     if (path == 0) path = spacing >= 7.0 ? 5 : (spacing >= 4.0 ? 3 : 1);
@@ -889,8 +923,25 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     }
     const int use_fast = ctx->label_fast_off ? 0 : 1;
     if (path == 5) {
+        if (!ctx->d_lab_fail) {
+            const int64_t q = (int64_t)((ctx->L + 7) / 8) * ((ctx->L + 7) / 8);
+            ctx->lab_fail_cap = q <= (1 << 24) ? (int32_t)q : 0;      // every quadrant fits, or no list at all
+            VOR_CUDA(cudaMalloc((void**)&ctx->d_lab_fail, (size_t)(ctx->lab_fail_cap + 1) * sizeof(int2)));
+            VOR_CUDA(cudaMalloc((void**)&ctx->d_lab_fail_n, 2 * sizeof(int32_t)));
+            VOR_CUDA(cudaMemsetAsync(ctx->d_lab_fail_n, 0, 2 * sizeof(int32_t), stream));
+        }
+        p.fail_items = ctx->d_lab_fail; p.fail_cap = ctx->lab_fail_cap;
+        p.fail_count = ctx->d_lab_fail_n + ctx->lab_fail_turn;
+        p.fail_count_next = ctx->d_lab_fail_n + (1 - ctx->lab_fail_turn);
+        ctx->lab_fail_turn = 1 - ctx->lab_fail_turn;
         dim3 grid((ctx->L + 8 * kCtaQX - 1) / (8 * kCtaQX), (ctx->L + 8 * kCtaQY - 1) / (8 * kCtaQY));
         VOR_LAUNCH(label_cta_kernel, grid, kCtaThreads, 0, stream, p, d_labels);
+        // second pass over the unproven quadrants with the 8 x 8 tile geometry
+        LabelParams p8 = p;
+        const double h8 = 128.0 * 7;
+        p8.r_tile = (int32_t)ceil(sqrt(2.0 * h8 * h8));
+        p8.halo0 = p8.r_tile + (int32_t)(0.75 * spacing * FP_ONE);
+        VOR_LAUNCH(label_fixup_kernel, 4 * ctx->num_sms, kWarpsPerCta * 32, 0, stream, p8, d_labels);
         return VOR_OK;
     }
     if (path == 4) {
