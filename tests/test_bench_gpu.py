@@ -1,0 +1,48 @@
+"""-m gpu: bench.py's contract on a reduced copy of config 5 (same density and structure): one JSON line
+with the keys the driver reads, a live roofline, an end-to-end leg with real copies, the oracle timed
+beside it, and kernels really launched."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def run_bench(*extra):
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", *extra],
+                       capture_output=True, text=True, timeout=900, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1, lines
+    return json.loads(lines[0])
+
+
+def test_bench_line_site_path():
+    d = run_bench("--workload", "cfg5@2048")
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches"):
+        assert k in d, k
+    assert d["n_gpus"] == 1 and d["steps"] == 3 and d["value"] > 0 and d["vs_baseline"] is None
+    assert d["config"]["workload"].startswith("cfg5") and d["data"] == "synthetic"
+    r = d["roofline"]
+    assert r["bound"] in ("hbm", "tensor", "alu") and 0 < r["frac"] < 1.5 and r["peak"] > 0 and "label" in r["kernel"]
+    assert d["rooflines_other"]["edges_stream_kernel"]["bound"] == "hbm"
+    assert d["gpu_launches"] >= 3 * 8                       # a1..a5 launch at least 8 kernels per step
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 8 * d["config"]["n_sites"] and e["d2h_bytes_per_step"] > 0
+    assert e["value"] <= 1.05 * d["value"]                  # copies cannot make it faster than device-resident
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and d["value"] > c["value"]
+    assert d["counts"]["n_edges"] > 2.9 * d["config"]["n_sites"]
+    assert d["events"]["global_trigger"] == 1
+
+
+def test_bench_line_field_path():
+    d = run_bench("--workload", "cfg3")
+    assert d["config"]["workload"].startswith("cfg3") and d["value"] > 0 and d["gpu_launches"] > 0
+    assert set(d["kernel_ms"]) == {"threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"}
+    assert d["roofline"]["bound"] == "hbm" and d["config"]["components"] > 1000
