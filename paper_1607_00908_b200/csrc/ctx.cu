@@ -31,7 +31,7 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     if (max_raw_keys > worst) max_raw_keys = worst;
     ctx->max_raw_keys = max_raw_keys;
     ctx->bucket_occ_x100 = 100;
-    ctx->label_halo_x100 = 90;
+    ctx->label_halo_x100 = 120;
     ctx->row_slots = kRowStride;
     if (const char* e = getenv("VOR_BUCKET_OCC_X100")) ctx->bucket_occ_x100 = atoll(e);
     ctx->fr_cur = -1;

@@ -631,6 +631,7 @@ struct CtaShared {
     int4 list[kListCap][kCtaQ];                       // [k][quadrant]: conflict-free across quadrants
     int4 tmp[kListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
     int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
+    int32_t nkept;                                    // gathered sites kept (inside the exact rectangle)
 };
 
 // Returns the number of gathered sites (0 = region unusable).  Region bounds relative to the CTA
@@ -644,9 +645,12 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
     const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
     const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
     if (ncols * p.w > half || nrows * p.w > half) return 0;
-    R[0] = q0 * p.w - cxm; R[1] = (q1 + 1) * p.w - cxm;
-    R[2] = r0 * p.w - cym; R[3] = (r1 + 1) * p.w - cym;
-    if (-R[0] > kCtaMaxExtent || R[1] > kCtaMaxExtent || -R[2] > kCtaMaxExtent || R[3] > kCtaMaxExtent) return 0;
+    // the buckets cover more than asked for; only the sites inside the exact rectangle
+    // [-HX-H, HX+H] x [-HY-H, HY+H] are kept (shorter lists for every quadrant), so that rectangle is
+    // the region the coverage test may rely on: R = {x lower (inclusive), x upper (exclusive), y ...}
+    R[0] = -(HX + H); R[1] = HX + H + 1;
+    R[2] = -(HY + H); R[3] = HY + H + 1;
+    if (R[1] > kCtaMaxExtent || R[3] > kCtaMaxExtent) return 0;
     const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
     const bool split = a0 + ncols > p.nb;
     const int32_t nseg = split ? 2 * nrows : nrows;
@@ -672,20 +676,32 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
     const int32_t total = __shfl_sync(full, inc, 31);
     if (total > kCtaCapSites) return 0;
     const int32_t exc = inc - cnt;
+    if (threadIdx.x == 0) sh.nkept = 0;
+    __syncthreads();
     if (32 * wid < total) {                            // warp-uniform: this warp owns items [32 wid, 32 wid + 32)
         const int32_t i = 32 * wid + lane;             // this thread's item
         int32_t seg = 0;
         for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= i);
         const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
+        int32_t rx = 0, ry = 0, idx = 0;
+        bool keep = false;
         if (i < total) {
             const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
-            int32_t rx = s.x - cxm, ry = s.y - cym;
+            rx = s.x - cxm; ry = s.y - cym; idx = s.z;
             rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
             ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
-            sh.sx[i] = rx; sh.sy[i] = ry; sh.si[i] = s.z;
+            keep = abs(rx) <= HX + H && abs(ry) <= HY + H;
+        }
+        const unsigned ball = __ballot_sync(full, keep);
+        int32_t base = 0;
+        if (lane == 0 && ball) base = atomicAdd(&sh.nkept, __popc(ball));
+        base = __shfl_sync(full, base, 0);
+        if (keep) {
+            const int32_t pos = base + __popc(ball & ((1u << lane) - 1u));
+            sh.sx[pos] = rx; sh.sy[pos] = ry; sh.si[pos] = idx;
         }
     }
-    return total;
+    return -1;                                         // the caller reads sh.nkept after its barrier
 }
 
 // 4 consecutive lanes (sub = 0..3) build the list of quadrant q; qcx, qcy: its centre relative to the
@@ -750,9 +766,10 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
         for (int attempt = 0; attempt < 2; ++attempt) {
             int32_t R[4] = {0, 0, 0, 0};
             const int32_t H = attempt == 0 ? p.halo_fast : 2 * p.halo_fast + p.w;
-            const int32_t ns = cta_gather(p, sh, lane, wid, FP_ONE * X0 + FP_HALF + HX,
-                                          FP_ONE * Y0 + FP_HALF + HY, H, R);
+            const int32_t got = cta_gather(p, sh, lane, wid, FP_ONE * X0 + FP_HALF + HX,
+                                           FP_ONE * Y0 + FP_HALF + HY, H, R);
             __syncthreads();
+            const int32_t ns = got ? sh.nkept : 0;
             cta_build_list(p, sh, q, sub, ns, R, 8 * FP_ONE * qx + QHW - HX, 8 * FP_ONE * qy + QHW - HY, active);
             __syncthreads();
             active = sh.count[q] < 0;
