@@ -226,6 +226,26 @@ __global__ void __launch_bounds__(kCompThreads) comp_write_kernel(Pred pred, Sin
 }
 
 // ------------------------------------------------------------------------------------ a7: centroids
+// floor(x / d) for 0 <= x < 2^32 with one multiply-high and two shifts (Granlund-Montgomery); the
+// accumulation splits two linear indices per cell into (x, y).
+struct FastDiv {
+    uint32_t m, s1, s2, d;
+    __device__ __forceinline__ uint32_t div(uint32_t x) const {
+        const uint32_t t = __umulhi(m, x);
+        return (t + ((x - t) >> s1)) >> s2;
+    }
+};
+inline FastDiv make_fastdiv(uint32_t d) {
+    uint32_t l = 0;
+    while (((uint64_t)1 << l) < d) ++l;
+    FastDiv f;
+    f.m = (uint32_t)((((uint64_t)1 << 32) * (((uint64_t)1 << l) - d)) / d + 1);
+    f.s1 = l < 1 ? l : 1;
+    f.s2 = l > 0 ? l - 1 : 0;
+    f.d = d;
+    return f;
+}
+
 struct RootPred {
     const int32_t* ccl;
     int64_t n;
@@ -249,14 +269,17 @@ struct RootSink {
 };
 
 __global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const int32_t* __restrict__ rank,
-                                  int32_t L, unsigned long long* __restrict__ acc, int32_t max_comp) {
+                                  int32_t L, FastDiv fd, unsigned long long* __restrict__ acc, int32_t max_comp) {
     const int64_t n = (int64_t)L * L;
     const int64_t nround = (n + 31) / 32 * 32;     // keep warps converged for the warp collectives
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (int64_t)gridDim.x * blockDim.x) {
         const int32_t r = i < n ? ccl[i] : -1;
-        const unsigned peers = __match_any_sync(0xffffffffu, r);
+        // most warps see one value (background or the inside of a bubble): no match needed then
+        const bool uniform = __all_sync(0xffffffffu, r == __shfl_sync(0xffffffffu, r, 0));
+        const unsigned peers = uniform ? 0xffffffffu : __match_any_sync(0xffffffffu, r);
         if (r < 0) continue;                        // whole peer group leaves together
-        const int32_t x = (int32_t)(i % L), y = (int32_t)(i / L), xr = r % L, yr = r / L;
+        const int32_t y = (int32_t)fd.div((uint32_t)i), x = (int32_t)i - y * L;
+        const int32_t yr = (int32_t)fd.div((uint32_t)r), xr = r - yr * L;
         int32_t dx = x - xr;
         if (2 * dx >= L) dx -= L; else if (2 * dx < -L) dx += L;
         int32_t dy = y - yr;
@@ -484,7 +507,7 @@ extern "C" int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_s
     VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kCompGrid, kCompThreads, 0, stream, rp, rs,
                ctx->d_blk_count);
     const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
-    VOR_LAUNCH(accumulate_kernel, grid, 256, 0, stream, d_ccl, ctx->d_rank, ctx->L,
+    VOR_LAUNCH(accumulate_kernel, grid, 256, 0, stream, d_ccl, ctx->d_rank, ctx->L, make_fastdiv((uint32_t)ctx->L),
                (unsigned long long*)ctx->d_acc, ctx->max_comp);
     SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
     CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->L, cap,
