@@ -63,7 +63,7 @@ __device__ __forceinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_
 }
 
 // ------------------------------------------------------------------------------------ emit
-constexpr int kHashSlots = 1024;
+constexpr int kHashSlots = 512;
 constexpr int kMaxProbe = 32;
 constexpr int kQueueCap = 32 + 256;     // < 32 pending + at most 8 pairs per lane per row
 
@@ -106,7 +106,7 @@ __device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned lon
 //   C  32 such records at a time: each of the 8 compared pairs that differ is inserted.
 // The CTA's hash set ends up holding every distinct key of its tile; it is appended to a global
 // raw-key list (one atomic per CTA) that the finish kernel inserts into the adjacency matrix.
-constexpr int kStrWarpsX = 2, kStrWarpsY = 4;
+constexpr int kStrWarpsX = 2, kStrWarpsY = 2;
 constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
 constexpr int kStrThreads = 32 * kStrWarps;                     // 256
 constexpr int kStripCols = 128;
@@ -170,7 +170,7 @@ __device__ __forceinline__ void hash_flush(const unsigned long long* table, cons
     }
 }
 
-__global__ void __launch_bounds__(kStrThreads, 4) edges_stream_kernel(const int32_t* __restrict__ labels,
+__global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int32_t* __restrict__ labels,
                                                                       int32_t L, const RowSet rs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     StreamShared& sh = *reinterpret_cast<StreamShared*>(smem_raw);
@@ -311,7 +311,7 @@ __global__ void __launch_bounds__(kStrThreads, 4) edges_stream_kernel(const int3
 }
 
 // ---- generic kernel (any L, any alignment): scalar loads, every discontinuity goes to the hash set.
-constexpr int kEmitThreads = 256;
+constexpr int kEmitThreads = 128;
 constexpr int kEmitCols = 128;          // per CTA tile: 32 lanes x 4 labels
 constexpr int kEmitRowsPerWarp = 16;
 constexpr int kEmitRows = (kEmitThreads / 32) * kEmitRowsPerWarp;   // 128
@@ -905,7 +905,7 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     rs.flags = ctx->d_flags;
     const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
     if (vec) {
-        static_assert(sizeof(StreamShared) <= 55 * 1024, "four CTAs per SM");
+        static_assert(sizeof(StreamShared) <= 27 * 1024, "eight CTAs per SM");
         VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(StreamShared)));
         dim3 grid((L + kStrWarpsX * kStripCols - 1) / (kStrWarpsX * kStripCols),
