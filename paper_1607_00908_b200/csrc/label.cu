@@ -606,10 +606,11 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_wide_kernel(const __g
 // ---------------------------------------------------------------- CTA three-phase path (default)
 // The per-quadrant candidate lists are inherently small, scalar work (a few dozen distance tests per
 // 8 x 8 quadrant), so they are built by a few threads per quadrant instead of one warp per tile.
-// A CTA of 128 threads covers 64 x 32 cells = 8 x 4 quadrants:
+// A CTA of 64 threads covers 32 x 32 cells = 4 x 4 quadrants:
 //   phase G  the sites of the cell-list buckets covering the CTA's cells plus the halo are gathered
 //            into shared memory (coalesced row segments, coordinates relative to the CTA centre);
-//            every warp computes the segment prefix, warp w loads items [32w, 32w+32);
+//            every warp computes the segment prefix, warp w loads items [32w, 32w+32); only the sites
+//            inside the exact rectangle box +/- halo are kept;
 //   phase A  4 lanes per quadrant build its candidate list from the shared site list:
 //            U_q = dist(quadrant centre, nearest gathered site) + quadrant radius; the gathered region
 //            must reach U_q beyond the quadrant box on every side; candidates = gathered sites within
@@ -618,10 +619,10 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_wide_kernel(const __g
 //            packed keys 16 * (|o|^2 - 2 c.o) + position: one integer min per (cell, candidate)
 //            gives the nearest site and the smallest-index tie-break; full 128-byte row stores.
 // A quadrant whose bound cannot be proven this way is marked and its cells take the general search.
-constexpr int kCtaQX = 8, kCtaQY = 4;                 // quadrants per CTA
+constexpr int kCtaQX = 4, kCtaQY = 4;                 // quadrants per CTA
 constexpr int kCtaQ = kCtaQX * kCtaQY;
-constexpr int kCtaThreads = 128;
-constexpr int kCtaCapSites = 128;                     // = kCtaThreads: one gathered site per thread
+constexpr int kCtaThreads = 64;
+constexpr int kCtaCapSites = 64;                      // = kCtaThreads: one gathered site per thread
 constexpr int kCtaMaxExtent = 23000;                  // |relative site coordinate| bound
 constexpr int kCtaMaxU = 20000;                       // |o| <= 896 + U <= 20896: t = |o|^2 - 2 c.o fits int32
 constexpr int kUnpackedFlag = 1 << 16;
@@ -779,7 +780,7 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
         }
     }
     // ---- phase B: warp = 32 x 16 cells, lane = column
-    const int wx = wid & 1, wy = wid >> 1;
+    const int wx = wid % (kCtaQX / 4), wy = wid / (kCtaQX / 4);
     const int32_t x = X0 + 32 * wx + lane;
     const int qx = 4 * wx + (lane >> 3);
     const int32_t cxr = FP_ONE * (lane & 7) - QHW;
