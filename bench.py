@@ -30,7 +30,7 @@ from paper_1607_00908_b200 import workloads as W  # noqa: E402
 # distance expansion, one min) + 1 store.
 LABEL_OPS_PER_CELL = 22
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1f_full_summary.md); config 5 only.
+# (profiles/r1g_full_summary.md); config 5 only.
 NCU_TRAFFIC_BYTES = {"label_cta_kernel": 1.035e9, "edges_stream_kernel": 1.098e9, "rows_insert_kernel": 0.082e9,
                      "edges_finish_kernel": 0.094e9, "diff_kernel": 0.048e9}
 
