@@ -59,6 +59,13 @@ int vor_sync_status(vor_ctx* ctx, void* stream);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t vor_launch_count(const vor_ctx* ctx);
 
+/* Diagnostics of the last call (synchronises the device; for tuning notes, never on the hot path):
+ *   "label_unproven_quadrants"  8x8-cell quadrants the CTA labelling kernel handed to its second pass
+ *   "edges_raw_keys"            CTA-distinct keys the emit kernel produced (before the rows de-duplicate)
+ *   "edges_overflow_keys"       keys that did not fit their adjacency row
+ * Unknown names -> VOR_EINVAL (negative). */
+int64_t vor_stat(vor_ctx* ctx, const char* name);
+
 /* Per-kernel timing for bench.py's roofline figures.  vor_profile_begin() arms the context: every
  * kernel the library launches afterwards (at most 256) is bracketed by CUDA events on its own stream.
  * vor_profile_end() disarms it, synchronises `stream`, and returns the number n of launches timed
@@ -72,7 +79,10 @@ int vor_profile_end(vor_ctx* ctx, void* stream, char* names, int32_t names_len, 
  *   "row_slots"              adjacency-matrix slots used per site in vor_edges: 4, 8, 12 or 16
  *                            (default 16); pairs that do not fit take the sorted overflow path,
  *                            so the result never depends on it
- *   "label_path", "label_halo_x100", "label_fast_off", "label_bits"   kernel selection for tests */
+ *   "sites_hint"             expected number of bubbles for field_frame_device (0 = max_sites)
+ *   "label_path" (0 auto, 1 general ring search, 2 warp-per-tile, 3 CTA), "label_halo_x100",
+ *   "label_fast_off", "edges_generic"   kernel selection for the parity tests; results never depend
+ *                            on them */
 int vor_set_option(vor_ctx* ctx, const char* name, int64_t value);
 
 /* ---- a1: counting-sort cell list of the sites (not in the paper, which loops over all centres,
@@ -81,6 +91,14 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value);
  * stream work has run. */
 int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
                     void* stream);
+
+/* Same with the number of sites in a DEVICE scalar (e.g. the bubble count field_centroids just wrote),
+ * so that a field-driven frame needs no host synchronisation.  Reads min(*d_n_sites, cap) sites;
+ * 1 <= cap <= max_sites.  n_hint (1..cap, else cap) is the expected number: it only sizes the buckets
+ * and selects kernels, results never depend on it.  Labels produced afterwards are < cap; zero sites
+ * give the label -1 everywhere.  *d_n_sites must stay valid until vor_label has run. */
+int vor_build_cells_dev(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, const int32_t* d_n_sites,
+                        int32_t cap, int32_t n_hint, void* stream);
 
 /* ---- a2: digital Voronoi colouring (§II region definition; PAPER.md:129-131
  * §III.B.1 "coloring itself with the label of the nearest center of mass", squared distance).
@@ -92,31 +110,49 @@ int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream);
 /* ---- a3+a4: site adjacency (digital Delaunay edge set; PAPER.md:121 adjacency matrix,
  * PAPER.md:207 compress by sort+unique).  Rule (R6): every 4-connected label
  * discontinuity, including across the periodic wrap, contributes the pair (min,max).
- * Reads d_labels[L*L] (values in [0, n_sites) of the last vor_build_cells, or any int32 >= 0
- * if label_bits is given through vor_edges_ex); writes the ascending unique keys to
- * d_edges[0..min(E,cap)) and E to *d_n_edges. */
+ * Reads d_labels[L*L] (any int32 >= 0; values below the n_sites of the last vor_build_cells - or
+ * below max_sites if there was none - take the fast adjacency-row path, larger ones the sorted
+ * overflow path); writes the ascending unique keys to d_edges[0..min(E,cap)) and E to *d_n_edges. */
 int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
               int64_t* d_n_edges, void* stream);
+/* Same, and also the offset of every site's row in the list: the keys (a, b), b > a, of site a are
+ * d_edges[d_row_ptr[a] .. d_row_ptr[a+1]) - the paper's adjacency matrix in compressed form
+ * (PAPER.md:207, 215).  d_row_ptr has n_rows + 1 entries, n_rows = n_sites of the last vor_build_cells
+ * (max_sites if there was none); keys whose smaller label is >= n_rows follow after d_row_ptr[n_rows].
+ * Offsets are clamped to cap; cap must be < 2^32.  d_row_ptr may be NULL (= vor_edges). */
+int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
+                   int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream);
 
 /* ---- a5: frame-to-frame comparison (§III.B.3 translation + comparison;
  * PAPER.md:223 appearing/disappearing bubbles excluded; §III.B.4 "breaking" = in
  * D_P only, "arising" = in D_N only).  d_prev/d_now are ascending unique key lists with device
- * counts.  d_p2n[i] (prev label -> now label or -1) and d_n2p (now -> prev or -1) may both be
+ * counts; cap_prev / cap_now are the capacities of the two buffers and a count above its capacity
+ * (an upstream overflow, already latched in the sticky status) is clamped to it, so a chained call
+ * never reads out of bounds.  d_p2n[i] (prev label -> now label or -1) and d_n2p (now -> prev or -1) may both be
  * NULL: persistent identity.  With maps: prev edges are translated, dropped if an endpoint is -1
  * or both endpoints collapse, re-sorted and uniqued; now edges with an unmatched endpoint are
  * dropped.  created = now \ prev, destroyed = prev \ now, ascending, in NOW index space.
  * n_prev_labels / n_now_labels bound the label values (needed only with maps; pass 0 otherwise). */
 int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
-             const uint64_t* d_now, const int64_t* d_n_now,
+             const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
              const int32_t* d_p2n, const int32_t* d_n2p, int32_t n_prev_labels, int32_t n_now_labels,
              uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
              int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
+/* The same comparison the way the paper does it ("each thread accesses a given row of
+ * (E_P)_PN and its isomorphic one in (E_N)_NN"): persistent identity, both lists with the row offsets
+ * vor_edges_rows returned for the SAME n_rows; keys beyond d_*_row_ptr[n_rows] are not compared.
+ * No searching and no count arguments: the offsets delimit everything that is read. */
+int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_t* d_prev_row_ptr,
+                  const uint64_t* d_now, const uint32_t* d_now_row_ptr, int32_t n_rows,
+                  uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
+                  int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
 
 /* ---- trigger and event counts: the paper's own outputs on top of the diff (PAPER.md:215-221
  * §III.B.3 local_trigger / global_trigger; §III.B.4 eventsIndices / eventsNumber;
  * PAPER.md:236 eventsCount for both triangulations).  All four lists are ascending unique key lists
  * in ONE index space with labels < n_labels (site path: as given to / returned by vor_diff; keys
  * with a label >= n_labels are ignored).  d_created / d_destroyed must be the diff of d_prev / d_now.
+ * cap_*: capacities of the four list buffers; device counts above them are clamped (see vor_diff).
  * Outputs, device memory owned by the caller:
  *   d_trigger[n_labels]         1 if the vertex's adjacency row changed (endpoint of a created or
  *                               destroyed edge), else 0
@@ -125,9 +161,10 @@ int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
  *   d_count_prev / d_count_now[n_labels]  for an active vertex: number of active vertices adjacent to
  *                               it in the past / present edge list; 0 for inactive vertices. */
 int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
-               const uint64_t* d_now, const int64_t* d_n_now,
+               const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
                const uint64_t* d_created, const int64_t* d_n_created,
-               const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int32_t n_labels,
+               const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int64_t cap_created,
+               int64_t cap_destroyed, int32_t n_labels,
                int32_t* d_trigger, int32_t* d_events_indices, int32_t* d_events_number,
                int32_t* d_global_trigger, int32_t* d_count_prev, int32_t* d_count_now, void* stream);
 
@@ -187,6 +224,31 @@ int vor_frame_reset(vor_ctx* ctx);
 int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const uint64_t** d_edges,
                       const uint64_t** d_created, const uint64_t** d_destroyed,
                       const int64_t** d_counts);
+
+/* ---- end-to-end, field-driven frames (PAPER.md:93-101 bubbles and centres of mass; PAPER.md:211-223
+ * the trigger: isomorphism, translation, comparison): a6 -> a7 -> a8 -> a1 -> a2 -> a3/a4 -> a5 with the
+ * maps, all enqueued on `stream` without a host synchronisation.  Bubbles are the sites (at most the
+ * context's max_sites; more latch VOR_ECAPACITY); matching radius in fixed-point units.  The first frame
+ * of a sequence has nothing to compare with: created = destroyed = empty.  Same pipeline rules as
+ * vor_frame_submit / vor_frame_collect (two frames in flight, results in submission order); do not mix
+ * site and field frames on one context.  h_counts[4] = {n_bubbles, n_edges, n_created, n_destroyed};
+ * lists in NOW index space.  vor_frame_reset() starts a new sequence. */
+int field_frame_device(vor_ctx* ctx, const float* d_field, float thr, int above, int32_t min_size,
+                       int32_t radius_fp, void* stream);
+int field_frame_submit(vor_ctx* ctx, const float* h_field, float thr, int above, int32_t min_size,
+                       int32_t radius_fp, void* stream);
+int field_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
+                        int64_t* h_counts);
+/* Device pointers to the context-owned results of the last field_frame_device / field_frame_submit:
+ * bubble image, Voronoi labels, per-bubble arrays (first counts[0] entries), the maps P->N and N->P
+ * (max_sites entries each), edges, created, destroyed, counts int64[4] (device; field_frame_device only).
+ * Any out-pointer may be NULL. */
+int field_frame_results(vor_ctx* ctx, const int32_t** d_ccl, const int32_t** d_labels,
+                        const double** d_cx, const double** d_cy, const int32_t** d_sx,
+                        const int32_t** d_sy, const int32_t** d_size, const int32_t** d_root,
+                        const int32_t** d_p2n, const int32_t** d_n2p, const uint64_t** d_edges,
+                        const uint64_t** d_created, const uint64_t** d_destroyed,
+                        const int64_t** d_counts);
 
 #ifdef __cplusplus
 }

@@ -21,7 +21,6 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(_build.build())
         _lib.orc_edges.restype = C.c_int64
-        _lib.orc_count_discontinuities.restype = C.c_int64
         _lib.orc_centroids.restype = C.c_int32
         _lib.orc_label_cells.restype = C.c_int
         _lib.orc_label_cells_at.restype = C.c_int
@@ -94,11 +93,6 @@ def edges(labels):
         buf = np.empty(m, dtype=np.uint64)
         m = lib().orc_edges(C.c_int32(L), _p(labels, C.c_int32), _p(buf, C.c_uint64), C.c_int64(len(buf)))
     return buf[:m].copy()
-
-
-def count_discontinuities(labels):
-    labels = _i32(labels)
-    return int(lib().orc_count_discontinuities(C.c_int32(labels.shape[0]), _p(labels, C.c_int32)))
 
 
 def diff(prev, now, p2n=None, n2p=None):

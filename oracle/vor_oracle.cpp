@@ -208,18 +208,6 @@ int64_t orc_edges(int32_t L, const int32_t* labels, uint64_t* out, int64_t cap) 
     return m;
 }
 
-// Number of raw (not de-duplicated) discontinuities — workload statistic only.
-int64_t orc_count_discontinuities(int32_t L, const int32_t* labels) {
-    int64_t m = 0;
-    for (int32_t y = 0; y < L; ++y)
-        for (int32_t x = 0; x < L; ++x) {
-            int32_t a = labels[(size_t)y * L + x];
-            m += a != labels[(size_t)y * L + (x + 1) % L];
-            m += a != labels[(size_t)((y + 1) % L) * L + x];
-        }
-    return m;
-}
-
 // O3 — frame-to-frame diff (PAPER.md:213-221 translation + comparison; PAPER.md:223
 // appearing/disappearing bubbles excluded; PAPER.md:266 breaking = in D_P only,
 // arising = in D_N only).  p2n / n2p may be NULL (persistent identity).

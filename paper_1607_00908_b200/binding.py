@@ -27,13 +27,18 @@ SIGNATURES = {
     "vor_sync_status": (C.c_int, [_P, _P]),
     "vor_launch_count": (C.c_int64, [_P]),
     "vor_set_option": (C.c_int, [_P, C.c_char_p, C.c_int64]),
+    "vor_stat": (C.c_int64, [_P, C.c_char_p]),
     "vor_profile_begin": (C.c_int, [_P]),
     "vor_profile_end": (C.c_int, [_P, _P, C.c_char_p, C.c_int32, C.POINTER(C.c_float), C.c_int32]),
     "vor_build_cells": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
+    "vor_build_cells_dev": (C.c_int, [_P, _P, _P, _P, C.c_int32, C.c_int32, _P]),
     "vor_label": (C.c_int, [_P, _P, _P]),
     "vor_edges": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P]),
-    "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
-    "vor_events": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, _P]),
+    "vor_edges_rows": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P, _P]),
+    "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
+    "vor_diff_rows": (C.c_int, [_P, _P, _P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
+    "vor_events": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, _P, C.c_int64, C.c_int64, C.c_int32,
+                             _P, _P, _P, _P, _P, _P, _P]),
     "field_threshold_ccl": (C.c_int, [_P, _P, C.c_float, C.c_int, _P, _P]),
     "field_centroids": (C.c_int, [_P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
     "match_sites": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P, _P]),
@@ -43,6 +48,10 @@ SIGNATURES = {
     "vor_frame_collect": (C.c_int, [_P, _P, _P, C.c_int64, _P]),
     "vor_frame_reset": (C.c_int, [_P]),
     "vor_frame_results": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P)]),
+    "field_frame_device": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, C.c_int32, _P]),
+    "field_frame_submit": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, C.c_int32, _P]),
+    "field_frame_collect": (C.c_int, [_P, _P, _P, C.c_int64, _P]),
+    "field_frame_results": (C.c_int, [_P] + [C.POINTER(_P)] * 14),
 }
 
 _lib = None
@@ -138,6 +147,12 @@ class Vor:
             self._check(n)
         return list(zip(names.value.decode().split("\n")[:n], [float(ms[i]) for i in range(n)]))
 
+    def vor_stat(self, name: str) -> int:
+        v = int(self.lib.vor_stat(self.h, name.encode()))
+        if v < 0:
+            self._check(v)
+        return v
+
     def vor_set_option(self, name: str, value: int):
         self._check(self.lib.vor_set_option(self.h, name.encode(), int(value)))
 
@@ -146,6 +161,12 @@ class Vor:
         assert sx.shape == sy.shape and sx.dim() == 1
         self._check(self.lib.vor_build_cells(self.h, _ptr(sx, torch.int32), _ptr(sy, torch.int32),
                                              sx.numel(), _stream()))
+
+    def vor_build_cells_dev(self, sx, sy, n_sites, n_hint=0):
+        """n_sites: int32[1] device scalar; sx/sy sized to the capacity."""
+        cap = min(sx.numel(), sy.numel())
+        self._check(self.lib.vor_build_cells_dev(self.h, _ptr(sx, torch.int32), _ptr(sy, torch.int32),
+                                                 _ptr(n_sites, torch.int32), cap, n_hint, _stream()))
 
     def vor_label(self, labels):
         assert labels.numel() == self.L * self.L
@@ -157,12 +178,29 @@ class Vor:
         self._check(self.lib.vor_edges(self.h, _ptr(labels, torch.int32), _ptr(edges, torch.int64),
                                        edges.numel(), _ptr(n_edges, torch.int64), _stream()))
 
+    def vor_edges_rows(self, labels, edges, n_edges, row_ptr):
+        """As vor_edges, plus row_ptr: int32 tensor (viewed as uint32) of n_rows + 1 row offsets."""
+        assert labels.numel() == self.L * self.L and n_edges.numel() >= 1
+        self._check(self.lib.vor_edges_rows(self.h, _ptr(labels, torch.int32), _ptr(edges, torch.int64),
+                                            edges.numel(), _ptr(n_edges, torch.int64),
+                                            _ptr(row_ptr, torch.int32), _stream()))
+
+    def vor_diff_rows(self, prev, prev_row_ptr, now, now_row_ptr, n_rows, created, destroyed, n_created,
+                      n_destroyed):
+        assert min(prev_row_ptr.numel(), now_row_ptr.numel()) >= n_rows + 1
+        cap = min(created.numel(), destroyed.numel())
+        self._check(self.lib.vor_diff_rows(
+            self.h, _ptr(prev, torch.int64), _ptr(prev_row_ptr, torch.int32), _ptr(now, torch.int64),
+            _ptr(now_row_ptr, torch.int32), n_rows, _ptr(created, torch.int64), _ptr(destroyed, torch.int64),
+            cap, _ptr(n_created, torch.int64), _ptr(n_destroyed, torch.int64), _stream()))
+
     def vor_diff(self, prev, n_prev, now, n_now, created, destroyed, n_created, n_destroyed,
                  p2n=None, n2p=None, n_prev_labels=0, n_now_labels=0):
         cap = min(created.numel(), destroyed.numel())
         self._check(self.lib.vor_diff(
             self.h, _ptr(prev, torch.int64), _ptr(n_prev, torch.int64), _ptr(now, torch.int64),
-            _ptr(n_now, torch.int64), _ptr(p2n, torch.int32), _ptr(n2p, torch.int32),
+            _ptr(n_now, torch.int64), prev.numel(), now.numel(),
+            _ptr(p2n, torch.int32), _ptr(n2p, torch.int32),
             n_prev_labels, n_now_labels, _ptr(created, torch.int64), _ptr(destroyed, torch.int64), cap,
             _ptr(n_created, torch.int64), _ptr(n_destroyed, torch.int64), _stream()))
 
@@ -172,7 +210,9 @@ class Vor:
         i64, i32 = torch.int64, torch.int32
         self._check(self.lib.vor_events(
             self.h, _ptr(prev, i64), _ptr(n_prev, i64), _ptr(now, i64), _ptr(n_now, i64),
-            _ptr(created, i64), _ptr(n_created, i64), _ptr(destroyed, i64), _ptr(n_destroyed, i64), n_labels,
+            prev.numel(), now.numel(),
+            _ptr(created, i64), _ptr(n_created, i64), _ptr(destroyed, i64), _ptr(n_destroyed, i64),
+            created.numel(), destroyed.numel(), n_labels,
             _ptr(trigger, i32), _ptr(events_indices, i32), _ptr(events_number, i32), _ptr(global_trigger, i32),
             _ptr(count_prev, i32), _ptr(count_now, i32), _stream()))
 
@@ -229,3 +269,30 @@ class Vor:
         ps = [C.c_void_p() for _ in range(5)]
         self._check(self.lib.vor_frame_results(self.h, *[C.byref(p) for p in ps]))
         return tuple(p.value for p in ps)
+
+    # ---- field-driven frames
+    def field_frame_device(self, field, thr: float, above: bool, min_size: int, radius_fp: int):
+        assert field.numel() == self.L * self.L
+        self._check(self.lib.field_frame_device(self.h, _ptr(field, torch.float32), C.c_float(thr),
+                                                1 if above else 0, min_size, radius_fp, _stream()))
+
+    def field_frame_submit(self, h_field, thr: float, above: bool, min_size: int, radius_fp: int):
+        """h_field: HOST float32 numpy array (L*L, C order); keep it alive and unchanged until collected."""
+        assert h_field.size == self.L * self.L and h_field.dtype.name == "float32" and h_field.flags.c_contiguous
+        self._check(self.lib.field_frame_submit(self.h, h_field.ctypes.data_as(_P), C.c_float(thr),
+                                                1 if above else 0, min_size, radius_fp, _stream()))
+
+    def field_frame_collect(self, h_created, h_destroyed, h_counts):
+        """h_counts: int64[4] = bubbles, edges, created, destroyed."""
+        cap = min(len(h_created), len(h_destroyed))
+        self._check(self.lib.field_frame_collect(self.h, h_created.ctypes.data_as(_P),
+                                                 h_destroyed.ctypes.data_as(_P), cap, h_counts.ctypes.data_as(_P)))
+
+    FIELD_RESULTS = ("ccl", "labels", "cx", "cy", "sx", "sy", "size", "root", "p2n", "n2p", "edges", "created",
+                     "destroyed", "counts")
+
+    def field_frame_results(self):
+        """dict of raw device pointers (ints), keys FIELD_RESULTS."""
+        ps = [C.c_void_p() for _ in self.FIELD_RESULTS]
+        self._check(self.lib.field_frame_results(self.h, *[C.byref(p) for p in ps]))
+        return {k: p.value for k, p in zip(self.FIELD_RESULTS, ps)}

@@ -15,9 +15,12 @@ constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 constexpr int kScanTile = kScanThreads * kScanItems;
 
+// n_dev (optional): the number of sites as a device scalar, clamped to n (the grid covers n threads)
 __global__ void count_sites_kernel(const int32_t* __restrict__ sx, const int32_t* __restrict__ sy,
-                                   int32_t n, int32_t w, int32_t nb, int32_t* __restrict__ fill) {
+                                   int32_t n, const int32_t* __restrict__ n_dev, int32_t w, int32_t nb,
+                                   int32_t* __restrict__ fill) {
     int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, *n_dev);
     if (i >= n) return;
     int32_t b = (sy[i] / w) * nb + (sx[i] / w);
     atomicAdd(&fill[b], 1);
@@ -104,10 +107,11 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(int32_t* __res
 }
 
 __global__ void scatter_sites_kernel(const int32_t* __restrict__ sx, const int32_t* __restrict__ sy,
-                                     int32_t n, int32_t w, int32_t nb,
+                                     int32_t n, const int32_t* __restrict__ n_dev, int32_t w, int32_t nb,
                                      const int32_t* __restrict__ start, int32_t* __restrict__ fill,
                                      int4* __restrict__ sorted) {
     int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n_dev) n = min(n, *n_dev);
     if (i >= n) return;
     int32_t x = sx[i], y = sy[i];
     int32_t b = (y / w) * nb + (x / w);
@@ -117,16 +121,12 @@ __global__ void scatter_sites_kernel(const int32_t* __restrict__ sx, const int32
 
 }  // namespace
 
-extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
-                               int32_t n_sites, void* stream_) {
-    if (!ctx) return VOR_EINVAL;
-    if (!d_sx || !d_sy) return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: null site array");
-    if (n_sites < 1 || n_sites > ctx->max_sites)
-        return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: n_sites out of range [1, max_sites]");
-    cudaStream_t stream = (cudaStream_t)stream_;
-
+// n_sites: number of sites, or their upper bound when d_n_dev (device scalar) holds the exact number;
+// n_hint sizes the buckets (about one site per bucket)
+static int build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
+                       const int32_t* d_n_dev, int32_t n_hint, cudaStream_t stream) {
     // buckets per side: the divisor of P nearest (in ratio) to sqrt(n / occupancy), bucket >= 2 cells
-    const double target = sqrt((double)n_sites * 100.0 / (double)ctx->bucket_occ_x100);
+    const double target = sqrt((double)n_hint * 100.0 / (double)ctx->bucket_occ_x100);
     int64_t lo = (int64_t)target, hi = (int64_t)target + 1;
     if (lo < 1) lo = 1;
     if (lo > ctx->nb_max) lo = ctx->nb_max;
@@ -137,12 +137,14 @@ extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t*
     ctx->nb = (int32_t)nb;
     ctx->w = (int32_t)(ctx->P / nb);
     ctx->n_sites = n_sites;
+    ctx->n_hint = n_hint;
+    ctx->d_n_dev = d_n_dev;
     const int64_t nbuckets = nb * nb;
 
     VOR_CUDA(cudaMemsetAsync(ctx->d_bucket_fill, 0, nbuckets * sizeof(int32_t), stream));
     const int threads = 256;
     const int grid = (n_sites + threads - 1) / threads;
-    VOR_LAUNCH(count_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, ctx->w, ctx->nb,
+    VOR_LAUNCH(count_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nb,
                ctx->d_bucket_fill);
     const int tiles = (int)((nbuckets + kScanTile - 1) / kScanTile);
     VOR_LAUNCH(scan_reduce_kernel, tiles, kScanThreads, 0, stream, ctx->d_bucket_fill, nbuckets,
@@ -150,7 +152,26 @@ extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t*
     VOR_LAUNCH(scan_partials_kernel, 1, kScanThreads, 0, stream, ctx->d_scan_part, tiles);
     VOR_LAUNCH(scan_apply_kernel, tiles, kScanThreads, 0, stream, ctx->d_bucket_fill, nbuckets,
                ctx->d_scan_part, ctx->d_bucket_start);
-    VOR_LAUNCH(scatter_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, ctx->w, ctx->nb,
+    VOR_LAUNCH(scatter_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nb,
                ctx->d_bucket_start, ctx->d_bucket_fill, ctx->d_sorted);
     return VOR_OK;
+}
+
+extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
+                               int32_t n_sites, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_sx || !d_sy) return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: null site array");
+    if (n_sites < 1 || n_sites > ctx->max_sites)
+        return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: n_sites out of range [1, max_sites]");
+    return build_cells(ctx, d_sx, d_sy, n_sites, nullptr, n_sites, (cudaStream_t)stream_);
+}
+
+extern "C" int vor_build_cells_dev(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
+                                   const int32_t* d_n_sites, int32_t cap, int32_t n_hint, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_sx || !d_sy || !d_n_sites) return vor_fail(ctx, VOR_EINVAL, "vor_build_cells_dev: null pointer");
+    if (cap < 1 || cap > ctx->max_sites)
+        return vor_fail(ctx, VOR_EINVAL, "vor_build_cells_dev: cap out of range [1, max_sites]");
+    if (n_hint < 1 || n_hint > cap) n_hint = cap;
+    return build_cells(ctx, d_sx, d_sy, cap, d_n_sites, n_hint, (cudaStream_t)stream_);
 }

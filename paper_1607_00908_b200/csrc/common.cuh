@@ -39,8 +39,7 @@ struct vor_ctx {
 
     // options
     int64_t bucket_occ_x100;
-    int64_t label_bits_override;   // 0 = derive from n_sites
-    int64_t label_path;            // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8
+    int64_t label_path;            // 0 auto, 1 general, 2 tile 8x8, 3 CTA
     int64_t label_halo_x100;       // fast-path halo = r_quad + this/100 * mean site spacing
     int64_t label_fast_off;        // 1 = skip the quadrant fast path (testing)
 
@@ -48,7 +47,9 @@ struct vor_ctx {
     int32_t nb_max;            // allocation bound for buckets per side
     int32_t nb;                // buckets per side of the last build (0 = none)
     int32_t w;                 // bucket width in fixed-point units, w * nb == P
-    int32_t n_sites;           // of the last build
+    int32_t n_sites;           // of the last build (vor_build_cells_dev: the upper bound `cap`)
+    int32_t n_hint;            // expected number of sites (kernel selection, bucket and halo sizes only)
+    const int32_t* d_n_dev;    // vor_build_cells_dev: the exact number lives on the device; else NULL
     int32_t* d_bucket_start;   // [nb_max^2 + 1]
     int32_t* d_bucket_fill;    // [nb_max^2]  (scatter cursors)
     int4* d_sorted;            // [max_sites]  (x, y, original index, bucket)
@@ -69,9 +70,17 @@ struct vor_ctx {
     uint64_t* d_keys_a;        // [max_raw_keys]  overflow keys / sort ping
     uint64_t* d_keys_b;        // [max_raw_keys]  sort pong
     int64_t* d_n_raw;          // device control block [8]: 0 = raw/overflow key count, 1 = filtered
-                               //   overflow count, 2 = OR of the overflow keys
+                               //   overflow count, 2 = OR of the overflow keys, 3 = raw key count
     uint32_t* d_hist;          // [kMaxCoopBlocks * 256] per-block digit histograms
     int64_t* d_blk_count;      // [2 * kMaxCoopBlocks] per-block counts for compactions
+
+    // ---- fused label -> edge path (vor_frame_*): compact border columns of the 32-cell tile columns
+    int32_t* d_fu_cols;        // [2][L / 32][L]: left, then right border column of every tile column
+    int64_t fuse;              // option: 1 = vor_frame_* labels and extracts the pairs in one kernel
+
+    // ---- row-by-row diff: membership mask per row [dr_rows], then the per-block counts
+    uint32_t* d_dr_scratch;
+    int64_t dr_rows;
 
     // ---- diff with maps: translated / filtered lists
     uint64_t* d_tr_prev;       // lazily sized to max_raw_keys
@@ -94,6 +103,8 @@ struct vor_ctx {
     int32_t* d_fr_labels;      // [L*L]
     uint64_t* d_fr_edges[2];   // ping-pong prev / now
     int64_t* d_fr_nedges[2];
+    uint32_t* d_fr_rowptr[2];  // [max_sites + 1] row offsets of the two lists (vor_edges_rows)
+    int32_t fr_prev_sites;     // number of sites of the previous frame
     uint64_t* d_fr_created;
     uint64_t* d_fr_destroyed;
     int64_t* d_fr_counts;      // [3]
@@ -103,6 +114,15 @@ struct vor_ctx {
     int64_t fr_cap;
     int fr_cur;                // index of the "now" buffer of the last frame; -1 = none
     int fr_have_prev;
+    // field-driven frames (field_frame_*): bubble image, two generations of bubble arrays, the isomorphism
+    int32_t* d_ff_ccl;         // [L*L]
+    double* d_ff_cxy[2];       // [2 * max_sites] cx, cy
+    int32_t* d_ff_comp[2];     // [4 * max_sites + 4] sx, sy, size, root, then the device count
+    int32_t* d_ff_maps;        // [2 * max_sites] p2n, n2p
+    int64_t* d_ff_tmpcount;    // [2] created / destroyed counts before they are gathered
+    float* d_ff_field[2];      // device copies of submitted host fields (lazily)
+    int ff_cur;                // generation of the last field frame; -1 = none
+    int32_t ff_hint;           // bubbles in the last collected frame (sizes the next cell list)
     // pipelined variant (vor_frame_submit / vor_frame_collect): two frames in flight, copies on own streams
     int32_t* d_pp_sx[2];
     int32_t* d_pp_sy[2];
@@ -117,7 +137,7 @@ struct vor_ctx {
 
     int32_t* d_flags;          // [1] sticky error bits
     int num_sms;               // of the device the context lives on
-    int coop_blocks[4];        // cached grid sizes of the cooperative kernels (0 = not yet queried)
+    int coop_blocks[8];        // cached grid sizes of the cooperative kernels (0 = not yet queried)
     int64_t launches;
     // per-launch timing (vor_profile_begin / vor_profile_end): events around every kernel launch
     int prof_on;
@@ -190,4 +210,3 @@ int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n
                          uint64_t* d_out, int64_t cap, int64_t* d_n_out, int flag_bit,
                          int64_t n_hint /* expected number of keys, 0 = unknown */, cudaStream_t stream);
 int vor_reset_rows(vor_ctx* ctx);
-int vor_label_bits(const vor_ctx* ctx);

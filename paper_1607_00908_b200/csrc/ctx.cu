@@ -33,8 +33,8 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
     ctx->bucket_occ_x100 = 100;
     ctx->label_halo_x100 = 120;
     ctx->row_slots = kRowStride;
-    if (const char* e = getenv("VOR_BUCKET_OCC_X100")) ctx->bucket_occ_x100 = atoll(e);
     ctx->fr_cur = -1;
+    ctx->ff_cur = -1;
     cudaError_t e = cudaGetDevice(&ctx->device);
     if (e != cudaSuccess) { free(ctx); return VOR_ECUDA; }
     int coop = 0;
@@ -77,13 +77,17 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
     cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
     cudaFree(ctx->d_lab_fail); cudaFree(ctx->d_lab_fail_n);
+    cudaFree(ctx->d_fu_cols);
     cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
-    cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts);
+    cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts); cudaFree(ctx->d_dr_scratch);
     cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
     cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best); cudaFree(ctx->d_mgrid);
     cudaFree(ctx->d_fr_sx); cudaFree(ctx->d_fr_sy); cudaFree(ctx->d_fr_labels);
     cudaFree(ctx->d_fr_edges[0]); cudaFree(ctx->d_fr_edges[1]);
     cudaFree(ctx->d_fr_nedges[0]); cudaFree(ctx->d_fr_nedges[1]);
+    cudaFree(ctx->d_fr_rowptr[0]); cudaFree(ctx->d_fr_rowptr[1]);
+    cudaFree(ctx->d_ff_ccl); cudaFree(ctx->d_ff_maps); cudaFree(ctx->d_ff_tmpcount);
+    for (int k = 0; k < 2; ++k) { cudaFree(ctx->d_ff_cxy[k]); cudaFree(ctx->d_ff_comp[k]); cudaFree(ctx->d_ff_field[k]); }
     cudaFree(ctx->d_fr_created); cudaFree(ctx->d_fr_destroyed); cudaFree(ctx->d_fr_counts);
     cudaFreeHost(ctx->h_fr_counts); cudaFreeHost(ctx->h_fr_sites); cudaFreeHost(ctx->h_fr_lists);
     for (int k = 0; k < 2; ++k) {
@@ -104,6 +108,24 @@ int vor_destroy(vor_ctx* ctx) {
 const char* vor_last_error(const vor_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
 int64_t vor_launch_count(const vor_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int64_t vor_stat(vor_ctx* ctx, const char* name) {
+    if (!ctx || !name) return VOR_EINVAL;
+    if (cudaDeviceSynchronize() != cudaSuccess) return VOR_ECUDA;
+    if (!strcmp(name, "label_unproven_quadrants")) {
+        if (!ctx->d_lab_fail_n) return 0;
+        int32_t v = 0;                                      // the counter the last vor_label call used
+        if (cudaMemcpy(&v, ctx->d_lab_fail_n + (1 - ctx->lab_fail_turn), sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess)
+            return VOR_ECUDA;
+        return v;
+    }
+    if (!strcmp(name, "edges_raw_keys") || !strcmp(name, "edges_overflow_keys")) {
+        int64_t v[4] = {0, 0, 0, 0};
+        if (cudaMemcpy(v, ctx->d_n_raw, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return VOR_ECUDA;
+        return name[6] == 'r' ? v[3] : v[0];
+    }
+    return vor_fail(ctx, VOR_EINVAL, "unknown statistic");
+}
 
 int vor_profile_begin(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
@@ -141,20 +163,24 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         ctx->bucket_occ_x100 = value;
         return VOR_OK;
     }
-    if (!strcmp(name, "label_bits")) {
-        if (value < 0 || value > 31) return vor_fail(ctx, VOR_EINVAL, "label_bits must be in [0,31]");
-        ctx->label_bits_override = value;
-        return VOR_OK;
-    }
     if (!strcmp(name, "label_halo_x100")) {
         if (value < 0 || value > 1000) return vor_fail(ctx, VOR_EINVAL, "label_halo_x100 must be in [0,1000]");
         ctx->label_halo_x100 = value;
+        return VOR_OK;
+    }
+    if (!strcmp(name, "sites_hint")) {
+        if (value < 0 || value > ctx->max_sites) return vor_fail(ctx, VOR_EINVAL, "sites_hint must be in [0, max_sites]");
+        ctx->ff_hint = (int32_t)value;
         return VOR_OK;
     }
     if (!strcmp(name, "row_slots")) {
         if (value < 4 || value > kRowStride || value % 4)
             return vor_fail(ctx, VOR_EINVAL, "row_slots must be 4, 8, 12 or 16");
         ctx->row_slots = value;
+        return VOR_OK;
+    }
+    if (!strcmp(name, "fuse")) {
+        ctx->fuse = value != 0;
         return VOR_OK;
     }
     if (!strcmp(name, "edges_generic")) {
@@ -166,7 +192,7 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         return VOR_OK;
     }
     if (!strcmp(name, "label_path")) {
-        if (value < 0 || value > 5) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,5]");
+        if (value < 0 || value > 3) return vor_fail(ctx, VOR_EINVAL, "label_path must be in [0,3]");
         ctx->label_path = value;
         return VOR_OK;
     }
@@ -197,13 +223,4 @@ int vor_sync_status(vor_ctx* ctx, void* stream) {
 int vor_reset_rows(vor_ctx* ctx) {
     VOR_CUDA(cudaMemset(ctx->d_row_cnt, 0, (size_t)ctx->max_sites * sizeof(uint32_t)));
     return VOR_OK;
-}
-
-// Number of significant bits of a label value (site index) for the radix sort.
-int vor_label_bits(const vor_ctx* ctx) {
-    if (ctx->label_bits_override > 0) return (int)ctx->label_bits_override;
-    if (ctx->n_sites <= 0) return 31;
-    int bits = 1;
-    while (bits < 31 && ((int64_t)1 << bits) < (int64_t)ctx->n_sites) ++bits;
-    return bits;
 }

@@ -71,6 +71,7 @@ __device__ __forceinline__ uint32_t absent_mask(const uint64_t* __restrict__ A, 
 struct DiffParams {
     const uint64_t* prev; const int64_t* n_prev;
     const uint64_t* now;  const int64_t* n_now;
+    int64_t cap_prev, cap_now;     // capacities of the input buffers: the device counts are clamped to them
     uint64_t* created; uint64_t* destroyed; int64_t cap;
     int64_t* n_created; int64_t* n_destroyed;
     int64_t* partial;          // [gridDim]
@@ -87,7 +88,8 @@ __global__ void __launch_bounds__(kDiffThreads, 3) diff_kernel(const DiffParams 
     const int me = second ? blockIdx.x - nb : blockIdx.x;
     const uint64_t* __restrict__ A = second ? p.prev : p.now;        // elements of A not in B
     const uint64_t* __restrict__ B = second ? p.now : p.prev;
-    const int64_t nA = second ? *p.n_prev : *p.n_now, nB = second ? *p.n_now : *p.n_prev;
+    const int64_t nP = min(*p.n_prev, p.cap_prev), nN = min(*p.n_now, p.cap_now);
+    const int64_t nA = second ? nP : nN, nB = second ? nN : nP;
     uint64_t* __restrict__ out = second ? p.destroyed : p.created;
     int64_t C = (nA + nb - 1) / nb;
     C = (C + 32 * kDiffKeys - 1) / (32 * kDiffKeys) * (32 * kDiffKeys);    // whole warps of full threads
@@ -152,13 +154,208 @@ __global__ void __launch_bounds__(kDiffThreads, 3) diff_kernel(const DiffParams 
     }
 }
 
+// ---------------------------------------------------------------- row-by-row comparison (site path)
+// PAPER.md:215-221 (§III.B.3): "each thread accesses a given row of (E_P)_PN and its isomorphic one in
+// (E_N)_NN" and compares them.  With persistent site identity both lists come from vor_edges_rows,
+// which also returns the offset of every site's row (row a = the keys (a, b), b > a, ascending), so
+// row a of the past list and row a of the present list are found without searching.
+// Two plain kernels, no grid synchronisation and nothing that waits on another block:
+//   diff_rows_mark_kernel   one thread per pair of rows: both rows are loaded at once (all loads
+//                           independent), every entry is looked up in the other row in registers; the
+//                           16 + 16 bit membership mask of the row goes to a scratch array, the block's
+//                           two counts to a per-block array;
+//   diff_rows_write_kernel  every block sums the counts of the blocks before it, scans its own masks
+//                           and writes the created / destroyed keys in ascending order (only the
+//                           changed keys are read again).
+// Rows longer than kDrFast entries (hubs, overflowed rows) take a two-pointer merge in both kernels.
+constexpr int kDrThreads = 256;
+constexpr int kDrPerThread = 2;                    // rows per thread
+constexpr int kDrRows = kDrThreads * kDrPerThread; // rows per block
+constexpr int kDrFast = 8;                         // row length handled in registers
+constexpr uint32_t kDrLong = 0xffffffffu;          // mask marker: a long row (never a valid mask: bits 8-15 stay 0)
+
+struct DiffRowsParams {
+    const uint64_t* prev; const uint32_t* prev_ptr;
+    const uint64_t* now;  const uint32_t* now_ptr;
+    int32_t n_rows;
+    uint64_t* created; uint64_t* destroyed; int64_t cap;
+    int64_t* n_created; int64_t* n_destroyed;
+    uint32_t* masks;               // [n_rows]
+    uint32_t* blk_counts;          // [2][n_blocks] created, destroyed keys of every block's rows
+    int32_t* flags;
+};
+
+__device__ __forceinline__ uint32_t key_lo(const uint64_t* __restrict__ k) {
+    return __ldg(reinterpret_cast<const uint32_t*>(k));            // little endian: the larger label b
+}
+
+// two-pointer merge of two long rows; emit == false only counts
+template <bool kEmit>
+__device__ void row_merge(const uint64_t* __restrict__ A, uint32_t a0, uint32_t a1,
+                          const uint64_t* __restrict__ B, uint32_t b0, uint32_t b1,
+                          uint32_t* ca, uint32_t* cb, uint64_t* outA, int64_t posA, uint64_t* outB, int64_t posB,
+                          int64_t cap) {
+    uint32_t i = a0, j = b0;
+    uint32_t na = 0, nb = 0;
+    while (i < a1 || j < b1) {
+        const uint64_t x = i < a1 ? __ldg(A + i) : ~0ull, y = j < b1 ? __ldg(B + j) : ~0ull;
+        if (x == y) { ++i; ++j; }
+        else if (x < y) { if (kEmit && posA + na < cap) outA[posA + na] = x; ++na; ++i; }
+        else { if (kEmit && posB + nb < cap) outB[posB + nb] = y; ++nb; ++j; }
+    }
+    *ca = na; *cb = nb;
+}
+
+// warp w of a block owns rows [r0, r0 + 32 * kDrPerThread): row = r0 + 32 k + lane
+__device__ __forceinline__ int64_t dr_row0(int wid) {
+    return (int64_t)blockIdx.x * kDrRows + (int64_t)wid * (32 * kDrPerThread);
+}
+
+__global__ void __launch_bounds__(kDrThreads) diff_rows_mark_kernel(const DiffRowsParams p) {
+    __shared__ uint2 wtot[kDrThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t r0 = dr_row0(wid);
+    uint32_t a0[kDrPerThread], na[kDrPerThread], b0[kDrPerThread], nb[kDrPerThread];
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        const int64_t a = r0 + 32 * k + lane;
+        a0[k] = na[k] = b0[k] = nb[k] = 0;
+        if (a < p.n_rows) {
+            a0[k] = __ldg(p.now_ptr + a); na[k] = __ldg(p.now_ptr + a + 1) - a0[k];
+            b0[k] = __ldg(p.prev_ptr + a); nb[k] = __ldg(p.prev_ptr + a + 1) - b0[k];
+        }
+    }
+    uint32_t ea[kDrPerThread][kDrFast], eb[kDrPerThread][kDrFast];
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        const bool fast = na[k] <= kDrFast && nb[k] <= kDrFast;
+#pragma unroll
+        for (int i = 0; i < kDrFast; ++i) {
+            ea[k][i] = fast && i < (int)na[k] ? key_lo(p.now + a0[k] + i) : 0xffffffffu;     // the padding never
+            eb[k][i] = fast && i < (int)nb[k] ? key_lo(p.prev + b0[k] + i) : 0xfffffffeu;    // equals a label
+        }
+    }
+    uint32_t c = 0, d = 0;
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        const int64_t a = r0 + 32 * k + lane;
+        uint32_t m;
+        if (na[k] <= kDrFast && nb[k] <= kDrFast) {
+            uint32_t found = 0;                                   // bit i: ea[i] in prev; bit 16 + j: eb[j] in now
+#pragma unroll
+            for (int i = 0; i < kDrFast; ++i)
+#pragma unroll
+                for (int j = 0; j < kDrFast; ++j)
+                    if (ea[k][i] == eb[k][j]) found |= (1u << i) | (1u << (16 + j));
+            m = (((1u << na[k]) - 1u) | (((1u << nb[k]) - 1u) << 16)) & ~found;
+            c += __popc(m & 0xffffu); d += __popc(m >> 16);
+        } else {
+            uint32_t ca, cb;
+            row_merge<false>(p.now, a0[k], a0[k] + na[k], p.prev, b0[k], b0[k] + nb[k], &ca, &cb, nullptr, 0, nullptr, 0, 0);
+            m = kDrLong; c += ca; d += cb;
+        }
+        if (a < p.n_rows) p.masks[a] = m;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { c += __shfl_xor_sync(0xffffffffu, c, o); d += __shfl_xor_sync(0xffffffffu, d, o); }
+    if (lane == 0) wtot[wid] = make_uint2(c, d);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t tc = 0, td = 0;
+#pragma unroll
+        for (int w = 0; w < kDrThreads / 32; ++w) { tc += wtot[w].x; td += wtot[w].y; }
+        p.blk_counts[blockIdx.x] = tc;
+        p.blk_counts[gridDim.x + blockIdx.x] = td;
+    }
+}
+
+__global__ void __launch_bounds__(kDrThreads) diff_rows_write_kernel(const DiffRowsParams p) {
+    __shared__ uint2 wtot[kDrThreads / 32];
+    __shared__ int64_t red[2][kDrThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t n_blocks = gridDim.x;
+    // ---- keys of the blocks before this one (and, in the last block, of all of them)
+    int64_t bc = 0, bd = 0;
+    for (int32_t b = threadIdx.x; b < (int32_t)blockIdx.x; b += kDrThreads) {
+        bc += __ldg(p.blk_counts + b); bd += __ldg(p.blk_counts + n_blocks + b);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { bc += __shfl_xor_sync(0xffffffffu, bc, o); bd += __shfl_xor_sync(0xffffffffu, bd, o); }
+    if (lane == 0) { red[0][wid] = bc; red[1][wid] = bd; }
+    // ---- this block's masks and counts; positions inside the warp (k-major), then inside the block
+    const int64_t r0 = dr_row0(wid);
+    uint32_t m[kDrPerThread], nc[kDrPerThread], nd[kDrPerThread];
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        const int64_t a = r0 + 32 * k + lane;
+        m[k] = a < p.n_rows ? __ldcs(p.masks + a) : 0u;
+        nc[k] = __popc(m[k] & 0xffffu); nd[k] = __popc(m[k] >> 16);
+        if (m[k] == kDrLong) {
+            const uint32_t a0 = __ldg(p.now_ptr + a), a1 = __ldg(p.now_ptr + a + 1);
+            const uint32_t b0 = __ldg(p.prev_ptr + a), b1 = __ldg(p.prev_ptr + a + 1);
+            row_merge<false>(p.now, a0, a1, p.prev, b0, b1, &nc[k], &nd[k], nullptr, 0, nullptr, 0, 0);
+        }
+    }
+    uint32_t prec[kDrPerThread], pred[kDrPerThread];
+    uint32_t wrc = 0, wrd = 0;                                    // running totals of the warp
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        uint32_t ic = nc[k], id = nd[k];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t tc = __shfl_up_sync(0xffffffffu, ic, o), td = __shfl_up_sync(0xffffffffu, id, o);
+            if (lane >= o) { ic += tc; id += td; }
+        }
+        prec[k] = wrc + ic - nc[k]; pred[k] = wrd + id - nd[k];
+        wrc += __shfl_sync(0xffffffffu, ic, 31); wrd += __shfl_sync(0xffffffffu, id, 31);
+    }
+    if (lane == 0) wtot[wid] = make_uint2(wrc, wrd);
+    __syncthreads();
+    bc = 0; bd = 0;
+    uint32_t totc = 0, totd = 0;
+#pragma unroll
+    for (int w = 0; w < kDrThreads / 32; ++w) {
+        bc += red[0][w]; bd += red[1][w];
+        const uint2 t = wtot[w];
+        if (w < wid) { bc += t.x; bd += t.y; }
+        totc += t.x; totd += t.y;
+    }
+    if (blockIdx.x == n_blocks - 1 && threadIdx.x == kDrThreads - 1) {   // the last warp: bc, bd exclude only itself
+        const int64_t allc = bc + wtot[wid].x, alld = bd + wtot[wid].y;
+        *p.n_created = allc; *p.n_destroyed = alld;
+        if (allc > p.cap || alld > p.cap) atomicOr(p.flags, FLAG_DIFF_CAP);
+    }
+    // ---- write: only the changed keys are read again
+#pragma unroll
+    for (int k = 0; k < kDrPerThread; ++k) {
+        if (m[k] == 0) continue;
+        const int64_t a = r0 + 32 * k + lane;
+        int64_t pc = bc + prec[k], pd = bd + pred[k];
+        const uint32_t a0 = __ldg(p.now_ptr + a), b0 = __ldg(p.prev_ptr + a);
+        if (m[k] == kDrLong) {
+            uint32_t x, y;
+            row_merge<true>(p.now, a0, __ldg(p.now_ptr + a + 1), p.prev, b0, __ldg(p.prev_ptr + a + 1), &x, &y,
+                            p.created, pc, p.destroyed, pd, p.cap);
+            continue;
+        }
+        for (uint32_t mc = m[k] & 0xffffu; mc; mc &= mc - 1) {
+            if (pc < p.cap) p.created[pc] = __ldg(p.now + a0 + (__ffs(mc) - 1));
+            ++pc;
+        }
+        for (uint32_t md = m[k] >> 16; md; md &= md - 1) {
+            if (pd < p.cap) p.destroyed[pd] = __ldg(p.prev + b0 + (__ffs(md) - 1));
+            ++pd;
+        }
+    }
+}
+
 // prev edge (i,j) -> (p2n[i], p2n[j]); dropped if an endpoint is -1 or both collapse (R22);
 // unordered append (sorted afterwards).
 __global__ void translate_prev_kernel(const uint64_t* __restrict__ prev, const int64_t* __restrict__ n_prev_p,
-                                      const int32_t* __restrict__ p2n, int32_t n_prev_labels,
+                                      int64_t cap_in, const int32_t* __restrict__ p2n, int32_t n_prev_labels,
                                       uint64_t* __restrict__ out, int64_t cap,
                                       unsigned long long* __restrict__ n_out, int32_t* __restrict__ flags) {
-    const int64_t n = *n_prev_p;
+    const int64_t n = min(*n_prev_p, cap_in);
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
         const uint64_t e = prev[k];
         const uint32_t a = (uint32_t)(e >> 32), b = (uint32_t)e;
@@ -173,10 +370,10 @@ __global__ void translate_prev_kernel(const uint64_t* __restrict__ prev, const i
 
 // now edge kept iff both endpoints have a partner in the previous frame
 __global__ void filter_now_kernel(const uint64_t* __restrict__ now, const int64_t* __restrict__ n_now_p,
-                                  const int32_t* __restrict__ n2p, int32_t n_now_labels,
+                                  int64_t cap_in, const int32_t* __restrict__ n2p, int32_t n_now_labels,
                                   uint64_t* __restrict__ out, int64_t cap,
                                   unsigned long long* __restrict__ n_out, int32_t* __restrict__ flags) {
-    const int64_t n = *n_now_p;
+    const int64_t n = min(*n_now_p, cap_in);
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
         const uint64_t e = now[k];
         const uint32_t a = (uint32_t)(e >> 32), b = (uint32_t)e;
@@ -197,14 +394,14 @@ int bits_for(int32_t n) {
 }  // namespace
 
 extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
-                        const uint64_t* d_now, const int64_t* d_n_now,
+                        const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
                         const int32_t* d_p2n, const int32_t* d_n2p,
                         int32_t n_prev_labels, int32_t n_now_labels,
                         uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
                         int64_t* d_n_created, int64_t* d_n_destroyed, void* stream_) {
     if (!ctx) return VOR_EINVAL;
     if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_created || !d_destroyed || !d_n_created ||
-        !d_n_destroyed || cap < 0)
+        !d_n_destroyed || cap < 0 || cap_prev < 0 || cap_now < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_diff: null pointer or negative capacity");
     if ((d_p2n == nullptr) != (d_n2p == nullptr))
         return vor_fail(ctx, VOR_EINVAL, "vor_diff: give both maps or neither");
@@ -213,6 +410,7 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
     const int64_t* nP = d_n_prev;
     const uint64_t* N = d_now;
     const int64_t* nN = d_n_now;
+    int64_t capP = cap_prev, capN = cap_now;
     if (d_p2n) {
         if (n_prev_labels < 1 || n_now_labels < 1)
             return vor_fail(ctx, VOR_EINVAL, "vor_diff: label counts required with maps");
@@ -223,7 +421,7 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
         const int bits = bits_for(n_now_labels);
         // translated prev -> d_keys_a -> sort/unique -> d_tr_prev
         VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, sizeof(int64_t), stream));
-        VOR_LAUNCH(translate_prev_kernel, 4 * kNumSMs, 256, 0, stream, d_prev, d_n_prev, d_p2n,
+        VOR_LAUNCH(translate_prev_kernel, 4 * kNumSMs, 256, 0, stream, d_prev, d_n_prev, cap_prev, d_p2n,
                    n_prev_labels, ctx->d_keys_a, ctx->max_raw_keys,
                    (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
         int rc = vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits, ctx->d_tr_prev,
@@ -232,7 +430,7 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
         if (rc != VOR_OK) return rc;
         // filtered now -> d_keys_a -> sort/unique -> d_tr_now
         VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, sizeof(int64_t), stream));
-        VOR_LAUNCH(filter_now_kernel, 4 * kNumSMs, 256, 0, stream, d_now, d_n_now, d_n2p, n_now_labels,
+        VOR_LAUNCH(filter_now_kernel, 4 * kNumSMs, 256, 0, stream, d_now, d_n_now, cap_now, d_n2p, n_now_labels,
                    ctx->d_keys_a, ctx->max_raw_keys, (unsigned long long*)ctx->d_n_raw, ctx->d_flags);
         rc = vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits, ctx->d_tr_now,
                                   ctx->max_raw_keys, &ctx->d_tr_counts[1], FLAG_RAWKEY_OVERFLOW,
@@ -240,12 +438,38 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
         if (rc != VOR_OK) return rc;
         P = ctx->d_tr_prev; nP = &ctx->d_tr_counts[0];
         N = ctx->d_tr_now;  nN = &ctx->d_tr_counts[1];
+        capP = capN = ctx->max_raw_keys;
     }
-    DiffParams dp{P, nP, N, nN, d_created, d_destroyed, cap, d_n_created, d_n_destroyed,
+    DiffParams dp{P, nP, N, nN, capP, capN, d_created, d_destroyed, cap, d_n_created, d_n_destroyed,
                   ctx->d_blk_count, ctx->d_flags};
     int grid = vor_coop_grid(ctx, 2, (const void*)diff_kernel, kDiffThreads, 3);
     grid &= ~1;                                         // one half per direction
     if (grid < 2) return vor_fail(ctx, VOR_ECUDA, "vor_diff: device too small for the cooperative grid");
     VOR_LAUNCH_COOP(diff_kernel, grid, kDiffThreads, stream, (void*)&dp);
+    return VOR_OK;
+}
+
+extern "C" int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_t* d_prev_row_ptr,
+                             const uint64_t* d_now, const uint32_t* d_now_row_ptr, int32_t n_rows,
+                             uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
+                             int64_t* d_n_created, int64_t* d_n_destroyed, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_prev || !d_prev_row_ptr || !d_now || !d_now_row_ptr || !d_created || !d_destroyed ||
+        !d_n_created || !d_n_destroyed || cap < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_diff_rows: null pointer or negative capacity");
+    if (n_rows < 1) return vor_fail(ctx, VOR_EINVAL, "vor_diff_rows: n_rows must be >= 1");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int64_t n_blocks = ((int64_t)n_rows + kDrRows - 1) / kDrRows;
+    if (!ctx->d_dr_scratch || ctx->dr_rows < n_rows) {
+        if (ctx->d_dr_scratch) { VOR_CUDA(cudaStreamSynchronize(stream)); VOR_CUDA(cudaFree(ctx->d_dr_scratch)); ctx->d_dr_scratch = nullptr; }
+        const int64_t rows = n_rows > ctx->max_sites ? n_rows : ctx->max_sites;
+        const int64_t blocks = (rows + kDrRows - 1) / kDrRows;
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_dr_scratch, ((size_t)rows + 2 * (size_t)blocks) * sizeof(uint32_t)));
+        ctx->dr_rows = rows;
+    }
+    DiffRowsParams dp{d_prev, d_prev_row_ptr, d_now, d_now_row_ptr, n_rows, d_created, d_destroyed, cap,
+                      d_n_created, d_n_destroyed, ctx->d_dr_scratch, ctx->d_dr_scratch + ctx->dr_rows, ctx->d_flags};
+    VOR_LAUNCH(diff_rows_mark_kernel, (unsigned)n_blocks, kDrThreads, 0, stream, dp);
+    VOR_LAUNCH(diff_rows_write_kernel, (unsigned)n_blocks, kDrThreads, 0, stream, dp);
     return VOR_OK;
 }

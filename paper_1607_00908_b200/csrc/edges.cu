@@ -22,45 +22,11 @@
 #include <cooperative_groups.h>
 
 #include "common.cuh"
+#include "rows.cuh"
 
 namespace cg = cooperative_groups;
 
 namespace {
-
-constexpr uint64_t kEmptyKey = ~0ull;
-
-struct RowSet {
-    uint32_t* rows;            // [n_rows * kRowStride]
-    uint32_t* cnt;             // [n_rows] entries appended to each row (may exceed S: the excess overflowed)
-    int32_t n_rows;
-    int32_t S;                 // slots used per row
-    uint64_t* ovf;             // overflow keys (unordered, may repeat)
-    int64_t ovf_cap;
-    unsigned long long* n_ovf;
-    uint64_t* raw;             // per-CTA distinct keys, appended by the emit kernels
-    int64_t raw_cap;
-    unsigned long long* n_raw;
-    int32_t* flags;
-};
-
-__device__ __forceinline__ void ovf_push(const RowSet& rs, uint32_t a, uint32_t b) {
-    const unsigned long long pos = atomicAdd(rs.n_ovf, 1ull);
-    if ((int64_t)pos < rs.ovf_cap) rs.ovf[pos] = ((uint64_t)a << 32) | b;
-    else atomicOr(rs.flags, FLAG_RAWKEY_OVERFLOW);
-}
-
-// Append b to row a (a < b).  The row may receive the same b more than once (from different CTAs):
-// the finish kernel drops the repeats when it sorts the row.
-__device__ __forceinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b) {
-    if (a < (uint32_t)rs.n_rows) {
-        const uint32_t slot = atomicAdd(rs.cnt + a, 1u);
-        if (slot < (uint32_t)rs.S) {
-            rs.rows[(size_t)a * kRowStride + slot] = b;
-            return;
-        }
-    }
-    ovf_push(rs, a, b);
-}
 
 // ------------------------------------------------------------------------------------ emit
 constexpr int kHashSlots = 512;
@@ -157,16 +123,15 @@ __device__ __forceinline__ void hash_flush(const unsigned long long* table, cons
     __shared__ long long base_sh;
     if (threadIdx.x == 0) base_sh = total ? (long long)atomicAdd(rs.n_raw, (unsigned long long)total) : 0;
     __syncthreads();
-    const int64_t base = base_sh;
-    if (base + total <= rs.raw_cap) {
-        int64_t pos = base + wbase + inc - cnt;
+    // a key whose reserved slot lies beyond the list's capacity goes straight to the matrix, so every
+    // slot below min(n_raw, raw_cap) is written and rows_insert_kernel never reads a stale one
+    int64_t pos = base_sh + wbase + inc - cnt;
 #pragma unroll
-        for (int k = 0; k < kPer; ++k)
-            if (mine[k] != kEmptyKey) rs.raw[pos++] = mine[k];
-    } else {
-#pragma unroll 1
-        for (int k = 0; k < kPer; ++k)
-            if (mine[k] != kEmptyKey) row_insert(rs, (uint32_t)(mine[k] >> 32), (uint32_t)mine[k]);
+    for (int k = 0; k < kPer; ++k) {
+        if (mine[k] == kEmptyKey) continue;
+        if (pos < rs.raw_cap) rs.raw[pos] = mine[k];
+        else row_insert(rs, (uint32_t)(mine[k] >> 32), (uint32_t)mine[k]);
+        ++pos;
     }
 }
 
@@ -693,6 +658,7 @@ struct FinishParams {
     int64_t cap;
     int64_t* n_out;
     int32_t* flags;
+    uint32_t* row_ptr;         // optional [n_rows + 1]: offset of each site's first key in `out`
 };
 
 __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const FinishParams p) {
@@ -788,15 +754,16 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
         int64_t pos = run + wbase + inc - n;
         run += total;
         __syncthreads();
+        const uint64_t hi = (uint64_t)a << 32;
+        int64_t o0 = 0, o1 = 0;
+        if (a < rend && n_ovf > 0) {
+            o0 = lower_bound_u64(ovf, n_ovf, hi);
+            o1 = lower_bound_u64(ovf, n_ovf, hi + (1ull << 32));
+            pos += o0;
+        }
+        if (a < rend && p.row_ptr) p.row_ptr[a] = (uint32_t)(pos < p.cap ? pos : p.cap);
         if (a < rend && n > 0) {
             const uint32_t* row = p.rows + (size_t)a * kRowStride;
-            const uint64_t hi = (uint64_t)a << 32;
-            int64_t o0 = 0, o1 = 0;
-            if (n_ovf > 0) {
-                o0 = lower_bound_u64(ovf, n_ovf, hi);
-                o1 = lower_bound_u64(ovf, n_ovf, hi + (1ull << 32));
-                pos += o0;
-            }
             if (o1 == o0) {
 #pragma unroll
                 for (int q = 0; q < kRowStride; q += 4) {
@@ -825,11 +792,121 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
         }
     }
     // ---- overflow keys whose smaller label has no row come last
+    int64_t t0 = 0;
+    if (n_ovf > 0) t0 = lower_bound_u64(ovf, n_ovf, (uint64_t)p.n_rows << 32);
+    if (p.row_ptr && blockIdx.x == 0 && threadIdx.x == 0)
+        p.row_ptr[p.n_rows] = (uint32_t)(all + t0 < p.cap ? all + t0 : p.cap);
     if (n_ovf > 0) {
-        const int64_t t0 = lower_bound_u64(ovf, n_ovf, (uint64_t)p.n_rows << 32);
         for (int64_t j = t0 + (int64_t)blockIdx.x * kSortThreads + threadIdx.x; j < n_ovf;
              j += (int64_t)gridDim.x * kSortThreads)
             if (all + j < p.cap) p.out[all + j] = ovf[j];
+    }
+}
+
+// ------------------------------------------------------------------------------------ fused path: seams and left-over tiles
+// The labelling kernel (label.cu, fused variant) leaves, per 32 x 32 tile, the distinct adjacent pairs
+// found INSIDE the tile in kTileKeys fixed slots of the raw-key list.  What is left: the pairs across
+// the tile borders, and the tiles it could not finish (an unproven quadrant: their labels came from the
+// second labelling pass).
+//   fused_tail_kernel  one CTA per "supertile" of 8 x 8 tiles: the tiles' raw keys (or, for a left-over
+//                      tile, the pairs inside it read from the label image) and the pairs across
+//                      the right / lower border of each of its tiles (vertical seams from the compact
+//                      border columns, horizontal seams from rows 32k+31 | 32k+32 of the label image, all
+//                      coalesced) go through one shared-memory hash set, so a pair seen by several tiles
+//                      and seams reaches the adjacency rows about once; then the set is inserted.
+constexpr int kSuper = 8;                       // tiles per supertile side
+constexpr int kTailThreads = 256;
+constexpr int kTailSlots = 2048;                // hash-set slots per supertile (about 900 distinct keys at config 5)
+
+__device__ __forceinline__ void tail_insert(uint32_t a, uint32_t b, unsigned long long* table, const RowSet& rs) {
+    const uint32_t lo = min(a, b), hi = max(a, b);
+    const unsigned long long key = ((unsigned long long)lo << 32) | hi;
+    uint32_t h = hash_key(lo, hi) & (kTailSlots - 1);
+    for (int probe = 0; probe < kMaxProbe; ++probe) {
+        const unsigned long long cur = table[h];
+        if (cur == key) return;
+        if (cur == kEmptyKey) {
+            const unsigned long long old = atomicCAS(&table[h], kEmptyKey, key);
+            if (old == kEmptyKey || old == key) return;
+        }
+        h = (h + 1) & (kTailSlots - 1);
+    }
+    row_insert(rs, lo, hi);
+}
+
+// A tile the labelling kernel could not finish (its labels came from the second pass): the pairs inside
+// it from the label image, lane = column, all 32 rows in flight at once.  Kept out of line: it is rare
+// and must not cost the common path registers.
+__device__ __noinline__ void tail_dirty_tile(const int32_t* __restrict__ p, int32_t L, int lane,
+                                             unsigned long long* table, const RowSet& rs) {
+    const unsigned full = 0xffffffffu;
+    int32_t v[32];
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = __ldg(p + (int64_t)r * L);
+    int32_t upr = 0;                                  // right neighbour of the row above
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+        // every shuffle is executed by the whole warp, outside the conditions
+        const int32_t cur = v[r], right = __shfl_down_sync(full, cur, 1);
+        const int32_t below = v[r < 31 ? r + 1 : 31];
+        const int32_t lc = __shfl_up_sync(full, cur, 1), lb = __shfl_up_sync(full, below, 1);
+        if (lane < 31 && cur != right && (r == 0 || cur != v[r > 0 ? r - 1 : 0] || right != upr))
+            tail_insert((uint32_t)cur, (uint32_t)right, table, rs);
+        if (r < 31 && cur != below && (lane == 0 || lc != cur || lb != below))
+            tail_insert((uint32_t)cur, (uint32_t)below, table, rs);
+        upr = right;
+    }
+}
+
+__global__ void __launch_bounds__(kTailThreads) fused_tail_kernel(const int32_t* __restrict__ labels,
+                                                                  const int32_t* __restrict__ col_left,
+                                                                  const int32_t* __restrict__ col_right,
+                                                                  int32_t L, const RowSet rs) {
+    __shared__ unsigned long long table[kTailSlots];
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int32_t nt = L >> 5;
+    const int32_t tx0 = blockIdx.x * kSuper, ty0 = blockIdx.y * kSuper;
+    const int32_t ntx = min(kSuper, nt - tx0), nty = min(kSuper, nt - ty0);        // tiles of this supertile
+    for (int i = threadIdx.x; i < kTailSlots; i += kTailThreads) table[i] = kEmptyKey;
+    __syncthreads();
+    // ---- the tiles' own keys: one warp per tile, one slot per lane
+    for (int t = wid; t < ntx * nty; t += kTailThreads / 32) {
+        const int32_t tile = (ty0 + t / ntx) * nt + tx0 + t % ntx;
+        static_assert(kTileKeys == 32, "one slot per lane");
+        const unsigned long long key = __ldcs(reinterpret_cast<const unsigned long long*>(rs.raw) + (size_t)tile * kTileKeys + lane);
+        if (__shfl_sync(full, key, 0) != kDirtyTileKey) {
+            if (key != kEmptyKey) tail_insert((uint32_t)(key >> 32), (uint32_t)key, table, rs);
+            continue;
+        }
+        tail_dirty_tile(labels + (int64_t)(tile / nt) * 32 * L + (tile % nt) * 32 + lane, L, lane, table, rs);
+    }
+    // ---- seams: line c (c < ntx: right border of tile column tx0 + c; else lower border of tile row
+    // ty0 + c - ntx), 32 * (tiles along it) pairs; a run of the same pair is reported once per warp
+    const int32_t len_v = 32 * nty, len_h = 32 * ntx;
+    for (int c = 0; c < ntx + nty; ++c) {
+        const bool vert = c < ntx;
+        const int32_t len = vert ? len_v : len_h;
+        for (int32_t i = threadIdx.x; i < len; i += kTailThreads) {     // len % 32 == 0: whole warps
+            int32_t a, b;
+            if (vert) {
+                const int32_t tc = tx0 + c, nx = tc + 1 == nt ? 0 : tc + 1;
+                a = __ldcs(col_right + (int64_t)tc * L + 32 * ty0 + i);
+                b = __ldcs(col_left + (int64_t)nx * L + 32 * ty0 + i);
+            } else {
+                const int32_t y = 32 * (ty0 + c - ntx) + 31, yn = y + 1 == L ? 0 : y + 1;
+                a = __ldg(labels + (int64_t)y * L + 32 * tx0 + i);
+                b = __ldg(labels + (int64_t)yn * L + 32 * tx0 + i);
+            }
+            const int32_t pa = __shfl_up_sync(full, a, 1), pb = __shfl_up_sync(full, b, 1);
+            if (a != b && (lane == 0 || pa != a || pb != b)) tail_insert((uint32_t)a, (uint32_t)b, table, rs);
+        }
+    }
+    __syncthreads();
+    // ---- the set goes to the adjacency rows
+    for (int i = threadIdx.x; i < kTailSlots; i += kTailThreads) {
+        const unsigned long long key = table[i];
+        if (key != kEmptyKey) row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
     }
 }
 
@@ -883,14 +960,8 @@ int vor_sort_unique_keys(vor_ctx* ctx, uint64_t* d_keys_in_a, const int64_t* d_n
     return VOR_OK;
 }
 
-extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
-                         int64_t* d_n_edges, void* stream_) {
-    if (!ctx) return VOR_EINVAL;
-    if (!d_labels || !d_edges || !d_n_edges || cap < 0)
-        return vor_fail(ctx, VOR_EINVAL, "vor_edges: null pointer or negative capacity");
-    cudaStream_t stream = (cudaStream_t)stream_;
-    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 4 * sizeof(int64_t), stream));
-    const int32_t L = ctx->L;
+// The RowSet of this context: adjacency matrix, raw-key list (keys_b) and overflow list (keys_a).
+RowSet vor_row_set(vor_ctx* ctx) {
     RowSet rs;
     rs.rows = ctx->d_rows;
     rs.cnt = ctx->d_row_cnt;
@@ -903,6 +974,45 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
     rs.raw_cap = ctx->max_raw_keys;
     rs.n_raw = (unsigned long long*)&ctx->d_n_raw[3];
     rs.flags = ctx->d_flags;
+    return rs;
+}
+
+int vor_edges_fused_tail(vor_ctx* ctx, const int32_t* d_labels, const RowSet& rs, cudaStream_t stream) {
+    const int32_t L = ctx->L, nt = L / 32;
+    const int32_t* col_left = ctx->d_fu_cols;
+    const int32_t* col_right = ctx->d_fu_cols + (size_t)nt * L;
+    const unsigned ns = (unsigned)((nt + kSuper - 1) / kSuper);
+    VOR_LAUNCH(fused_tail_kernel, dim3(ns, ns), kTailThreads, 0, stream, d_labels, col_left, col_right, L, rs);
+    return VOR_OK;
+}
+
+// [insert the raw keys into the matrix, then] sort / merge / concatenate the rows (see the file header)
+int vor_edges_finish(vor_ctx* ctx, const RowSet& rs, uint64_t* d_edges, int64_t cap, int64_t* d_n_edges,
+                     uint32_t* d_row_ptr, bool have_raw, cudaStream_t stream) {
+    FinishParams fp{rs, ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
+                    ctx->d_n_raw, ctx->d_hist, ctx->d_blk_count, d_edges, cap, d_n_edges, ctx->d_flags, d_row_ptr};
+    if (have_raw) VOR_LAUNCH(rows_insert_kernel, 8 * ctx->num_sms, kInsertThreads, 0, stream, rs);
+    const int fgrid = vor_coop_grid(ctx, 0, (const void*)edges_finish_kernel, kSortThreads, 1);
+    VOR_LAUNCH_COOP(edges_finish_kernel, fgrid, kSortThreads, stream, (void*)&fp);
+    return VOR_OK;
+}
+
+extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
+                         int64_t* d_n_edges, void* stream_) {
+    return vor_edges_rows(ctx, d_labels, d_edges, cap, d_n_edges, nullptr, stream_);
+}
+
+extern "C" int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
+                              int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_labels || !d_edges || !d_n_edges || cap < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_edges: null pointer or negative capacity");
+    if (d_row_ptr && cap > 0xffffffffll)
+        return vor_fail(ctx, VOR_EINVAL, "vor_edges_rows: row offsets are 32-bit, cap must be < 2^32");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 8 * sizeof(int64_t), stream));
+    const int32_t L = ctx->L;
+    RowSet rs = vor_row_set(ctx);
     const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
     if (vec) {
         static_assert(sizeof(StreamShared) <= 27 * 1024, "eight CTAs per SM");
@@ -915,10 +1025,5 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
         dim3 grid((L + kEmitCols - 1) / kEmitCols, (L + kEmitRows - 1) / kEmitRows);
         VOR_LAUNCH(edges_emit_kernel, grid, kEmitThreads, 0, stream, d_labels, L, rs);
     }
-    FinishParams fp{rs, ctx->d_rows, rs.n_rows, rs.S, ctx->d_keys_a, ctx->d_keys_b, ctx->max_raw_keys,
-                    ctx->d_n_raw, ctx->d_hist, ctx->d_blk_count, d_edges, cap, d_n_edges, ctx->d_flags};
-    VOR_LAUNCH(rows_insert_kernel, 8 * ctx->num_sms, kInsertThreads, 0, stream, rs);
-    const int fgrid = vor_coop_grid(ctx, 0, (const void*)edges_finish_kernel, kSortThreads, 1);
-    VOR_LAUNCH_COOP(edges_finish_kernel, fgrid, kSortThreads, stream, (void*)&fp);
-    return VOR_OK;
+    return vor_edges_finish(ctx, rs, d_edges, cap, d_n_edges, d_row_ptr, true, stream);
 }

@@ -20,8 +20,9 @@ constexpr int kEvBatch = kEvThreads * kEvItems;
 
 __global__ void ev_mark_kernel(const uint64_t* __restrict__ created, const int64_t* __restrict__ n_created,
                                const uint64_t* __restrict__ destroyed, const int64_t* __restrict__ n_destroyed,
-                               int32_t n, int32_t* __restrict__ trigger) {
-    const int64_t nc = *n_created, nd = *n_destroyed;
+                               int64_t cap_created, int64_t cap_destroyed, int32_t n,
+                               int32_t* __restrict__ trigger) {
+    const int64_t nc = min(*n_created, cap_created), nd = min(*n_destroyed, cap_destroyed);
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nc + nd; k += (int64_t)gridDim.x * blockDim.x) {
         const uint64_t e = k < nc ? created[k] : destroyed[k - nc];
         const uint32_t i = (uint32_t)(e >> 32), j = (uint32_t)e;
@@ -115,12 +116,12 @@ __global__ void __launch_bounds__(kEvThreads) ev_write_kernel(const int32_t* __r
 // blocks [0, gridDim/2): past list -> count_prev; the rest: present list -> count_now
 __global__ void ev_degree_kernel(const uint64_t* __restrict__ prev, const int64_t* __restrict__ n_prev,
                                  const uint64_t* __restrict__ now, const int64_t* __restrict__ n_now,
-                                 const int32_t* __restrict__ trigger, int32_t n,
+                                 int64_t cap_prev, int64_t cap_now, const int32_t* __restrict__ trigger, int32_t n,
                                  int32_t* __restrict__ count_prev, int32_t* __restrict__ count_now) {
     const int half = gridDim.x >> 1;
     const bool second = (int)blockIdx.x >= half;
     const uint64_t* __restrict__ E = second ? now : prev;
-    const int64_t m = second ? *n_now : *n_prev;
+    const int64_t m = second ? min(*n_now, cap_now) : min(*n_prev, cap_prev);
     int32_t* __restrict__ cnt = second ? count_now : count_prev;
     const int b = second ? blockIdx.x - half : blockIdx.x;
     for (int64_t k = (int64_t)b * blockDim.x + threadIdx.x; k < m; k += (int64_t)half * blockDim.x) {
@@ -134,9 +135,11 @@ __global__ void ev_degree_kernel(const uint64_t* __restrict__ prev, const int64_
 }  // namespace
 
 extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
-                          const uint64_t* d_now, const int64_t* d_n_now,
+                          const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
                           const uint64_t* d_created, const int64_t* d_n_created,
-                          const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int32_t n_labels,
+                          const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int64_t cap_created,
+                          int64_t cap_destroyed,
+                          int32_t n_labels,
                           int32_t* d_trigger, int32_t* d_events_indices, int32_t* d_events_number,
                           int32_t* d_global_trigger, int32_t* d_count_prev, int32_t* d_count_now,
                           void* stream_) {
@@ -145,7 +148,8 @@ extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d
         !d_n_destroyed || !d_trigger || !d_events_indices || !d_events_number || !d_global_trigger ||
         !d_count_prev || !d_count_now)
         return vor_fail(ctx, VOR_EINVAL, "vor_events: null pointer");
-    if (n_labels < 1) return vor_fail(ctx, VOR_EINVAL, "vor_events: n_labels must be >= 1");
+    if (n_labels < 1 || cap_prev < 0 || cap_now < 0 || cap_created < 0 || cap_destroyed < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_events: n_labels must be >= 1, capacities >= 0");
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t bytes = (size_t)n_labels * sizeof(int32_t);
     VOR_CUDA(cudaMemsetAsync(d_trigger, 0, bytes, stream));
@@ -153,11 +157,11 @@ extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d
     VOR_CUDA(cudaMemsetAsync(d_count_now, 0, bytes, stream));
     const int grid = 4 * ctx->num_sms;                      // <= 2 * kMaxCoopBlocks partials
     VOR_LAUNCH(ev_mark_kernel, grid, 256, 0, stream, d_created, d_n_created, d_destroyed, d_n_destroyed,
-               n_labels, d_trigger);
+               cap_created, cap_destroyed, n_labels, d_trigger);
     VOR_LAUNCH(ev_count_kernel, grid, kEvThreads, 0, stream, d_trigger, n_labels, ctx->d_blk_count);
     VOR_LAUNCH(ev_write_kernel, grid, kEvThreads, 0, stream, d_trigger, n_labels, ctx->d_blk_count,
                d_events_indices, d_events_number, d_global_trigger);
-    VOR_LAUNCH(ev_degree_kernel, 2 * grid, 256, 0, stream, d_prev, d_n_prev, d_now, d_n_now, d_trigger,
-               n_labels, d_count_prev, d_count_now);
+    VOR_LAUNCH(ev_degree_kernel, 2 * grid, 256, 0, stream, d_prev, d_n_prev, d_now, d_n_now, cap_prev, cap_now,
+               d_trigger, n_labels, d_count_prev, d_count_now);
     return VOR_OK;
 }

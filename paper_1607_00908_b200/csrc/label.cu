@@ -29,7 +29,10 @@
 //    cell's own bucket every other site has |dx| or |dy| > r*w, so the search stops once
 //    best_d2 <= (r*w)^2; when the ring would wrap onto itself it scans all sites.  Used for tiny
 //    lattices, very dense or very sparse sites, and as per-tile fallback of the tile path.
+#include <type_traits>
+
 #include "common.cuh"
+#include "rows.cuh"
 
 namespace {
 
@@ -38,7 +41,8 @@ struct LabelParams {
     int32_t P;                 // 256 * L  (L <= 2^22 -> P <= 2^30)
     int32_t nb;
     int32_t w;
-    int32_t n;
+    int32_t n;                 // number of sites (upper bound if n_dev is given)
+    const int32_t* __restrict__ n_dev;        // exact number as a device scalar, or NULL
     const int32_t* __restrict__ bucket_start;
     const int4* __restrict__ sorted;
     int32_t tiles_x;
@@ -52,7 +56,21 @@ struct LabelParams {
     int32_t* fail_count;
     int32_t* fail_count_next;  // counter of the next call: zeroed by label_fixup_kernel
     int32_t fail_cap;
+    // fused label -> edge path (vor_label_edges): left / right border column of every 32-cell tile column
+    // in compact form, col[tile_x * L + y]
+    int32_t* col_left;
+    int32_t* col_right;
 };
+
+// fused path: a label written by the second pass also goes to the compact border columns
+__device__ __forceinline__ void store_label(const LabelParams& p, int32_t* __restrict__ labels, int32_t x,
+                                            int32_t y, int32_t v) {
+    labels[(int64_t)y * p.L + x] = v;
+    if (p.col_left) {
+        if ((x & 31) == 0) p.col_left[(int64_t)(x >> 5) * p.L + y] = v;
+        if ((x & 31) == 31) p.col_right[(int64_t)(x >> 5) * p.L + y] = v;
+    }
+}
 
 __device__ __forceinline__ int32_t div_w(const LabelParams& p, int32_t x /* >= 0 */) {
     const uint32_t t = __umulhi(p.div_m, (uint32_t)x);
@@ -94,8 +112,9 @@ __device__ int32_t label_cell_general(const LabelParams& p, int32_t x, int32_t y
     for (int32_t r = 0;; ++r) {
         if (2 * r + 1 >= p.nb) {            // the ring would wrap onto itself: scan everything once
             best = INT64_MAX; besti = INT32_MAX;
-            for (int32_t k = 0; k < p.n; ++k) consider(p.sorted[k], cx, cy, P, best, besti);
-            return besti;
+            const int32_t n = p.n_dev ? min(p.n, *p.n_dev) : p.n;
+            for (int32_t k = 0; k < n; ++k) consider(p.sorted[k], cx, cy, P, best, besti);
+            return n > 0 ? besti : -1;       // no site at all: background
         }
         for (int32_t oy = -r; oy <= r; ++oy) {
             const int32_t qy = pos_mod(by + oy, p.nb);
@@ -207,13 +226,9 @@ struct FastScratch {
     int32_t sx[32], sy[32], si[32];          // gathered sites in ascending original index
     int4 list[4][kListCap];                  // per quadrant: (2*rx, 2*ry, rx^2+ry^2, original index)
 };
-struct WideScratch {
-    int4 list[8][kListCap];                  // per 8x8 quadrant: packed-key candidate entries
-};
 union TileScratch {
     WarpScratch generic;
     FastScratch fast;
-    WideScratch wide;
 };
 
 // ceil(sqrt(f)) or slightly more, f >= 0: one MUFU.RSQ; relative error of the product < 2^-21
@@ -427,181 +442,14 @@ __device__ __noinline__ bool tile_generic(const LabelParams& p, WarpScratch& ws,
 #pragma unroll
         for (int j = 0; j < ROWS; ++j) {
             const int32_t y = ty0 + ly0 + j;
-            if (y < p.L) labels[(int64_t)y * p.L + x] = ws.cand[bi[j]].w;
+            if (y < p.L) store_label(p, labels, x, y, ws.cand[bi[j]].w);
         }
     }
     return true;
 }
 
-// Wide fast path: one warp per 32 x 16 tile = 4 x 2 quadrants of 8 x 8 cells; lane = column.
-// Same exactness argument as tile_fast, per quadrant.  Candidate keys are packed as
-// 16 * (|s|^2 - 2 c.s) + k  (coordinates relative to the quadrant centre, k = position in the
-// index-ordered list), so that one integer min per (cell, candidate) yields both the nearest site
-// and the smallest-index tie-break.  |key| < 2^31 is guaranteed by U_q <= kMaxUWide.
-constexpr int kMaxUWide = 6400;
-
-__device__ __forceinline__ bool tile_wide(const LabelParams& p, WideScratch& wsx, int lane,
-                                          int32_t tx0, int32_t ty0, int32_t* __restrict__ labels) {
-    constexpr int HX = FP_HALF * 31, HY = FP_HALF * 15;
-    constexpr int QC = 4 * FP_ONE;                 // quadrant centres at -3QC/4.. : (2*qx-3)*QC/... see qcx()
-    constexpr int QHW = FP_HALF * 7;               // quadrant box half extent (cell centres)
-    const unsigned full = 0xffffffffu;
-    const int32_t cxm = FP_ONE * tx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HY;
-    const int32_t H = p.halo_fast, P = p.P, half = p.P >> 1;
-
-    // ---- bucket range of the region
-    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
-    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
-    const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
-    if (ncols * p.w > half || nrows * p.w > half) return false;
-    const int32_t RX0 = q0 * p.w - cxm, RX1 = (q1 + 1) * p.w - cxm;
-    const int32_t RY0 = r0 * p.w - cym, RY1 = (r1 + 1) * p.w - cym;
-    if (-RX0 > kMaxRel || RX1 > kMaxRel || -RY0 > kMaxRel || RY1 > kMaxRel) return false;
-    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
-    const bool split = a0 + ncols > p.nb;
-    const int32_t nseg = split ? 2 * nrows : nrows;
-    if (nseg > 32) return false;
-
-    int32_t beg = 0, cnt = 0;
-    if (lane < nseg) {
-        const int32_t row = split ? lane >> 1 : lane;
-        int32_t ay = r0 + row;
-        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
-        int32_t c0, c1;
-        if (!split) { c0 = a0; c1 = a0 + ncols; }
-        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
-        else { c0 = 0; c1 = a0 + ncols - p.nb; }
-        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
-        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
-    }
-    int32_t inc = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int32_t t = __shfl_up_sync(full, inc, o);
-        if (lane >= o) inc += t;
-    }
-    const int32_t total = __shfl_sync(full, inc, 31);
-    if (total == 0 || total > 32) return false;
-    const int32_t exc = inc - cnt;
-    int32_t seg = 0;
-    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= lane);
-    const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
-    const bool valid = lane < total;
-    int32_t rx = 0, ry = 0, idx = INT32_MAX;
-    if (valid) {
-        const int4 s = __ldg(&p.sorted[sbeg + (lane - sexc)]);
-        rx = s.x - cxm; ry = s.y - cym; idx = s.z;
-        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
-        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
-    }
-    // ---- rank by original index (indices distinct; invalid lanes rank last)
-    int32_t rank = 0;
-    for (int32_t b = 0; b < total; ++b) rank += (__shfl_sync(full, idx, b) < idx);
-    const unsigned rbit = valid ? (1u << rank) : 0u, rlt = (1u << rank) - 1u;
-
-    // ---- per quadrant: offsets from the quadrant centre, bound U_q, exactness check
-    int32_t ox[4], oy[2], ox2[4], oy2[2];
-#pragma unroll
-    for (int qx = 0; qx < 4; ++qx) { ox[qx] = rx - (2 * qx - 3) * QC; ox2[qx] = ox[qx] * ox[qx]; }
-#pragma unroll
-    for (int qy = 0; qy < 2; ++qy) { oy[qy] = ry - (2 * qy - 1) * QC; oy2[qy] = oy[qy] * oy[qy]; }
-    int32_t U[8];
-    bool ok = true;
-#pragma unroll
-    for (int qy = 0; qy < 2; ++qy) {
-        const int32_t my = min((2 * qy - 1) * QC - QHW - RY0 + 1, RY1 - ((2 * qy - 1) * QC + QHW));
-#pragma unroll
-        for (int qx = 0; qx < 4; ++qx) {
-            const int32_t mx = min((2 * qx - 3) * QC - QHW - RX0 + 1, RX1 - ((2 * qx - 3) * QC + QHW));
-            const int32_t f = __reduce_min_sync(full, valid ? ox2[qx] + oy2[qy] : INT32_MAX);
-            const int32_t u = isqrt_up(f) + p.r_quad;
-            U[qy * 4 + qx] = u;
-            ok = ok && u < min(mx, my) && u <= kMaxUWide;
-        }
-    }
-    if (!ok) return false;
-
-    // ---- candidate lists: sites within U_q of the quadrant box, ascending index, packed keys
-    int32_t ex2[4], ey2[2];
-#pragma unroll
-    for (int qx = 0; qx < 4; ++qx) { const int32_t e = max(abs(ox[qx]) - QHW, 0); ex2[qx] = e * e; }
-#pragma unroll
-    for (int qy = 0; qy < 2; ++qy) { const int32_t e = max(abs(oy[qy]) - QHW, 0); ey2[qy] = e * e; }
-    unsigned M[8];
-    bool fits = true;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        const int qx = q & 3, qy = q >> 2;
-        const bool keep = valid && ex2[qx] + ey2[qy] <= U[q] * U[q];
-        M[q] = __reduce_or_sync(full, keep ? rbit : 0u);
-        fits = fits && __popc(M[q]) <= kListCap;
-        if (keep) {
-            const int32_t pos = __popc(M[q] & rlt);
-            if (pos < kListCap)
-                wsx.list[q][pos] = make_int4(-32 * ox[qx], -32 * oy[qy], 16 * (ox2[qx] + oy2[qy]) + pos, idx);
-        }
-    }
-    if (!fits) return false;
-    __syncwarp();
-
-    // ---- scan: lane = column; rows 0-7 use quadrant (qx, 0), rows 8-15 quadrant (qx, 1)
-    const int qx = lane >> 3;
-    const int32_t cxr = FP_ONE * (lane & 7) - QHW;
-    const int32_t x = tx0 + lane;
-#pragma unroll
-    for (int qy = 0; qy < 2; ++qy) {
-        const unsigned Mq = qx == 0 ? M[qy * 4] : (qx == 1 ? M[qy * 4 + 1] : (qx == 2 ? M[qy * 4 + 2] : M[qy * 4 + 3]));
-        const int32_t n = __popc(Mq);
-        const int4* __restrict__ list = wsx.list[qy * 4 + qx];
-        int32_t best[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) best[j] = INT32_MAX;
-        for (int32_t k = 0; k < n; ++k) {
-            const int4 c = list[k];
-            const int32_t a = c.z + cxr * c.x;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) best[j] = min(best[j], a + (FP_ONE * j - QHW) * c.y);
-        }
-        if (x < p.L) {
-            int32_t* __restrict__ out = labels + (int64_t)(ty0 + 8 * qy) * p.L + x;
-#pragma unroll
-            for (int j = 0; j < 8; ++j)
-                if (ty0 + 8 * qy + j < p.L) out[(int64_t)j * p.L] = list[best[j] & (kListCap - 1)].w;
-        }
-    }
-    return true;
-}
-
-// fallback of the wide kernel: the two 16 x 16 halves through the narrower paths
-__device__ __noinline__ void tile_wide_fallback(const LabelParams& p, TileScratch& ts, int lane,
-                                                int32_t tx0, int32_t ty0, int32_t* __restrict__ labels) {
-    constexpr int HX = FP_HALF * 15;
-    for (int h = 0; h < 2; ++h) {
-        const int32_t hx0 = tx0 + 16 * h;
-        if (hx0 >= p.L) break;
-        const int32_t cxm = FP_ONE * hx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HX;
-        __syncwarp();
-        if (tile_fast<16, 16>(p, ts.fast, lane, hx0, ty0, cxm, cym, labels)) continue;
-        __syncwarp();
-        if (tile_generic<16, 16>(p, ts.generic, lane, hx0, ty0, cxm, cym, labels)) continue;
-        const int32_t x = hx0 + (lane & 15), yb = ty0 + (lane >> 4) * 8;
-        for (int j = 0; j < 8; ++j)
-            if (x < p.L && yb + j < p.L) labels[(int64_t)(yb + j) * p.L + x] = label_cell_general(p, x, yb + j);
-    }
-}
-
-__global__ void __launch_bounds__(kWarpsPerCta * 32) label_wide_kernel(const __grid_constant__ LabelParams p,
-                                                                       int32_t* __restrict__ labels) {
-    __shared__ TileScratch scratch[kWarpsPerCta];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + wid;
-    if (tile >= (int64_t)p.tiles_x * p.tiles_y) return;
-    const int32_t tiy = (int32_t)(tile / p.tiles_x);
-    const int32_t tx0 = (int32_t)(tile - (int64_t)tiy * p.tiles_x) * 32, ty0 = tiy * 16;
-    if (tile_wide(p, scratch[wid].wide, lane, tx0, ty0, labels)) return;
-    tile_wide_fallback(p, scratch[wid], lane, tx0, ty0, labels);
-}
-
+// |packed key| < 2^31 needs U_q <= kMaxUPacked (packed-key scan of the CTA path)
+constexpr int kMaxUPacked = 6400;
 
 // ---------------------------------------------------------------- CTA three-phase path (default)
 // The per-quadrant candidate lists are inherently small, scalar work (a few dozen distance tests per
@@ -634,6 +482,15 @@ struct CtaShared {
     int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
     int32_t nkept;                                    // gathered sites kept (inside the exact rectangle)
 };
+// fused path: (label, slot of the site in sx/sy/si) of every list entry, fetched with one 64-bit load;
+// the CTA's 64 x 64 bit matrix of adjacent slots; the first row of the lower warp
+struct CtaFusedShared {
+    int2 fin[kListCap][kCtaQ];
+    uint8_t tslot[kListCap][kCtaQ];                   // slot of the unsorted survivors
+    uint32_t bm[kCtaCapSites * kCtaCapSites / 32];
+    uint32_t seam[32];                                // row 15 of the tile (last row of the upper warp)
+};
+struct CtaNoFused {};
 
 // Returns the number of gathered sites (0 = region unusable).  Region bounds relative to the CTA
 // centre are returned through R[4] = {RX0, RX1, RY0, RY1}.
@@ -707,7 +564,8 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
 
 // 4 consecutive lanes (sub = 0..3) build the list of quadrant q; qcx, qcy: its centre relative to the
 // CTA centre.  Lane sub == 0 publishes sh.count[q] = length | flags, or -1.
-__device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& sh, int q, int sub,
+template <bool kFused, typename FS>
+__device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& sh, FS& fs, int q, int sub,
                                                int32_t ns, const int32_t* R, int32_t qcx, int32_t qcy,
                                                bool active) {
     constexpr int QHW = FP_HALF * 7;
@@ -731,7 +589,10 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
             const int32_t ex = min(max(abs(ox) - QHW, 0), U + 1), ey = min(max(abs(oy) - QHW, 0), U + 1);
             if (ex * ex + ey * ey <= U2) {
                 const int32_t slot = atomicAdd(&sh.count[q], 1);
-                if (slot < kListCap) sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, ox * ox + oy * oy, sh.si[i]);
+                if (slot < kListCap) {
+                    sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, ox * ox + oy * oy, sh.si[i]);
+                    if constexpr (kFused) fs.tslot[slot][q] = (uint8_t)i;
+                }
             }
         }
     }
@@ -745,21 +606,79 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
             int32_t r = 0;
             for (int32_t j = 0; j < n; ++j) r += (sh.tmp[j][q].w < e.w);
             sh.list[r][q] = e;
+            if constexpr (kFused) fs.fin[r][q] = make_int2(e.w, (int32_t)fs.tslot[k][q]);
         }
     }
     if (sub == 0 && active)
-        sh.count[q] = (ok && n <= kListCap) ? (U <= kMaxUWide ? n : n | kUnpackedFlag) : -1;
+        sh.count[q] = (ok && n <= kListCap) ? (U <= kMaxUPacked ? n : n | kUnpackedFlag) : -1;
 }
 
-__global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_constant__ LabelParams p,
-                                                                int32_t* __restrict__ labels) {
+// ---- fused path: the adjacent pairs of a CTA's 32 x 32 cells, straight from the labelling registers.
+// Every cell carries the SLOT (0..63) of its site in the CTA's gathered list, one byte per cell, four
+// rows per register (lane = column).  Right neighbours come from one shuffle per register, lower
+// neighbours from a byte shift.  A differing pair of slots sets one bit of the CTA's 64 x 64 bit
+// matrix in shared memory (the de-duplication), which is decoded into (label, label) keys at the end.
+__device__ __forceinline__ void bm_set(uint32_t* bm, uint32_t a, uint32_t b) {
+    const uint32_t idx = min(a, b) * kCtaCapSites + max(a, b);
+    atomicOr(&bm[idx >> 5], 1u << (idx & 31));
+}
+
+// one bit-matrix entry per non-zero byte of x: the pair (byte of aw, byte of bw) at that position
+__device__ __forceinline__ void emit_bytes(uint32_t x, uint32_t aw, uint32_t bw, uint32_t* bm) {
+    while (__any_sync(0xffffffffu, x != 0)) {
+        if (x) {
+            const int s = (__ffs(x) - 1) & ~7;
+            bm_set(bm, (aw >> s) & 255u, (bw >> s) & 255u);
+            x &= ~(255u << s);
+        }
+    }
+}
+
+// 0xff in every byte of v that is not zero
+__device__ __forceinline__ uint32_t nonzero_bytes(uint32_t v) {
+    const uint32_t t = (((v & 0x7f7f7f7fu) + 0x7f7f7f7fu) | v) & 0x80808080u;
+    return (t >> 7) * 255u;
+}
+
+// W[i]: slots of rows 4i .. 4i+3 of this lane's column (a warp's 16 rows).  Pairs with the column to
+// the right (lanes 0..30) and with the row below (rows 0..14); the row below row 15 is the other
+// warp's or the next tile's business.
+__device__ __forceinline__ void cta_pairs(const uint32_t (&W)[4], uint32_t* bm) {
+    const unsigned full = 0xffffffffu;
+    uint32_t D[4], PD[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        PD[i] = i < 3 ? (W[i] >> 8) | (W[i + 1] << 24) : (W[3] >> 8) | (W[3] & 0xff000000u);
+        D[i] = W[i] ^ PD[i];                                   // byte b: rows 4i+b and 4i+b+1 differ
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t R = __shfl_down_sync(full, W[i], 1);    // lane 31 reads itself: no pair
+        // a horizontal pair that repeats the row above (same slot on both sides) is skipped: "changed"
+        // marks the rows whose own or right slot differs from the row above; row 0 always counts
+        const uint32_t UW = i ? (D[i] << 8) | (D[i - 1] >> 24) : (D[0] << 8) | 0xffu;
+        const uint32_t changed = UW | __shfl_down_sync(full, UW, 1);
+        emit_bytes((W[i] ^ R) & nonzero_bytes(changed), W[i], R, bm);
+        emit_bytes(D[i], W[i], PD[i], bm);
+    }
+}
+
+template <bool kFused>
+__global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kernel(const __grid_constant__ LabelParams p,
+                                                                int32_t* __restrict__ labels,
+                                                                const __grid_constant__ RowSet rs) {
     constexpr int QHW = FP_HALF * 7;
     constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
     __shared__ CtaShared sh;
+    __shared__ typename std::conditional<kFused, CtaFusedShared, CtaNoFused>::type fs;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int32_t X0 = blockIdx.x * (8 * kCtaQX), Y0 = blockIdx.y * (8 * kCtaQY);
     // ---- phases G + A; quadrants whose bound could not be proven get one retry with a wider halo
     if (threadIdx.x < kCtaQ) sh.count[threadIdx.x] = 0;
+    if constexpr (kFused) {
+        for (int i = threadIdx.x; i < kCtaCapSites * kCtaCapSites / 32; i += kCtaThreads) fs.bm[i] = 0;
+    }
+    bool any_fail = false;
     {
         const int q = threadIdx.x >> 2, sub = threadIdx.x & 3;
         const int qx = q % kCtaQX, qy = q / kCtaQX;
@@ -771,19 +690,27 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
                                            FP_ONE * Y0 + FP_HALF + HY, H, R);
             __syncthreads();
             const int32_t ns = got ? sh.nkept : 0;
-            cta_build_list(p, sh, q, sub, ns, R, 8 * FP_ONE * qx + QHW - HX, 8 * FP_ONE * qy + QHW - HY, active);
+            cta_build_list<kFused>(p, sh, fs, q, sub, ns, R, 8 * FP_ONE * qx + QHW - HX, 8 * FP_ONE * qy + QHW - HY, active);
             __syncthreads();
             active = sh.count[q] < 0;
-            if (!__syncthreads_or(active)) break;
+            any_fail = __syncthreads_or(active);
+            if (!any_fail) break;
             if (attempt == 0 && active && sub == 0) sh.count[q] = 0;     // reset the survivor counter
             __syncthreads();
         }
+    }
+    // fused: a tile with an unproven quadrant gets its pairs from the label image later (tile list)
+    if constexpr (kFused) {
+        if (any_fail && threadIdx.x < kTileKeys)         // slot 0 tells fused_tail_kernel to read the tile itself
+            rs.raw[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * kTileKeys + threadIdx.x] =
+                threadIdx.x == 0 ? kDirtyTileKey : kEmptyKey;
     }
     // ---- phase B: warp = 32 x 16 cells, lane = column
     const int wx = wid % (kCtaQX / 4), wy = wid / (kCtaQX / 4);
     const int32_t x = X0 + 32 * wx + lane;
     const int qx = 4 * wx + (lane >> 3);
     const int32_t cxr = FP_ONE * (lane & 7) - QHW;
+    uint32_t W[4] = {0, 0, 0, 0};                        // fused: slots of the lane's 16 cells
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
         const int q = (2 * wy + h) * kCtaQX + qx;
@@ -798,8 +725,12 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
             if (p.fail_cap > 0) {
                 if ((lane & 7) == 0) p.fail_items[atomicAdd(p.fail_count, 1)] = make_int2(x, y0);
             } else {
-                for (int j = 0; j < 8; ++j)
-                    if (y0 + j < p.L) out[(int64_t)j * p.L] = label_cell_general(p, x, y0 + j);
+                for (int j = 0; j < 8; ++j) {
+                    if (y0 + j >= p.L) break;
+                    const int32_t v = label_cell_general(p, x, y0 + j);
+                    if constexpr (kFused) store_label(p, labels, x, y0 + j, v);
+                    else out[(int64_t)j * p.L] = v;
+                }
             }
             continue;
         }
@@ -841,13 +772,72 @@ __global__ void __launch_bounds__(kCtaThreads) label_cta_kernel(const __grid_con
                 }
             }
         }
-        if (y0 + 8 <= p.L) {
+        if constexpr (kFused) {                          // L % 32 == 0: no ragged rows
+            int32_t lab[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int2 f = fs.fin[sel[j]][q];         // (label, slot)
+                *out = f.x; out += p.L;
+                lab[j] = f.x;
+                W[2 * h + (j >> 2)] |= (uint32_t)f.y << (8 * (j & 3));
+            }
+            if (lane == 0 || lane == 31) {               // the tile's border columns, 8 labels = two 16-byte stores
+                int4* __restrict__ c = reinterpret_cast<int4*>((lane ? p.col_right : p.col_left) + (int64_t)blockIdx.x * p.L + y0);
+                c[0] = make_int4(lab[0], lab[1], lab[2], lab[3]);
+                c[1] = make_int4(lab[4], lab[5], lab[6], lab[7]);
+            }
+        } else if (y0 + 8 <= p.L) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) { *out = sh.list[sel[j]][q].w; out += p.L; }
         } else {
             for (int j = 0; j < 8; ++j)
                 if (y0 + j < p.L) out[(int64_t)j * p.L] = sh.list[sel[j]][q].w;
         }
+    }
+    if constexpr (kFused) {
+        if (any_fail) return;                            // CTA-uniform
+        cta_pairs(W, fs.bm);
+        if (wid == 0) fs.seam[lane] = W[3] >> 24;        // row 15 of the tile
+        __syncthreads();
+        if (wid == 0) return;
+        // the lower warp finishes alone (no further barrier): rows 15 | 16, then the bit matrix is decoded
+        // into the tile's kTileKeys slots of the raw-key list (plain stores, no atomics: nothing here waits
+        // for memory); slots left over are marked empty, keys that do not fit go straight to the rows
+        {
+            const uint32_t a = fs.seam[lane], b = W[0] & 255u;
+            const uint32_t pa = __shfl_up_sync(0xffffffffu, a, 1), pb = __shfl_up_sync(0xffffffffu, b, 1);
+            if (a != b && (lane == 0 || pa != a || pb != b)) bm_set(fs.bm, a, b);
+        }
+        __syncwarp();
+        constexpr int kWords = kCtaCapSites * kCtaCapSites / 32 / 32;      // bit-matrix words per lane (4)
+        uint32_t m[kWords];
+        int cnt = 0;
+#pragma unroll
+        for (int k = 0; k < kWords; ++k) { m[k] = fs.bm[kWords * lane + k]; cnt += __popc(m[k]); }
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, inc, 31);
+        int pos = inc - cnt;
+        unsigned long long* __restrict__ slots =
+            (unsigned long long*)rs.raw + (size_t)(blockIdx.y * gridDim.x + blockIdx.x) * kTileKeys;
+#pragma unroll
+        for (int k = 0; k < kWords; ++k) {
+            uint32_t mk = m[k];
+            while (mk) {
+                const uint32_t idx = 32u * (kWords * lane + k) + (__ffs(mk) - 1);
+                mk &= mk - 1;
+                const uint32_t la = (uint32_t)sh.si[idx / kCtaCapSites], lb = (uint32_t)sh.si[idx % kCtaCapSites];
+                const uint32_t lo = min(la, lb), hi = max(la, lb);
+                if (pos < kTileKeys) slots[pos] = ((unsigned long long)lo << 32) | hi;
+                else row_insert(rs, lo, hi);
+                ++pos;
+            }
+        }
+        for (int k = total + lane; k < kTileKeys; k += 32) slots[k] = kEmptyKey;
     }
 }
 
@@ -897,26 +887,31 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_fixup_kernel(LabelPar
         const int32_t x = tx0 + (lane & 7), yb = ty0 + (lane >> 3) * 2;
 #pragma unroll 1
         for (int j = 0; j < 2; ++j)
-            if (x < p.L && yb + j < p.L) labels[(int64_t)(yb + j) * p.L + x] = label_cell_general(p, x, yb + j);
+            if (x < p.L && yb + j < p.L) store_label(p, labels, x, yb + j, label_cell_general(p, x, yb + j));
     }
 }
 
 }  // namespace
 
-extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
-    if (!ctx) return VOR_EINVAL;
-    if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label: null labels");
-    if (ctx->nb <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label: call vor_build_cells first");
-    cudaStream_t stream = (cudaStream_t)stream_;
+// which labelling kernel the current cell list gets: 1 general, 2 warp per tile, 3 CTA
+static int label_path_for(const vor_ctx* ctx, double spacing) {
+    int path = (int)ctx->label_path;
+    if (path == 0) path = spacing >= 7.0 ? 3 : (spacing >= 4.0 ? 2 : 1);
+    if (ctx->L < 16) path = 1;
+    return path;
+}
+
+// fused: rs != NULL -> the CTA kernel also extracts the adjacent pairs of every 32 x 32 tile (path 3 only)
+static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaStream_t stream) {
     LabelParams p;
     p.L = ctx->L; p.P = (int32_t)ctx->P; p.nb = ctx->nb; p.w = ctx->w; p.n = ctx->n_sites;
+    p.n_dev = ctx->d_n_dev;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
     p.fail_items = nullptr; p.fail_count = nullptr; p.fail_count_next = nullptr; p.fail_cap = 0;
-    const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_sites);   // cells
-    int path = (int)ctx->label_path;    // 0 auto, 1 general, 2 tile 16x16, 3 tile 8x8, 4 wide 32x16, 5 CTA
-    if (path == 0) path = spacing >= 7.0 ? 5 : (spacing >= 4.0 ? 3 : 1);
-    if (ctx->L < 16) path = 1;
-    const int tw = (path == 2 || path >= 4) ? 16 : 8;
+    p.col_left = nullptr; p.col_right = nullptr;
+    const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint);    // cells
+    const int path = label_path_for(ctx, spacing);
+    const int tw = path == 3 ? 16 : 8;
     if (path == 1) {
         const int64_t bw = (ctx->L + 15) / 16;
         const int64_t blocks = bw * bw;
@@ -940,7 +935,7 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
         p.div_s2 = l > 0 ? l - 1 : 0;
     }
     const int use_fast = ctx->label_fast_off ? 0 : 1;
-    if (path == 5) {
+    if (path == 3) {
         if (!ctx->d_lab_fail) {
             const int64_t q = (int64_t)((ctx->L + 7) / 8) * ((ctx->L + 7) / 8);
             ctx->lab_fail_cap = q <= (1 << 24) ? (int32_t)q : 0;      // every quadrant fits, or no list at all
@@ -953,7 +948,13 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
         p.fail_count_next = ctx->d_lab_fail_n + (1 - ctx->lab_fail_turn);
         ctx->lab_fail_turn = 1 - ctx->lab_fail_turn;
         dim3 grid((ctx->L + 8 * kCtaQX - 1) / (8 * kCtaQX), (ctx->L + 8 * kCtaQY - 1) / (8 * kCtaQY));
-        VOR_LAUNCH(label_cta_kernel, grid, kCtaThreads, 0, stream, p, d_labels);
+        if (rs) {
+            p.col_left = ctx->d_fu_cols;
+            p.col_right = ctx->d_fu_cols + (size_t)(ctx->L / 32) * ctx->L;
+            VOR_LAUNCH(label_cta_kernel<true>, grid, kCtaThreads, 0, stream, p, d_labels, *rs);
+        } else {
+            VOR_LAUNCH(label_cta_kernel<false>, grid, kCtaThreads, 0, stream, p, d_labels, RowSet{});
+        }
         // second pass over the unproven quadrants with the 8 x 8 tile geometry
         LabelParams p8 = p;
         const double h8 = 128.0 * 7;
@@ -962,19 +963,32 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
         VOR_LAUNCH(label_fixup_kernel, 4 * ctx->num_sms, kWarpsPerCta * 32, 0, stream, p8, d_labels);
         return VOR_OK;
     }
-    if (path == 4) {
-        p.tiles_x = (ctx->L + 31) / 32;
-        p.tiles_y = (ctx->L + 15) / 16;
-        const int64_t wtiles = (int64_t)p.tiles_x * p.tiles_y;
-        VOR_LAUNCH(label_wide_kernel, (unsigned)((wtiles + kWarpsPerCta - 1) / kWarpsPerCta),
-                   kWarpsPerCta * 32, 0, stream, p, d_labels);
-        return VOR_OK;
-    }
     const int64_t tiles = (int64_t)p.tiles_x * p.tiles_y;
     const unsigned grid = (unsigned)((tiles + kWarpsPerCta - 1) / kWarpsPerCta);
-    if (path == 2)
-        VOR_LAUNCH((label_tile_kernel<16, 16>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels, use_fast);
-    else
-        VOR_LAUNCH((label_tile_kernel<8, 8>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels, use_fast);
+    VOR_LAUNCH((label_tile_kernel<8, 8>), grid, kWarpsPerCta * 32, 0, stream, p, d_labels, use_fast);
     return VOR_OK;
+}
+
+extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label: null labels");
+    if (ctx->nb <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label: call vor_build_cells first");
+    return label_launch(ctx, d_labels, nullptr, (cudaStream_t)stream_);
+}
+
+// Can the current cell list take the fused label -> edge path (vor_label_edges)?  It is written for the
+// CTA kernel's 32 x 32 tiles on a lattice they tile exactly.
+bool vor_label_fusable(const vor_ctx* ctx) {
+    if (ctx->nb <= 0 || ctx->L % 32 != 0 || !ctx->fuse) return false;
+    if ((int64_t)(ctx->L / 32) * (ctx->L / 32) * kTileKeys > ctx->max_raw_keys) return false;   // raw slots per tile
+    return label_path_for(ctx, sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint)) == 3;
+}
+
+// Labels + the adjacent pairs inside every 32 x 32 tile (inserted into the rows of rs); fills the compact
+// border columns and the list of tiles left to vor_edges_fused_tail (edges.cu).
+int vor_label_fused(vor_ctx* ctx, int32_t* d_labels, const RowSet& rs, cudaStream_t stream) {
+    if (!ctx->d_fu_cols) {
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_cols, 2 * (size_t)(ctx->L / 32) * ctx->L * sizeof(int32_t)));
+    }
+    return label_launch(ctx, d_labels, &rs, stream);
 }

@@ -39,6 +39,31 @@ def gpu_edges(v: Vor, labels, cap=None):
     return u64(out, int(n.item())).copy()
 
 
+def gpu_edges_rows(v: Vor, labels, n_rows, cap=None):
+    """vor_edges_rows on a host label image -> (keys, row_ptr[n_rows + 1])."""
+    cap = cap or max(1024, 8 * v.max_sites)
+    d = dev(labels.astype(np.int32).ravel())
+    out = torch.empty(cap, dtype=torch.int64, device="cuda")
+    n = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ptr = torch.full((n_rows + 1,), -1, dtype=torch.int32, device="cuda")
+    v.vor_edges_rows(d, out, n, ptr)
+    v.vor_sync_status()
+    return u64(out, int(n.item())).copy(), ptr.cpu().numpy().view(np.uint32).astype(np.int64)
+
+
+def gpu_diff_rows(v: Vor, prev, prev_ptr, now, now_ptr, n_rows):
+    cap = max(1, len(prev) + len(now))
+    mk = lambda a: dev(np.asarray(a, np.uint64).view(np.int64)) if len(a) else torch.empty(1, dtype=torch.int64, device="cuda")
+    mp = lambda a: dev(np.asarray(a, np.int64).astype(np.uint32).view(np.int32))
+    c = torch.empty(cap, dtype=torch.int64, device="cuda")
+    d = torch.empty(cap, dtype=torch.int64, device="cuda")
+    nc = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nd = torch.zeros(1, dtype=torch.int64, device="cuda")
+    v.vor_diff_rows(mk(prev), mp(prev_ptr), mk(now), mp(now_ptr), n_rows, c, d, nc, nd)
+    v.vor_sync_status()
+    return u64(c, int(nc.item())).copy(), u64(d, int(nd.item())).copy()
+
+
 def gpu_diff(v: Vor, prev, now, p2n=None, n2p=None):
     cap = max(1, len(prev) + len(now))
     dp = dev(np.asarray(prev, np.uint64).view(np.int64)) if len(prev) else torch.empty(1, dtype=torch.int64, device="cuda")

@@ -30,13 +30,13 @@ def rnd(seed, L, n):
 
 
 # ------------------------------------------------------------------ labels (a1 + a2)
-def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3, 4, 5), ref=None, occ=None):
+def check_labels(G, L, sx, sy, paths=(0, 1, 2, 3), ref=None, occ=None):
     ref = oracle.label_brute(L, sx, sy) if ref is None else ref
     v = make(L, max(len(sx), 1))
     if occ:
         v.vor_set_option("bucket_occupancy_x100", occ)
     for path in paths:
-        for fast_off in ((0, 1) if path in (0, 2, 3) else (0,)):
+        for fast_off in ((0, 1) if path in (0, 2) else (0,)):
             v.vor_set_option("label_path", path)
             v.vor_set_option("label_fast_off", fast_off)
             got = G.gpu_labels(v, sx, sy)
@@ -114,7 +114,7 @@ def test_labels_halo_independent(G, halo):
     ref = oracle.label_cells(512, sx, sy, 16)
     v = make(512, len(sx))
     v.vor_set_option("label_halo_x100", halo)
-    for path in (2, 3, 4, 5):
+    for path in (2, 3):
         v.vor_set_option("label_path", path)
         assert np.array_equal(G.gpu_labels(v, sx, sy), ref)
     v.close()
@@ -203,6 +203,110 @@ def test_edges_capacity_overflow_is_reported(G):
     v.close()
 
 
+def test_edges_tiny_raw_key_scratch_is_still_exact(G):
+    """max_raw_keys far below the number of CTA-distinct keys: the emit kernels' raw list fills up and the
+    remaining keys go straight to the adjacency rows; the result must not change."""
+    w = W.scaled(5, 1024)
+    sx, sy = next(iter(w.frames(1)))
+    lab = oracle.label_cells(w.L, sx, sy, 16)
+    ref = oracle.edges(lab)
+    for generic in (0, 1):
+        v = make(w.L, w.n_sites, max_raw_keys=1000)
+        v.vor_set_option("edges_generic", generic)
+        for _ in range(2):                              # twice: stale keys of the first call must not leak
+            assert np.array_equal(G.gpu_edges(v, lab, cap=len(ref) + 10), ref)
+        v.close()
+
+
+def row_offsets(keys, n_rows):
+    """row_ptr by definition: offset of the first key whose smaller label is >= a."""
+    return np.searchsorted(keys >> np.uint64(32), np.arange(n_rows + 1, dtype=np.uint64), side="left")
+
+
+@pytest.mark.parametrize("slots", [16, 4])
+def test_edges_rows_offsets_and_row_diff(G, slots):
+    """vor_edges_rows returns the compressed adjacency matrix; vor_diff_rows compares
+    two of them row by row.  Also with rows that spilled to the sorted overflow path (4 slots)."""
+    w = W.scaled(5, 1024)
+    v = make(w.L, w.n_sites)
+    v.vor_set_option("row_slots", slots)
+    lists = []
+    for sx, sy in w.frames(3):
+        lab = oracle.label_cells(w.L, sx, sy, 16)
+        e, ptr = G.gpu_edges_rows(v, lab, w.n_sites)
+        ref = oracle.edges(lab)
+        assert np.array_equal(e, ref)
+        assert np.array_equal(ptr, row_offsets(ref, w.n_sites))
+        lists.append((e, ptr))
+    empty = (np.empty(0, np.uint64), np.zeros(w.n_sites + 1, np.int64))
+    for (a, pa), (b, pb) in ((empty, lists[0]), (lists[0], lists[1]), (lists[1], lists[2]), (lists[2], lists[2]),
+                             (lists[2], empty)):
+        c, d = G.gpu_diff_rows(v, a, pa, b, pb, w.n_sites)
+        rc, rd = oracle.diff(a, b)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd)
+    v.close()
+
+
+def test_diff_rows_long_rows_and_random_graphs(G):
+    """Rows longer than the in-register path (hubs), empty rows, several batches per block."""
+    rng = np.random.default_rng(23)
+    v = make(64, 64)
+    for n, m in ((1, 0), (5, 6), (300, 2000), (3000, 9000), (700000, 2000000)):
+        def graph(hub):
+            i = rng.integers(0, n, m); j = rng.integers(0, n, m)
+            if hub and n > 100:                            # vertex 3 touches ~half of the others: a long row
+                i = np.concatenate([i, np.full(n // 2, 3)]); j = np.concatenate([j, rng.integers(0, n, n // 2)])
+            keep = i != j
+            lo, hi = np.minimum(i, j)[keep].astype(np.uint64), np.maximum(i, j)[keep].astype(np.uint64)
+            return np.unique((lo << np.uint64(32)) | hi)
+        a = graph(True)
+        b = np.unique(np.concatenate([a[rng.random(len(a)) < 0.9], graph(False)[: max(1, m // 10)]])) if m else a
+        c, d = G.gpu_diff_rows(v, a, row_offsets(a, n), b, row_offsets(b, n), n)
+        rc, rd = oracle.diff(a, b)
+        assert np.array_equal(c, rc) and np.array_equal(d, rd), (n, m)
+    v.close()
+
+
+def test_overflowed_lists_chain_safely(G):
+    """a vor_edges call whose output overflowed reports the REQUIRED count; vor_diff and
+    vor_events chained behind it clamp to the buffer capacities instead of reading past them."""
+    from paper_1607_00908_b200.binding import VorError, VOR_ECAPACITY
+    w = W.scaled(5, 512)
+    fr = list(w.frames(2))
+    labs = [oracle.label_cells(w.L, sx, sy, 16) for sx, sy in fr]
+    refs = [oracle.edges(l) for l in labs]
+    v = make(w.L, w.n_sites)
+    cap = 500                                            # far below the ~2900 edges
+    i64 = dict(dtype=torch.int64, device="cuda"); i32 = dict(dtype=torch.int32, device="cuda")
+    e = [torch.full((cap + 64,), -1, **i64) for _ in range(2)]
+    n = [torch.zeros(1, **i64) for _ in range(2)]
+    for k in range(2):
+        v.lib.vor_edges(v.h, G.dev(labs[k].ravel()).data_ptr(), e[k].data_ptr(), cap, n[k].data_ptr(), None)
+    c, d = torch.full((cap + 64,), -1, **i64), torch.full((cap + 64,), -1, **i64)
+    nc, nd = torch.zeros(1, **i64), torch.zeros(1, **i64)
+    v.lib.vor_diff(v.h, e[0].data_ptr(), n[0].data_ptr(), e[1].data_ptr(), n[1].data_ptr(), cap, cap, None, None, 0, 0,
+                   c.data_ptr(), d.data_ptr(), cap, nc.data_ptr(), nd.data_ptr(), None)
+    nl = w.n_sites
+    trig, idx, cp, cn = (torch.empty(nl, **i32) for _ in range(4))
+    m, g = torch.zeros(1, **i32), torch.zeros(1, **i32)
+    v.lib.vor_events(v.h, e[0].data_ptr(), n[0].data_ptr(), e[1].data_ptr(), n[1].data_ptr(), cap, cap,
+                     c.data_ptr(), nc.data_ptr(), d.data_ptr(), nd.data_ptr(), cap, cap, nl,
+                     trig.data_ptr(), idx.data_ptr(), m.data_ptr(), g.data_ptr(), cp.data_ptr(), cn.data_ptr(), None)
+    with pytest.raises(VorError) as ex:
+        v.vor_sync_status()
+    assert ex.value.status == VOR_ECAPACITY
+    assert [int(t.item()) for t in n] == [len(r) for r in refs]          # required counts
+    for k in range(2):                                                   # guards untouched, prefix correct
+        assert bool((e[k][cap:] == -1).all()) and np.array_equal(G.u64(e[k], cap), refs[k][:cap])
+    # the chained calls saw exactly the clamped lists
+    rc, rd = oracle.diff(refs[0][:cap], refs[1][:cap])
+    assert int(nc.item()) == len(rc) and int(nd.item()) == len(rd)
+    assert np.array_equal(G.u64(c, min(cap, len(rc))), rc[:cap]) and bool((c[cap:] == -1).all())
+    ev = oracle.events(refs[0][:cap], refs[1][:cap], nl)
+    assert np.array_equal(trig.cpu().numpy(), ev["trigger"])
+    v.close()
+
+
 # ------------------------------------------------------------------ diff (a5)
 def test_diff_hand_and_random(G):
     v = make(64, 64)
@@ -267,7 +371,7 @@ def test_rhombus_flip_end_to_end_golden(G):
 
 
 # ------------------------------------------------------------------ frame pipeline (a1..a5 chained)
-@pytest.mark.parametrize("cfg,L,nfr", [(1, None, 2), (2, None, 4), (5, 1024, 4)])
+@pytest.mark.parametrize("cfg,L,nfr", [(1, None, 2), (2, None, 100), (5, 1024, 10)])
 def test_frame_host_sequence_matches_oracle(G, cfg, L, nfr):
     w = W.config(cfg) if L is None else W.scaled(cfg, L)
     v = make(w.L, w.n_sites)
@@ -286,6 +390,45 @@ def test_frame_host_sequence_matches_oracle(G, cfg, L, nfr):
         assert np.array_equal(G.u64(G.from_device_ptr(pe, len(e), torch.int64)), e)
         prev = e
     v.close()
+
+
+FUSED_CASES = [a for a in ADVERSARIAL if a[1] % 32 == 0] + [
+    ("uniform_sparse", 512, lambda rng, P: (rng.integers(0, P, 400).astype(np.int32), rng.integers(0, P, 400).astype(np.int32))),
+    ("two_sites", 32, lambda rng, P: (np.array([100, 5000], np.int32), np.array([200, 7000], np.int32))),
+    ("stripes", 256, lambda rng, P: ((np.arange(12) * (P // 12) + 77).astype(np.int32), np.full(12, P // 2, np.int32))),
+]
+
+
+@pytest.mark.parametrize("name,L,gen", FUSED_CASES, ids=[a[0] for a in FUSED_CASES])
+def test_frame_fused_label_edges_adversarial(G, name, L, gen):
+    """vor_frame_* labels and extracts the pairs in ONE kernel where the lattice allows it (L % 32 == 0,
+    CTA labelling path); tiles with an unproven quadrant, the tile seams and the periodic wrap take the
+    side paths.  Labels, edge list and flips must equal the oracle's, and the unfused calls' results."""
+    rng = np.random.default_rng(abs(hash(name)) % 2**32)
+    P = FP * L
+    sx, sy = gen(rng, P)
+    frames = [(sx, sy), (((sx.astype(np.int64) + rng.integers(-600, 600, len(sx))) % P).astype(np.int32),
+                         ((sy.astype(np.int64) + rng.integers(-600, 600, len(sy))) % P).astype(np.int32))]
+    cap = max(64, 16 * len(sx))
+    for fuse_off in (0, 1):
+        v = make(L, len(sx))
+        v.vor_set_option("fuse", 1 - fuse_off)
+        v.vor_set_option("label_path", 3)            # the fused path belongs to the CTA kernel
+        hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+        prev = np.empty(0, np.uint64)
+        for fx, fy in frames:
+            v.vor_frame_host(fx, fy, hc, hd, cnt)
+            lab = oracle.label_brute(L, fx, fy)
+            e = oracle.edges(lab)
+            rc, rd = oracle.diff(prev, e)
+            pl, pe, _, _, _ = v.vor_frame_results()
+            got = G.from_device_ptr(pl, L * L, torch.int32).cpu().numpy().reshape(L, L)
+            assert np.array_equal(got, lab), (fuse_off, int((got != lab).sum()))
+            assert cnt.tolist() == [len(e), len(rc), len(rd)], (fuse_off, cnt.tolist(), len(e), len(rc), len(rd))
+            assert np.array_equal(G.u64(G.from_device_ptr(pe, len(e), torch.int64)), e)
+            assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd)
+            prev = e
+        v.close()
 
 
 @pytest.mark.parametrize("pin", [False, True])
@@ -414,6 +557,102 @@ def test_field_pipeline_scaled_configs(G, cfg, L, nfr):
     v.close()
 
 
+def oracle_field_chain(w, fields):
+    """The oracle's chain a6 -> a7 -> a8 -> a1..a5 (maps) frame by frame: (K, edges, created, destroyed, parts)."""
+    L, R = w.L, int(w.match_radius_cells * FP)
+    prev_c, prev_e = None, None
+    for field in fields:
+        ccl = oracle.threshold_ccl(field, w.threshold, True)
+        c = oracle.centroids(ccl, w.min_size)
+        lab = oracle.label_cells(L, c["sx"], c["sy"], 16 if L % 16 == 0 else 1)
+        e = oracle.edges(lab)
+        if prev_c is None:
+            rc = rd = np.empty(0, np.uint64)
+            maps = None
+        else:
+            maps = oracle.match(L, prev_c["sx"], prev_c["sy"], c["sx"], c["sy"], R)
+            rc, rd = oracle.diff(prev_e, e, *maps)
+        yield len(c["sx"]), e, rc, rd, dict(ccl=ccl, comp=c, labels=lab, maps=maps)
+        prev_c, prev_e = c, e
+
+
+@pytest.mark.parametrize("cfg,L,nfr", [(3, 512, 4), (4, 512, 3), (3, None, None), (4, None, None)])
+def test_field_frames_chained_on_the_device(G, cfg, L, nfr):
+    """field_frame_submit / field_frame_collect: the whole field-driven frame chained on the device (GPU
+    bubbles -> GPU centroids -> GPU maps -> GPU labels -> GPU edges -> GPU diff with the GPU maps, no host
+    sync in between), compared with the oracle chain.  L = None: every frame of the configuration at its
+    full BASELINE.json size (config 3: 50 frames of 2048^2, config 4: 20 frames of 4096^2)."""
+    w = W.config(cfg) if L is None else W.scaled(cfg, L)
+    L = w.L
+    v = make(L, 65536)
+    R = int(w.match_radius_cells * FP)
+    cap = 8 * 65536
+    hc, hd, cnt = np.empty(cap, np.uint64), np.empty(cap, np.uint64), np.zeros(4, np.int64)
+    fields = list(w.frames(nfr))
+    refs = oracle_field_chain(w, fields)
+
+    def collect(k):
+        v.field_frame_collect(hc, hd, cnt)
+        K, e, rc, rd, _ = next(refs)
+        assert cnt.tolist() == [K, len(e), len(rc), len(rd)], (k, cnt.tolist(), K, len(e), len(rc), len(rd))
+        assert np.array_equal(hc[:cnt[2]], rc) and np.array_equal(hd[:cnt[3]], rd), k
+        assert K > 3
+
+    v.field_frame_submit(fields[0].ravel(), w.threshold, True, w.min_size, R)
+    for k in range(1, len(fields)):
+        v.field_frame_submit(fields[k].ravel(), w.threshold, True, w.min_size, R)
+        collect(k - 1)
+    collect(len(fields) - 1)
+    v.close()
+
+
+def test_field_frame_device_results(G):
+    """field_frame_device on device-resident fields: every intermediate the context exposes (bubble image,
+    centroids, maps, labels, edges) equals the oracle's, and a new sequence starts after vor_frame_reset."""
+    w = W.scaled(3, 512)
+    L = w.L
+    v = make(L, 4096)
+    R = int(w.match_radius_cells * FP)
+    fields = list(w.frames(3))
+    for rep in range(2):
+        for k, (K, e, rc, rd, parts) in enumerate(oracle_field_chain(w, fields)):
+            v.field_frame_device(G.dev(fields[k].ravel()), w.threshold, True, w.min_size, R)
+            v.vor_sync_status()
+            r = v.field_frame_results()
+            get = lambda name, n, dt: G.from_device_ptr(r[name], n, dt).cpu().numpy()
+            assert get("counts", 4, torch.int64).tolist() == [K, len(e), len(rc), len(rd)]
+            assert np.array_equal(get("ccl", L * L, torch.int32).reshape(L, L), parts["ccl"])
+            assert np.array_equal(get("labels", L * L, torch.int32).reshape(L, L), parts["labels"])
+            for name in ("sx", "sy", "size", "root"):
+                assert np.array_equal(get(name, K, torch.int32), parts["comp"][name]), name
+            assert np.abs(get("cx", K, torch.float64) - parts["comp"]["cx"]).max() <= 1e-9
+            assert np.abs(get("cy", K, torch.float64) - parts["comp"]["cy"]).max() <= 1e-9
+            assert np.array_equal(get("edges", len(e), torch.int64).view(np.uint64), e)
+            assert np.array_equal(get("created", len(rc), torch.int64).view(np.uint64), rc)
+            assert np.array_equal(get("destroyed", len(rd), torch.int64).view(np.uint64), rd)
+            if parts["maps"] is not None:
+                assert np.array_equal(get("p2n", len(parts["maps"][0]), torch.int32), parts["maps"][0])
+                assert np.array_equal(get("n2p", K, torch.int32), parts["maps"][1])
+        v.vor_frame_reset()
+    v.close()
+
+
+def test_build_cells_dev_count_on_the_device(G):
+    """vor_build_cells_dev: the number of sites is a device scalar below the capacity; labels equal the
+    oracle's on the first n sites whatever the hint; zero sites give -1 everywhere."""
+    L = 256
+    sx, sy = rnd(3, L, 500)
+    v = make(L, 500)
+    lab = torch.empty(L * L, dtype=torch.int32, device="cuda")
+    for n, hint in ((500, 0), (137, 500), (137, 10), (1, 0), (0, 0)):
+        v.vor_build_cells_dev(G.dev(sx), G.dev(sy), torch.tensor([n], dtype=torch.int32, device="cuda"), hint)
+        v.vor_label(lab)
+        v.vor_sync_status()
+        ref = oracle.label_brute(L, sx[:n], sy[:n]) if n else np.full((L, L), -1, np.int32)
+        assert np.array_equal(lab.cpu().numpy().reshape(L, L), ref), (n, hint)
+    v.close()
+
+
 def test_match_invariants_and_random(G):
     v = make(64, 256)
     rng = np.random.default_rng(13)
@@ -494,30 +733,37 @@ def test_events_hand_random_and_golden(G):
 
 
 # ------------------------------------------------------------------ full size, bench.py's launch configuration
-def test_config5_full_size_two_frames(G):
-    """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites) through the same calls, buffers
-    and capacities bench.py times.  Every label, edge key and flip is compared with the oracle
-    (O1b finishes a full frame in seconds), and O1b itself is cross-checked here against brute force
-    over all 10^6 sites on sampled cells."""
+def test_config5_full_size_all_frames(G):
+    """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites), ALL 10 frames of the random walk,
+    through the same calls, buffers and capacities bench.py times.  Every label, edge key, row offset and
+    flip of every frame is compared with the oracle (O1b finishes a full frame in seconds), and O1b itself
+    is cross-checked here against brute force over all 10^6 sites on sampled cells.  The later frames are
+    the disordered regime (candidate lists overflow, quadrants go to the fix-up pass)."""
     w = W.config(5)
     L, n = w.L, w.n_sites
     v = make(L, n, max_raw_keys=max(1 << 20, 16 * n))
     cap_e = 4 * n + 1024
-    labels = torch.empty(L * L, dtype=torch.int32, device="cuda")
-    edges = [torch.empty(cap_e, dtype=torch.int64, device="cuda") for _ in range(2)]
-    n_edges = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(2)]
-    created = torch.empty(cap_e, dtype=torch.int64, device="cuda")
-    destroyed = torch.empty(cap_e, dtype=torch.int64, device="cuda")
-    n_c = torch.zeros(1, dtype=torch.int64, device="cuda")
-    n_d = torch.zeros(1, dtype=torch.int64, device="cuda")
+    i64 = dict(dtype=torch.int64, device="cuda"); i32 = dict(dtype=torch.int32, device="cuda")
+    labels = torch.empty(L * L, **i32)
+    edges = [torch.empty(cap_e, **i64) for _ in range(2)]
+    n_edges = [torch.zeros(1, **i64) for _ in range(2)]
+    row_ptr = [torch.zeros(n + 1, **i32) for _ in range(2)]
+    created, destroyed = torch.empty(cap_e, **i64), torch.empty(cap_e, **i64)
+    created2, destroyed2 = torch.empty(cap_e, **i64), torch.empty(cap_e, **i64)
+    n_c, n_d, n_c2, n_d2 = (torch.zeros(1, **i64) for _ in range(4))
     rng = np.random.default_rng(5)
     prev = np.empty(0, np.uint64)
-    for i, (sx, sy) in enumerate(w.frames(2)):
+    assert w.n_frames == 10
+    vf = make(L, n, max_raw_keys=max(1 << 20, 16 * n))   # the frame call, with the fused label -> edge kernel
+    vf.vor_set_option("fuse", 1)
+    for i, (sx, sy) in enumerate(w.frames()):
         now, prv = i & 1, 1 - (i & 1)
+        vf.vor_frame_device(G.dev(sx), G.dev(sy))
         v.vor_build_cells(G.dev(sx), G.dev(sy))
         v.vor_label(labels)
-        v.vor_edges(labels, edges[now], n_edges[now])
-        v.vor_diff(edges[prv], n_edges[prv], edges[now], n_edges[now], created, destroyed, n_c, n_d)
+        v.vor_edges_rows(labels, edges[now], n_edges[now], row_ptr[now])
+        v.vor_diff_rows(edges[prv], row_ptr[prv], edges[now], row_ptr[now], n, created, destroyed, n_c, n_d)
+        v.vor_diff(edges[prv], n_edges[prv], edges[now], n_edges[now], created2, destroyed2, n_c2, n_d2)
         v.vor_sync_status()
         ref = oracle.label_cells(L, sx, sy, w.bucket_cells)
         got = labels.cpu().numpy().reshape(L, L)
@@ -525,12 +771,20 @@ def test_config5_full_size_two_frames(G):
         cells = rng.integers(0, L * L, 1500)
         assert np.array_equal(ref.ravel()[cells], oracle.label_brute_at(L, sx, sy, cells))
         e = oracle.edges(ref)
-        assert np.array_equal(G.u64(edges[now], int(n_edges[now].item())), e)
+        assert np.array_equal(G.u64(edges[now], int(n_edges[now].item())), e), i
+        assert np.array_equal(row_ptr[now].cpu().numpy().view(np.uint32), row_offsets(e, n)), i
         rc, rd = oracle.diff(prev, e)
-        assert np.array_equal(G.u64(created, int(n_c.item())), rc)
-        assert np.array_equal(G.u64(destroyed, int(n_d.item())), rd)
-        if i == 1:                                  # event layer at full size, on the device-resident lists
-            i32 = dict(dtype=torch.int32, device="cuda")
+        for c_, d_, nc_, nd_ in ((created, destroyed, n_c, n_d), (created2, destroyed2, n_c2, n_d2)):
+            assert np.array_equal(G.u64(c_, int(nc_.item())), rc), i
+            assert np.array_equal(G.u64(d_, int(nd_.item())), rd), i
+        vf.vor_sync_status()
+        pl, pe, pc, pd, pn = vf.vor_frame_results()
+        assert G.from_device_ptr(pn, 3, torch.int64).cpu().tolist() == [len(e), len(rc), len(rd)], i
+        assert bool((G.from_device_ptr(pl, L * L, torch.int32) == labels).all()), i
+        assert np.array_equal(G.u64(G.from_device_ptr(pe, len(e), torch.int64)), e), i
+        assert np.array_equal(G.u64(G.from_device_ptr(pc, len(rc), torch.int64)), rc), i
+        assert np.array_equal(G.u64(G.from_device_ptr(pd, len(rd), torch.int64)), rd), i
+        if i in (1, 9):                             # event layer at full size, on the device-resident lists
             trig, idx, cp, cn = (torch.empty(n, **i32) for _ in range(4))
             m, g = torch.zeros(1, **i32), torch.zeros(1, **i32)
             v.vor_events(edges[prv], n_edges[prv], edges[now], n_edges[now], created, n_c, destroyed, n_d,
@@ -543,4 +797,4 @@ def test_config5_full_size_two_frames(G):
         prev = e
         del ref, got
     assert 2.9 * n < len(prev) < 3.0 * n            # E slightly below 3N (R6), as the survey's probe found
-    v.close()
+    v.close(); vf.close()

@@ -80,3 +80,16 @@ def test_rhombus_construction_golden():
     assert ev["events_indices"].tolist() == g["events_indices"]
     assert ev["count_prev"][:4].tolist() == g["count_prev"] and ev["count_now"][:4].tolist() == g["count_now"]
     assert ev["global_trigger"] == 1 and ev["trigger"].sum() == 4
+
+
+def test_keys_with_a_label_beyond_n_are_ignored():
+    """vor.h: "keys with a label >= n_labels are ignored" - pinned against the python-set brute force on
+    the lists with those keys removed by hand."""
+    prev = [(0, 1), (1, 2), (0, 2), (1, 5), (2, 7), (5, 7)]
+    now = [(0, 1), (1, 2), (2, 6), (0, 5), (5, 7)]
+    n = 4
+    ev = oracle.events(pack(prev), pack(now), n)
+    trig, idx, cp, cn = brute([p for p in prev if max(p) < n], [p for p in now if max(p) < n], n)
+    assert trig == [1, 0, 1, 0]                    # only (0,2) disappeared among the labels < 4
+    assert ev["trigger"].tolist() == trig and ev["events_indices"].tolist() == idx
+    assert ev["count_prev"].tolist() == cp == [1, 0, 1, 0] and ev["count_now"].tolist() == cn == [0, 0, 0, 0]

@@ -117,6 +117,27 @@ def test_centroid_hand_case_floor_rounding():
     assert c["sx"][0] == 5 * FP + 128 - 86 and abs(c["cx"][0] - (5.5 - 1 / 3)) < 1e-12
 
 
+def test_centroid_upper_wrap_branch_hand_case():
+    """Root (minimum index) at x = L-2 with the lower rows wrapping to x = 0..3: the unwrapped mean lies
+    beyond L and must come back by -L (the `>= L` branch).  Expected value by hand: unwrapped cell
+    centres x = 14.5, 15.5 | 15.5, 16.5, 17.5, 18.5, 19.5 | 16.5, 17.5, 18.5, 19.5 -> sum 189.5, n 11."""
+    L = 16
+    f = np.zeros((L, L), np.float32)
+    f[3, 14] = f[3, 15] = 2
+    f[4, 15] = f[4, 0] = f[4, 1] = f[4, 2] = f[4, 3] = 2
+    f[5, 0] = f[5, 1] = f[5, 2] = f[5, 3] = 2
+    for g, (kx, ky, ks, kt) in ((f, ("cx", "cy", "sx", "sy")), (np.ascontiguousarray(f.T), ("cy", "cx", "sy", "sx"))):
+        c = oracle.centroids(oracle.threshold_ccl(g, 1.0), 1)
+        assert len(c["cx"]) == 1 and c["size"][0] == 11
+        assert abs(c[kx][0] - (189.5 / 11 - L)) < 1e-12          # 1.2272...: wrapped back into [0, L)
+        assert abs(c[ky][0] - (3.5 * 2 + 4.5 * 5 + 5.5 * 4) / 11) < 1e-12
+        # fixed point: floor(256 * 30 / 11) = 698 past the root's centre 14.5, mod P
+        assert c[ks][0] == (14 * FP + 128 + (FP * 30) // 11) % (FP * L)
+        assert c[kt][0] == 3 * FP + 128 + (FP * (5 + 8)) // 11
+    # the root itself: row-major minimum (3,14) for f; for the transpose the minimum index is (0,4)
+    assert oracle.centroids(oracle.threshold_ccl(f, 1.0), 1)["root"][0] == 3 * L + 14
+
+
 def test_centroids_shift_equivariance_and_min_size():
     rng = np.random.default_rng(9)
     L = 96
