@@ -25,14 +25,29 @@ sys.path.insert(0, ROOT)
 
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
-# Algorithmic integer work of exact labelling per lattice cell: 7 candidate sites (a
-# Voronoi region has 6 neighbours on average, plus the owner) x 3 ops (two multiply-adds of the
-# distance expansion, one min) + 1 store.
-LABEL_OPS_PER_CELL = 22
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1g_full_summary.md); config 5 only.
-NCU_TRAFFIC_BYTES = {"label_cta_kernel": 1.035e9, "edges_stream_kernel": 1.098e9, "rows_insert_kernel": 0.082e9,
-                     "edges_finish_kernel": 0.094e9, "diff_kernel": 0.048e9}
+# Per-launch ncu figures of the committed `ncu --set full` capture (config 5 only): DRAM bytes read + written,
+# issue-slot utilisation, warp instructions.  profiles/r2_traffic.md names the command that produced the table.
+NCU_TABLE = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+
+
+def ncu_table():
+    """kernel name -> dict of floats; {} when the table is missing."""
+    out = {}
+    if os.path.exists(NCU_TABLE):
+        import csv
+        with open(NCU_TABLE) as f:
+            for row in csv.DictReader(f):
+                out[row["kernel"]] = {k: float(v) for k, v in row.items() if k != "kernel" and v not in ("", None)}
+    return out
+
+
+def ncu_for(table, name):
+    """ncu row of the kernel whose name starts like `name` (template arguments are spelled differently)."""
+    base = name.split("<")[0]
+    for k, v in table.items():
+        if k.split("<")[0] == base:
+            return v
+    return {}
 
 
 def edges_bytes(cells, n_edges):
@@ -52,6 +67,7 @@ def parse():
     ap.add_argument("--workload", default="cfg5", help="cfg5 (default) | cfg1 | cfg2 | cfg5@L e.g. cfg5@4096 | cfg3 | cfg4 (field path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-field-leg", action="store_true", help="skip the short config-4 field-path leg of the default line")
     ap.add_argument("--cpu-sample-L", type=int, default=0,
                     help="lattice side of the oracle's sample (0 = full workload for ours, 4096 for reference)")
     return ap.parse_args()
@@ -146,13 +162,14 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle legs
-def oracle_frame_seconds(w, frames):
-    """Time the oracle, as it stands, on `frames` (list of (sx, sy)); returns (seconds, cells)."""
+def oracle_frame_seconds(w, frames, threads=0):
+    """Time the oracle, as it stands, on `frames` (list of (sx, sy)); returns (seconds, cells).
+    threads: OpenMP threads of the labelling (0 = all the process may use); edges and diff are serial."""
     import oracle
     prev = np.empty(0, np.uint64)
     t0 = time.perf_counter()
     for sx, sy in frames:
-        lab = oracle.label_cells(w.L, sx, sy, w.bucket_cells)
+        lab = oracle.label_cells(w.L, sx, sy, w.bucket_cells, threads)
         e = oracle.edges(lab)
         oracle.diff(prev, e)
         prev = e
@@ -187,6 +204,13 @@ def run_reference(args, w):
 
 
 # ------------------------------------------------------------------------------------------ our arm
+def frame_algorithmic_bytes(cells, n_sites, e_prev, e_now, n_c, n_d):
+    """What one site-driven frame must move: the label image written (a2) and read (a3),
+    the edge list written (a4) and both lists read by the comparison (a5), the flip lists written, and the
+    cell list (about 40 B per site)."""
+    return 8.0 * cells + 8.0 * e_now + 8.0 * (e_prev + e_now) + 8.0 * (n_c + n_d) + 40.0 * n_sites
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
@@ -195,6 +219,8 @@ def run_ours(args, w):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
@@ -221,6 +247,7 @@ def run_ours(args, w):
     labels = torch.empty(L * L, dtype=torch.int32, device="cuda")
     edges = [torch.empty(cap_e, dtype=torch.int64, device="cuda") for _ in range(2)]
     n_edges = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(2)]
+    row_ptr = [torch.zeros(n + 1, dtype=torch.int32, device="cuda") for _ in range(2)]
     created = torch.empty(cap_e, dtype=torch.int64, device="cuda")
     destroyed = torch.empty(cap_e, dtype=torch.int64, device="cuda")
     n_c = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -228,6 +255,8 @@ def run_ours(args, w):
     stream = torch.cuda.current_stream()
     names = ["build_cells", "label", "edges", "diff"]
 
+    # One step = a1..a5 through the C ABI: cell list, labels, edge list with its row offsets (the
+    # compressed adjacency matrix), row-by-row comparison with the previous frame's list.
     def step(i, ev=None):
         now, prev = i & 1, 1 - (i & 1)
         sx, sy = dframes[i]
@@ -236,9 +265,9 @@ def run_ours(args, w):
         if ev: ev[1].record(stream)
         v.vor_label(labels)
         if ev: ev[2].record(stream)
-        v.vor_edges(labels, edges[now], n_edges[now])
+        v.vor_edges_rows(labels, edges[now], n_edges[now], row_ptr[now])
         if ev: ev[3].record(stream)
-        v.vor_diff(edges[prev], n_edges[prev], edges[now], n_edges[now], created, destroyed, n_c, n_d)
+        v.vor_diff_rows(edges[prev], row_ptr[prev], edges[now], row_ptr[now], n, created, destroyed, n_c, n_d)
         if ev: ev[4].record(stream)
 
     # nvidia-smi samples every 100 ms and the K timed steps take ~14 ms: the sampler runs from the
@@ -262,8 +291,9 @@ def run_ours(args, w):
     ms_total = max_over_ranks(t_beg.elapsed_time(t_end))
     kernel_ms = {nm: float(np.mean([evs[k][j].elapsed_time(evs[k][j + 1]) for k in range(K)]))
                  for j, nm in enumerate(names)}
-    counts = {"n_edges": int(n_edges[(W_ + K - 1) & 1].item()), "n_created": int(n_c.item()),
-              "n_destroyed": int(n_d.item())}
+    last = (W_ + K - 1) & 1
+    counts = {"n_edges": int(n_edges[last].item()), "n_edges_prev": int(n_edges[1 - last].item()),
+              "n_created": int(n_c.item()), "n_destroyed": int(n_d.item())}
     cells_per_step = L * L
     value = whole_job_value(world, K, cells_per_step, ms_total)
 
@@ -283,7 +313,6 @@ def run_ours(args, w):
     i32 = dict(dtype=torch.int32, device="cuda")
     ev_bufs = [torch.empty(n, **i32) for _ in range(4)]
     ev_m, ev_g = torch.zeros(1, **i32), torch.zeros(1, **i32)
-    last = (W_ + K - 1) & 1
     def events():
         v.vor_events(edges[1 - last], n_edges[1 - last], edges[last], n_edges[last], created, n_c, destroyed, n_d,
                      ev_bufs[0], ev_bufs[1], ev_m, ev_g, ev_bufs[2], ev_bufs[3])
@@ -346,48 +375,61 @@ def run_ours(args, w):
                "sync_api": "vor_frame_host, one frame at a time (copies not overlapped)"}
 
     clocks = sampler.stop()
+    v.close()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     hbm_peak, peak_src, sm_max_mhz = peaks()
-    # Dominant kernel = label_cta_kernel (one launch per step).  It is bound by plain
-    # integer issue, not by HBM: `roofline` reports it against the INT32 lane peak DESIGN.md §5.9
-    # derives (SMs x 128 lanes x max SM clock); algorithmic work = 22 integer ops per cell.
+    is_cfg5 = wr.name.startswith("cfg5_throughput_stress")
+    ncu = ncu_table() if is_cfg5 else {}
+
+    # every kernel is reported against the measured HBM copy rate with ITS algorithmic
+    # bytes; `traffic` = DRAM bytes of one launch in the committed ncu capture (config 5 only).
+    def hbm_roof(name, nbytes, what, ms=None):
+        if ms is None:
+            if name not in kernel_launch_ms:
+                return None
+            ms = kernel_launch_ms[name]
+        t = ncu_for(ncu, name)
+        r = {"kernel": name, "bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+             "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": t.get("dram_bytes"), "launch_ms": ms,
+             "algorithmic": what, "peak_source": peak_src}
+        if t:
+            r["ncu"] = {"issue_active_pct": t.get("issue_active_pct"), "warp_inst_per_cell":
+                        t["warp_inst"] / cells_per_step if "warp_inst" in t else None,
+                        "source": "profiles/r2_traffic.csv"}
+        return r
+
+    # The dominant kernel is the labelling kernel (one launch per step).  Its §8(d) unit is the 4 B/cell it
+    # writes; what actually limits it is integer issue (the nested ncu figures: issue slots busy, warp
+    # instructions per cell), which only fewer instructions can improve.
     lab_name = max((nm for nm in kernel_launch_ms if "label" in nm), key=lambda nm: kernel_launch_ms[nm])
-    label_s = kernel_launch_ms[lab_name] * 1e-3
-    alu_peak = 148 * 128 * sm_max_mhz * 1e6 / 1e12            # Tera int32 lane-ops / s
-    alu_ops = LABEL_OPS_PER_CELL * cells_per_step
-    roofline = {"kernel": lab_name, "bound": "alu", "achieved": alu_ops / label_s / 1e12, "peak": alu_peak,
-                "unit": "Tera int32 op/s", "frac": alu_ops / label_s / 1e12 / alu_peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(lab_name) if wr.name == "cfg5_throughput_stress" else None,
-                "launch_ms": kernel_launch_ms[lab_name],
-                "peak_source": "148 SMs x 128 INT32 lanes x max SM clock (DESIGN.md 5.9)",
-                "algorithmic": f"{LABEL_OPS_PER_CELL} int32 ops/cell x {cells_per_step} cells",
-                "hbm_view": {"achieved": 4.0 * cells_per_step / label_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                             "frac": 4.0 * cells_per_step / label_s / 1e9 / hbm_peak,
-                             "algorithmic": "4 B/cell label write", "peak_source": peak_src}}
-
-    def hbm_roof(name, nbytes, what):
-        if name not in kernel_launch_ms:
-            return None
-        sec = kernel_launch_ms[name] * 1e-3
-        return {"bound": "hbm", "achieved": nbytes / sec / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": nbytes / sec / 1e9 / hbm_peak, "launch_ms": kernel_launch_ms[name],
-                "traffic": NCU_TRAFFIC_BYTES.get(name) if wr.name == "cfg5_throughput_stress" else None, "algorithmic": what, "peak_source": peak_src}
-
-    ne = counts["n_edges"]
+    roofline = hbm_roof(lab_name, 4.0 * cells_per_step, "4 B/cell label write")
+    roofline["limited_by"] = "integer issue slots, not HBM (DESIGN.md 5.2, 5.9)"
+    ne, nep = counts["n_edges"], counts["n_edges_prev"]
+    ncd = counts["n_created"] + counts["n_destroyed"]
+    diff_ms = sum(kernel_launch_ms.get(k, 0.0) for k in ("diff_rows_mark_kernel", "diff_rows_write_kernel"))
     others = {
         "edges_stream_kernel": hbm_roof("edges_stream_kernel", 4.0 * cells_per_step, "4 B/cell label read"),
-        "diff_kernel": hbm_roof("diff_kernel", 16.0 * ne + 8.0 * (counts["n_created"] + counts["n_destroyed"]),
-                                "8 B x (E_prev + E_now) read + 8 B x (created + destroyed) written; L2-resident"),
-        "vor_edges (stream + insert + finish)": {
-            "bound": "hbm", "achieved": edges_bytes(cells_per_step, ne) / (kernel_ms["edges"] * 1e-3) / 1e9,
-            "peak": hbm_peak, "unit": "GB/s",
-            "frac": edges_bytes(cells_per_step, ne) / (kernel_ms["edges"] * 1e-3) / 1e9 / hbm_peak,
-            "algorithmic": "4 B/cell label read + 8 B/edge written"},
+        "vor_diff_rows (mark + write)": hbm_roof(
+            "diff_rows", 8.0 * (ne + nep) + 8.0 * ncd + 8.0 * n,
+            "8 B x (E_prev + E_now) read + 8 B x (created + destroyed) written + 2 x 4 B/site row offsets; "
+            "L2-resident", ms=diff_ms) if diff_ms > 0 else None,
+        "vor_edges_rows (stream + insert + finish)": hbm_roof(
+            "vor_edges_rows", edges_bytes(cells_per_step, ne), "4 B/cell label read + 8 B/edge written",
+            ms=kernel_ms["edges"]),
     }
+    frame_bytes = frame_algorithmic_bytes(cells_per_step, n, nep, ne, counts["n_created"], counts["n_destroyed"])
+    step_s = ms_total / K * 1e-3
+    frame_roofline = {"bound": "hbm", "achieved": frame_bytes / step_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                      "frac": frame_bytes / step_s / 1e9 / hbm_peak, "algorithmic_bytes_per_frame": frame_bytes,
+                      "algorithmic": "label image written + read, edge list written, both lists read by the "
+                                     "comparison, flip lists written, 40 B/site cell list",
+                      "peak_source": peak_src}
+    if e2e:
+        frame_roofline["e2e_frac"] = frame_bytes / (e2e["ms_per_step"] * 1e-3) / 1e9 / hbm_peak
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
         "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -400,11 +442,14 @@ def run_ours(args, w):
         "kernel_launch_ms": kernel_launch_ms, "kernel_launches_per_step": kernel_launches_per_step,
         "roofline": roofline,
         "rooflines_other": {k: r for k, r in others.items() if r},
+        "frame_roofline": frame_roofline,
         "events": events_info,
         "clocks": clocks, "gpu_launches": int(launches),
     }
     if e2e:
         out["e2e"] = e2e
+    if not args.no_field_leg and world == 1 and is_cfg5:
+        out["field_path"] = field_leg(W.config(4), 2, 4)
     if not args.no_cpu_baseline and world == 1:
         import oracle
         Ls = args.cpu_sample_L or w.L
@@ -414,100 +459,134 @@ def run_ours(args, w):
         out["cpu_baseline"] = {"value": cells / secs, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                                "sample": f"1 frame of {ws.name} ({ws.L}^2 cells, {ws.n_sites} sites): "
                                          f"label_cells + edges + diff, {secs:.1f} s"}
+        # the same oracle on ONE thread, on a 1/16-area copy of the workload
+        w1 = W.scaled(5, max(256, ws.L // 4)) if ws.kind == "jittered_grid" and ws.L >= 1024 else ws
+        s1, c1 = oracle_frame_seconds(w1, list(w1.frames(1)), threads=1)
+        out["cpu_baseline"]["single_thread"] = {
+            "value": c1 / s1, "unit": UNIT, "cores": 1,
+            "sample": f"1 frame of {w1.name} ({w1.L}^2 cells, {w1.n_sites} sites), {s1:.1f} s"}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
 # ------------------------------------------------------------------------------------------ field path
-def run_field(args, w):
-    """--workload cfg3 | cfg4: one step = one frame of the field-derived path, rows a6..a8 then a1..a5
-    (threshold+CCL -> centroids -> match -> cell list -> label -> edges -> diff with maps).  Single GPU;
-    not the default bench line (the metric is quoted on config 5) - reported for the §8(a) field rows."""
+FIELD_GROUPS = (("threshold_ccl", ("ccl_",)), ("centroids", ("comp_", "accumulate", "centroid")),
+                ("match", ("match_",)), ("build_cells", ("count_sites", "scan_", "scatter_sites")),
+                ("label", ("label_",)), ("edges", ("edges_", "rows_insert")),
+                ("diff", ("translate_", "filter_", "sort_unique", "diff_", "maps_")))
+
+
+def field_group(kernel_name: str) -> str:
+    for g, prefixes in FIELD_GROUPS:
+        if any(kernel_name.startswith(p) for p in prefixes):
+            return g
+    return "other"
+
+
+def field_leg(w, warmup: int, steps: int):
+    """Frames of a field-derived workload (config 3 or 4) through field_frame_device: rows a6..a8 then a1..a5
+    chained on the device without a host synchronisation (the bubble count stays in a device scalar).
+    Returns per-frame time (CUDA events around the K frames), per-kernel launch times from a second pass
+    and the §8(d) fractions of the field kernels."""
     import torch
     from paper_1607_00908_b200.binding import Vor
-    torch.cuda.set_device(0)
-    W_, K = args.warmup, args.steps
     L = w.L
-    frames = [torch.from_numpy(f).cuda().reshape(-1) for f in w.frames(W_ + K)]
-    cap = 1 << 16
-    v = Vor(L, cap)
-    i32 = dict(dtype=torch.int32, device="cuda")
-    ccl = torch.empty(L * L, **i32)
-    labels = torch.empty(L * L, **i32)
-    comp = [dict(cx=torch.empty(cap, dtype=torch.float64, device="cuda"), cy=torch.empty(cap, dtype=torch.float64, device="cuda"),
-                 sx=torch.empty(cap, **i32), sy=torch.empty(cap, **i32), size=torch.empty(cap, **i32),
-                 root=torch.empty(cap, **i32), n=torch.zeros(1, **i32)) for _ in range(2)]
-    p2n, n2p = torch.empty(cap, **i32), torch.empty(cap, **i32)
-    cap_e = 8 * cap
-    edges = [torch.empty(cap_e, dtype=torch.int64, device="cuda") for _ in range(2)]
-    n_edges = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(2)]
-    created, destroyed = torch.empty(cap_e, dtype=torch.int64, device="cuda"), torch.empty(cap_e, dtype=torch.int64, device="cuda")
-    n_c, n_d = torch.zeros(1, dtype=torch.int64, device="cuda"), torch.zeros(1, dtype=torch.int64, device="cuda")
-    stream = torch.cuda.current_stream()
-    names = ["threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"]
+    frames = [torch.from_numpy(f).cuda().reshape(-1) for f in w.frames(warmup + steps)]
+    v = Vor(L, 1 << 16)
     R = int(w.match_radius_cells * W.FP_ONE)
-    kn = [0, 0]
+    stream = torch.cuda.current_stream()
 
-    def step(i, ev=None):
-        now, prv = i & 1, 1 - (i & 1)
-        c, pc = comp[now], comp[prv]
-        rec = (lambda j: ev[j].record(stream)) if ev else (lambda j: None)
-        rec(0); v.field_threshold_ccl(frames[i], w.threshold, True, ccl)
-        rec(1); v.field_centroids(ccl, w.min_size, c["cx"], c["cy"], c["sx"], c["sy"], c["size"], c["root"], c["n"])
-        rec(2)
-        if i > 0:
-            v.match_sites(pc["sx"], pc["sy"], pc["n"], c["sx"], c["sy"], c["n"], R, p2n, n2p)
-        kn[now] = int(c["n"].item())               # vor_build_cells takes n_sites on the host: one sync per frame
-        rec(3); v.vor_build_cells(c["sx"][:kn[now]], c["sy"][:kn[now]])
-        rec(4); v.vor_label(labels)
-        rec(5); v.vor_edges(labels, edges[now], n_edges[now])
-        rec(6)
-        if i > 0:
-            v.vor_diff(edges[prv], n_edges[prv], edges[now], n_edges[now], created, destroyed, n_c, n_d,
-                       p2n=p2n, n2p=n2p, n_prev_labels=max(kn[prv], 1), n_now_labels=max(kn[now], 1))
-        rec(7)
+    def step(i):
+        v.field_frame_device(frames[i], w.threshold, True, w.min_size, R)
 
-    for i in range(W_):
+    for i in range(warmup):
         step(i)
     v.vor_sync_status()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in range(K)]
-    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
-    sampler.start()
     l0 = v.vor_launch_count()
-    t0 = time.perf_counter()
-    for k in range(K):
-        step(W_ + k, evs[k])
+    e0.record(stream)
+    for k in range(steps):
+        step(warmup + k)
+    e1.record(stream)
     torch.cuda.synchronize()
-    secs = time.perf_counter() - t0
-    clocks = sampler.stop()
     launches = v.vor_launch_count() - l0
+    ms = e0.elapsed_time(e1) / steps
+    counts_host = v.vor_download(v.field_frame_results()["counts"], np.zeros(5, np.int64))
+    v.vor_profile_begin()
+    for k in range(steps):
+        step(warmup + k)
+    prof = v.vor_profile_end()
     v.vor_sync_status()
-    kernel_ms = {nm: float(np.mean([evs[k][j].elapsed_time(evs[k][j + 1]) for k in range(K)])) for j, nm in enumerate(names)}
+    per_kernel, groups = {}, {}
+    for nm, t in prof:
+        per_kernel.setdefault(nm, []).append(t)
+    kernel_launch_ms = {nm: float(np.sum(x)) / steps for nm, x in per_kernel.items()}
+    for nm, t in kernel_launch_ms.items():
+        groups[field_group(nm)] = groups.get(field_group(nm), 0.0) + t
     hbm_peak, peak_src, _ = peaks()
     cells = L * L
-    def roof(ms, nbytes, what):
-        return {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "algorithmic": what, "peak_source": peak_src}
-    out = {"metric": METRIC, "value": K * cells / secs, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W_,
-           "ms_per_step": 1e3 * secs / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "int32", "data": "synthetic",
-           "config": {"workload": w.name, "L": L, "components": kn[(W_ + K - 1) & 1], "frames": K,
-                      "timing": "wall clock around K frames (one host sync per frame for the component count)"},
-           "frames_per_s": K / secs, "kernel_ms": kernel_ms,
-           "counts": {"n_edges": int(n_edges[(W_ + K - 1) & 1].item()), "n_created": int(n_c.item()), "n_destroyed": int(n_d.item())},
-           "roofline": dict(roof(kernel_ms["threshold_ccl"], 8.0 * cells, "4 B/cell field read + 4 B/cell label written"),
-                            kernel="field_threshold_ccl (3 kernels)"),
-           "rooflines_other": {"field_centroids": roof(kernel_ms["centroids"], 4.0 * cells, "4 B/cell read")},
-           "clocks": clocks, "gpu_launches": int(launches)}
-    print(json.dumps(out), flush=True)
+
+    def roof(ms_, nbytes, what):
+        return {"bound": "hbm", "achieved": nbytes / (ms_ * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": nbytes / (ms_ * 1e-3) / 1e9 / hbm_peak, "launch_ms": ms_, "algorithmic": what,
+                "peak_source": peak_src}
+    out = {"workload": w.name, "L": L, "frames": steps, "ms_per_frame": ms, "frames_per_s": 1e3 / ms,
+           "cells_per_s": cells / (ms * 1e-3), "gpu_launches_per_frame": launches / steps,
+           "api": "field_frame_device (a6 -> a7 -> a8 -> a1..a5 on the device, no host synchronisation)",
+           "counts": {"bubbles": int(counts_host[0]), "n_edges": int(counts_host[1]), "n_created": int(counts_host[2]),
+                      "n_destroyed": int(counts_host[3])},
+           "kernel_ms": groups, "kernel_launch_ms": kernel_launch_ms,
+           "rooflines": {
+               "field_threshold_ccl": roof(groups.get("threshold_ccl", float("nan")), 8.0 * cells,
+                                           "4 B/cell field read + 4 B/cell bubble label written"),
+               "field_centroids": roof(groups.get("centroids", float("nan")), 4.0 * cells, "4 B/cell read")}}
     v.close()
+    return out
+
+
+def run_field(args, w):
+    """--workload cfg3 | cfg4: one step = one frame of the field-derived path (rows a6..a8, then a1..a5 with
+    the isomorphism).  Single GPU; not the default bench line (the metric is quoted on config 5)."""
+    import torch
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    leg = field_leg(w, args.warmup, args.steps)
+    clocks = sampler.stop()
+    out = {"metric": METRIC, "value": leg["cells_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": leg["ms_per_frame"], "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+           "config": {"workload": w.name, "L": w.L, "components": leg["counts"]["bubbles"], "frames": args.steps,
+                      "timing": "CUDA events around K frames of field_frame_device (no host synchronisation)"},
+           "frames_per_s": leg["frames_per_s"], "kernel_ms": leg["kernel_ms"], "kernel_launch_ms": leg["kernel_launch_ms"],
+           "counts": leg["counts"],
+           "roofline": dict(leg["rooflines"]["field_threshold_ccl"], kernel="field_threshold_ccl"),
+           "rooflines_other": {"field_centroids": leg["rooflines"]["field_centroids"]},
+           "clocks": clocks, "gpu_launches": int(round(leg["gpu_launches_per_frame"] * args.steps))}
+    print(json.dumps(out), flush=True)
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (torch.distributed.run, one
+    process per GPU, rendezvous on 127.0.0.1) and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    return subprocess.call(cmd, env=env)
 
 
 def main():
     args = parse()
     w = get_workload(args.workload)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(spawn_ranks(args))
     if isinstance(w, W.FieldWorkload):
         if args.impl == "reference" or args.gpus != 1:
             raise SystemExit("field workloads: --impl ours --gpus 1 only")

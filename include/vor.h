@@ -59,6 +59,11 @@ int vor_sync_status(vor_ctx* ctx, void* stream);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t vor_launch_count(const vor_ctx* ctx);
 
+/* Copy `bytes` bytes from device memory (e.g. a pointer returned by vor_frame_results /
+ * field_frame_results) to the host buffer h_dst on `stream` and wait for the copy.  For callers
+ * that hold only raw pointers; a torch caller copies its own tensors. */
+int vor_download(vor_ctx* ctx, const void* d_src, void* h_dst, int64_t bytes, void* stream);
+
 /* Diagnostics of the last call (synchronises the device; for tuning notes, never on the hot path):
  *   "label_unproven_quadrants"  8x8-cell quadrants the CTA labelling kernel handed to its second pass
  *   "edges_raw_keys"            CTA-distinct keys the emit kernel produced (before the rows de-duplicate)

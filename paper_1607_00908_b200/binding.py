@@ -26,6 +26,7 @@ SIGNATURES = {
     "vor_last_error": (C.c_char_p, [_P]),
     "vor_sync_status": (C.c_int, [_P, _P]),
     "vor_launch_count": (C.c_int64, [_P]),
+    "vor_download": (C.c_int, [_P, _P, _P, C.c_int64, _P]),
     "vor_set_option": (C.c_int, [_P, C.c_char_p, C.c_int64]),
     "vor_stat": (C.c_int64, [_P, C.c_char_p]),
     "vor_profile_begin": (C.c_int, [_P]),
@@ -130,6 +131,11 @@ class Vor:
     # ---- plumbing
     def vor_sync_status(self):
         self._check(self.lib.vor_sync_status(self.h, _stream()))
+
+    def vor_download(self, d_ptr: int, h_array):
+        """Copy len(h_array) elements from the raw device pointer d_ptr into the HOST numpy array h_array."""
+        self._check(self.lib.vor_download(self.h, C.c_void_p(d_ptr), h_array.ctypes.data_as(_P), h_array.nbytes, _stream()))
+        return h_array
 
     def vor_launch_count(self) -> int:
         return int(self.lib.vor_launch_count(self.h))

@@ -107,6 +107,15 @@ int vor_destroy(vor_ctx* ctx) {
 
 const char* vor_last_error(const vor_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
+int vor_download(vor_ctx* ctx, const void* d_src, void* h_dst, int64_t bytes, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_src || !h_dst || bytes < 0) return vor_fail(ctx, VOR_EINVAL, "vor_download: null pointer or negative size");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    VOR_CUDA(cudaMemcpyAsync(h_dst, d_src, (size_t)bytes, cudaMemcpyDeviceToHost, stream));
+    VOR_CUDA(cudaStreamSynchronize(stream));
+    return VOR_OK;
+}
+
 int64_t vor_launch_count(const vor_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 int64_t vor_stat(vor_ctx* ctx, const char* name) {

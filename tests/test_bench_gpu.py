@@ -29,7 +29,8 @@ def test_bench_line_site_path():
     assert d["n_gpus"] == 1 and d["steps"] == 3 and d["value"] > 0 and d["vs_baseline"] is None
     assert d["config"]["workload"].startswith("cfg5") and d["data"] == "synthetic"
     r = d["roofline"]
-    assert r["bound"] in ("hbm", "tensor", "alu") and 0 < r["frac"] < 1.5 and r["peak"] > 0 and "label" in r["kernel"]
+    assert r["bound"] == "hbm" and 0 < r["frac"] < 1.5 and r["peak"] > 0 and "label" in r["kernel"]
+    assert 0 < d["frame_roofline"]["frac"] < 1.5 and d["cpu_baseline"]["single_thread"]["cores"] == 1
     assert d["rooflines_other"]["edges_stream_kernel"]["bound"] == "hbm"
     assert d["gpu_launches"] >= 3 * 8                       # a1..a5 launch at least 8 kernels per step
     e = d["e2e"]
@@ -46,5 +47,6 @@ def test_bench_line_site_path():
 def test_bench_line_field_path():
     d = run_bench("--workload", "cfg3")
     assert d["config"]["workload"].startswith("cfg3") and d["value"] > 0 and d["gpu_launches"] > 0
-    assert set(d["kernel_ms"]) == {"threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"}
+    assert {"threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"} <= set(d["kernel_ms"])
     assert d["roofline"]["bound"] == "hbm" and d["config"]["components"] > 1000
+    assert "no host synchronisation" in d["config"]["timing"]
