@@ -67,7 +67,6 @@ struct vor_ctx {
                                //   finish kernel restores that), so stale row contents are never read
     int64_t row_slots;         // slots used per row (option; 4..kRowStride, multiple of 4)
     int64_t edges_generic;     // 1 = force the generic emit kernel (testing)
-    int64_t edges_path;        // 0 = bulk-copy streaming kernel, 1 = per-lane-load streaming kernel
     uint64_t* d_keys_a;        // [max_raw_keys]  overflow keys / sort ping
     uint64_t* d_keys_b;        // [max_raw_keys]  sort pong
     int64_t* d_n_raw;          // device control block [8]: 0 = raw/overflow key count, 1 = filtered

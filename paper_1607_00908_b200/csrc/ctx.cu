@@ -192,11 +192,6 @@ int vor_set_option(vor_ctx* ctx, const char* name, int64_t value) {
         ctx->fuse = value != 0;
         return VOR_OK;
     }
-    if (!strcmp(name, "edges_path")) {
-        if (value < 0 || value > 1) return vor_fail(ctx, VOR_EINVAL, "edges_path must be 0 or 1");
-        ctx->edges_path = value;
-        return VOR_OK;
-    }
     if (!strcmp(name, "edges_generic")) {
         ctx->edges_generic = value != 0;
         return VOR_OK;

@@ -277,211 +277,6 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
     hash_flush(sh.table, rs, sh.scan);
 }
 
-// ---- bulk-copy streaming kernel (L % 4 == 0, 16-byte aligned image): the default.
-// The same three stages as above, but the image is moved by the copy engine instead of per-lane loads:
-// every warp owns a strip of 128 columns x kTmSegRows rows and walks down it in boxes of 8 rows.  A box
-// (its 8 rows, the row above them and the 4 columns to the right: 9 x 528 bytes) is fetched into the
-// warp's own shared-memory ring with one 1-D bulk copy per row (cp.async.bulk, completion counted on an
-// mbarrier); the box after it is in flight while this one is examined, so no lane ever waits on a
-// global load, no register holds prefetched rows and no address is computed per row.  Stage A reads
-// the rows from shared memory and queues only a 16-bit reference (row, lane) per dirty lane-row; stages
-// B and C fetch the 9 labels of a reference from the box, which stays in place until the warp has
-// drained its queues.  Warps never synchronise with each other before the final flush.
-constexpr int kTmWarpsX = 2, kTmWarpsY = 2;
-constexpr int kTmWarps = kTmWarpsX * kTmWarpsY;
-static_assert(32 * kTmWarps == kStrThreads, "hash_flush is written for one block size");
-constexpr int kTmCols = 128;
-constexpr int kTmBoxRows = 8;
-constexpr int kTmSegRows = 64;                                  // rows per warp
-constexpr int kTmPitch = kTmCols + 4;                           // words per staged row (4 halo columns)
-constexpr int kTmBoxWords = (kTmBoxRows + 1) * kTmPitch;        // row 0 = the row above the box
-constexpr int kTmStages = 2;
-constexpr int kTmSlots = 1024;                                  // hash-set slots per CTA (256 x 128 cells)
-constexpr int kTmRefCap = kTmBoxRows * 32;
-constexpr int kTmMultiCap = 64;                                 // < 32 pending + 32 per batch
-
-struct TmShared {
-    int32_t box[kTmWarps][kTmStages][kTmBoxWords];              // 16-byte aligned stages (4752 bytes each)
-    unsigned long long table[kTmSlots];
-    unsigned long long full[kTmWarps][kTmStages];               // mbarriers: bytes of a box have landed
-    uint16_t ref[kTmWarps][kTmRefCap];                          // dirty lane-rows of the current box: row << 5 | lane
-    uint16_t mref[kTmWarps][kTmMultiCap];                       // those with three or more labels
-    int32_t scan[kTmWarps + 1];
-};
-static_assert((kTmBoxWords * 4) % 16 == 0, "bulk copies need 16-byte aligned destinations");
-
-__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// global -> shared bulk copy; bytes and both addresses are multiples of 16
-__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
-__global__ void __launch_bounds__(kStrThreads, 4) edges_bulk_kernel(const int32_t* __restrict__ labels,
-                                                                    int32_t L, const RowSet rs) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    TmShared& sh = *reinterpret_cast<TmShared*>(smem_raw);
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const unsigned lt = (1u << lane) - 1u;
-    for (int i = threadIdx.x; i < kTmSlots; i += kStrThreads) sh.table[i] = kEmptyKey;
-    if (threadIdx.x < kTmWarps * kTmStages) mbar_init(smem_addr(&sh.full[0][0] + threadIdx.x), 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncthreads();
-
-    const int32_t xbase = (blockIdx.x * kTmWarpsX + (wid % kTmWarpsX)) * kTmCols;
-    const int32_t ybeg = (blockIdx.y * kTmWarpsY + (wid / kTmWarpsX)) * kTmSegRows;
-    const int32_t yend = min(ybeg + kTmSegRows, L);
-    if (xbase < L && ybeg < L) {                   // warp-uniform
-        const int32_t cols = min(kTmCols, L - xbase);              // multiple of 4
-        const bool edge = xbase + kTmCols >= L;                    // the right neighbour of the strip is column 0
-        const uint32_t rowbytes = 4u * (uint32_t)(edge ? cols : cols + 4);
-        const uint32_t amask = 4 * lane < cols ? 0xffffffffu : 0u;
-        const uint32_t bar0 = smem_addr(&sh.full[wid][0]);
-        const uint32_t box0 = smem_addr(&sh.box[wid][0][0]);
-        uint16_t* __restrict__ ref = sh.ref[wid];
-        uint16_t* __restrict__ mref = sh.mref[wid];
-        const int nbox = (yend - ybeg + kTmBoxRows - 1) / kTmBoxRows;
-
-        // box k: staged row 0 = image row ybeg + 8k - 1 (wrapped), staged rows 1..nr = the box
-        auto issue = [&](int k) {
-            const int st = k & 1;
-            const int32_t y0 = ybeg + kTmBoxRows * k;
-            const int nr = min(kTmBoxRows, yend - y0);
-            const uint32_t bar = bar0 + 8u * st;
-            if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)(nr + 1) * rowbytes);
-            __syncwarp();
-            if (lane <= nr) {
-                const int32_t y = lane == 0 ? (y0 == 0 ? L - 1 : y0 - 1) : y0 + lane - 1;
-                bulk_copy_g2s(box0 + 4u * (uint32_t)(st * kTmBoxWords + lane * kTmPitch),
-                              labels + (int64_t)y * L + xbase, rowbytes, bar);
-            }
-        };
-        issue(0);
-#pragma unroll 1
-        for (int k = 0; k < nbox; ++k) {
-            // the other stage was drained at the end of the previous iteration: refill it now
-            if (k + 1 < nbox) issue(k + 1);
-            const int32_t* __restrict__ bx = sh.box[wid][k & 1];
-            const int32_t y0 = ybeg + kTmBoxRows * k;
-            const int nr = min(kTmBoxRows, yend - y0);
-            mbar_wait(bar0 + 8u * (k & 1), (uint32_t)(k >> 1) & 1u);
-            if (edge) {                            // periodic wrap: the strip's right neighbour is column 0
-                if (lane <= nr) {
-                    const int32_t y = lane == 0 ? (y0 == 0 ? L - 1 : y0 - 1) : y0 + lane - 1;
-                    sh.box[wid][k & 1][lane * kTmPitch + cols] = __ldg(labels + (int64_t)y * L);
-                }
-                __syncwarp();
-            }
-            // ---- stage A: which lane-rows hold a discontinuity not already reported by the row above
-            int rn = 0, mn = 0;
-            int4 pc = *reinterpret_cast<const int4*>(bx + 4 * lane);
-            int32_t prr3 = bx[4 * lane + 4];
-            uint32_t force = y0 == 0 ? 1u : 0u;    // row 0 ends every chain: nothing is skipped there
-#pragma unroll
-            for (int r = 1; r <= kTmBoxRows; ++r) {
-                if (r <= nr) {                     // warp-uniform
-                    const int4 c = *reinterpret_cast<const int4*>(bx + r * kTmPitch + 4 * lane);
-                    const int32_t rr3 = bx[r * kTmPitch + 4 * lane + 4];
-                    const uint32_t dh = (c.x ^ c.y) | (c.y ^ c.z) | (c.z ^ c.w) | (c.w ^ rr3);
-                    const uint32_t dv = (pc.x ^ c.x) | (pc.y ^ c.y) | (pc.z ^ c.z) | (pc.w ^ c.w);
-                    uint32_t any = (dv | dh) & amask;
-                    uint32_t dv5 = dv | (uint32_t)(rr3 ^ prr3) | force;
-                    asm volatile("" : "+r"(any), "+r"(dv5));     // keep the OR-of-XOR form (LOP3)
-                    const bool dirty = (any != 0) & (dv5 != 0);
-                    const unsigned m = __ballot_sync(full, dirty);
-                    if (m) {
-                        if (dirty) ref[rn + __popc(m & lt)] = (uint16_t)(r << 5 | lane);
-                        rn += __popc(m);
-                    }
-                    pc = c; prr3 = rr3; force = 0;
-                }
-            }
-            __syncwarp();
-            // ---- stage C: every differing pair of `take` queued multi-label references.  Label j of a
-            // window: j < 5 -> row, columns 0..4; else the row above, columns 0..3.  Pair q < 4 = (j, j + 1);
-            // pair q >= 4 = (row above, row) of column q - 4.
-            auto process_multi = [&](int take) {
-                mn -= take;
-                unsigned bits = 0;
-                const int32_t* __restrict__ w = bx;
-                if (lane < take) {
-                    const uint32_t e = mref[mn + lane];
-                    w = bx + (e >> 5) * kTmPitch + 4 * (e & 31u);
-                    const int4 c = *reinterpret_cast<const int4*>(w);
-                    const int4 p = *reinterpret_cast<const int4*>(w - kTmPitch);
-                    const int32_t rr3 = w[4];
-                    bits = (unsigned)(c.x != c.y) | (unsigned)(c.y != c.z) << 1 | (unsigned)(c.z != c.w) << 2 |
-                           (unsigned)(c.w != rr3) << 3 | (unsigned)(p.x != c.x) << 4 | (unsigned)(p.y != c.y) << 5 |
-                           (unsigned)(p.z != c.z) << 6 | (unsigned)(p.w != c.w) << 7;
-                }
-                while (__any_sync(full, bits != 0)) {  // every trip is dense over the lanes that still have pairs
-                    if (bits) {
-                        const int q = __ffs(bits) - 1;
-                        bits &= bits - 1;
-                        const int32_t a = q < 4 ? w[q] : w[q - 4 - kTmPitch];
-                        const int32_t b = q < 4 ? w[q + 1] : w[q - 4];
-                        hash_insert<kTmSlots>((uint32_t)a, (uint32_t)b, sh.table, rs);
-                    }
-                }
-                __syncwarp();
-            };
-            // ---- stage B: 32 references at a time; two labels -> one key, more -> stage C
-            for (int base = 0; base < rn; base += 32) {
-                const int take = min(32, rn - base);
-                int4 c = make_int4(0, 0, 0, 0), p = c;
-                int32_t rr3 = 0;
-                uint32_t e = 0;
-                if (lane < take) {
-                    e = ref[base + lane];
-                    const int32_t* __restrict__ w = bx + (e >> 5) * kTmPitch + 4 * (e & 31u);
-                    c = *reinterpret_cast<const int4*>(w);
-                    p = *reinterpret_cast<const int4*>(w - kTmPitch);
-                    rr3 = w[4];
-                }
-                const uint32_t a = (uint32_t)c.x;
-                const uint32_t t1 = c.y ^ a, t2 = c.z ^ a, t3 = c.w ^ a, t4 = rr3 ^ a;
-                const uint32_t t5 = p.x ^ a, t6 = p.y ^ a, t7 = p.z ^ a, t8 = p.w ^ a;
-                // two labels {a, b}  <=>  every non-zero t equals the largest one (b = a ^ max t)
-                const uint32_t mx = max(max(max(t1, t2), max(t3, t4)), max(max(t5, t6), max(t7, t8)));
-                const uint32_t lo = min(min(min(t1 - 1u, t2 - 1u), min(t3 - 1u, t4 - 1u)),
-                                        min(min(t5 - 1u, t6 - 1u), min(t7 - 1u, t8 - 1u)));   // 0 -> 2^32 - 1
-                const bool any = mx != 0, two = lo == mx - 1u;
-                if (any && two) hash_insert<kTmSlots>(a, a ^ mx, sh.table, rs);
-                const bool multi = any && !two;
-                const unsigned mm = __ballot_sync(full, multi);
-                if (mm) {
-                    if (multi) mref[mn + __popc(mm & lt)] = (uint16_t)e;
-                    mn += __popc(mm);
-                    __syncwarp();
-                    if (mn >= 32) process_multi(32);
-                }
-            }
-            if (mn > 0) process_multi(mn);         // the references die with the box
-            __syncwarp();
-        }
-    }
-    __syncthreads();
-    hash_flush<kTmSlots>(sh.table, rs, sh.scan);
-}
-
 // ---- generic kernel (any L, any alignment): scalar loads, every discontinuity goes to the hash set.
 constexpr int kEmitThreads = 128;
 constexpr int kEmitCols = 128;          // per CTA tile: 32 lanes x 4 labels
@@ -1221,13 +1016,7 @@ extern "C" int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d
     const int32_t L = ctx->L;
     RowSet rs = vor_row_set(ctx);
     const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
-    if (vec && ctx->edges_path != 1) {
-        VOR_CUDA(cudaFuncSetAttribute(edges_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(TmShared)));
-        dim3 grid((L + kTmWarpsX * kTmCols - 1) / (kTmWarpsX * kTmCols),
-                  (L + kTmWarpsY * kTmSegRows - 1) / (kTmWarpsY * kTmSegRows));
-        VOR_LAUNCH(edges_bulk_kernel, grid, kStrThreads, sizeof(TmShared), stream, d_labels, L, rs);
-    } else if (vec) {
+    if (vec) {
         static_assert(sizeof(StreamShared) <= 27 * 1024, "eight CTAs per SM");
         VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       (int)sizeof(StreamShared)));

@@ -135,13 +135,10 @@ def check_edges(G, labels, max_sites, row_slots=(16,)):
     ref = oracle.edges(labels)
     for s in row_slots:
         v.vor_set_option("row_slots", s)
-        # (generic, path): bulk-copy streaming kernel, generic kernel, per-lane-load streaming kernel, and the
-        # first again: the rows must be left empty by every call
-        for generic, path in ((0, 0), (1, 0), (0, 1), (0, 0)):
+        for generic in (0, 1, 0):                      # repeated: the rows must be left empty
             v.vor_set_option("edges_generic", generic)
-            v.vor_set_option("edges_path", path)
             got = G.gpu_edges(v, labels, cap=max(1024, 2 * L * L))
-            assert got.dtype == np.uint64 and np.array_equal(got, ref), (s, generic, path, len(got), len(ref))
+            assert got.dtype == np.uint64 and np.array_equal(got, ref), (s, generic, len(got), len(ref))
     v.close()
 
 
@@ -213,10 +210,9 @@ def test_edges_tiny_raw_key_scratch_is_still_exact(G):
     sx, sy = next(iter(w.frames(1)))
     lab = oracle.label_cells(w.L, sx, sy, 16)
     ref = oracle.edges(lab)
-    for generic, path in ((0, 0), (1, 0), (0, 1)):
+    for generic in (0, 1):
         v = make(w.L, w.n_sites, max_raw_keys=1000)
         v.vor_set_option("edges_generic", generic)
-        v.vor_set_option("edges_path", path)
         for _ in range(2):                              # twice: stale keys of the first call must not leak
             assert np.array_equal(G.gpu_edges(v, lab, cap=len(ref) + 10), ref)
         v.close()
