@@ -162,6 +162,22 @@ def events(prev, now, n):
                 global_trigger=int(g))
 
 
+def t1(prev, now, n):
+    """O8: couples of active vertices, their class, common-neighbour counts and T1 partner."""
+    prev = np.ascontiguousarray(prev, dtype=np.uint64)
+    now = np.ascontiguousarray(now, dtype=np.uint64)
+    cap = max(1, len(prev) + len(now))
+    couples = np.empty(cap, np.uint64); partner = np.empty(cap, np.uint64)
+    cls = np.empty(cap, np.int32); cp = np.empty(cap, np.int32); cn = np.empty(cap, np.int32)
+    lib().orc_t1.restype = C.c_int64
+    m = lib().orc_t1(_p(prev, C.c_uint64), C.c_int64(len(prev)), _p(now, C.c_uint64), C.c_int64(len(now)),
+                     C.c_int32(n), _p(couples, C.c_uint64), _p(cls, C.c_int32), _p(cp, C.c_int32),
+                     _p(cn, C.c_int32), _p(partner, C.c_uint64), C.c_int64(cap))
+    assert m <= cap
+    return dict(couples=couples[:m].copy(), cls=cls[:m].copy(), common_prev=cp[:m].copy(),
+                common_now=cn[:m].copy(), partner=partner[:m].copy())
+
+
 def unpack(keys):
     """uint64 packed keys -> (i, j) int64 arrays."""
     keys = np.asarray(keys, dtype=np.uint64)

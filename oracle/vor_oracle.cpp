@@ -25,6 +25,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <queue>
+#include <set>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -390,6 +391,73 @@ int32_t orc_events(const u64* prev, i64 n_prev, const u64* now, i64 n_now, int32
         for (int32_t j : rn[i]) count_now[i] += trigger[j];
     }
     return any;
+}
+
+// O8 — couples of active vertices and T1 pairing (§III.B.4: "we find which of the active
+// points are connected and store them as couples ... discard those couples that are given by a simple
+// permutation of another couple ... checks whether or not the couple is connected in both configurations.
+// If the couple is connected in only one configuration, then this is dubbed either breaking or arising if
+// it is found to be in D_P or in D_N"; an edge whose end points share two neighbours is
+// in the bulk, one neighbour: on the boundary; PAPER.md:238 and Fig. 8: in a T1 event the breaking link
+// is replaced by the arising link between its two common neighbours, the number of links is conserved).
+// Inputs as O7.  A couple is a pair i < j of active vertices (trigger = 1, O7) connected in D_P or D_N.
+// Outputs, one entry per couple in ascending (i, j) order:
+//   couples      packed key (i << 32 | j)
+//   cls          0 connected in both, 1 breaking (D_P only), 2 arising (D_N only)
+//   common_prev  number of common neighbours of i and j in D_P, -1 if the couple is not connected there
+//   common_now   the same in D_N
+//   partner      breaking couple: if it has exactly two common neighbours c < d in D_P and (c, d) is an
+//                arising couple, that couple's key (the T1 quadruple is {i, j, c, d}); arising couple: the
+//                mirror statement in D_N with a breaking couple; otherwise ~0.
+// Returns the number of couples (cap is only checked, never exceeded).
+i64 orc_t1(const u64* prev, i64 n_prev, const u64* now, i64 n_now, int32_t n,
+           u64* couples, int32_t* cls, int32_t* common_prev, int32_t* common_now, u64* partner, i64 cap) {
+    std::vector<std::set<int32_t>> rp(n), rn(n);
+    for (i64 k = 0; k < n_prev; ++k) {
+        const int32_t i = (int32_t)(prev[k] >> 32), j = (int32_t)(prev[k] & 0xffffffffu);
+        if (i < n && j < n) { rp[i].insert(j); rp[j].insert(i); }
+    }
+    for (i64 k = 0; k < n_now; ++k) {
+        const int32_t i = (int32_t)(now[k] >> 32), j = (int32_t)(now[k] & 0xffffffffu);
+        if (i < n && j < n) { rn[i].insert(j); rn[j].insert(i); }
+    }
+    std::vector<char> active(n);
+    for (int32_t i = 0; i < n; ++i) active[i] = rp[i] != rn[i];
+    auto shared = [](const std::set<int32_t>& a, const std::set<int32_t>& b) {
+        std::vector<int32_t> c;
+        for (int32_t v : a) if (b.count(v)) c.push_back(v);
+        return c;                                        // ascending
+    };
+    const u64 none = ~(u64)0;
+    i64 m = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        if (!active[i]) continue;
+        std::set<int32_t> nb = rp[i];
+        nb.insert(rn[i].begin(), rn[i].end());
+        for (int32_t j : nb) {
+            if (j <= i || !active[j]) continue;          // a permutation of a couple is the same couple
+            const bool in_p = rp[i].count(j) != 0, in_n = rn[i].count(j) != 0;
+            const std::vector<int32_t> sp = shared(rp[i], rp[j]), sn = shared(rn[i], rn[j]);
+            u64 pt = none;
+            if (in_p && !in_n && sp.size() == 2) {       // breaking: do its two common neighbours arise?
+                const int32_t c = sp[0], d = sp[1];
+                if (rn[c].count(d) && !rp[c].count(d)) pt = ((u64)(uint32_t)c << 32) | (uint32_t)d;
+            }
+            if (in_n && !in_p && sn.size() == 2) {       // arising: do its two common neighbours break?
+                const int32_t c = sn[0], d = sn[1];
+                if (rp[c].count(d) && !rn[c].count(d)) pt = ((u64)(uint32_t)c << 32) | (uint32_t)d;
+            }
+            if (m < cap) {
+                couples[m] = ((u64)(uint32_t)i << 32) | (uint32_t)j;
+                cls[m] = in_p && in_n ? 0 : (in_p ? 1 : 2);
+                common_prev[m] = in_p ? (int32_t)sp.size() : -1;
+                common_now[m] = in_n ? (int32_t)sn.size() : -1;
+                partner[m] = pt;
+            }
+            ++m;
+        }
+    }
+    return m;
 }
 
 int orc_num_threads(int threads) { return resolve_threads(threads); }
