@@ -173,6 +173,32 @@ int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
                int32_t* d_trigger, int32_t* d_events_indices, int32_t* d_events_number,
                int32_t* d_global_trigger, int32_t* d_count_prev, int32_t* d_count_now, void* stream);
 
+/* ---- couples of active vertices and T1 pairing: the paper's final output (§III.B.4: the
+ * active points that are connected are stored as couples, a permutation of a couple is the same couple, a
+ * couple connected in only one configuration is "breaking" (D_P only) or "arising" (D_N only);
+ * an edge whose end points share two neighbours lies in the bulk, one: on the boundary;
+ * PAPER.md:238 and Fig. 8: a T1 event replaces the breaking link by the arising link between its two common
+ * neighbours).  Lists, counts and capacities as for vor_events; d_trigger[n_labels] as vor_events wrote it.
+ * A couple is a pair i < j of active vertices connected in the past or the present list.  Outputs (device,
+ * caller-owned, capacity `cap` each), one entry per couple in ascending key order, *d_n_couples of them
+ * (the REQUIRED number; more than cap latches VOR_ECAPACITY and nothing is written past cap):
+ *   d_couples      packed key
+ *   d_class        0 connected in both, 1 breaking, 2 arising
+ *   d_common_prev  number of common neighbours of i and j in the past list, -1 if not connected there
+ *   d_common_now   the same in the present list
+ *   d_partner      breaking couple with exactly two common neighbours c < d in the past list whose pair
+ *                  (c, d) is arising: that key - {i, j, c, d} is the T1 quadruple; arising couple: the mirror
+ *                  statement in the present list with a breaking pair; otherwise ~0.
+ * The context builds both adjacency matrices in compressed symmetric form (sorted rows) in
+ * its own scratch, sized on the first call from the capacities; cap_prev + cap_now must be < 2^31. */
+int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+                  const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
+                  const uint64_t* d_created, const int64_t* d_n_created,
+                  const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int64_t cap_created,
+                  int64_t cap_destroyed, const int32_t* d_trigger, int32_t n_labels,
+                  uint64_t* d_couples, int32_t* d_class, int32_t* d_common_prev, int32_t* d_common_now,
+                  uint64_t* d_partner, int64_t cap, int64_t* d_n_couples, void* stream);
+
 /* ---- a6: bubble identification (§III.A: threshold -> two-valued variable ->
  * cluster labelling).  mask = above ? field > thr : field < thr (strict; NaN -> background).
  * 4-connected periodic components; d_ccl[c] = smallest linear index in c's component, or -1. */

@@ -40,6 +40,8 @@ SIGNATURES = {
     "vor_diff_rows": (C.c_int, [_P, _P, _P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
     "vor_events": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, _P, C.c_int64, C.c_int64, C.c_int32,
                              _P, _P, _P, _P, _P, _P, _P]),
+    "vor_t1_events": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, C.c_int32,
+                                _P, _P, _P, _P, _P, C.c_int64, _P, _P]),
     "field_threshold_ccl": (C.c_int, [_P, _P, C.c_float, C.c_int, _P, _P]),
     "field_centroids": (C.c_int, [_P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
     "match_sites": (C.c_int, [_P, _P, _P, _P, _P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P, _P]),
@@ -221,6 +223,18 @@ class Vor:
             created.numel(), destroyed.numel(), n_labels,
             _ptr(trigger, i32), _ptr(events_indices, i32), _ptr(events_number, i32), _ptr(global_trigger, i32),
             _ptr(count_prev, i32), _ptr(count_now, i32), _stream()))
+
+    def vor_t1_events(self, prev, n_prev, now, n_now, created, n_created, destroyed, n_destroyed, trigger,
+                      couples, cls, common_prev, common_now, partner, n_couples):
+        cap = min(t.numel() for t in (couples, cls, common_prev, common_now, partner))
+        i64, i32 = torch.int64, torch.int32
+        self._check(self.lib.vor_t1_events(
+            self.h, _ptr(prev, i64), _ptr(n_prev, i64), _ptr(now, i64), _ptr(n_now, i64),
+            prev.numel(), now.numel(),
+            _ptr(created, i64), _ptr(n_created, i64), _ptr(destroyed, i64), _ptr(n_destroyed, i64),
+            created.numel(), destroyed.numel(), _ptr(trigger, i32), trigger.numel(),
+            _ptr(couples, i64), _ptr(cls, i32), _ptr(common_prev, i32), _ptr(common_now, i32),
+            _ptr(partner, i64), cap, _ptr(n_couples, i64), _stream()))
 
     # ---- field path
     def field_threshold_ccl(self, field, thr: float, above: bool, ccl):

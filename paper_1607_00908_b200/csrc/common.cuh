@@ -82,6 +82,10 @@ struct vor_ctx {
     uint32_t* d_dr_scratch;
     int64_t dr_rows;
 
+    // ---- vor_t1_events: degrees, offsets, unsorted and sorted adjacency lists, union list (lazily sized)
+    void* d_t1[5];
+    size_t t1_bytes[5];
+
     // ---- diff with maps: translated / filtered lists
     uint64_t* d_tr_prev;       // lazily sized to max_raw_keys
     uint64_t* d_tr_now;

@@ -26,8 +26,9 @@ __global__ void ev_mark_kernel(const uint64_t* __restrict__ created, const int64
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nc + nd; k += (int64_t)gridDim.x * blockDim.x) {
         const uint64_t e = k < nc ? created[k] : destroyed[k - nc];
         const uint32_t i = (uint32_t)(e >> 32), j = (uint32_t)e;
-        if (i < (uint32_t)n) trigger[i] = 1;
-        if (j < (uint32_t)n) trigger[j] = 1;
+        if (i >= (uint32_t)n || j >= (uint32_t)n) continue;     // keys with a label >= n_labels are ignored
+        trigger[i] = 1;
+        trigger[j] = 1;
     }
 }
 
@@ -163,5 +164,370 @@ extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d
                d_events_indices, d_events_number, d_global_trigger);
     VOR_LAUNCH(ev_degree_kernel, 2 * grid, 256, 0, stream, d_prev, d_n_prev, d_now, d_n_now, cap_prev, cap_now,
                d_trigger, n_labels, d_count_prev, d_count_now);
+    return VOR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Couples of active vertices and T1 pairing (§III.B.4: the active
+// points that are connected are stored as couples, permutations dropped, each couple connected in only one
+// configuration is "breaking" (D_P) or "arising" (D_N); end points sharing two neighbours
+// = bulk edge, one = boundary edge; PAPER.md:238 and Fig. 8: a T1 event replaces the breaking link by the
+// arising link between its two common neighbours).
+//
+// Data structures (all context scratch):
+//   adjacency lists of BOTH triangulations in compressed symmetric form - the paper's adjacency matrix with
+//   sorted rows, row v = all neighbours of v ascending: off[n+1], adj[2E].  Built from the
+//   i<j key lists by degree count -> exclusive scan -> atomic fill -> rank within the row (keys are unique,
+//   so the rank of a neighbour is the number of smaller ones in its row).
+//   union list U = now ∪ destroyed in key order (a key's slot = its own index + its lower bound in the other
+//   list), class in the two bits that a packed key never uses (bit 63: breaking, bit 31: arising), or kDrop
+//   when an end point is inactive or >= n_labels.  Couples = order-preserving compaction of U.
+namespace {
+
+constexpr uint64_t kDrop = ~(uint64_t)0;
+constexpr uint64_t kBitBreak = (uint64_t)1 << 63, kBitArise = (uint64_t)1 << 31;
+
+struct T1Graph {
+    const uint64_t* keys;
+    const int64_t* n_dev;
+    int64_t cap;
+    uint32_t* deg;      // [n + 1] degrees, then fill cursors
+    uint32_t* off;      // [n + 1]
+    uint32_t* adj_u;    // unsorted rows
+    uint32_t* adj_s;    // sorted rows
+};
+
+__device__ __forceinline__ int64_t t1_len(const T1Graph& g) { return min(max(*g.n_dev, (int64_t)0), g.cap); }
+
+__device__ __forceinline__ bool t1_edge(const T1Graph& g, int64_t k, int32_t n, uint32_t* i, uint32_t* j) {
+    const uint64_t e = g.keys[k];
+    *i = (uint32_t)(e >> 32); *j = (uint32_t)e;
+    return *i < (uint32_t)n && *j < (uint32_t)n;
+}
+
+// blockIdx.y selects the triangulation
+__global__ void t1_degree_kernel(T1Graph gp, T1Graph gn, int32_t n) {
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    const int64_t m = t1_len(g);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t i, j;
+        if (!t1_edge(g, k, n, &i, &j)) continue;
+        atomicAdd(g.deg + i, 1u);
+        atomicAdd(g.deg + j, 1u);
+    }
+}
+
+__device__ __forceinline__ void t1_chunk(int64_t n, int batch, int64_t* beg, int64_t* end) {
+    int64_t C = (n + gridDim.x - 1) / gridDim.x;
+    C = (C + batch - 1) / batch * batch;
+    const int64_t s = (int64_t)blockIdx.x * C;
+    *beg = s < n ? s : n;
+    *end = s + C < n ? s + C : n;
+}
+
+// exclusive scan of deg[0..n) -> off[0..n], in two kernels: per-chunk sums, then every block adds the sums of
+// the chunks before it and scans its own chunk; deg is zeroed for its second life as fill cursor
+__global__ void __launch_bounds__(kEvThreads) t1_scan_sum_kernel(T1Graph gp, T1Graph gn, int32_t n,
+                                                                 int64_t* __restrict__ partial) {
+    __shared__ int64_t sh[32];
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    int64_t beg, end;
+    t1_chunk(n, kEvThreads, &beg, &end);
+    int64_t c = 0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kEvThreads) c += g.deg[i];
+    c = ev_block_sum(c, sh);
+    if (threadIdx.x == 0) partial[blockIdx.y * gridDim.x + blockIdx.x] = c;
+}
+
+__global__ void __launch_bounds__(kEvThreads) t1_scan_apply_kernel(T1Graph gp, T1Graph gn, int32_t n,
+                                                                   const int64_t* __restrict__ partial) {
+    __shared__ int64_t sh[32];
+    __shared__ uint32_t wsum[kEvThreads / 32];
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int64_t beg, end;
+    t1_chunk(n, kEvThreads, &beg, &end);
+    int64_t before = 0, all = 0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += kEvThreads) {
+        const int64_t v = partial[blockIdx.y * gridDim.x + b];
+        all += v;
+        if (b < (int)blockIdx.x) before += v;
+    }
+    before = ev_block_sum(before, sh);
+    all = ev_block_sum(all, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) g.off[n] = (uint32_t)all;
+    uint32_t run = (uint32_t)before;
+    for (int64_t sub = beg; sub < end; sub += kEvThreads) {
+        const int64_t i = sub + threadIdx.x;
+        const uint32_t v = i < end ? g.deg[i] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) wsum[wid] = inc;
+        __syncthreads();
+        uint32_t wbase = 0, total = 0;
+        for (int w = 0; w < kEvThreads / 32; ++w) {
+            const uint32_t t = wsum[w];
+            if (w < wid) wbase += t;
+            total += t;
+        }
+        if (i < end) { g.off[i] = run + wbase + inc - v; g.deg[i] = 0u; }
+        run += total;
+        __syncthreads();
+    }
+}
+
+__global__ void t1_fill_kernel(T1Graph gp, T1Graph gn, int32_t n) {
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    const int64_t m = t1_len(g);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t i, j;
+        if (!t1_edge(g, k, n, &i, &j)) continue;
+        g.adj_u[g.off[i] + atomicAdd(g.deg + i, 1u)] = j;
+        g.adj_u[g.off[j] + atomicAdd(g.deg + j, 1u)] = i;
+    }
+}
+
+__device__ __forceinline__ void t1_place(const T1Graph& g, uint32_t v, uint32_t e) {
+    const uint32_t b = g.off[v], end = g.off[v + 1];
+    uint32_t r = 0;
+    for (uint32_t p = b; p < end; ++p) r += g.adj_u[p] < e;
+    g.adj_s[b + r] = e;
+}
+
+__global__ void t1_rank_kernel(T1Graph gp, T1Graph gn, int32_t n) {
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    const int64_t m = t1_len(g);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t i, j;
+        if (!t1_edge(g, k, n, &i, &j)) continue;
+        t1_place(g, i, j);
+        t1_place(g, j, i);
+    }
+}
+
+__device__ __forceinline__ int64_t t1_lower_bound(const uint64_t* __restrict__ a, int64_t n, uint64_t key) {
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (a[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+struct T1Lists {
+    const uint64_t* now; const int64_t* n_now; int64_t cap_now;
+    const uint64_t* created; const int64_t* n_created; int64_t cap_created;
+    const uint64_t* destroyed; const int64_t* n_destroyed; int64_t cap_destroyed;
+};
+
+__global__ void t1_union_kernel(T1Lists l, const int32_t* __restrict__ trigger, int32_t n, uint64_t* __restrict__ U) {
+    const int64_t nn = min(max(*l.n_now, (int64_t)0), l.cap_now), nc = min(max(*l.n_created, (int64_t)0), l.cap_created),
+                  nd = min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nn + nd; k += (int64_t)gridDim.x * blockDim.x) {
+        uint64_t key, bits;
+        int64_t pos;
+        if (k < nn) {
+            key = l.now[k];
+            pos = k + t1_lower_bound(l.destroyed, nd, key);
+            const int64_t c = t1_lower_bound(l.created, nc, key);
+            bits = (c < nc && l.created[c] == key) ? kBitArise : 0;
+        } else {
+            key = l.destroyed[k - nn];
+            pos = (k - nn) + t1_lower_bound(l.now, nn, key);
+            bits = kBitBreak;
+        }
+        const uint32_t i = (uint32_t)(key >> 32), j = (uint32_t)key;
+        const bool keep = i < (uint32_t)n && j < (uint32_t)n && trigger[i] != 0 && trigger[j] != 0;
+        U[pos] = keep ? (key | bits) : kDrop;
+    }
+}
+
+__global__ void __launch_bounds__(kEvThreads) t1_count_kernel(const uint64_t* __restrict__ U, T1Lists l,
+                                                              int64_t* __restrict__ partial) {
+    __shared__ int64_t sh[32];
+    const int64_t m = min(max(*l.n_now, (int64_t)0), l.cap_now) + min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
+    int64_t beg, end;
+    t1_chunk(m, kEvBatch, &beg, &end);
+    int64_t c = 0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kEvThreads) c += U[i] != kDrop;
+    c = ev_block_sum(c, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = c;
+}
+
+__global__ void __launch_bounds__(kEvThreads) t1_write_kernel(const uint64_t* __restrict__ U, T1Lists l,
+                                                              const int64_t* __restrict__ partial,
+                                                              uint64_t* __restrict__ couples, int32_t* __restrict__ cls,
+                                                              int64_t cap, int64_t* __restrict__ n_couples,
+                                                              int32_t* __restrict__ flags) {
+    __shared__ int64_t sh[32];
+    __shared__ int32_t wtot[kEvThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t m = min(max(*l.n_now, (int64_t)0), l.cap_now) + min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
+    int64_t beg, end;
+    t1_chunk(m, kEvBatch, &beg, &end);
+    int64_t before = 0, all = 0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += kEvThreads) {
+        const int64_t v = partial[b];
+        all += v;
+        if (b < (int)blockIdx.x) before += v;
+    }
+    before = ev_block_sum(before, sh);
+    all = ev_block_sum(all, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        *n_couples = all;
+        if (all > cap) atomicOr(flags, FLAG_DIFF_CAP);
+    }
+    int64_t run = before;
+    for (int64_t sub = beg; sub < end; sub += kEvBatch) {
+        const int64_t wb = sub + (int64_t)wid * (32 * kEvItems) + lane;
+        unsigned ball[kEvItems];
+        uint64_t u[kEvItems];
+        int32_t mine = 0;
+#pragma unroll
+        for (int k = 0; k < kEvItems; ++k) {
+            const int64_t i = wb + 32 * k;
+            u[k] = i < end ? U[i] : kDrop;
+            ball[k] = __ballot_sync(0xffffffffu, u[k] != kDrop);
+            mine += __popc(ball[k]);
+        }
+        if (lane == 0) wtot[wid] = mine;
+        __syncthreads();
+        int32_t wbase = 0, total = 0;
+        for (int w = 0; w < kEvThreads / 32; ++w) {
+            const int32_t t = wtot[w];
+            if (w < wid) wbase += t;
+            total += t;
+        }
+        int64_t pos = run + wbase;
+#pragma unroll
+        for (int k = 0; k < kEvItems; ++k) {
+            const int64_t at = pos + __popc(ball[k] & ((1u << lane) - 1u));
+            if ((ball[k] >> lane & 1u) && at < cap) {
+                couples[at] = u[k] & ~(kBitBreak | kBitArise);
+                cls[at] = (u[k] & kBitBreak) ? 1 : ((u[k] & kBitArise) ? 2 : 0);
+            }
+            pos += __popc(ball[k]);
+        }
+        run += total;
+        __syncthreads();
+    }
+}
+
+// common neighbours of i and j (rows ascending): their number, the first two in c2
+__device__ __forceinline__ int32_t t1_common(const T1Graph& g, uint32_t i, uint32_t j, uint32_t* c2) {
+    uint32_t a = g.off[i], ae = g.off[i + 1], b = g.off[j], be = g.off[j + 1];
+    int32_t cnt = 0;
+    if (a == ae || b == be) return 0;
+    uint32_t x = g.adj_s[a], y = g.adj_s[b];
+    for (;;) {
+        if (x == y) {
+            if (cnt < 2) c2[cnt] = x;
+            ++cnt;
+        }
+        const bool sa = x <= y, sb = y <= x;
+        if (sa) { if (++a == ae) break; x = g.adj_s[a]; }
+        if (sb) { if (++b == be) break; y = g.adj_s[b]; }
+    }
+    return cnt;
+}
+
+__device__ __forceinline__ bool t1_linked(const T1Graph& g, uint32_t v, uint32_t e) {
+    uint32_t lo = g.off[v], hi = g.off[v + 1];
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (g.adj_s[mid] < e) lo = mid + 1; else hi = mid;
+    }
+    return lo < g.off[v + 1] && g.adj_s[lo] == e;
+}
+
+__global__ void t1_pair_kernel(T1Graph gp, T1Graph gn, const uint64_t* __restrict__ couples,
+                               const int32_t* __restrict__ cls, const int64_t* __restrict__ n_couples, int64_t cap,
+                               int32_t* __restrict__ common_prev, int32_t* __restrict__ common_now,
+                               uint64_t* __restrict__ partner) {
+    const int64_t m = min(*n_couples, cap);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        const uint64_t key = couples[k];
+        const uint32_t i = (uint32_t)(key >> 32), j = (uint32_t)key;
+        const int32_t c = cls[k];
+        uint32_t c2[2] = {0, 0};
+        uint64_t pt = kDrop;
+        int32_t cp = -1, cn = -1;
+        if (c != 2) {
+            cp = t1_common(gp, i, j, c2);
+            if (c == 1 && cp == 2 && t1_linked(gn, c2[0], c2[1]) && !t1_linked(gp, c2[0], c2[1]))
+                pt = ((uint64_t)c2[0] << 32) | c2[1];
+        }
+        if (c != 1) {
+            cn = t1_common(gn, i, j, c2);
+            if (c == 2 && cn == 2 && t1_linked(gp, c2[0], c2[1]) && !t1_linked(gn, c2[0], c2[1]))
+                pt = ((uint64_t)c2[0] << 32) | c2[1];
+        }
+        common_prev[k] = cp;
+        common_now[k] = cn;
+        partner[k] = pt;
+    }
+}
+
+int t1_scratch(vor_ctx* ctx, int slot, size_t bytes, void** out) {
+    if (ctx->t1_bytes[slot] < bytes) {
+        if (ctx->d_t1[slot]) VOR_CUDA(cudaFree(ctx->d_t1[slot]));   // cudaFree waits for the work that uses it
+        ctx->d_t1[slot] = nullptr; ctx->t1_bytes[slot] = 0;
+        VOR_CUDA(cudaMalloc(&ctx->d_t1[slot], bytes));
+        ctx->t1_bytes[slot] = bytes;
+    }
+    *out = ctx->d_t1[slot];
+    return VOR_OK;
+}
+
+}  // namespace
+
+extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+                             const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
+                             const uint64_t* d_created, const int64_t* d_n_created,
+                             const uint64_t* d_destroyed, const int64_t* d_n_destroyed, int64_t cap_created,
+                             int64_t cap_destroyed, const int32_t* d_trigger, int32_t n_labels,
+                             uint64_t* d_couples, int32_t* d_class, int32_t* d_common_prev, int32_t* d_common_now,
+                             uint64_t* d_partner, int64_t cap, int64_t* d_n_couples, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_created || !d_n_created || !d_destroyed || !d_n_destroyed ||
+        !d_trigger || !d_couples || !d_class || !d_common_prev || !d_common_now || !d_partner || !d_n_couples)
+        return vor_fail(ctx, VOR_EINVAL, "vor_t1_events: null pointer");
+    if (n_labels < 1 || cap_prev < 0 || cap_now < 0 || cap_created < 0 || cap_destroyed < 0 || cap < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_t1_events: n_labels must be >= 1, capacities >= 0");
+    if (2 * (cap_prev + cap_now) >= ((int64_t)1 << 32))
+        return vor_fail(ctx, VOR_EINVAL, "vor_t1_events: cap_prev + cap_now must be below 2^31");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t n1 = (size_t)n_labels + 1;
+    uint32_t *deg, *off, *adj_u, *adj_s;
+    uint64_t* U;
+    int rc;
+    const size_t n_adj = 2 * (size_t)(cap_prev + cap_now) + 1;
+    if ((rc = t1_scratch(ctx, 0, 2 * n1 * sizeof(uint32_t), (void**)&deg)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 1, 2 * n1 * sizeof(uint32_t), (void**)&off)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 2, n_adj * sizeof(uint32_t), (void**)&adj_u)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 3, n_adj * sizeof(uint32_t), (void**)&adj_s)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 4, ((size_t)(cap_now + cap_destroyed) + 1) * sizeof(uint64_t), (void**)&U)) != VOR_OK) return rc;
+    T1Graph gp{d_prev, d_n_prev, cap_prev, deg, off, adj_u, adj_s};
+    T1Graph gn{d_now, d_n_now, cap_now, deg + n1, off + n1, adj_u + 2 * cap_prev, adj_s + 2 * cap_prev};
+    T1Lists l{d_now, d_n_now, cap_now, d_created, d_n_created, cap_created, d_destroyed, d_n_destroyed, cap_destroyed};
+
+    VOR_CUDA(cudaMemsetAsync(deg, 0, 2 * n1 * sizeof(uint32_t), stream));
+    const int grid = 4 * ctx->num_sms;                      // 2 * grid partials <= 2 * kMaxCoopBlocks
+    const dim3 both(grid, 2);
+    VOR_LAUNCH(t1_degree_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    VOR_LAUNCH(t1_scan_sum_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_scan_apply_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_fill_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    VOR_LAUNCH(t1_rank_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    VOR_LAUNCH(t1_union_kernel, 2 * grid, 256, 0, stream, l, d_trigger, n_labels, U);
+    VOR_LAUNCH(t1_count_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count);
+    VOR_LAUNCH(t1_write_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count, d_couples, d_class, cap,
+               d_n_couples, ctx->d_flags);
+    VOR_LAUNCH(t1_pair_kernel, 4 * grid, 256, 0, stream, gp, gn, d_couples, d_class, d_n_couples, cap,
+               d_common_prev, d_common_now, d_partner);
     return VOR_OK;
 }

@@ -102,6 +102,42 @@ def gpu_events(v: Vor, prev, now, n):
                 count_prev=cp.cpu().numpy(), count_now=cn.cpu().numpy(), global_trigger=int(g.item()))
 
 
+def gpu_t1(v: Vor, prev, now, n, cap=None):
+    """vor_diff -> vor_events -> vor_t1_events on host lists; returns the same dict as oracle.t1()
+    plus n_couples (the required number, which may exceed cap)."""
+    mk = lambda a: dev(np.asarray(a, np.uint64).view(np.int64)) if len(a) else torch.empty(1, dtype=torch.int64, device="cuda")
+    dp, dn = mk(prev), mk(now)
+    i64 = dict(dtype=torch.int64, device="cuda"); i32 = dict(dtype=torch.int32, device="cuda")
+    npv, nnv = torch.tensor([len(prev)], **i64), torch.tensor([len(now)], **i64)
+    lc = max(1, len(prev) + len(now))
+    c, d = torch.empty(lc, **i64), torch.empty(lc, **i64)
+    nc, nd = torch.zeros(1, **i64), torch.zeros(1, **i64)
+    v.vor_diff(dp, npv, dn, nnv, c, d, nc, nd)
+    trig, idx, cp, cn = (torch.empty(n, **i32) for _ in range(4))
+    m, g = torch.zeros(1, **i32), torch.zeros(1, **i32)
+    v.vor_events(dp, npv, dn, nnv, c, nc, d, nd, trig, idx, m, g, cp, cn)
+    cap = lc if cap is None else cap
+    pad = 3                                                # guard entries behind the capacity
+    couples = torch.full((cap + pad,), -7, **i64); partner = torch.full((cap + pad,), -7, **i64)
+    cls, kp, kn = (torch.full((cap + pad,), -7, **i32) for _ in range(3))
+    nk = torch.full((1,), -7, **i64)
+    v.vor_t1_events(dp, npv, dn, nnv, c, nc, d, nd, trig, couples[:cap], cls[:cap], kp[:cap], kn[:cap],
+                    partner[:cap], nk)
+    try:
+        v.vor_sync_status()
+        overflow = False
+    except Exception as e:                                 # VOR_ECAPACITY: the caller decides whether it was expected
+        overflow = "ECAPACITY" in str(e)
+        if not overflow:
+            raise
+    for t in (couples, partner, cls, kp, kn):
+        assert (t[cap:] == -7).all(), "write past the capacity"
+    k = min(int(nk.item()), cap)
+    return dict(couples=u64(couples, k).copy(), cls=cls[:k].cpu().numpy(), common_prev=kp[:k].cpu().numpy(),
+                common_now=kn[:k].cpu().numpy(), partner=u64(partner, k).copy(), n_couples=int(nk.item()),
+                overflow=overflow)
+
+
 def gpu_ccl(v: Vor, field, thr, above=True):
     f = dev(field.astype(np.float32).ravel())
     ccl = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")

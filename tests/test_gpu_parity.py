@@ -732,6 +732,79 @@ def test_events_hand_random_and_golden(G):
     v.close()
 
 
+# ------------------------------------------------------------------ couples of active vertices, T1 pairing
+T1_KEYS = ("couples", "cls", "common_prev", "common_now", "partner")
+
+
+def check_t1(G, v, prev, now, n):
+    got, ref = G.gpu_t1(v, prev, now, n), oracle.t1(prev, now, n)
+    assert got["n_couples"] == len(ref["couples"]) and not got["overflow"]
+    for k in T1_KEYS:
+        assert np.array_equal(got[k], ref[k]), k
+    return got
+
+
+def random_graph_pair(rng, n, deg, keep=0.9, fresh=0.1):
+    """Two ascending unique key lists over n vertices sharing most of their edges."""
+    def draw(m):
+        i = rng.integers(0, n, m); j = rng.integers(0, n, m)
+        ok = i != j
+        return (np.minimum(i, j)[ok].astype(np.uint64) << np.uint64(32)) | np.maximum(i, j)[ok].astype(np.uint64)
+    a = np.unique(draw(deg * n // 2))
+    b = np.unique(np.concatenate([a[rng.random(len(a)) < keep], draw(max(1, int(fresh * deg * n / 2)))]))
+    return a, b
+
+
+def test_t1_events_hand_graphs_random_graphs_and_golden(G):
+    v = make(64, 64)
+    key = lambda i, j: (min(i, j) << 32) | max(i, j)
+    common = [(0, 1), (1, 2), (2, 3), (0, 3), (0, 4), (1, 4), (2, 5), (3, 5), (4, 5)]
+    r = check_t1(G, v, pack(common + [(1, 3)]), pack(common + [(0, 2)]), 6)              # one T1
+    k = r["couples"].tolist()
+    assert int(r["partner"][k.index(key(1, 3))]) == key(0, 2) and int(r["partner"][k.index(key(0, 2))]) == key(1, 3)
+    rh = lambda o: [(o, o + 1), (o + 1, o + 2), (o + 2, o + 3), (o, o + 3)]
+    glue = [(3, 4), (2, 4), (2, 5)]
+    check_t1(G, v, pack(rh(0) + rh(4) + glue + [(1, 3), (4, 6)]), pack(rh(0) + rh(4) + glue + [(0, 2), (5, 7)]), 8)
+    check_t1(G, v, pack([(0, 1), (1, 2), (0, 2)]), pack([(0, 1), (1, 2)]), 3)            # Fig. 8 boundary event
+    full = [(0, 1), (0, 2), (0, 3), (1, 2), (1, 3), (2, 3)]
+    check_t1(G, v, pack(full), pack(full[1:]), 4)                                        # tetrahedron: no partner
+    check_t1(G, v, pack(common), pack(common), 6)                                        # nothing happened
+    check_t1(G, v, np.empty(0, np.uint64), np.empty(0, np.uint64), 3)
+    check_t1(G, v, np.empty(0, np.uint64), pack([(0, 2)]), 3)
+    check_t1(G, v, pack([(0, 1), (1, 2), (0, 2), (1, 5)]), pack([(0, 1), (1, 2), (2, 6)]), 3)   # labels >= n ignored
+    check_events(G, v, pack([(0, 1)]), pack([(0, 1), (0, 7)]), 3)                        # ... by the trigger as well
+    rng = np.random.default_rng(23)
+    for n, deg in ((2, 1), (7, 3), (33, 6), (1000, 6), (5000, 6), (300, 40)):
+        for _ in range(3):
+            a, b = random_graph_pair(rng, n, deg)
+            check_t1(G, v, a, b, n)
+    # hubs: two adjacent vertices joined to (almost) everybody, long rows through the merge intersection
+    n = 3000
+    a, b = random_graph_pair(rng, n, 4)
+    hub = lambda h, skip: np.array([key(h, t) for t in range(n) if t != h and t % 7 != skip], np.uint64)
+    a = np.unique(np.concatenate([a, hub(5, 0), hub(1700, 1), np.array([key(5, 1700)], np.uint64)]))
+    b = np.unique(np.concatenate([b, hub(5, 2), hub(1700, 1)]))
+    check_t1(G, v, a, b, n)
+    # capacity: the required number is reported, nothing is written past cap, the status says so
+    ref = oracle.t1(a, b, n)
+    got = G.gpu_t1(v, a, b, n, cap=100)
+    assert got["overflow"] and got["n_couples"] == len(ref["couples"]) > 100
+    assert np.array_equal(got["couples"], ref["couples"][:100]) and np.array_equal(got["partner"], ref["partner"][:100])
+    v.close()
+    g = read_golden("rhombus_flip.txt")
+    L = g["L"][0]
+    v = make(L, 16)
+    lists = []
+    for h in (g["h_prev"][0], g["h_now"][0]):
+        sx, sy = rhombus_sites(L, h)
+        lists.append(G.gpu_edges(v, G.gpu_labels(v, sx, sy)))
+    r = check_t1(G, v, lists[0], lists[1], g["n_sites"][0])
+    k = r["couples"].tolist()
+    assert int(r["partner"][k.index(key(*g["destroyed"]))]) == key(*g["created"])
+    assert int(r["partner"][k.index(key(*g["created"]))]) == key(*g["destroyed"])
+    v.close()
+
+
 # ------------------------------------------------------------------ full size, bench.py's launch configuration
 def test_config5_full_size_all_frames(G):
     """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites), ALL 10 frames of the random walk,
@@ -794,6 +867,21 @@ def test_config5_full_size_all_frames(G):
             assert np.array_equal(trig.cpu().numpy(), ev["trigger"]) and int(g.item()) == 1
             assert np.array_equal(idx[:int(m.item())].cpu().numpy(), ev["events_indices"])
             assert np.array_equal(cp.cpu().numpy(), ev["count_prev"]) and np.array_equal(cn.cpu().numpy(), ev["count_now"])
+            couples, partner = torch.empty(cap_e, **i64), torch.empty(cap_e, **i64)   # couples and T1 quadruples
+            cls, kp, kn = (torch.empty(cap_e, **i32) for _ in range(3))
+            nk = torch.zeros(1, **i64)
+            v.vor_t1_events(edges[prv], n_edges[prv], edges[now], n_edges[now], created, n_c, destroyed, n_d, trig,
+                            couples, cls, kp, kn, partner, nk)
+            v.vor_sync_status()
+            t1 = oracle.t1(prev, e, n)
+            k = int(nk.item())
+            assert k == len(t1["couples"]) and np.array_equal(G.u64(couples, k), t1["couples"]), i
+            assert np.array_equal(G.u64(partner, k), t1["partner"]) and np.array_equal(cls[:k].cpu().numpy(), t1["cls"]), i
+            assert np.array_equal(kp[:k].cpu().numpy(), t1["common_prev"]), i
+            assert np.array_equal(kn[:k].cpu().numpy(), t1["common_now"]), i
+            n_t1 = int(((t1["cls"] == 1) & (t1["partner"] != np.uint64(0xFFFFFFFFFFFFFFFF))).sum())
+            assert n_t1 > 0.3 * len(rd)               # about half the breaking links of such a frame are isolated T1 events
+            del couples, partner, cls, kp, kn, t1
         prev = e
         del ref, got
     assert 2.9 * n < len(prev) < 3.0 * n            # E slightly below 3N (R6), as the survey's probe found
