@@ -70,12 +70,13 @@ struct vor_ctx {
     uint64_t* d_keys_a;        // [max_raw_keys]  overflow keys / sort ping
     uint64_t* d_keys_b;        // [max_raw_keys]  sort pong
     int64_t* d_n_raw;          // device control block [8]: 0 = raw/overflow key count, 1 = filtered
-                               //   overflow count, 2 = OR of the overflow keys, 3 = raw key count
+                               //   overflow count, 2 = OR of the overflow keys, 3 = raw key count, 4 = dirty tiles (fused path)
     uint32_t* d_hist;          // [kMaxCoopBlocks * 256] per-block digit histograms
     int64_t* d_blk_count;      // [2 * kMaxCoopBlocks] per-block counts for compactions
 
     // ---- fused label -> edge path (vor_frame_*): compact border columns of the 32-cell tile columns
     int32_t* d_fu_cols;        // [2][L / 32][L]: left, then right border column of every tile column
+    int32_t* d_fu_dirty;       // [(L / 32)^2] tiles whose pairs the labelling kernel could not extract itself
     int64_t fuse;              // option: 1 = vor_frame_* labels and extracts the pairs in one kernel
 
     // ---- row-by-row diff: membership mask per row [dr_rows], then the per-block counts

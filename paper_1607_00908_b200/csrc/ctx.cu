@@ -77,7 +77,7 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_bucket_start); cudaFree(ctx->d_bucket_fill); cudaFree(ctx->d_sorted);
     cudaFree(ctx->d_scan_part); cudaFree(ctx->d_keys_a); cudaFree(ctx->d_keys_b);
     cudaFree(ctx->d_lab_fail); cudaFree(ctx->d_lab_fail_n);
-    cudaFree(ctx->d_fu_cols);
+    cudaFree(ctx->d_fu_cols); cudaFree(ctx->d_fu_dirty);
     cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
     cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts); cudaFree(ctx->d_dr_scratch);
     for (int k = 0; k < 5; ++k) cudaFree(ctx->d_t1[k]);

@@ -806,39 +806,64 @@ __global__ void __launch_bounds__(kSortThreads) edges_finish_kernel(const Finish
 }
 
 // ------------------------------------------------------------------------------------ fused path: seams and left-over tiles
-// The labelling kernel (label.cu, fused variant) leaves, per 32 x 32 tile, the distinct adjacent pairs
-// found INSIDE the tile in kTileKeys fixed slots of the raw-key list.  What is left: the pairs across
-// the tile borders, and the tiles it could not finish (an unproven quadrant: their labels came from the
-// second labelling pass).
-//   fused_tail_kernel  one CTA per "supertile" of 8 x 8 tiles: the tiles' raw keys (or, for a left-over
-//                      tile, the pairs inside it read from the label image) and the pairs across
-//                      the right / lower border of each of its tiles (vertical seams from the compact
-//                      border columns, horizontal seams from rows 32k+31 | 32k+32 of the label image, all
-//                      coalesced) go through one shared-memory hash set, so a pair seen by several tiles
-//                      and seams reaches the adjacency rows about once; then the set is inserted.
-constexpr int kSuper = 8;                       // tiles per supertile side
+// The labelling kernel (label.cu, fused variant) appends the distinct adjacent pairs found INSIDE every
+// 32 x 32 tile to the adjacency rows itself.  What is left:
+//   fused_seam_kernel   the pairs across the tile borders.  Line c < L/32: the vertical seam right of tile
+//                       column c, from the compact border columns the labelling kernel wrote; the other
+//                       L/32 lines: the horizontal seam below tile row c - L/32, rows 32k+31 | 32k+32 of the
+//                       label image.  Both are coalesced reads of 1/16 of the image.  A run of the same pair
+//                       along a line is reported once per warp; a CTA de-duplicates its 2048 positions
+//                       through a small hash set before it touches the rows.
+//   fused_dirty_kernel  the tiles the labelling kernel could not finish (an unproven quadrant: their labels
+//                       came from the second labelling pass): the pairs inside them, from the label image.
+constexpr int kSeamThreads = 256;
+constexpr int kSeamPer = 8;                     // positions per thread
+constexpr int kSeamSlots = 512;                 // about 200 distinct pairs cross 2048 positions at config 5
 constexpr int kTailThreads = 256;
-constexpr int kTailSlots = 2048;                // hash-set slots per supertile (about 900 distinct keys at config 5)
+constexpr int kTailSlots = 2048;
 
-__device__ __forceinline__ void tail_insert(uint32_t a, uint32_t b, unsigned long long* table, const RowSet& rs) {
-    const uint32_t lo = min(a, b), hi = max(a, b);
-    const unsigned long long key = ((unsigned long long)lo << 32) | hi;
-    uint32_t h = hash_key(lo, hi) & (kTailSlots - 1);
-    for (int probe = 0; probe < kMaxProbe; ++probe) {
-        const unsigned long long cur = table[h];
-        if (cur == key) return;
-        if (cur == kEmptyKey) {
-            const unsigned long long old = atomicCAS(&table[h], kEmptyKey, key);
-            if (old == kEmptyKey || old == key) return;
-        }
-        h = (h + 1) & (kTailSlots - 1);
+__global__ void __launch_bounds__(kSeamThreads) fused_seam_kernel(const int32_t* __restrict__ labels,
+                                                                  const int32_t* __restrict__ col_left,
+                                                                  const int32_t* __restrict__ col_right,
+                                                                  int32_t L, const RowSet rs) {
+    __shared__ unsigned long long table[kSeamSlots];
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int32_t nt = L >> 5, c = blockIdx.y;
+    for (int i = threadIdx.x; i < kSeamSlots; i += kSeamThreads) table[i] = kEmptyKey;
+    __syncthreads();
+    const int32_t* __restrict__ pa;
+    const int32_t* __restrict__ pb;
+    if (c < nt) {
+        pa = col_right + (int64_t)c * L;
+        pb = col_left + (int64_t)(c + 1 == nt ? 0 : c + 1) * L;
+    } else {
+        const int32_t y = 32 * (c - nt) + 31;
+        pa = labels + (int64_t)y * L;
+        pb = labels + (int64_t)(y + 1 == L ? 0 : y + 1) * L;
     }
-    row_insert(rs, lo, hi);
+    const int32_t i0 = blockIdx.x * (kSeamThreads * kSeamPer) + threadIdx.x;
+    int32_t a[kSeamPer], b[kSeamPer];
+#pragma unroll
+    for (int k = 0; k < kSeamPer; ++k) {           // L % 32 == 0: whole warps are in or out of range
+        const int32_t i = i0 + k * kSeamThreads;
+        a[k] = i < L ? __ldcs(pa + i) : 0;
+        b[k] = i < L ? __ldcs(pb + i) : 0;
+    }
+#pragma unroll
+    for (int k = 0; k < kSeamPer; ++k) {
+        const int32_t qa = __shfl_up_sync(full, a[k], 1), qb = __shfl_up_sync(full, b[k], 1);
+        if (a[k] != b[k] && (lane == 0 || qa != a[k] || qb != b[k]))
+            hash_insert<kSeamSlots>((uint32_t)a[k], (uint32_t)b[k], table, rs);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kSeamSlots; i += kSeamThreads) {
+        const unsigned long long key = table[i];
+        if (key != kEmptyKey) row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
+    }
 }
 
-// A tile the labelling kernel could not finish (its labels came from the second pass): the pairs inside
-// it from the label image, lane = column, all 32 rows in flight at once.  Kept out of line: it is rare
-// and must not cost the common path registers.
+// The pairs inside one 32 x 32 tile from the label image, lane = column, all 32 rows in flight at once.
 __device__ __noinline__ void tail_dirty_tile(const int32_t* __restrict__ p, int32_t L, int lane,
                                              unsigned long long* table, const RowSet& rs) {
     const unsigned full = 0xffffffffu;
@@ -853,59 +878,28 @@ __device__ __noinline__ void tail_dirty_tile(const int32_t* __restrict__ p, int3
         const int32_t below = v[r < 31 ? r + 1 : 31];
         const int32_t lc = __shfl_up_sync(full, cur, 1), lb = __shfl_up_sync(full, below, 1);
         if (lane < 31 && cur != right && (r == 0 || cur != v[r > 0 ? r - 1 : 0] || right != upr))
-            tail_insert((uint32_t)cur, (uint32_t)right, table, rs);
+            hash_insert<kTailSlots>((uint32_t)cur, (uint32_t)right, table, rs);
         if (r < 31 && cur != below && (lane == 0 || lc != cur || lb != below))
-            tail_insert((uint32_t)cur, (uint32_t)below, table, rs);
+            hash_insert<kTailSlots>((uint32_t)cur, (uint32_t)below, table, rs);
         upr = right;
     }
 }
 
-__global__ void __launch_bounds__(kTailThreads) fused_tail_kernel(const int32_t* __restrict__ labels,
-                                                                  const int32_t* __restrict__ col_left,
-                                                                  const int32_t* __restrict__ col_right,
-                                                                  int32_t L, const RowSet rs) {
+__global__ void __launch_bounds__(kTailThreads) fused_dirty_kernel(const int32_t* __restrict__ labels,
+                                                                   const int32_t* __restrict__ dirty_tiles,
+                                                                   const int32_t* __restrict__ dirty_count,
+                                                                   int32_t L, const RowSet rs) {
     __shared__ unsigned long long table[kTailSlots];
-    const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int32_t nt = L >> 5;
-    const int32_t tx0 = blockIdx.x * kSuper, ty0 = blockIdx.y * kSuper;
-    const int32_t ntx = min(kSuper, nt - tx0), nty = min(kSuper, nt - ty0);        // tiles of this supertile
+    const int32_t nt = L >> 5, n = *dirty_count;
+    if ((int32_t)(blockIdx.x * (kTailThreads / 32)) >= n) return;
     for (int i = threadIdx.x; i < kTailSlots; i += kTailThreads) table[i] = kEmptyKey;
     __syncthreads();
-    // ---- the tiles' own keys: one warp per tile, one slot per lane
-    for (int t = wid; t < ntx * nty; t += kTailThreads / 32) {
-        const int32_t tile = (ty0 + t / ntx) * nt + tx0 + t % ntx;
-        static_assert(kTileKeys == 32, "one slot per lane");
-        const unsigned long long key = __ldcs(reinterpret_cast<const unsigned long long*>(rs.raw) + (size_t)tile * kTileKeys + lane);
-        if (__shfl_sync(full, key, 0) != kDirtyTileKey) {
-            if (key != kEmptyKey) tail_insert((uint32_t)(key >> 32), (uint32_t)key, table, rs);
-            continue;
-        }
+    for (int32_t t = blockIdx.x * (kTailThreads / 32) + wid; t < n; t += gridDim.x * (kTailThreads / 32)) {
+        const int32_t tile = dirty_tiles[t];
         tail_dirty_tile(labels + (int64_t)(tile / nt) * 32 * L + (tile % nt) * 32 + lane, L, lane, table, rs);
     }
-    // ---- seams: line c (c < ntx: right border of tile column tx0 + c; else lower border of tile row
-    // ty0 + c - ntx), 32 * (tiles along it) pairs; a run of the same pair is reported once per warp
-    const int32_t len_v = 32 * nty, len_h = 32 * ntx;
-    for (int c = 0; c < ntx + nty; ++c) {
-        const bool vert = c < ntx;
-        const int32_t len = vert ? len_v : len_h;
-        for (int32_t i = threadIdx.x; i < len; i += kTailThreads) {     // len % 32 == 0: whole warps
-            int32_t a, b;
-            if (vert) {
-                const int32_t tc = tx0 + c, nx = tc + 1 == nt ? 0 : tc + 1;
-                a = __ldcs(col_right + (int64_t)tc * L + 32 * ty0 + i);
-                b = __ldcs(col_left + (int64_t)nx * L + 32 * ty0 + i);
-            } else {
-                const int32_t y = 32 * (ty0 + c - ntx) + 31, yn = y + 1 == L ? 0 : y + 1;
-                a = __ldg(labels + (int64_t)y * L + 32 * tx0 + i);
-                b = __ldg(labels + (int64_t)yn * L + 32 * tx0 + i);
-            }
-            const int32_t pa = __shfl_up_sync(full, a, 1), pb = __shfl_up_sync(full, b, 1);
-            if (a != b && (lane == 0 || pa != a || pb != b)) tail_insert((uint32_t)a, (uint32_t)b, table, rs);
-        }
-    }
     __syncthreads();
-    // ---- the set goes to the adjacency rows
     for (int i = threadIdx.x; i < kTailSlots; i += kTailThreads) {
         const unsigned long long key = table[i];
         if (key != kEmptyKey) row_insert(rs, (uint32_t)(key >> 32), (uint32_t)key);
@@ -983,8 +977,10 @@ int vor_edges_fused_tail(vor_ctx* ctx, const int32_t* d_labels, const RowSet& rs
     const int32_t L = ctx->L, nt = L / 32;
     const int32_t* col_left = ctx->d_fu_cols;
     const int32_t* col_right = ctx->d_fu_cols + (size_t)nt * L;
-    const unsigned ns = (unsigned)((nt + kSuper - 1) / kSuper);
-    VOR_LAUNCH(fused_tail_kernel, dim3(ns, ns), kTailThreads, 0, stream, d_labels, col_left, col_right, L, rs);
+    const dim3 grid((L + kSeamThreads * kSeamPer - 1) / (kSeamThreads * kSeamPer), 2 * nt);
+    VOR_LAUNCH(fused_seam_kernel, grid, kSeamThreads, 0, stream, d_labels, col_left, col_right, L, rs);
+    VOR_LAUNCH(fused_dirty_kernel, 4 * ctx->num_sms, kTailThreads, 0, stream, d_labels, ctx->d_fu_dirty,
+               (const int32_t*)&ctx->d_n_raw[4], L, rs);
     return VOR_OK;
 }
 

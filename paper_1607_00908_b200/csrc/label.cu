@@ -60,6 +60,8 @@ struct LabelParams {
     // in compact form, col[tile_x * L + y]
     int32_t* col_left;
     int32_t* col_right;
+    int32_t* dirty_tiles;      // tiles with an unproven quadrant: their pairs are taken from the label image
+    int32_t* dirty_count;
 };
 
 // fused path: a label written by the second pass also goes to the compact border columns
@@ -615,51 +617,62 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
 
 // ---- fused path: the adjacent pairs of a CTA's 32 x 32 cells, straight from the labelling registers.
 // Every cell carries the SLOT (0..63) of its site in the CTA's gathered list, one byte per cell, four
-// rows per register (lane = column).  Right neighbours come from one shuffle per register, lower
-// neighbours from a byte shift.  A differing pair of slots sets one bit of the CTA's 64 x 64 bit
-// matrix in shared memory (the de-duplication), which is decoded into (label, label) keys at the end.
+// rows per register (lane = column); all comparisons below work on four rows at once.
+// The compared pairs ("links": H = cell | right neighbour, V = cell | cell below) that join the same two
+// slots form chains along the common border of the two regions.  Order the links of a warp's 32 x 16
+// block by (row, H before V, column).  A link is reported only if none of the chain neighbours that
+// PRECEDE it in that order joins the same two slots:
+//   H link (a | b), u and v the cells above a and b:   u == b  (the V link u|a)   v == a  (the V link v|b)
+//                                                      u == a and v == b  (the H link above)
+//   V link (a over d), p and q the cells left of a and d, s the cell right of a:
+//                                                      p == d  (the H link p|a)   s == d  (the H link a|s)
+//                                                      p == a and q == d  (the V link to the left)
+// The first link of every pair of slots in the block has no predecessor, so every adjacent pair is
+// reported at least once - and a straight or staircase border exactly once, which is what keeps the work
+// per cell small.  Reported links set one bit of the CTA's 64 x 64 bit matrix in shared memory (the
+// de-duplication across the two warps), decoded into (label, label) keys at the end.
 __device__ __forceinline__ void bm_set(uint32_t* bm, uint32_t a, uint32_t b) {
     const uint32_t idx = min(a, b) * kCtaCapSites + max(a, b);
     atomicOr(&bm[idx >> 5], 1u << (idx & 31));
 }
 
-// one bit-matrix entry per non-zero byte of x: the pair (byte of aw, byte of bw) at that position
-__device__ __forceinline__ void emit_bytes(uint32_t x, uint32_t aw, uint32_t bw, uint32_t* bm) {
-    while (__any_sync(0xffffffffu, x != 0)) {
-        if (x) {
-            const int s = (__ffs(x) - 1) & ~7;
-            bm_set(bm, (aw >> s) & 255u, (bw >> s) & 255u);
-            x &= ~(255u << s);
-        }
+// most significant bit of every byte: that byte of x (all bytes < 0x80) is not zero
+__device__ __forceinline__ uint32_t nz7(uint32_t x) { return x + 0x7f7f7f7fu; }
+
+// one bit-matrix entry per flagged byte (bit 7) of m: the pair (byte of aw, byte of bw) at that position
+__device__ __forceinline__ void emit_flagged(uint32_t m, uint32_t aw, uint32_t bw, uint32_t* bm) {
+    while (m) {
+        const int s = (__ffs(m) - 1) & ~7;
+        m &= m - 1;
+        bm_set(bm, (aw >> s) & 255u, (bw >> s) & 255u);
     }
 }
 
-// 0xff in every byte of v that is not zero
-__device__ __forceinline__ uint32_t nonzero_bytes(uint32_t v) {
-    const uint32_t t = (((v & 0x7f7f7f7fu) + 0x7f7f7f7fu) | v) & 0x80808080u;
-    return (t >> 7) * 255u;
-}
-
-// W[i]: slots of rows 4i .. 4i+3 of this lane's column (a warp's 16 rows).  Pairs with the column to
+// W[i]: slots of rows 4i .. 4i+3 of this lane's column (a warp's 16 rows).  Links with the column to
 // the right (lanes 0..30) and with the row below (rows 0..14); the row below row 15 is the other
-// warp's or the next tile's business.
-__device__ __forceinline__ void cta_pairs(const uint32_t (&W)[4], uint32_t* bm) {
+// warp's or the next tile's business, the column right of lane 31 the seam kernel's.
+__device__ __forceinline__ void cta_pairs(const uint32_t (&W)[4], int lane, uint32_t* bm) {
     const unsigned full = 0xffffffffu;
-    uint32_t D[4], PD[4];
+    constexpr uint32_t kNone = 0x7f7f7f7fu;                // a slot no cell carries
+    uint32_t R[4], PL[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        PD[i] = i < 3 ? (W[i] >> 8) | (W[i + 1] << 24) : (W[3] >> 8) | (W[3] & 0xff000000u);
-        D[i] = W[i] ^ PD[i];                                   // byte b: rows 4i+b and 4i+b+1 differ
+        R[i] = __shfl_down_sync(full, W[i], 1);            // lane 31 reads itself: no H link, no cell to the right
+        PL[i] = __shfl_up_sync(full, W[i], 1);
+        if (lane == 0) PL[i] = kNone;                      // nothing to the left
     }
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint32_t R = __shfl_down_sync(full, W[i], 1);    // lane 31 reads itself: no pair
-        // a horizontal pair that repeats the row above (same slot on both sides) is skipped: "changed"
-        // marks the rows whose own or right slot differs from the row above; row 0 always counts
-        const uint32_t UW = i ? (D[i] << 8) | (D[i - 1] >> 24) : (D[0] << 8) | 0xffu;
-        const uint32_t changed = UW | __shfl_down_sync(full, UW, 1);
-        emit_bytes((W[i] ^ R) & nonzero_bytes(changed), W[i], R, bm);
-        emit_bytes(D[i], W[i], PD[i], bm);
+        const uint32_t a = W[i], b = R[i];
+        const uint32_t u = i ? __funnelshift_l(W[i - 1], W[i], 8) : (W[0] << 8) | 0x7fu;   // the rows above
+        const uint32_t v = i ? __funnelshift_l(R[i - 1], R[i], 8) : (R[0] << 8) | 0x7fu;
+        const uint32_t mh = nz7(a ^ b) & nz7(u ^ b) & nz7(v ^ a) & nz7((u ^ a) | (v ^ b)) & 0x80808080u;
+        emit_flagged(mh, a, b, bm);
+        const uint32_t d = i < 3 ? __funnelshift_r(W[i], W[i + 1], 8) : (W[3] >> 8) | (W[3] & 0xff000000u);
+        const uint32_t p = PL[i];
+        const uint32_t q = i < 3 ? __funnelshift_r(PL[i], PL[i + 1], 8) : (PL[3] >> 8) | (PL[3] & 0xff000000u);
+        const uint32_t mv = nz7(a ^ d) & nz7(p ^ d) & nz7(b ^ d) & nz7((p ^ a) | (q ^ d)) & 0x80808080u;
+        emit_flagged(mv, a, d, bm);
     }
 }
 
@@ -701,9 +714,8 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     }
     // fused: a tile with an unproven quadrant gets its pairs from the label image later (tile list)
     if constexpr (kFused) {
-        if (any_fail && threadIdx.x < kTileKeys)         // slot 0 tells fused_tail_kernel to read the tile itself
-            rs.raw[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * kTileKeys + threadIdx.x] =
-                threadIdx.x == 0 ? kDirtyTileKey : kEmptyKey;
+        if (any_fail && threadIdx.x == 0)
+            p.dirty_tiles[atomicAdd(p.dirty_count, 1)] = blockIdx.y * gridDim.x + blockIdx.x;
     }
     // ---- phase B: warp = 32 x 16 cells, lane = column
     const int wx = wid % (kCtaQX / 4), wy = wid / (kCtaQX / 4);
@@ -796,13 +808,12 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     }
     if constexpr (kFused) {
         if (any_fail) return;                            // CTA-uniform
-        cta_pairs(W, fs.bm);
+        cta_pairs(W, lane, fs.bm);
         if (wid == 0) fs.seam[lane] = W[3] >> 24;        // row 15 of the tile
         __syncthreads();
         if (wid == 0) return;
         // the lower warp finishes alone (no further barrier): rows 15 | 16, then the bit matrix is decoded
-        // into the tile's kTileKeys slots of the raw-key list (plain stores, no atomics: nothing here waits
-        // for memory); slots left over are marked empty, keys that do not fit go straight to the rows
+        // and every distinct pair of the tile is appended to its adjacency row
         {
             const uint32_t a = fs.seam[lane], b = W[0] & 255u;
             const uint32_t pa = __shfl_up_sync(0xffffffffu, a, 1), pb = __shfl_up_sync(0xffffffffu, b, 1);
@@ -810,34 +821,16 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
         }
         __syncwarp();
         constexpr int kWords = kCtaCapSites * kCtaCapSites / 32 / 32;      // bit-matrix words per lane (4)
-        uint32_t m[kWords];
-        int cnt = 0;
-#pragma unroll
-        for (int k = 0; k < kWords; ++k) { m[k] = fs.bm[kWords * lane + k]; cnt += __popc(m[k]); }
-        int inc = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        const int total = __shfl_sync(0xffffffffu, inc, 31);
-        int pos = inc - cnt;
-        unsigned long long* __restrict__ slots =
-            (unsigned long long*)rs.raw + (size_t)(blockIdx.y * gridDim.x + blockIdx.x) * kTileKeys;
 #pragma unroll
         for (int k = 0; k < kWords; ++k) {
-            uint32_t mk = m[k];
+            uint32_t mk = fs.bm[kWords * lane + k];
             while (mk) {
                 const uint32_t idx = 32u * (kWords * lane + k) + (__ffs(mk) - 1);
                 mk &= mk - 1;
                 const uint32_t la = (uint32_t)sh.si[idx / kCtaCapSites], lb = (uint32_t)sh.si[idx % kCtaCapSites];
-                const uint32_t lo = min(la, lb), hi = max(la, lb);
-                if (pos < kTileKeys) slots[pos] = ((unsigned long long)lo << 32) | hi;
-                else row_insert(rs, lo, hi);
-                ++pos;
+                row_insert(rs, min(la, lb), max(la, lb));
             }
         }
-        for (int k = total + lane; k < kTileKeys; k += 32) slots[k] = kEmptyKey;
     }
 }
 
@@ -908,7 +901,7 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaS
     p.n_dev = ctx->d_n_dev;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
     p.fail_items = nullptr; p.fail_count = nullptr; p.fail_count_next = nullptr; p.fail_cap = 0;
-    p.col_left = nullptr; p.col_right = nullptr;
+    p.col_left = nullptr; p.col_right = nullptr; p.dirty_tiles = nullptr; p.dirty_count = nullptr;
     const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint);    // cells
     const int path = label_path_for(ctx, spacing);
     const int tw = path == 3 ? 16 : 8;
@@ -951,6 +944,8 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaS
         if (rs) {
             p.col_left = ctx->d_fu_cols;
             p.col_right = ctx->d_fu_cols + (size_t)(ctx->L / 32) * ctx->L;
+            p.dirty_tiles = ctx->d_fu_dirty;
+            p.dirty_count = (int32_t*)&ctx->d_n_raw[4];
             VOR_LAUNCH(label_cta_kernel<true>, grid, kCtaThreads, 0, stream, p, d_labels, *rs);
         } else {
             VOR_LAUNCH(label_cta_kernel<false>, grid, kCtaThreads, 0, stream, p, d_labels, RowSet{});
@@ -980,7 +975,6 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
 // CTA kernel's 32 x 32 tiles on a lattice they tile exactly.
 bool vor_label_fusable(const vor_ctx* ctx) {
     if (ctx->nb <= 0 || ctx->L % 32 != 0 || !ctx->fuse) return false;
-    if ((int64_t)(ctx->L / 32) * (ctx->L / 32) * kTileKeys > ctx->max_raw_keys) return false;   // raw slots per tile
     return label_path_for(ctx, sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint)) == 3;
 }
 
@@ -989,6 +983,7 @@ bool vor_label_fusable(const vor_ctx* ctx) {
 int vor_label_fused(vor_ctx* ctx, int32_t* d_labels, const RowSet& rs, cudaStream_t stream) {
     if (!ctx->d_fu_cols) {
         VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_cols, 2 * (size_t)(ctx->L / 32) * ctx->L * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_dirty, (size_t)(ctx->L / 32) * (ctx->L / 32) * sizeof(int32_t)));
     }
     return label_launch(ctx, d_labels, &rs, stream);
 }

@@ -1,5 +1,5 @@
 // Adjacency rows shared by the kernels that find label discontinuities (edges.cu: from a label image;
-// fused.cu: straight from the labelling kernel's registers): row a of the matrix collects the
+// label.cu, fused variant: straight from the labelling kernel's registers): row a of the matrix collects the
 // larger-index neighbours b of site a (§III.B: one row per label, pre-filled with a
 // sentinel).  See edges.cu for how the rows become the sorted edge list.
 #pragma once
@@ -7,8 +7,6 @@
 #include "common.cuh"
 
 constexpr uint64_t kEmptyKey = ~0ull;
-constexpr int kTileKeys = 32;              // fused path: raw-key slots per 32 x 32 tile
-constexpr uint64_t kDirtyTileKey = ~1ull;   // in slot 0: the tile's pairs must be taken from the label image
 
 struct RowSet {
     uint32_t* rows;            // [n_rows * kRowStride]
