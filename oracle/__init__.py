@@ -178,6 +178,110 @@ def t1(prev, now, n):
                 common_now=cn[:m].copy(), partner=partner[:m].copy())
 
 
+# ---- O9: the same definitions on a rectangular lattice with periodic or walled axes (see vor_oracle.cpp)
+def label_brute_g(Lx, Ly, per_x, per_y, sx, sy, threads=0):
+    sx, sy = _i32(sx), _i32(sy)
+    out = np.empty((Ly, Lx), dtype=np.int32)
+    lib().orc_label_brute_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), C.c_int32(len(sx)),
+                            _p(sx, C.c_int32), _p(sy, C.c_int32), _p(out, C.c_int32), C.c_int(threads))
+    return out
+
+
+def label_brute_at_g(Lx, Ly, per_x, per_y, sx, sy, cells, threads=0):
+    sx, sy = _i32(sx), _i32(sy)
+    cells = np.ascontiguousarray(cells, dtype=np.int64)
+    out = np.empty(len(cells), dtype=np.int32)
+    lib().orc_label_brute_at_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), C.c_int32(len(sx)),
+                               _p(sx, C.c_int32), _p(sy, C.c_int32), C.c_int64(len(cells)), _p(cells, C.c_int64),
+                               _p(out, C.c_int32), C.c_int(threads))
+    return out
+
+
+def label_cells_g(Lx, Ly, per_x, per_y, sx, sy, bucket_cells, threads=0):
+    sx, sy = _i32(sx), _i32(sy)
+    out = np.empty((Ly, Lx), dtype=np.int32)
+    lib().orc_label_cells_g.restype = C.c_int
+    rc = lib().orc_label_cells_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), C.c_int32(len(sx)),
+                                 _p(sx, C.c_int32), _p(sy, C.c_int32), C.c_int32(bucket_cells),
+                                 _p(out, C.c_int32), C.c_int(threads))
+    if rc != 0:
+        raise ValueError("bucket_cells must divide Lx and Ly")
+    return out
+
+
+def edges_g(labels, per_x=1, per_y=1, exclude=-1):
+    labels = _i32(labels)
+    Ly, Lx = labels.shape
+    buf = np.empty(2 * Lx * Ly + 1, dtype=np.uint64)
+    lib().orc_edges_g.restype = C.c_int64
+    m = lib().orc_edges_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), C.c_int32(exclude),
+                          _p(labels, C.c_int32), _p(buf, C.c_uint64), C.c_int64(len(buf)))
+    return buf[:m].copy()
+
+
+def apply_obstacles(labels, obstacle_mask, colour):
+    """obstacle sites take a fixed large colour (MAXLINK) instead of a bubble's label."""
+    return np.where(np.asarray(obstacle_mask) != 0, np.int32(colour), _i32(labels)).astype(np.int32)
+
+
+def threshold_ccl_g(field, thr, above=True, per_x=1, per_y=1, connectivity=4):
+    field = np.ascontiguousarray(field, dtype=np.float32)
+    Ly, Lx = field.shape
+    out = np.empty((Ly, Lx), dtype=np.int32)
+    lib().orc_threshold_ccl_g.restype = C.c_int
+    rc = lib().orc_threshold_ccl_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y),
+                                   _p(field, C.c_float), C.c_float(thr), C.c_int(1 if above else 0),
+                                   C.c_int(connectivity), _p(out, C.c_int32))
+    if rc != 0:
+        raise ValueError("connectivity must be 4 or 8")
+    return out
+
+
+def centroids_g(ccl, min_size, per_x=1, per_y=1, field=None):
+    ccl = _i32(ccl)
+    Ly, Lx = ccl.shape
+    cap = max(1, (Lx * Ly + 1) // 2)
+    cx = np.empty(cap); cy = np.empty(cap)
+    sx = np.empty(cap, dtype=np.int32); sy = np.empty(cap, dtype=np.int32)
+    size = np.empty(cap, dtype=np.int32); root = np.empty(cap, dtype=np.int32)
+    fp = None
+    if field is not None:
+        field = np.ascontiguousarray(field, dtype=np.float32)
+        assert field.shape == ccl.shape
+        fp = _p(field, C.c_float)
+    lib().orc_centroids_g.restype = C.c_int32
+    K = lib().orc_centroids_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), _p(ccl, C.c_int32), fp,
+                              C.c_int32(min_size), _p(cx, C.c_double), _p(cy, C.c_double), _p(sx, C.c_int32),
+                              _p(sy, C.c_int32), _p(size, C.c_int32), _p(root, C.c_int32), C.c_int32(cap))
+    return dict(cx=cx[:K].copy(), cy=cy[:K].copy(), sx=sx[:K].copy(), sy=sy[:K].copy(),
+                size=size[:K].copy(), root=root[:K].copy())
+
+
+def match_g(Lx, Ly, per_x, per_y, px, py, nx, ny, radius_fp):
+    px, py, nx, ny = _i32(px), _i32(py), _i32(nx), _i32(ny)
+    p2n = np.empty(len(px), dtype=np.int32)
+    n2p = np.empty(len(nx), dtype=np.int32)
+    lib().orc_match_g(C.c_int32(Lx), C.c_int32(Ly), C.c_int(per_x), C.c_int(per_y), _p(px, C.c_int32),
+                      _p(py, C.c_int32), C.c_int32(len(px)), _p(nx, C.c_int32), _p(ny, C.c_int32),
+                      C.c_int32(len(nx)), C.c_int32(radius_fp), _p(p2n, C.c_int32), _p(n2p, C.c_int32))
+    return p2n, n2p
+
+
+def size_histogram(size, bin_width, n_bins):
+    size = _i32(size)
+    hist = np.zeros(n_bins, dtype=np.int64)
+    lib().orc_size_histogram(_p(size, C.c_int32), C.c_int32(len(size)), C.c_int32(bin_width), C.c_int32(n_bins),
+                             _p(hist, C.c_int64))
+    return hist
+
+
+def edge_commons(edges, n):
+    edges = np.ascontiguousarray(edges, dtype=np.uint64)
+    out = np.empty(len(edges), dtype=np.int32)
+    lib().orc_edge_commons(_p(edges, C.c_uint64), C.c_int64(len(edges)), C.c_int32(n), _p(out, C.c_int32))
+    return out
+
+
 def unpack(keys):
     """uint64 packed keys -> (i, j) int64 arrays."""
     keys = np.asarray(keys, dtype=np.uint64)

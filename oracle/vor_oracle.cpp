@@ -460,6 +460,278 @@ i64 orc_t1(const u64* prev, i64 n_prev, const u64* now, i64 n_now, int32_t n,
     return m;
 }
 
+// ------------------------------------------------------------------------------------------------------
+// O9 — the same definitions on the paper's own geometry: a rectangular
+// Lx x Ly lattice (§IV: "Lx x Ly = 2048 x 1024"), each axis either periodic or closed by walls
+// (§III.B.2: on the domain boundaries "the frame is given by all nearest neighbours that do
+// not lie outside the domain"), obstacle sites carrying an excluded colour (§III.B.1: MAXLINK,
+// "regions of the lattice with undefined colour which automatically will not be considered for the
+// Delaunay triangulation"), 8-connected bubbles (reachable "along the directions of the
+// Lattice Boltzmann model", D2Q9), density-weighted centres (§II eq. for z*), the bubble-size
+// histogram ("characterize them according to their size"), bulk / boundary
+// edges.  With Lx == Ly, both axes periodic, no exclusion, 4-connectivity and no weights
+// these functions compute what O1..O6 compute (pinned by equality in tests/test_oracle_geometry.py).
+// Conventions: cell (x, y), 0 <= x < Lx, 0 <= y < Ly, linear index y*Lx + x; Px = 256*Lx, Py = 256*Ly;
+// on a walled axis the distance is the plain difference and nothing wraps.
+
+namespace {
+
+inline i64 axis_dist(i64 c, i64 s, i64 P, int periodic) {
+    i64 a = c > s ? c - s : s - c;
+    return periodic && P - a < a ? P - a : a;
+}
+
+inline int32_t brute_one_g(int32_t Lx, int32_t Ly, int px, int py, int32_t n, const int32_t* sx,
+                           const int32_t* sy, i64 x, i64 y) {
+    const i64 Px = 256 * (i64)Lx, Py = 256 * (i64)Ly;
+    const i64 cx = 256 * x + 128, cy = 256 * y + 128;
+    i64 best = INT64_MAX;
+    int32_t besti = -1;
+    for (int32_t i = 0; i < n; ++i) {
+        const i64 dx = axis_dist(cx, sx[i], Px, px), dy = axis_dist(cy, sy[i], Py, py);
+        const i64 d2 = dx * dx + dy * dy;
+        if (d2 < best) { best = d2; besti = i; }
+    }
+    return besti;
+}
+
+}  // namespace
+
+// O1a on the general geometry.  labels[y*Lx + x]; no site at all -> -1.
+void orc_label_brute_g(int32_t Lx, int32_t Ly, int per_x, int per_y, int32_t n, const int32_t* sx,
+                       const int32_t* sy, int32_t* labels, int threads) {
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int32_t y = 0; y < Ly; ++y)
+        for (int32_t x = 0; x < Lx; ++x)
+            labels[(size_t)y * Lx + x] = brute_one_g(Lx, Ly, per_x, per_y, n, sx, sy, x, y);
+}
+
+void orc_label_brute_at_g(int32_t Lx, int32_t Ly, int per_x, int per_y, int32_t n, const int32_t* sx,
+                          const int32_t* sy, int64_t m, const int64_t* cells, int32_t* out, int threads) {
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int64_t k = 0; k < m; ++k)
+        out[k] = brute_one_g(Lx, Ly, per_x, per_y, n, sx, sy, cells[k] % Lx, cells[k] / Lx);
+}
+
+// O1b on the general geometry: the ring search of reading R3 over nbx x nby buckets of bucket_cells cells.
+// A ring position outside a walled axis holds no bucket; on a periodic axis it wraps.  The stop rule is
+// unchanged (after ring r every unscanned site has |dx| or |dy| > r*w).  When a ring would wrap onto
+// itself on a periodic axis, or has left the lattice on every side, the cell is finished by O1a.
+int orc_label_cells_g(int32_t Lx, int32_t Ly, int per_x, int per_y, int32_t n, const int32_t* sx,
+                      const int32_t* sy, int32_t bucket_cells, int32_t* labels, int threads) {
+    if (bucket_cells < 1 || Lx % bucket_cells != 0 || Ly % bucket_cells != 0) return -1;
+    const int32_t nbx = Lx / bucket_cells, nby = Ly / bucket_cells;
+    const i64 w = 256 * (i64)bucket_cells, Px = 256 * (i64)Lx, Py = 256 * (i64)Ly;
+    std::vector<int32_t> start((size_t)nbx * nby + 1, 0), items(n);
+    for (int32_t i = 0; i < n; ++i) start[(size_t)(sy[i] / w) * nbx + sx[i] / w + 1]++;
+    for (size_t b = 0; b < (size_t)nbx * nby; ++b) start[b + 1] += start[b];
+    {
+        std::vector<int32_t> fill(start.begin(), start.end() - 1);
+        for (int32_t i = 0; i < n; ++i) items[fill[(size_t)(sy[i] / w) * nbx + sx[i] / w]++] = i;
+    }
+    int nt = resolve_threads(threads);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int32_t y = 0; y < Ly; ++y) {
+        for (int32_t x = 0; x < Lx; ++x) {
+            const i64 cx = 256 * (i64)x + 128, cy = 256 * (i64)y + 128;
+            const int32_t bx = (int32_t)(cx / w), by = (int32_t)(cy / w);
+            i64 best = INT64_MAX;
+            int32_t besti = -1, result = -2;
+            for (int32_t r = 0; result == -2; ++r) {
+                const bool wraps = (per_x && 2 * r + 1 >= nbx) || (per_y && 2 * r + 1 >= nby);
+                const bool outside = r > std::max(nbx, nby);
+                if (wraps || outside) { result = brute_one_g(Lx, Ly, per_x, per_y, n, sx, sy, x, y); break; }
+                for (int32_t oy = -r; oy <= r; ++oy) {
+                    for (int32_t ox = -r; ox <= r; ++ox) {
+                        if (std::max(std::abs(ox), std::abs(oy)) != r) continue;
+                        int32_t qx = bx + ox, qy = by + oy;
+                        if (per_x) qx = (qx % nbx + nbx) % nbx; else if (qx < 0 || qx >= nbx) continue;
+                        if (per_y) qy = (qy % nby + nby) % nby; else if (qy < 0 || qy >= nby) continue;
+                        const size_t b = (size_t)qy * nbx + qx;
+                        for (int32_t k = start[b]; k < start[b + 1]; ++k) {
+                            const int32_t i = items[k];
+                            const i64 dx = axis_dist(cx, sx[i], Px, per_x), dy = axis_dist(cy, sy[i], Py, per_y);
+                            const i64 d2 = dx * dx + dy * dy;
+                            if (d2 < best || (d2 == best && i < besti)) { best = d2; besti = i; }
+                        }
+                    }
+                }
+                const i64 rw = (i64)r * w;
+                if (besti >= 0 && r >= 1 && best <= rw * rw) result = besti;
+            }
+            labels[(size_t)y * Lx + x] = result;
+        }
+    }
+    return 0;
+}
+
+// O2 on the general geometry: every cell against its right and its lower neighbour; a neighbour beyond a
+// wall does not exist; a pair with the excluded colour on either side is not an edge.
+// exclude < 0: nothing is excluded.
+int64_t orc_edges_g(int32_t Lx, int32_t Ly, int per_x, int per_y, int32_t exclude, const int32_t* labels,
+                    uint64_t* out, int64_t cap) {
+    std::vector<u64> keys;
+    auto add = [&](int32_t a, int32_t b) {
+        if (a == b) return;
+        if (exclude >= 0 && (a == exclude || b == exclude)) return;
+        keys.push_back(((u64)(uint32_t)std::min(a, b) << 32) | (uint32_t)std::max(a, b));
+    };
+    for (int32_t y = 0; y < Ly; ++y) {
+        for (int32_t x = 0; x < Lx; ++x) {
+            const int32_t a = labels[(size_t)y * Lx + x];
+            if (x + 1 < Lx) add(a, labels[(size_t)y * Lx + x + 1]);
+            else if (per_x) add(a, labels[(size_t)y * Lx]);
+            if (y + 1 < Ly) add(a, labels[(size_t)(y + 1) * Lx + x]);
+            else if (per_y) add(a, labels[x]);
+        }
+    }
+    std::sort(keys.begin(), keys.end());
+    keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+    const int64_t m = (int64_t)keys.size();
+    for (int64_t k = 0; k < m && k < cap; ++k) out[k] = keys[k];
+    return m;
+}
+
+// O4 on the general geometry; connectivity 4 (reading R9) or 8 (the D2Q9 directions of PAPER.md:95, 147).
+int orc_threshold_ccl_g(int32_t Lx, int32_t Ly, int per_x, int per_y, const float* field, float thr, int above,
+                        int connectivity, int32_t* ccl) {
+    if (connectivity != 4 && connectivity != 8) return -1;
+    const size_t n = (size_t)Lx * Ly;
+    std::vector<uint8_t> mask(n);
+    for (size_t i = 0; i < n; ++i) mask[i] = above ? (field[i] > thr) : (field[i] < thr);
+    for (size_t i = 0; i < n; ++i) ccl[i] = -1;
+    static const int DX[8] = {1, -1, 0, 0, 1, 1, -1, -1}, DY[8] = {0, 0, 1, -1, 1, -1, 1, -1};
+    std::vector<int32_t> queue;
+    for (size_t seed = 0; seed < n; ++seed) {
+        if (!mask[seed] || ccl[seed] != -1) continue;
+        queue.clear();
+        queue.push_back((int32_t)seed);
+        ccl[seed] = (int32_t)seed;
+        for (size_t head = 0; head < queue.size(); ++head) {
+            const int32_t c = queue[head], x = c % Lx, y = c / Lx;
+            for (int k = 0; k < connectivity; ++k) {
+                int32_t u = x + DX[k], v = y + DY[k];
+                if (u < 0 || u >= Lx) { if (!per_x) continue; u = (u + Lx) % Lx; }
+                if (v < 0 || v >= Ly) { if (!per_y) continue; v = (v + Ly) % Ly; }
+                const size_t q = (size_t)v * Lx + u;
+                if (mask[q] && ccl[q] == -1) { ccl[q] = (int32_t)seed; queue.push_back((int32_t)q); }
+            }
+        }
+    }
+    return 0;
+}
+
+// O5 on the general geometry, optionally weighted by the density (z* = sum(y rho) / sum(rho)).
+// Weight of a cell: w = floor(rho * 65536) limited to [1, 2^24] (NaN -> 1): a fixed-point density, so that
+// the sums are integers and do not depend on the order of accumulation (reading R10 carried over);
+// field == NULL: w = 1, which is O5.  Offsets from the root cell are unwrapped on periodic axes only.
+// sx = (256 xr + 128 + floor(256 Sx / W)) mod Px with Sx = sum(w dx), W = sum(w); cx = xr + 0.5 + Sx / W.
+// size = number of cells (the weights do not enter min_size).
+int32_t orc_centroids_g(int32_t Lx, int32_t Ly, int per_x, int per_y, const int32_t* ccl, const float* field,
+                        int32_t min_size, double* cx, double* cy, int32_t* sx, int32_t* sy,
+                        int32_t* size, int32_t* root, int32_t cap) {
+    const size_t n = (size_t)Lx * Ly;
+    const i64 Px = 256 * (i64)Lx, Py = 256 * (i64)Ly;
+    std::vector<i64> cnt(n, 0), W(n, 0), Sx(n, 0), Sy(n, 0);
+    for (size_t i = 0; i < n; ++i) {
+        const int32_t r = ccl[i];
+        if (r < 0) continue;
+        i64 dx = (i64)(i % Lx) - r % Lx, dy = (i64)(i / Lx) - r / Lx;
+        if (per_x) { if (2 * dx >= Lx) dx -= Lx; else if (2 * dx < -(i64)Lx) dx += Lx; }
+        if (per_y) { if (2 * dy >= Ly) dy -= Ly; else if (2 * dy < -(i64)Ly) dy += Ly; }
+        i64 w = 1;
+        if (field) {
+            const double s = (double)field[i] * 65536.0;      // exact: a power-of-two scale
+            w = s >= 16777216.0 ? 16777216 : (s >= 1.0 ? (i64)s : 1);   // NaN fails both tests -> 1
+        }
+        cnt[r] += 1; W[r] += w; Sx[r] += w * dx; Sy[r] += w * dy;
+    }
+    auto floor_div = [](__int128 a, __int128 b) { return a >= 0 ? a / b : -((-a + b - 1) / b); };
+    int32_t K = 0;
+    for (size_t r = 0; r < n; ++r) {
+        if (cnt[r] == 0 || cnt[r] < min_size) continue;
+        if (K < cap) {
+            const i64 xr = (i64)(r % Lx), yr = (i64)(r / Lx);
+            const i64 fx = (i64)floor_div((__int128)256 * Sx[r], W[r]), fy = (i64)floor_div((__int128)256 * Sy[r], W[r]);
+            sx[K] = (int32_t)((((256 * xr + 128 + fx) % Px) + Px) % Px);
+            sy[K] = (int32_t)((((256 * yr + 128 + fy) % Py) + Py) % Py);
+            double ux = (double)xr + 0.5 + (double)Sx[r] / (double)W[r];
+            double uy = (double)yr + 0.5 + (double)Sy[r] / (double)W[r];
+            if (ux < 0) ux += Lx; else if (ux >= Lx) ux -= Lx;
+            if (uy < 0) uy += Ly; else if (uy >= Ly) uy -= Ly;
+            cx[K] = ux; cy[K] = uy;
+            size[K] = (int32_t)cnt[r];
+            root[K] = (int32_t)r;
+        }
+        ++K;
+    }
+    return K;
+}
+
+// O6 on the general geometry.
+void orc_match_g(int32_t Lx, int32_t Ly, int per_x, int per_y, const int32_t* px, const int32_t* py,
+                 int32_t n_prev, const int32_t* nx, const int32_t* ny, int32_t n_now, int32_t radius_fp,
+                 int32_t* p2n, int32_t* n2p) {
+    const i64 Px = 256 * (i64)Lx, Py = 256 * (i64)Ly, r2 = (i64)radius_fp * radius_fp;
+    auto d2 = [&](i64 ax, i64 ay, i64 bx, i64 by) {
+        const i64 dx = axis_dist(ax, bx, Px, per_x), dy = axis_dist(ay, by, Py, per_y);
+        return dx * dx + dy * dy;
+    };
+    std::vector<int32_t> bp(n_now, -1), bn(n_prev, -1);
+    for (int32_t j = 0; j < n_now; ++j) {
+        i64 best = INT64_MAX;
+        for (int32_t i = 0; i < n_prev; ++i) {
+            const i64 d = d2(nx[j], ny[j], px[i], py[i]);
+            if (d < best) { best = d; bp[j] = i; }
+        }
+        if (best > r2) bp[j] = -1;
+    }
+    for (int32_t i = 0; i < n_prev; ++i) {
+        i64 best = INT64_MAX;
+        for (int32_t j = 0; j < n_now; ++j) {
+            const i64 d = d2(px[i], py[i], nx[j], ny[j]);
+            if (d < best) { best = d; bn[i] = j; }
+        }
+        if (best > r2) bn[i] = -1;
+    }
+    for (int32_t i = 0; i < n_prev; ++i) p2n[i] = (bn[i] >= 0 && bp[bn[i]] == i) ? bn[i] : -1;
+    for (int32_t j = 0; j < n_now; ++j) n2p[j] = (bp[j] >= 0 && bn[bp[j]] == j) ? bp[j] : -1;
+}
+
+// Bubble-size histogram: hist[b] = number of bubbles with size in
+// [b*bin_width, (b+1)*bin_width); the last bin also takes every larger bubble.
+void orc_size_histogram(const int32_t* size, int32_t K, int32_t bin_width, int32_t n_bins, int64_t* hist) {
+    for (int32_t b = 0; b < n_bins; ++b) hist[b] = 0;
+    for (int32_t k = 0; k < K; ++k) {
+        i64 b = size[k] / bin_width;
+        if (b >= n_bins) b = n_bins - 1;
+        if (b >= 0) hist[b] += 1;
+    }
+}
+
+// Bulk / boundary edges: for every edge (i, j) of an ascending unique list over n
+// vertices, the number of neighbours i and j share - "two: the edge is in the bulk; only one: on the
+// boundary".  Keys with a label >= n take no part and get -1.
+void orc_edge_commons(const u64* edges, i64 n_edges, int32_t n, int32_t* commons) {
+    std::vector<std::set<int32_t>> row(n);
+    for (i64 k = 0; k < n_edges; ++k) {
+        const int32_t i = (int32_t)(edges[k] >> 32), j = (int32_t)(edges[k] & 0xffffffffu);
+        if (i < n && j < n) { row[i].insert(j); row[j].insert(i); }
+    }
+    for (i64 k = 0; k < n_edges; ++k) {
+        const int32_t i = (int32_t)(edges[k] >> 32), j = (int32_t)(edges[k] & 0xffffffffu);
+        if (i >= n || j >= n) { commons[k] = -1; continue; }
+        int32_t c = 0;
+        for (int32_t v : row[i]) c += (int32_t)row[j].count(v);
+        commons[k] = c;
+    }
+}
+
 int orc_num_threads(int threads) { return resolve_threads(threads); }
 
 }  // extern "C"
