@@ -48,6 +48,15 @@ typedef enum {
  * de-duplicated) edge keys before sorting; 0 selects a default (max(2^20, 16*max_sites), never
  * more than the hard worst case 2*L*L).  Allocates device memory on the CURRENT device. */
 int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys);
+/* The paper's own geometry: an Lx x Ly lattice (§IV: 2048 x 1024),
+ * each axis periodic (1) or closed by walls (0; beyond the domain boundary there are no
+ * neighbours).  Cell (x, y) has linear index y*Lx + x; label and field images are Ly rows of Lx entries; site
+ * coordinates lie in [0, 256 Lx) x [0, 256 Ly).  On a walled axis distances are plain differences and nothing
+ * wraps, in every call on this context (labels, edges, bubbles, centres, matching).  vor_create(L) is
+ * vor_create_geom(L, L, 1, 1).  2 <= Lx, Ly <= 2^22 (2^21 on a walled axis).  The labelling kernels treat a
+ * walled axis as a window of a periodic lattice twice as long, where the minimum image is the plain distance. */
+int vor_create_geom(vor_ctx** out, int32_t Lx, int32_t Ly, int32_t periodic_x, int32_t periodic_y,
+                    int32_t max_sites, int64_t max_raw_keys);
 int vor_destroy(vor_ctx* ctx);
 
 /* Text of the last failure on this context (ctx-owned storage; never free it). */
@@ -111,6 +120,15 @@ int vor_build_cells_dev(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, 
  * exact integer arithmetic, ties to the smallest index.  Uses the cell list of the last
  * vor_build_cells on this context (none -> VOR_ESTATE).  Writes d_labels[L*L]. */
 int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream);
+/* The same for the strip of rows [y0, y0 + n_rows) of the lattice only (y0 + n_rows <= Ly): writes n_rows * Lx
+ * labels.  One rank of a row-strip decomposition labels its rows plus the first row of the next strip
+ * (PAPER.md:304 multi-GPU as future work) - no halo exchange. */
+int vor_label_rows(vor_ctx* ctx, int32_t y0, int32_t n_rows, int32_t* d_labels, void* stream);
+/* Obstacles (§III.B.1): sites where d_mask[i] != 0 take the fixed colour `colour` (the paper's
+ * MAXLINK, any value >= the number of sites) instead of a label; d_mask and d_labels hold n_rows * Lx entries.
+ * Pass the same colour as `exclude` to vor_edges_image: such sites take part in no edge. */
+int vor_paint_obstacles(vor_ctx* ctx, const uint8_t* d_mask, int32_t colour, int32_t* d_labels, int32_t n_rows,
+                        void* stream);
 
 /* ---- a3+a4: site adjacency (digital Delaunay edge set; PAPER.md:121 adjacency matrix,
  * PAPER.md:207 compress by sort+unique).  Rule (R6): every 4-connected label
@@ -127,6 +145,14 @@ int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t 
  * Offsets are clamped to cap; cap must be < 2^32.  d_row_ptr may be NULL (= vor_edges). */
 int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
                    int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream);
+
+/* General form of vor_edges_rows.  The image has n_rows rows of Lx labels: the whole domain (n_rows = Ly,
+ * wrap_y = the context's periodicity in y) or a strip of consecutive rows (wrap_y = 0: nothing is adjacent
+ * across its first and last row; the last row of a strip is the first row of the next one, so that the union
+ * of the strips' lists is the lattice's list).  The x axis wraps as the context says.  exclude >= 0: pairs
+ * with that label on either side are not edges (obstacle colour); -1: none.  d_row_ptr may be NULL. */
+int vor_edges_image(vor_ctx* ctx, const int32_t* d_labels, int32_t n_rows, int32_t wrap_y, int32_t exclude,
+                    uint64_t* d_edges, int64_t cap, int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream);
 
 /* ---- a5: frame-to-frame comparison (§III.B.3 translation + comparison;
  * PAPER.md:223 appearing/disappearing bubbles excluded; §III.B.4 "breaking" = in
@@ -199,11 +225,23 @@ int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
                   uint64_t* d_couples, int32_t* d_class, int32_t* d_common_prev, int32_t* d_common_now,
                   uint64_t* d_partner, int64_t cap, int64_t* d_n_couples, void* stream);
 
+/* ---- bulk and boundary edges (§III.B.4: "if two connected points share two neighbours,
+ * then the edge is in the bulk; if two connected points share only one neighbour, then the edge is on the
+ * boundary").  d_commons[k] = number of neighbours the two end points of edge k share in the ascending unique
+ * list d_edges (device count clamped to cap_edges < 2^31; labels < n_labels, keys with a larger label get -1).
+ * On a torus every edge of a triangulation is a bulk edge; walls and obstacles create boundary edges. */
+int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int64_t* d_n_edges, int64_t cap_edges,
+                     int32_t n_labels, int32_t* d_commons, void* stream);
+
 /* ---- a6: bubble identification (§III.A: threshold -> two-valued variable ->
  * cluster labelling).  mask = above ? field > thr : field < thr (strict; NaN -> background).
  * 4-connected periodic components; d_ccl[c] = smallest linear index in c's component, or -1. */
 int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr, int above,
                         int32_t* d_ccl, void* stream);
+/* The same with connectivity 4 (above) or 8: cells touching at a corner belong to one bubble - "moving along
+ * the directions of the Lattice Boltzmann model" (D2Q9). */
+int field_threshold_ccl_conn(vor_ctx* ctx, const float* d_field, float thr, int above, int32_t connectivity,
+                             int32_t* d_ccl, void* stream);
 
 /* ---- a7: bubble sizes and centres of mass (§III.A: count the lattice points
  * of each bubble; sum the coordinates and divide by the size).  Unweighted, periodic unwrap
@@ -213,6 +251,19 @@ int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr, int above
 int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_size,
                     double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
                     int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp, void* stream);
+
+/* Density-weighted centres of mass (§II: z* = sum(y rho) / sum(rho)).  d_field[Lx*Ly] is the
+ * density; the weight of a cell is the fixed-point value floor(rho * 65536) limited to [1, 2^24] (NaN -> 1), so
+ * that the sums stay integers and the result does not depend on the order of the atomic additions.  size is
+ * still the number of cells (min_size applies to it); d_field == NULL is field_centroids. */
+int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, const float* d_field, int32_t min_size,
+                             double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
+                             int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp, void* stream);
+/* Bubble-size histogram ("characterize them according to their size"):
+ * d_hist[b] = number of bubbles among the first min(*d_n_comp, cap) entries of d_size whose size lies in
+ * [b * bin_width, (b + 1) * bin_width); the last of the n_bins bins also takes every larger bubble. */
+int field_size_histogram(vor_ctx* ctx, const int32_t* d_size, const int32_t* d_n_comp, int32_t cap,
+                         int32_t bin_width, int32_t n_bins, int64_t* d_hist, void* stream);
 
 /* ---- a8: isomorphism Phi P->N "by simply comparing the two sets of centers of mass"
  * (§III.B.3); unmatched = appeared / disappeared.  Mutual nearest

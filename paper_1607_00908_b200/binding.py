@@ -22,6 +22,7 @@ _STATUS = {0: "VOR_OK", -1: "VOR_EINVAL", -2: "VOR_ECAPACITY", -3: "VOR_ECUDA", 
 _P = C.c_void_p
 SIGNATURES = {
     "vor_create": (C.c_int, [C.POINTER(_P), C.c_int32, C.c_int32, C.c_int64]),
+    "vor_create_geom": (C.c_int, [C.POINTER(_P), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int64]),
     "vor_destroy": (C.c_int, [_P]),
     "vor_last_error": (C.c_char_p, [_P]),
     "vor_sync_status": (C.c_int, [_P, _P]),
@@ -34,6 +35,13 @@ SIGNATURES = {
     "vor_build_cells": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
     "vor_build_cells_dev": (C.c_int, [_P, _P, _P, _P, C.c_int32, C.c_int32, _P]),
     "vor_label": (C.c_int, [_P, _P, _P]),
+    "vor_label_rows": (C.c_int, [_P, C.c_int32, C.c_int32, _P, _P]),
+    "vor_paint_obstacles": (C.c_int, [_P, _P, C.c_int32, _P, C.c_int32, _P]),
+    "vor_edges_image": (C.c_int, [_P, _P, C.c_int32, C.c_int32, C.c_int32, _P, C.c_int64, _P, _P, _P]),
+    "vor_edge_commons": (C.c_int, [_P, _P, _P, C.c_int64, C.c_int32, _P, _P]),
+    "field_threshold_ccl_conn": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, _P, _P]),
+    "field_centroids_weighted": (C.c_int, [_P, _P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
+    "field_size_histogram": (C.c_int, [_P, _P, _P, C.c_int32, C.c_int32, C.c_int32, _P, _P]),
     "vor_edges": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P]),
     "vor_edges_rows": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P, _P]),
     "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
@@ -101,18 +109,28 @@ def _stream():
 class Vor:
     """One libvor context on the current CUDA device.  Methods carry the C names."""
 
-    def __init__(self, L: int, max_sites: int, max_raw_keys: int = 0):
+    def __init__(self, L: int, max_sites: int, max_raw_keys: int = 0, Ly: int | None = None,
+                 periodic: tuple = (1, 1)):
+        """L x L periodic lattice (vor_create), or with Ly / periodic given: L x Ly cells, each axis periodic
+        (1) or walled (0) (vor_create_geom)."""
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise RuntimeError("libvor needs a CUDA device; there is no CPU fallback")
         torch.cuda.init()
         torch.zeros(1, device="cuda")        # make sure the primary context exists
         h = C.c_void_p()
-        rc = self.lib.vor_create(C.byref(h), L, max_sites, max_raw_keys)
+        if Ly is None and tuple(periodic) == (1, 1):
+            rc = self.lib.vor_create(C.byref(h), L, max_sites, max_raw_keys)
+        else:
+            rc = self.lib.vor_create_geom(C.byref(h), L, L if Ly is None else Ly, int(periodic[0]), int(periodic[1]),
+                                          max_sites, max_raw_keys)
         if rc != VOR_OK:
             raise VorError(rc, "vor_create failed")
         self.h = h
-        self.L = L
+        self.L = self.Lx = L
+        self.Ly = L if Ly is None else Ly
+        self.cells = self.Lx * self.Ly
+        self.periodic = (int(periodic[0]), int(periodic[1]))
         self.max_sites = max_sites
 
     def close(self):
@@ -177,18 +195,40 @@ class Vor:
                                                  _ptr(n_sites, torch.int32), cap, n_hint, _stream()))
 
     def vor_label(self, labels):
-        assert labels.numel() == self.L * self.L
+        assert labels.numel() == self.cells
         self._check(self.lib.vor_label(self.h, _ptr(labels, torch.int32), _stream()))
+
+    def vor_label_rows(self, y0: int, n_rows: int, labels):
+        assert labels.numel() == n_rows * self.Lx
+        self._check(self.lib.vor_label_rows(self.h, y0, n_rows, _ptr(labels, torch.int32), _stream()))
+
+    def vor_paint_obstacles(self, mask, colour: int, labels):
+        """mask: uint8 tensor, labels: int32 tensor of the same size (whole rows of Lx cells)."""
+        assert mask.numel() == labels.numel() and labels.numel() % self.Lx == 0
+        self._check(self.lib.vor_paint_obstacles(self.h, _ptr(mask, torch.uint8), colour, _ptr(labels, torch.int32),
+                                                 labels.numel() // self.Lx, _stream()))
+
+    def vor_edges_image(self, labels, wrap_y: bool, exclude: int, edges, n_edges, row_ptr=None):
+        """labels: whole rows of Lx cells (the domain or a strip); exclude: obstacle colour or -1."""
+        assert labels.numel() % self.Lx == 0 and n_edges.numel() >= 1
+        self._check(self.lib.vor_edges_image(self.h, _ptr(labels, torch.int32), labels.numel() // self.Lx,
+                                             1 if wrap_y else 0, exclude, _ptr(edges, torch.int64), edges.numel(),
+                                             _ptr(n_edges, torch.int64), _ptr(row_ptr, torch.int32), _stream()))
+
+    def vor_edge_commons(self, edges, n_edges, n_labels: int, commons):
+        assert commons.numel() >= edges.numel()
+        self._check(self.lib.vor_edge_commons(self.h, _ptr(edges, torch.int64), _ptr(n_edges, torch.int64),
+                                              edges.numel(), n_labels, _ptr(commons, torch.int32), _stream()))
 
     def vor_edges(self, labels, edges, n_edges):
         """edges: int64/uint64 tensor viewed as packed keys; n_edges: int64[1] device scalar."""
-        assert labels.numel() == self.L * self.L and n_edges.numel() >= 1
+        assert labels.numel() == self.cells and n_edges.numel() >= 1
         self._check(self.lib.vor_edges(self.h, _ptr(labels, torch.int32), _ptr(edges, torch.int64),
                                        edges.numel(), _ptr(n_edges, torch.int64), _stream()))
 
     def vor_edges_rows(self, labels, edges, n_edges, row_ptr):
         """As vor_edges, plus row_ptr: int32 tensor (viewed as uint32) of n_rows + 1 row offsets."""
-        assert labels.numel() == self.L * self.L and n_edges.numel() >= 1
+        assert labels.numel() == self.cells and n_edges.numel() >= 1
         self._check(self.lib.vor_edges_rows(self.h, _ptr(labels, torch.int32), _ptr(edges, torch.int64),
                                             edges.numel(), _ptr(n_edges, torch.int64),
                                             _ptr(row_ptr, torch.int32), _stream()))
@@ -238,9 +278,26 @@ class Vor:
 
     # ---- field path
     def field_threshold_ccl(self, field, thr: float, above: bool, ccl):
-        assert field.numel() == self.L * self.L == ccl.numel()
+        assert field.numel() == self.cells == ccl.numel()
         self._check(self.lib.field_threshold_ccl(self.h, _ptr(field, torch.float32), C.c_float(thr),
                                                  1 if above else 0, _ptr(ccl, torch.int32), _stream()))
+
+    def field_threshold_ccl_conn(self, field, thr: float, above: bool, connectivity: int, ccl):
+        assert field.numel() == self.cells == ccl.numel()
+        self._check(self.lib.field_threshold_ccl_conn(self.h, _ptr(field, torch.float32), C.c_float(thr),
+                                                      1 if above else 0, connectivity, _ptr(ccl, torch.int32), _stream()))
+
+    def field_centroids_weighted(self, ccl, field, min_size: int, cx, cy, sx, sy, size, root, n_comp):
+        cap = min(t.numel() for t in (cx, cy, sx, sy, size, root))
+        assert field is None or field.numel() == self.cells
+        self._check(self.lib.field_centroids_weighted(
+            self.h, _ptr(ccl, torch.int32), _ptr(field, torch.float32), min_size, _ptr(cx, torch.float64),
+            _ptr(cy, torch.float64), _ptr(sx, torch.int32), _ptr(sy, torch.int32), _ptr(size, torch.int32),
+            _ptr(root, torch.int32), cap, _ptr(n_comp, torch.int32), _stream()))
+
+    def field_size_histogram(self, size, n_comp, bin_width: int, hist):
+        self._check(self.lib.field_size_histogram(self.h, _ptr(size, torch.int32), _ptr(n_comp, torch.int32),
+                                                  size.numel(), bin_width, hist.numel(), _ptr(hist, torch.int64), _stream()))
 
     def field_centroids(self, ccl, min_size: int, cx, cy, sx, sy, size, root, n_comp):
         cap = min(t.numel() for t in (cx, cy, sx, sy, size, root))
@@ -292,13 +349,13 @@ class Vor:
 
     # ---- field-driven frames
     def field_frame_device(self, field, thr: float, above: bool, min_size: int, radius_fp: int):
-        assert field.numel() == self.L * self.L
+        assert field.numel() == self.cells
         self._check(self.lib.field_frame_device(self.h, _ptr(field, torch.float32), C.c_float(thr),
                                                 1 if above else 0, min_size, radius_fp, _stream()))
 
     def field_frame_submit(self, h_field, thr: float, above: bool, min_size: int, radius_fp: int):
         """h_field: HOST float32 numpy array (L*L, C order); keep it alive and unchanged until collected."""
-        assert h_field.size == self.L * self.L and h_field.dtype.name == "float32" and h_field.flags.c_contiguous
+        assert h_field.size == self.cells and h_field.dtype.name == "float32" and h_field.flags.c_contiguous
         self._check(self.lib.field_frame_submit(self.h, h_field.ctypes.data_as(_P), C.c_float(thr),
                                                 1 if above else 0, min_size, radius_fp, _stream()))
 

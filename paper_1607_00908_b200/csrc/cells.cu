@@ -1,8 +1,8 @@
 // a1 — counting-sort cell list of the sites (BASELINE.json north_star; the paper itself loops over
-// all centres).  Buckets are nb x nb squares of width w fixed-point units with
-// w * nb == P exactly, so that bucket arithmetic wraps consistently on the torus.
+// all centres).  Buckets are squares of width w fixed-point units, nbx x nby of them with
+// w * nbx == Px and w * nby == Py exactly, so that bucket arithmetic wraps consistently on the torus.
 //
-// Layout: d_bucket_start[nb*nb + 1] (exclusive prefix), d_sorted[n] = int4(x, y, original index,
+// Layout: d_bucket_start[nbx*nby + 1] (exclusive prefix), d_sorted[n] = int4(x, y, original index,
 // bucket) in bucket order.  Order inside a bucket is arbitrary (atomic cursors); the label kernel
 // never depends on it because ties are resolved by the original index explicitly.
 #include <math.h>
@@ -125,26 +125,36 @@ __global__ void scatter_sites_kernel(const int32_t* __restrict__ sx, const int32
 // n_hint sizes the buckets (about one site per bucket)
 static int build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
                        const int32_t* d_n_dev, int32_t n_hint, cudaStream_t stream) {
-    // buckets per side: the divisor of P nearest (in ratio) to sqrt(n / occupancy), bucket >= 2 cells
-    const double target = sqrt((double)n_hint * 100.0 / (double)ctx->bucket_occ_x100);
-    int64_t lo = (int64_t)target, hi = (int64_t)target + 1;
-    if (lo < 1) lo = 1;
-    if (lo > ctx->nb_max) lo = ctx->nb_max;
-    while (lo > 1 && ctx->P % lo != 0) --lo;
-    while (hi <= ctx->nb_max && ctx->P % hi != 0) ++hi;
-    int64_t nb = lo;
-    if (hi <= ctx->nb_max && (double)hi / target < target / (double)lo) nb = hi;
-    ctx->nb = (int32_t)nb;
-    ctx->w = (int32_t)(ctx->P / nb);
+    // bucket width w: the common divisor of Px and Py nearest (in ratio) to the width at which a bucket of
+    // the DOMAIN holds `occupancy` sites on average; at least 2 cells, at most 4096 buckets per axis
+    const double target = FP_ONE * sqrt((double)ctx->Lx * ctx->Ly * (double)ctx->bucket_occ_x100 / (100.0 * (double)n_hint));
+    const int64_t g = ctx->w_gcd;
+    int64_t best = 0;
+    auto consider = [&](int64_t w) {
+        if (w < ctx->w_min) return;
+        const double r = w > target ? w / target : target / w;
+        if (best == 0) { best = w; return; }
+        const double rb = best > target ? best / target : target / best;
+        if (r < rb || (r == rb && w < best)) best = w;
+    };
+    for (int64_t d = 1; d * d <= g; ++d) {
+        if (g % d) continue;
+        consider(d);
+        consider(g / d);
+    }
+    if (best == 0) best = g;
+    ctx->w = (int32_t)best;
+    ctx->nbx = (int32_t)(ctx->Px / best);
+    ctx->nby = (int32_t)(ctx->Py / best);
     ctx->n_sites = n_sites;
     ctx->n_hint = n_hint;
     ctx->d_n_dev = d_n_dev;
-    const int64_t nbuckets = nb * nb;
+    const int64_t nbuckets = (int64_t)ctx->nbx * ctx->nby;
 
     VOR_CUDA(cudaMemsetAsync(ctx->d_bucket_fill, 0, nbuckets * sizeof(int32_t), stream));
     const int threads = 256;
     const int grid = (n_sites + threads - 1) / threads;
-    VOR_LAUNCH(count_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nb,
+    VOR_LAUNCH(count_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nbx,
                ctx->d_bucket_fill);
     const int tiles = (int)((nbuckets + kScanTile - 1) / kScanTile);
     VOR_LAUNCH(scan_reduce_kernel, tiles, kScanThreads, 0, stream, ctx->d_bucket_fill, nbuckets,
@@ -152,7 +162,7 @@ static int build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, i
     VOR_LAUNCH(scan_partials_kernel, 1, kScanThreads, 0, stream, ctx->d_scan_part, tiles);
     VOR_LAUNCH(scan_apply_kernel, tiles, kScanThreads, 0, stream, ctx->d_bucket_fill, nbuckets,
                ctx->d_scan_part, ctx->d_bucket_start);
-    VOR_LAUNCH(scatter_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nb,
+    VOR_LAUNCH(scatter_sites_kernel, grid, threads, 0, stream, d_sx, d_sy, n_sites, d_n_dev, ctx->w, ctx->nbx,
                ctx->d_bucket_start, ctx->d_bucket_fill, ctx->d_sorted);
     return VOR_OK;
 }

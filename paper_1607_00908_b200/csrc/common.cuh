@@ -31,8 +31,13 @@ enum : int {
 };
 
 struct vor_ctx {
-    int32_t L;
-    int64_t P;                 // 256 * L
+    int32_t Lx, Ly;            // the domain: label / field images are Ly rows of Lx cells
+    int32_t per_x, per_y;      // 1 = periodic axis, 0 = closed by walls
+    // the LABELLING lattice: the domain itself on a periodic axis, twice the domain on a walled axis (inside
+    // the domain the minimum image on the doubled period is the plain distance, so the periodic kernels label
+    // a walled domain as a window of it); the cell list covers this lattice
+    int32_t FLx, FLy;
+    int64_t Px, Py;            // 256 * FLx, 256 * FLy
     int32_t max_sites;
     int64_t max_raw_keys;
     int device;
@@ -44,14 +49,15 @@ struct vor_ctx {
     int64_t label_fast_off;        // 1 = skip the quadrant fast path (testing)
 
     // ---- cell list (a1)
-    int32_t nb_max;            // allocation bound for buckets per side
-    int32_t nb;                // buckets per side of the last build (0 = none)
-    int32_t w;                 // bucket width in fixed-point units, w * nb == P
+    int64_t nbuckets_max;      // allocation bound for nbx * nby
+    int64_t w_min, w_gcd;      // smallest admissible bucket width; gcd(Px, Py) (every width divides it)
+    int32_t nbx, nby;          // buckets per axis of the last build (0 = none)
+    int32_t w;                 // bucket width in fixed-point units, w * nbx == Px, w * nby == Py
     int32_t n_sites;           // of the last build (vor_build_cells_dev: the upper bound `cap`)
     int32_t n_hint;            // expected number of sites (kernel selection, bucket and halo sizes only)
     const int32_t* d_n_dev;    // vor_build_cells_dev: the exact number lives on the device; else NULL
-    int32_t* d_bucket_start;   // [nb_max^2 + 1]
-    int32_t* d_bucket_fill;    // [nb_max^2]  (scatter cursors)
+    int32_t* d_bucket_start;   // [nbuckets_max + 1]
+    int32_t* d_bucket_fill;    // [nbuckets_max]  (scatter cursors)
     int4* d_sorted;            // [max_sites]  (x, y, original index, bucket)
     int32_t* d_scan_part;      // scratch for device scans
 
@@ -75,8 +81,8 @@ struct vor_ctx {
     int64_t* d_blk_count;      // [2 * kMaxCoopBlocks] per-block counts for compactions
 
     // ---- fused label -> edge path (vor_frame_*): compact border columns of the 32-cell tile columns
-    int32_t* d_fu_cols;        // [2][L / 32][L]: left, then right border column of every tile column
-    int32_t* d_fu_dirty;       // [(L / 32)^2] tiles whose pairs the labelling kernel could not extract itself
+    int32_t* d_fu_cols;        // [2][Lx / 32][Ly]: left, then right border column of every tile column
+    int32_t* d_fu_dirty;       // [(Lx / 32) * (Ly / 32)] tiles whose pairs the labelling kernel could not extract itself
     int64_t fuse;              // option: 1 = vor_frame_* labels and extracts the pairs in one kernel
 
     // ---- row-by-row diff: membership mask per row [dr_rows], then the per-block counts
@@ -93,7 +99,7 @@ struct vor_ctx {
     int64_t* d_tr_counts;      // [4]
 
     // ---- field path (a6..a8)
-    int32_t* d_rank;           // [L*L] root -> component rank
+    int32_t* d_rank;           // [Lx*Ly] root -> component rank
     int64_t* d_acc;            // [3 * max_comp] n, Sx, Sy
     int32_t* d_comp_root;      // [max_comp]
     int32_t max_comp;
@@ -105,7 +111,7 @@ struct vor_ctx {
     // ---- frame pipeline (e2e)
     int32_t* d_fr_sx;
     int32_t* d_fr_sy;
-    int32_t* d_fr_labels;      // [L*L]
+    int32_t* d_fr_labels;      // [Lx*Ly]
     uint64_t* d_fr_edges[2];   // ping-pong prev / now
     int64_t* d_fr_nedges[2];
     uint32_t* d_fr_rowptr[2];  // [max_sites + 1] row offsets of the two lists (vor_edges_rows)
@@ -120,7 +126,7 @@ struct vor_ctx {
     int fr_cur;                // index of the "now" buffer of the last frame; -1 = none
     int fr_have_prev;
     // field-driven frames (field_frame_*): bubble image, two generations of bubble arrays, the isomorphism
-    int32_t* d_ff_ccl;         // [L*L]
+    int32_t* d_ff_ccl;         // [Lx*Ly]
     double* d_ff_cxy[2];       // [2 * max_sites] cx, cy
     int32_t* d_ff_comp[2];     // [4 * max_sites + 4] sx, sy, size, root, then the device count
     int32_t* d_ff_maps;        // [2 * max_sites] p2n, n2p

@@ -15,15 +15,25 @@ cudaError_t dmalloc(T** p, size_t n) {
 extern "C" {
 
 int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys) {
+    return vor_create_geom(out, L, L, 1, 1, max_sites, max_raw_keys);
+}
+
+int vor_create_geom(vor_ctx** out, int32_t Lx, int32_t Ly, int32_t periodic_x, int32_t periodic_y,
+                    int32_t max_sites, int64_t max_raw_keys) {
     if (!out) return VOR_EINVAL;
     *out = nullptr;
-    if (L < 2 || L > (1 << 22) || max_sites < 1) return VOR_EINVAL;
+    const int32_t lim_x = periodic_x ? (1 << 22) : (1 << 21), lim_y = periodic_y ? (1 << 22) : (1 << 21);
+    if (Lx < 2 || Ly < 2 || Lx > lim_x || Ly > lim_y || max_sites < 1) return VOR_EINVAL;
     vor_ctx* ctx = (vor_ctx*)calloc(1, sizeof(vor_ctx));
     if (!ctx) return VOR_ECUDA;
-    ctx->L = L;
-    ctx->P = (int64_t)FP_ONE * L;
+    ctx->Lx = Lx; ctx->Ly = Ly;
+    ctx->per_x = periodic_x != 0; ctx->per_y = periodic_y != 0;
+    ctx->FLx = ctx->per_x ? Lx : 2 * Lx;
+    ctx->FLy = ctx->per_y ? Ly : 2 * Ly;
+    ctx->Px = (int64_t)FP_ONE * ctx->FLx;
+    ctx->Py = (int64_t)FP_ONE * ctx->FLy;
     ctx->max_sites = max_sites;
-    const int64_t worst = 2 * (int64_t)L * L;
+    const int64_t worst = 2 * (int64_t)Lx * Ly;
     if (max_raw_keys <= 0) {
         max_raw_keys = 16 * (int64_t)max_sites;
         if (max_raw_keys < (1 << 20)) max_raw_keys = 1 << 20;
@@ -45,8 +55,23 @@ int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys
         return VOR_ECUDA;
     }
 
-    ctx->nb_max = L / 2 < 1 ? 1 : (L / 2 > 4096 ? 4096 : L / 2);
-    const size_t nbuckets = (size_t)ctx->nb_max * ctx->nb_max;
+    // bucket widths are common divisors of Px and Py; the smallest one vor_build_cells may pick is at least
+    // 2 cells wide and gives at most 4096 buckets per axis - or, when no divisor does, the largest divisor
+    {
+        int64_t g = ctx->Px, t = ctx->Py;
+        while (t) { const int64_t r = g % t; g = t; t = r; }
+        int64_t wmin = g;
+        for (int64_t d = 1; d * d <= g; ++d) {
+            if (g % d) continue;
+            const int64_t c[2] = {d, g / d};
+            for (int k = 0; k < 2; ++k)
+                if (c[k] >= 2 * FP_ONE && ctx->Px / c[k] <= 4096 && ctx->Py / c[k] <= 4096 && c[k] < wmin) wmin = c[k];
+        }
+        ctx->w_min = wmin;
+        ctx->w_gcd = g;
+        ctx->nbuckets_max = (ctx->Px / wmin) * (ctx->Py / wmin);
+    }
+    const size_t nbuckets = (size_t)ctx->nbuckets_max;
     bool ok = true;
     ok = ok && dmalloc(&ctx->d_bucket_start, nbuckets + 1) == cudaSuccess;
     ok = ok && dmalloc(&ctx->d_bucket_fill, nbuckets) == cudaSuccess;

@@ -42,6 +42,7 @@ template <int kSlots = kHashSlots>
 __device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned long long* table,
                                             const RowSet& rs) {
     const uint32_t lo = min(a, b), hi = max(a, b);
+    if (lo == rs.exclude || hi == rs.exclude) return;       // obstacle colour: no edge
     const unsigned long long key = ((unsigned long long)lo << 32) | hi;
     uint32_t h = hash_key(lo, hi) & (kSlots - 1);
     for (int probe = 0; probe < kMaxProbe; ++probe) {
@@ -137,8 +138,11 @@ __device__ __forceinline__ void hash_flush(const unsigned long long* table, cons
     }
 }
 
+// The image has H rows of W labels (W % 4 == 0); wrap_x / wrap_y: the last column / row is adjacent to the
+// first one (periodic axis); otherwise the image ends there (a wall, or the end of a strip of rows).
 __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int32_t* __restrict__ labels,
-                                                                      int32_t L, const RowSet rs) {
+                                                                      int32_t W, int32_t H, int wrap_x, int wrap_y,
+                                                                      const RowSet rs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     StreamShared& sh = *reinterpret_cast<StreamShared*>(smem_raw);
     for (int i = threadIdx.x; i < kHashSlots; i += kStrThreads) sh.table[i] = kEmptyKey;
@@ -149,7 +153,7 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
     const int32_t xbase = (blockIdx.x * kStrWarpsX + (wid % kStrWarpsX)) * kStripCols;
     const int32_t x0 = xbase + 4 * lane;
     const int32_t ybeg = (blockIdx.y * kStrWarpsY + (wid / kStrWarpsX)) * kStripRows;
-    const int32_t yend = min(ybeg + kStripRows, L);
+    const int32_t yend = min(ybeg + kStripRows, H);
     RecQueue& rq = sh.rec[wid];
     int32_t* __restrict__ mq = sh.multi[wid];
     int rn = 0, mn = 0;                            // warp-uniform queue fills
@@ -203,19 +207,21 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
         }
     };
 
-    if (xbase < L && ybeg < L) {                   // warp-uniform
-        const bool active = x0 < L;                // L % 4 == 0: a lane's 4 columns are all in or all out
-        const bool halo = active && (lane == 31 || x0 + 4 >= L);   // right neighbour not in the next lane
+    if (xbase < W && ybeg < H) {                   // warp-uniform
+        const bool active = x0 < W;                // W % 4 == 0: a lane's 4 columns are all in or all out
+        const bool halo = active && (lane == 31 || x0 + 4 >= W);   // right neighbour not in the next lane
         const uint32_t amask = active ? 0xffffffffu : 0u;
         // inactive lanes (ragged last strip) read a valid address and never report anything
         const uint32_t col = active ? x0 : xbase;
-        const uint32_t colh = halo ? (x0 + 4 >= L ? 0 : x0 + 4) : xbase;
-        const int32_t* __restrict__ p = labels + (int64_t)ybeg * L + col;      // load cursors: main, halo
-        const int32_t* __restrict__ ph = labels + (int64_t)ybeg * L + colh;
+        // beyond the last column: column 0 (periodic) or the last column itself (wall: no pair)
+        const uint32_t colh = halo ? (x0 + 4 >= W ? (wrap_x ? 0 : x0 + 3) : x0 + 4) : xbase;
+        const int32_t* __restrict__ p = labels + (int64_t)ybeg * W + col;      // load cursors: main, halo
+        const int32_t* __restrict__ ph = labels + (int64_t)ybeg * W + colh;
         int4 pc;
         int32_t prr3;
         {
-            const int32_t* __restrict__ up = labels + (int64_t)(ybeg == 0 ? L - 1 : ybeg - 1) * L;   // wrapped
+            // above row 0: the last row (periodic) or row 0 itself (no pair)
+            const int32_t* __restrict__ up = labels + (int64_t)(ybeg == 0 ? (wrap_y ? H - 1 : 0) : ybeg - 1) * W;
             pc = __ldg(reinterpret_cast<const int4*>(up + col));
             const int32_t hup = __ldg(up + colh);
             const int32_t nb = __shfl_down_sync(full, pc.x, 1);
@@ -231,7 +237,7 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
         for (int j = 0; j < kPf; ++j) {
             buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
             hb[j] = __ldg(ph);
-            const int32_t step = ahead > 0 ? L : 0;
+            const int32_t step = ahead > 0 ? W : 0;
             p += step; ph += step;
             --ahead;
         }
@@ -243,7 +249,7 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
                 const int32_t hc = hb[j];
                 buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
                 hb[j] = __ldg(ph);
-                const int32_t step = ahead > 0 ? L : 0;
+                const int32_t step = ahead > 0 ? W : 0;
                 p += step; ph += step;
                 --ahead;
                 const int32_t nb = __shfl_down_sync(full, c.x, 1);
@@ -284,7 +290,8 @@ constexpr int kEmitRowsPerWarp = 16;
 constexpr int kEmitRows = (kEmitThreads / 32) * kEmitRowsPerWarp;   // 128
 
 __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t* __restrict__ labels,
-                                                                  int32_t L, const RowSet rs) {
+                                                                  int32_t W, int32_t H, int wrap_x, int wrap_y,
+                                                                  const RowSet rs) {
     __shared__ unsigned long long table[kHashSlots];
     __shared__ uint2 queue[kEmitThreads / 32][kQueueCap];
     __shared__ int32_t scan[kEmitThreads / 32 + 1];
@@ -297,30 +304,31 @@ __global__ void __launch_bounds__(kEmitThreads) edges_emit_kernel(const int32_t*
     const int32_t ybeg = blockIdx.y * kEmitRows + wid * kEmitRowsPerWarp;
     uint2* __restrict__ q = queue[wid];
     int qn = 0;                                    // warp-uniform queue fill
-    if (ybeg < L) {
+    if (ybeg < H) {
         auto load_row = [&](const int32_t* __restrict__ row, int32_t* v) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) v[k] = x0 + k < L ? __ldg(row + x0 + k) : 0;
+            for (int k = 0; k < 4; ++k) v[k] = x0 + k < W ? __ldg(row + x0 + k) : 0;
         };
         int32_t c[4], nx[4];
-        load_row(labels + (int64_t)ybeg * L, c);
-        const int32_t yend = min(ybeg + kEmitRowsPerWarp, L);
+        load_row(labels + (int64_t)ybeg * W, c);
+        const int32_t yend = min(ybeg + kEmitRowsPerWarp, H);
         for (int32_t y = ybeg; y < yend; ++y) {
-            const int32_t* __restrict__ row = labels + (int64_t)y * L;
-            load_row(labels + (int64_t)(y + 1 == L ? 0 : y + 1) * L, nx);
+            const int32_t* __restrict__ row = labels + (int64_t)y * W;
+            // below the last row: row 0 (periodic) or the row itself (no pair)
+            load_row(labels + (int64_t)(y + 1 == H ? (wrap_y ? 0 : y) : y + 1) * W, nx);
             // right neighbours: next column, next lane's first column, or column 0 through the wrap
             int32_t rr[4] = {c[1], c[2], c[3], __shfl_down_sync(full, c[0], 1)};
-            if (lane == 31 && x0 + 4 < L) rr[3] = __ldg(row + x0 + 4);
-            if (x0 + 4 >= L && x0 < L) {
+            if (lane == 31 && x0 + 4 < W) rr[3] = __ldg(row + x0 + 4);
+            if (x0 + 4 >= W && x0 < W) {
                 const int32_t first = __ldg(row);
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
-                    if (x0 + k + 1 >= L) rr[k] = first;
+                    if (x0 + k + 1 >= W) rr[k] = wrap_x ? first : c[k];
             }
             unsigned bits = 0;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const bool valid = x0 + k < L;
+                const bool valid = x0 + k < W;
                 bits |= (unsigned)(valid && c[k] != rr[k]) << k;
                 bits |= (unsigned)(valid && c[k] != nx[k]) << (4 + k);
             }
@@ -825,30 +833,31 @@ constexpr int kTailSlots = 2048;
 __global__ void __launch_bounds__(kSeamThreads) fused_seam_kernel(const int32_t* __restrict__ labels,
                                                                   const int32_t* __restrict__ col_left,
                                                                   const int32_t* __restrict__ col_right,
-                                                                  int32_t L, const RowSet rs) {
+                                                                  int32_t Lx, int32_t Ly, const RowSet rs) {
     __shared__ unsigned long long table[kSeamSlots];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const int32_t nt = L >> 5, c = blockIdx.y;
+    const int32_t nt = Lx >> 5, c = blockIdx.y;
     for (int i = threadIdx.x; i < kSeamSlots; i += kSeamThreads) table[i] = kEmptyKey;
     __syncthreads();
     const int32_t* __restrict__ pa;
     const int32_t* __restrict__ pb;
+    const int32_t len = c < nt ? Ly : Lx;              // positions along this seam line
     if (c < nt) {
-        pa = col_right + (int64_t)c * L;
-        pb = col_left + (int64_t)(c + 1 == nt ? 0 : c + 1) * L;
+        pa = col_right + (int64_t)c * Ly;
+        pb = col_left + (int64_t)(c + 1 == nt ? 0 : c + 1) * Ly;
     } else {
         const int32_t y = 32 * (c - nt) + 31;
-        pa = labels + (int64_t)y * L;
-        pb = labels + (int64_t)(y + 1 == L ? 0 : y + 1) * L;
+        pa = labels + (int64_t)y * Lx;
+        pb = labels + (int64_t)(y + 1 == Ly ? 0 : y + 1) * Lx;
     }
     const int32_t i0 = blockIdx.x * (kSeamThreads * kSeamPer) + threadIdx.x;
     int32_t a[kSeamPer], b[kSeamPer];
 #pragma unroll
-    for (int k = 0; k < kSeamPer; ++k) {           // L % 32 == 0: whole warps are in or out of range
+    for (int k = 0; k < kSeamPer; ++k) {           // Lx, Ly % 32 == 0: whole warps are in or out of range
         const int32_t i = i0 + k * kSeamThreads;
-        a[k] = i < L ? __ldcs(pa + i) : 0;
-        b[k] = i < L ? __ldcs(pb + i) : 0;
+        a[k] = i < len ? __ldcs(pa + i) : 0;
+        b[k] = i < len ? __ldcs(pb + i) : 0;
     }
 #pragma unroll
     for (int k = 0; k < kSeamPer; ++k) {
@@ -891,7 +900,7 @@ __global__ void __launch_bounds__(kTailThreads) fused_dirty_kernel(const int32_t
                                                                    int32_t L, const RowSet rs) {
     __shared__ unsigned long long table[kTailSlots];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int32_t nt = L >> 5, n = *dirty_count;
+    const int32_t nt = L >> 5, n = *dirty_count;           // L = Lx: tiles per tile row, label pitch
     if ((int32_t)(blockIdx.x * (kTailThreads / 32)) >= n) return;
     for (int i = threadIdx.x; i < kTailSlots; i += kTailThreads) table[i] = kEmptyKey;
     __syncthreads();
@@ -970,17 +979,19 @@ RowSet vor_row_set(vor_ctx* ctx) {
     rs.raw_cap = ctx->max_raw_keys;
     rs.n_raw = (unsigned long long*)&ctx->d_n_raw[3];
     rs.flags = ctx->d_flags;
+    rs.exclude = 0xffffffffu;
     return rs;
 }
 
 int vor_edges_fused_tail(vor_ctx* ctx, const int32_t* d_labels, const RowSet& rs, cudaStream_t stream) {
-    const int32_t L = ctx->L, nt = L / 32;
+    const int32_t Lx = ctx->Lx, Ly = ctx->Ly, ntx = Lx / 32, nty = Ly / 32;
     const int32_t* col_left = ctx->d_fu_cols;
-    const int32_t* col_right = ctx->d_fu_cols + (size_t)nt * L;
-    const dim3 grid((L + kSeamThreads * kSeamPer - 1) / (kSeamThreads * kSeamPer), 2 * nt);
-    VOR_LAUNCH(fused_seam_kernel, grid, kSeamThreads, 0, stream, d_labels, col_left, col_right, L, rs);
+    const int32_t* col_right = ctx->d_fu_cols + (size_t)ntx * Ly;
+    const int32_t longest = Lx > Ly ? Lx : Ly;
+    const dim3 grid((longest + kSeamThreads * kSeamPer - 1) / (kSeamThreads * kSeamPer), ntx + nty);
+    VOR_LAUNCH(fused_seam_kernel, grid, kSeamThreads, 0, stream, d_labels, col_left, col_right, Lx, Ly, rs);
     VOR_LAUNCH(fused_dirty_kernel, 4 * ctx->num_sms, kTailThreads, 0, stream, d_labels, ctx->d_fu_dirty,
-               (const int32_t*)&ctx->d_n_raw[4], L, rs);
+               (const int32_t*)&ctx->d_n_raw[4], Lx, rs);
     return VOR_OK;
 }
 
@@ -995,6 +1006,30 @@ int vor_edges_finish(vor_ctx* ctx, const RowSet& rs, uint64_t* d_edges, int64_t 
     return VOR_OK;
 }
 
+// labels: n_rows rows of Lx labels; wrap_y: the last row is adjacent to the first one
+static int edges_image(vor_ctx* ctx, const int32_t* d_labels, int32_t n_rows, int wrap_y, int32_t exclude,
+                       uint64_t* d_edges, int64_t cap, int64_t* d_n_edges, uint32_t* d_row_ptr,
+                       cudaStream_t stream) {
+    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 8 * sizeof(int64_t), stream));
+    const int32_t W = ctx->Lx, H = n_rows;
+    RowSet rs = vor_row_set(ctx);
+    if (exclude >= 0) rs.exclude = (uint32_t)exclude;
+    const bool vec = (W % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
+    if (vec) {
+        static_assert(sizeof(StreamShared) <= 27 * 1024, "eight CTAs per SM");
+        VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)sizeof(StreamShared)));
+        dim3 grid((W + kStrWarpsX * kStripCols - 1) / (kStrWarpsX * kStripCols),
+                  (H + kStrWarpsY * kStripRows - 1) / (kStrWarpsY * kStripRows));
+        VOR_LAUNCH(edges_stream_kernel, grid, kStrThreads, sizeof(StreamShared), stream, d_labels, W, H,
+                   ctx->per_x, wrap_y, rs);
+    } else {
+        dim3 grid((W + kEmitCols - 1) / kEmitCols, (H + kEmitRows - 1) / kEmitRows);
+        VOR_LAUNCH(edges_emit_kernel, grid, kEmitThreads, 0, stream, d_labels, W, H, ctx->per_x, wrap_y, rs);
+    }
+    return vor_edges_finish(ctx, rs, d_edges, cap, d_n_edges, d_row_ptr, true, stream);
+}
+
 extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
                          int64_t* d_n_edges, void* stream_) {
     return vor_edges_rows(ctx, d_labels, d_edges, cap, d_n_edges, nullptr, stream_);
@@ -1003,25 +1038,40 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
 extern "C" int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
                               int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    return vor_edges_image(ctx, d_labels, ctx->Ly, ctx->per_y, -1, d_edges, cap, d_n_edges, d_row_ptr, stream_);
+}
+
+extern "C" int vor_edges_image(vor_ctx* ctx, const int32_t* d_labels, int32_t n_rows, int32_t wrap_y,
+                               int32_t exclude, uint64_t* d_edges, int64_t cap, int64_t* d_n_edges,
+                               uint32_t* d_row_ptr, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
     if (!d_labels || !d_edges || !d_n_edges || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_edges: null pointer or negative capacity");
+    if (n_rows < 1) return vor_fail(ctx, VOR_EINVAL, "vor_edges_image: n_rows must be >= 1");
     if (d_row_ptr && cap > 0xffffffffll)
         return vor_fail(ctx, VOR_EINVAL, "vor_edges_rows: row offsets are 32-bit, cap must be < 2^32");
-    cudaStream_t stream = (cudaStream_t)stream_;
-    VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 8 * sizeof(int64_t), stream));
-    const int32_t L = ctx->L;
-    RowSet rs = vor_row_set(ctx);
-    const bool vec = (L % 4 == 0) && (((uintptr_t)d_labels & 15) == 0) && !ctx->edges_generic;
-    if (vec) {
-        static_assert(sizeof(StreamShared) <= 27 * 1024, "eight CTAs per SM");
-        VOR_CUDA(cudaFuncSetAttribute(edges_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(StreamShared)));
-        dim3 grid((L + kStrWarpsX * kStripCols - 1) / (kStrWarpsX * kStripCols),
-                  (L + kStrWarpsY * kStripRows - 1) / (kStrWarpsY * kStripRows));
-        VOR_LAUNCH(edges_stream_kernel, grid, kStrThreads, sizeof(StreamShared), stream, d_labels, L, rs);
-    } else {
-        dim3 grid((L + kEmitCols - 1) / kEmitCols, (L + kEmitRows - 1) / kEmitRows);
-        VOR_LAUNCH(edges_emit_kernel, grid, kEmitThreads, 0, stream, d_labels, L, rs);
-    }
-    return vor_edges_finish(ctx, rs, d_edges, cap, d_n_edges, d_row_ptr, true, stream);
+    return edges_image(ctx, d_labels, n_rows, wrap_y != 0, exclude, d_edges, cap, d_n_edges, d_row_ptr,
+                       (cudaStream_t)stream_);
+}
+
+// Obstacle sites take a fixed large colour instead of a bubble's label (§III.B.1: "a
+// supplementary binary field which takes the value 1 on those sites which are considered obstacles ... we can
+// set their colour to be a fixed large number, MAXLINK").  Pass the same colour as `exclude` to vor_edges_image.
+namespace {
+__global__ void paint_obstacles_kernel(const uint8_t* __restrict__ mask, int32_t colour, int64_t n,
+                                       int32_t* __restrict__ labels) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        if (mask[i]) labels[i] = colour;
+}
+}  // namespace
+
+extern "C" int vor_paint_obstacles(vor_ctx* ctx, const uint8_t* d_mask, int32_t colour, int32_t* d_labels,
+                                   int32_t n_rows, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_mask || !d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_paint_obstacles: null pointer");
+    if (colour < 0 || n_rows < 1) return vor_fail(ctx, VOR_EINVAL, "vor_paint_obstacles: colour >= 0, n_rows >= 1");
+    const int64_t n = (int64_t)ctx->Lx * n_rows;
+    const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
+    VOR_LAUNCH(paint_obstacles_kernel, grid, 256, 0, (cudaStream_t)stream_, d_mask, colour, n, d_labels);
+    return VOR_OK;
 }

@@ -531,3 +531,47 @@ extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t
                d_common_prev, d_common_now, d_partner);
     return VOR_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// Bulk / boundary edges: "if two connected points share two neighbours, then the edge is in
+// the bulk; if two connected points share only one neighbour, then the edge is on the boundary".  One thread
+// per edge intersects the two sorted adjacency rows built as for vor_t1_events.
+namespace {
+
+__global__ void edge_commons_kernel(T1Graph g, int32_t n, int32_t* __restrict__ commons) {
+    const int64_t m = t1_len(g);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t i, j, c2[2];
+        commons[k] = t1_edge(g, k, n, &i, &j) ? t1_common(g, i, j, c2) : -1;
+    }
+}
+
+}  // namespace
+
+extern "C" int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int64_t* d_n_edges, int64_t cap_edges,
+                                int32_t n_labels, int32_t* d_commons, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_edges || !d_n_edges || !d_commons) return vor_fail(ctx, VOR_EINVAL, "vor_edge_commons: null pointer");
+    if (n_labels < 1 || cap_edges < 0 || 2 * cap_edges >= ((int64_t)1 << 32))
+        return vor_fail(ctx, VOR_EINVAL, "vor_edge_commons: n_labels >= 1, 0 <= cap_edges < 2^31");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t n1 = (size_t)n_labels + 1;
+    uint32_t *deg, *off, *adj_u, *adj_s;
+    int rc;
+    const size_t n_adj = 2 * (size_t)cap_edges + 1;
+    if ((rc = t1_scratch(ctx, 0, 2 * n1 * sizeof(uint32_t), (void**)&deg)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 1, 2 * n1 * sizeof(uint32_t), (void**)&off)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 2, n_adj * sizeof(uint32_t), (void**)&adj_u)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 3, n_adj * sizeof(uint32_t), (void**)&adj_s)) != VOR_OK) return rc;
+    T1Graph g{d_edges, d_n_edges, cap_edges, deg, off, adj_u, adj_s};
+    VOR_CUDA(cudaMemsetAsync(deg, 0, n1 * sizeof(uint32_t), stream));
+    const int grid = 4 * ctx->num_sms;
+    const dim3 one(grid, 1);                                 // blockIdx.y == 0: the kernels read only the first graph
+    VOR_LAUNCH(t1_degree_kernel, one, 256, 0, stream, g, g, n_labels);
+    VOR_LAUNCH(t1_scan_sum_kernel, one, kEvThreads, 0, stream, g, g, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_scan_apply_kernel, one, kEvThreads, 0, stream, g, g, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_fill_kernel, one, 256, 0, stream, g, g, n_labels);
+    VOR_LAUNCH(t1_rank_kernel, one, 256, 0, stream, g, g, n_labels);
+    VOR_LAUNCH(edge_commons_kernel, 4 * grid, 256, 0, stream, g, n_labels, d_commons);
+    return VOR_OK;
+}

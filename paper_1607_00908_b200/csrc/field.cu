@@ -56,8 +56,9 @@ __device__ __forceinline__ void suf_union(int32_t* parent, int32_t a, int32_t b)
     }
 }
 
+// conn8: cells that touch at a corner are connected too (the D2Q9 directions)
 __global__ void __launch_bounds__(kTileThreads) ccl_tile_kernel(const float* __restrict__ field, float thr,
-                                                                int above, int32_t L,
+                                                                int above, int32_t Lx, int32_t Ly, int conn8,
                                                                 int32_t* __restrict__ parent) {
     __shared__ int32_t lab[kTileH * kTileW];
     const int32_t X0 = blockIdx.x * kTileW, Y0 = blockIdx.y * kTileH;
@@ -70,8 +71,8 @@ __global__ void __launch_bounds__(kTileThreads) ccl_tile_kernel(const float* __r
     for (int j = 0; j < kTileRows; ++j) {
         const int32_t y = Y0 + ly0 + j;
         bool m = false;
-        if (x < L && y < L) {
-            const float v = __ldcs(field + (int64_t)y * L + x);
+        if (x < Lx && y < Ly) {
+            const float v = __ldcs(field + (int64_t)y * Lx + x);
             m = above ? (v > thr) : (v < thr);             // NaN compares false both ways
         }
         const unsigned bits = __ballot_sync(0xffffffffu, m);
@@ -87,52 +88,71 @@ __global__ void __launch_bounds__(kTileThreads) ccl_tile_kernel(const float* __r
         const int li = (ly0 + j) * kTileW + lx;
         if (lab[li] < 0) continue;
         if (lx == 32 && lab[li - 1] >= 0) suf_union(lab, li, li - 1);
-        if (ly0 + j + 1 < kTileH && lab[li + kTileW] >= 0 &&
-            (lx == 0 || lab[li - 1] < 0 || lab[li + kTileW - 1] < 0))
-            suf_union(lab, li, li + kTileW);
+        if (ly0 + j + 1 < kTileH) {
+            if (lab[li + kTileW] >= 0) {
+                if (lx == 0 || lab[li - 1] < 0 || lab[li + kTileW - 1] < 0) suf_union(lab, li, li + kTileW);
+            } else if (conn8) {
+                // the cell below is background: a diagonal neighbour is reachable only through the corner
+                // (were the cell below set, it would join both through its own row)
+                if (lx + 1 < kTileW && lab[li + kTileW + 1] >= 0) suf_union(lab, li, li + kTileW + 1);
+                if (lx > 0 && lab[li + kTileW - 1] >= 0) suf_union(lab, li, li + kTileW - 1);
+            }
+        }
     }
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kTileRows; ++j) {
         const int32_t y = Y0 + ly0 + j;
-        if (x >= L || y >= L) continue;
+        if (x >= Lx || y >= Ly) continue;
         const int li = (ly0 + j) * kTileW + lx;
         int32_t out = -1;
         if (lab[li] >= 0) {
             const int32_t r = suf_find(lab, li);
-            out = (int32_t)((int64_t)(Y0 + r / kTileW) * L + X0 + (r & (kTileW - 1)));
+            out = (int32_t)((int64_t)(Y0 + r / kTileW) * Lx + X0 + (r & (kTileW - 1)));
         }
-        parent[(int64_t)y * L + x] = out;
+        parent[(int64_t)y * Lx + x] = out;
     }
 }
 
 // Seam stage: the pairs that straddle tile borders (including the periodic wrap and the ragged last
-// tiles) are united in the global array.  Items [0, ntx * L): vertical seam lines (cell | right
-// neighbour); items [ntx * L, (ntx + nty) * L): horizontal seam lines (cell | down neighbour).
-__global__ void ccl_seam_kernel(int32_t L, int32_t ntx, int32_t nty, int32_t* __restrict__ parent) {
-    const int64_t n = (int64_t)(ntx + nty) * L;
+// tiles) are united in the global array.  Items [0, ntx * Ly): vertical seam lines (cell | right
+// neighbour, with conn8 also its upper and lower right neighbour); items [ntx * Ly, ntx * Ly + nty * Lx):
+// horizontal seam lines (cell | lower neighbour, with conn8 also lower left and lower right).  A neighbour
+// beyond a walled axis does not exist.
+__global__ void ccl_seam_kernel(int32_t Lx, int32_t Ly, int per_x, int per_y, int conn8, int32_t ntx, int32_t nty,
+                                int32_t* __restrict__ parent) {
+    const int64_t nv = (int64_t)ntx * Ly, n = nv + (int64_t)nty * Lx;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        int64_t a, b;
-        if (i < (int64_t)ntx * L) {
-            const int32_t k = (int32_t)(i / L), y = (int32_t)(i % L);
-            const int32_t x = min((k + 1) * kTileW - 1, L - 1);
-            a = (int64_t)y * L + x;
-            b = (int64_t)y * L + (x + 1 == L ? 0 : x + 1);
+        int32_t x, y, dx0, dy0;                          // the cell and the direction of its plain neighbour
+        if (i < nv) {
+            y = (int32_t)(i % Ly);
+            x = min((int32_t)(i / Ly + 1) * kTileW - 1, Lx - 1);
+            dx0 = 1; dy0 = 0;
         } else {
-            const int64_t r = i - (int64_t)ntx * L;
-            const int32_t k = (int32_t)(r / L), x = (int32_t)(r % L);
-            const int32_t y = min((k + 1) * kTileH - 1, L - 1);
-            a = (int64_t)y * L + x;
-            b = (int64_t)(y + 1 == L ? 0 : y + 1) * L + x;
+            const int64_t r = i - nv;
+            x = (int32_t)(r % Lx);
+            y = min((int32_t)(r / Lx + 1) * kTileH - 1, Ly - 1);
+            dx0 = 0; dy0 = 1;
         }
-        if (a != b && parent[a] >= 0 && parent[b] >= 0) uf_union(parent, (int32_t)a, (int32_t)b);
+        const int64_t a = (int64_t)y * Lx + x;
+        if (parent[a] < 0) continue;
+        for (int t = -1; t <= 1; ++t) {
+            if (t != 0 && !conn8) continue;
+            int32_t u = x + (dx0 ? 1 : t), v = y + (dy0 ? 1 : t);
+            if (u < 0 || u >= Lx) { if (!per_x) continue; u = u < 0 ? u + Lx : u - Lx; }
+            if (v < 0 || v >= Ly) { if (!per_y) continue; v = v < 0 ? v + Ly : v - Ly; }
+            const int64_t b = (int64_t)v * Lx + u;
+            if (a != b && parent[b] >= 0) uf_union(parent, (int32_t)a, (int32_t)b);
+        }
     }
 }
 
 __global__ void ccl_flatten_kernel(int64_t n, int32_t* __restrict__ parent) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        if (parent[i] < 0) continue;
-        parent[i] = uf_find(parent, (int32_t)i);
+        const int32_t q = parent[i];
+        if (q < 0) continue;
+        const int32_t r = uf_find(parent, q);
+        if (r != q) parent[i] = r;                          // most cells already point at their root
     }
 }
 
@@ -258,19 +278,34 @@ struct RootSink {
     int32_t max_comp;
     int32_t* n_raw;
     int32_t* flags;
+    long long* acc;            // accumulators of the components found are zeroed here (no full memset)
+    int n_acc;
     __device__ void total(int64_t t) const {
         *n_raw = (int32_t)(t < max_comp ? t : max_comp);
         if (t > max_comp) atomicOr(flags, FLAG_COMP_CAP);
     }
     __device__ void put(int64_t pos, int64_t i) const {
         rank[i] = pos < max_comp ? (int32_t)pos : -1;
-        if (pos < max_comp) comp_root[pos] = (int32_t)i;
+        if (pos < max_comp) {
+            comp_root[pos] = (int32_t)i;
+            for (int a = 0; a < n_acc; ++a) acc[(size_t)a * max_comp + pos] = 0;
+        }
     }
 };
 
-__global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const int32_t* __restrict__ rank,
-                                  int32_t L, FastDiv fd, unsigned long long* __restrict__ acc, int32_t max_comp) {
-    const int64_t n = (int64_t)L * L;
+// fixed-point density of a cell (the centre of mass weighted by rho): floor(rho * 65536)
+// limited to [1, 2^24]; NaN -> 1.  Integer weights keep the sums independent of the accumulation order.
+__device__ __forceinline__ int64_t cell_weight(float rho) {
+    const float s = rho * 65536.0f;                             // exact: a power-of-two scale
+    return s >= 16777216.0f ? 16777216 : (s >= 1.0f ? (int64_t)s : 1);
+}
+
+// acc: [0] cells, [1] sum of w dx, [2] sum of w dy, [3] sum of w (weighted only), each max_comp entries
+template <bool kWeighted>
+__global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const float* __restrict__ field,
+                                  const int32_t* __restrict__ rank, int32_t Lx, int32_t Ly, int per_x, int per_y,
+                                  FastDiv fd, unsigned long long* __restrict__ acc, int32_t max_comp) {
+    const int64_t n = (int64_t)Lx * Ly;
     const int64_t nround = (n + 31) / 32 * 32;     // keep warps converged for the warp collectives
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (int64_t)gridDim.x * blockDim.x) {
         const int32_t r = i < n ? ccl[i] : -1;
@@ -278,20 +313,52 @@ __global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const int32_t
         const bool uniform = __all_sync(0xffffffffu, r == __shfl_sync(0xffffffffu, r, 0));
         const unsigned peers = uniform ? 0xffffffffu : __match_any_sync(0xffffffffu, r);
         if (r < 0) continue;                        // whole peer group leaves together
-        const int32_t y = (int32_t)fd.div((uint32_t)i), x = (int32_t)i - y * L;
-        const int32_t yr = (int32_t)fd.div((uint32_t)r), xr = r - yr * L;
+        const int32_t y = (int32_t)fd.div((uint32_t)i), x = (int32_t)i - y * Lx;
+        const int32_t yr = (int32_t)fd.div((uint32_t)r), xr = r - yr * Lx;
         int32_t dx = x - xr;
-        if (2 * dx >= L) dx -= L; else if (2 * dx < -L) dx += L;
+        if (per_x) { if (2 * dx >= Lx) dx -= Lx; else if (2 * dx < -Lx) dx += Lx; }
         int32_t dy = y - yr;
-        if (2 * dy >= L) dy -= L; else if (2 * dy < -L) dy += L;
-        const int32_t sx = __reduce_add_sync(peers, dx);
-        const int32_t sy = __reduce_add_sync(peers, dy);
-        if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
-            const int32_t k = rank[r];
-            if (k >= 0) {
-                atomicAdd(&acc[k], (unsigned long long)__popc(peers));
-                atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)(long long)sx);
-                atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)(long long)sy);
+        if (per_y) { if (2 * dy >= Ly) dy -= Ly; else if (2 * dy < -Ly) dy += Ly; }
+        const bool leader = (int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31);
+        if constexpr (!kWeighted) {
+            const int32_t sx = __reduce_add_sync(peers, dx);
+            const int32_t sy = __reduce_add_sync(peers, dy);
+            if (leader) {
+                const int32_t k = rank[r];
+                if (k >= 0) {
+                    atomicAdd(&acc[k], (unsigned long long)__popc(peers));
+                    atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)(long long)sx);
+                    atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)(long long)sy);
+                }
+            }
+        } else {
+            // 64-bit sums over the peer group: w <= 2^24, |dx| < 2^22, 32 peers
+            const int64_t w = cell_weight(field[i]);
+            int64_t sw = w, sx = w * dx, sy = w * dy;
+            if (uniform) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    sw += __shfl_xor_sync(0xffffffffu, sw, o);
+                    sx += __shfl_xor_sync(0xffffffffu, sx, o);
+                    sy += __shfl_xor_sync(0xffffffffu, sy, o);
+                }
+                if (leader) {
+                    const int32_t k = rank[r];
+                    if (k >= 0) {
+                        atomicAdd(&acc[k], 32ull);
+                        atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)sx);
+                        atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)sy);
+                        atomicAdd(&acc[3 * (size_t)max_comp + k], (unsigned long long)sw);
+                    }
+                }
+            } else {                                  // a bubble's edge: every cell adds its own terms
+                const int32_t k = rank[r];
+                if (k >= 0) {
+                    if (leader) atomicAdd(&acc[k], (unsigned long long)__popc(peers));
+                    atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)sx);
+                    atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)sy);
+                    atomicAdd(&acc[3 * (size_t)max_comp + k], (unsigned long long)sw);
+                }
             }
         }
     }
@@ -307,28 +374,29 @@ struct SizePred {
 struct CentroidSink {
     const long long* acc;
     const int32_t* comp_root;
-    int32_t max_comp, L, cap;
+    int32_t max_comp, Lx, Ly, cap, weighted;
     double* cx; double* cy; int32_t* sx; int32_t* sy; int32_t* size; int32_t* root;
     int32_t* n_comp; int32_t* flags;
     __device__ void total(int64_t t) const {
         *n_comp = (int32_t)t;
         if (t > cap) atomicOr(flags, FLAG_COMP_CAP);
     }
-    __device__ static long long floor_div(long long a, long long b) {      // b > 0
-        return a >= 0 ? a / b : -((-a + b - 1) / b);
+    __device__ static long long floor_div(__int128 a, __int128 b) {        // b > 0
+        return (long long)(a >= 0 ? a / b : -((-a + b - 1) / b));
     }
     __device__ void put(int64_t pos, int64_t k) const {
         if (pos >= cap) return;
         const long long m = acc[k], Sx = acc[(size_t)max_comp + k], Sy = acc[2 * (size_t)max_comp + k];
+        const long long W = weighted ? acc[3 * (size_t)max_comp + k] : m;     // total weight
         const int32_t r = comp_root[k];
-        const long long xr = r % L, yr = r / L, P = (long long)FP_ONE * L;
-        const long long fx = floor_div(FP_ONE * Sx, m), fy = floor_div(FP_ONE * Sy, m);
-        sx[pos] = (int32_t)((((FP_ONE * xr + FP_HALF + fx) % P) + P) % P);
-        sy[pos] = (int32_t)((((FP_ONE * yr + FP_HALF + fy) % P) + P) % P);
-        double ux = __dadd_rn(__dadd_rn((double)xr, 0.5), __ddiv_rn((double)Sx, (double)m));
-        double uy = __dadd_rn(__dadd_rn((double)yr, 0.5), __ddiv_rn((double)Sy, (double)m));
-        if (ux < 0) ux += L; else if (ux >= L) ux -= L;
-        if (uy < 0) uy += L; else if (uy >= L) uy -= L;
+        const long long xr = r % Lx, yr = r / Lx, Px = (long long)FP_ONE * Lx, Py = (long long)FP_ONE * Ly;
+        const long long fx = floor_div((__int128)FP_ONE * Sx, W), fy = floor_div((__int128)FP_ONE * Sy, W);
+        sx[pos] = (int32_t)((((FP_ONE * xr + FP_HALF + fx) % Px) + Px) % Px);
+        sy[pos] = (int32_t)((((FP_ONE * yr + FP_HALF + fy) % Py) + Py) % Py);
+        double ux = __dadd_rn(__dadd_rn((double)xr, 0.5), __ddiv_rn((double)Sx, (double)W));
+        double uy = __dadd_rn(__dadd_rn((double)yr, 0.5), __ddiv_rn((double)Sy, (double)W));
+        if (ux < 0) ux += Lx; else if (ux >= Lx) ux -= Lx;
+        if (uy < 0) uy += Ly; else if (uy >= Ly) uy -= Ly;
         cx[pos] = ux; cy[pos] = uy;
         size[pos] = (int32_t)m;
         root[pos] = r;
@@ -350,6 +418,19 @@ struct MatchGrid {
     int32_t* overflow;         // device flag
 };
 
+// periods of the two axes in fixed point and whether each axis wraps (a walled axis: plain distance)
+struct MatchGeom {
+    long long Px, Py;
+    int per_x, per_y;
+    __device__ __forceinline__ long long d2(long long ax, long long ay, long long vx, long long vy) const {
+        long long dx = ax > vx ? ax - vx : vx - ax;
+        if (per_x && Px - dx < dx) dx = Px - dx;
+        long long dy = ay > vy ? ay - vy : vy - ay;
+        if (per_y && Py - dy < dy) dy = Py - dy;
+        return dx * dx + dy * dy;
+    }
+};
+
 __device__ __forceinline__ int32_t mbucket(int32_t v, long long P, int32_t nbm) {
     return (int32_t)(((long long)v * nbm) / P);
 }
@@ -357,13 +438,13 @@ __device__ __forceinline__ int32_t mbucket(int32_t v, long long P, int32_t nbm) 
 __global__ void match_fill_kernel(const int32_t* __restrict__ px, const int32_t* __restrict__ py,
                                   const int32_t* __restrict__ n_prev_p, const int32_t* __restrict__ nx,
                                   const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
-                                  int32_t cap_prev, int32_t cap_now, long long P, MatchGrid g) {
+                                  int32_t cap_prev, int32_t cap_now, MatchGeom geo, MatchGrid g) {
     const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
     for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_prev + n_now; i += gridDim.x * blockDim.x) {
         const int set = i >= n_prev;
         const int32_t k = set ? i - n_prev : i;
         const int32_t x = set ? nx[k] : px[k], y = set ? ny[k] : py[k];
-        const int32_t b = mbucket(y, P, g.nbm) * g.nbm + mbucket(x, P, g.nbm);
+        const int32_t b = mbucket(y, geo.Py, g.nbm) * g.nbm + mbucket(x, geo.Px, g.nbm);
         const int32_t slot = atomicAdd(&g.cnt[set][b], 1);
         if (slot < kMatchSlots) g.ids[set][(size_t)b * kMatchSlots + slot] = k;
         else *g.overflow = 1;
@@ -374,7 +455,7 @@ __global__ void match_fill_kernel(const int32_t* __restrict__ px, const int32_t*
 __global__ void match_grid_kernel(const int32_t* __restrict__ px, const int32_t* __restrict__ py,
                                   const int32_t* __restrict__ n_prev_p, const int32_t* __restrict__ nx,
                                   const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
-                                  int32_t cap_prev, int32_t cap_now, long long P, long long r2, MatchGrid g,
+                                  int32_t cap_prev, int32_t cap_now, MatchGeom geo, long long r2, MatchGrid g,
                                   int32_t* __restrict__ best) {
     const int32_t n_prev = min(*n_prev_p, cap_prev), n_now = min(*n_now_p, cap_now);
     for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_prev + n_now; i += gridDim.x * blockDim.x) {
@@ -384,22 +465,21 @@ __global__ void match_grid_kernel(const int32_t* __restrict__ px, const int32_t*
         const int32_t* __restrict__ tx = q_is_now ? px : nx;
         const int32_t* __restrict__ ty = q_is_now ? py : ny;
         const long long ax = q_is_now ? nx[q] : px[q], ay = q_is_now ? ny[q] : py[q];
-        const int32_t bx = mbucket((int32_t)ax, P, g.nbm), by = mbucket((int32_t)ay, P, g.nbm);
+        const int32_t bx = mbucket((int32_t)ax, geo.Px, g.nbm), by = mbucket((int32_t)ay, geo.Py, g.nbm);
         long long bd = INT64_MAX;
         int32_t bi = -1;
         const int span = g.nbm >= 3 ? 3 : g.nbm;             // tiny grids: every bucket once
         for (int oy = 0; oy < span; ++oy) {
-            const int32_t cy = g.nbm >= 3 ? (by + oy - 1 + g.nbm) % g.nbm : oy;
+            int32_t cy = g.nbm >= 3 ? by + oy - 1 : oy;      // beyond a walled axis there is no bucket
+            if (cy < 0 || cy >= g.nbm) { if (!geo.per_y) continue; cy = cy < 0 ? cy + g.nbm : cy - g.nbm; }
             for (int ox = 0; ox < span; ++ox) {
-                const int32_t cx = g.nbm >= 3 ? (bx + ox - 1 + g.nbm) % g.nbm : ox;
+                int32_t cx = g.nbm >= 3 ? bx + ox - 1 : ox;
+                if (cx < 0 || cx >= g.nbm) { if (!geo.per_x) continue; cx = cx < 0 ? cx + g.nbm : cx - g.nbm; }
                 const int32_t b = cy * g.nbm + cx;
                 const int32_t c = min(g.cnt[tset][b], kMatchSlots);
                 for (int32_t s = 0; s < c; ++s) {
                     const int32_t t = g.ids[tset][(size_t)b * kMatchSlots + s];
-                    const long long vx = tx[t], vy = ty[t];
-                    long long dx = ax > vx ? ax - vx : vx - ax; dx = dx < P - dx ? dx : P - dx;
-                    long long dy = ay > vy ? ay - vy : vy - ay; dy = dy < P - dy ? dy : P - dy;
-                    const long long d2 = dx * dx + dy * dy;
+                    const long long d2 = geo.d2(ax, ay, tx[t], ty[t]);
                     if (d2 < bd || (d2 == bd && t < bi)) { bd = d2; bi = t; }
                 }
             }
@@ -412,7 +492,7 @@ __global__ void match_grid_kernel(const int32_t* __restrict__ px, const int32_t*
 __global__ void __launch_bounds__(kMatchThreads) match_best_kernel(
         const int32_t* __restrict__ px, const int32_t* __restrict__ py, const int32_t* __restrict__ n_prev_p,
         const int32_t* __restrict__ nx, const int32_t* __restrict__ ny, const int32_t* __restrict__ n_now_p,
-        int32_t cap_prev, int32_t cap_now, int32_t blocks_now, long long P, long long r2,
+        int32_t cap_prev, int32_t cap_now, int32_t blocks_now, MatchGeom geo, long long r2,
         int32_t* __restrict__ best, int32_t* __restrict__ flags, const int32_t* __restrict__ needed) {
     __shared__ int32_t tx[kMatchThreads], ty[kMatchThreads];
     if (blockIdx.x == 0 && threadIdx.x == 0 && (*n_prev_p > cap_prev || *n_now_p > cap_now))
@@ -436,9 +516,7 @@ __global__ void __launch_bounds__(kMatchThreads) match_best_kernel(
         __syncthreads();
         const int32_t lim = min(kMatchThreads, nt - base);
         for (int32_t k = 0; k < lim; ++k) {
-            long long dx = ax > tx[k] ? ax - tx[k] : tx[k] - ax; dx = dx < P - dx ? dx : P - dx;
-            long long dy = ay > ty[k] ? ay - ty[k] : ty[k] - ay; dy = dy < P - dy ? dy : P - dy;
-            const long long d2 = dx * dx + dy * dy;
+            const long long d2 = geo.d2(ax, ay, tx[k], ty[k]);
             if (d2 < bd) { bd = d2; bi = base + k; }
         }
     }
@@ -465,20 +543,44 @@ __global__ void match_combine_kernel(const int32_t* __restrict__ n_prev_p, const
     }
 }
 
+
+
+// ------------------------------------------------------------------------------------ size histogram
+__global__ void size_hist_kernel(const int32_t* __restrict__ size, const int32_t* __restrict__ n_comp, int32_t cap,
+                                 int32_t bin_width, int32_t n_bins, unsigned long long* __restrict__ hist) {
+    const int32_t n = min(*n_comp, cap);
+    for (int32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
+        const int32_t s = size[k];
+        if (s < 0) continue;
+        const int32_t b = min(s / bin_width, n_bins - 1);
+        atomicAdd(&hist[b], 1ull);
+    }
+}
+
 }  // namespace
 
 extern "C" int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr, int above,
                                    int32_t* d_ccl, void* stream_) {
+    return field_threshold_ccl_conn(ctx, d_field, thr, above, 4, d_ccl, stream_);
+}
+
+extern "C" int field_threshold_ccl_conn(vor_ctx* ctx, const float* d_field, float thr, int above,
+                                        int32_t connectivity, int32_t* d_ccl, void* stream_) {
     if (!ctx) return VOR_EINVAL;
     if (!d_field || !d_ccl) return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: null pointer");
+    if (connectivity != 4 && connectivity != 8)
+        return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: connectivity must be 4 or 8");
+    const int64_t n = (int64_t)ctx->Lx * ctx->Ly;
+    if (n > INT32_MAX) return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: Lx * Ly must fit a 32-bit cell index");
     cudaStream_t stream = (cudaStream_t)stream_;
-    const int64_t n = (int64_t)ctx->L * ctx->L;
+    const int conn8 = connectivity == 8;
     const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
-    const int32_t ntx = (ctx->L + kTileW - 1) / kTileW, nty = (ctx->L + kTileH - 1) / kTileH;
-    VOR_LAUNCH(ccl_tile_kernel, dim3(ntx, nty), kTileThreads, 0, stream, d_field, thr, above ? 1 : 0, ctx->L, d_ccl);
-    const int64_t seams = (int64_t)(ntx + nty) * ctx->L;
+    const int32_t ntx = (ctx->Lx + kTileW - 1) / kTileW, nty = (ctx->Ly + kTileH - 1) / kTileH;
+    VOR_LAUNCH(ccl_tile_kernel, dim3(ntx, nty), kTileThreads, 0, stream, d_field, thr, above ? 1 : 0, ctx->Lx, ctx->Ly,
+               conn8, d_ccl);
+    const int64_t seams = (int64_t)ntx * ctx->Ly + (int64_t)nty * ctx->Lx;
     const int sgrid = (int)((seams + 255) / 256 < 8 * kNumSMs ? (seams + 255) / 256 : 8 * kNumSMs);
-    VOR_LAUNCH(ccl_seam_kernel, sgrid, 256, 0, stream, ctx->L, ntx, nty, d_ccl);
+    VOR_LAUNCH(ccl_seam_kernel, sgrid, 256, 0, stream, ctx->Lx, ctx->Ly, ctx->per_x, ctx->per_y, conn8, ntx, nty, d_ccl);
     VOR_LAUNCH(ccl_flatten_kernel, grid, 256, 0, stream, n, d_ccl);
     return VOR_OK;
 }
@@ -487,34 +589,61 @@ extern "C" int field_centroids(vor_ctx* ctx, const int32_t* d_ccl, int32_t min_s
                                double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
                                int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp,
                                void* stream_) {
+    return field_centroids_weighted(ctx, d_ccl, nullptr, min_size, d_cx, d_cy, d_sx, d_sy, d_size, d_root, cap,
+                                    d_n_comp, stream_);
+}
+
+extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, const float* d_field, int32_t min_size,
+                                        double* d_cx, double* d_cy, int32_t* d_sx, int32_t* d_sy,
+                                        int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp,
+                                        void* stream_) {
     if (!ctx) return VOR_EINVAL;
     if (!d_ccl || !d_cx || !d_cy || !d_sx || !d_sy || !d_size || !d_root || !d_n_comp || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "field_centroids: null pointer or negative capacity");
     cudaStream_t stream = (cudaStream_t)stream_;
-    const int64_t n = (int64_t)ctx->L * ctx->L;
+    const int64_t n = (int64_t)ctx->Lx * ctx->Ly;
+    if (n > INT32_MAX) return vor_fail(ctx, VOR_EINVAL, "field_centroids: Lx * Ly must fit a 32-bit cell index");
     if (!ctx->d_rank) {
         int64_t mc = (n + 1) / 2;
         if (mc > (1 << 22)) mc = 1 << 22;
         ctx->max_comp = (int32_t)mc;
         VOR_CUDA(cudaMalloc((void**)&ctx->d_rank, n * sizeof(int32_t)));
-        VOR_CUDA(cudaMalloc((void**)&ctx->d_acc, 3 * (size_t)mc * sizeof(int64_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_acc, 4 * (size_t)mc * sizeof(int64_t)));
         VOR_CUDA(cudaMalloc((void**)&ctx->d_comp_root, (size_t)mc * sizeof(int32_t)));
     }
-    VOR_CUDA(cudaMemsetAsync(ctx->d_acc, 0, 3 * (size_t)ctx->max_comp * sizeof(int64_t), stream));
+    const int weighted = d_field != nullptr;
     RootPred rp{d_ccl, n};
-    RootSink rs{ctx->d_comp_root, ctx->d_rank, ctx->max_comp, &ctx->d_comp_count[0], ctx->d_flags};
+    RootSink rs{ctx->d_comp_root, ctx->d_rank, ctx->max_comp, &ctx->d_comp_count[0], ctx->d_flags,
+                (long long*)ctx->d_acc, weighted ? 4 : 3};
     VOR_LAUNCH(comp_count_kernel<RootPred>, kCompGrid, kCompThreads, 0, stream, rp, ctx->d_blk_count);
     VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kCompGrid, kCompThreads, 0, stream, rp, rs,
                ctx->d_blk_count);
     const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
-    VOR_LAUNCH(accumulate_kernel, grid, 256, 0, stream, d_ccl, ctx->d_rank, ctx->L, make_fastdiv((uint32_t)ctx->L),
-               (unsigned long long*)ctx->d_acc, ctx->max_comp);
+    if (weighted)
+        VOR_LAUNCH(accumulate_kernel<true>, grid, 256, 0, stream, d_ccl, d_field, ctx->d_rank, ctx->Lx, ctx->Ly,
+                   ctx->per_x, ctx->per_y, make_fastdiv((uint32_t)ctx->Lx), (unsigned long long*)ctx->d_acc, ctx->max_comp);
+    else
+        VOR_LAUNCH(accumulate_kernel<false>, grid, 256, 0, stream, d_ccl, d_field, ctx->d_rank, ctx->Lx, ctx->Ly,
+                   ctx->per_x, ctx->per_y, make_fastdiv((uint32_t)ctx->Lx), (unsigned long long*)ctx->d_acc, ctx->max_comp);
     SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
-    CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->L, cap,
+    CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->Lx, ctx->Ly, cap, weighted,
                     d_cx, d_cy, d_sx, d_sy, d_size, d_root, d_n_comp, ctx->d_flags};
     VOR_LAUNCH(comp_count_kernel<SizePred>, kCompGrid, kCompThreads, 0, stream, sp, ctx->d_blk_count);
     VOR_LAUNCH((comp_write_kernel<SizePred, CentroidSink>), kCompGrid, kCompThreads, 0, stream, sp, cs,
                ctx->d_blk_count);
+    return VOR_OK;
+}
+
+extern "C" int field_size_histogram(vor_ctx* ctx, const int32_t* d_size, const int32_t* d_n_comp, int32_t cap,
+                                    int32_t bin_width, int32_t n_bins, int64_t* d_hist, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_size || !d_n_comp || !d_hist) return vor_fail(ctx, VOR_EINVAL, "field_size_histogram: null pointer");
+    if (cap < 0 || bin_width < 1 || n_bins < 1)
+        return vor_fail(ctx, VOR_EINVAL, "field_size_histogram: cap >= 0, bin_width >= 1, n_bins >= 1");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    VOR_CUDA(cudaMemsetAsync(d_hist, 0, (size_t)n_bins * sizeof(int64_t), stream));
+    VOR_LAUNCH(size_hist_kernel, 2 * ctx->num_sms, 256, 0, stream, d_size, d_n_comp, cap, bin_width, n_bins,
+               (unsigned long long*)d_hist);
     return VOR_OK;
 }
 
@@ -537,7 +666,10 @@ extern "C" int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_p
     const int bn = (cap_now + kMatchThreads - 1) / kMatchThreads, bp = (cap_prev + kMatchThreads - 1) / kMatchThreads;
     const long long r2 = (long long)radius_fp * radius_fp;
     // grid path: bucket width P / nbm >= radius
-    int64_t nbm = radius_fp > 0 ? ctx->P / radius_fp : kMatchGrid;
+    // the matching lives on the DOMAIN: periods 256 * Lx, 256 * Ly, a walled axis does not wrap
+    const MatchGeom geo{(long long)FP_ONE * ctx->Lx, (long long)FP_ONE * ctx->Ly, ctx->per_x, ctx->per_y};
+    const long long pmin = geo.Px < geo.Py ? geo.Px : geo.Py;
+    int64_t nbm = radius_fp > 0 ? pmin / radius_fp : kMatchGrid;
     if (nbm > kMatchGrid) nbm = kMatchGrid;
     if (nbm < 1) nbm = 1;
     const size_t cells = (size_t)kMatchGrid * kMatchGrid;
@@ -551,11 +683,11 @@ extern "C" int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_p
     VOR_CUDA(cudaMemsetAsync(ctx->d_mgrid, 0, 2 * cells * sizeof(int32_t), stream));
     VOR_CUDA(cudaMemsetAsync(g.overflow, 0, sizeof(int32_t), stream));
     VOR_LAUNCH(match_fill_kernel, 2 * kNumSMs, 256, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny, d_n_now,
-               cap_prev, cap_now, (long long)ctx->P, g);
+               cap_prev, cap_now, geo, g);
     VOR_LAUNCH(match_grid_kernel, 4 * kNumSMs, 128, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny, d_n_now,
-               cap_prev, cap_now, (long long)ctx->P, r2, g, ctx->d_best);
+               cap_prev, cap_now, geo, r2, g, ctx->d_best);
     VOR_LAUNCH(match_best_kernel, bn + bp, kMatchThreads, 0, stream, d_px, d_py, d_n_prev, d_nx, d_ny,
-               d_n_now, cap_prev, cap_now, bn, (long long)ctx->P, r2,
+               d_n_now, cap_prev, cap_now, bn, geo, r2,
                ctx->d_best, ctx->d_flags, (const int32_t*)g.overflow);
     VOR_LAUNCH(match_combine_kernel, 2 * kNumSMs, 256, 0, stream, d_n_prev, d_n_now, cap_prev, cap_now,
                ctx->d_best, d_p2n, d_n2p);

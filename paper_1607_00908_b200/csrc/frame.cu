@@ -85,7 +85,7 @@ bool is_pinned(const void* p) {
 
 int ensure_frame_buffers(vor_ctx* ctx) {
     if (ctx->d_fr_labels) return VOR_OK;
-    const size_t cells = (size_t)ctx->L * ctx->L;
+    const size_t cells = (size_t)ctx->Lx * ctx->Ly;
     int64_t cap = 4 * (int64_t)ctx->max_sites + 1024;
     if (cap > ctx->max_raw_keys) cap = ctx->max_raw_keys;
     if (cap > 0xffffffffll) cap = 0xffffffffll;            // 32-bit row offsets
@@ -124,7 +124,7 @@ __global__ void gather_field_counts_kernel(const int32_t* __restrict__ n_comp, c
 
 int ensure_field_buffers(vor_ctx* ctx) {
     if (ctx->d_ff_ccl) return VOR_OK;
-    const size_t cells = (size_t)ctx->L * ctx->L, K = (size_t)ctx->max_sites;
+    const size_t cells = (size_t)ctx->Lx * ctx->Ly, K = (size_t)ctx->max_sites;
     VOR_CUDA(cudaMalloc((void**)&ctx->d_ff_ccl, cells * sizeof(int32_t)));
     for (int k = 0; k < 2; ++k) {
         VOR_CUDA(cudaMalloc((void**)&ctx->d_ff_cxy[k], 2 * K * sizeof(double)));
@@ -348,7 +348,7 @@ extern "C" int field_frame_submit(vor_ctx* ctx, const float* h_field, float thr,
         return vor_fail(ctx, VOR_ESTATE, "field_frame_submit: two frames in flight, collect one first");
     cudaStream_t stream = (cudaStream_t)stream_;
     const int s = (int)(ctx->pp_head & 1);
-    const size_t bytes = (size_t)ctx->L * ctx->L * sizeof(float);
+    const size_t bytes = (size_t)ctx->Lx * ctx->Ly * sizeof(float);
     if (!ctx->d_ff_field[s]) VOR_CUDA(cudaMalloc((void**)&ctx->d_ff_field[s], bytes));
     // pinned caller memory is DMA'd directly; pageable memory goes through the driver's staging copy
     VOR_CUDA(cudaMemcpyAsync(ctx->d_ff_field[s], h_field, bytes, cudaMemcpyHostToDevice, ctx->pp_h2d));

@@ -37,10 +37,13 @@
 namespace {
 
 struct LabelParams {
-    int32_t L;
-    int32_t P;                 // 256 * L  (L <= 2^22 -> P <= 2^30)
-    int32_t nb;
+    int32_t Px, Py;            // periods of the labelling lattice in fixed point (<= 2^30)
+    int32_t nbx, nby;          // buckets per axis, w * nbx == Px, w * nby == Py
     int32_t w;
+    // window of the lattice that is labelled: cells [wx0, wx1) x [wy0, wy1), stored row-major with `pitch`
+    // columns starting at the window's first cell (the whole domain, or a strip of rows)
+    int32_t wx0, wy0, wx1, wy1;
+    int32_t pitch;
     int32_t n;                 // number of sites (upper bound if n_dev is given)
     const int32_t* __restrict__ n_dev;        // exact number as a device scalar, or NULL
     const int32_t* __restrict__ bucket_start;
@@ -67,10 +70,10 @@ struct LabelParams {
 // fused path: a label written by the second pass also goes to the compact border columns
 __device__ __forceinline__ void store_label(const LabelParams& p, int32_t* __restrict__ labels, int32_t x,
                                             int32_t y, int32_t v) {
-    labels[(int64_t)y * p.L + x] = v;
-    if (p.col_left) {
-        if ((x & 31) == 0) p.col_left[(int64_t)(x >> 5) * p.L + y] = v;
-        if ((x & 31) == 31) p.col_right[(int64_t)(x >> 5) * p.L + y] = v;
+    labels[(int64_t)(y - p.wy0) * p.pitch + (x - p.wx0)] = v;
+    if (p.col_left) {                                    // fused path: the window is the whole lattice
+        if ((x & 31) == 0) p.col_left[(int64_t)(x >> 5) * p.wy1 + y] = v;
+        if ((x & 31) == 31) p.col_right[(int64_t)(x >> 5) * p.wy1 + y] = v;
     }
 }
 
@@ -95,38 +98,38 @@ __device__ __forceinline__ int32_t pos_mod(int32_t a, int32_t b) {
 }
 
 // ---------------------------------------------------------------- general path (exact, int64)
-__device__ __forceinline__ void consider(const int4 s, int64_t cx, int64_t cy, int64_t P,
+__device__ __forceinline__ void consider(const int4 s, int64_t cx, int64_t cy, int64_t Px, int64_t Py,
                                          int64_t& best, int32_t& besti) {
     int64_t ax = cx > s.x ? cx - s.x : s.x - cx;
-    int64_t dx = ax < P - ax ? ax : P - ax;
+    int64_t dx = ax < Px - ax ? ax : Px - ax;
     int64_t ay = cy > s.y ? cy - s.y : s.y - cy;
-    int64_t dy = ay < P - ay ? ay : P - ay;
+    int64_t dy = ay < Py - ay ? ay : Py - ay;
     int64_t d2 = dx * dx + dy * dy;
     if (d2 < best || (d2 == best && s.z < besti)) { best = d2; besti = s.z; }
 }
 
 __device__ int32_t label_cell_general(const LabelParams& p, int32_t x, int32_t y) {
-    const int64_t P = p.P;
+    const int64_t Px = p.Px, Py = p.Py;
     const int64_t cx = (int64_t)FP_ONE * x + FP_HALF, cy = (int64_t)FP_ONE * y + FP_HALF;
     const int32_t bx = (int32_t)(cx / p.w), by = (int32_t)(cy / p.w);
     int64_t best = INT64_MAX;
     int32_t besti = INT32_MAX;
     for (int32_t r = 0;; ++r) {
-        if (2 * r + 1 >= p.nb) {            // the ring would wrap onto itself: scan everything once
+        if (2 * r + 1 >= min(p.nbx, p.nby)) {   // the ring would wrap onto itself: scan everything once
             best = INT64_MAX; besti = INT32_MAX;
             const int32_t n = p.n_dev ? min(p.n, *p.n_dev) : p.n;
-            for (int32_t k = 0; k < n; ++k) consider(p.sorted[k], cx, cy, P, best, besti);
+            for (int32_t k = 0; k < n; ++k) consider(p.sorted[k], cx, cy, Px, Py, best, besti);
             return n > 0 ? besti : -1;       // no site at all: background
         }
         for (int32_t oy = -r; oy <= r; ++oy) {
-            const int32_t qy = pos_mod(by + oy, p.nb);
+            const int32_t qy = pos_mod(by + oy, p.nby);
             const bool edge_row = (oy == -r || oy == r);
             for (int32_t ox = -r; ox <= r; ox += (edge_row || r == 0) ? 1 : 2 * r) {
-                const int32_t qx = pos_mod(bx + ox, p.nb);
-                const int32_t b = qy * p.nb + qx;
+                const int32_t qx = pos_mod(bx + ox, p.nbx);
+                const int32_t b = qy * p.nbx + qx;
                 const int32_t e = p.bucket_start[b + 1];
                 for (int32_t k = p.bucket_start[b]; k < e; ++k)
-                    consider(p.sorted[k], cx, cy, P, best, besti);
+                    consider(p.sorted[k], cx, cy, Px, Py, best, besti);
             }
         }
         const int64_t rw = (int64_t)r * p.w;
@@ -137,10 +140,10 @@ __device__ int32_t label_cell_general(const LabelParams& p, int32_t x, int32_t y
 __global__ void __launch_bounds__(256) label_general_kernel(LabelParams p, int32_t* __restrict__ labels) {
     const int64_t cell = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     // 16 x 16 blocks of cells per CTA keep a warp's cells inside few buckets
-    const int32_t bw = (p.L + 15) / 16;
+    const int32_t bw = (p.wx1 - p.wx0 + 15) / 16;
     const int32_t blk = (int32_t)(cell >> 8), in = (int32_t)(cell & 255);
-    const int32_t x = (blk % bw) * 16 + (in & 15), y = (blk / bw) * 16 + (in >> 4);
-    if (x < p.L && y < p.L) labels[(int64_t)y * p.L + x] = label_cell_general(p, x, y);
+    const int32_t x = p.wx0 + (blk % bw) * 16 + (in & 15), y = p.wy0 + (blk / bw) * 16 + (in >> 4);
+    if (x < p.wx1 && y < p.wy1) labels[(int64_t)(y - p.wy0) * p.pitch + (x - p.wx0)] = label_cell_general(p, x, y);
 }
 
 // ---------------------------------------------------------------- tile path
@@ -163,11 +166,11 @@ __device__ __forceinline__ int32_t gather_region(const LabelParams& p, WarpScrat
     const int32_t r0 = floor_div(cym - HY - H, p.w), r1 = floor_div(cym + HY + H, p.w);
     const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
     const int32_t RX0 = q0 * p.w, RX1 = (q1 + 1) * p.w, RY0 = r0 * p.w, RY1 = (r1 + 1) * p.w;
-    const int32_t half = p.P >> 1;
-    if (RX1 - RX0 > half || RY1 - RY0 > half) return -1;
+    const int32_t halfx = p.Px >> 1, halfy = p.Py >> 1;
+    if (RX1 - RX0 > halfx || RY1 - RY0 > halfy) return -1;
     if (cxm - RX0 > kMaxRel || RX1 - cxm > kMaxRel || cym - RY0 > kMaxRel || RY1 - cym > kMaxRel) return -1;
-    const int32_t a0 = pos_mod(q0, p.nb);
-    const bool split = a0 + ncols > p.nb;
+    const int32_t a0 = pos_mod(q0, p.nbx);
+    const bool split = a0 + ncols > p.nbx;
     const int32_t nseg = split ? 2 * nrows : nrows;
     if (nseg > kMaxSeg) return -1;
     {
@@ -181,13 +184,13 @@ __device__ __forceinline__ int32_t gather_region(const LabelParams& p, WarpScrat
     int32_t beg = 0, cnt = 0;
     if (lane < nseg) {
         const int32_t row = split ? lane >> 1 : lane;
-        const int32_t ay = pos_mod(r0 + row, p.nb);
+        const int32_t ay = pos_mod(r0 + row, p.nby);
         int32_t c0, c1;                                  // bucket columns [c0, c1)
         if (!split) { c0 = a0; c1 = a0 + ncols; }
-        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
-        else { c0 = 0; c1 = a0 + ncols - p.nb; }
-        beg = p.bucket_start[ay * p.nb + c0];
-        cnt = p.bucket_start[ay * p.nb + c1] - beg;
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nbx; }
+        else { c0 = 0; c1 = a0 + ncols - p.nbx; }
+        beg = p.bucket_start[ay * p.nbx + c0];
+        cnt = p.bucket_start[ay * p.nbx + c1] - beg;
     }
     int32_t inc = cnt;
 #pragma unroll
@@ -209,8 +212,8 @@ __device__ __forceinline__ int32_t gather_region(const LabelParams& p, WarpScrat
         if (i < total) {
             const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
             int32_t rx = s.x - cxm, ry = s.y - cym;
-            rx = rx >= half ? rx - p.P : (rx < -half ? rx + p.P : rx);
-            ry = ry >= half ? ry - p.P : (ry < -half ? ry + p.P : ry);
+            rx = rx >= halfx ? rx - p.Px : (rx < -halfx ? rx + p.Px : rx);
+            ry = ry >= halfy ? ry - p.Py : (ry < -halfy ? ry + p.Py : ry);
             ws.g_rx[i] = rx; ws.g_ry[i] = ry; ws.g_idx[i] = s.z;
             best = min(best, rx * rx + ry * ry);
         }
@@ -253,18 +256,18 @@ __device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs,
     constexpr int GROUPS = 32 / TW, ROWS = TH / GROUPS;
     static_assert(QH % ROWS == 0, "a lane's rows must lie in one quadrant");
     const unsigned full = 0xffffffffu;
-    const int32_t H = p.halo_fast, P = p.P, half = p.P >> 1;
+    const int32_t H = p.halo_fast, Px = p.Px, Py = p.Py, halfx = p.Px >> 1, halfy = p.Py >> 1;
 
     // ---- bucket range of the region, relative bounds
-    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
-    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
+    const int32_t q0 = div_w(p, cxm - HX - H + Px) - p.nbx, q1 = div_w(p, cxm + HX + H + Px) - p.nbx;
+    const int32_t r0 = div_w(p, cym - HY - H + Py) - p.nby, r1 = div_w(p, cym + HY + H + Py) - p.nby;
     const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
-    if (ncols * p.w > half || nrows * p.w > half) return false;
+    if (ncols * p.w > halfx || nrows * p.w > halfy) return false;
     const int32_t RX0 = q0 * p.w - cxm, RX1 = (q1 + 1) * p.w - cxm;     // region [RX0, RX1) rel. to centre
     const int32_t RY0 = r0 * p.w - cym, RY1 = (r1 + 1) * p.w - cym;
     if (-RX0 > kMaxRel || RX1 > kMaxRel || -RY0 > kMaxRel || RY1 > kMaxRel) return false;
-    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
-    const bool split = a0 + ncols > p.nb;
+    const int32_t a0 = q0 < 0 ? q0 + p.nbx : (q0 >= p.nbx ? q0 - p.nbx : q0);
+    const bool split = a0 + ncols > p.nbx;
     const int32_t nseg = split ? 2 * nrows : nrows;
     if (nseg > 32) return false;
 
@@ -273,13 +276,13 @@ __device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs,
     if (lane < nseg) {
         const int32_t row = split ? lane >> 1 : lane;
         int32_t ay = r0 + row;
-        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
+        ay = ay < 0 ? ay + p.nby : (ay >= p.nby ? ay - p.nby : ay);
         int32_t c0, c1;
         if (!split) { c0 = a0; c1 = a0 + ncols; }
-        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
-        else { c0 = 0; c1 = a0 + ncols - p.nb; }
-        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
-        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nbx; }
+        else { c0 = 0; c1 = a0 + ncols - p.nbx; }
+        beg = __ldg(&p.bucket_start[ay * p.nbx + c0]);
+        cnt = __ldg(&p.bucket_start[ay * p.nbx + c1]) - beg;
     }
     int32_t inc = cnt;
 #pragma unroll
@@ -300,8 +303,8 @@ __device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs,
     if (valid) {
         const int4 s = __ldg(&p.sorted[sbeg + (lane - sexc)]);
         rx = s.x - cxm; ry = s.y - cym; idx = s.z;
-        rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
-        ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+        rx = rx >= halfx ? rx - Px : (rx < -halfx ? rx + Px : rx);
+        ry = ry >= halfy ? ry - Py : (ry < -halfy ? ry + Py : ry);
     }
     // ---- sort by original index: rank = number of sites with a smaller index (indices distinct)
     int32_t rank = 0;
@@ -366,11 +369,11 @@ __device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs,
         }
     }
     const int32_t x = tx0 + lx;
-    if (x < p.L) {
-        int32_t* __restrict__ out = labels + (int64_t)(ty0 + ly0) * p.L + x;
+    if (x < p.wx1) {
+        int32_t* __restrict__ out = labels + (int64_t)(ty0 + ly0 - p.wy0) * p.pitch + (x - p.wx0);
 #pragma unroll
         for (int j = 0; j < ROWS; ++j)
-            if (ty0 + ly0 + j < p.L) out[(int64_t)j * p.L] = list[bi[j]].w;
+            if (ty0 + ly0 + j < p.wy1) out[(int64_t)j * p.pitch] = list[bi[j]].w;
     }
     return true;
 }
@@ -440,11 +443,11 @@ __device__ __noinline__ bool tile_generic(const LabelParams& p, WarpScratch& ws,
         }
     }
     const int32_t x = tx0 + lx;
-    if (x < p.L) {
+    if (x < p.wx1) {
 #pragma unroll
         for (int j = 0; j < ROWS; ++j) {
             const int32_t y = ty0 + ly0 + j;
-            if (y < p.L) store_label(p, labels, x, y, ws.cand[bi[j]].w);
+            if (y < p.wy1) store_label(p, labels, x, y, ws.cand[bi[j]].w);
         }
     }
     return true;
@@ -500,32 +503,32 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
                                               int32_t cxm, int32_t cym, int32_t H, int32_t* R) {
     constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
     const unsigned full = 0xffffffffu;
-    const int32_t P = p.P, half = p.P >> 1;
-    const int32_t q0 = div_w(p, cxm - HX - H + P) - p.nb, q1 = div_w(p, cxm + HX + H + P) - p.nb;
-    const int32_t r0 = div_w(p, cym - HY - H + P) - p.nb, r1 = div_w(p, cym + HY + H + P) - p.nb;
+    const int32_t Px = p.Px, Py = p.Py, halfx = p.Px >> 1, halfy = p.Py >> 1;
+    const int32_t q0 = div_w(p, cxm - HX - H + Px) - p.nbx, q1 = div_w(p, cxm + HX + H + Px) - p.nbx;
+    const int32_t r0 = div_w(p, cym - HY - H + Py) - p.nby, r1 = div_w(p, cym + HY + H + Py) - p.nby;
     const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
-    if (ncols * p.w > half || nrows * p.w > half) return 0;
+    if (ncols * p.w > halfx || nrows * p.w > halfy) return 0;
     // the buckets cover more than asked for; only the sites inside the exact rectangle
     // [-HX-H, HX+H] x [-HY-H, HY+H] are kept (shorter lists for every quadrant), so that rectangle is
     // the region the coverage test may rely on: R = {x lower (inclusive), x upper (exclusive), y ...}
     R[0] = -(HX + H); R[1] = HX + H + 1;
     R[2] = -(HY + H); R[3] = HY + H + 1;
     if (R[1] > kCtaMaxExtent || R[3] > kCtaMaxExtent) return 0;
-    const int32_t a0 = q0 < 0 ? q0 + p.nb : (q0 >= p.nb ? q0 - p.nb : q0);
-    const bool split = a0 + ncols > p.nb;
+    const int32_t a0 = q0 < 0 ? q0 + p.nbx : (q0 >= p.nbx ? q0 - p.nbx : q0);
+    const bool split = a0 + ncols > p.nbx;
     const int32_t nseg = split ? 2 * nrows : nrows;
     if (nseg > 32) return 0;
     int32_t beg = 0, cnt = 0;
     if (lane < nseg) {
         const int32_t row = split ? lane >> 1 : lane;
         int32_t ay = r0 + row;
-        ay = ay < 0 ? ay + p.nb : (ay >= p.nb ? ay - p.nb : ay);
+        ay = ay < 0 ? ay + p.nby : (ay >= p.nby ? ay - p.nby : ay);
         int32_t c0, c1;
         if (!split) { c0 = a0; c1 = a0 + ncols; }
-        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nb; }
-        else { c0 = 0; c1 = a0 + ncols - p.nb; }
-        beg = __ldg(&p.bucket_start[ay * p.nb + c0]);
-        cnt = __ldg(&p.bucket_start[ay * p.nb + c1]) - beg;
+        else if ((lane & 1) == 0) { c0 = a0; c1 = p.nbx; }
+        else { c0 = 0; c1 = a0 + ncols - p.nbx; }
+        beg = __ldg(&p.bucket_start[ay * p.nbx + c0]);
+        cnt = __ldg(&p.bucket_start[ay * p.nbx + c1]) - beg;
     }
     int32_t inc = cnt;
 #pragma unroll
@@ -548,8 +551,8 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
         if (i < total) {
             const int4 s = __ldg(&p.sorted[sbeg + (i - sexc)]);
             rx = s.x - cxm; ry = s.y - cym; idx = s.z;
-            rx = rx >= half ? rx - P : (rx < -half ? rx + P : rx);
-            ry = ry >= half ? ry - P : (ry < -half ? ry + P : ry);
+            rx = rx >= halfx ? rx - Px : (rx < -halfx ? rx + Px : rx);
+            ry = ry >= halfy ? ry - Py : (ry < -halfy ? ry + Py : ry);
             keep = abs(rx) <= HX + H && abs(ry) <= HY + H;
         }
         const unsigned ball = __ballot_sync(full, keep);
@@ -685,7 +688,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     __shared__ CtaShared sh;
     __shared__ typename std::conditional<kFused, CtaFusedShared, CtaNoFused>::type fs;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int32_t X0 = blockIdx.x * (8 * kCtaQX), Y0 = blockIdx.y * (8 * kCtaQY);
+    const int32_t X0 = p.wx0 + blockIdx.x * (8 * kCtaQX), Y0 = p.wy0 + blockIdx.y * (8 * kCtaQY);
     // ---- phases G + A; quadrants whose bound could not be proven get one retry with a wider halo
     if (threadIdx.x < kCtaQ) sh.count[threadIdx.x] = 0;
     if constexpr (kFused) {
@@ -727,9 +730,9 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     for (int h = 0; h < 2; ++h) {
         const int q = (2 * wy + h) * kCtaQX + qx;
         const int32_t y0 = Y0 + 16 * wy + 8 * h;
-        if (x >= p.L || y0 >= p.L) continue;
+        if (x >= p.wx1 || y0 >= p.wy1) continue;
         const int32_t cnt = sh.count[q];
-        int32_t* __restrict__ out = labels + (int64_t)y0 * p.L + x;
+        int32_t* __restrict__ out = labels + (int64_t)(y0 - p.wy0) * p.pitch + (x - p.wx0);
         if (cnt < 0) {
             // not proven: the quadrant goes to label_fixup_kernel (one warp per quadrant, adaptive
             // halo).  The list holds every quadrant of the lattice, or is disabled (fail_cap == 0) and
@@ -738,10 +741,10 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
                 if ((lane & 7) == 0) p.fail_items[atomicAdd(p.fail_count, 1)] = make_int2(x, y0);
             } else {
                 for (int j = 0; j < 8; ++j) {
-                    if (y0 + j >= p.L) break;
+                    if (y0 + j >= p.wy1) break;
                     const int32_t v = label_cell_general(p, x, y0 + j);
                     if constexpr (kFused) store_label(p, labels, x, y0 + j, v);
-                    else out[(int64_t)j * p.L] = v;
+                    else out[(int64_t)j * p.pitch] = v;
                 }
             }
             continue;
@@ -789,21 +792,21 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const int2 f = fs.fin[sel[j]][q];         // (label, slot)
-                *out = f.x; out += p.L;
+                *out = f.x; out += p.pitch;
                 lab[j] = f.x;
                 W[2 * h + (j >> 2)] |= (uint32_t)f.y << (8 * (j & 3));
             }
             if (lane == 0 || lane == 31) {               // the tile's border columns, 8 labels = two 16-byte stores
-                int4* __restrict__ c = reinterpret_cast<int4*>((lane ? p.col_right : p.col_left) + (int64_t)blockIdx.x * p.L + y0);
+                int4* __restrict__ c = reinterpret_cast<int4*>((lane ? p.col_right : p.col_left) + (int64_t)blockIdx.x * p.wy1 + y0);
                 c[0] = make_int4(lab[0], lab[1], lab[2], lab[3]);
                 c[1] = make_int4(lab[4], lab[5], lab[6], lab[7]);
             }
-        } else if (y0 + 8 <= p.L) {
+        } else if (y0 + 8 <= p.wy1) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) { *out = sh.list[sel[j]][q].w; out += p.L; }
+            for (int j = 0; j < 8; ++j) { *out = sh.list[sel[j]][q].w; out += p.pitch; }
         } else {
             for (int j = 0; j < 8; ++j)
-                if (y0 + j < p.L) out[(int64_t)j * p.L] = sh.list[sel[j]][q].w;
+                if (y0 + j < p.wy1) out[(int64_t)j * p.pitch] = sh.list[sel[j]][q].w;
         }
     }
     if constexpr (kFused) {
@@ -847,7 +850,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelPara
     const int64_t tile = (int64_t)blockIdx.x * kWarpsPerCta + wid;
     if (tile >= (int64_t)p.tiles_x * p.tiles_y) return;
     const int32_t tiy = (int32_t)(tile / p.tiles_x);
-    const int32_t tx0 = (int32_t)(tile - (int64_t)tiy * p.tiles_x) * TW, ty0 = tiy * TH;
+    const int32_t tx0 = p.wx0 + (int32_t)(tile - (int64_t)tiy * p.tiles_x) * TW, ty0 = p.wy0 + tiy * TH;
     const int32_t cxm = FP_ONE * tx0 + FP_HALF + HX, cym = FP_ONE * ty0 + FP_HALF + HY;
 
     if (use_fast && tile_fast<TW, TH>(p, scratch[wid].fast, lane, tx0, ty0, cxm, cym, labels)) return;
@@ -858,7 +861,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_tile_kernel(LabelPara
 #pragma unroll 1
     for (int j = 0; j < ROWS; ++j) {
         const int32_t y = ty0 + ly0 + j;
-        if (x < p.L && y < p.L) labels[(int64_t)y * p.L + x] = label_cell_general(p, x, y);
+        if (x < p.wx1 && y < p.wy1) labels[(int64_t)(y - p.wy0) * p.pitch + (x - p.wx0)] = label_cell_general(p, x, y);
     }
 }
 
@@ -880,7 +883,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_fixup_kernel(LabelPar
         const int32_t x = tx0 + (lane & 7), yb = ty0 + (lane >> 3) * 2;
 #pragma unroll 1
         for (int j = 0; j < 2; ++j)
-            if (x < p.L && yb + j < p.L) store_label(p, labels, x, yb + j, label_cell_general(p, x, yb + j));
+            if (x < p.wx1 && yb + j < p.wy1) store_label(p, labels, x, yb + j, label_cell_general(p, x, yb + j));
     }
 }
 
@@ -890,29 +893,37 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) label_fixup_kernel(LabelPar
 static int label_path_for(const vor_ctx* ctx, double spacing) {
     int path = (int)ctx->label_path;
     if (path == 0) path = spacing >= 7.0 ? 3 : (spacing >= 4.0 ? 2 : 1);
-    if (ctx->L < 16) path = 1;
+    if (ctx->Lx < 16 || ctx->Ly < 16) path = 1;
     return path;
 }
 
-// fused: rs != NULL -> the CTA kernel also extracts the adjacent pairs of every 32 x 32 tile (path 3 only)
-static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaStream_t stream) {
+static double site_spacing(const vor_ctx* ctx) {               // mean distance between sites, in cells
+    return sqrt((double)ctx->Lx * ctx->Ly / (double)ctx->n_hint);
+}
+
+// Labels the window [x0, x0 + ww) x [y0, y0 + wh) of the lattice into d_labels (row-major, ww columns).
+// fused: rs != NULL -> the CTA kernel also extracts the adjacent pairs of every 32 x 32 tile (path 3 only,
+// whole periodic lattice only)
+static int label_launch(vor_ctx* ctx, int32_t* d_labels, int32_t x0, int32_t y0, int32_t ww, int32_t wh,
+                        const RowSet* rs, cudaStream_t stream) {
     LabelParams p;
-    p.L = ctx->L; p.P = (int32_t)ctx->P; p.nb = ctx->nb; p.w = ctx->w; p.n = ctx->n_sites;
+    p.Px = (int32_t)ctx->Px; p.Py = (int32_t)ctx->Py; p.nbx = ctx->nbx; p.nby = ctx->nby; p.w = ctx->w;
+    p.wx0 = x0; p.wy0 = y0; p.wx1 = x0 + ww; p.wy1 = y0 + wh; p.pitch = ww;
+    p.n = ctx->n_sites;
     p.n_dev = ctx->d_n_dev;
     p.bucket_start = ctx->d_bucket_start; p.sorted = ctx->d_sorted;
     p.fail_items = nullptr; p.fail_count = nullptr; p.fail_count_next = nullptr; p.fail_cap = 0;
     p.col_left = nullptr; p.col_right = nullptr; p.dirty_tiles = nullptr; p.dirty_count = nullptr;
-    const double spacing = sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint);    // cells
+    const double spacing = site_spacing(ctx);
     const int path = label_path_for(ctx, spacing);
     const int tw = path == 3 ? 16 : 8;
     if (path == 1) {
-        const int64_t bw = (ctx->L + 15) / 16;
-        const int64_t blocks = bw * bw;
+        const int64_t blocks = (int64_t)((ww + 15) / 16) * ((wh + 15) / 16);
         VOR_LAUNCH(label_general_kernel, (unsigned)blocks, 256, 0, stream, p, d_labels);
         return VOR_OK;
     }
-    p.tiles_x = (ctx->L + tw - 1) / tw;
-    p.tiles_y = p.tiles_x;
+    p.tiles_x = (ww + tw - 1) / tw;
+    p.tiles_y = (wh + tw - 1) / tw;
     const double hx = 128.0 * (tw - 1);
     p.r_tile = (int32_t)ceil(sqrt(2.0 * hx * hx));
     p.halo0 = p.r_tile + (int32_t)(0.75 * spacing * FP_ONE);
@@ -930,7 +941,7 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaS
     const int use_fast = ctx->label_fast_off ? 0 : 1;
     if (path == 3) {
         if (!ctx->d_lab_fail) {
-            const int64_t q = (int64_t)((ctx->L + 7) / 8) * ((ctx->L + 7) / 8);
+            const int64_t q = (int64_t)((ctx->Lx + 7) / 8 + 1) * ((ctx->Ly + 7) / 8 + 1);   // any window's quadrants
             ctx->lab_fail_cap = q <= (1 << 24) ? (int32_t)q : 0;      // every quadrant fits, or no list at all
             VOR_CUDA(cudaMalloc((void**)&ctx->d_lab_fail, (size_t)(ctx->lab_fail_cap + 1) * sizeof(int2)));
             VOR_CUDA(cudaMalloc((void**)&ctx->d_lab_fail_n, 2 * sizeof(int32_t)));
@@ -940,10 +951,10 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaS
         p.fail_count = ctx->d_lab_fail_n + ctx->lab_fail_turn;
         p.fail_count_next = ctx->d_lab_fail_n + (1 - ctx->lab_fail_turn);
         ctx->lab_fail_turn = 1 - ctx->lab_fail_turn;
-        dim3 grid((ctx->L + 8 * kCtaQX - 1) / (8 * kCtaQX), (ctx->L + 8 * kCtaQY - 1) / (8 * kCtaQY));
+        dim3 grid((ww + 8 * kCtaQX - 1) / (8 * kCtaQX), (wh + 8 * kCtaQY - 1) / (8 * kCtaQY));
         if (rs) {
             p.col_left = ctx->d_fu_cols;
-            p.col_right = ctx->d_fu_cols + (size_t)(ctx->L / 32) * ctx->L;
+            p.col_right = ctx->d_fu_cols + (size_t)(ctx->Lx / 32) * ctx->Ly;
             p.dirty_tiles = ctx->d_fu_dirty;
             p.dirty_count = (int32_t*)&ctx->d_n_raw[4];
             VOR_LAUNCH(label_cta_kernel<true>, grid, kCtaThreads, 0, stream, p, d_labels, *rs);
@@ -967,23 +978,32 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, const RowSet* rs, cudaS
 extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     if (!ctx) return VOR_EINVAL;
     if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label: null labels");
-    if (ctx->nb <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label: call vor_build_cells first");
-    return label_launch(ctx, d_labels, nullptr, (cudaStream_t)stream_);
+    if (ctx->nbx <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label: call vor_build_cells first");
+    return label_launch(ctx, d_labels, 0, 0, ctx->Lx, ctx->Ly, nullptr, (cudaStream_t)stream_);
 }
 
-// Can the current cell list take the fused label -> edge path (vor_label_edges)?  It is written for the
-// CTA kernel's 32 x 32 tiles on a lattice they tile exactly.
+extern "C" int vor_label_rows(vor_ctx* ctx, int32_t y0, int32_t n_rows, int32_t* d_labels, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label_rows: null labels");
+    if (ctx->nbx <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label_rows: call vor_build_cells first");
+    if (y0 < 0 || n_rows < 1 || (int64_t)y0 + n_rows > ctx->Ly)
+        return vor_fail(ctx, VOR_EINVAL, "vor_label_rows: rows [y0, y0 + n_rows) must lie inside the lattice");
+    return label_launch(ctx, d_labels, 0, y0, ctx->Lx, n_rows, nullptr, (cudaStream_t)stream_);
+}
+
+// Can the current cell list take the fused label -> edge path (vor_frame_*)?  It is written for the
+// CTA kernel's 32 x 32 tiles on a periodic lattice they tile exactly.
 bool vor_label_fusable(const vor_ctx* ctx) {
-    if (ctx->nb <= 0 || ctx->L % 32 != 0 || !ctx->fuse) return false;
-    return label_path_for(ctx, sqrt((double)ctx->L * ctx->L / (double)ctx->n_hint)) == 3;
+    if (ctx->nbx <= 0 || ctx->Lx % 32 != 0 || ctx->Ly % 32 != 0 || !ctx->per_x || !ctx->per_y || !ctx->fuse) return false;
+    return label_path_for(ctx, site_spacing(ctx)) == 3;
 }
 
 // Labels + the adjacent pairs inside every 32 x 32 tile (inserted into the rows of rs); fills the compact
 // border columns and the list of tiles left to vor_edges_fused_tail (edges.cu).
 int vor_label_fused(vor_ctx* ctx, int32_t* d_labels, const RowSet& rs, cudaStream_t stream) {
     if (!ctx->d_fu_cols) {
-        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_cols, 2 * (size_t)(ctx->L / 32) * ctx->L * sizeof(int32_t)));
-        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_dirty, (size_t)(ctx->L / 32) * (ctx->L / 32) * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_cols, 2 * (size_t)(ctx->Lx / 32) * ctx->Ly * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_fu_dirty, (size_t)(ctx->Lx / 32) * (ctx->Ly / 32) * sizeof(int32_t)));
     }
-    return label_launch(ctx, d_labels, &rs, stream);
+    return label_launch(ctx, d_labels, 0, 0, ctx->Lx, ctx->Ly, &rs, stream);
 }

@@ -20,6 +20,7 @@ struct RowSet {
     int64_t raw_cap;
     unsigned long long* n_raw;
     int32_t* flags;
+    uint32_t exclude;          // label that takes part in no edge (obstacle colour), 0xffffffff = none
 };
 
 __device__ __forceinline__ void ovf_push(const RowSet& rs, uint32_t a, uint32_t b) {
@@ -31,6 +32,7 @@ __device__ __forceinline__ void ovf_push(const RowSet& rs, uint32_t a, uint32_t 
 // Append b to row a (a < b).  The row may receive the same b more than once (from different CTAs):
 // the finish kernel drops the repeats when it sorts the row.
 __device__ __forceinline__ void row_insert(const RowSet& rs, uint32_t a, uint32_t b) {
+    if (a == rs.exclude || b == rs.exclude) return;
     if (a < (uint32_t)rs.n_rows) {
         const uint32_t slot = atomicAdd(rs.cnt + a, 1u);
         if (slot < (uint32_t)rs.S) {

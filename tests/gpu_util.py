@@ -21,11 +21,44 @@ def u64(t, n=None):
 
 def gpu_labels(v: Vor, sx, sy):
     dsx, dsy = dev(sx), dev(sy)
-    lab = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")
+    lab = torch.empty(v.cells, dtype=torch.int32, device="cuda")
     v.vor_build_cells(dsx, dsy)
     v.vor_label(lab)
     v.vor_sync_status()
-    return lab.cpu().numpy().reshape(v.L, v.L)
+    return lab.cpu().numpy().reshape(v.Ly, v.Lx)
+
+
+def gpu_label_rows(v: Vor, y0, n_rows):
+    """vor_label_rows on the cell list built last -> (n_rows, Lx) array; guard rows around the strip."""
+    buf = torch.full(((n_rows + 2) * v.Lx,), -9, dtype=torch.int32, device="cuda")
+    v.vor_label_rows(y0, n_rows, buf[v.Lx:(n_rows + 1) * v.Lx])
+    v.vor_sync_status()
+    out = buf.cpu().numpy().reshape(n_rows + 2, v.Lx)
+    assert (out[0] == -9).all() and (out[-1] == -9).all(), "write outside the strip"
+    return out[1:-1].copy()
+
+
+def gpu_edges_image(v: Vor, labels, wrap_y, exclude=-1, cap=None, n_rows_ptr=None):
+    """vor_edges_image on a host image of whole rows -> keys (and row_ptr if n_rows_ptr is given)."""
+    cap = cap or max(1024, 8 * v.max_sites)
+    d = dev(np.ascontiguousarray(labels, dtype=np.int32).ravel())
+    out = torch.empty(cap, dtype=torch.int64, device="cuda")
+    n = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ptr = None if n_rows_ptr is None else torch.full((n_rows_ptr + 1,), -1, dtype=torch.int32, device="cuda")
+    v.vor_edges_image(d, wrap_y, exclude, out, n, ptr)
+    v.vor_sync_status()
+    keys = u64(out, int(n.item())).copy()
+    return keys if ptr is None else (keys, ptr.cpu().numpy().view(np.uint32).astype(np.int64))
+
+
+def gpu_edge_commons(v: Vor, edges, n_labels):
+    e = dev(np.asarray(edges, np.uint64).view(np.int64)) if len(edges) else torch.empty(1, dtype=torch.int64, device="cuda")
+    n = torch.tensor([len(edges)], dtype=torch.int64, device="cuda")
+    c = torch.full((max(len(edges), 1) + 2,), -9, dtype=torch.int32, device="cuda")
+    v.vor_edge_commons(e[:max(len(edges), 1)], n, n_labels, c[:max(len(edges), 1)])
+    v.vor_sync_status()
+    assert (c[max(len(edges), 1):] == -9).all()
+    return c[:len(edges)].cpu().numpy()
 
 
 def gpu_edges(v: Vor, labels, cap=None):
@@ -138,21 +171,28 @@ def gpu_t1(v: Vor, prev, now, n, cap=None):
                 overflow=overflow)
 
 
-def gpu_ccl(v: Vor, field, thr, above=True):
+def gpu_ccl(v: Vor, field, thr, above=True, connectivity=None):
     f = dev(field.astype(np.float32).ravel())
-    ccl = torch.empty(v.L * v.L, dtype=torch.int32, device="cuda")
-    v.field_threshold_ccl(f, thr, above, ccl)
+    ccl = torch.empty(v.cells, dtype=torch.int32, device="cuda")
+    if connectivity is None:
+        v.field_threshold_ccl(f, thr, above, ccl)
+    else:
+        v.field_threshold_ccl_conn(f, thr, above, connectivity, ccl)
     v.vor_sync_status()
     return ccl
 
 
-def gpu_centroids(v: Vor, ccl_dev, min_size, cap=None):
-    cap = cap or max(16, v.L * v.L // 2)
+def gpu_centroids(v: Vor, ccl_dev, min_size, cap=None, field=None):
+    cap = cap or max(16, v.cells // 2)
     cx = torch.empty(cap, dtype=torch.float64, device="cuda"); cy = torch.empty_like(cx)
     sx = torch.empty(cap, dtype=torch.int32, device="cuda"); sy = torch.empty_like(sx)
     size = torch.empty_like(sx); root = torch.empty_like(sx)
     n = torch.zeros(1, dtype=torch.int32, device="cuda")
-    v.field_centroids(ccl_dev, min_size, cx, cy, sx, sy, size, root, n)
+    if field is None:
+        v.field_centroids(ccl_dev, min_size, cx, cy, sx, sy, size, root, n)
+    else:
+        v.field_centroids_weighted(ccl_dev, dev(np.ascontiguousarray(field, dtype=np.float32).ravel()), min_size,
+                                   cx, cy, sx, sy, size, root, n)
     v.vor_sync_status()
     K = int(n.item())
     g = lambda t: t[:K].cpu().numpy()
