@@ -154,6 +154,13 @@ int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int
 int vor_edges_image(vor_ctx* ctx, const int32_t* d_labels, int32_t n_rows, int32_t wrap_y, int32_t exclude,
                     uint64_t* d_edges, int64_t cap, int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream);
 
+/* Union of n_lists key lists (row strips of one lattice, one per rank, brought together by an all-gather;
+ * SURVEY.md §8e): list l occupies d_lists[l * stride .. l * stride + min(d_counts[l], stride)); the ascending
+ * unique union goes to d_out[0..min(E, cap)), E to *d_n_out.  Labels are < n_labels.  stride * n_lists must not
+ * exceed the context's max_raw_keys. */
+int vor_merge_lists(vor_ctx* ctx, const uint64_t* d_lists, int64_t stride, const int64_t* d_counts,
+                    int32_t n_lists, int32_t n_labels, uint64_t* d_out, int64_t cap, int64_t* d_n_out, void* stream);
+
 /* ---- a5: frame-to-frame comparison (§III.B.3 translation + comparison;
  * PAPER.md:223 appearing/disappearing bubbles excluded; §III.B.4 "breaking" = in
  * D_P only, "arising" = in D_N only).  d_prev/d_now are ascending unique key lists with device

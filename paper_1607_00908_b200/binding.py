@@ -38,6 +38,7 @@ SIGNATURES = {
     "vor_label_rows": (C.c_int, [_P, C.c_int32, C.c_int32, _P, _P]),
     "vor_paint_obstacles": (C.c_int, [_P, _P, C.c_int32, _P, C.c_int32, _P]),
     "vor_edges_image": (C.c_int, [_P, _P, C.c_int32, C.c_int32, C.c_int32, _P, C.c_int64, _P, _P, _P]),
+    "vor_merge_lists": (C.c_int, [_P, _P, C.c_int64, _P, C.c_int32, C.c_int32, _P, C.c_int64, _P, _P]),
     "vor_edge_commons": (C.c_int, [_P, _P, _P, C.c_int64, C.c_int32, _P, _P]),
     "field_threshold_ccl_conn": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, _P, _P]),
     "field_centroids_weighted": (C.c_int, [_P, _P, _P, C.c_int32, _P, _P, _P, _P, _P, _P, C.c_int32, _P, _P]),
@@ -214,6 +215,13 @@ class Vor:
         self._check(self.lib.vor_edges_image(self.h, _ptr(labels, torch.int32), labels.numel() // self.Lx,
                                              1 if wrap_y else 0, exclude, _ptr(edges, torch.int64), edges.numel(),
                                              _ptr(n_edges, torch.int64), _ptr(row_ptr, torch.int32), _stream()))
+
+    def vor_merge_lists(self, lists, counts, n_labels: int, out, n_out):
+        """lists: int64[n_lists, stride] (row l = list l), counts: int64[n_lists] device."""
+        assert lists.dim() == 2 and counts.numel() == lists.shape[0]
+        self._check(self.lib.vor_merge_lists(self.h, _ptr(lists, torch.int64), lists.shape[1], _ptr(counts, torch.int64),
+                                             lists.shape[0], n_labels, _ptr(out, torch.int64), out.numel(),
+                                             _ptr(n_out, torch.int64), _stream()))
 
     def vor_edge_commons(self, edges, n_edges, n_labels: int, commons):
         assert commons.numel() >= edges.numel()

@@ -473,3 +473,48 @@ extern "C" int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_
     VOR_LAUNCH(diff_rows_write_kernel, (unsigned)n_blocks, kDrThreads, 0, stream, dp);
     return VOR_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// Union of several key lists (multi-GPU row strips: every rank extracts the keys of its strip,
+// one all-gather brings the lists together, "followed by a merge-unique"): the valid parts of the n_lists
+// buffers are packed into the sort scratch, then radix-sorted and uniqued by the same cooperative kernel as
+// the overflow path of vor_edges.
+namespace {
+
+__global__ void pack_lists_kernel(const uint64_t* __restrict__ lists, int64_t stride,
+                                  const int64_t* __restrict__ counts, int32_t n_lists, uint64_t* __restrict__ out,
+                                  int64_t cap_out, int64_t* __restrict__ n_out, int32_t* __restrict__ flags) {
+    // blockIdx.y = list; its offset = sum of the clamped counts before it (n_lists is small)
+    const int l = blockIdx.y;
+    int64_t off = 0, all = 0;
+    for (int k = 0; k < n_lists; ++k) {
+        const int64_t c = min(max(counts[k], (int64_t)0), stride);
+        if (k < l) off += c;
+        all += c;
+    }
+    if (l == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
+        *n_out = all;
+        if (all > cap_out) atomicOr(flags, FLAG_RAWKEY_OVERFLOW);
+    }
+    const int64_t m = min(max(counts[l], (int64_t)0), stride);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
+        if (off + i < cap_out) out[off + i] = lists[(int64_t)l * stride + i];
+}
+
+}  // namespace
+
+extern "C" int vor_merge_lists(vor_ctx* ctx, const uint64_t* d_lists, int64_t stride, const int64_t* d_counts,
+                               int32_t n_lists, int32_t n_labels, uint64_t* d_out, int64_t cap, int64_t* d_n_out,
+                               void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (!d_lists || !d_counts || !d_out || !d_n_out) return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: null pointer");
+    if (stride < 0 || n_lists < 1 || n_lists > 1024 || n_labels < 1 || cap < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: stride >= 0, 1 <= n_lists <= 1024, n_labels >= 1, cap >= 0");
+    if (stride * n_lists > ctx->max_raw_keys)
+        return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: stride * n_lists exceeds the context's max_raw_keys scratch");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    VOR_LAUNCH(pack_lists_kernel, dim3(2 * kNumSMs, n_lists), 256, 0, stream, d_lists, stride, d_counts, n_lists,
+               ctx->d_keys_a, ctx->max_raw_keys, ctx->d_n_raw, ctx->d_flags);
+    return vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits_for(n_labels), d_out, cap, d_n_out,
+                                FLAG_EDGE_CAP, 0, stream);
+}

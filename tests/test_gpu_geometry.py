@@ -346,3 +346,36 @@ def test_channel_sequence_field_to_events(G):
             assert np.array_equal(cr, r_cr) and np.array_equal(de, r_de)
         prev = (r_c, r_e)
     v.close()
+
+
+# ------------------------------------------------------------------ row strips of one lattice (NEXT-4)
+def test_strip_decomposition_on_one_gpu(G):
+    """Every strip of a 1-, 2-, 3- and 5-way decomposition computed by the product class (explicit rank /
+    world, no process group), merged by vor_merge_lists: the lattice's list, bit for bit.  The collective
+    itself is covered on CPU (tests/test_strips_ranks.py, gloo)."""
+    from paper_1607_00908_b200.strips import StripFrame
+    rng = np.random.default_rng(8)
+    for Lx, Ly, per, spacing in ((256, 512, (1, 1), 12.0), (192, 320, (0, 1), 16.0), (128, 200, (1, 0), 9.0)):
+        sx, sy = jitter_sites(rng, Lx, Ly, spacing)
+        n = len(sx)
+        ref = oracle.edges_g(oracle.label_brute_g(Lx, Ly, per[0], per[1], sx, sy), per[0], per[1])
+        v = make(Lx, Ly, per, n)
+        dsx, dsy = G.dev(sx), G.dev(sy)
+        cap = 8 * n
+        for world in (1, 2, 3, 5):
+            lists = torch.zeros(world, cap, dtype=torch.int64, device="cuda")
+            counts = torch.zeros(world, dtype=torch.int64, device="cuda")
+            for r in range(world):
+                f = StripFrame(v, n, cap, cap, rank=r, world=world)
+                loc, nl = f.compute_local(dsx, dsy)
+                lists[r].copy_(loc); counts[r] = nl[0]
+            out = torch.empty(cap, dtype=torch.int64, device="cuda")
+            n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+            v.vor_merge_lists(lists, counts, n, out, n_out)
+            v.vor_sync_status()
+            assert np.array_equal(G.u64(out, int(n_out.item())), ref), (Lx, Ly, world)
+        f = StripFrame(v, n, cap, cap)                          # no process group: one strip, the whole lattice
+        e, ne = f.compute(dsx, dsy)
+        v.vor_sync_status()
+        assert np.array_equal(G.u64(e, int(ne.item())), ref)
+        v.close()
