@@ -26,8 +26,8 @@ sys.path.insert(0, ROOT)
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
 # Per-launch ncu figures of the committed `ncu --set full` capture (config 5 only): DRAM bytes read + written,
-# issue-slot utilisation, warp instructions.  profiles/r2_traffic.md names the command that produced the table.
-NCU_TABLE = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+# issue-slot utilisation, warp instructions.  profiles/r2b_traffic.md names the command that produced the table.
+NCU_TABLE = os.path.join(ROOT, "profiles", "r2b_traffic.csv")
 
 
 def ncu_table():
@@ -326,6 +326,26 @@ def run_ours(args, w):
     torch.cuda.synchronize()
     events_info = {"ms": e0.elapsed_time(e1) / 10, "events_number": int(ev_m.item()), "global_trigger": int(ev_g.item()),
                    "api": "vor_events: local_trigger, eventsIndices, eventsCount past/now (PAPER.md:215-236)"}
+    # couples of active vertices, breaking / arising class, T1 partner
+    t1_keys, t1_partner = torch.empty(cap_e, dtype=torch.int64, device="cuda"), torch.empty(cap_e, dtype=torch.int64, device="cuda")
+    t1_cls, t1_cp, t1_cn = (torch.empty(cap_e, **i32) for _ in range(3))
+    t1_n = torch.zeros(1, dtype=torch.int64, device="cuda")
+    def t1():
+        v.vor_t1_events(edges[1 - last], n_edges[1 - last], edges[last], n_edges[last], created, n_c, destroyed, n_d,
+                        ev_bufs[0], t1_keys, t1_cls, t1_cp, t1_cn, t1_partner, t1_n)
+    for _ in range(3):
+        t1()
+    e0.record(stream)
+    for _ in range(10):
+        t1()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    k_ = int(t1_n.item())
+    events_info["t1"] = {"ms": e0.elapsed_time(e1) / 10, "couples": k_,
+                         "breaking": int((t1_cls[:k_] == 1).sum().item()), "arising": int((t1_cls[:k_] == 2).sum().item()),
+                         "t1_quadruples": int(((t1_cls[:k_] == 1) & (t1_partner[:k_] != -1)).sum().item()),
+                         "api": "vor_t1_events: couples, breaking / arising, common neighbours, T1 partner (PAPER.md:238, 248-266)"}
+    del t1_keys, t1_partner, t1_cls, t1_cp, t1_cn
 
     # ---- e2e: the same frames through vor_frame_host (host buffers, H2D + D2H inside the timed region)
     e2e = None
@@ -478,6 +498,7 @@ FIELD_GROUPS = (("threshold_ccl", ("ccl_",)), ("centroids", ("comp_", "accumulat
 
 
 def field_group(kernel_name: str) -> str:
+    kernel_name = kernel_name.strip("()")
     for g, prefixes in FIELD_GROUPS:
         if any(kernel_name.startswith(p) for p in prefixes):
             return g

@@ -96,6 +96,7 @@ struct vor_ctx {
     // ---- diff with maps: translated / filtered lists
     uint64_t* d_tr_prev;       // lazily sized to max_raw_keys
     uint64_t* d_tr_now;
+    uint32_t* d_tr_rowptr[2];  // [max_sites + 1] row offsets of the two lists (rows path)
     int64_t* d_tr_counts;      // [4]
 
     // ---- field path (a6..a8)
@@ -133,7 +134,8 @@ struct vor_ctx {
     int64_t* d_ff_tmpcount;    // [2] created / destroyed counts before they are gathered
     float* d_ff_field[2];      // device copies of submitted host fields (lazily)
     int ff_cur;                // generation of the last field frame; -1 = none
-    int32_t ff_hint;           // bubbles in the last collected frame (sizes the next cell list)
+    int32_t ff_hint;           // bubbles in an earlier frame (sizes the next cell list)
+    int32_t* h_ff_count;       // pinned [1]: bubble count of the latest frame whose kernels have finished
     // pipelined variant (vor_frame_submit / vor_frame_collect): two frames in flight, copies on own streams
     int32_t* d_pp_sx[2];
     int32_t* d_pp_sy[2];

@@ -104,7 +104,7 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_lab_fail); cudaFree(ctx->d_lab_fail_n);
     cudaFree(ctx->d_fu_cols); cudaFree(ctx->d_fu_dirty);
     cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
-    cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_counts); cudaFree(ctx->d_dr_scratch);
+    cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_rowptr[0]); cudaFree(ctx->d_tr_rowptr[1]); cudaFree(ctx->d_tr_counts); cudaFree(ctx->d_dr_scratch);
     for (int k = 0; k < 5; ++k) cudaFree(ctx->d_t1[k]);
     cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
     cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best); cudaFree(ctx->d_mgrid);
@@ -112,7 +112,7 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_fr_edges[0]); cudaFree(ctx->d_fr_edges[1]);
     cudaFree(ctx->d_fr_nedges[0]); cudaFree(ctx->d_fr_nedges[1]);
     cudaFree(ctx->d_fr_rowptr[0]); cudaFree(ctx->d_fr_rowptr[1]);
-    cudaFree(ctx->d_ff_ccl); cudaFree(ctx->d_ff_maps); cudaFree(ctx->d_ff_tmpcount);
+    cudaFree(ctx->d_ff_ccl); cudaFree(ctx->d_ff_maps); cudaFree(ctx->d_ff_tmpcount); cudaFreeHost(ctx->h_ff_count);
     for (int k = 0; k < 2; ++k) { cudaFree(ctx->d_ff_cxy[k]); cudaFree(ctx->d_ff_comp[k]); cudaFree(ctx->d_ff_field[k]); }
     cudaFree(ctx->d_fr_created); cudaFree(ctx->d_fr_destroyed); cudaFree(ctx->d_fr_counts);
     cudaFreeHost(ctx->h_fr_counts); cudaFreeHost(ctx->h_fr_sites); cudaFreeHost(ctx->h_fr_lists);

@@ -12,6 +12,7 @@
 #include <cooperative_groups.h>
 
 #include "common.cuh"
+#include "rows.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -385,6 +386,35 @@ __global__ void filter_now_kernel(const uint64_t* __restrict__ now, const int64_
     }
 }
 
+// the same two filters feeding the adjacency rows directly (row a collects b > a; rows.cuh): the finish
+// kernel of vor_edges then returns the sorted unique list with its row offsets, without a radix sort
+__global__ void translate_prev_rows_kernel(const uint64_t* __restrict__ prev, const int64_t* __restrict__ n_prev_p,
+                                           int64_t cap_in, const int32_t* __restrict__ p2n, int32_t n_prev_labels,
+                                           const RowSet rs) {
+    const int64_t n = min(*n_prev_p, cap_in);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        const uint64_t e = prev[k];
+        const uint32_t a = (uint32_t)(e >> 32), b = (uint32_t)e;
+        if (a >= (uint32_t)n_prev_labels || b >= (uint32_t)n_prev_labels) continue;
+        const int32_t i = p2n[a], j = p2n[b];
+        if (i < 0 || j < 0 || i == j) continue;
+        row_insert(rs, (uint32_t)min(i, j), (uint32_t)max(i, j));
+    }
+}
+
+__global__ void filter_now_rows_kernel(const uint64_t* __restrict__ now, const int64_t* __restrict__ n_now_p,
+                                       int64_t cap_in, const int32_t* __restrict__ n2p, int32_t n_now_labels,
+                                       const RowSet rs) {
+    const int64_t n = min(*n_now_p, cap_in);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        const uint64_t e = now[k];
+        const uint32_t a = (uint32_t)(e >> 32), b = (uint32_t)e;
+        if (a >= (uint32_t)n_now_labels || b >= (uint32_t)n_now_labels) continue;
+        if (n2p[a] < 0 || n2p[b] < 0) continue;
+        row_insert(rs, a, b);
+    }
+}
+
 int bits_for(int32_t n) {
     int bits = 1;
     while (bits < 31 && ((int64_t)1 << bits) < (int64_t)n) ++bits;
@@ -417,6 +447,30 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
         if (!ctx->d_tr_prev) {
             VOR_CUDA(cudaMalloc((void**)&ctx->d_tr_prev, ctx->max_raw_keys * sizeof(uint64_t)));
             VOR_CUDA(cudaMalloc((void**)&ctx->d_tr_now, ctx->max_raw_keys * sizeof(uint64_t)));
+        }
+        if (n_now_labels <= ctx->max_sites) {
+            // both lists go through the adjacency rows (one row per now label): sorted, unique, with row
+            // offsets - then the row-by-row comparison.  No radix sort, no cooperative searching kernel.
+            if (!ctx->d_tr_rowptr[0]) {
+                VOR_CUDA(cudaMalloc((void**)&ctx->d_tr_rowptr[0], ((size_t)ctx->max_sites + 1) * sizeof(uint32_t)));
+                VOR_CUDA(cudaMalloc((void**)&ctx->d_tr_rowptr[1], ((size_t)ctx->max_sites + 1) * sizeof(uint32_t)));
+            }
+            RowSet rs = vor_row_set(ctx);
+            rs.n_rows = n_now_labels;
+            VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 8 * sizeof(int64_t), stream));
+            VOR_LAUNCH(translate_prev_rows_kernel, 4 * kNumSMs, 256, 0, stream, d_prev, d_n_prev, cap_prev, d_p2n,
+                       n_prev_labels, rs);
+            int rc = vor_edges_finish(ctx, rs, ctx->d_tr_prev, ctx->max_raw_keys, &ctx->d_tr_counts[0],
+                                      ctx->d_tr_rowptr[0], false, stream);
+            if (rc != VOR_OK) return rc;
+            VOR_CUDA(cudaMemsetAsync(ctx->d_n_raw, 0, 8 * sizeof(int64_t), stream));
+            VOR_LAUNCH(filter_now_rows_kernel, 4 * kNumSMs, 256, 0, stream, d_now, d_n_now, cap_now, d_n2p,
+                       n_now_labels, rs);
+            rc = vor_edges_finish(ctx, rs, ctx->d_tr_now, ctx->max_raw_keys, &ctx->d_tr_counts[1],
+                                  ctx->d_tr_rowptr[1], false, stream);
+            if (rc != VOR_OK) return rc;
+            return vor_diff_rows(ctx, ctx->d_tr_prev, ctx->d_tr_rowptr[0], ctx->d_tr_now, ctx->d_tr_rowptr[1],
+                                 n_now_labels, d_created, d_destroyed, cap, d_n_created, d_n_destroyed, stream_);
         }
         const int bits = bits_for(n_now_labels);
         // translated prev -> d_keys_a -> sort/unique -> d_tr_prev

@@ -34,7 +34,7 @@ __global__ void ev_mark_kernel(const uint64_t* __restrict__ created, const int64
 
 __device__ __forceinline__ void ev_chunk(int64_t n, int64_t* beg, int64_t* end) {
     int64_t C = (n + gridDim.x - 1) / gridDim.x;
-    C = (C + kEvBatch - 1) / kEvBatch * kEvBatch;
+    C = (C + 32 * kEvItems - 1) / (32 * kEvItems) * (32 * kEvItems);     // whole warp tiles
     const int64_t s = (int64_t)blockIdx.x * C;
     *beg = s < n ? s : n;
     *end = s + C < n ? s + C : n;
@@ -351,7 +351,7 @@ __global__ void __launch_bounds__(kEvThreads) t1_count_kernel(const uint64_t* __
     __shared__ int64_t sh[32];
     const int64_t m = min(max(*l.n_now, (int64_t)0), l.cap_now) + min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
     int64_t beg, end;
-    t1_chunk(m, kEvBatch, &beg, &end);
+    t1_chunk(m, 32 * kEvItems, &beg, &end);
     int64_t c = 0;
     for (int64_t i = beg + threadIdx.x; i < end; i += kEvThreads) c += U[i] != kDrop;
     c = ev_block_sum(c, sh);
@@ -368,7 +368,7 @@ __global__ void __launch_bounds__(kEvThreads) t1_write_kernel(const uint64_t* __
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int64_t m = min(max(*l.n_now, (int64_t)0), l.cap_now) + min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
     int64_t beg, end;
-    t1_chunk(m, kEvBatch, &beg, &end);
+    t1_chunk(m, 32 * kEvItems, &beg, &end);
     int64_t before = 0, all = 0;
     for (int b = threadIdx.x; b < (int)gridDim.x; b += kEvThreads) {
         const int64_t v = partial[b];

@@ -164,8 +164,9 @@ constexpr int kCompBatch = kCompThreads * kCompItems;
 constexpr int kCompGrid = 4 * kNumSMs;             // <= 2 * kMaxCoopBlocks entries of d_blk_count
 
 __device__ __forceinline__ void comp_chunk(int64_t n, int64_t* beg, int64_t* end) {
+    // chunks are whole warp tiles (32 x kCompItems items), so that short lists spread over many blocks
     int64_t C = (n + gridDim.x - 1) / gridDim.x;
-    C = (C + kCompBatch - 1) / kCompBatch * kCompBatch;
+    C = (C + 32 * kCompItems - 1) / (32 * kCompItems) * (32 * kCompItems);
     int64_t s = (int64_t)blockIdx.x * C;
     *beg = s < n ? s : n;
     *end = s + C < n ? s + C : n;
@@ -381,7 +382,13 @@ struct CentroidSink {
         *n_comp = (int32_t)t;
         if (t > cap) atomicOr(flags, FLAG_COMP_CAP);
     }
-    __device__ static long long floor_div(__int128 a, __int128 b) {        // b > 0
+    // floor(256 S / W), W > 0; 64-bit arithmetic whenever 256 |S| fits (always, without weights)
+    __device__ static long long floor_div256(long long S, long long W) {
+        if (S > -((long long)1 << 54) && S < ((long long)1 << 54)) {
+            const long long a = FP_ONE * S;
+            return a >= 0 ? a / W : -((-a + W - 1) / W);
+        }
+        const __int128 a = (__int128)FP_ONE * S, b = W;
         return (long long)(a >= 0 ? a / b : -((-a + b - 1) / b));
     }
     __device__ void put(int64_t pos, int64_t k) const {
@@ -390,7 +397,7 @@ struct CentroidSink {
         const long long W = weighted ? acc[3 * (size_t)max_comp + k] : m;     // total weight
         const int32_t r = comp_root[k];
         const long long xr = r % Lx, yr = r / Lx, Px = (long long)FP_ONE * Lx, Py = (long long)FP_ONE * Ly;
-        const long long fx = floor_div((__int128)FP_ONE * Sx, W), fy = floor_div((__int128)FP_ONE * Sy, W);
+        const long long fx = floor_div256(Sx, W), fy = floor_div256(Sy, W);
         sx[pos] = (int32_t)((((FP_ONE * xr + FP_HALF + fx) % Px) + Px) % Px);
         sy[pos] = (int32_t)((((FP_ONE * yr + FP_HALF + fy) % Py) + Py) % Py);
         double ux = __dadd_rn(__dadd_rn((double)xr, 0.5), __ddiv_rn((double)Sx, (double)W));

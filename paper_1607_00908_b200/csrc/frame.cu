@@ -132,6 +132,8 @@ int ensure_field_buffers(vor_ctx* ctx) {
     }
     VOR_CUDA(cudaMalloc((void**)&ctx->d_ff_maps, 2 * K * sizeof(int32_t)));
     VOR_CUDA(cudaMalloc((void**)&ctx->d_ff_tmpcount, 2 * sizeof(int64_t)));
+    VOR_CUDA(cudaMallocHost((void**)&ctx->h_ff_count, sizeof(int32_t)));
+    *ctx->h_ff_count = 0;
     ctx->ff_cur = -1;
     return VOR_OK;
 }
@@ -147,9 +149,14 @@ int field_frame_compute(vor_ctx* ctx, const float* d_field, const FieldArgs& fa,
     double* cx = ctx->d_ff_cxy[now]; double* cy = cx + K;
     int32_t* c = ctx->d_ff_comp[now]; const int32_t* pc = ctx->d_ff_comp[prev];
     int32_t* p2n = ctx->d_ff_maps; int32_t* n2p = p2n + K;
+    // the bubble count of an earlier frame, copied to page-locked memory behind that frame's kernels: whatever
+    // has arrived by now sizes this frame's buckets and halo (a hint: results never depend on it), no waiting
+    const int32_t seen = *(volatile int32_t*)ctx->h_ff_count;
+    if (seen > 0) ctx->ff_hint = seen < K ? seen : K;
     if ((rc = field_threshold_ccl(ctx, d_field, fa.thr, fa.above, ctx->d_ff_ccl, stream)) != VOR_OK) return rc;
     if ((rc = field_centroids(ctx, ctx->d_ff_ccl, fa.min_size, cx, cy, c, c + K, c + 2 * K, c + 3 * K, K,
                               c + 4 * K, stream)) != VOR_OK) return rc;
+    VOR_CUDA(cudaMemcpyAsync(ctx->h_ff_count, c + 4 * K, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
     if (have_prev && (rc = match_sites(ctx, pc, pc + K, pc + 4 * K, c, c + K, c + 4 * K, K, K, fa.radius_fp,
                                        p2n, n2p, stream)) != VOR_OK) return rc;
     if ((rc = vor_build_cells_dev(ctx, c, c + K, c + 4 * K, K, ctx->ff_hint > 0 ? ctx->ff_hint : K, stream)) != VOR_OK)
