@@ -46,7 +46,8 @@ typedef enum {
 /* Create a context for an L x L lattice (2 <= L <= 2^22) and at most max_sites sites
  * (1 <= max_sites < 2^31).  max_raw_keys sizes the scratch that receives the (partly
  * de-duplicated) edge keys before sorting; 0 selects a default (max(2^20, 16*max_sites), never
- * more than the hard worst case 2*L*L).  Allocates device memory on the CURRENT device. */
+ * more than the hard worst case 2*L*L).  Allocates device memory on the CURRENT device;
+ * every later call on the context must be made with that device current (VOR_ESTATE otherwise). */
 int vor_create(vor_ctx** out, int32_t L, int32_t max_sites, int64_t max_raw_keys);
 /* The paper's own geometry: an Lx x Ly lattice (§IV: 2048 x 1024),
  * each axis periodic (1) or closed by walls (0; beyond the domain boundary there are no

@@ -170,6 +170,7 @@ static int build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, i
 extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
                                int32_t n_sites, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_sx || !d_sy) return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: null site array");
     if (n_sites < 1 || n_sites > ctx->max_sites)
         return vor_fail(ctx, VOR_EINVAL, "vor_build_cells: n_sites out of range [1, max_sites]");
@@ -179,6 +180,7 @@ extern "C" int vor_build_cells(vor_ctx* ctx, const int32_t* d_sx, const int32_t*
 extern "C" int vor_build_cells_dev(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
                                    const int32_t* d_n_sites, int32_t cap, int32_t n_hint, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_sx || !d_sy || !d_n_sites) return vor_fail(ctx, VOR_EINVAL, "vor_build_cells_dev: null pointer");
     if (cap < 1 || cap > ctx->max_sites)
         return vor_fail(ctx, VOR_EINVAL, "vor_build_cells_dev: cap out of range [1, max_sites]");

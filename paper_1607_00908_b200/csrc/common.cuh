@@ -176,6 +176,14 @@ inline int vor_cuda_fail(vor_ctx* ctx, cudaError_t e, const char* where) {
     return VOR_ECUDA;
 }
 
+// Every entry point that enqueues work or allocates lazily runs on the device the context was created on.
+inline int vor_check_device(vor_ctx* ctx) {
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess || d != ctx->device)
+        return vor_fail(ctx, VOR_ESTATE, "the current CUDA device is not the one this context was created on");
+    return VOR_OK;
+}
+
 #define VOR_CUDA(call)                                                          \
     do {                                                                        \
         cudaError_t e_ = (call);                                                \

@@ -430,6 +430,7 @@ extern "C" int vor_diff(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n
                         uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
                         int64_t* d_n_created, int64_t* d_n_destroyed, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_created || !d_destroyed || !d_n_created ||
         !d_n_destroyed || cap < 0 || cap_prev < 0 || cap_now < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_diff: null pointer or negative capacity");
@@ -508,6 +509,7 @@ extern "C" int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_
                              uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
                              int64_t* d_n_created, int64_t* d_n_destroyed, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_prev || !d_prev_row_ptr || !d_now || !d_now_row_ptr || !d_created || !d_destroyed ||
         !d_n_created || !d_n_destroyed || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_diff_rows: null pointer or negative capacity");
@@ -561,6 +563,7 @@ extern "C" int vor_merge_lists(vor_ctx* ctx, const uint64_t* d_lists, int64_t st
                                int32_t n_lists, int32_t n_labels, uint64_t* d_out, int64_t cap, int64_t* d_n_out,
                                void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_lists || !d_counts || !d_out || !d_n_out) return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: null pointer");
     if (stride < 0 || n_lists < 1 || n_lists > 1024 || n_labels < 1 || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: stride >= 0, 1 <= n_lists <= 1024, n_labels >= 1, cap >= 0");

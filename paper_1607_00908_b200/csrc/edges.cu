@@ -1038,6 +1038,7 @@ extern "C" int vor_edges(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edge
 extern "C" int vor_edges_rows(vor_ctx* ctx, const int32_t* d_labels, uint64_t* d_edges, int64_t cap,
                               int64_t* d_n_edges, uint32_t* d_row_ptr, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     return vor_edges_image(ctx, d_labels, ctx->Ly, ctx->per_y, -1, d_edges, cap, d_n_edges, d_row_ptr, stream_);
 }
 
@@ -1045,6 +1046,7 @@ extern "C" int vor_edges_image(vor_ctx* ctx, const int32_t* d_labels, int32_t n_
                                int32_t exclude, uint64_t* d_edges, int64_t cap, int64_t* d_n_edges,
                                uint32_t* d_row_ptr, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_labels || !d_edges || !d_n_edges || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_edges: null pointer or negative capacity");
     if (n_rows < 1) return vor_fail(ctx, VOR_EINVAL, "vor_edges_image: n_rows must be >= 1");
@@ -1068,6 +1070,7 @@ __global__ void paint_obstacles_kernel(const uint8_t* __restrict__ mask, int32_t
 extern "C" int vor_paint_obstacles(vor_ctx* ctx, const uint8_t* d_mask, int32_t colour, int32_t* d_labels,
                                    int32_t n_rows, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_mask || !d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_paint_obstacles: null pointer");
     if (colour < 0 || n_rows < 1) return vor_fail(ctx, VOR_EINVAL, "vor_paint_obstacles: colour >= 0, n_rows >= 1");
     const int64_t n = (int64_t)ctx->Lx * n_rows;

@@ -145,6 +145,7 @@ extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d
                           int32_t* d_global_trigger, int32_t* d_count_prev, int32_t* d_count_now,
                           void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_created || !d_n_created || !d_destroyed ||
         !d_n_destroyed || !d_trigger || !d_events_indices || !d_events_number || !d_global_trigger ||
         !d_count_prev || !d_count_now)
@@ -493,6 +494,7 @@ extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t
                              uint64_t* d_couples, int32_t* d_class, int32_t* d_common_prev, int32_t* d_common_now,
                              uint64_t* d_partner, int64_t cap, int64_t* d_n_couples, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_created || !d_n_created || !d_destroyed || !d_n_destroyed ||
         !d_trigger || !d_couples || !d_class || !d_common_prev || !d_common_now || !d_partner || !d_n_couples)
         return vor_fail(ctx, VOR_EINVAL, "vor_t1_events: null pointer");
@@ -551,6 +553,7 @@ __global__ void edge_commons_kernel(T1Graph g, int32_t n, int32_t* __restrict__ 
 extern "C" int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int64_t* d_n_edges, int64_t cap_edges,
                                 int32_t n_labels, int32_t* d_commons, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_edges || !d_n_edges || !d_commons) return vor_fail(ctx, VOR_EINVAL, "vor_edge_commons: null pointer");
     if (n_labels < 1 || cap_edges < 0 || 2 * cap_edges >= ((int64_t)1 << 32))
         return vor_fail(ctx, VOR_EINVAL, "vor_edge_commons: n_labels >= 1, 0 <= cap_edges < 2^31");

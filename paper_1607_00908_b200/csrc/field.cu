@@ -301,65 +301,107 @@ __device__ __forceinline__ int64_t cell_weight(float rho) {
     return s >= 16777216.0f ? 16777216 : (s >= 1.0f ? (int64_t)s : 1);
 }
 
-// acc: [0] cells, [1] sum of w dx, [2] sum of w dy, [3] sum of w (weighted only), each max_comp entries
+// acc: [0] cells, [1] sum of w dx, [2] sum of w dy, [3] sum of w (weighted only), each max_comp entries.
+// A thread takes kAccCells consecutive cells of one row (Lx % kAccCells == 0: one 16-byte load), merges the ones
+// that carry its first bubble label (inside a bubble and on its edge that is all of them), and the warp merges
+// the threads that hold the same label (`match_any`; skipped when the whole warp agrees) before ONE lane adds
+// to the component's accumulators.  Cells of a second bubble inside the same four (rare) add their own terms.
+constexpr int kAccCells = 4;
+
 template <bool kWeighted>
-__global__ void accumulate_kernel(const int32_t* __restrict__ ccl, const float* __restrict__ field,
-                                  const int32_t* __restrict__ rank, int32_t Lx, int32_t Ly, int per_x, int per_y,
-                                  FastDiv fd, unsigned long long* __restrict__ acc, int32_t max_comp) {
-    const int64_t n = (int64_t)Lx * Ly;
-    const int64_t nround = (n + 31) / 32 * 32;     // keep warps converged for the warp collectives
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (int64_t)gridDim.x * blockDim.x) {
-        const int32_t r = i < n ? ccl[i] : -1;
-        // most warps see one value (background or the inside of a bubble): no match needed then
-        const bool uniform = __all_sync(0xffffffffu, r == __shfl_sync(0xffffffffu, r, 0));
-        const unsigned peers = uniform ? 0xffffffffu : __match_any_sync(0xffffffffu, r);
-        if (r < 0) continue;                        // whole peer group leaves together
-        const int32_t y = (int32_t)fd.div((uint32_t)i), x = (int32_t)i - y * Lx;
-        const int32_t yr = (int32_t)fd.div((uint32_t)r), xr = r - yr * Lx;
-        int32_t dx = x - xr;
-        if (per_x) { if (2 * dx >= Lx) dx -= Lx; else if (2 * dx < -Lx) dx += Lx; }
-        int32_t dy = y - yr;
-        if (per_y) { if (2 * dy >= Ly) dy -= Ly; else if (2 * dy < -Ly) dy += Ly; }
-        const bool leader = (int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31);
-        if constexpr (!kWeighted) {
-            const int32_t sx = __reduce_add_sync(peers, dx);
-            const int32_t sy = __reduce_add_sync(peers, dy);
-            if (leader) {
-                const int32_t k = rank[r];
-                if (k >= 0) {
-                    atomicAdd(&acc[k], (unsigned long long)__popc(peers));
-                    atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)(long long)sx);
-                    atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)(long long)sy);
+__device__ __forceinline__ void acc_add(unsigned long long* __restrict__ acc, int32_t max_comp, int32_t k,
+                                        int64_t n, int64_t sx, int64_t sy, int64_t sw) {
+    atomicAdd(&acc[k], (unsigned long long)n);
+    atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)sx);
+    atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)sy);
+    if constexpr (kWeighted) atomicAdd(&acc[3 * (size_t)max_comp + k], (unsigned long long)sw);
+}
+
+template <bool kWeighted, int kCells>
+__global__ void __launch_bounds__(256) accumulate_kernel(const int32_t* __restrict__ ccl, const float* __restrict__ field,
+                                                         const int32_t* __restrict__ rank, int32_t Lx, int32_t Ly,
+                                                         int per_x, int per_y, FastDiv fd,
+                                                         unsigned long long* __restrict__ acc, int32_t max_comp) {
+    const unsigned full = 0xffffffffu;
+    const int64_t n = (int64_t)Lx * Ly, groups = n / kCells;           // kCells divides Lx
+    const int64_t ground = (groups + 31) / 32 * 32;                    // keep warps converged for the collectives
+    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < ground; g += (int64_t)gridDim.x * blockDim.x) {
+        int32_t r[kCells];
+        float rho[kCells];
+        if (g < groups) {
+            if constexpr (kCells == 4) {
+                const int4 v = __ldcs(reinterpret_cast<const int4*>(ccl) + g);
+                r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w;
+                if constexpr (kWeighted) {
+                    const float4 f = __ldcs(reinterpret_cast<const float4*>(field) + g);
+                    rho[0] = f.x; rho[1] = f.y; rho[2] = f.z; rho[3] = f.w;
                 }
+            } else {
+                r[0] = ccl[g];
+                if constexpr (kWeighted) rho[0] = field[g];
             }
         } else {
-            // 64-bit sums over the peer group: w <= 2^24, |dx| < 2^22, 32 peers
-            const int64_t w = cell_weight(field[i]);
-            int64_t sw = w, sx = w * dx, sy = w * dy;
+#pragma unroll
+            for (int c = 0; c < kCells; ++c) r[c] = -1;
+        }
+        // the thread's label: the first bubble label among its cells
+        int32_t key = -1;
+#pragma unroll
+        for (int c = kCells - 1; c >= 0; --c) key = r[c] >= 0 ? r[c] : key;
+        const bool uniform = __all_sync(full, key == __shfl_sync(full, key, 0));
+        const unsigned peers = uniform ? full : __match_any_sync(full, key);
+        if (key < 0) continue;                                  // whole peer group leaves together
+        const uint32_t i0 = (uint32_t)(g * kCells);
+        const int32_t y = (int32_t)fd.div(i0), x0 = (int32_t)(i0 - (uint32_t)y * (uint32_t)Lx);
+        const int32_t yr = (int32_t)fd.div((uint32_t)key), xr = key - yr * Lx;
+        int32_t dy = y - yr;
+        if (per_y) { if (2 * dy >= Ly) dy -= Ly; else if (2 * dy < -Ly) dy += Ly; }
+        int64_t tn = 0, tsx = 0, tsy = 0, tsw = 0;
+#pragma unroll
+        for (int c = 0; c < kCells; ++c) {
+            if (r[c] < 0) continue;
+            int64_t w = 1;
+            if constexpr (kWeighted) w = cell_weight(rho[c]);
+            if (r[c] == key) {
+                int32_t dx = x0 + c - xr;
+                if (per_x) { if (2 * dx >= Lx) dx -= Lx; else if (2 * dx < -Lx) dx += Lx; }
+                tn += 1; tsx += w * dx; tsy += w * dy; tsw += w;
+            } else {                                            // a second bubble within the same cells
+                const int32_t k2 = rank[r[c]];
+                if (k2 >= 0) {
+                    const int32_t yr2 = (int32_t)fd.div((uint32_t)r[c]), xr2 = r[c] - yr2 * Lx;
+                    int32_t dx = x0 + c - xr2, dy2 = y - yr2;
+                    if (per_x) { if (2 * dx >= Lx) dx -= Lx; else if (2 * dx < -Lx) dx += Lx; }
+                    if (per_y) { if (2 * dy2 >= Ly) dy2 -= Ly; else if (2 * dy2 < -Ly) dy2 += Ly; }
+                    acc_add<kWeighted>(acc, max_comp, k2, 1, w * dx, w * dy2, w);
+                }
+            }
+        }
+        // sums over the peer group; 32-bit reductions when nothing can overflow (no weights: |dx| < 2^22, 128 cells)
+        if constexpr (!kWeighted) {
+            const int32_t pn = __reduce_add_sync(peers, (int32_t)tn);
+            const int32_t px = __reduce_add_sync(peers, (int32_t)tsx);
+            const int32_t py = __reduce_add_sync(peers, (int32_t)tsy);
+            if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
+                const int32_t k = rank[key];
+                if (k >= 0) acc_add<false>(acc, max_comp, k, pn, px, py, 0);
+            }
+        } else {
             if (uniform) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
-                    sw += __shfl_xor_sync(0xffffffffu, sw, o);
-                    sx += __shfl_xor_sync(0xffffffffu, sx, o);
-                    sy += __shfl_xor_sync(0xffffffffu, sy, o);
+                    tn += __shfl_xor_sync(full, tn, o);
+                    tsx += __shfl_xor_sync(full, tsx, o);
+                    tsy += __shfl_xor_sync(full, tsy, o);
+                    tsw += __shfl_xor_sync(full, tsw, o);
                 }
-                if (leader) {
-                    const int32_t k = rank[r];
-                    if (k >= 0) {
-                        atomicAdd(&acc[k], 32ull);
-                        atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)sx);
-                        atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)sy);
-                        atomicAdd(&acc[3 * (size_t)max_comp + k], (unsigned long long)sw);
-                    }
+                if ((threadIdx.x & 31) == 0) {
+                    const int32_t k = rank[key];
+                    if (k >= 0) acc_add<true>(acc, max_comp, k, tn, tsx, tsy, tsw);
                 }
-            } else {                                  // a bubble's edge: every cell adds its own terms
-                const int32_t k = rank[r];
-                if (k >= 0) {
-                    if (leader) atomicAdd(&acc[k], (unsigned long long)__popc(peers));
-                    atomicAdd(&acc[(size_t)max_comp + k], (unsigned long long)sx);
-                    atomicAdd(&acc[2 * (size_t)max_comp + k], (unsigned long long)sy);
-                    atomicAdd(&acc[3 * (size_t)max_comp + k], (unsigned long long)sw);
-                }
+            } else {
+                const int32_t k = rank[key];
+                if (k >= 0) acc_add<true>(acc, max_comp, k, tn, tsx, tsy, tsw);
             }
         }
     }
@@ -574,6 +616,7 @@ extern "C" int field_threshold_ccl(vor_ctx* ctx, const float* d_field, float thr
 extern "C" int field_threshold_ccl_conn(vor_ctx* ctx, const float* d_field, float thr, int above,
                                         int32_t connectivity, int32_t* d_ccl, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_field || !d_ccl) return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: null pointer");
     if (connectivity != 4 && connectivity != 8)
         return vor_fail(ctx, VOR_EINVAL, "field_threshold_ccl: connectivity must be 4 or 8");
@@ -605,6 +648,7 @@ extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, cons
                                         int32_t* d_size, int32_t* d_root, int32_t cap, int32_t* d_n_comp,
                                         void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_ccl || !d_cx || !d_cy || !d_sx || !d_sy || !d_size || !d_root || !d_n_comp || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "field_centroids: null pointer or negative capacity");
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -625,13 +669,19 @@ extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, cons
     VOR_LAUNCH(comp_count_kernel<RootPred>, kCompGrid, kCompThreads, 0, stream, rp, ctx->d_blk_count);
     VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kCompGrid, kCompThreads, 0, stream, rp, rs,
                ctx->d_blk_count);
-    const int grid = (int)((n + 255) / 256 < 8 * kNumSMs ? (n + 255) / 256 : 8 * kNumSMs);
-    if (weighted)
-        VOR_LAUNCH(accumulate_kernel<true>, grid, 256, 0, stream, d_ccl, d_field, ctx->d_rank, ctx->Lx, ctx->Ly,
-                   ctx->per_x, ctx->per_y, make_fastdiv((uint32_t)ctx->Lx), (unsigned long long*)ctx->d_acc, ctx->max_comp);
-    else
-        VOR_LAUNCH(accumulate_kernel<false>, grid, 256, 0, stream, d_ccl, d_field, ctx->d_rank, ctx->Lx, ctx->Ly,
-                   ctx->per_x, ctx->per_y, make_fastdiv((uint32_t)ctx->Lx), (unsigned long long*)ctx->d_acc, ctx->max_comp);
+    {
+        const bool vec = ctx->Lx % kAccCells == 0 && ((uintptr_t)d_ccl & 15) == 0 && (!weighted || ((uintptr_t)d_field & 15) == 0);
+        const int64_t items = vec ? n / kAccCells : n;
+        const int agrid = (int)((items + 255) / 256 < 8 * kNumSMs ? (items + 255) / 256 : 8 * kNumSMs);
+        const FastDiv fd = make_fastdiv((uint32_t)ctx->Lx);
+        unsigned long long* acc = (unsigned long long*)ctx->d_acc;
+#define VOR_ACC(W, C)                                                                                            \
+        VOR_LAUNCH((accumulate_kernel<W, C>), agrid, 256, 0, stream, d_ccl, d_field, ctx->d_rank, ctx->Lx, ctx->Ly, \
+                   ctx->per_x, ctx->per_y, fd, acc, ctx->max_comp)
+        if (weighted) { if (vec) VOR_ACC(true, 4); else VOR_ACC(true, 1); }
+        else { if (vec) VOR_ACC(false, 4); else VOR_ACC(false, 1); }
+#undef VOR_ACC
+    }
     SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
     CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->Lx, ctx->Ly, cap, weighted,
                     d_cx, d_cy, d_sx, d_sy, d_size, d_root, d_n_comp, ctx->d_flags};
@@ -644,6 +694,7 @@ extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, cons
 extern "C" int field_size_histogram(vor_ctx* ctx, const int32_t* d_size, const int32_t* d_n_comp, int32_t cap,
                                     int32_t bin_width, int32_t n_bins, int64_t* d_hist, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_size || !d_n_comp || !d_hist) return vor_fail(ctx, VOR_EINVAL, "field_size_histogram: null pointer");
     if (cap < 0 || bin_width < 1 || n_bins < 1)
         return vor_fail(ctx, VOR_EINVAL, "field_size_histogram: cap >= 0, bin_width >= 1, n_bins >= 1");
@@ -659,6 +710,7 @@ extern "C" int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_p
                            const int32_t* d_n_now, int32_t cap_prev, int32_t cap_now,
                            int32_t radius_fp, int32_t* d_p2n, int32_t* d_n2p, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_px || !d_py || !d_n_prev || !d_nx || !d_ny || !d_n_now || !d_p2n || !d_n2p)
         return vor_fail(ctx, VOR_EINVAL, "match_sites: null pointer");
     if (cap_prev < 1 || cap_now < 1 || radius_fp < 0)

@@ -178,6 +178,7 @@ int field_frame_compute(vor_ctx* ctx, const float* d_field, const FieldArgs& fa,
 
 extern "C" int vor_frame_reset(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     ctx->fr_cur = -1;
     ctx->ff_cur = -1;
     if (ctx->pp_h2d) {                                   // drop frames still in flight
@@ -192,6 +193,7 @@ extern "C" int vor_frame_reset(vor_ctx* ctx) {
 extern "C" int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy,
                                 int32_t n_sites, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     int rc = ensure_frame_buffers(ctx);
     if (rc != VOR_OK) return rc;
     return frame_compute(ctx, d_sx, d_sy, n_sites, ctx->d_fr_created, ctx->d_fr_destroyed, ctx->d_fr_counts,
@@ -202,6 +204,7 @@ extern "C" int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* 
                               uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
                               int64_t* h_counts, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!h_sx || !h_sy || !h_counts || cap < 0 || (cap > 0 && (!h_created || !h_destroyed)))
         return vor_fail(ctx, VOR_EINVAL, "vor_frame_host: null pointer or negative capacity");
     if (n_sites < 1 || n_sites > ctx->max_sites)
@@ -253,6 +256,7 @@ extern "C" int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const u
                                  const uint64_t** d_created, const uint64_t** d_destroyed,
                                  const int64_t** d_counts) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (ctx->fr_cur < 0 || !ctx->d_fr_labels) return vor_fail(ctx, VOR_ESTATE, "no frame processed yet");
     if (d_labels) *d_labels = ctx->d_fr_labels;
     if (d_edges) *d_edges = ctx->d_fr_edges[ctx->fr_cur];
@@ -265,6 +269,7 @@ extern "C" int vor_frame_results(vor_ctx* ctx, const int32_t** d_labels, const u
 extern "C" int vor_frame_submit(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
                                 void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!h_sx || !h_sy) return vor_fail(ctx, VOR_EINVAL, "vor_frame_submit: null pointer");
     if (n_sites < 1 || n_sites > ctx->max_sites)
         return vor_fail(ctx, VOR_EINVAL, "vor_frame_submit: n_sites out of range");
@@ -301,6 +306,7 @@ extern "C" int vor_frame_submit(vor_ctx* ctx, const int32_t* h_sx, const int32_t
 extern "C" int vor_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
                                  int64_t* h_counts) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!h_counts || cap < 0 || (cap > 0 && (!h_created || !h_destroyed)))
         return vor_fail(ctx, VOR_EINVAL, "vor_frame_collect: null pointer or negative capacity");
     if (!ctx->pp_h2d || ctx->pp_tail == ctx->pp_head)
@@ -337,6 +343,7 @@ extern "C" int vor_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_
 extern "C" int field_frame_device(vor_ctx* ctx, const float* d_field, float thr, int above, int32_t min_size,
                                   int32_t radius_fp, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_field || radius_fp < 0) return vor_fail(ctx, VOR_EINVAL, "field_frame_device: null field or negative radius");
     int rc = ensure_frame_buffers(ctx);
     if (rc != VOR_OK || (rc = ensure_field_buffers(ctx)) != VOR_OK) return rc;
@@ -348,6 +355,7 @@ extern "C" int field_frame_device(vor_ctx* ctx, const float* d_field, float thr,
 extern "C" int field_frame_submit(vor_ctx* ctx, const float* h_field, float thr, int above, int32_t min_size,
                                   int32_t radius_fp, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!h_field || radius_fp < 0) return vor_fail(ctx, VOR_EINVAL, "field_frame_submit: null field or negative radius");
     int rc = ensure_frame_buffers(ctx);
     if (rc != VOR_OK || (rc = ensure_field_buffers(ctx)) != VOR_OK || (rc = ensure_pipe_buffers(ctx)) != VOR_OK) return rc;
@@ -375,6 +383,7 @@ extern "C" int field_frame_submit(vor_ctx* ctx, const float* h_field, float thr,
 extern "C" int field_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, int64_t cap,
                                    int64_t* h_counts) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!h_counts || cap < 0 || (cap > 0 && (!h_created || !h_destroyed)))
         return vor_fail(ctx, VOR_EINVAL, "field_frame_collect: null pointer or negative capacity");
     if (!ctx->pp_h2d || !ctx->d_ff_ccl || ctx->pp_tail == ctx->pp_head)
@@ -414,6 +423,7 @@ extern "C" int field_frame_results(vor_ctx* ctx, const int32_t** d_ccl, const in
                                    const uint64_t** d_created, const uint64_t** d_destroyed,
                                    const int64_t** d_counts) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!ctx->d_ff_ccl || ctx->ff_cur < 0) return vor_fail(ctx, VOR_ESTATE, "no field frame processed yet");
     const int32_t K = ctx->max_sites;
     const int32_t* c = ctx->d_ff_comp[ctx->ff_cur];

@@ -977,6 +977,7 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, int32_t x0, int32_t y0,
 
 extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label: null labels");
     if (ctx->nbx <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label: call vor_build_cells first");
     return label_launch(ctx, d_labels, 0, 0, ctx->Lx, ctx->Ly, nullptr, (cudaStream_t)stream_);
@@ -984,6 +985,7 @@ extern "C" int vor_label(vor_ctx* ctx, int32_t* d_labels, void* stream_) {
 
 extern "C" int vor_label_rows(vor_ctx* ctx, int32_t y0, int32_t n_rows, int32_t* d_labels, void* stream_) {
     if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_labels) return vor_fail(ctx, VOR_EINVAL, "vor_label_rows: null labels");
     if (ctx->nbx <= 0) return vor_fail(ctx, VOR_ESTATE, "vor_label_rows: call vor_build_cells first");
     if (y0 < 0 || n_rows < 1 || (int64_t)y0 + n_rows > ctx->Ly)
