@@ -379,3 +379,78 @@ def test_strip_decomposition_on_one_gpu(G):
         v.vor_sync_status()
         assert np.array_equal(G.u64(e, int(ne.item())), ref)
         v.close()
+
+
+# ------------------------------------------------------------------ seeded random sweep over geometries
+def test_random_sweep_frames_on_random_geometries(G):
+    """40 seeded draws of (Lx, Ly, periodicity, site count, motion): three frames each through vor_frame_host
+    (with the fused label -> edge kernel wherever it applies) against the oracle chain on the same geometry -
+    labels, edge counts, created / destroyed lists."""
+    rng = np.random.default_rng(20260)
+    for case in range(40):
+        Lx = int(rng.choice([32, 36, 64, 96, 100, 128, 160, 257, 320]))
+        Ly = int(rng.choice([32, 40, 64, 96, 128, 130, 192, 288]))
+        per = (int(rng.integers(0, 2)), int(rng.integers(0, 2)))
+        spacing = float(rng.choice([3.0, 5.0, 8.0, 12.0, 20.0, 40.0]))
+        if rng.random() < 0.5:
+            sx, sy = jitter_sites(rng, Lx, Ly, spacing)
+        else:
+            sx, sy = rand_sites(rng, Lx, Ly, max(1, int(Lx * Ly / spacing ** 2)))
+        n = len(sx)
+        v = make(Lx, Ly, per, n)
+        fuse = int(rng.integers(0, 2))
+        v.vor_set_option("fuse", fuse)
+        cap = 2 * Lx * Ly + 16
+        hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+        prev = np.empty(0, np.uint64)
+        sigma = float(rng.choice([0.0, 0.3, 2.0])) * FP
+        for t in range(3):
+            v.vor_frame_host(sx, sy, hc, hd, cnt)
+            lab = oracle.label_brute_g(Lx, Ly, per[0], per[1], sx, sy)
+            pl = v.vor_frame_results()[0]
+            got = G.from_device_ptr(pl, Lx * Ly, torch.int32).cpu().numpy().reshape(Ly, Lx)
+            assert np.array_equal(got, lab), (case, t, Lx, Ly, per, n, fuse, int((got != lab).sum()))
+            e = oracle.edges_g(lab, per[0], per[1])
+            rc, rd = oracle.diff(prev, e)
+            assert cnt.tolist() == [len(e), len(rc), len(rd)], (case, t, Lx, Ly, per, n, fuse)
+            assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd), (case, t)
+            prev = e
+            sx = ((sx.astype(np.int64) + np.rint(rng.normal(0, sigma, n)).astype(np.int64)) % (FP * Lx)).astype(np.int32)
+            sy = ((sy.astype(np.int64) + np.rint(rng.normal(0, sigma, n)).astype(np.int64)) % (FP * Ly)).astype(np.int32)
+        v.close()
+
+
+def test_random_sweep_field_chain(G):
+    """24 seeded draws: threshold + bubbles (4 / 8-connected) + centres (weighted or not) + matching between two
+    fields on random geometries, every output against oracle O9."""
+    rng = np.random.default_rng(777)
+    for case in range(24):
+        Lx = int(rng.choice([32, 48, 100, 128, 200, 257]))
+        Ly = int(rng.choice([32, 40, 96, 130, 256]))
+        per = (int(rng.integers(0, 2)), int(rng.integers(0, 2)))
+        conn = int(rng.choice([4, 8]))
+        p = float(rng.choice([0.1, 0.3, 0.45, 0.6]))
+        weighted = bool(rng.integers(0, 2))
+        min_size = int(rng.choice([1, 3, 10]))
+        v = make(Lx, Ly, per, max(16, Lx * Ly // 2))
+        cents = []
+        base = rng.random((Ly, Lx)).astype(np.float32)
+        for t in range(2):
+            f = np.roll(base, (t, 2 * t), axis=(0, 1)) + (rng.random((Ly, Lx)) * 0.05).astype(np.float32)
+            ccl = G.gpu_ccl(v, f, 1.0 - p, True, conn)
+            ref_ccl = oracle.threshold_ccl_g(f, 1.0 - p, True, per[0], per[1], conn)
+            assert np.array_equal(ccl.cpu().numpy().reshape(Ly, Lx), ref_ccl), (case, t)
+            got = G.gpu_centroids(v, ccl, min_size, field=f if weighted else None)
+            ref = oracle.centroids_g(ref_ccl, min_size, per[0], per[1], f if weighted else None)
+            for k in ("sx", "sy", "size", "root"):
+                assert np.array_equal(got[k], ref[k]), (case, t, k)
+            if len(ref["cx"]):
+                assert np.abs(got["cx"] - ref["cx"]).max() <= 1e-9 and np.abs(got["cy"] - ref["cy"]).max() <= 1e-9
+            cents.append(ref)
+        a, b = cents
+        if len(a["sx"]) and len(b["sx"]):
+            R = int(rng.choice([FP, 3 * FP, 6 * FP]))
+            p2n, n2p = G.gpu_match(v, a["sx"], a["sy"], b["sx"], b["sy"], R)
+            r1, r2 = oracle.match_g(Lx, Ly, per[0], per[1], a["sx"], a["sy"], b["sx"], b["sy"], R)
+            assert np.array_equal(p2n, r1) and np.array_equal(n2p, r2), case
+        v.close()
