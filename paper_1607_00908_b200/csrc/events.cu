@@ -325,38 +325,50 @@ struct T1Lists {
     const uint64_t* destroyed; const int64_t* n_destroyed; int64_t cap_destroyed;
 };
 
-__global__ void t1_union_kernel(T1Lists l, const int32_t* __restrict__ trigger, int32_t n, uint64_t* __restrict__ U) {
+// Union list by merge path: every thread owns kT1Merge consecutive slots of the union, finds where they start in
+// the two lists (one co-rank search per thread instead of one search per key), then merges sequentially; the
+// class of a present key follows a cursor in `created` (one lower bound per thread).  The block also counts
+// the couples of its chunk (the chunks are those of the compaction that follows).
+constexpr int kT1Merge = 8;
+
+__global__ void __launch_bounds__(kEvThreads) t1_union_kernel(T1Lists l, const int32_t* __restrict__ trigger, int32_t n,
+                                                              uint64_t* __restrict__ U, int64_t* __restrict__ partial) {
+    __shared__ int64_t sh[32];
     const int64_t nn = min(max(*l.n_now, (int64_t)0), l.cap_now), nc = min(max(*l.n_created, (int64_t)0), l.cap_created),
                   nd = min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nn + nd; k += (int64_t)gridDim.x * blockDim.x) {
-        uint64_t key, bits;
-        int64_t pos;
-        if (k < nn) {
-            key = l.now[k];
-            pos = k + t1_lower_bound(l.destroyed, nd, key);
-            const int64_t c = t1_lower_bound(l.created, nc, key);
-            bits = (c < nc && l.created[c] == key) ? kBitArise : 0;
-        } else {
-            key = l.destroyed[k - nn];
-            pos = (k - nn) + t1_lower_bound(l.now, nn, key);
-            bits = kBitBreak;
-        }
-        const uint32_t i = (uint32_t)(key >> 32), j = (uint32_t)key;
-        const bool keep = i < (uint32_t)n && j < (uint32_t)n && trigger[i] != 0 && trigger[j] != 0;
-        U[pos] = keep ? (key | bits) : kDrop;
-    }
-}
-
-__global__ void __launch_bounds__(kEvThreads) t1_count_kernel(const uint64_t* __restrict__ U, T1Lists l,
-                                                              int64_t* __restrict__ partial) {
-    __shared__ int64_t sh[32];
-    const int64_t m = min(max(*l.n_now, (int64_t)0), l.cap_now) + min(max(*l.n_destroyed, (int64_t)0), l.cap_destroyed);
+    const uint64_t* __restrict__ A = l.now;
+    const uint64_t* __restrict__ B = l.destroyed;
     int64_t beg, end;
-    t1_chunk(m, 32 * kEvItems, &beg, &end);
-    int64_t c = 0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kEvThreads) c += U[i] != kDrop;
-    c = ev_block_sum(c, sh);
-    if (threadIdx.x == 0) partial[blockIdx.x] = c;
+    t1_chunk(nn + nd, 32 * kEvItems, &beg, &end);
+    int64_t kept = 0;
+    for (int64_t d0 = beg + (int64_t)threadIdx.x * kT1Merge; d0 < end; d0 += (int64_t)kEvThreads * kT1Merge) {
+        const int64_t d1 = min(d0 + kT1Merge, end);
+        // co-rank of slot d0: i keys of `now` and d0 - i keys of `destroyed` precede it (the lists are disjoint)
+        int64_t lo = max((int64_t)0, d0 - nd), hi = min(d0, nn);
+        while (lo < hi) {
+            const int64_t mid = (lo + hi) >> 1, j = d0 - mid;
+            if (j > 0 && B[j - 1] > A[mid]) lo = mid + 1; else hi = mid;
+        }
+        int64_t i = lo, j = d0 - lo;
+        int64_t c = i < nn ? t1_lower_bound(l.created, nc, A[i]) : nc;      // cursor in `created`
+        for (int64_t d = d0; d < d1; ++d) {
+            uint64_t key, bits;
+            if (j >= nd || (i < nn && A[i] < B[j])) {
+                key = A[i++];
+                while (c < nc && l.created[c] < key) ++c;
+                bits = (c < nc && l.created[c] == key) ? kBitArise : 0;
+            } else {
+                key = B[j++];
+                bits = kBitBreak;
+            }
+            const uint32_t a = (uint32_t)(key >> 32), b = (uint32_t)key;
+            const bool keep = a < (uint32_t)n && b < (uint32_t)n && trigger[a] != 0 && trigger[b] != 0;
+            U[d] = keep ? (key | bits) : kDrop;
+            kept += keep;
+        }
+    }
+    kept = ev_block_sum(kept, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = kept;
 }
 
 __global__ void __launch_bounds__(kEvThreads) t1_write_kernel(const uint64_t* __restrict__ U, T1Lists l,
@@ -525,11 +537,10 @@ extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t
     VOR_LAUNCH(t1_scan_apply_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
     VOR_LAUNCH(t1_fill_kernel, both, 256, 0, stream, gp, gn, n_labels);
     VOR_LAUNCH(t1_rank_kernel, both, 256, 0, stream, gp, gn, n_labels);
-    VOR_LAUNCH(t1_union_kernel, 2 * grid, 256, 0, stream, l, d_trigger, n_labels, U);
-    VOR_LAUNCH(t1_count_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count);
+    VOR_LAUNCH(t1_union_kernel, grid, kEvThreads, 0, stream, l, d_trigger, n_labels, U, ctx->d_blk_count);
     VOR_LAUNCH(t1_write_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count, d_couples, d_class, cap,
                d_n_couples, ctx->d_flags);
-    VOR_LAUNCH(t1_pair_kernel, 4 * grid, 256, 0, stream, gp, gn, d_couples, d_class, d_n_couples, cap,
+    VOR_LAUNCH(t1_pair_kernel, 16 * grid, 256, 0, stream, gp, gn, d_couples, d_class, d_n_couples, cap,
                d_common_prev, d_common_now, d_partner);
     return VOR_OK;
 }
