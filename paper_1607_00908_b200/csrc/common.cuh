@@ -103,6 +103,7 @@ struct vor_ctx {
     int32_t* d_rank;           // [Lx*Ly] root -> component rank
     int64_t* d_acc;            // [3 * max_comp] n, Sx, Sy
     int32_t* d_comp_root;      // [max_comp]
+    int32_t* d_comp_wcount;    // per-warp counts of the compactions
     int32_t max_comp;
     int32_t* d_comp_count;     // device scalars [4]
     int32_t* d_best;           // [best_cap] best partner per prev / now (lazily sized)

@@ -106,7 +106,7 @@ int vor_destroy(vor_ctx* ctx) {
     cudaFree(ctx->d_rows); cudaFree(ctx->d_row_cnt); cudaFree(ctx->d_n_raw); cudaFree(ctx->d_hist); cudaFree(ctx->d_blk_count);
     cudaFree(ctx->d_tr_prev); cudaFree(ctx->d_tr_now); cudaFree(ctx->d_tr_rowptr[0]); cudaFree(ctx->d_tr_rowptr[1]); cudaFree(ctx->d_tr_counts); cudaFree(ctx->d_dr_scratch);
     for (int k = 0; k < 5; ++k) cudaFree(ctx->d_t1[k]);
-    cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root);
+    cudaFree(ctx->d_rank); cudaFree(ctx->d_acc); cudaFree(ctx->d_comp_root); cudaFree(ctx->d_comp_wcount);
     cudaFree(ctx->d_comp_count); cudaFree(ctx->d_best); cudaFree(ctx->d_mgrid);
     cudaFree(ctx->d_fr_sx); cudaFree(ctx->d_fr_sy); cudaFree(ctx->d_fr_labels);
     cudaFree(ctx->d_fr_edges[0]); cudaFree(ctx->d_fr_edges[1]);

@@ -157,92 +157,77 @@ __global__ void ccl_flatten_kernel(int64_t n, int32_t* __restrict__ parent) {
 }
 
 // ------------------------------------------------------------------------------------ compaction
-// Order-preserving compaction of the items i in [0, n) that satisfy pred(i); persistent chunks.
+// Order-preserving compaction of the items i in [0, n) that satisfy pred(i).  Every WARP owns one contiguous
+// range of whole 256-item tiles; consecutive ranges go to different blocks, so that short lists spread over
+// the SMs.  The count kernel leaves one count per warp; the write kernel derives every warp's offset from
+// those (row sums over the blocks, in the block's prologue) and then each warp streams its range with
+// ballots only - no barrier inside the loop.
 constexpr int kCompThreads = 512;
-constexpr int kCompItems = 8;                      // items per thread per batch (warp-strided: coalesced)
-constexpr int kCompBatch = kCompThreads * kCompItems;
-constexpr int kCompGrid = 4 * kNumSMs;             // <= 2 * kMaxCoopBlocks entries of d_blk_count
+constexpr int kCompWarps = kCompThreads / 32;
+constexpr int kCompItems = 8;                      // items per lane per tile (warp-strided: coalesced)
+constexpr int kCompTile = 32 * kCompItems;
+constexpr int kCompGrid = 4 * kNumSMs;             // kCompWarps * kCompGrid warp counts in ctx->d_comp_wcount
 
-__device__ __forceinline__ void comp_chunk(int64_t n, int64_t* beg, int64_t* end) {
-    // chunks are whole warp tiles (32 x kCompItems items), so that short lists spread over many blocks
-    int64_t C = (n + gridDim.x - 1) / gridDim.x;
-    C = (C + 32 * kCompItems - 1) / (32 * kCompItems) * (32 * kCompItems);
-    int64_t s = (int64_t)blockIdx.x * C;
+// range of warp W = wid * gridDim.x + blockIdx.x among gridDim.x * kCompWarps warps
+__device__ __forceinline__ void comp_range(int64_t n, int64_t* beg, int64_t* end) {
+    const int64_t nw = (int64_t)gridDim.x * kCompWarps, W = (int64_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    int64_t C = (n + nw - 1) / nw;
+    C = (C + kCompTile - 1) / kCompTile * kCompTile;
+    const int64_t s = W * C;
     *beg = s < n ? s : n;
     *end = s + C < n ? s + C : n;
 }
 
-__device__ __forceinline__ int64_t comp_block_sum(int64_t v, int64_t* sh) {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) sh[wid] = v;
-    __syncthreads();
-    int64_t t = lane < (int)(blockDim.x >> 5) ? sh[lane] : 0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    __syncthreads();
-    return t;
-}
-
 template <typename Pred>
-__global__ void __launch_bounds__(kCompThreads) comp_count_kernel(Pred pred, int64_t* __restrict__ blk_count) {
-    __shared__ int64_t sh[32];
-    const int64_t n = pred.size();
+__global__ void __launch_bounds__(kCompThreads) comp_count_kernel(Pred pred, int32_t* __restrict__ wcount) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int64_t beg, end;
-    comp_chunk(n, &beg, &end);
-    int64_t c = 0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kCompThreads) c += pred(i);
-    c = comp_block_sum(c, sh);
-    if (threadIdx.x == 0) blk_count[blockIdx.x] = c;
+    comp_range(pred.size(), &beg, &end);
+    int32_t c = 0;
+    for (int64_t i = beg + lane; i < end; i += 32) c += pred(i);
+    c = __reduce_add_sync(0xffffffffu, c);
+    if (lane == 0) wcount[wid * gridDim.x + blockIdx.x] = c;
 }
 
 template <typename Pred, typename Sink>
 __global__ void __launch_bounds__(kCompThreads) comp_write_kernel(Pred pred, Sink sink,
-                                                                  const int64_t* __restrict__ blk_count) {
-    __shared__ int64_t sh[32];
-    __shared__ int32_t wtot[kCompThreads / 32];
+                                                                  const int32_t* __restrict__ wcount) {
+    __shared__ int64_t rowsum[kCompWarps];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t n = pred.size();
-    int64_t beg, end;
-    comp_chunk(n, &beg, &end);
-    int64_t before = 0, all = 0;
-    for (int b = threadIdx.x; b < (int)gridDim.x; b += kCompThreads) {
-        const int64_t v = blk_count[b];
-        all += v;
-        if (b < (int)blockIdx.x) before += v;
+    const int G = gridDim.x;
+    // warp `wid` sums row `wid` of the counts: all of it, and the part that belongs to earlier blocks
+    int64_t rs = 0, rp = 0;
+    for (int b = lane; b < G; b += 32) {
+        const int64_t v = wcount[wid * G + b];
+        rs += v;
+        if (b < (int)blockIdx.x) rp += v;
     }
-    before = comp_block_sum(before, sh);
-    all = comp_block_sum(all, sh);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { rs += __shfl_xor_sync(0xffffffffu, rs, o); rp += __shfl_xor_sync(0xffffffffu, rp, o); }
+    if (lane == 0) rowsum[wid] = rs;
+    __syncthreads();
+    int64_t run = rp, all = 0;
+#pragma unroll
+    for (int w = 0; w < kCompWarps; ++w) {
+        const int64_t t = rowsum[w];
+        all += t;
+        if (w < wid) run += t;
+    }
     if (blockIdx.x == 0 && threadIdx.x == 0) sink.total(all);
-    int64_t run = before;
-    for (int64_t sub = beg; sub < end; sub += kCompBatch) {
-        // warp w owns items [sub + 256 w, sub + 256 w + 256): item = base + 32 k + lane, k = 0..7
-        const int64_t wb = sub + (int64_t)wid * (32 * kCompItems) + lane;
+    int64_t beg, end;
+    comp_range(pred.size(), &beg, &end);
+    for (int64_t sub = beg; sub < end; sub += kCompTile) {
         unsigned ball[kCompItems];
-        int32_t mine = 0;
 #pragma unroll
         for (int k = 0; k < kCompItems; ++k) {
-            const int64_t i = wb + 32 * k;
+            const int64_t i = sub + 32 * k + lane;
             ball[k] = __ballot_sync(0xffffffffu, i < end && pred(i));
-            mine += __popc(ball[k]);
         }
-        if (lane == 0) wtot[wid] = mine;
-        __syncthreads();
-        int32_t wbase = 0, total = 0;
-        for (int w = 0; w < kCompThreads / 32; ++w) {
-            const int32_t t = wtot[w];
-            if (w < wid) wbase += t;
-            total += t;
-        }
-        int64_t pos = run + wbase;
 #pragma unroll
         for (int k = 0; k < kCompItems; ++k) {
-            if (ball[k] >> lane & 1u) sink.put(pos + __popc(ball[k] & ((1u << lane) - 1u)), wb + 32 * k);
-            pos += __popc(ball[k]);
+            if (ball[k] >> lane & 1u) sink.put(run + __popc(ball[k] & ((1u << lane) - 1u)), sub + 32 * k + lane);
+            run += __popc(ball[k]);
         }
-        run += total;
-        __syncthreads();
     }
 }
 
@@ -661,14 +646,15 @@ extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, cons
         VOR_CUDA(cudaMalloc((void**)&ctx->d_rank, n * sizeof(int32_t)));
         VOR_CUDA(cudaMalloc((void**)&ctx->d_acc, 4 * (size_t)mc * sizeof(int64_t)));
         VOR_CUDA(cudaMalloc((void**)&ctx->d_comp_root, (size_t)mc * sizeof(int32_t)));
+        VOR_CUDA(cudaMalloc((void**)&ctx->d_comp_wcount, (size_t)kCompWarps * kCompGrid * sizeof(int32_t)));
     }
     const int weighted = d_field != nullptr;
     RootPred rp{d_ccl, n};
     RootSink rs{ctx->d_comp_root, ctx->d_rank, ctx->max_comp, &ctx->d_comp_count[0], ctx->d_flags,
                 (long long*)ctx->d_acc, weighted ? 4 : 3};
-    VOR_LAUNCH(comp_count_kernel<RootPred>, kCompGrid, kCompThreads, 0, stream, rp, ctx->d_blk_count);
+    VOR_LAUNCH(comp_count_kernel<RootPred>, kCompGrid, kCompThreads, 0, stream, rp, ctx->d_comp_wcount);
     VOR_LAUNCH((comp_write_kernel<RootPred, RootSink>), kCompGrid, kCompThreads, 0, stream, rp, rs,
-               ctx->d_blk_count);
+               ctx->d_comp_wcount);
     {
         const bool vec = ctx->Lx % kAccCells == 0 && ((uintptr_t)d_ccl & 15) == 0 && (!weighted || ((uintptr_t)d_field & 15) == 0);
         const int64_t items = vec ? n / kAccCells : n;
@@ -685,9 +671,9 @@ extern "C" int field_centroids_weighted(vor_ctx* ctx, const int32_t* d_ccl, cons
     SizePred sp{(const long long*)ctx->d_acc, &ctx->d_comp_count[0], min_size};
     CentroidSink cs{(const long long*)ctx->d_acc, ctx->d_comp_root, ctx->max_comp, ctx->Lx, ctx->Ly, cap, weighted,
                     d_cx, d_cy, d_sx, d_sy, d_size, d_root, d_n_comp, ctx->d_flags};
-    VOR_LAUNCH(comp_count_kernel<SizePred>, kCompGrid, kCompThreads, 0, stream, sp, ctx->d_blk_count);
+    VOR_LAUNCH(comp_count_kernel<SizePred>, kCompGrid, kCompThreads, 0, stream, sp, ctx->d_comp_wcount);
     VOR_LAUNCH((comp_write_kernel<SizePred, CentroidSink>), kCompGrid, kCompThreads, 0, stream, sp, cs,
-               ctx->d_blk_count);
+               ctx->d_comp_wcount);
     return VOR_OK;
 }
 
