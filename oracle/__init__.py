@@ -282,6 +282,17 @@ def edge_commons(edges, n):
     return out
 
 
+def event_vertices(prev, now, n):
+    """O10: boundary vertices of both triangulations and the bulk / boundary event class of every active vertex
+    (PAPER.md:248-256)."""
+    prev = np.ascontiguousarray(prev, dtype=np.uint64)
+    now = np.ascontiguousarray(now, dtype=np.uint64)
+    bp = np.zeros(n, np.int32); bn = np.zeros(n, np.int32); vc = np.zeros(n, np.int32)
+    lib().orc_event_vertices(_p(prev, C.c_uint64), C.c_int64(len(prev)), _p(now, C.c_uint64), C.c_int64(len(now)),
+                             C.c_int32(n), _p(bp, C.c_int32), _p(bn, C.c_int32), _p(vc, C.c_int32))
+    return dict(boundary_prev=bp, boundary_now=bn, vclass=vc)
+
+
 def unpack(keys):
     """uint64 packed keys -> (i, j) int64 arrays."""
     keys = np.asarray(keys, dtype=np.uint64)

@@ -732,6 +732,48 @@ void orc_edge_commons(const u64* edges, i64 n_edges, int32_t n, int32_t* commons
     }
 }
 
+// O10 — bulk and boundary vertices of an event (§III.B.4): "two points connected by a boundary
+// edge belong to the boundary" (a boundary edge: its end points share only one neighbour); a point is involved
+// in a BULK event if it is "connected to, at least, three other active points", in a BOUNDARY event if it is
+// "connected to, at least, one other active boundary point" - for each of the two triangulations.
+// Inputs as O7 (two ascending unique lists in one index space, n vertices); active = O7's trigger.
+// Outputs: boundary_prev[n], boundary_now[n] (0/1, for every vertex), vclass[n] = bit 0 bulk event in D_P,
+// bit 1 boundary event in D_P, bit 2 bulk event in D_N, bit 3 boundary event in D_N; 0 for inactive vertices.
+void orc_event_vertices(const u64* prev, i64 n_prev, const u64* now, i64 n_now, int32_t n,
+                        int32_t* boundary_prev, int32_t* boundary_now, int32_t* vclass) {
+    std::vector<std::set<int32_t>> row[2];
+    row[0].resize(n); row[1].resize(n);
+    const u64* lists[2] = {prev, now};
+    const i64 counts[2] = {n_prev, n_now};
+    for (int t = 0; t < 2; ++t)
+        for (i64 k = 0; k < counts[t]; ++k) {
+            const int32_t i = (int32_t)(lists[t][k] >> 32), j = (int32_t)(lists[t][k] & 0xffffffffu);
+            if (i < n && j < n) { row[t][i].insert(j); row[t][j].insert(i); }
+        }
+    std::vector<char> active(n);
+    for (int32_t v = 0; v < n; ++v) active[v] = row[0][v] != row[1][v];
+    int32_t* boundary[2] = {boundary_prev, boundary_now};
+    for (int t = 0; t < 2; ++t)
+        for (int32_t v = 0; v < n; ++v) {
+            boundary[t][v] = 0;
+            for (int32_t u : row[t][v]) {
+                int32_t shared = 0;
+                for (int32_t w : row[t][v]) shared += (int32_t)row[t][u].count(w);
+                if (shared == 1) boundary[t][v] = 1;
+            }
+        }
+    for (int32_t v = 0; v < n; ++v) {
+        vclass[v] = 0;
+        if (!active[v]) continue;
+        for (int t = 0; t < 2; ++t) {
+            int32_t act = 0, bnd = 0;
+            for (int32_t u : row[t][v]) { act += active[u]; bnd += active[u] && boundary[t][u]; }
+            if (act >= 3) vclass[v] |= 1 << (2 * t);
+            if (bnd >= 1) vclass[v] |= 2 << (2 * t);
+        }
+    }
+}
+
 int orc_num_threads(int threads) { return resolve_threads(threads); }
 
 }  // extern "C"

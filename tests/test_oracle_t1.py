@@ -136,3 +136,83 @@ def test_rhombus_construction_golden():
     assert r["common_prev"][k.index(b)] == g["breaking_common_prev"][0]
     assert r["common_now"][k.index(a)] == g["arising_common_now"][0]
     assert (r["common_prev"][r["cls"] == 0] == 2).all() and (r["common_now"][r["cls"] == 0] == 2).all()
+
+
+# ------------------------------------------------------------------ O10: bulk / boundary vertices of an event
+def brute_vertices(prev_pairs, now_pairs, n):
+    def rows(ps):
+        r = [set() for _ in range(n)]
+        for i, j in ps:
+            if i < n and j < n:
+                r[i].add(j); r[j].add(i)
+        return r
+    R = [rows(prev_pairs), rows(now_pairs)]
+    act = [R[0][v] != R[1][v] for v in range(n)]
+    bnd = [[int(any(len(r[v] & r[u]) == 1 for u in r[v])) for v in range(n)] for r in R]
+    vc = []
+    for v in range(n):
+        c = 0
+        if act[v]:
+            for t, r in enumerate(R):
+                if sum(act[u] for u in r[v]) >= 3:
+                    c |= 1 << (2 * t)
+                if any(act[u] and bnd[t][u] for u in r[v]):
+                    c |= 2 << (2 * t)
+        vc.append(c)
+    return bnd[0], bnd[1], vc
+
+
+def check_vertices(prev_pairs, now_pairs, n):
+    r = oracle.event_vertices(pack(prev_pairs), pack(now_pairs), n)
+    bp, bn, vc = brute_vertices(prev_pairs, now_pairs, n)
+    assert r["boundary_prev"].tolist() == bp and r["boundary_now"].tolist() == bn and r["vclass"].tolist() == vc
+    return r
+
+
+def test_event_vertices_bulk_t1_and_boundary_event():
+    # Fig. 8 top: the T1 of the rhombus 0-1-2-3 inside closed triangles.  In D_P the end points of the breaking
+    # link (1, 3) see three active points, in D_N those of the arising link (0, 2) do: bulk events, no boundary
+    common = [(0, 1), (1, 2), (2, 3), (0, 3), (0, 4), (1, 4), (2, 5), (3, 5), (4, 5)]
+    r = check_vertices(common + [(1, 3)], common + [(0, 2)], 6)
+    assert [c & 5 for c in r["vclass"].tolist()[:4]] == [4, 1, 4, 1] and r["vclass"].tolist()[4:] == [0, 0]
+    # the same flip inside a triangulation of the torus (the rhombus construction): no boundary anywhere, so the
+    # four points carry exactly the bulk bit of the triangulation in which they see three active points
+    g = read_golden("rhombus_flip.txt")
+    lists = []
+    for h in (g["h_prev"][0], g["h_now"][0]):
+        sx, sy = rhombus_sites(g["L"][0], h)
+        lists.append(oracle.edges(oracle.label_brute(g["L"][0], sx, sy)))
+    t = oracle.event_vertices(lists[0], lists[1], g["n_sites"][0])
+    assert t["boundary_prev"].sum() == 0 and t["boundary_now"].sum() == 0
+    assert t["vclass"].tolist()[:4] == [4, 1, 4, 1] and t["vclass"][4:].sum() == 0
+    # Fig. 8 bottom: a triangle loses one side.  All three sides are boundary edges (one common neighbour); the
+    # two active end points are connected in D_P to an active boundary point (each other): a boundary event
+    r = check_vertices([(0, 1), (1, 2), (0, 2)], [(0, 1), (1, 2)], 3)
+    assert r["boundary_prev"].tolist() == [1, 1, 1] and r["boundary_now"].tolist() == [0, 0, 0]
+    assert r["vclass"].tolist() == [2, 0, 2]
+    # the zig-zag strip of triangles: every vertex lies on the boundary; nothing active, no class
+    strip = [(0, 1), (0, 2), (1, 2), (1, 3), (2, 3), (2, 4), (3, 4), (3, 5), (4, 5)]
+    r = check_vertices(strip, strip, 6)
+    assert r["boundary_prev"].tolist() == [1] * 6 and r["vclass"].tolist() == [0] * 6
+    # a vertex in both kinds of event at once (Fig. 9): hub 0 of a fan loses two spokes of its rim
+    fan = [(0, k) for k in range(1, 7)] + [(k, k + 1) for k in range(1, 6)]
+    r = check_vertices(fan, [e for e in fan if e not in ((0, 1), (0, 3))], 7)
+    assert r["vclass"][0] & 1 == 0 and r["vclass"][0] & 2                     # D_P: two active neighbours, on the rim
+
+
+def test_event_vertices_random_graphs_and_torus():
+    rng = np.random.default_rng(31)
+    for n in (4, 9, 20, 40):
+        allp = [(i, j) for i in range(n) for j in range(i + 1, n)]
+        for _ in range(6):
+            a = [p for p in allp if rng.random() < 0.3]
+            b = sorted(set([p for p in a if rng.random() < 0.85] + [p for p in allp if rng.random() < 0.04]))
+            check_vertices(a, b, n)
+    check_vertices([(0, 1), (1, 2), (0, 2), (1, 5)], [(0, 1), (1, 2), (2, 6)], 3)     # labels >= n are ignored
+    # a well-resolved triangulation of the torus has no boundary vertex (every edge has two common neighbours)
+    from helpers import hex_sites
+    L = 256
+    sx, sy = hex_sites(L, 16, 18, 0.8, seed=3)
+    e = oracle.edges(oracle.label_brute(L, sx, sy))
+    r = oracle.event_vertices(e, e, len(sx))
+    assert r["boundary_prev"].sum() == 0 and r["vclass"].sum() == 0
