@@ -241,6 +241,18 @@ int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
 int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int64_t* d_n_edges, int64_t cap_edges,
                      int32_t n_labels, int32_t* d_commons, void* stream);
 
+/* Bulk and boundary vertices of an event (§III.B.4): "two points connected by a boundary edge
+ * belong to the boundary"; an active point takes part in a BULK event if it is "connected to, at least, three
+ * other active points", in a BOUNDARY event if it is "connected to, at least, one other active boundary point" -
+ * evaluated in each of the two triangulations.  Lists, counts, capacities and d_trigger as for vor_t1_events.
+ * Outputs (device, n_labels entries each): d_boundary_prev / d_boundary_now 1 for a boundary vertex of the past /
+ * present triangulation, else 0; d_vclass bit 0 bulk event in D_P, bit 1 boundary event in D_P, bit 2 bulk
+ * event in D_N, bit 3 boundary event in D_N, 0 for inactive vertices. */
+int vor_event_vertices(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+                       const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
+                       const int32_t* d_trigger, int32_t n_labels, int32_t* d_boundary_prev,
+                       int32_t* d_boundary_now, int32_t* d_vclass, void* stream);
+
 /* ---- a6: bubble identification (§III.A: threshold -> two-valued variable ->
  * cluster labelling).  mask = above ? field > thr : field < thr (strict; NaN -> background).
  * 4-connected periodic components; d_ccl[c] = smallest linear index in c's component, or -1. */

@@ -38,6 +38,7 @@ SIGNATURES = {
     "vor_label_rows": (C.c_int, [_P, C.c_int32, C.c_int32, _P, _P]),
     "vor_paint_obstacles": (C.c_int, [_P, _P, C.c_int32, _P, C.c_int32, _P]),
     "vor_edges_image": (C.c_int, [_P, _P, C.c_int32, C.c_int32, C.c_int32, _P, C.c_int64, _P, _P, _P]),
+    "vor_event_vertices": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, C.c_int32, _P, _P, _P, _P]),
     "vor_merge_lists": (C.c_int, [_P, _P, C.c_int64, _P, C.c_int32, C.c_int32, _P, C.c_int64, _P, _P]),
     "vor_edge_commons": (C.c_int, [_P, _P, _P, C.c_int64, C.c_int32, _P, _P]),
     "field_threshold_ccl_conn": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, _P, _P]),
@@ -215,6 +216,13 @@ class Vor:
         self._check(self.lib.vor_edges_image(self.h, _ptr(labels, torch.int32), labels.numel() // self.Lx,
                                              1 if wrap_y else 0, exclude, _ptr(edges, torch.int64), edges.numel(),
                                              _ptr(n_edges, torch.int64), _ptr(row_ptr, torch.int32), _stream()))
+
+    def vor_event_vertices(self, prev, n_prev, now, n_now, trigger, boundary_prev, boundary_now, vclass):
+        n_labels = min(t.numel() for t in (trigger, boundary_prev, boundary_now, vclass))
+        i64, i32 = torch.int64, torch.int32
+        self._check(self.lib.vor_event_vertices(
+            self.h, _ptr(prev, i64), _ptr(n_prev, i64), _ptr(now, i64), _ptr(n_now, i64), prev.numel(), now.numel(),
+            _ptr(trigger, i32), n_labels, _ptr(boundary_prev, i32), _ptr(boundary_now, i32), _ptr(vclass, i32), _stream()))
 
     def vor_merge_lists(self, lists, counts, n_labels: int, out, n_out):
         """lists: int64[n_lists, stride] (row l = list l), counts: int64[n_lists] device."""

@@ -498,6 +498,36 @@ int t1_scratch(vor_ctx* ctx, int slot, size_t bytes, void** out) {
 
 }  // namespace
 
+// Both triangulations as symmetric adjacency lists with sorted rows in the context's scratch.
+static int t1_graphs(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev, const uint64_t* d_now,
+                     const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now, int32_t n_labels, T1Graph* gp,
+                     T1Graph* gn) {
+    const size_t n1 = (size_t)n_labels + 1;
+    uint32_t *deg, *off, *adj_u, *adj_s;
+    int rc;
+    const size_t n_adj = 2 * (size_t)(cap_prev + cap_now) + 1;
+    if ((rc = t1_scratch(ctx, 0, 2 * n1 * sizeof(uint32_t), (void**)&deg)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 1, 2 * n1 * sizeof(uint32_t), (void**)&off)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 2, n_adj * sizeof(uint32_t), (void**)&adj_u)) != VOR_OK) return rc;
+    if ((rc = t1_scratch(ctx, 3, n_adj * sizeof(uint32_t), (void**)&adj_s)) != VOR_OK) return rc;
+    *gp = T1Graph{d_prev, d_n_prev, cap_prev, deg, off, adj_u, adj_s};
+    *gn = T1Graph{d_now, d_n_now, cap_now, deg + n1, off + n1, adj_u + 2 * cap_prev, adj_s + 2 * cap_prev};
+    return VOR_OK;
+}
+
+static int t1_build_graphs(vor_ctx* ctx, const T1Graph& gp, const T1Graph& gn, int32_t n_labels, cudaStream_t stream) {
+    const size_t n1 = (size_t)n_labels + 1;
+    VOR_CUDA(cudaMemsetAsync(gp.deg, 0, 2 * n1 * sizeof(uint32_t), stream));
+    const int grid = 4 * ctx->num_sms;
+    const dim3 both(grid, 2);
+    VOR_LAUNCH(t1_degree_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    VOR_LAUNCH(t1_scan_sum_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_scan_apply_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
+    VOR_LAUNCH(t1_fill_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    VOR_LAUNCH(t1_rank_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    return VOR_OK;
+}
+
 extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
                              const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
                              const uint64_t* d_created, const int64_t* d_n_created,
@@ -515,28 +545,15 @@ extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t
     if (2 * (cap_prev + cap_now) >= ((int64_t)1 << 32))
         return vor_fail(ctx, VOR_EINVAL, "vor_t1_events: cap_prev + cap_now must be below 2^31");
     cudaStream_t stream = (cudaStream_t)stream_;
-    const size_t n1 = (size_t)n_labels + 1;
-    uint32_t *deg, *off, *adj_u, *adj_s;
     uint64_t* U;
     int rc;
-    const size_t n_adj = 2 * (size_t)(cap_prev + cap_now) + 1;
-    if ((rc = t1_scratch(ctx, 0, 2 * n1 * sizeof(uint32_t), (void**)&deg)) != VOR_OK) return rc;
-    if ((rc = t1_scratch(ctx, 1, 2 * n1 * sizeof(uint32_t), (void**)&off)) != VOR_OK) return rc;
-    if ((rc = t1_scratch(ctx, 2, n_adj * sizeof(uint32_t), (void**)&adj_u)) != VOR_OK) return rc;
-    if ((rc = t1_scratch(ctx, 3, n_adj * sizeof(uint32_t), (void**)&adj_s)) != VOR_OK) return rc;
+    T1Graph gp, gn;
+    if ((rc = t1_graphs(ctx, d_prev, d_n_prev, d_now, d_n_now, cap_prev, cap_now, n_labels, &gp, &gn)) != VOR_OK) return rc;
     if ((rc = t1_scratch(ctx, 4, ((size_t)(cap_now + cap_destroyed) + 1) * sizeof(uint64_t), (void**)&U)) != VOR_OK) return rc;
-    T1Graph gp{d_prev, d_n_prev, cap_prev, deg, off, adj_u, adj_s};
-    T1Graph gn{d_now, d_n_now, cap_now, deg + n1, off + n1, adj_u + 2 * cap_prev, adj_s + 2 * cap_prev};
     T1Lists l{d_now, d_n_now, cap_now, d_created, d_n_created, cap_created, d_destroyed, d_n_destroyed, cap_destroyed};
 
-    VOR_CUDA(cudaMemsetAsync(deg, 0, 2 * n1 * sizeof(uint32_t), stream));
     const int grid = 4 * ctx->num_sms;                      // 2 * grid partials <= 2 * kMaxCoopBlocks
-    const dim3 both(grid, 2);
-    VOR_LAUNCH(t1_degree_kernel, both, 256, 0, stream, gp, gn, n_labels);
-    VOR_LAUNCH(t1_scan_sum_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
-    VOR_LAUNCH(t1_scan_apply_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
-    VOR_LAUNCH(t1_fill_kernel, both, 256, 0, stream, gp, gn, n_labels);
-    VOR_LAUNCH(t1_rank_kernel, both, 256, 0, stream, gp, gn, n_labels);
+    if ((rc = t1_build_graphs(ctx, gp, gn, n_labels, stream)) != VOR_OK) return rc;
     VOR_LAUNCH(t1_union_kernel, grid, kEvThreads, 0, stream, l, d_trigger, n_labels, U, ctx->d_blk_count);
     VOR_LAUNCH(t1_write_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count, d_couples, d_class, cap,
                d_n_couples, ctx->d_flags);
@@ -587,5 +604,74 @@ extern "C" int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int
     VOR_LAUNCH(t1_fill_kernel, one, 256, 0, stream, g, g, n_labels);
     VOR_LAUNCH(t1_rank_kernel, one, 256, 0, stream, g, g, n_labels);
     VOR_LAUNCH(edge_commons_kernel, 4 * grid, 256, 0, stream, g, n_labels, d_commons);
+    return VOR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Bulk and boundary vertices of an event: boundary vertices = end points of an edge with
+// exactly one common neighbour; an active vertex takes part in a bulk event of a triangulation if at least
+// three of its neighbours there are active, in a boundary event if at least one of them is an active boundary
+// vertex.
+namespace {
+
+// blockIdx.y selects the triangulation; every boundary edge marks its two end points
+__global__ void ev_boundary_kernel(T1Graph gp, T1Graph gn, int32_t n, int32_t* __restrict__ boundary_prev,
+                                   int32_t* __restrict__ boundary_now) {
+    const T1Graph& g = blockIdx.y ? gn : gp;
+    int32_t* __restrict__ out = blockIdx.y ? boundary_now : boundary_prev;
+    const int64_t m = t1_len(g);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < m; k += (int64_t)gridDim.x * blockDim.x) {
+        uint32_t i, j, c2[2];
+        if (!t1_edge(g, k, n, &i, &j)) continue;
+        if (t1_common(g, i, j, c2) == 1) { out[i] = 1; out[j] = 1; }
+    }
+}
+
+__global__ void ev_vclass_kernel(T1Graph gp, T1Graph gn, const int32_t* __restrict__ trigger, int32_t n,
+                                 const int32_t* __restrict__ boundary_prev, const int32_t* __restrict__ boundary_now,
+                                 int32_t* __restrict__ vclass) {
+    for (int32_t v = blockIdx.x * blockDim.x + threadIdx.x; v < n; v += gridDim.x * blockDim.x) {
+        int32_t c = 0;
+        if (trigger[v]) {
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const T1Graph& g = t ? gn : gp;
+                const int32_t* __restrict__ bnd = t ? boundary_now : boundary_prev;
+                int32_t act = 0, ab = 0;
+                for (uint32_t p = g.off[v]; p < g.off[v + 1]; ++p) {
+                    const uint32_t u = g.adj_s[p];
+                    if (trigger[u]) { ++act; ab += bnd[u]; }
+                }
+                if (act >= 3) c |= 1 << (2 * t);
+                if (ab >= 1) c |= 2 << (2 * t);
+            }
+        }
+        vclass[v] = c;
+    }
+}
+
+}  // namespace
+
+extern "C" int vor_event_vertices(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_prev,
+                                  const uint64_t* d_now, const int64_t* d_n_now, int64_t cap_prev, int64_t cap_now,
+                                  const int32_t* d_trigger, int32_t n_labels, int32_t* d_boundary_prev,
+                                  int32_t* d_boundary_now, int32_t* d_vclass, void* stream_) {
+    if (!ctx) return VOR_EINVAL;
+    if (int drc_ = vor_check_device(ctx)) return drc_;
+    if (!d_prev || !d_n_prev || !d_now || !d_n_now || !d_trigger || !d_boundary_prev || !d_boundary_now || !d_vclass)
+        return vor_fail(ctx, VOR_EINVAL, "vor_event_vertices: null pointer");
+    if (n_labels < 1 || cap_prev < 0 || cap_now < 0 || 2 * (cap_prev + cap_now) >= ((int64_t)1 << 32))
+        return vor_fail(ctx, VOR_EINVAL, "vor_event_vertices: n_labels >= 1, capacities >= 0, cap_prev + cap_now < 2^31");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    int rc;
+    T1Graph gp, gn;
+    if ((rc = t1_graphs(ctx, d_prev, d_n_prev, d_now, d_n_now, cap_prev, cap_now, n_labels, &gp, &gn)) != VOR_OK) return rc;
+    if ((rc = t1_build_graphs(ctx, gp, gn, n_labels, stream)) != VOR_OK) return rc;
+    VOR_CUDA(cudaMemsetAsync(d_boundary_prev, 0, (size_t)n_labels * sizeof(int32_t), stream));
+    VOR_CUDA(cudaMemsetAsync(d_boundary_now, 0, (size_t)n_labels * sizeof(int32_t), stream));
+    const int grid = 4 * ctx->num_sms;
+    VOR_LAUNCH(ev_boundary_kernel, dim3(4 * grid, 2), 256, 0, stream, gp, gn, n_labels, d_boundary_prev, d_boundary_now);
+    VOR_LAUNCH(ev_vclass_kernel, 4 * grid, 256, 0, stream, gp, gn, d_trigger, n_labels, d_boundary_prev, d_boundary_now,
+               d_vclass);
     return VOR_OK;
 }

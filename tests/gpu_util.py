@@ -171,6 +171,25 @@ def gpu_t1(v: Vor, prev, now, n, cap=None):
                 overflow=overflow)
 
 
+def gpu_event_vertices(v: Vor, prev, now, n):
+    """vor_diff -> vor_events -> vor_event_vertices on host lists; returns the same dict as oracle.event_vertices()."""
+    mk = lambda a: dev(np.asarray(a, np.uint64).view(np.int64)) if len(a) else torch.empty(1, dtype=torch.int64, device="cuda")
+    dp, dn = mk(prev), mk(now)
+    i64 = dict(dtype=torch.int64, device="cuda"); i32 = dict(dtype=torch.int32, device="cuda")
+    npv, nnv = torch.tensor([len(prev)], **i64), torch.tensor([len(now)], **i64)
+    lc = max(1, len(prev) + len(now))
+    c, d = torch.empty(lc, **i64), torch.empty(lc, **i64)
+    nc, nd = torch.zeros(1, **i64), torch.zeros(1, **i64)
+    v.vor_diff(dp, npv, dn, nnv, c, d, nc, nd)
+    trig, idx, cp, cn = (torch.empty(n, **i32) for _ in range(4))
+    m, g = torch.zeros(1, **i32), torch.zeros(1, **i32)
+    v.vor_events(dp, npv, dn, nnv, c, nc, d, nd, trig, idx, m, g, cp, cn)
+    bp, bn, vc = (torch.full((n,), -9, **i32) for _ in range(3))
+    v.vor_event_vertices(dp, npv, dn, nnv, trig, bp, bn, vc)
+    v.vor_sync_status()
+    return dict(boundary_prev=bp.cpu().numpy(), boundary_now=bn.cpu().numpy(), vclass=vc.cpu().numpy())
+
+
 def gpu_ccl(v: Vor, field, thr, above=True, connectivity=None):
     f = dev(field.astype(np.float32).ravel())
     ccl = torch.empty(v.cells, dtype=torch.int32, device="cuda")

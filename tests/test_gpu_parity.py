@@ -805,6 +805,45 @@ def test_t1_events_hand_graphs_random_graphs_and_golden(G):
     v.close()
 
 
+def test_event_vertices_bulk_and_boundary(G):
+    def check(prev, now, n):
+        got, ref = G.gpu_event_vertices(v, prev, now, n), oracle.event_vertices(prev, now, n)
+        for k in ("boundary_prev", "boundary_now", "vclass"):
+            assert np.array_equal(got[k], ref[k]), k
+        return got
+    v = make(64, 64)
+    common = [(0, 1), (1, 2), (2, 3), (0, 3), (0, 4), (1, 4), (2, 5), (3, 5), (4, 5)]
+    r = check(pack(common + [(1, 3)]), pack(common + [(0, 2)]), 6)
+    assert [c & 5 for c in r["vclass"][:4].tolist()] == [4, 1, 4, 1]
+    r = check(pack([(0, 1), (1, 2), (0, 2)]), pack([(0, 1), (1, 2)]), 3)               # Fig. 8 bottom
+    assert r["vclass"].tolist() == [2, 0, 2] and r["boundary_prev"].tolist() == [1, 1, 1]
+    check(pack(common), pack(common), 6)
+    check(np.empty(0, np.uint64), pack([(0, 2)]), 3)
+    check(pack([(0, 1), (1, 2), (0, 2), (1, 5)]), pack([(0, 1), (1, 2), (2, 6)]), 3)
+    rng = np.random.default_rng(41)
+    for n, deg in ((7, 3), (33, 6), (1000, 6), (5000, 6), (300, 40)):
+        a, b = random_graph_pair(rng, n, deg)
+        check(a, b, n)
+    v.close()
+    # walled lattice: the triangulation has a boundary; two frames of moving sites
+    import importlib
+    geo = importlib.import_module("test_gpu_geometry")
+    Lx, Ly = 256, 192
+    sx, sy = geo.jitter_sites(rng, Lx, Ly, 14.0)
+    vg = geo.make(Lx, Ly, (0, 0), len(sx))
+    lists = []
+    for t in range(2):
+        lists.append(G.gpu_edges_image(vg, G.gpu_labels(vg, sx, sy), False))
+        sx = np.clip(sx + rng.integers(-500, 500, len(sx)), 0, FP * Lx - 1).astype(np.int32)
+        sy = np.clip(sy + rng.integers(-500, 500, len(sy)), 0, FP * Ly - 1).astype(np.int32)
+    got = G.gpu_event_vertices(vg, lists[0], lists[1], len(sx))
+    ref = oracle.event_vertices(lists[0], lists[1], len(sx))
+    for k in ("boundary_prev", "boundary_now", "vclass"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert ref["boundary_prev"].sum() > 20 and (ref["vclass"] & 1).sum() > 5 and (ref["vclass"] & 2).sum() > 0
+    vg.close()
+
+
 # ------------------------------------------------------------------ full size, bench.py's launch configuration
 def test_config5_full_size_all_frames(G):
     """BASELINE config 5 at its full size (16384^2 cells, 10^6 sites), ALL 10 frames of the random walk,
