@@ -319,6 +319,13 @@ int vor_frame_collect(vor_ctx* ctx, uint64_t* h_created, uint64_t* h_destroyed, 
  * context-owned device buffers (vor_frame_results).  bench.py's device-resident leg. */
 int vor_frame_device(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_t n_sites,
                      void* stream);
+/* Variants of the frame calls (vor_frame_* and field_frame_*), kept until changed: bubbles 4- or 8-connected
+ * (field_threshold_ccl_conn), density-weighted centres (field_centroids_weighted with the frame's field), and an
+ * obstacle mask d_obstacles[Lx*Ly] (device memory that must stay valid; NULL = none) whose sites take
+ * obstacle_colour after labelling and take part in no edge (vor_paint_obstacles, vor_edges_image) - together with
+ * walled axes (vor_create_geom) the paper's own set-up: a confined channel with posts. */
+int vor_frame_options(vor_ctx* ctx, int32_t connectivity, int32_t weighted, const uint8_t* d_obstacles,
+                      int32_t obstacle_colour);
 /* Forget the previous frame's edge list (start a new sequence). */
 int vor_frame_reset(vor_ctx* ctx);
 /* Device pointers to the context-owned results of the last vor_frame_* call:

@@ -60,6 +60,7 @@ SIGNATURES = {
     "vor_frame_submit": (C.c_int, [_P, _P, _P, C.c_int32, _P]),
     "vor_frame_collect": (C.c_int, [_P, _P, _P, C.c_int64, _P]),
     "vor_frame_reset": (C.c_int, [_P]),
+    "vor_frame_options": (C.c_int, [_P, C.c_int32, C.c_int32, _P, C.c_int32]),
     "vor_frame_results": (C.c_int, [_P, C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P), C.POINTER(_P)]),
     "field_frame_device": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, C.c_int32, _P]),
     "field_frame_submit": (C.c_int, [_P, _P, C.c_float, C.c_int, C.c_int32, C.c_int32, _P]),
@@ -333,6 +334,12 @@ class Vor:
     # ---- frame pipeline
     def vor_frame_reset(self):
         self._check(self.lib.vor_frame_reset(self.h))
+
+    def vor_frame_options(self, connectivity: int = 4, weighted: bool = False, obstacles=None, obstacle_colour: int = -1):
+        """obstacles: uint8 CUDA tensor of Lx*Ly entries (keep it alive) or None."""
+        self._obstacles = obstacles
+        self._check(self.lib.vor_frame_options(self.h, connectivity, 1 if weighted else 0, _ptr(obstacles, torch.uint8),
+                                               obstacle_colour))
 
     def vor_frame_device(self, sx, sy):
         self._check(self.lib.vor_frame_device(self.h, _ptr(sx, torch.int32), _ptr(sy, torch.int32),

@@ -135,6 +135,11 @@ struct vor_ctx {
     int64_t* d_ff_tmpcount;    // [2] created / destroyed counts before they are gathered
     float* d_ff_field[2];      // device copies of submitted host fields (lazily)
     int ff_cur;                // generation of the last field frame; -1 = none
+    // vor_frame_options: variants of the frame calls
+    int32_t fo_connectivity;   // bubbles: 4 (default, also when 0) or 8
+    int32_t fo_weighted;       // density-weighted centres
+    const uint8_t* d_fo_mask;  // obstacle sites (caller-owned, may be NULL)
+    int32_t fo_colour;
     int32_t ff_hint;           // bubbles in an earlier frame (sizes the next cell list)
     int32_t* h_ff_count;       // pinned [1]: bubble count of the latest frame whose kernels have finished
     // pipelined variant (vor_frame_submit / vor_frame_collect): two frames in flight, copies on own streams

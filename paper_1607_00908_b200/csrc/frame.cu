@@ -36,8 +36,11 @@ int frame_compute(vor_ctx* ctx, const int32_t* d_sx, const int32_t* d_sy, int32_
                                    ctx->d_fr_rowptr[now], false, stream)) != VOR_OK) return rc;
     } else {
         if ((rc = vor_label(ctx, ctx->d_fr_labels, stream)) != VOR_OK) return rc;
-        if ((rc = vor_edges_rows(ctx, ctx->d_fr_labels, ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now],
-                                 ctx->d_fr_rowptr[now], stream)) != VOR_OK) return rc;
+        if (ctx->d_fo_mask &&
+            (rc = vor_paint_obstacles(ctx, ctx->d_fo_mask, ctx->fo_colour, ctx->d_fr_labels, ctx->Ly, stream)) != VOR_OK) return rc;
+        if ((rc = vor_edges_image(ctx, ctx->d_fr_labels, ctx->Ly, ctx->per_y, ctx->d_fo_mask ? ctx->fo_colour : -1,
+                                  ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now], ctx->d_fr_rowptr[now],
+                                  stream)) != VOR_OK) return rc;
     }
     if (n_sites == ctx->fr_prev_sites)
         rc = vor_diff_rows(ctx, ctx->d_fr_edges[prev], ctx->d_fr_rowptr[prev], ctx->d_fr_edges[now],
@@ -153,17 +156,20 @@ int field_frame_compute(vor_ctx* ctx, const float* d_field, const FieldArgs& fa,
     // has arrived by now sizes this frame's buckets and halo (a hint: results never depend on it), no waiting
     const int32_t seen = *(volatile int32_t*)ctx->h_ff_count;
     if (seen > 0) ctx->ff_hint = seen < K ? seen : K;
-    if ((rc = field_threshold_ccl(ctx, d_field, fa.thr, fa.above, ctx->d_ff_ccl, stream)) != VOR_OK) return rc;
-    if ((rc = field_centroids(ctx, ctx->d_ff_ccl, fa.min_size, cx, cy, c, c + K, c + 2 * K, c + 3 * K, K,
-                              c + 4 * K, stream)) != VOR_OK) return rc;
+    if ((rc = field_threshold_ccl_conn(ctx, d_field, fa.thr, fa.above, ctx->fo_connectivity == 8 ? 8 : 4, ctx->d_ff_ccl,
+                                       stream)) != VOR_OK) return rc;
+    if ((rc = field_centroids_weighted(ctx, ctx->d_ff_ccl, ctx->fo_weighted ? d_field : nullptr, fa.min_size, cx, cy, c,
+                                       c + K, c + 2 * K, c + 3 * K, K, c + 4 * K, stream)) != VOR_OK) return rc;
     VOR_CUDA(cudaMemcpyAsync(ctx->h_ff_count, c + 4 * K, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
     if (have_prev && (rc = match_sites(ctx, pc, pc + K, pc + 4 * K, c, c + K, c + 4 * K, K, K, fa.radius_fp,
                                        p2n, n2p, stream)) != VOR_OK) return rc;
     if ((rc = vor_build_cells_dev(ctx, c, c + K, c + 4 * K, K, ctx->ff_hint > 0 ? ctx->ff_hint : K, stream)) != VOR_OK)
         return rc;
     if ((rc = vor_label(ctx, ctx->d_fr_labels, stream)) != VOR_OK) return rc;
-    if ((rc = vor_edges(ctx, ctx->d_fr_labels, ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now],
-                        stream)) != VOR_OK) return rc;
+    if (ctx->d_fo_mask &&
+        (rc = vor_paint_obstacles(ctx, ctx->d_fo_mask, ctx->fo_colour, ctx->d_fr_labels, ctx->Ly, stream)) != VOR_OK) return rc;
+    if ((rc = vor_edges_image(ctx, ctx->d_fr_labels, ctx->Ly, ctx->per_y, ctx->d_fo_mask ? ctx->fo_colour : -1,
+                              ctx->d_fr_edges[now], ctx->fr_cap, ctx->d_fr_nedges[now], nullptr, stream)) != VOR_OK) return rc;
     if (have_prev && (rc = vor_diff(ctx, ctx->d_fr_edges[prev], ctx->d_fr_nedges[prev], ctx->d_fr_edges[now],
                                     ctx->d_fr_nedges[now], ctx->fr_cap, ctx->fr_cap, p2n, n2p, K, K,
                                     d_created, d_destroyed, ctx->fr_cap, &ctx->d_ff_tmpcount[0],
@@ -175,6 +181,20 @@ int field_frame_compute(vor_ctx* ctx, const float* d_field, const FieldArgs& fa,
     return VOR_OK;
 }
 }  // namespace
+
+extern "C" int vor_frame_options(vor_ctx* ctx, int32_t connectivity, int32_t weighted, const uint8_t* d_obstacles,
+                                 int32_t obstacle_colour) {
+    if (!ctx) return VOR_EINVAL;
+    if (connectivity != 4 && connectivity != 8)
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_options: connectivity must be 4 or 8");
+    if (d_obstacles && obstacle_colour < 0)
+        return vor_fail(ctx, VOR_EINVAL, "vor_frame_options: the obstacle colour must be >= 0");
+    ctx->fo_connectivity = connectivity;
+    ctx->fo_weighted = weighted != 0;
+    ctx->d_fo_mask = d_obstacles;
+    ctx->fo_colour = obstacle_colour;
+    return VOR_OK;
+}
 
 extern "C" int vor_frame_reset(vor_ctx* ctx) {
     if (!ctx) return VOR_EINVAL;

@@ -996,7 +996,8 @@ extern "C" int vor_label_rows(vor_ctx* ctx, int32_t y0, int32_t n_rows, int32_t*
 // Can the current cell list take the fused label -> edge path (vor_frame_*)?  It is written for the
 // CTA kernel's 32 x 32 tiles on a periodic lattice they tile exactly.
 bool vor_label_fusable(const vor_ctx* ctx) {
-    if (ctx->nbx <= 0 || ctx->Lx % 32 != 0 || ctx->Ly % 32 != 0 || !ctx->per_x || !ctx->per_y || !ctx->fuse) return false;
+    if (ctx->nbx <= 0 || ctx->Lx % 32 != 0 || ctx->Ly % 32 != 0 || !ctx->per_x || !ctx->per_y || !ctx->fuse || ctx->d_fo_mask)
+        return false;
     return label_path_for(ctx, site_spacing(ctx)) == 3;
 }
 

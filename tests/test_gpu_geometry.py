@@ -454,3 +454,82 @@ def test_random_sweep_field_chain(G):
             r1, r2 = oracle.match_g(Lx, Ly, per[0], per[1], a["sx"], a["sy"], b["sx"], b["sy"], R)
             assert np.array_equal(p2n, r1) and np.array_equal(n2p, r2), case
         v.close()
+
+
+# ------------------------------------------------------------------ the frame calls on the paper's set-up
+def test_frame_calls_with_walls_obstacles_weights(G):
+    """field_frame_device with vor_frame_options(8-connected, weighted, obstacle mask) on a walled channel, and
+    vor_frame_host with the same obstacles: counts, maps and flip lists of every frame against the oracle chain."""
+    rng = np.random.default_rng(44)
+    Lx, Ly, per = 384, 256, (0, 1)
+    MAXLINK = 0x77777777
+    obst = np.zeros((Ly, Lx), np.uint8)
+    for k in range(4):
+        obst[64 * k + 8: 64 * k + 32, :30] = 1
+    d_obst = G.dev(obst.ravel())
+    cx0, cy0 = jitter_sites(rng, Lx, Ly, 32.0, jitter=0.25)
+    cx0 = cx0 / FP; cy0 = cy0 / FP
+    keep = cx0 > 50
+    cx0, cy0 = cx0[keep], cy0[keep]
+    yy, xx = np.mgrid[0:Ly, 0:Lx]
+    v = make(Lx, Ly, per, 512)
+    v.vor_frame_options(8, True, d_obst, MAXLINK)
+    R = 4 * FP
+    prev = None
+    for t in range(4):
+        cx = cx0 + 0.7 * t * np.sin(cy0 / 19.0) + rng.normal(0, 0.5, len(cx0))
+        cy = (cy0 + 1.2 * t * (cx0 / Lx) + rng.normal(0, 0.5, len(cx0))) % Ly
+        rho = np.full((Ly, Lx), 1.2, np.float32)
+        for a, b in zip(cx, cy):
+            x0, x1 = int(max(0, a - 14)), int(min(Lx, a + 15))
+            ys = np.arange(int(b) - 14, int(b) + 15) % Ly
+            dx = xx[0, x0:x1][None, :] + 0.5 - a
+            dy = (ys[:, None] + 0.5 - b + Ly / 2) % Ly - Ly / 2
+            d = np.sqrt(dx * dx + dy * dy)
+            sub = np.ix_(ys, np.arange(x0, x1))
+            rho[sub] = np.minimum(rho[sub], (0.2 + 1.0 / (1.0 + np.exp(-(d - 11.0)))).astype(np.float32))
+        rho = 1.4 - rho                                           # bubbles where the field is ABOVE the threshold
+        v.field_frame_device(G.dev(rho.ravel()), 0.7, True, 20, R)
+        v.vor_sync_status()
+        r_ccl = oracle.threshold_ccl_g(rho, 0.7, True, per[0], per[1], 8)
+        r_c = oracle.centroids_g(r_ccl, 20, per[0], per[1], rho)
+        r_lab = oracle.apply_obstacles(oracle.label_brute_g(Lx, Ly, per[0], per[1], r_c["sx"], r_c["sy"]), obst, MAXLINK)
+        r_e = oracle.edges_g(r_lab, per[0], per[1], MAXLINK)
+        res = v.field_frame_results()
+        counts = G.from_device_ptr(res["counts"], 4, torch.int64).cpu().tolist()
+        K = len(r_c["sx"])
+        assert counts[0] == K and counts[1] == len(r_e), (t, counts, K, len(r_e))
+        assert np.array_equal(G.from_device_ptr(res["ccl"], Lx * Ly, torch.int32).cpu().numpy().reshape(Ly, Lx), r_ccl)
+        assert np.array_equal(G.from_device_ptr(res["labels"], Lx * Ly, torch.int32).cpu().numpy().reshape(Ly, Lx), r_lab)
+        assert np.array_equal(G.from_device_ptr(res["sx"], K, torch.int32).cpu().numpy(), r_c["sx"])
+        assert np.array_equal(G.u64(G.from_device_ptr(res["edges"], len(r_e), torch.int64)), r_e)
+        if prev is not None:
+            p_c, p_e = prev
+            r_p2n, r_n2p = oracle.match_g(Lx, Ly, per[0], per[1], p_c["sx"], p_c["sy"], r_c["sx"], r_c["sy"], R)
+            r_cr, r_de = oracle.diff(p_e, r_e, r_p2n, r_n2p)
+            assert counts[2] == len(r_cr) and counts[3] == len(r_de), (t, counts)
+            assert np.array_equal(G.u64(G.from_device_ptr(res["created"], len(r_cr), torch.int64)), r_cr)
+            assert np.array_equal(G.u64(G.from_device_ptr(res["destroyed"], len(r_de), torch.int64)), r_de)
+        prev = (r_c, r_e)
+    v.close()
+    # site-driven frames with the same obstacles
+    sx, sy = jitter_sites(rng, Lx, Ly, 24.0)
+    v = make(Lx, Ly, per, len(sx))
+    v.vor_frame_options(4, False, d_obst, MAXLINK)
+    cap = 16 * len(sx)
+    hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+    pe = np.empty(0, np.uint64)
+    for t in range(3):
+        v.vor_frame_host(sx, sy, hc, hd, cnt)
+        e = oracle.edges_g(oracle.apply_obstacles(oracle.label_brute_g(Lx, Ly, per[0], per[1], sx, sy), obst, MAXLINK),
+                           per[0], per[1], MAXLINK)
+        rc, rd = oracle.diff(pe, e)
+        assert cnt.tolist() == [len(e), len(rc), len(rd)], t
+        assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd)
+        pe = e
+        sx = np.clip(sx + rng.integers(-300, 300, len(sx)), 0, FP * Lx - 1).astype(np.int32)
+        sy = ((sy.astype(np.int64) + rng.integers(-300, 300, len(sy))) % (FP * Ly)).astype(np.int32)
+    v.vor_frame_options(4, False, None, -1)
+    v.close()
+    with pytest.raises(Exception):
+        make(64, 64, (1, 1), 8).vor_frame_options(6, False, None, -1)
