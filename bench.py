@@ -65,6 +65,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", help="cfg5 (default) | cfg1 | cfg2 | cfg5@L e.g. cfg5@4096 | cfg3 | cfg4 (field path)")
+    ap.add_argument("--shard", default="sequences", choices=["sequences", "strips"],
+                    help="N > 1: independent sequences per rank (default, weak scaling) or row strips of ONE lattice "
+                         "(strong scaling: strips.py, one all-gather + merge per frame)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-field-leg", action="store_true", help="skip the short config-4 field-path leg of the default line")
@@ -603,6 +606,79 @@ def spawn_ranks(args) -> int:
     return subprocess.call(cmd, env=env)
 
 
+def run_strips(args, w):
+    """--shard strips: ONE lattice per step, its rows split over the ranks.  Every rank labels its
+    strip (+ the next strip's first row), extracts its keys, all-gathers the lists, merges them and compares the
+    merged list with the previous frame's.  value = L^2 * K / time: strong scaling."""
+    import torch
+    import torch.distributed as dist
+    from paper_1607_00908_b200.binding import Vor
+    from paper_1607_00908_b200.strips import StripFrame
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    W_, K = args.warmup, args.steps
+    frames = [(torch.from_numpy(sx).cuda(), torch.from_numpy(sy).cuda()) for sx, sy in w.frames(W_ + K)]   # same on every rank
+    L, n = w.L, w.n_sites
+    cap_e = 4 * n + 1024
+    v = Vor(L, n, max(1 << 20, 16 * n, world * cap_e))
+    fr = [StripFrame(v, n, cap_e, cap_e) for _ in range(2)]                # ping-pong: this frame's / the previous list
+    created = torch.empty(cap_e, dtype=torch.int64, device="cuda"); destroyed = torch.empty_like(created)
+    n_c = torch.zeros(1, dtype=torch.int64, device="cuda"); n_d = torch.zeros_like(n_c)
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        now, prev = fr[i & 1], fr[1 - (i & 1)]
+        now.compute(*frames[i])
+        v.vor_diff(prev.edges, prev.n_edges, now.edges, now.n_edges, created, destroyed, n_c, n_d)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    for i in range(W_):
+        step(i)
+    v.vor_sync_status()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = v.vor_launch_count()
+    t0.record(stream)
+    for k in range(K):
+        step(W_ + k)
+    t1.record(stream)
+    barrier()
+    launches = v.vor_launch_count() - l0
+    v.vor_sync_status()
+    ms_total = reduce_max(t0.elapsed_time(t1), world, "cuda")
+    v.vor_profile_begin()
+    for k in range(K):
+        step(W_ + k)
+    per = {}
+    for nm, ms in v.vor_profile_end():
+        per[nm] = per.get(nm, 0.0) + ms / K
+    clocks = sampler.stop()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": L * L * K / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+                          "warmup": W_, "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+                          "config": {"workload": w.name, "L": L, "n_sites": n, "parallelism": f"row strips x {world}",
+                                     "rows_per_rank": fr[0].rows, "l2_policy": "strip image exceeds L2"},
+                          "kernel_launch_ms": per, "gpu_launches": launches, "clocks": clocks,
+                          "counts": {"n_edges": int(fr[(W_ + K - 1) & 1].n_edges.item()), "n_created": int(n_c.item()),
+                                     "n_destroyed": int(n_d.item())}}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     w = get_workload(args.workload)
@@ -614,6 +690,8 @@ def main():
         run_field(args, w)
     elif args.impl == "reference":
         run_reference(args, w)
+    elif args.shard == "strips":
+        run_strips(args, w)
     else:
         run_ours(args, w)
 
