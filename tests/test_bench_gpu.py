@@ -50,3 +50,15 @@ def test_bench_line_field_path():
     assert {"threshold_ccl", "centroids", "match", "build_cells", "label", "edges", "diff"} <= set(d["kernel_ms"])
     assert d["roofline"]["bound"] == "hbm" and d["config"]["components"] > 1000
     assert "no host synchronisation" in d["config"]["timing"]
+
+
+def test_bench_line_row_strips_and_event_layer():
+    d = run_bench("--workload", "cfg5@2048", "--shard", "strips")
+    assert d["scaling"] == "strong" and d["n_gpus"] == 1 and d["value"] > 0 and d["gpu_launches"] > 0
+    assert "row strips" in d["config"]["parallelism"] and d["config"]["rows_per_rank"] == 2048
+    assert {"pack_lists_kernel", "sort_unique_kernel"} <= set(d["kernel_launch_ms"])
+    s = run_bench("--workload", "cfg5@2048", "--no-cpu-baseline", "--no-e2e", "--no-field-leg")
+    assert d["counts"]["n_edges"] == s["counts"]["n_edges"]            # the merged list is the lattice's list
+    t1 = s["events"]["t1"]
+    assert t1["couples"] > 0 and t1["breaking"] == s["counts"]["n_destroyed"] and t1["arising"] == s["counts"]["n_created"]
+    assert 0 < t1["t1_quadruples"] <= t1["breaking"]
