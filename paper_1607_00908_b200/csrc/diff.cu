@@ -531,30 +531,147 @@ extern "C" int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Union of several key lists (multi-GPU row strips: every rank extracts the keys of its strip,
-// one all-gather brings the lists together, "followed by a merge-unique"): the valid parts of the n_lists
-// buffers are packed into the sort scratch, then radix-sorted and uniqued by the same cooperative kernel as
-// the overflow path of vor_edges.
+// Union of several ASCENDING key lists (multi-GPU row strips: every rank extracts the keys of its
+// strip, one all-gather brings the lists together, "followed by a merge-unique").  The lists are merged pairwise
+// in ceil(log2 n_lists) rounds by merge path (one co-rank search per 8 output slots, then a sequential merge;
+// repeats are kept, so every round's layout is the concatenation given by the prefix sums of the counts), then
+// one order-preserving pass drops the repeats.
 namespace {
 
-__global__ void pack_lists_kernel(const uint64_t* __restrict__ lists, int64_t stride,
-                                  const int64_t* __restrict__ counts, int32_t n_lists, uint64_t* __restrict__ out,
-                                  int64_t cap_out, int64_t* __restrict__ n_out, int32_t* __restrict__ flags) {
-    // blockIdx.y = list; its offset = sum of the clamped counts before it (n_lists is small)
-    const int l = blockIdx.y;
-    int64_t off = 0, all = 0;
-    for (int k = 0; k < n_lists; ++k) {
-        const int64_t c = min(max(counts[k], (int64_t)0), stride);
-        if (k < l) off += c;
-        all += c;
+constexpr int kMlThreads = 256, kMlPer = 8, kMlMaxLists = 1024;
+
+struct MergeRound {
+    const uint64_t* src;       // round 0: the caller's buffers, list l at l * stride; later: concatenated
+    int round0;
+    int64_t stride;
+    uint64_t* dst;             // concatenated
+    const int64_t* counts;
+    int32_t n_lists;
+    int32_t span;              // lists per input segment (1, 2, 4, ...); output segments hold 2 * span lists
+    int64_t* total;            // sum of the (clamped) counts
+};
+
+__global__ void __launch_bounds__(kMlThreads) merge_round_kernel(const MergeRound m) {
+    __shared__ int64_t pre[kMlMaxLists + 1];
+    for (int l = threadIdx.x; l < m.n_lists; l += kMlThreads) pre[l + 1] = min(max(m.counts[l], (int64_t)0), m.stride);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        pre[0] = 0;
+        for (int l = 0; l < m.n_lists; ++l) pre[l + 1] += pre[l];
+        if (blockIdx.x == 0) *m.total = pre[m.n_lists];
     }
-    if (l == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
-        *n_out = all;
-        if (all > cap_out) atomicOr(flags, FLAG_RAWKEY_OVERFLOW);
+    __syncthreads();
+    const int64_t total = pre[m.n_lists];
+    const int32_t two = 2 * m.span, nseg = (m.n_lists + two - 1) / two;
+    for (int64_t p0 = ((int64_t)blockIdx.x * kMlThreads + threadIdx.x) * kMlPer; p0 < total;
+         p0 += (int64_t)gridDim.x * kMlThreads * kMlPer) {
+        int64_t p = p0;
+        const int64_t p_end = min(p0 + kMlPer, total);
+        while (p < p_end) {
+            // the output segment that holds slot p: the last S with pre[S * two] <= p
+            int32_t lo = 0, hi = nseg - 1;
+            while (lo < hi) {
+                const int32_t mid = (lo + hi + 1) >> 1;
+                if (pre[min(mid * two, m.n_lists)] <= p) lo = mid; else hi = mid - 1;
+            }
+            const int32_t l0 = lo * two, l1 = min(l0 + m.span, m.n_lists), l2 = min(l0 + two, m.n_lists);
+            const int64_t s0 = pre[l0], nA = pre[l1] - s0, nB = pre[l2] - pre[l1];
+            if (nA + nB == 0) { ++p; continue; }          // cannot happen for p < total; keeps the loop finite
+            const uint64_t* __restrict__ A = m.round0 ? m.src + (int64_t)l0 * m.stride : m.src + s0;
+            const uint64_t* __restrict__ B = m.round0 ? m.src + (int64_t)l1 * m.stride : m.src + s0 + nA;
+            const int64_t d0 = p - s0;
+            int64_t a = max((int64_t)0, d0 - nB), b = min(d0, nA);
+            while (a < b) {                                 // co-rank: a keys of A and d0 - a keys of B precede slot d0
+                const int64_t mid = (a + b) >> 1, j = d0 - mid;
+                if (j > 0 && B[j - 1] >= A[mid]) a = mid + 1; else b = mid;   // ties: A first
+            }
+            int64_t i = a, j = d0 - a;
+            const int64_t seg_end = min(p_end, s0 + nA + nB);
+            for (; p < seg_end; ++p) {
+                uint64_t key;
+                if (j >= nB || (i < nA && A[i] <= B[j])) key = A[i++]; else key = B[j++];
+                m.dst[p] = key;
+            }
+        }
     }
-    const int64_t m = min(max(counts[l], (int64_t)0), stride);
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += (int64_t)gridDim.x * blockDim.x)
-        if (off + i < cap_out) out[off + i] = lists[(int64_t)l * stride + i];
+}
+
+struct UniqueParams {
+    const uint64_t* in; const int64_t* n_in; int64_t cap_in;
+    uint64_t* out; int64_t cap; int64_t* n_out; int64_t* partial; int32_t* flags; int flag_bit;
+};
+
+__device__ __forceinline__ void ml_chunk(int64_t n, int64_t* beg, int64_t* end) {
+    int64_t C = (n + gridDim.x - 1) / gridDim.x;
+    C = (C + kMlThreads - 1) / kMlThreads * kMlThreads;
+    const int64_t s = (int64_t)blockIdx.x * C;
+    *beg = s < n ? s : n;
+    *end = s + C < n ? s + C : n;
+}
+
+__device__ __forceinline__ int64_t ml_block_sum(int64_t v, int64_t* sh) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    int64_t t = lane < kMlThreads / 32 ? sh[lane] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    __syncthreads();
+    return t;
+}
+
+__global__ void __launch_bounds__(kMlThreads) unique_count_kernel(const UniqueParams p) {
+    __shared__ int64_t sh[32];
+    const int64_t n = min(*p.n_in, p.cap_in);
+    int64_t beg, end;
+    ml_chunk(n, &beg, &end);
+    int64_t c = 0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kMlThreads) c += i == 0 || p.in[i] != p.in[i - 1];
+    c = ml_block_sum(c, sh);
+    if (threadIdx.x == 0) p.partial[blockIdx.x] = c;
+}
+
+__global__ void __launch_bounds__(kMlThreads) unique_write_kernel(const UniqueParams p) {
+    __shared__ int64_t sh[32];
+    __shared__ int32_t wtot[kMlThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t n = min(*p.n_in, p.cap_in);
+    int64_t beg, end;
+    ml_chunk(n, &beg, &end);
+    int64_t before = 0, all = 0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += kMlThreads) {
+        const int64_t v = p.partial[b];
+        all += v;
+        if (b < (int)blockIdx.x) before += v;
+    }
+    before = ml_block_sum(before, sh);
+    all = ml_block_sum(all, sh);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        *p.n_out = all;
+        if (all > p.cap) atomicOr(p.flags, p.flag_bit);
+    }
+    int64_t run = before;
+    for (int64_t sub = beg; sub < end; sub += kMlThreads) {
+        const int64_t i = sub + threadIdx.x;
+        const uint64_t key = i < end ? p.in[i] : 0;
+        const bool keep = i < end && (i == 0 || key != p.in[i - 1]);
+        const unsigned ball = __ballot_sync(0xffffffffu, keep);
+        if (lane == 0) wtot[wid] = __popc(ball);
+        __syncthreads();
+        int32_t wbase = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kMlThreads / 32; ++w) {
+            const int32_t t = wtot[w];
+            if (w < wid) wbase += t;
+            total += t;
+        }
+        const int64_t pos = run + wbase + __popc(ball & ((1u << lane) - 1u));
+        if (keep && pos < p.cap) p.out[pos] = key;
+        run += total;
+        __syncthreads();
+    }
 }
 
 }  // namespace
@@ -565,13 +682,24 @@ extern "C" int vor_merge_lists(vor_ctx* ctx, const uint64_t* d_lists, int64_t st
     if (!ctx) return VOR_EINVAL;
     if (int drc_ = vor_check_device(ctx)) return drc_;
     if (!d_lists || !d_counts || !d_out || !d_n_out) return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: null pointer");
-    if (stride < 0 || n_lists < 1 || n_lists > 1024 || n_labels < 1 || cap < 0)
+    if (stride < 0 || n_lists < 1 || n_lists > kMlMaxLists || n_labels < 1 || cap < 0)
         return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: stride >= 0, 1 <= n_lists <= 1024, n_labels >= 1, cap >= 0");
     if (stride * n_lists > ctx->max_raw_keys)
         return vor_fail(ctx, VOR_EINVAL, "vor_merge_lists: stride * n_lists exceeds the context's max_raw_keys scratch");
     cudaStream_t stream = (cudaStream_t)stream_;
-    VOR_LAUNCH(pack_lists_kernel, dim3(2 * kNumSMs, n_lists), 256, 0, stream, d_lists, stride, d_counts, n_lists,
-               ctx->d_keys_a, ctx->max_raw_keys, ctx->d_n_raw, ctx->d_flags);
-    return vor_sort_unique_keys(ctx, ctx->d_keys_a, ctx->d_n_raw, bits_for(n_labels), d_out, cap, d_n_out,
-                                FLAG_EDGE_CAP, 0, stream);
+    const int grid = 8 * ctx->num_sms;
+    uint64_t* buf[2] = {ctx->d_keys_a, ctx->d_keys_b};
+    const uint64_t* src = d_lists;
+    int which = 0;
+    for (int32_t span = 1, round = 0; round == 0 || span < n_lists; span *= 2, ++round) {
+        MergeRound m{src, round == 0, stride, buf[which], d_counts, n_lists, span, ctx->d_n_raw};
+        VOR_LAUNCH(merge_round_kernel, grid, kMlThreads, 0, stream, m);
+        src = buf[which];
+        which ^= 1;
+    }
+    UniqueParams up{src, ctx->d_n_raw, ctx->max_raw_keys, d_out, cap, d_n_out, ctx->d_blk_count, ctx->d_flags, FLAG_EDGE_CAP};
+    const int ugrid = 4 * ctx->num_sms;                     // <= 2 * kMaxCoopBlocks partials
+    VOR_LAUNCH(unique_count_kernel, ugrid, kMlThreads, 0, stream, up);
+    VOR_LAUNCH(unique_write_kernel, ugrid, kMlThreads, 0, stream, up);
+    return VOR_OK;
 }

@@ -56,7 +56,7 @@ def test_bench_line_row_strips_and_event_layer():
     d = run_bench("--workload", "cfg5@2048", "--shard", "strips")
     assert d["scaling"] == "strong" and d["n_gpus"] == 1 and d["value"] > 0 and d["gpu_launches"] > 0
     assert "row strips" in d["config"]["parallelism"] and d["config"]["rows_per_rank"] == 2048
-    assert {"pack_lists_kernel", "sort_unique_kernel"} <= set(d["kernel_launch_ms"])
+    assert {"merge_round_kernel", "unique_write_kernel"} <= set(d["kernel_launch_ms"])
     s = run_bench("--workload", "cfg5@2048", "--no-cpu-baseline", "--no-e2e", "--no-field-leg")
     assert d["counts"]["n_edges"] == s["counts"]["n_edges"]            # the merged list is the lattice's list
     t1 = s["events"]["t1"]

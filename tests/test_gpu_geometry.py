@@ -533,3 +533,38 @@ def test_frame_calls_with_walls_obstacles_weights(G):
     v.close()
     with pytest.raises(Exception):
         make(64, 64, (1, 1), 8).vor_frame_options(6, False, None, -1)
+
+
+def test_merge_lists_many_lists_empty_lists_and_capacity(G):
+    rng = np.random.default_rng(91)
+    v = make(1024, 1024, (1, 1), 4096, max_raw_keys=1 << 20)
+    for n_lists, stride in ((1, 5000), (2, 3000), (7, 2000), (16, 1500), (33, 700), (64, 64)):
+        lists = torch.zeros(n_lists, stride, dtype=torch.int64, device="cuda")
+        counts = torch.zeros(n_lists, dtype=torch.int64, device="cuda")
+        parts = []
+        for l in range(n_lists):
+            m = 0 if l % 5 == 3 else int(rng.integers(1, stride + 1))
+            i = rng.integers(0, 4000, m); j = rng.integers(0, 4000, m)
+            ok = i != j
+            keys = np.unique((np.minimum(i, j)[ok].astype(np.uint64) << np.uint64(32)) | np.maximum(i, j)[ok].astype(np.uint64))
+            lists[l, : len(keys)] = torch.from_numpy(keys.view(np.int64)).cuda()
+            counts[l] = len(keys)
+            parts.append(keys)
+        counts[0] = counts[0] + (stride if n_lists == 7 else 0)          # a count above the buffer is clamped
+        if n_lists == 7:
+            parts[0] = lists[0].cpu().numpy().view(np.uint64)[:stride]
+            lists[0] = torch.sort(lists[0]).values                        # keep the clamped list ascending
+            parts[0] = lists[0].cpu().numpy().view(np.uint64)
+        ref = np.unique(np.concatenate(parts))
+        out = torch.full((len(ref) + 3,), -5, dtype=torch.int64, device="cuda")
+        n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+        v.vor_merge_lists(lists, counts, 4096, out[: len(ref)], n_out)
+        v.vor_sync_status()
+        assert int(n_out.item()) == len(ref) and np.array_equal(G.u64(out, len(ref)), ref), n_lists
+        assert (out[len(ref):] == -5).all()
+        if len(ref) > 10:                                                 # too small an output: required count + status
+            v.vor_merge_lists(lists, counts, 4096, out[:10], n_out)
+            with pytest.raises(Exception, match="ECAPACITY"):
+                v.vor_sync_status()
+            assert int(n_out.item()) == len(ref) and np.array_equal(G.u64(out, 10), ref[:10])
+    v.close()
