@@ -486,6 +486,12 @@ struct CtaShared {
     int4 tmp[kListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
     int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
     int32_t nkept;                                    // gathered sites kept (inside the exact rectangle)
+    // which residues |o|^2 mod 256 a quadrant's survivors have taken, and whether two of them share one.
+    // Cell centres are odd multiples of 128 units away from the quadrant centre, so the compared value
+    // t = |o|^2 - 2 c.o is congruent to |o|^2 mod 256: candidates with different residues never tie on any cell
+    // of the quadrant, and then the order of the list does not matter (no ranking by index needed).
+    uint32_t res[kCtaQ][8];
+    int32_t coll[kCtaQ];
 };
 // fused path: (label, slot of the site in sx/sy/si) of every list entry, fetched with one 64-bit load;
 // the CTA's 64 x 64 bit matrix of adjacent slots; the first row of the lower warp
@@ -591,12 +597,20 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     if (ok) {
         for (int32_t i = sub; i < ns; i += 4) {
             const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
-            const int32_t ex = min(max(abs(ox) - QHW, 0), U + 1), ey = min(max(abs(oy) - QHW, 0), U + 1);
+            // |ox|, |oy| <= kCtaMaxExtent + 3968 < 27000: the sum of the two squares stays below 2^31
+            const int32_t ex = max(abs(ox) - QHW, 0), ey = max(abs(oy) - QHW, 0);
             if (ex * ex + ey * ey <= U2) {
                 const int32_t slot = atomicAdd(&sh.count[q], 1);
                 if (slot < kListCap) {
-                    sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, ox * ox + oy * oy, sh.si[i]);
-                    if constexpr (kFused) fs.tslot[slot][q] = (uint8_t)i;
+                    const int32_t d = ox * ox + oy * oy;
+                    if constexpr (kFused) {
+                        sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, d, sh.si[i]);
+                        fs.tslot[slot][q] = (uint8_t)i;
+                    } else {
+                        sh.list[slot][q] = make_int4(-2 * ox, -2 * oy, d, sh.si[i]);
+                        const uint32_t bit = 1u << (d & 31);
+                        if (atomicOr(&sh.res[q][(d >> 5) & 7], bit) & bit) sh.coll[q] = 1;
+                    }
                 }
             }
         }
@@ -604,14 +618,29 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     __syncwarp();
     const int32_t n = sh.count[q];
     __syncwarp();
-    if (ok && n <= kListCap) {
-        // order by original index: rank = number of survivors with a smaller index (indices distinct)
-        for (int32_t k = sub; k < n; k += 4) {
-            const int4 e = sh.tmp[k][q];
-            int32_t r = 0;
-            for (int32_t j = 0; j < n; ++j) r += (sh.tmp[j][q].w < e.w);
-            sh.list[r][q] = e;
-            if constexpr (kFused) fs.fin[r][q] = make_int2(e.w, (int32_t)fs.tslot[k][q]);
+    if constexpr (kFused) {
+        if (ok && n <= kListCap) {
+            // order by original index: rank = number of survivors with a smaller index (indices distinct)
+            for (int32_t k = sub; k < n; k += 4) {
+                const int4 e = sh.tmp[k][q];
+                int32_t r = 0;
+                for (int32_t j = 0; j < n; ++j) r += (sh.tmp[j][q].w < e.w);
+                sh.list[r][q] = e;
+                fs.fin[r][q] = make_int2(e.w, (int32_t)fs.tslot[k][q]);
+            }
+        }
+    } else {
+        // two survivors share a residue (about 3 % of the quadrants): a tie is possible somewhere, so the list is
+        // put in index order - the smallest-index rule then comes with the position in the packed key
+        if (ok && n <= kListCap && sh.coll[q]) {
+            for (int32_t k = sub; k < n; k += 4) {
+                const int4 e = sh.list[k][q];
+                int32_t r = 0;
+                for (int32_t j = 0; j < n; ++j) r += (sh.list[j][q].w < e.w);
+                sh.tmp[r][q] = e;
+            }
+            __syncwarp(0xfu << ((threadIdx.x & 31) & ~3));          // the quadrant's four lanes (they branch together)
+            for (int32_t k = sub; k < n; k += 4) sh.list[k][q] = sh.tmp[k][q];
         }
     }
     if (sub == 0 && active)
@@ -690,7 +719,9 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int32_t X0 = p.wx0 + blockIdx.x * (8 * kCtaQX), Y0 = p.wy0 + blockIdx.y * (8 * kCtaQY);
     // ---- phases G + A; quadrants whose bound could not be proven get one retry with a wider halo
-    if (threadIdx.x < kCtaQ) sh.count[threadIdx.x] = 0;
+    if (threadIdx.x < kCtaQ) { sh.count[threadIdx.x] = 0; sh.coll[threadIdx.x] = 0; }
+    (&sh.res[0][0])[threadIdx.x] = 0; (&sh.res[0][0])[threadIdx.x + kCtaThreads] = 0;
+    static_assert(kCtaQ * 8 == 2 * kCtaThreads, "two residue words per thread");
     if constexpr (kFused) {
         for (int i = threadIdx.x; i < kCtaCapSites * kCtaCapSites / 32; i += kCtaThreads) fs.bm[i] = 0;
     }
@@ -711,7 +742,10 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
             active = sh.count[q] < 0;
             any_fail = __syncthreads_or(active);
             if (!any_fail) break;
-            if (attempt == 0 && active && sub == 0) sh.count[q] = 0;     // reset the survivor counter
+            if (attempt == 0 && active) {                                // reset the survivor counter and the residues
+                sh.res[q][2 * sub] = 0; sh.res[q][2 * sub + 1] = 0;
+                if (sub == 0) { sh.count[q] = 0; sh.coll[q] = 0; }
+            }
             __syncthreads();
         }
     }
