@@ -82,6 +82,18 @@ __device__ __forceinline__ int32_t div_w(const LabelParams& p, int32_t x /* >= 0
     return (int32_t)((t + (((uint32_t)x - t) >> p.div_s1)) >> p.div_s2);
 }
 
+// Segment of item i: the number of segments s < nseg whose inclusive prefix inc_s (held by lane s, nondecreasing)
+// is <= i.  Binary lifting over the lanes: five shuffles instead of one per segment.  Whole warp, converged.
+__device__ __forceinline__ int32_t segment_of(int32_t inc, int32_t nseg, int32_t i) {
+    int32_t seg = 0;
+#pragma unroll
+    for (int step = 16; step > 0; step >>= 1) {
+        const int32_t v = __shfl_sync(0xffffffffu, inc, (seg + step - 1) & 31);
+        if (seg + step <= nseg && v <= i) seg += step;
+    }
+    return seg;
+}
+
 constexpr int kWarpsPerCta = 8;
 constexpr int kCapGather = 160;    // gathered sites per tile
 constexpr int kCapCand = 64;       // surviving candidates per tile
@@ -205,8 +217,7 @@ __device__ __forceinline__ int32_t gather_region(const LabelParams& p, WarpScrat
     for (int32_t base = 0; base < total; base += 32) {
         const int32_t i = base + lane;
         // segment of item i = number of segments whose inclusive prefix is <= i
-        int32_t seg = 0;
-        for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(0xffffffffu, inc, s) <= i);
+        const int32_t seg = segment_of(inc, nseg, i);
         const int32_t sbeg = __shfl_sync(0xffffffffu, beg, seg & 31);
         const int32_t sexc = __shfl_sync(0xffffffffu, exc, seg & 31);
         if (i < total) {
@@ -295,8 +306,7 @@ __device__ __forceinline__ bool tile_fast(const LabelParams& p, FastScratch& fs,
     const int32_t exc = inc - cnt;
 
     // ---- one lane per site
-    int32_t seg = 0;
-    for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= lane);
+    const int32_t seg = segment_of(inc, nseg, lane);
     const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
     const bool valid = lane < total;
     int32_t rx = 0, ry = 0, idx = INT32_MAX;
@@ -549,8 +559,7 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
     __syncthreads();
     if (32 * wid < total) {                            // warp-uniform: this warp owns items [32 wid, 32 wid + 32)
         const int32_t i = 32 * wid + lane;             // this thread's item
-        int32_t seg = 0;
-        for (int32_t s = 0; s < nseg; ++s) seg += (__shfl_sync(full, inc, s) <= i);
+        const int32_t seg = segment_of(inc, nseg, i);
         const int32_t sbeg = __shfl_sync(full, beg, seg & 31), sexc = __shfl_sync(full, exc, seg & 31);
         int32_t rx = 0, ry = 0, idx = 0;
         bool keep = false;
