@@ -591,27 +591,36 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     constexpr int QHW = FP_HALF * 7;
     const unsigned full = 0xffffffffu;
     if (!active) ns = 0;
-    int32_t f = INT32_MAX;
+    // s*: the gathered site nearest to the quadrant centre (any one of them if several are)
+    int32_t f = INT32_MAX, fi = 0;
     for (int32_t i = sub; i < ns; i += 4) {
         const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
-        f = min(f, ox * ox + oy * oy);
+        const int32_t d = ox * ox + oy * oy;
+        if (d < f) { f = d; fi = i; }
     }
-    f = min(f, __shfl_xor_sync(full, f, 1));
-    f = min(f, __shfl_xor_sync(full, f, 2));
+#pragma unroll
+    for (int o = 1; o <= 2; o <<= 1) {
+        const int32_t g = __shfl_xor_sync(full, f, o), gi = __shfl_xor_sync(full, fi, o);
+        if (g < f || (g == f && gi < fi)) { f = g; fi = gi; }
+    }
     const int32_t U = isqrt_up(f) + p.r_quad;
     int32_t margin = min(qcx - QHW - R[0] + 1, R[1] - (qcx + QHW));
     margin = min(margin, min(qcy - QHW - R[2] + 1, R[3] - (qcy + QHW)));
     const bool ok = ns > 0 && U < margin && U <= kCtaMaxU;
-    const int32_t U2 = U * U;
     if (ok) {
+        // Candidates: the sites that can be at least as near as s* to SOME cell of the quadrant.  For a site t,
+        // g(c) = |c - t|^2 - |c - s*|^2 is linear in c, so over the box of cell centres [-QHW, QHW]^2 it is smallest
+        // at a corner: min g = |o_t|^2 - |o_s|^2 - 2 QHW (|dx| + |dy|), (dx, dy) = o_t - o_s.  min g > 0: s* is
+        // strictly nearer than t on every cell and t never wins (nor ties).  Every site kept lies within U of the
+        // box (it is at most as far from some corner as s*), so the bounds on the packed keys still hold.
+        const int32_t osx = sh.sx[fi] - qcx, osy = sh.sy[fi] - qcy;
         for (int32_t i = sub; i < ns; i += 4) {
             const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
-            // |ox|, |oy| <= kCtaMaxExtent + 3968 < 27000: the sum of the two squares stays below 2^31
-            const int32_t ex = max(abs(ox) - QHW, 0), ey = max(abs(oy) - QHW, 0);
-            if (ex * ex + ey * ey <= U2) {
+            const int32_t d = ox * ox + oy * oy;
+            // |ox|, |oy| < 27000: d < 2^31; 2 QHW (|dx| + |dy|) < 1792 * 108000 < 2^31
+            if (d - f <= 2 * QHW * (abs(ox - osx) + abs(oy - osy))) {
                 const int32_t slot = atomicAdd(&sh.count[q], 1);
                 if (slot < kListCap) {
-                    const int32_t d = ox * ox + oy * oy;
                     if constexpr (kFused) {
                         sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, d, sh.si[i]);
                         fs.tslot[slot][q] = (uint8_t)i;
