@@ -485,6 +485,7 @@ constexpr int kMaxUPacked = 6400;
 constexpr int kCtaQX = 4, kCtaQY = 4;                 // quadrants per CTA
 constexpr int kCtaQ = kCtaQX * kCtaQY;
 constexpr int kCtaThreads = 64;
+constexpr int kCtaListCap = 12;                       // candidates per quadrant (the exact test leaves about 3)
 constexpr int kCtaCapSites = 64;                      // = kCtaThreads: one gathered site per thread
 constexpr int kCtaMaxExtent = 23000;                  // |relative site coordinate| bound
 constexpr int kCtaMaxU = 20000;                       // |o| <= 896 + U <= 20896: t = |o|^2 - 2 c.o fits int32
@@ -492,8 +493,8 @@ constexpr int kUnpackedFlag = 1 << 16;
 
 struct CtaShared {
     int32_t sx[kCtaCapSites], sy[kCtaCapSites], si[kCtaCapSites];
-    int4 list[kListCap][kCtaQ];                       // [k][quadrant]: conflict-free across quadrants
-    int4 tmp[kListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
+    int4 list[kCtaListCap][kCtaQ];                       // [k][quadrant]: conflict-free across quadrants
+    int4 tmp[kCtaListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
     int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
     int32_t nkept;                                    // gathered sites kept (inside the exact rectangle)
     // which residues |o|^2 mod 256 a quadrant's survivors have taken, and whether two of them share one.
@@ -506,8 +507,8 @@ struct CtaShared {
 // fused path: (label, slot of the site in sx/sy/si) of every list entry, fetched with one 64-bit load;
 // the CTA's 64 x 64 bit matrix of adjacent slots; the first row of the lower warp
 struct CtaFusedShared {
-    int2 fin[kListCap][kCtaQ];
-    uint8_t tslot[kListCap][kCtaQ];                   // slot of the unsorted survivors
+    int2 fin[kCtaListCap][kCtaQ];
+    uint8_t tslot[kCtaListCap][kCtaQ];                   // slot of the unsorted survivors
     uint32_t bm[kCtaCapSites * kCtaCapSites / 32];
     uint32_t seam[32];                                // row 15 of the tile (last row of the upper warp)
 };
@@ -620,7 +621,7 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
             // |ox|, |oy| < 27000: d < 2^31; 2 QHW (|dx| + |dy|) < 1792 * 108000 < 2^31
             if (d - f <= 2 * QHW * (abs(ox - osx) + abs(oy - osy))) {
                 const int32_t slot = atomicAdd(&sh.count[q], 1);
-                if (slot < kListCap) {
+                if (slot < kCtaListCap) {
                     if constexpr (kFused) {
                         sh.tmp[slot][q] = make_int4(-2 * ox, -2 * oy, d, sh.si[i]);
                         fs.tslot[slot][q] = (uint8_t)i;
@@ -637,7 +638,7 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     const int32_t n = sh.count[q];
     __syncwarp();
     if constexpr (kFused) {
-        if (ok && n <= kListCap) {
+        if (ok && n <= kCtaListCap) {
             // order by original index: rank = number of survivors with a smaller index (indices distinct)
             for (int32_t k = sub; k < n; k += 4) {
                 const int4 e = sh.tmp[k][q];
@@ -650,7 +651,7 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     } else {
         // two survivors share a residue (about 3 % of the quadrants): a tie is possible somewhere, so the list is
         // put in index order - the smallest-index rule then comes with the position in the packed key
-        if (ok && n <= kListCap && sh.coll[q]) {
+        if (ok && n <= kCtaListCap && sh.coll[q]) {
             for (int32_t k = sub; k < n; k += 4) {
                 const int4 e = sh.list[k][q];
                 int32_t r = 0;
@@ -662,7 +663,7 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
         }
     }
     if (sub == 0 && active)
-        sh.count[q] = (ok && n <= kListCap) ? (U <= kMaxUPacked ? n : n | kUnpackedFlag) : -1;
+        sh.count[q] = (ok && n <= kCtaListCap) ? (U <= kMaxUPacked ? n : n | kUnpackedFlag) : -1;
 }
 
 // ---- fused path: the adjacent pairs of a CTA's 32 x 32 cells, straight from the labelling registers.
@@ -823,7 +824,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
                 for (int j = 0; j < 8; ++j) best[j] = min(best[j], a0 + (FP_ONE * j - QHW) * y0s);
             }
 #pragma unroll
-            for (int j = 0; j < 8; ++j) sel[j] = best[j] & (kListCap - 1);
+            for (int j = 0; j < 8; ++j) sel[j] = best[j] & 15;                   // key = 16 t + position
         } else {
             // far sites (large U): same scan with an explicit (value, position) pair
             int32_t best[8];
