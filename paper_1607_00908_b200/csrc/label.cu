@@ -492,7 +492,8 @@ constexpr int kCtaMaxU = 20000;                       // |o| <= 896 + U <= 20896
 constexpr int kUnpackedFlag = 1 << 16;
 
 struct CtaShared {
-    int32_t sx[kCtaCapSites], sy[kCtaCapSites], si[kCtaCapSites];
+    int2 sxy[kCtaCapSites];                              // site coordinates relative to the CTA centre (one 64-bit load)
+    int32_t si[kCtaCapSites];
     int4 list[kCtaListCap][kCtaQ];                       // [k][quadrant]: conflict-free across quadrants
     int4 tmp[kCtaListCap][kCtaQ];                        // unsorted survivors (phase A scratch)
     int32_t count[kCtaQ];                             // survivors per quadrant (phase A), then list length | flags
@@ -577,7 +578,7 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
         base = __shfl_sync(full, base, 0);
         if (keep) {
             const int32_t pos = base + __popc(ball & ((1u << lane) - 1u));
-            sh.sx[pos] = rx; sh.sy[pos] = ry; sh.si[pos] = idx;
+            sh.sxy[pos] = make_int2(rx, ry); sh.si[pos] = idx;
         }
     }
     return -1;                                         // the caller reads sh.nkept after its barrier
@@ -595,7 +596,8 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     // s*: the gathered site nearest to the quadrant centre (any one of them if several are)
     int32_t f = INT32_MAX, fi = 0;
     for (int32_t i = sub; i < ns; i += 4) {
-        const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
+        const int2 s2 = sh.sxy[i];
+        const int32_t ox = s2.x - qcx, oy = s2.y - qcy;
         const int32_t d = ox * ox + oy * oy;
         if (d < f) { f = d; fi = i; }
     }
@@ -614,9 +616,10 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
         // at a corner: min g = |o_t|^2 - |o_s|^2 - 2 QHW (|dx| + |dy|), (dx, dy) = o_t - o_s.  min g > 0: s* is
         // strictly nearer than t on every cell and t never wins (nor ties).  Every site kept lies within U of the
         // box (it is at most as far from some corner as s*), so the bounds on the packed keys still hold.
-        const int32_t osx = sh.sx[fi] - qcx, osy = sh.sy[fi] - qcy;
+        const int32_t osx = sh.sxy[fi].x - qcx, osy = sh.sxy[fi].y - qcy;
         for (int32_t i = sub; i < ns; i += 4) {
-            const int32_t ox = sh.sx[i] - qcx, oy = sh.sy[i] - qcy;
+            const int2 s2 = sh.sxy[i];
+            const int32_t ox = s2.x - qcx, oy = s2.y - qcy;
             const int32_t d = ox * ox + oy * oy;
             // |ox|, |oy| < 27000: d < 2^31; 2 QHW (|dx| + |dy|) < 1792 * 108000 < 2^31
             if (d - f <= 2 * QHW * (abs(ox - osx) + abs(oy - osy))) {
