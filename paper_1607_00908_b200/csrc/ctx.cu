@@ -41,7 +41,7 @@ int vor_create_geom(vor_ctx** out, int32_t Lx, int32_t Ly, int32_t periodic_x, i
     if (max_raw_keys > worst) max_raw_keys = worst;
     ctx->max_raw_keys = max_raw_keys;
     ctx->bucket_occ_x100 = 100;
-    ctx->label_halo_x100 = 120;
+    ctx->label_halo_x100 = 130;
     ctx->row_slots = kRowStride;
     ctx->fr_cur = -1;
     ctx->ff_cur = -1;

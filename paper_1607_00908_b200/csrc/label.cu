@@ -482,8 +482,10 @@ constexpr int kMaxUPacked = 6400;
 //            packed keys 16 * (|o|^2 - 2 c.o) + position: one integer min per (cell, candidate)
 //            gives the nearest site and the smallest-index tie-break; full 128-byte row stores.
 // A quadrant whose bound cannot be proven this way is marked and its cells take the general search.
-constexpr int kCtaQX = 4, kCtaQY = 4;                 // quadrants per CTA
+constexpr int kQW = 16, kQH = 8;                      // cells per quadrant (one candidate list each)
+constexpr int kCtaQX = 2, kCtaQY = 4;                 // quadrants per CTA: 32 x 32 cells
 constexpr int kCtaQ = kCtaQX * kCtaQY;
+constexpr int kQHWX = FP_HALF * (kQW - 1), kQHWY = FP_HALF * (kQH - 1);   // half extents of a quadrant's box of cell centres
 constexpr int kCtaThreads = 64;
 constexpr int kCtaListCap = 12;                       // candidates per quadrant (the exact test leaves about 3)
 constexpr int kCtaCapSites = 64;                      // = kCtaThreads: one gathered site per thread
@@ -519,7 +521,7 @@ struct CtaNoFused {};
 // centre are returned through R[4] = {RX0, RX1, RY0, RY1}.
 __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& sh, int lane, int wid,
                                               int32_t cxm, int32_t cym, int32_t H, int32_t* R) {
-    constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
+    constexpr int HX = FP_HALF * (kQW * kCtaQX - 1), HY = FP_HALF * (kQH * kCtaQY - 1);
     const unsigned full = 0xffffffffu;
     const int32_t Px = p.Px, Py = p.Py, halfx = p.Px >> 1, halfy = p.Py >> 1;
     const int32_t q0 = div_w(p, cxm - HX - H + Px) - p.nbx, q1 = div_w(p, cxm + HX + H + Px) - p.nbx;
@@ -590,39 +592,39 @@ template <bool kFused, typename FS>
 __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& sh, FS& fs, int q, int sub,
                                                int32_t ns, const int32_t* R, int32_t qcx, int32_t qcy,
                                                bool active) {
-    constexpr int QHW = FP_HALF * 7;
+    constexpr int kLanes = kCtaThreads / kCtaQ;         // lanes per quadrant (8)
     const unsigned full = 0xffffffffu;
     if (!active) ns = 0;
     // s*: the gathered site nearest to the quadrant centre (any one of them if several are)
     int32_t f = INT32_MAX, fi = 0;
-    for (int32_t i = sub; i < ns; i += 4) {
+    for (int32_t i = sub; i < ns; i += kLanes) {
         const int2 s2 = sh.sxy[i];
         const int32_t ox = s2.x - qcx, oy = s2.y - qcy;
         const int32_t d = ox * ox + oy * oy;
         if (d < f) { f = d; fi = i; }
     }
 #pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
+    for (int o = 1; o < kLanes; o <<= 1) {
         const int32_t g = __shfl_xor_sync(full, f, o), gi = __shfl_xor_sync(full, fi, o);
         if (g < f || (g == f && gi < fi)) { f = g; fi = gi; }
     }
     const int32_t U = isqrt_up(f) + p.r_quad;
-    int32_t margin = min(qcx - QHW - R[0] + 1, R[1] - (qcx + QHW));
-    margin = min(margin, min(qcy - QHW - R[2] + 1, R[3] - (qcy + QHW)));
+    int32_t margin = min(qcx - kQHWX - R[0] + 1, R[1] - (qcx + kQHWX));
+    margin = min(margin, min(qcy - kQHWY - R[2] + 1, R[3] - (qcy + kQHWY)));
     const bool ok = ns > 0 && U < margin && U <= kCtaMaxU;
     if (ok) {
         // Candidates: the sites that can be at least as near as s* to SOME cell of the quadrant.  For a site t,
-        // g(c) = |c - t|^2 - |c - s*|^2 is linear in c, so over the box of cell centres [-QHW, QHW]^2 it is smallest
-        // at a corner: min g = |o_t|^2 - |o_s|^2 - 2 QHW (|dx| + |dy|), (dx, dy) = o_t - o_s.  min g > 0: s* is
+        // g(c) = |c - t|^2 - |c - s*|^2 is linear in c, so over the box of cell centres [-hx, hx] x [-hy, hy] it is smallest
+        // at a corner: min g = |o_t|^2 - |o_s|^2 - 2 (hx |dx| + hy |dy|), (dx, dy) = o_t - o_s.  min g > 0: s* is
         // strictly nearer than t on every cell and t never wins (nor ties).  Every site kept lies within U of the
         // box (it is at most as far from some corner as s*), so the bounds on the packed keys still hold.
         const int32_t osx = sh.sxy[fi].x - qcx, osy = sh.sxy[fi].y - qcy;
-        for (int32_t i = sub; i < ns; i += 4) {
+        for (int32_t i = sub; i < ns; i += kLanes) {
             const int2 s2 = sh.sxy[i];
             const int32_t ox = s2.x - qcx, oy = s2.y - qcy;
             const int32_t d = ox * ox + oy * oy;
-            // |ox|, |oy| < 27000: d < 2^31; 2 QHW (|dx| + |dy|) < 1792 * 108000 < 2^31
-            if (d - f <= 2 * QHW * (abs(ox - osx) + abs(oy - osy))) {
+            // |ox|, |oy| < 27000: d < 2^31; 2 (hx |dx| + hy |dy|) < 2 * 1920 * 108000 < 2^31
+            if (d - f <= 2 * (kQHWX * abs(ox - osx) + kQHWY * abs(oy - osy))) {
                 const int32_t slot = atomicAdd(&sh.count[q], 1);
                 if (slot < kCtaListCap) {
                     if constexpr (kFused) {
@@ -643,7 +645,7 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
     if constexpr (kFused) {
         if (ok && n <= kCtaListCap) {
             // order by original index: rank = number of survivors with a smaller index (indices distinct)
-            for (int32_t k = sub; k < n; k += 4) {
+            for (int32_t k = sub; k < n; k += kLanes) {
                 const int4 e = sh.tmp[k][q];
                 int32_t r = 0;
                 for (int32_t j = 0; j < n; ++j) r += (sh.tmp[j][q].w < e.w);
@@ -655,14 +657,14 @@ __device__ __forceinline__ void cta_build_list(const LabelParams& p, CtaShared& 
         // two survivors share a residue (about 3 % of the quadrants): a tie is possible somewhere, so the list is
         // put in index order - the smallest-index rule then comes with the position in the packed key
         if (ok && n <= kCtaListCap && sh.coll[q]) {
-            for (int32_t k = sub; k < n; k += 4) {
+            for (int32_t k = sub; k < n; k += kLanes) {
                 const int4 e = sh.list[k][q];
                 int32_t r = 0;
                 for (int32_t j = 0; j < n; ++j) r += (sh.list[j][q].w < e.w);
                 sh.tmp[r][q] = e;
             }
-            __syncwarp(0xfu << ((threadIdx.x & 31) & ~3));          // the quadrant's four lanes (they branch together)
-            for (int32_t k = sub; k < n; k += 4) sh.list[k][q] = sh.tmp[k][q];
+            __syncwarp(((1u << kLanes) - 1u) << ((threadIdx.x & 31) & ~(kLanes - 1)));   // the quadrant's lanes (they branch together)
+            for (int32_t k = sub; k < n; k += kLanes) sh.list[k][q] = sh.tmp[k][q];
         }
     }
     if (sub == 0 && active)
@@ -734,22 +736,22 @@ template <bool kFused>
 __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kernel(const __grid_constant__ LabelParams p,
                                                                 int32_t* __restrict__ labels,
                                                                 const __grid_constant__ RowSet rs) {
-    constexpr int QHW = FP_HALF * 7;
-    constexpr int HX = FP_HALF * (8 * kCtaQX - 1), HY = FP_HALF * (8 * kCtaQY - 1);
+    constexpr int kLanes = kCtaThreads / kCtaQ;
+    constexpr int HX = FP_HALF * (kQW * kCtaQX - 1), HY = FP_HALF * (kQH * kCtaQY - 1);
     __shared__ CtaShared sh;
     __shared__ typename std::conditional<kFused, CtaFusedShared, CtaNoFused>::type fs;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int32_t X0 = p.wx0 + blockIdx.x * (8 * kCtaQX), Y0 = p.wy0 + blockIdx.y * (8 * kCtaQY);
+    const int32_t X0 = p.wx0 + blockIdx.x * (kQW * kCtaQX), Y0 = p.wy0 + blockIdx.y * (kQH * kCtaQY);
     // ---- phases G + A; quadrants whose bound could not be proven get one retry with a wider halo
     if (threadIdx.x < kCtaQ) { sh.count[threadIdx.x] = 0; sh.coll[threadIdx.x] = 0; }
-    (&sh.res[0][0])[threadIdx.x] = 0; (&sh.res[0][0])[threadIdx.x + kCtaThreads] = 0;
-    static_assert(kCtaQ * 8 == 2 * kCtaThreads, "two residue words per thread");
+    (&sh.res[0][0])[threadIdx.x] = 0;
+    static_assert(kCtaQ * 8 == kCtaThreads, "one residue word per thread");
     if constexpr (kFused) {
         for (int i = threadIdx.x; i < kCtaCapSites * kCtaCapSites / 32; i += kCtaThreads) fs.bm[i] = 0;
     }
     bool any_fail = false;
     {
-        const int q = threadIdx.x >> 2, sub = threadIdx.x & 3;
+        const int q = threadIdx.x / kLanes, sub = threadIdx.x % kLanes;
         const int qx = q % kCtaQX, qy = q / kCtaQX;
         bool active = true;
         for (int attempt = 0; attempt < 2; ++attempt) {
@@ -759,13 +761,13 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
                                            FP_ONE * Y0 + FP_HALF + HY, H, R);
             __syncthreads();
             const int32_t ns = got ? sh.nkept : 0;
-            cta_build_list<kFused>(p, sh, fs, q, sub, ns, R, 8 * FP_ONE * qx + QHW - HX, 8 * FP_ONE * qy + QHW - HY, active);
+            cta_build_list<kFused>(p, sh, fs, q, sub, ns, R, kQW * FP_ONE * qx + kQHWX - HX, kQH * FP_ONE * qy + kQHWY - HY, active);
             __syncthreads();
             active = sh.count[q] < 0;
             any_fail = __syncthreads_or(active);
             if (!any_fail) break;
             if (attempt == 0 && active) {                                // reset the survivor counter and the residues
-                sh.res[q][2 * sub] = 0; sh.res[q][2 * sub + 1] = 0;
+                sh.res[q][sub] = 0;
                 if (sub == 0) { sh.count[q] = 0; sh.coll[q] = 0; }
             }
             __syncthreads();
@@ -777,10 +779,11 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
             p.dirty_tiles[atomicAdd(p.dirty_count, 1)] = blockIdx.y * gridDim.x + blockIdx.x;
     }
     // ---- phase B: warp = 32 x 16 cells, lane = column
-    const int wx = wid % (kCtaQX / 4), wy = wid / (kCtaQX / 4);
+    const int wx = 0, wy = wid;                          // a warp covers the tile's 32 columns and 16 of its rows
+    static_assert(kQW * kCtaQX == 32 && kQH == 8 && kCtaQY == 4, "lane = column; two quadrant rows per warp");
     const int32_t x = X0 + 32 * wx + lane;
-    const int qx = 4 * wx + (lane >> 3);
-    const int32_t cxr = FP_ONE * (lane & 7) - QHW;
+    const int qx = lane / kQW;
+    const int32_t cxr = FP_ONE * (lane % kQW) - kQHWX;
     uint32_t W[4] = {0, 0, 0, 0};                        // fused: slots of the lane's 16 cells
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -818,13 +821,13 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
                 const int32_t a1 = 16 * (c1.z + cxr * c1.x) + k + 1, y1s = 16 * c1.y;
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
-                    best[j] = min(best[j], min(a0 + (FP_ONE * j - QHW) * y0s, a1 + (FP_ONE * j - QHW) * y1s));
+                    best[j] = min(best[j], min(a0 + (FP_ONE * j - kQHWY) * y0s, a1 + (FP_ONE * j - kQHWY) * y1s));
             }
             if (k < n) {
                 const int4 c0 = sh.list[k][q];
                 const int32_t a0 = 16 * (c0.z + cxr * c0.x) + k, y0s = 16 * c0.y;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) best[j] = min(best[j], a0 + (FP_ONE * j - QHW) * y0s);
+                for (int j = 0; j < 8; ++j) best[j] = min(best[j], a0 + (FP_ONE * j - kQHWY) * y0s);
             }
 #pragma unroll
             for (int j = 0; j < 8; ++j) sel[j] = best[j] & 15;                   // key = 16 t + position
@@ -838,7 +841,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
                 const int32_t a = c.z + cxr * c.x;
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
-                    const int32_t t = a + (FP_ONE * j - QHW) * c.y;
+                    const int32_t t = a + (FP_ONE * j - kQHWY) * c.y;
                     if (t < best[j]) { best[j] = t; sel[j] = k; }
                 }
             }
@@ -985,6 +988,7 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, int32_t x0, int32_t y0,
     p.halo0 = p.r_tile + (int32_t)(0.75 * spacing * FP_ONE);
     const double qh = 128.0 * (tw / 2 - 1);
     p.r_quad = (int32_t)ceil(sqrt(2.0 * qh * qh));
+    if (path == 3) p.r_quad = (int32_t)ceil(sqrt((double)kQHWX * kQHWX + (double)kQHWY * kQHWY));   // 16 x 8 quadrants
     p.halo_fast = p.r_quad + (int32_t)(0.01 * (double)ctx->label_halo_x100 * spacing * FP_ONE);
     {   // magic numbers for floor(x / w), x < 2^32
         const uint32_t d = (uint32_t)ctx->w;
@@ -1007,7 +1011,7 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, int32_t x0, int32_t y0,
         p.fail_count = ctx->d_lab_fail_n + ctx->lab_fail_turn;
         p.fail_count_next = ctx->d_lab_fail_n + (1 - ctx->lab_fail_turn);
         ctx->lab_fail_turn = 1 - ctx->lab_fail_turn;
-        dim3 grid((ww + 8 * kCtaQX - 1) / (8 * kCtaQX), (wh + 8 * kCtaQY - 1) / (8 * kCtaQY));
+        dim3 grid((ww + kQW * kCtaQX - 1) / (kQW * kCtaQX), (wh + kQH * kCtaQY - 1) / (kQH * kCtaQY));
         if (rs) {
             p.col_left = ctx->d_fu_cols;
             p.col_right = ctx->d_fu_cols + (size_t)(ctx->Lx / 32) * ctx->Ly;
