@@ -26,8 +26,8 @@ sys.path.insert(0, ROOT)
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
 # Per-launch ncu figures of the committed `ncu --set full` capture (config 5 only): DRAM bytes read + written,
-# issue-slot utilisation, warp instructions.  profiles/r2f_traffic.md names the command that produced the table.
-NCU_TABLE = os.path.join(ROOT, "profiles", "r2f_traffic.csv")
+# issue-slot utilisation, warp instructions.  profiles/r2g_traffic.md names the command that produced the table.
+NCU_TABLE = os.path.join(ROOT, "profiles", "r2g_traffic.csv")
 
 
 def ncu_table():
