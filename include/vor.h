@@ -40,7 +40,8 @@ typedef enum {
     VOR_EINVAL = -1,    /* bad argument (null pointer, size out of range) */
     VOR_ECAPACITY = -2, /* an output or scratch buffer was too small (sticky, see above) */
     VOR_ECUDA = -3,     /* a CUDA runtime call failed; vor_last_error() has the text */
-    VOR_ESTATE = -4     /* call order violation (e.g. vor_label before vor_build_cells) */
+    VOR_ESTATE = -4,    /* call order violation (e.g. vor_label before vor_build_cells) */
+    VOR_ELIMIT = -5     /* a size exceeds a fixed, compiled-in maximum (vor_diff_rows_static only) */
 } vor_status;
 
 /* Create a context for an L x L lattice (2 <= L <= 2^22) and at most max_sites sites
@@ -185,6 +186,38 @@ int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_t* d_prev_r
                   const uint64_t* d_now, const uint32_t* d_now_row_ptr, int32_t n_rows,
                   uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
                   int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
+
+/* ---- a5 for callers that must not allocate.
+ * Who needs this: code that runs where a device allocation is forbidden or impossible - inside a host framework
+ * whose memory pool owns the whole GPU and hands out only the buffers it was asked for up front, in a
+ * process that fixed its memory budget at start-up, or on a latency path where cudaMalloc's implicit device-wide
+ * synchronisation is not acceptable.  Every other call of this library needs a vor_ctx, and vor_create (plus
+ * a few lazily sized buffers, vor_diff_rows' among them) calls cudaMalloc.  This call takes NO context and
+ * never calls cudaMalloc, cudaFree or any routine that allocates: the comparison's working memory (one mask
+ * word per row and two counters per block of 512 rows) is a fixed array that is part of the library image.
+ *
+ * The result is exactly vor_diff_rows': created = now \ prev, destroyed = prev \ now, ascending; the counts
+ * hold the REQUIRED numbers and nothing is written past `cap`.  There is no context to latch an overflow in:
+ * compare *d_n_created / *d_n_destroyed with cap yourself.  All pointers are device memory owned by the
+ * caller; the call enqueues two kernels on `stream` and returns.
+ *
+ * Limit: n_rows <= VOR_DIFF_ROWS_STATIC_MAX_ROWS (2^20 rows; the array costs 4.02 MiB of device memory on
+ * every GPU that loads libvor, from load until the process exits).  A larger n_rows returns VOR_ELIMIT and
+ * does nothing; a null pointer, cap < 0 or n_rows < 1 returns VOR_EINVAL.
+ *
+ * First call on each device: the library looks up the array's device address (cudaGetSymbolAddress, with the
+ * caller's current device - keep the device whose memory you pass current).  Make that first call during
+ * set-up, before you start any stream capture on that device.  Later calls only launch.
+ *
+ * The array is shared by every call in the process on that device and keeps whatever the last call left in
+ * it.  Nothing in it has to start at zero: each call overwrites every word it later reads.  For the same
+ * reason two calls whose kernels can run at the same time on one GPU (different streams, different threads)
+ * corrupt each other: issue them on one stream, or order them with events. */
+#define VOR_DIFF_ROWS_STATIC_MAX_ROWS (1 << 20)
+int vor_diff_rows_static(const uint64_t* d_prev, const uint32_t* d_prev_row_ptr,
+                         const uint64_t* d_now, const uint32_t* d_now_row_ptr, int32_t n_rows,
+                         uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
+                         int64_t* d_n_created, int64_t* d_n_destroyed, void* stream);
 
 /* ---- trigger and event counts: the paper's own outputs on top of the diff (PAPER.md:215-221
  * §III.B.3 local_trigger / global_trigger; §III.B.4 eventsIndices / eventsNumber;

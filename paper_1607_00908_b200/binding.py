@@ -15,8 +15,9 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvor.so")
 
-VOR_OK, VOR_EINVAL, VOR_ECAPACITY, VOR_ECUDA, VOR_ESTATE = 0, -1, -2, -3, -4
-_STATUS = {0: "VOR_OK", -1: "VOR_EINVAL", -2: "VOR_ECAPACITY", -3: "VOR_ECUDA", -4: "VOR_ESTATE"}
+VOR_OK, VOR_EINVAL, VOR_ECAPACITY, VOR_ECUDA, VOR_ESTATE, VOR_ELIMIT = 0, -1, -2, -3, -4, -5
+_STATUS = {0: "VOR_OK", -1: "VOR_EINVAL", -2: "VOR_ECAPACITY", -3: "VOR_ECUDA", -4: "VOR_ESTATE", -5: "VOR_ELIMIT"}
+VOR_DIFF_ROWS_STATIC_MAX_ROWS = 1 << 20      # include/vor.h
 
 # name -> (restype, argtypes); mirrors include/vor.h one to one
 _P = C.c_void_p
@@ -48,6 +49,7 @@ SIGNATURES = {
     "vor_edges_rows": (C.c_int, [_P, _P, _P, C.c_int64, _P, _P, _P]),
     "vor_diff": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, C.c_int32, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
     "vor_diff_rows": (C.c_int, [_P, _P, _P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
+    "vor_diff_rows_static": (C.c_int, [_P, _P, _P, _P, C.c_int32, _P, _P, C.c_int64, _P, _P, _P]),
     "vor_events": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, _P, C.c_int64, C.c_int64, C.c_int32,
                              _P, _P, _P, _P, _P, _P, _P]),
     "vor_t1_events": (C.c_int, [_P, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, _P, _P, _P, C.c_int64, C.c_int64, _P, C.c_int32,
@@ -107,6 +109,32 @@ def _ptr(t, dtype=None):
 
 def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def vor_diff_rows_static(prev, prev_row_ptr, now, now_row_ptr, n_rows, created, destroyed, n_created, n_destroyed):
+    """vor_diff_rows without a context and without any device allocation inside the library.
+
+    For programs that cannot let a library call cudaMalloc: the GPU's memory belongs to someone else's pool
+    (you only hold the tensors you were given), the memory budget was fixed at start-up, or the call sits on a
+    path where an allocation's device-wide synchronisation is unacceptable.  The working memory is a fixed
+    4 MiB array inside libvor.so, so n_rows is limited to VOR_DIFF_ROWS_STATIC_MAX_ROWS (2^20); more raises
+    VorError(VOR_ELIMIT).  All tensors are the caller's; same result as Vor.vor_diff_rows.  An overflow of
+    created / destroyed is NOT latched anywhere: compare the counts with the capacities.  The array is shared
+    by all calls on a device - keep them on one stream.  Make the first call on a device before any stream
+    capture (it looks up the array's address)."""
+    lib = load_library()
+    assert min(prev_row_ptr.numel(), now_row_ptr.numel()) >= n_rows + 1
+    cap = min(created.numel(), destroyed.numel())
+    rc = lib.vor_diff_rows_static(
+        _ptr(prev, torch.int64), _ptr(prev_row_ptr, torch.int32), _ptr(now, torch.int64),
+        _ptr(now_row_ptr, torch.int32), n_rows, _ptr(created, torch.int64), _ptr(destroyed, torch.int64),
+        cap, _ptr(n_created, torch.int64), _ptr(n_destroyed, torch.int64), _stream())
+    if rc == VOR_ELIMIT:
+        raise VorError(rc, f"vor_diff_rows_static: n_rows = {n_rows} exceeds the built-in maximum "
+                           f"VOR_DIFF_ROWS_STATIC_MAX_ROWS = {VOR_DIFF_ROWS_STATIC_MAX_ROWS}; use Vor.vor_diff_rows")
+    if rc != VOR_OK:
+        raise VorError(rc, "vor_diff_rows_static: null pointer, cap < 0 or n_rows < 1" if rc == VOR_EINVAL
+                       else "vor_diff_rows_static: a CUDA call failed")
 
 
 class Vor:

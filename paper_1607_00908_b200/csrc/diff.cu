@@ -11,6 +11,8 @@
 // across the grid sync that separates counting from the order-preserving write.
 #include <cooperative_groups.h>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "rows.cuh"
 
@@ -527,6 +529,69 @@ extern "C" int vor_diff_rows(vor_ctx* ctx, const uint64_t* d_prev, const uint32_
                       d_n_created, d_n_destroyed, ctx->d_dr_scratch, ctx->d_dr_scratch + ctx->dr_rows, ctx->d_flags};
     VOR_LAUNCH(diff_rows_mark_kernel, (unsigned)n_blocks, kDrThreads, 0, stream, dp);
     VOR_LAUNCH(diff_rows_write_kernel, (unsigned)n_blocks, kDrThreads, 0, stream, dp);
+    return VOR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// vor_diff_rows_static: the row-by-row comparison for callers that may not allocate device memory (a host
+// framework that owns the GPU's memory pool, a process with a memory budget fixed at start-up, a latency path
+// that cannot take cudaMalloc's device-wide synchronisation).  Same two kernels as vor_diff_rows; their working
+// memory is the file-scope array below instead of a context buffer.  include/vor.h states the contract.
+namespace {
+
+constexpr int64_t kStaticMaxRows = VOR_DIFF_ROWS_STATIC_MAX_ROWS;
+constexpr int64_t kStaticMaxBlocks = (kStaticMaxRows + kDrRows - 1) / kDrRows;
+constexpr int64_t kStaticWords = kStaticMaxRows + 2 * kStaticMaxBlocks + 64;   // masks | block counts | flag word
+
+// 4.02 MiB in the image of every GPU that loads the library.  HOST code must not use this name as a pointer:
+// there it is only a handle for cudaGetSymbolAddress (static_scratch_address below).
+static __device__ __align__(256) uint32_t g_static_scratch[kStaticWords];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+uint32_t* g_static_addr[kStaticMaxDevices];     // device address of g_static_scratch, per device ordinal
+
+// Device address of the array on the CURRENT device; looked up once per device, with that device current.
+cudaError_t static_scratch_address(uint32_t** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[dev]) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_static_addr[dev] = static_cast<uint32_t*>(ptr);
+    }
+    *out = g_static_addr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int vor_diff_rows_static(const uint64_t* d_prev, const uint32_t* d_prev_row_ptr,
+                                    const uint64_t* d_now, const uint32_t* d_now_row_ptr, int32_t n_rows,
+                                    uint64_t* d_created, uint64_t* d_destroyed, int64_t cap,
+                                    int64_t* d_n_created, int64_t* d_n_destroyed, void* stream_) {
+    if (!d_prev || !d_prev_row_ptr || !d_now || !d_now_row_ptr || !d_created || !d_destroyed ||
+        !d_n_created || !d_n_destroyed || cap < 0 || n_rows < 1)
+        return VOR_EINVAL;
+    if (n_rows > kStaticMaxRows) return VOR_ELIMIT;       // before any CUDA call: nothing is enqueued
+    uint32_t* scratch = nullptr;
+    if (static_scratch_address(&scratch) != cudaSuccess) return VOR_ECUDA;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const unsigned n_blocks = (unsigned)(((int64_t)n_rows + kDrRows - 1) / kDrRows);
+    // masks: words [0, n_rows); block counts: 2 * n_blocks words from kStaticMaxRows on; the last word takes the
+    // kernels' overflow bit, which nobody reads here (the caller compares the counts with cap).  Every word the
+    // second kernel reads is written by the first one, so stale contents of an earlier call never matter.
+    DiffRowsParams dp{d_prev, d_prev_row_ptr, d_now, d_now_row_ptr, n_rows, d_created, d_destroyed, cap,
+                      d_n_created, d_n_destroyed, scratch, scratch + kStaticMaxRows,
+                      reinterpret_cast<int32_t*>(scratch + kStaticWords - 1)};
+    diff_rows_mark_kernel<<<n_blocks, kDrThreads, 0, stream>>>(dp);
+    if (cudaGetLastError() != cudaSuccess) return VOR_ECUDA;
+    diff_rows_write_kernel<<<n_blocks, kDrThreads, 0, stream>>>(dp);
+    if (cudaGetLastError() != cudaSuccess) return VOR_ECUDA;
     return VOR_OK;
 }
 
