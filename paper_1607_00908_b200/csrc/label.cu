@@ -4,8 +4,13 @@
 // one thread per lattice site looping over ALL centres; this file computes the same argmin over a
 // pruned candidate set that provably contains every cell's nearest site.
 //
-// Two code paths, both exact:
-//  * tile path (fast): one warp per TW x TH tile of cells.
+// Three code paths, all exact (vor_set_option "label_path"; 0 = the library picks):
+//  * CTA path (3; the DEFAULT wherever the site density allows it, e.g. every BASELINE config): label_cta_kernel
+//    further down - 64 threads per 32 x 32 cells, one shared gather, eight 16 x 8 quadrants with exact bisector
+//    candidate lists, packed-key scan; label_fixup_kernel takes the quadrants it cannot prove.  Described at its
+//    definition ("A CTA of 64 threads ...").
+//  * tile path (2): one warp per TW x TH tile of cells - the round-1 design, kept for lattices the CTA path
+//    does not take and as a parity cross-check.
 //      1. gather the sites of the cell-list buckets covering the tile's bounding box grown by a halo
 //         H (bucket rows are contiguous in the bucket-ordered site array: coalesced loads);
 //      2. dc = distance from the tile centre to its nearest gathered site.  The nearest-site
@@ -24,7 +29,7 @@
 //    the candidates per cell; each lane's cells lie in one quadrant, so it scans that quadrant's list.
 //    Anything the lean variant cannot prove (too many sites, halo too small) falls back to the
 //    generic tile code above, and from there to the general path.
-//  * general path: one thread per cell, ring search over cell-list buckets in int64 with the
+//  * general path (1): one thread per cell, ring search over cell-list buckets in int64 with the
 //    minimum-image metric.  After scanning all buckets within Chebyshev bucket distance r of the
 //    cell's own bucket every other site has |dx| or |dy| > r*w, so the search stops once
 //    best_d2 <= (r*w)^2; when the ring would wrap onto itself it scans all sites.  Used for tiny
@@ -468,13 +473,13 @@ constexpr int kMaxUPacked = 6400;
 
 // ---------------------------------------------------------------- CTA three-phase path (default)
 // The per-quadrant candidate lists are inherently small, scalar work (a few dozen distance tests per
-// 8 x 8 quadrant), so they are built by a few threads per quadrant instead of one warp per tile.
-// A CTA of 64 threads covers 32 x 32 cells = 4 x 4 quadrants:
+// quadrant), so they are built by a few threads per quadrant instead of one warp per tile.
+// A CTA of 64 threads covers 32 x 32 cells = 2 x 4 quadrants of 16 x 8 cells:
 //   phase G  the sites of the cell-list buckets covering the CTA's cells plus the halo are gathered
 //            into shared memory (coalesced row segments, coordinates relative to the CTA centre);
 //            every warp computes the segment prefix, warp w loads items [32w, 32w+32); only the sites
 //            inside the exact rectangle box +/- halo are kept;
-//   phase A  4 lanes per quadrant build its candidate list from the shared site list:
+//   phase A  8 lanes per quadrant build its candidate list from the shared site list:
 //            U_q = dist(quadrant centre, nearest gathered site) + quadrant radius; the gathered region
 //            must reach U_q beyond the quadrant box on every side; candidates = gathered sites within
 //            U_q of the box, ordered by original index;
@@ -524,10 +529,14 @@ __device__ __forceinline__ int32_t cta_gather(const LabelParams& p, CtaShared& s
     constexpr int HX = FP_HALF * (kQW * kCtaQX - 1), HY = FP_HALF * (kQH * kCtaQY - 1);
     const unsigned full = 0xffffffffu;
     const int32_t Px = p.Px, Py = p.Py, halfx = p.Px >> 1, halfy = p.Py >> 1;
+    // a region wider than half a period is unusable (the test on the bucket span below would say the same); asked
+    // first, it keeps div_w's arguments >= 0 and the products below inside int32 on small lattices, where the halo
+    // (the retry's above all) can exceed the period
+    if (2 * (HX + H) > halfx || 2 * (HY + H) > halfy) return 0;
     const int32_t q0 = div_w(p, cxm - HX - H + Px) - p.nbx, q1 = div_w(p, cxm + HX + H + Px) - p.nbx;
     const int32_t r0 = div_w(p, cym - HY - H + Py) - p.nby, r1 = div_w(p, cym + HY + H + Py) - p.nby;
     const int32_t ncols = q1 - q0 + 1, nrows = r1 - r0 + 1;
-    if (ncols * p.w > halfx || nrows * p.w > halfy) return 0;
+    if ((int64_t)ncols * p.w > halfx || (int64_t)nrows * p.w > halfy) return 0;
     // the buckets cover more than asked for; only the sites inside the exact rectangle
     // [-HX-H, HX+H] x [-HY-H, HY+H] are kept (shorter lists for every quadrant), so that rectangle is
     // the region the coverage test may rely on: R = {x lower (inclusive), x upper (exclusive), y ...}
@@ -749,7 +758,11 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     if constexpr (kFused) {
         for (int i = threadIdx.x; i < kCtaCapSites * kCtaCapSites / 32; i += kCtaThreads) fs.bm[i] = 0;
     }
-    bool any_fail = false;
+    // first_fail: some quadrant was not proven with the first gather.  The retry gathers a different, larger site
+    // list, so the slots (fin.y) of the quadrants proven first and of those proven on the retry index different
+    // lists: the fused kernel never pairs them and hands such a tile to the label-image path (labels use fin.x
+    // and are right either way).
+    bool any_fail = false, first_fail = false;
     {
         const int q = threadIdx.x / kLanes, sub = threadIdx.x % kLanes;
         const int qx = q % kCtaQX, qy = q / kCtaQX;
@@ -765,6 +778,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
             __syncthreads();
             active = sh.count[q] < 0;
             any_fail = __syncthreads_or(active);
+            if (attempt == 0) first_fail = any_fail;
             if (!any_fail) break;
             if (attempt == 0 && active) {                                // reset the survivor counter and the residues
                 sh.res[q][sub] = 0;
@@ -775,7 +789,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
     }
     // fused: a tile with an unproven quadrant gets its pairs from the label image later (tile list)
     if constexpr (kFused) {
-        if (any_fail && threadIdx.x == 0)
+        if (first_fail && threadIdx.x == 0)
             p.dirty_tiles[atomicAdd(p.dirty_count, 1)] = blockIdx.y * gridDim.x + blockIdx.x;
     }
     // ---- phase B: warp = 32 x 16 cells, lane = column
@@ -869,7 +883,7 @@ __global__ void __launch_bounds__(kCtaThreads, kFused ? 20 : 24) label_cta_kerne
         }
     }
     if constexpr (kFused) {
-        if (any_fail) return;                            // CTA-uniform
+        if (first_fail) return;                          // CTA-uniform
         cta_pairs(W, lane, fs.bm);
         if (wid == 0) fs.seam[lane] = W[3] >> 24;        // row 15 of the tile
         __syncthreads();
@@ -989,7 +1003,11 @@ static int label_launch(vor_ctx* ctx, int32_t* d_labels, int32_t x0, int32_t y0,
     const double qh = 128.0 * (tw / 2 - 1);
     p.r_quad = (int32_t)ceil(sqrt(2.0 * qh * qh));
     if (path == 3) p.r_quad = (int32_t)ceil(sqrt((double)kQHWX * kQHWX + (double)kQHWY * kQHWY));   // 16 x 8 quadrants
-    p.halo_fast = p.r_quad + (int32_t)(0.01 * (double)ctx->label_halo_x100 * spacing * FP_ONE);
+    {   // limited to 2^24 units (65536 cells: far beyond any usable gather region), so that the retry's
+        // 2 * halo_fast + w stays inside int32 for a handful of sites on a huge lattice
+        const double hf = 0.01 * (double)ctx->label_halo_x100 * spacing * FP_ONE;
+        p.halo_fast = p.r_quad + (int32_t)(hf < 16777216.0 ? hf : 16777216.0);
+    }
     {   // magic numbers for floor(x / w), x < 2^32
         const uint32_t d = (uint32_t)ctx->w;
         uint32_t l = 0;

@@ -2,6 +2,8 @@
 
 Integer / index work: bit-exact.  Centroids (float64): |diff| <= 1e-9 lattice units (north_star).
 """
+import zlib
+
 import numpy as np
 import pytest
 
@@ -409,7 +411,7 @@ def test_frame_fused_label_edges_adversarial(G, name, L, gen):
     """vor_frame_* labels and extracts the pairs in ONE kernel where the lattice allows it (L % 32 == 0,
     CTA labelling path); tiles with an unproven quadrant, the tile seams and the periodic wrap take the
     side paths.  Labels, edge list and flips must equal the oracle's, and the unfused calls' results."""
-    rng = np.random.default_rng(abs(hash(name)) % 2**32)
+    rng = np.random.default_rng(zlib.crc32(name.encode()))   # fixed per case: str hashes change per process
     P = FP * L
     sx, sy = gen(rng, P)
     frames = [(sx, sy), (((sx.astype(np.int64) + rng.integers(-600, 600, len(sx))) % P).astype(np.int32),
@@ -434,6 +436,39 @@ def test_frame_fused_label_edges_adversarial(G, name, L, gen):
             assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd)
             prev = e
         v.close()
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_frame_fused_retry_with_wider_halo(G, seed):
+    """a dense half and a sparse half on one lattice.  The halo follows the MEAN spacing (~9.5 cells), so
+    in the sparse half (spacing ~24 cells) most quadrants fail the first attempt of the CTA kernel and succeed on
+    its retry with the wider halo (<= 64 sites gathered).  The fused kernel must not pair slots of the two
+    attempts' site lists: such a tile takes its pairs from the label image."""
+    L = 1024
+    P = FP * L
+    rng = np.random.default_rng(seed)
+    nd, ns = (L // 2) * L // 49, (L // 2) * L // 576
+    sx = np.concatenate([rng.integers(0, P // 2, nd), rng.integers(P // 2, P, ns)]).astype(np.int32)
+    sy = rng.integers(0, P, nd + ns).astype(np.int32)
+    perm = rng.permutation(nd + ns)
+    sx, sy = sx[perm], sy[perm]
+    lab = oracle.label_cells(L, sx, sy, 16)
+    e = oracle.edges(lab)
+    cap = 16 * len(sx)
+    res = []
+    for fuse in (1, 0):
+        v = make(L, len(sx))
+        v.vor_set_option("fuse", fuse)
+        v.vor_set_option("label_path", 3)
+        hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+        v.vor_frame_host(sx, sy, hc, hd, cnt)
+        pl, pe, _, _, _ = v.vor_frame_results()
+        got = G.from_device_ptr(pl, L * L, torch.int32).cpu().numpy().reshape(L, L)
+        assert np.array_equal(got, lab), (fuse, int((got != lab).sum()))
+        ge = G.u64(G.from_device_ptr(pe, min(int(cnt[0]), cap), torch.int64))
+        res.append((int(cnt[0]), len(np.setdiff1d(ge, e)), len(np.setdiff1d(e, ge))))
+        v.close()
+    assert res == [(len(e), 0, 0)] * 2, f"(count, spurious, missing) fused / unfused: {res}, expected {len(e)}"
 
 
 @pytest.mark.parametrize("pin", [False, True])
