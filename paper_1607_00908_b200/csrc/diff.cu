@@ -614,11 +614,18 @@ struct MergeRound {
     int32_t n_lists;
     int32_t span;              // lists per input segment (1, 2, 4, ...); output segments hold 2 * span lists
     int64_t* total;            // sum of the (clamped) counts
+    int32_t* flags;            // sticky status: FLAG_EDGE_CAP when a count exceeds the stride
 };
 
 __global__ void __launch_bounds__(kMlThreads) merge_round_kernel(const MergeRound m) {
     __shared__ int64_t pre[kMlMaxLists + 1];
-    for (int l = threadIdx.x; l < m.n_lists; l += kMlThreads) pre[l + 1] = min(max(m.counts[l], (int64_t)0), m.stride);
+    for (int l = threadIdx.x; l < m.n_lists; l += kMlThreads) {
+        const int64_t c = m.counts[l];
+        pre[l + 1] = min(max(c, (int64_t)0), m.stride);
+        // a list that overflowed its slot upstream is merged truncated: every rank that merges it must hear of it,
+        // not only the rank that produced it (its own vor_edges_image latched the same bit there)
+        if (m.round0 && blockIdx.x == 0 && c > m.stride) atomicOr(m.flags, FLAG_EDGE_CAP);
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
         pre[0] = 0;
@@ -757,13 +764,13 @@ extern "C" int vor_merge_lists(vor_ctx* ctx, const uint64_t* d_lists, int64_t st
     const uint64_t* src = d_lists;
     int which = 0;
     for (int32_t span = 1, round = 0; round == 0 || span < n_lists; span *= 2, ++round) {
-        MergeRound m{src, round == 0, stride, buf[which], d_counts, n_lists, span, ctx->d_n_raw};
+        MergeRound m{src, round == 0, stride, buf[which], d_counts, n_lists, span, ctx->d_n_raw, ctx->d_flags};
         VOR_LAUNCH(merge_round_kernel, grid, kMlThreads, 0, stream, m);
         src = buf[which];
         which ^= 1;
     }
     UniqueParams up{src, ctx->d_n_raw, ctx->max_raw_keys, d_out, cap, d_n_out, ctx->d_blk_count, ctx->d_flags, FLAG_EDGE_CAP};
-    const int ugrid = 4 * ctx->num_sms;                     // <= 2 * kMaxCoopBlocks partials
+    const int ugrid = min(4 * ctx->num_sms, 2 * kMaxCoopBlocks);   // one partial per block in d_blk_count
     VOR_LAUNCH(unique_count_kernel, ugrid, kMlThreads, 0, stream, up);
     VOR_LAUNCH(unique_write_kernel, ugrid, kMlThreads, 0, stream, up);
     return VOR_OK;

@@ -157,7 +157,7 @@ extern "C" int vor_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d
     VOR_CUDA(cudaMemsetAsync(d_trigger, 0, bytes, stream));
     VOR_CUDA(cudaMemsetAsync(d_count_prev, 0, bytes, stream));
     VOR_CUDA(cudaMemsetAsync(d_count_now, 0, bytes, stream));
-    const int grid = 4 * ctx->num_sms;                      // <= 2 * kMaxCoopBlocks partials
+    const int grid = min(4 * ctx->num_sms, kMaxCoopBlocks);   // d_blk_count holds 2 * kMaxCoopBlocks partials
     VOR_LAUNCH(ev_mark_kernel, grid, 256, 0, stream, d_created, d_n_created, d_destroyed, d_n_destroyed,
                cap_created, cap_destroyed, n_labels, d_trigger);
     VOR_LAUNCH(ev_count_kernel, grid, kEvThreads, 0, stream, d_trigger, n_labels, ctx->d_blk_count);
@@ -518,7 +518,7 @@ static int t1_graphs(vor_ctx* ctx, const uint64_t* d_prev, const int64_t* d_n_pr
 static int t1_build_graphs(vor_ctx* ctx, const T1Graph& gp, const T1Graph& gn, int32_t n_labels, cudaStream_t stream) {
     const size_t n1 = (size_t)n_labels + 1;
     VOR_CUDA(cudaMemsetAsync(gp.deg, 0, 2 * n1 * sizeof(uint32_t), stream));
-    const int grid = 4 * ctx->num_sms;
+    const int grid = min(4 * ctx->num_sms, kMaxCoopBlocks);
     const dim3 both(grid, 2);
     VOR_LAUNCH(t1_degree_kernel, both, 256, 0, stream, gp, gn, n_labels);
     VOR_LAUNCH(t1_scan_sum_kernel, both, kEvThreads, 0, stream, gp, gn, n_labels, ctx->d_blk_count);
@@ -552,7 +552,7 @@ extern "C" int vor_t1_events(vor_ctx* ctx, const uint64_t* d_prev, const int64_t
     if ((rc = t1_scratch(ctx, 4, ((size_t)(cap_now + cap_destroyed) + 1) * sizeof(uint64_t), (void**)&U)) != VOR_OK) return rc;
     T1Lists l{d_now, d_n_now, cap_now, d_created, d_n_created, cap_created, d_destroyed, d_n_destroyed, cap_destroyed};
 
-    const int grid = 4 * ctx->num_sms;                      // 2 * grid partials <= 2 * kMaxCoopBlocks
+    const int grid = min(4 * ctx->num_sms, kMaxCoopBlocks);   // 2 * grid partials in d_blk_count
     if ((rc = t1_build_graphs(ctx, gp, gn, n_labels, stream)) != VOR_OK) return rc;
     VOR_LAUNCH(t1_union_kernel, grid, kEvThreads, 0, stream, l, d_trigger, n_labels, U, ctx->d_blk_count);
     VOR_LAUNCH(t1_write_kernel, grid, kEvThreads, 0, stream, U, l, ctx->d_blk_count, d_couples, d_class, cap,
@@ -596,7 +596,7 @@ extern "C" int vor_edge_commons(vor_ctx* ctx, const uint64_t* d_edges, const int
     if ((rc = t1_scratch(ctx, 3, n_adj * sizeof(uint32_t), (void**)&adj_s)) != VOR_OK) return rc;
     T1Graph g{d_edges, d_n_edges, cap_edges, deg, off, adj_u, adj_s};
     VOR_CUDA(cudaMemsetAsync(deg, 0, n1 * sizeof(uint32_t), stream));
-    const int grid = 4 * ctx->num_sms;
+    const int grid = min(4 * ctx->num_sms, kMaxCoopBlocks);
     const dim3 one(grid, 1);                                 // blockIdx.y == 0: the kernels read only the first graph
     VOR_LAUNCH(t1_degree_kernel, one, 256, 0, stream, g, g, n_labels);
     VOR_LAUNCH(t1_scan_sum_kernel, one, kEvThreads, 0, stream, g, g, n_labels, ctx->d_blk_count);
@@ -669,7 +669,7 @@ extern "C" int vor_event_vertices(vor_ctx* ctx, const uint64_t* d_prev, const in
     if ((rc = t1_build_graphs(ctx, gp, gn, n_labels, stream)) != VOR_OK) return rc;
     VOR_CUDA(cudaMemsetAsync(d_boundary_prev, 0, (size_t)n_labels * sizeof(int32_t), stream));
     VOR_CUDA(cudaMemsetAsync(d_boundary_now, 0, (size_t)n_labels * sizeof(int32_t), stream));
-    const int grid = 4 * ctx->num_sms;
+    const int grid = min(4 * ctx->num_sms, kMaxCoopBlocks);
     VOR_LAUNCH(ev_boundary_kernel, dim3(4 * grid, 2), 256, 0, stream, gp, gn, n_labels, d_boundary_prev, d_boundary_now);
     VOR_LAUNCH(ev_vclass_kernel, 4 * grid, 256, 0, stream, gp, gn, d_trigger, n_labels, d_boundary_prev, d_boundary_now,
                d_vclass);

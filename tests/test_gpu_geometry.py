@@ -384,7 +384,7 @@ def test_strip_decomposition_on_one_gpu(G):
 # ------------------------------------------------------------------ seeded random sweep over geometries
 def test_random_sweep_frames_on_random_geometries(G):
     """40 seeded draws of (Lx, Ly, periodicity, site count, motion): three frames each through vor_frame_host
-    (with the fused label -> edge kernel wherever it applies) against the oracle chain on the same geometry -
+    (with and without the fused label -> edge kernel, which applies where Lx % 32 == 0) against the oracle chain on the same geometry -
     labels, edge counts, created / destroyed lists."""
     rng = np.random.default_rng(20260)
     for case in range(40):
@@ -397,27 +397,32 @@ def test_random_sweep_frames_on_random_geometries(G):
         else:
             sx, sy = rand_sites(rng, Lx, Ly, max(1, int(Lx * Ly / spacing ** 2)))
         n = len(sx)
-        v = make(Lx, Ly, per, n)
-        fuse = int(rng.integers(0, 2))
-        v.vor_set_option("fuse", fuse)
-        cap = 2 * Lx * Ly + 16
-        hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
-        prev = np.empty(0, np.uint64)
+        rng.integers(0, 2)                                 # (keeps the draws of earlier rounds' cases)
         sigma = float(rng.choice([0.0, 0.3, 2.0])) * FP
+        frames = []
         for t in range(3):
-            v.vor_frame_host(sx, sy, hc, hd, cnt)
-            lab = oracle.label_brute_g(Lx, Ly, per[0], per[1], sx, sy)
-            pl = v.vor_frame_results()[0]
-            got = G.from_device_ptr(pl, Lx * Ly, torch.int32).cpu().numpy().reshape(Ly, Lx)
-            assert np.array_equal(got, lab), (case, t, Lx, Ly, per, n, fuse, int((got != lab).sum()))
-            e = oracle.edges_g(lab, per[0], per[1])
-            rc, rd = oracle.diff(prev, e)
-            assert cnt.tolist() == [len(e), len(rc), len(rd)], (case, t, Lx, Ly, per, n, fuse)
-            assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd), (case, t)
-            prev = e
+            frames.append((sx, sy))
             sx = ((sx.astype(np.int64) + np.rint(rng.normal(0, sigma, n)).astype(np.int64)) % (FP * Lx)).astype(np.int32)
             sy = ((sy.astype(np.int64) + np.rint(rng.normal(0, sigma, n)).astype(np.int64)) % (FP * Ly)).astype(np.int32)
-        v.close()
+        refs, prev = [], np.empty(0, np.uint64)
+        for fx, fy in frames:
+            lab = oracle.label_brute_g(Lx, Ly, per[0], per[1], fx, fy)
+            e = oracle.edges_g(lab, per[0], per[1])
+            refs.append((lab, e) + oracle.diff(prev, e))
+            prev = e
+        cap = 2 * Lx * Ly + 16
+        for fuse in (0, 1):                                # every geometry with and without the fused kernel
+            v = make(Lx, Ly, per, n)
+            v.vor_set_option("fuse", fuse)
+            hc = np.empty(cap, np.uint64); hd = np.empty(cap, np.uint64); cnt = np.zeros(3, np.int64)
+            for t, ((fx, fy), (lab, e, rc, rd)) in enumerate(zip(frames, refs)):
+                v.vor_frame_host(fx, fy, hc, hd, cnt)
+                pl = v.vor_frame_results()[0]
+                got = G.from_device_ptr(pl, Lx * Ly, torch.int32).cpu().numpy().reshape(Ly, Lx)
+                assert np.array_equal(got, lab), (case, t, Lx, Ly, per, n, fuse, int((got != lab).sum()))
+                assert cnt.tolist() == [len(e), len(rc), len(rd)], (case, t, Lx, Ly, per, n, fuse)
+                assert np.array_equal(hc[:cnt[1]], rc) and np.array_equal(hd[:cnt[2]], rd), (case, t, fuse)
+            v.close()
 
 
 def test_random_sweep_field_chain(G):
@@ -559,7 +564,11 @@ def test_merge_lists_many_lists_empty_lists_and_capacity(G):
         out = torch.full((len(ref) + 3,), -5, dtype=torch.int64, device="cuda")
         n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
         v.vor_merge_lists(lists, counts, 4096, out[: len(ref)], n_out)
-        v.vor_sync_status()
+        if n_lists == 7:                               # the truncated list is reported on the merging side too
+            with pytest.raises(Exception, match="ECAPACITY"):
+                v.vor_sync_status()
+        else:
+            v.vor_sync_status()
         assert int(n_out.item()) == len(ref) and np.array_equal(G.u64(out, len(ref)), ref), n_lists
         assert (out[len(ref):] == -5).all()
         if len(ref) > 10:                                                 # too small an output: required count + status
