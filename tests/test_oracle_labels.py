@@ -8,6 +8,8 @@ What fixes the expected values (none of it is the oracle's own formula retyped):
    convention (R2) and the minimum-image wrap;
  - O1b == O1a on adversarial inputs (proves the R3 stop rule).
 """
+import zlib
+
 import numpy as np
 import pytest
 from scipy.spatial import cKDTree
@@ -137,7 +139,7 @@ ADVERSARIAL = [
 
 @pytest.mark.parametrize("name,L,bs,gen", ADVERSARIAL, ids=[a[0] for a in ADVERSARIAL])
 def test_cell_list_equals_brute_adversarial(name, L, bs, gen):
-    rng = np.random.default_rng(hash(name) % 2**32)
+    rng = np.random.default_rng(zlib.crc32(name.encode()))   # fixed per case: str hashes change per process
     sx, sy = gen(rng, FP * L)
     assert np.array_equal(oracle.label_cells(L, sx, sy, bs), oracle.label_brute(L, sx, sy))
 
