@@ -27,7 +27,11 @@ from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
 # Per-launch ncu figures of the committed `ncu --set full` capture (config 5 only): DRAM bytes read + written,
 # issue-slot utilisation, warp instructions.  profiles/r2g_traffic.md names the command that produced the table.
-NCU_TABLE = os.path.join(ROOT, "profiles", "r2g_traffic.csv")
+# These figures are REPLAYED from that committed capture, never measured by a bench run: every object that carries
+# them says so ("measured_in_this_run": false) and names the file and the commit the capture was taken from.
+NCU_TABLE_REL = "profiles/r2g_traffic.csv"
+NCU_TABLE = os.path.join(ROOT, *NCU_TABLE_REL.split("/"))
+NCU_TABLE_COMMIT = "7850d95"     # the kernels in the table are unchanged since (label / edges / diff kernels)
 
 
 def ncu_table():
@@ -72,7 +76,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-field-leg", action="store_true", help="skip the short config-4 field-path leg of the default line")
     ap.add_argument("--cpu-sample-L", type=int, default=0,
-                    help="lattice side of the oracle's sample (0 = full workload for ours, 4096 for reference)")
+                    help="lattice side of the oracle's sample (0 = the full workload, in both arms)")
     return ap.parse_args()
 
 
@@ -185,7 +189,7 @@ def run_reference(args, w):
     if rank != 0:
         return
     import oracle
-    Ls = args.cpu_sample_L or min(4096, w.L)
+    Ls = args.cpu_sample_L or w.L                   # the FULL workload (config 5: ~4.3 s per frame on 16 cores)
     ws = w if Ls == w.L else W.scaled(5, Ls) if w.kind == "jittered_grid" else w
     frames = list(ws.frames(args.warmup + args.steps))
     for sx, sy in frames[:args.warmup]:
@@ -193,14 +197,16 @@ def run_reference(args, w):
     secs, cells = oracle_frame_seconds(ws, frames[args.warmup:])
     cores = oracle.num_threads()
     val = cells / secs
-    sample = (f"{args.steps} frames of {ws.name} ({ws.L}^2 cells, {ws.n_sites} sites: same density and "
-              f"structure as {w.name}); label_cells + edges + diff")
+    sample = (f"{args.steps} frames of {ws.name} ({ws.L}^2 cells, {ws.n_sites} sites"
+              + ("" if ws.L == w.L else f": same density and structure as {w.name}")
+              + f"); label_cells on {cores} threads, edges + diff on 1 (serial in the oracle)")
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64",
            "data": "synthetic", "config": {"workload": w.name, "L": w.L, "n_sites": w.n_sites,
                                            "sample_L": ws.L, "sample_sites": ws.n_sites},
-           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                            "threads": {"label_cells": cores, "edges": 1, "diff": 1}},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out), flush=True)
@@ -409,7 +415,8 @@ def run_ours(args, w):
     ncu = ncu_table() if is_cfg5 else {}
 
     # every kernel is reported against the measured HBM copy rate with ITS algorithmic
-    # bytes; `traffic` = DRAM bytes of one launch in the committed ncu capture (config 5 only).
+    # bytes; `traffic` = DRAM bytes of one launch REPLAYED from the committed ncu capture (config 5 only;
+    # `traffic_source` says so); `achieved`, `frac` and `launch_ms` are measured live by this run.
     def hbm_roof(name, nbytes, what, ms=None):
         if ms is None:
             if name not in kernel_launch_ms:
@@ -420,9 +427,10 @@ def run_ours(args, w):
              "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": t.get("dram_bytes"), "launch_ms": ms,
              "algorithmic": what, "peak_source": peak_src}
         if t:
+            replayed = {"measured_in_this_run": False, "source": NCU_TABLE_REL, "capture_commit": NCU_TABLE_COMMIT}
+            r["traffic_source"] = replayed
             r["ncu"] = {"issue_active_pct": t.get("issue_active_pct"), "warp_inst_per_cell":
-                        t["warp_inst"] / cells_per_step if "warp_inst" in t else None,
-                        "source": "profiles/r2_traffic.csv"}
+                        t["warp_inst"] / cells_per_step if "warp_inst" in t else None, **replayed}
         return r
 
     # The dominant kernel is the labelling kernel (one launch per step).  Its §8(d) unit is the 4 B/cell it
@@ -479,9 +487,11 @@ def run_ours(args, w):
         ws = w if Ls == w.L else W.scaled(5, Ls)
         fr = list(ws.frames(1))
         secs, cells = oracle_frame_seconds(ws, fr)
-        out["cpu_baseline"] = {"value": cells / secs, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                               "sample": f"1 frame of {ws.name} ({ws.L}^2 cells, {ws.n_sites} sites): "
-                                         f"label_cells + edges + diff, {secs:.1f} s"}
+        nt = oracle.num_threads()
+        out["cpu_baseline"] = {"value": cells / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
+                               "threads": {"label_cells": nt, "edges": 1, "diff": 1},
+                               "sample": f"1 frame of {ws.name} ({ws.L}^2 cells, {ws.n_sites} sites): label_cells on "
+                                         f"{nt} threads, edges + diff on 1 (serial in the oracle), {secs:.1f} s"}
         # the same oracle on ONE thread, on a 1/16-area copy of the workload
         w1 = W.scaled(5, max(256, ws.L // 4)) if ws.kind == "jittered_grid" and ws.L >= 1024 else ws
         s1, c1 = oracle_frame_seconds(w1, list(w1.frames(1)), threads=1)
