@@ -3,7 +3,8 @@
  * NVIDIA B200 (sm_100a).  "PAPER.md:n" cites a line of the paper text plus its section.
  *
  * Conventions
- *   L            lattice side; the lattice is an L x L torus.  P = 256*L is the period in
+ *   L            lattice side: vor_create makes an L x L torus; vor_create_geom an Lx x Ly lattice whose axes
+ *                are periodic or walled (then read Lx / Ly for L below).  P = 256*L is the period in
  *                fixed-point units (1 cell = 256 units).
  *   cell (x,y)   0 <= x,y < L, centre (256x+128, 256y+128), linear index y*L + x.
  *   sites        SoA int32 arrays sx[n], sy[n], each coordinate in [0, P).  Coordinates outside
@@ -333,7 +334,7 @@ int match_sites(vor_ctx* ctx, const int32_t* d_px, const int32_t* d_py, const in
  * previous call on this context (the first call diffs against an empty list), copies the
  * created/destroyed lists (at most cap each) and h_counts[3] = {n_edges, n_created, n_destroyed}
  * back, and synchronises.  The label image stays on the device (not copying it is
- * the point of the method); vor_frame_labels() exposes it. */
+ * the point of the method); vor_frame_results() exposes it. */
 int vor_frame_host(vor_ctx* ctx, const int32_t* h_sx, const int32_t* h_sy, int32_t n_sites,
                    uint64_t* h_created, uint64_t* h_destroyed, int64_t cap, int64_t* h_counts,
                    void* stream);

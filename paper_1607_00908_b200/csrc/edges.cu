@@ -76,7 +76,7 @@ __device__ __forceinline__ void hash_insert(uint32_t a, uint32_t b, unsigned lon
 // raw-key list (one atomic per CTA) that the finish kernel inserts into the adjacency matrix.
 constexpr int kStrWarpsX = 2, kStrWarpsY = 2;
 constexpr int kStrWarps = kStrWarpsX * kStrWarpsY;
-constexpr int kStrThreads = 32 * kStrWarps;                     // 256
+constexpr int kStrThreads = 32 * kStrWarps;                     // 128
 constexpr int kStripCols = 128;
 constexpr int kStripRows = 32;                                  // rows per warp
 constexpr int kPf = 4;                                          // rows in flight per lane
