@@ -223,7 +223,8 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
             // above row 0: the last row (periodic) or row 0 itself (no pair)
             const int32_t* __restrict__ up = labels + (int64_t)(ybeg == 0 ? (wrap_y ? H - 1 : 0) : ybeg - 1) * W;
             pc = __ldg(reinterpret_cast<const int4*>(up + col));
-            const int32_t hup = __ldg(up + colh);
+            int32_t hup = 0;
+            if (halo) hup = __ldg(up + colh);
             const int32_t nb = __shfl_down_sync(full, pc.x, 1);
             prr3 = halo ? hup : nb;
         }
@@ -232,11 +233,11 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
         // row equals the row above it, so it is never dirty.  Every strip runs kStripRows rows.
         int32_t ahead = yend - ybeg - 1;           // rows below the cursor
         int4 buf[kPf];
-        int32_t hb[kPf];
+        int32_t hb[kPf] = {0, 0, 0, 0};
 #pragma unroll
         for (int j = 0; j < kPf; ++j) {
             buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
-            hb[j] = __ldg(ph);
+            if (halo) hb[j] = __ldg(ph);        // only the lane next to the strip border uses it
             const int32_t step = ahead > 0 ? W : 0;
             p += step; ph += step;
             --ahead;
@@ -248,7 +249,7 @@ __global__ void __launch_bounds__(kStrThreads, 8) edges_stream_kernel(const int3
                 const int4 c = buf[j];
                 const int32_t hc = hb[j];
                 buf[j] = __ldcs(reinterpret_cast<const int4*>(p));
-                hb[j] = __ldg(ph);
+                if (halo) hb[j] = __ldg(ph);        // only the lane next to the strip border uses it
                 const int32_t step = ahead > 0 ? W : 0;
                 p += step; ph += step;
                 --ahead;
