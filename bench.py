@@ -26,12 +26,12 @@ sys.path.insert(0, ROOT)
 from paper_1607_00908_b200 import workloads as W  # noqa: E402
 
 # Per-launch ncu figures of the committed `ncu --set full` capture (config 5 only): DRAM bytes read + written,
-# issue-slot utilisation, warp instructions.  profiles/r2g_traffic.md names the command that produced the table.
+# issue-slot utilisation, warp instructions.  profiles/r3_traffic.md names the command that produced the table.
 # These figures are REPLAYED from that committed capture, never measured by a bench run: every object that carries
 # them says so ("measured_in_this_run": false) and names the file and the commit the capture was taken from.
-NCU_TABLE_REL = "profiles/r2g_traffic.csv"
+NCU_TABLE_REL = "profiles/r3_traffic.csv"
 NCU_TABLE = os.path.join(ROOT, *NCU_TABLE_REL.split("/"))
-NCU_TABLE_COMMIT = "7850d95"     # the kernels in the table are unchanged since (label / edges / diff kernels)
+NCU_TABLE_COMMIT = "55183a2"     # the kernels in the table are unchanged since (label / edges / diff kernels)
 
 
 def ncu_table():
