@@ -59,6 +59,25 @@ def test_labels_config2_two_frames(G):
         check_labels(G, w.L, sx, sy)
 
 
+@pytest.mark.parametrize("L,n,halo", [(16, 4, 130), (16, 2, 1000), (32, 9, 130), (48, 20, 400), (75, 30, 130),
+                                        (75, 3, 1000), (96, 12, 700), (128, 5, 1000)])
+def test_labels_small_lattices_where_the_halo_exceeds_the_period(G, L, n, halo):
+    """on small lattices the gather halo of the CTA path (above all the retry's 2 * halo + bucket width) is
+    larger than half a period or than the period itself; the kernel must refuse such a region up front (no negative
+    argument to its bucket division, no int32 overflow in the span test) and fall back - same labels on every path,
+    for the default and for very wide halos."""
+    rng = np.random.default_rng(1000 * L + n)
+    sx, sy = rng.integers(0, FP * L, n).astype(np.int32), rng.integers(0, FP * L, n).astype(np.int32)
+    ref = oracle.label_brute(L, sx, sy)
+    v = make(L, n)
+    v.vor_set_option("label_halo_x100", halo)
+    for path in (3, 2, 0):
+        v.vor_set_option("label_path", path)
+        got = G.gpu_labels(v, sx, sy)
+        assert np.array_equal(got, ref), (path, int((got != ref).sum()))
+    v.close()
+
+
 @pytest.mark.parametrize("L", [512, 1024])
 def test_labels_scaled_config5(G, L):
     w = W.scaled(5, L)
